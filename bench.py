@@ -1,0 +1,211 @@
+#!/usr/bin/env python
+"""bench.py -- batch-1 decode throughput of the DF-SSM step on B200 (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2] [--batch 1]
+
+A "step" is one pass of the whole hot path (S0, L x (S1..S7), S8: include/dfssm.h) over one batch of
+tokens, i.e. one decoded token per sequence.  The workload is BASELINE.json configs[2] (Mamba-2
+1.3B shape, batch 1): seeded synthetic weights, a uniform-random prompt fed
+through the step path (the warm-up steps), then greedy decode with the token kept on the device
+(the timed steps).  Prints ONE JSON line (rank 0).
+
+Own arm ("ours"): every step runs in libdfssm.so's CUDA kernels through the C ABI.
+Reference arm ("--impl reference"): the CPU oracle as it stands (oracle/), timed on the host cores.
+N > 1: independent replicas, one per GPU ("replicas only"); no collective in the
+data path; value = tokens of all ranks / max-over-ranks device time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+import dfssm_synth as ds  # noqa: E402
+
+METRIC = "batch-1 decode tokens/s, 1.3B-shape DF-SSM; achieved HBM GB/s vs peak"
+UNIT = "tokens/s"
+NOMINAL_HBM_GBS = 8000.0          # BASELINE.json north_star: "~8 TB/s peak"
+FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+def n_cores() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def measured_peak():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        try:
+            return float(json.loads(p.read_text())["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+# ---------------------------------------------------------------------------------------------
+# algorithmic bytes: what the method itself must move
+# ---------------------------------------------------------------------------------------------
+def algorithmic_bytes(s, batch: int) -> dict:
+    dm, di, dip, r, cd, nh = s.d_model, s.d_inner, s.d_in_proj, s.lora_rank, s.conv_dim, s.nheads
+    scaffold = s.n_layers * (dip * dm + dm * di) // 8
+    lora = s.n_layers * r * (dm + dip + di + dm)
+    state = s.n_layers * batch * 2 * (nh * s.headdim * s.d_state * 4)
+    lm_head = s.vocab * dm
+    per_layer_small = (4 * dm + 2 * dip + 4 * r + 4 * dip + 16 * cd + 4 * cd + 12 * nh + 4 * di
+                       + 2 * dm + 4 * r + 4 * dm)
+    conv_state = s.n_layers * batch * 2 * cd * 3 * 4
+    other = s.n_layers * per_layer_small + conv_state + 4 * s.vocab + 4 * dm + batch * (dm + 4) \
+        + batch * 4 * s.vocab
+    return dict(scaffold=scaffold, lora=lora, state=state, lm_head=lm_head, other=other,
+                bj_formula=scaffold + lora + state, total=scaffold + lora + state + lm_head + other)
+
+
+def kernel_class_bytes(s, batch: int) -> dict:
+    """Algorithmic bytes ONE launch of each kernel class moves (weights once, state r+w once)."""
+    dm, di, dip, r, cd, nh = s.d_model, s.d_inner, s.d_in_proj, s.lora_rank, s.conv_dim, s.nheads
+    B = batch
+    return {
+        "embed": B * (dm + 4 + 4 * dm),
+        "normquant": B * (4 * di + 2 * di) + 4 * di,
+        "proj_in": dip * dm // 8 + r * dm + B * (2 * dm + 4 * dip + 4 * r),
+        "ssm": B * (2 * nh * s.headdim * s.d_state * 4 + 2 * cd * 4 * 4 + 4 * dip + 4 * di)
+        + 2 * dip + dip * r + 4 * dip + 20 * cd + 12 * nh,
+        "proj_out": dm * di // 8 + r * di + B * (2 * di + 4 * dm + 4 * r),
+        "epi_out": 2 * dm + dm * r + 4 * dm + B * (4 * dm + 8 * dm),
+        "lmhead": s.vocab * dm + 4 * s.vocab + B * (dm + 4 * s.vocab),
+        "argmax": B * 4 * s.vocab,
+    }
+
+
+# ---------------------------------------------------------------------------------------------
+# clocks: nvidia-smi sampled DURING the timed region
+# ---------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.samples = []
+        self.proc = None
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.samples.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.samples:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------
+# the oracle, as it stands, on the host cores (cpu_baseline leg and --impl reference)
+# ---------------------------------------------------------------------------------------------
+def time_oracle(s, blob, cfg_idx: int, batch: int, budget_s: float, max_steps: int, n_prompt: int = 2):
+    """Feed `n_prompt` prompt tokens (untimed), then time greedy decode steps until the budget or
+    max_steps is reached.  Returns (tokens/s, steps, seconds, threads)."""
+    import oracle
+    oracle.build()
+    oracle.set_threads(n_cores())
+    m = oracle.OracleModel(blob, batch)
+    prompt = ds.token_batch(s.vocab, n_prompt, seed=cfg_idx, batch=batch)
+    for t in range(n_prompt):
+        m.step(prompt[t])
+    tok = np.array(m.next_tokens()[:batch], np.int32)
+    steps, t0 = 0, time.perf_counter()
+    while steps < max_steps:
+        m.step(tok)
+        tok = np.array(m.next_tokens()[:batch], np.int32)
+        steps += 1
+        if time.perf_counter() - t0 >= budget_s:
+            break
+    dt = time.perf_counter() - t0
+    return batch * steps / dt, steps, dt, oracle.get_threads()
+
+
+def run_reference(args, s, blob):
+    """--impl reference: the oracle timed on the host cores, same config / metric / unit."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    # warm-up steps and timed steps both run; the timed sample is bounded to ~2 minutes
+    import oracle
+    oracle.build()
+    oracle.set_threads(n_cores())
+    m = oracle.OracleModel(blob, args.batch)
+    toks = ds.token_batch(s.vocab, max(1, min(args.warmup, 8)), seed=args.config, batch=args.batch)
+    for t in range(toks.shape[0]):
+        m.step(toks[t])
+    tok = np.array(m.next_tokens()[:args.batch], np.int32)
+    steps, t0 = 0, time.perf_counter()
+    while steps < args.steps and time.perf_counter() - t0 < 120.0:
+        m.step(tok)
+        tok = np.array(m.next_tokens()[:args.batch], np.int32)
+        steps += 1
+    dt = time.perf_counter() - t0
+    val = args.batch * steps / dt
+    sample = (f"{steps} greedy decode steps of config {args.config} batch {args.batch} after {toks.shape[0]} prompt steps "
+              f"(bounded to 120 s; {args.steps} steps requested)")
+    out = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": int(toks.shape[0]), "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "int8 x {-1,+1} -> int32; fp32 state", "data": "synthetic",
+        "config": {"workload": workload_name(args.config, args.batch), "seed": args.config},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.get_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(out), flush=True)
+
+
+def workload_name(cfg_idx: int, batch: int) -> str:
+    names = {0: "cfg0 tiny DF-SSM (2 layers, d_model 256)", 1: "cfg1 Mamba-2-130M-shape DF-SSM",
+             2: "cfg2 Mamba-2-1.3B-shape DF-SSM (48 layers, d_model 2048, d_state 128, LoRA r32)",
+             3: "cfg3 Mamba-2-1.3B-shape DF-SSM batch sweep", 4: "cfg4 Mamba-2-2.7B-shape DF-SSM"}
+    return f"{names.get(cfg_idx, f'cfg{cfg_idx}')}, batch {batch}, greedy decode after a uniform-random prompt"

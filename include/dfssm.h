@@ -1,0 +1,180 @@
+/*
+ * dfssm.h -- C ABI of the DF-SSM per-token decode step for one NVIDIA B200 (sm_100a).
+ *
+ * What the library computes (citations: "P:NN" = line NN of the paper text PAPER.md of
+ * arxiv/paper_2606_10932; "R#" = a reading listed in DESIGN.md section 4):
+ *
+ *   for every sequence s of a batch, independently, with persistent per-sequence state,
+ *     S0  u = e_s[tok] * float(E[tok,:])                       int8 per-row embedding
+ *     for each layer:
+ *     S1  RMSNorm(u) -> per-token absmax int8 (xq, s_x)        (R4, R13)
+ *     S2  acc_i = sum_k sign_ik * xq_k, sign in {-1,+1}        bit-packed scaffold, int32
+ *     S3  t_j = sum_k A_jk xq_k (int32);  zxbcdt_i = s_x*(w_s[i]*acc_i + b_s[i]*sum_j B_ij*(a_s[j]*t_j))
+ *                                                              int8 LoRA, Eq. 3            (R5-R7)
+ *     S4  causal depthwise 4-tap conv step over a rolling state, then SiLU   (R9)
+ *     S5  h <- exp(dt*A)*h + (dt*x) (x) B ;  y = C.h + D*x     fp32 state                  (Table 12; R10-R12)
+ *     S6  g = y*silu(z) ; RMSNorm(g) -> int8 (gq, s_g)         gate first, then norm
+ *     S7  out_proj as S2/S3 on gq ; u <- u + out
+ *     S8  RMSNorm(u) -> int8 ; logits_v = float(sum_k E_vk hq_k) * (s_h*e_s[v]) ; argmax (tied head; R16)
+ *
+ * Conventions
+ *   - every function returns an int status (DFSSM_OK == 0, errors negative) unless stated;
+ *     nothing throws, prints, or keeps global state; a handle is not thread-safe.
+ *   - "dev" pointers are CUDA device pointers, "host" pointers are ordinary host pointers.
+ *   - the CALLER owns the device arena, the CUDA stream and every host buffer; the LIBRARY
+ *     owns what it places inside the arena and hands out BORROWED device pointers that stay
+ *     valid until dfssm_destroy (their contents change at every dfssm_step).
+ *   - all device work is enqueued on the stream given to dfssm_create; functions documented as
+ *     "async" do not synchronise with the host.
+ *   - there is no CPU fallback: on a device that is not compute capability 10.x
+ *     dfssm_create fails with DFSSM_E_ARCH.
+ */
+#ifndef DFSSM_H
+#define DFSSM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DFSSM_ABI_VERSION 1u
+
+#if defined(__GNUC__)
+#define DFSSM_API __attribute__((visibility("default")))
+#else
+#define DFSSM_API
+#endif
+
+enum {
+    DFSSM_OK      = 0,
+    DFSSM_E_ARG   = -1,   /* null pointer, batch out of range, bad index, unsupported shape */
+    DFSSM_E_SIZE  = -2,   /* arena or blob too small / blob size does not match its header   */
+    DFSSM_E_STATE = -3,   /* call out of order (step before load_weights, ...)               */
+    DFSSM_E_CUDA  = -4,   /* a CUDA call failed; text in dfssm_last_error                    */
+    DFSSM_E_ARCH  = -5,   /* device is not sm_100                                            */
+    DFSSM_E_TOKEN = -6    /* a token id outside [0, vocab) was seen (it was clamped)          */
+};
+
+/* dfssm_config.flags */
+#define DFSSM_FLAG_TAPS      1u  /* allocate per-layer debug taps and record them every step (slower)   */
+#define DFSSM_FLAG_NO_GRAPH  2u  /* launch the step's kernels one by one instead of one CUDA-graph launch */
+
+/* Shape of the model (the paper's Mamba-2-shaped student, Table 1) + capacity.
+ * nheads = d_inner/headdim ; d_in_proj = 2*d_inner + 2*ngroups*d_state + nheads ;
+ * conv_dim = d_inner + 2*ngroups*d_state.  Requirements: d_model % 32 == 0, d_inner % 32 == 0,
+ * d_inner % headdim == 0, nheads % ngroups == 0, d_conv == 4, d_state % 32 == 0, headdim % 16 == 0,
+ * 1 <= lora_rank <= 64, d_model <= 8192, d_inner <= 8192, 1 <= max_batch <= 256. */
+typedef struct dfssm_config {
+    uint32_t abi_version;   /* DFSSM_ABI_VERSION */
+    int32_t  n_layers, d_model, d_inner, headdim, d_state, ngroups, d_conv, vocab, lora_rank;
+    int32_t  max_batch;     /* number of independent sequences the state is sized for */
+    float    norm_eps;      /* RMSNorm epsilon (R13: 1e-5) */
+    uint32_t flags;         /* DFSSM_FLAG_* */
+} dfssm_config;
+
+typedef struct dfssm_ctx dfssm_ctx;   /* opaque */
+
+/* Debug taps (`which` of dfssm_debug_tensor), per layer and per sequence; recorded only with
+ * DFSSM_FLAG_TAPS.  Same meaning as the rows of the step list above. */
+enum {
+    DFSSM_TAP_XQ_IN = 0,   /* int8  [d_model]    S1 codes                         */
+    DFSSM_TAP_S_IN,        /* f32   [1]          S1 scale s_x                      */
+    DFSSM_TAP_ACC_IN,      /* int32 [d_in_proj]  S2                                */
+    DFSSM_TAP_T_IN,        /* int32 [lora_rank]  S3 stage 1                        */
+    DFSSM_TAP_ZXBCDT,      /* f32   [d_in_proj]  S3 output, order z|x|B|C|dt       */
+    DFSSM_TAP_XBC_CONV,    /* f32   [conv_dim]   S4 output (after SiLU)            */
+    DFSSM_TAP_DT,          /* f32   [nheads]     softplus(dt_raw + dt_bias)        */
+    DFSSM_TAP_Y,           /* f32   [d_inner]    S5 output                         */
+    DFSSM_TAP_G,           /* f32   [d_inner]    y*silu(z)                         */
+    DFSSM_TAP_GQ,          /* int8  [d_inner]    S6 codes                          */
+    DFSSM_TAP_S_G,         /* f32   [1]          S6 scale                          */
+    DFSSM_TAP_ACC_OUT,     /* int32 [d_model]    S7 scaffold                       */
+    DFSSM_TAP_T_OUT,       /* int32 [lora_rank]  S7 LoRA stage 1                   */
+    DFSSM_TAP_HIDDEN,      /* f32   [d_model]    residual stream after the layer   */
+    DFSSM_TAP_COUNT
+};
+
+/* Device bytes the caller must provide for `cfg` (weights + per-sequence state + activations
+ * [+ taps]).  Returns 0 if cfg is null or invalid. */
+DFSSM_API size_t dfssm_arena_bytes(const dfssm_config* cfg);
+
+/* Create a context on the CURRENT CUDA device.  dev_arena: device memory, 256-byte aligned,
+ * at least dfssm_arena_bytes(cfg) bytes, owned by the caller and untouched by anyone else while
+ * the context lives.  cuda_stream: a cudaStream_t (NULL = the legacy default stream).
+ * The state is zeroed (as by dfssm_reset_state(ctx, -1)).  Synchronises the stream. */
+DFSSM_API int dfssm_create(const dfssm_config* cfg, void* dev_arena, size_t arena_bytes, void* cuda_stream,
+                 dfssm_ctx** out);
+
+/* Load the canonical weight blob (layout: DESIGN.md section 3; header must match cfg).
+ * host_blob is read during the call only.  Validates, copies to the arena, builds the per-layer
+ * tables and the whole-step CUDA graph.  Synchronises the stream. */
+DFSSM_API int dfssm_load_weights(dfssm_ctx* ctx, const void* host_blob, size_t nbytes);
+
+/* Zero the conv + SSM state of sequence seq_index (or all sequences if < 0).  Async.
+ * "State tensors ... are preallocated and persist across tokens". */
+DFSSM_API int dfssm_reset_state(dfssm_ctx* ctx, int seq_index);
+
+/* One decode step for sequences 0..batch-1: tokens_dev[s] is the input token of sequence s
+ * (device int32[batch]; it may be the pointer returned by dfssm_next_tokens -- greedy decode
+ * without leaving the device).  Async: exactly one launch (a CUDA graph) unless
+ * DFSSM_FLAG_NO_GRAPH or DFSSM_FLAG_TAPS is set.  Token ids outside [0, vocab) are clamped on the
+ * device and a sticky error is raised, reported as DFSSM_E_TOKEN by the next dfssm_sync. */
+DFSSM_API int dfssm_step(dfssm_ctx* ctx, const int32_t* tokens_dev, int batch);
+
+/* Host-buffer form of the same step (the end-to-end call): copies tokens_host[batch] to the
+ * device, runs the step, copies the greedy next tokens to next_host[batch] and, if logits_host is
+ * non-null, the logits to logits_host[batch*vocab]; synchronises the stream before returning.
+ * For best speed the host buffers should be page-locked; pageable memory also works. */
+DFSSM_API int dfssm_step_host(dfssm_ctx* ctx, const int32_t* tokens_host, int batch, int32_t* next_host,
+                    float* logits_host);
+
+/* Borrowed device pointers to the results of the last step: logits f32 [batch][vocab] (row
+ * stride = vocab), greedy tokens int32 [batch] (lowest index on ties), final residual stream
+ * f32 [batch][d_model] (before the final norm).  No synchronisation: stream order applies. */
+DFSSM_API int dfssm_logits(dfssm_ctx* ctx, const float** logits_dev);
+DFSSM_API int dfssm_next_tokens(dfssm_ctx* ctx, const int32_t** next_dev);
+DFSSM_API int dfssm_hidden(dfssm_ctx* ctx, const float** hidden_dev);
+
+/* Borrowed device pointer + byte count of one debug tap of (layer, sequence).  DFSSM_E_STATE if
+ * the context was created without DFSSM_FLAG_TAPS. */
+DFSSM_API int dfssm_debug_tensor(dfssm_ctx* ctx, int layer, int which, int seq, const void** dev, size_t* nbytes);
+
+/* Copy the recurrent state of (layer, seq) to / from HOST memory and synchronise.
+ *   ssm  : f32 [nheads][headdim][d_state]   (may be null to skip)
+ *   conv : f32 [conv_dim][3], oldest sample first   (may be null to skip)
+ * The *_bytes arguments must equal the exact sizes (DFSSM_E_SIZE otherwise). */
+DFSSM_API int dfssm_get_state(dfssm_ctx* ctx, int layer, int seq, float* ssm_host, size_t ssm_bytes,
+                    float* conv_host, size_t conv_bytes);
+DFSSM_API int dfssm_set_state(dfssm_ctx* ctx, int layer, int seq, const float* ssm_host, size_t ssm_bytes,
+                    const float* conv_host, size_t conv_bytes);
+
+/* Wait for the stream; returns DFSSM_E_TOKEN once if a bad token id was clamped since the last
+ * call, DFSSM_E_CUDA on a device fault. */
+DFSSM_API int dfssm_sync(dfssm_ctx* ctx);
+
+/* Number of kernels of this library that one dfssm_step(batch) launches (graph nodes).  >= 1. */
+DFSSM_API int dfssm_launches_per_step(dfssm_ctx* ctx, int batch);
+
+/* Device-timed profile of the last `dfssm_step` when run with per-kernel events is not offered;
+ * use dfssm_time_kernels: runs `iters` steps with CUDA events around every kernel class and
+ * writes the mean microseconds per step of each class to out_us[DFSSM_KCLASS_COUNT].  Sync. */
+enum {
+    DFSSM_KCLASS_EMBED = 0, DFSSM_KCLASS_NORMQUANT, DFSSM_KCLASS_PROJ_IN, DFSSM_KCLASS_SSM,
+    DFSSM_KCLASS_PROJ_OUT, DFSSM_KCLASS_EPI_OUT, DFSSM_KCLASS_LMHEAD, DFSSM_KCLASS_ARGMAX,
+    DFSSM_KCLASS_COUNT
+};
+DFSSM_API int dfssm_time_kernels(dfssm_ctx* ctx, const int32_t* tokens_dev, int batch, int iters,
+                       float* out_us /* [DFSSM_KCLASS_COUNT] */);
+
+/* Human-readable text for the last error of this context ("" if none).  Never null. */
+DFSSM_API const char* dfssm_last_error(const dfssm_ctx* ctx);
+
+/* Release the context (never frees the arena).  Safe on null. */
+DFSSM_API void dfssm_destroy(dfssm_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DFSSM_H */

@@ -1,0 +1,654 @@
+// Host side of libdfssm.so: the C ABI of include/dfssm.h.
+// Arena carving, canonical-blob parsing (this is the CUDA path's own parser),
+// the kernel chain of one decode step and its CUDA-graph launcher ("CUDA graph capture ...
+// primary source of the large batch=1 speedup").
+#include "../../include/dfssm.h"
+
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "dfssm_kernels.cuh"
+
+using namespace dfssm;
+
+namespace {
+
+constexpr size_t ARENA_ALIGN = 256;
+inline size_t up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct Carve {                 // byte offsets inside the arena
+    size_t blob, ssm, conv, pos, u, xq, xqp, sx, qsum, acc, t, g, logits, next, tok, err, taps, total;
+    size_t ssm_elems, ldq, ld_acc;
+    uint32_t tap_stride;
+    TapLayout tl;
+};
+
+struct GraphEntry { int batch; cudaGraphExec_t exec; };
+
+}  // namespace
+
+struct dfssm_ctx {
+    dfssm_config cfg;
+    Dims dm;
+    Carve cv;
+    uint8_t* arena;
+    cudaStream_t stream;
+    bool loaded;
+    size_t blob_bytes;
+    std::vector<LayerW> layers;
+    const int8_t* emb; const float* emb_s; const float* normf_w;
+    std::vector<GraphEntry> graphs;
+    int last_batch;
+    int32_t* pinned_tok;       // page-locked staging for dfssm_step_host
+    int* pinned_err;
+    char err[512];
+};
+
+namespace {
+
+int fail(dfssm_ctx* c, int code, const char* fmt, ...)
+{
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof c->err, fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define CK(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(ctx, DFSSM_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_));        \
+    } while (0)
+
+bool valid_cfg(const dfssm_config* c)
+{
+    if (!c || c->abi_version != DFSSM_ABI_VERSION) return false;
+    if (c->n_layers < 0 || c->d_model <= 0 || c->d_inner <= 0 || c->headdim <= 0 || c->d_state <= 0 ||
+        c->ngroups <= 0 || c->vocab <= 0)
+        return false;
+    if (c->d_conv != 4) return false;
+    if (c->d_model % 32 || c->d_inner % 32 || c->d_model > 8192 || c->d_inner > 8192) return false;
+    if (c->d_inner % c->headdim || c->headdim % SSM_PB || c->d_state % 4) return false;
+    if ((c->d_inner / c->headdim) % c->ngroups) return false;
+    if (c->lora_rank < 1 || c->lora_rank > 64) return false;
+    if (c->max_batch < 1 || c->max_batch > 256) return false;
+    if (!(c->norm_eps > 0.0f)) return false;
+    return true;
+}
+
+Dims make_dims(const dfssm_config& c)
+{
+    Dims d;
+    d.n_layers = c.n_layers; d.d_model = c.d_model; d.d_inner = c.d_inner; d.headdim = c.headdim;
+    d.d_state = c.d_state; d.ngroups = c.ngroups; d.vocab = c.vocab; d.r = c.lora_rank;
+    d.nheads = c.d_inner / c.headdim;
+    d.d_in_proj = 2 * c.d_inner + 2 * c.ngroups * c.d_state + d.nheads;
+    d.conv_dim = c.d_inner + 2 * c.ngroups * c.d_state;
+    d.eps = c.norm_eps;
+    return d;
+}
+
+// canonical blob: 256-byte header, tensors in fixed order, 64-byte aligned
+struct BlobWalk {
+    size_t off = 256;
+    size_t take(size_t bytes) { off = up(off, 64); size_t o = off; off += bytes; return o; }
+};
+
+size_t blob_bytes_for(const Dims& d)
+{
+    BlobWalk w;
+    const size_t dm = d.d_model, di = d.d_inner, dip = d.d_in_proj, r = d.r, cd = d.conv_dim, nh = d.nheads;
+    for (int l = 0; l < d.n_layers; ++l) {
+        w.take(4 * dm); w.take(4 * dip * (dm / 32)); w.take(2 * dip); w.take(r * dm); w.take(4 * r);
+        w.take(dip * r); w.take(4 * dip); w.take(16 * cd); w.take(4 * cd); w.take(4 * nh); w.take(4 * nh);
+        w.take(4 * nh); w.take(4 * di); w.take(4 * dm * (di / 32)); w.take(2 * dm); w.take(r * di);
+        w.take(4 * r); w.take(dm * r); w.take(4 * dm);
+    }
+    w.take((size_t)d.vocab * dm); w.take(4 * (size_t)d.vocab); w.take(4 * dm);
+    return up(w.off, 64);
+}
+
+Carve carve(const dfssm_config& c)
+{
+    const Dims d = make_dims(c);
+    Carve v;
+    memset(&v, 0, sizeof v);
+    const size_t B = c.max_batch, nl = c.n_layers > 0 ? c.n_layers : 1;
+    v.ssm_elems = (size_t)d.nheads * d.headdim * d.d_state;
+    v.ldq = up((size_t)(d.d_model > d.d_inner ? d.d_model : d.d_inner), 64);
+    v.ld_acc = up((size_t)(d.d_in_proj > d.d_model ? d.d_in_proj : d.d_model), 4);
+    size_t o = 0;
+    auto put = [&](size_t bytes) { o = up(o, ARENA_ALIGN); size_t at = o; o += bytes; return at; };
+    v.blob = put(blob_bytes_for(d));
+    v.ssm = put(nl * B * v.ssm_elems * 4);
+    v.conv = put(nl * B * (size_t)d.conv_dim * 16);
+    v.pos = put(B * 4);
+    v.u = put(B * d.d_model * 4);
+    v.xq = put(B * v.ldq);
+    v.xqp = put(B * v.ldq);
+    v.sx = put(B * 4);
+    v.qsum = put(B * 4);
+    v.acc = put(B * v.ld_acc * 4);
+    v.t = put(B * T_STRIDE * 4);
+    v.g = put(B * d.d_inner * 4);
+    v.logits = put(B * (size_t)d.vocab * 4);
+    v.next = put(B * 4);
+    v.tok = put(B * 4);
+    v.err = put(16);
+    const size_t sizes[DFSSM_TAP_COUNT] = {
+        (size_t)d.d_model, 4, 4 * (size_t)d.d_in_proj, 4 * (size_t)d.r, 4 * (size_t)d.d_in_proj,
+        4 * (size_t)d.conv_dim, 4 * (size_t)d.nheads, 4 * (size_t)d.d_inner, 4 * (size_t)d.d_inner,
+        (size_t)d.d_inner, 4, 4 * (size_t)d.d_model, 4 * (size_t)d.r, 4 * (size_t)d.d_model };
+    size_t to = 0;
+    for (int i = 0; i < DFSSM_TAP_COUNT; ++i) { v.tl.off[i] = (uint32_t)to; to = up(to + sizes[i], 64); }
+    v.tl.off[DFSSM_TAP_COUNT] = (uint32_t)to;
+    v.tap_stride = (uint32_t)to;
+    v.taps = (c.flags & DFSSM_FLAG_TAPS) ? put(nl * B * to) : 0;
+    v.total = up(o, ARENA_ALIGN);
+    return v;
+}
+
+size_t tap_bytes(const Dims& d, int which)
+{
+    switch (which) {
+        case DFSSM_TAP_XQ_IN: return d.d_model;
+        case DFSSM_TAP_S_IN: case DFSSM_TAP_S_G: return 4;
+        case DFSSM_TAP_ACC_IN: case DFSSM_TAP_ZXBCDT: return 4 * (size_t)d.d_in_proj;
+        case DFSSM_TAP_T_IN: case DFSSM_TAP_T_OUT: return 4 * (size_t)d.r;
+        case DFSSM_TAP_XBC_CONV: return 4 * (size_t)d.conv_dim;
+        case DFSSM_TAP_DT: return 4 * (size_t)d.nheads;
+        case DFSSM_TAP_Y: case DFSSM_TAP_G: return 4 * (size_t)d.d_inner;
+        case DFSSM_TAP_GQ: return d.d_inner;
+        case DFSSM_TAP_ACC_OUT: case DFSSM_TAP_HIDDEN: return 4 * (size_t)d.d_model;
+    }
+    return 0;
+}
+
+template <typename T> T* at(dfssm_ctx* c, size_t off) { return reinterpret_cast<T*>(c->arena + off); }
+
+}  // namespace
+
+// =================================================================================================
+// the kernel chain of one step
+// =================================================================================================
+namespace {
+
+struct KTimer {                       // optional per-kernel-class device timing (dfssm_time_kernels)
+    std::vector<cudaEvent_t> ev;
+    std::vector<int> cls;
+    cudaStream_t st;
+    bool on = false;
+    void begin(int k)
+    {
+        if (!on) return;
+        cudaEvent_t a, b;
+        cudaEventCreate(&a); cudaEventCreate(&b);
+        cudaEventRecord(a, st);
+        ev.push_back(a); ev.push_back(b); cls.push_back(k);
+    }
+    void end()
+    {
+        if (!on) return;
+        cudaEventRecord(ev.back(), st);
+    }
+};
+
+size_t proj_smem(int K) { return (size_t)PROJ_BT * 2 * K; }
+size_t lm_smem(int K) { return (size_t)PROJ_BT * K; }
+size_t ssm_smem(const Dims& d) { return sizeof(float) * (64 + 2 * (size_t)d.d_state + 2 * SSM_PB + 4); }
+
+int proj_grid(int rows_total)
+{
+    const int per = PROJ_THREADS / 32;
+    int g = (rows_total + per - 1) / per;
+    const int cap = 148 * 8;
+    return g < cap ? g : cap;
+}
+
+// Enqueue S0, L x (S1..S7), S8 for `batch` sequences on the context's stream.  The input tokens are
+// read from the arena's own token buffer (cv.tok), which the argmax kernel also refreshes with the
+// greedy tokens -- so a graph captured once per batch size serves every caller pointer.
+int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
+{
+    dfssm_ctx* ctx = c;
+    const Dims& d = c->dm;
+    const Carve& v = c->cv;
+    cudaStream_t st = c->stream;
+    const size_t B = c->cfg.max_batch;
+    KTimer dummy;
+    if (!tm) tm = &dummy;
+    int nl = 0;
+
+    float* u = at<float>(c, v.u);
+    int8_t* xq = at<int8_t>(c, v.xq);
+    int8_t* xqp = at<int8_t>(c, v.xqp);
+    float* sx = at<float>(c, v.sx);
+    int32_t* qsum = at<int32_t>(c, v.qsum);
+    int32_t* acc = at<int32_t>(c, v.acc);
+    int32_t* t = at<int32_t>(c, v.t);
+    float* g = at<float>(c, v.g);
+    float* logits = at<float>(c, v.logits);
+    int32_t* next = at<int32_t>(c, v.next);
+    int32_t* tokens = at<int32_t>(c, v.tok);
+    int32_t* pos = at<int32_t>(c, v.pos);
+    int* err = at<int>(c, v.err);
+    const bool taps_on = (c->cfg.flags & DFSSM_FLAG_TAPS) != 0;
+    const int ldq = (int)v.ldq, ld_acc = (int)v.ld_acc;
+
+    tm->begin(DFSSM_KCLASS_EMBED);
+    k_embed<<<dim3((d.d_model + 255) / 256, batch), 256, 0, st>>>(tokens, c->emb, c->emb_s, d.vocab, d.d_model, u, err);
+    tm->end(); ++nl;
+
+    for (int l = 0; l < d.n_layers; ++l) {
+        const LayerW& L = c->layers[l];
+        uint8_t* tp = taps_on ? at<uint8_t>(c, v.taps) + (size_t)l * B * v.tap_stride : nullptr;
+        float* ssm = at<float>(c, v.ssm) + (size_t)l * B * v.ssm_elems;
+        float* conv = at<float>(c, v.conv) + (size_t)l * B * (size_t)d.conv_dim * 4;
+
+        tm->begin(DFSSM_KCLASS_NORMQUANT);
+        k_normquant<<<batch, NQ_THREADS, 0, st>>>(u, d.d_model, L.norm_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum,
+                                                  tp, v.tap_stride, v.tl.off[DFSSM_TAP_XQ_IN], v.tl.off[DFSSM_TAP_S_IN]);
+        tm->end(); ++nl;
+
+        tm->begin(DFSSM_KCLASS_PROJ_IN);
+        k_proj<<<dim3(proj_grid(d.d_in_proj + d.r), (batch + PROJ_BT - 1) / PROJ_BT), PROJ_THREADS,
+                 proj_smem(d.d_model), st>>>(L.in_sign, L.in_A, d.d_in_proj, d.r, d.d_model, xq, xqp, ldq, qsum,
+                                             batch, acc, ld_acc, t);
+        tm->end(); ++nl;
+        if (tp) {
+            k_tap_copy_i32<<<dim3((d.d_in_proj + 255) / 256, batch), 256, 0, st>>>(acc, ld_acc, d.d_in_proj, tp,
+                                                                                  v.tap_stride, v.tl.off[DFSSM_TAP_ACC_IN]);
+            k_tap_copy_i32<<<dim3(1, batch), 64, 0, st>>>(t, T_STRIDE, d.r, tp, v.tap_stride, v.tl.off[DFSSM_TAP_T_IN]);
+            nl += 2;
+        }
+
+        tm->begin(DFSSM_KCLASS_SSM);
+        k_ssm<<<dim3(d.nheads * (d.headdim / SSM_PB), batch), SSM_THREADS, ssm_smem(d), st>>>(
+            L, d, acc, ld_acc, t, sx, conv, pos, ssm, g, tp, v.tap_stride, v.tl);
+        tm->end(); ++nl;
+
+        tm->begin(DFSSM_KCLASS_NORMQUANT);
+        k_normquant<<<batch, NQ_THREADS, 0, st>>>(g, d.d_inner, L.gnorm_w, d.d_inner, d.eps, xq, xqp, ldq, sx, qsum,
+                                                  tp, v.tap_stride, v.tl.off[DFSSM_TAP_GQ], v.tl.off[DFSSM_TAP_S_G]);
+        tm->end(); ++nl;
+
+        tm->begin(DFSSM_KCLASS_PROJ_OUT);
+        k_proj<<<dim3(proj_grid(d.d_model + d.r), (batch + PROJ_BT - 1) / PROJ_BT), PROJ_THREADS,
+                 proj_smem(d.d_inner), st>>>(L.out_sign, L.out_A, d.d_model, d.r, d.d_inner, xq, xqp, ldq, qsum,
+                                             batch, acc, ld_acc, t);
+        tm->end(); ++nl;
+        if (tp) {
+            k_tap_copy_i32<<<dim3((d.d_model + 255) / 256, batch), 256, 0, st>>>(acc, ld_acc, d.d_model, tp,
+                                                                                v.tap_stride, v.tl.off[DFSSM_TAP_ACC_OUT]);
+            k_tap_copy_i32<<<dim3(1, batch), 64, 0, st>>>(t, T_STRIDE, d.r, tp, v.tap_stride, v.tl.off[DFSSM_TAP_T_OUT]);
+            nl += 2;
+        }
+
+        tm->begin(DFSSM_KCLASS_EPI_OUT);
+        k_epi_out<<<dim3((d.d_model + EPI_THREADS - 1) / EPI_THREADS, batch), EPI_THREADS, 0, st>>>(
+            L, d.d_model, d.r, acc, ld_acc, t, sx, u, tp, v.tap_stride, v.tl.off[DFSSM_TAP_HIDDEN]);
+        tm->end(); ++nl;
+    }
+
+    tm->begin(DFSSM_KCLASS_NORMQUANT);
+    k_normquant<<<batch, NQ_THREADS, 0, st>>>(u, d.d_model, c->normf_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum,
+                                              nullptr, 0, 0, 0);
+    tm->end(); ++nl;
+
+    tm->begin(DFSSM_KCLASS_LMHEAD);
+    {
+        const int per = LM_THREADS / 32;
+        int gx = (d.vocab + per - 1) / per;
+        if (gx > 148 * 16) gx = 148 * 16;
+        k_lmhead<<<dim3(gx, (batch + PROJ_BT - 1) / PROJ_BT), LM_THREADS, lm_smem(d.d_model), st>>>(
+            c->emb, c->emb_s, d.vocab, d.d_model, xq, ldq, sx, batch, logits);
+    }
+    tm->end(); ++nl;
+
+    tm->begin(DFSSM_KCLASS_ARGMAX);
+    k_argmax<<<batch, AM_THREADS, 0, st>>>(logits, d.vocab, next, tokens, pos);
+    tm->end(); ++nl;
+
+    if (n_launch) *n_launch = nl;
+    CK(cudaGetLastError());
+    return DFSSM_OK;
+}
+
+int get_graph(dfssm_ctx* c, int batch, cudaGraphExec_t* out)
+{
+    dfssm_ctx* ctx = c;
+    for (auto& e : c->graphs)
+        if (e.batch == batch) { *out = e.exec; return DFSSM_OK; }
+    cudaGraph_t graph = nullptr;
+    CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+    const int rc = enqueue_step(c, batch, nullptr, nullptr);
+    cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    if (rc != DFSSM_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if (e != cudaSuccess) return fail(c, DFSSM_E_CUDA, "cudaStreamEndCapture failed: %s", cudaGetErrorString(e));
+    cudaGraphExec_t exec = nullptr;
+    e = cudaGraphInstantiate(&exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) return fail(c, DFSSM_E_CUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e));
+    if (c->graphs.size() >= 16) {               // bounded cache: drop the oldest
+        cudaGraphExecDestroy(c->graphs.front().exec);
+        c->graphs.erase(c->graphs.begin());
+    }
+    c->graphs.push_back({ batch, exec });
+    *out = exec;
+    return DFSSM_OK;
+}
+
+}  // namespace
+
+// =================================================================================================
+// exported C ABI
+// =================================================================================================
+extern "C" {
+
+size_t dfssm_arena_bytes(const dfssm_config* cfg)
+{
+    if (!valid_cfg(cfg)) return 0;
+    return carve(*cfg).total;
+}
+
+int dfssm_create(const dfssm_config* cfg, void* dev_arena, size_t arena_bytes, void* cuda_stream, dfssm_ctx** out)
+{
+    if (!out) return DFSSM_E_ARG;
+    *out = nullptr;
+    if (!valid_cfg(cfg) || !dev_arena || ((uintptr_t)dev_arena % ARENA_ALIGN)) return DFSSM_E_ARG;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return DFSSM_E_CUDA;
+    if (prop.major != 10) return DFSSM_E_ARCH;
+    dfssm_ctx* ctx = new (std::nothrow) dfssm_ctx();
+    if (!ctx) return DFSSM_E_ARG;
+    ctx->cfg = *cfg;
+    ctx->dm = make_dims(*cfg);
+    ctx->cv = carve(*cfg);
+    ctx->arena = (uint8_t*)dev_arena;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    ctx->loaded = false;
+    ctx->last_batch = 0;
+    ctx->pinned_tok = nullptr;
+    ctx->pinned_err = nullptr;
+    ctx->err[0] = 0;
+    *out = ctx;                       // handed out even on failure below so last_error can be read
+    if (arena_bytes < ctx->cv.total)
+        return fail(ctx, DFSSM_E_SIZE, "arena too small: %zu < %zu", arena_bytes, ctx->cv.total);
+    CK(cudaMallocHost((void**)&ctx->pinned_tok, sizeof(int32_t) * 2 * (size_t)cfg->max_batch));
+    CK(cudaMallocHost((void**)&ctx->pinned_err, sizeof(int)));
+    CK(cudaFuncSetAttribute(k_proj, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)proj_smem(8192)));
+    CK(cudaFuncSetAttribute(k_lmhead, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lm_smem(8192)));
+    // zero everything behind the weights: state, ring positions, activations, error flag
+    CK(cudaMemsetAsync(ctx->arena + ctx->cv.ssm, 0, ctx->cv.total - ctx->cv.ssm, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return DFSSM_OK;
+}
+
+int dfssm_load_weights(dfssm_ctx* ctx, const void* host_blob, size_t nbytes)
+{
+    if (!ctx || !host_blob) return DFSSM_E_ARG;
+    const Dims& d = ctx->dm;
+    const uint8_t* hb = (const uint8_t*)host_blob;
+    if (nbytes < 256 || memcmp(hb, "DFSSMW1\0", 8) != 0) return fail(ctx, DFSSM_E_SIZE, "bad magic or short blob");
+    uint32_t ver; int32_t hdr[9]; float eps; uint64_t total;
+    memcpy(&ver, hb + 8, 4); memcpy(hdr, hb + 12, 36); memcpy(&eps, hb + 48, 4); memcpy(&total, hb + 56, 8);
+    if (ver != 1) return fail(ctx, DFSSM_E_ARG, "unsupported blob version %u", ver);
+    const int32_t want[9] = { d.n_layers, d.d_model, d.d_inner, d.headdim, d.d_state, d.ngroups, 4, d.vocab, d.r };
+    for (int i = 0; i < 9; ++i)
+        if (hdr[i] != want[i]) return fail(ctx, DFSSM_E_ARG, "blob header field %d = %d does not match the config (%d)", i, hdr[i], want[i]);
+    if (eps != d.eps) return fail(ctx, DFSSM_E_ARG, "blob norm_eps does not match the config");
+    const size_t expect = blob_bytes_for(d);
+    if (total != nbytes || nbytes != expect)
+        return fail(ctx, DFSSM_E_SIZE, "blob size %zu does not match its header (%llu) / the shape (%zu)", nbytes,
+                    (unsigned long long)total, expect);
+
+    uint8_t* db = ctx->arena + ctx->cv.blob;
+    CK(cudaMemcpyAsync(db, hb, nbytes, cudaMemcpyHostToDevice, ctx->stream));
+    BlobWalk w;
+    const size_t dm = d.d_model, di = d.d_inner, dip = d.d_in_proj, r = d.r, cd = d.conv_dim, nh = d.nheads;
+    ctx->layers.assign((size_t)d.n_layers, LayerW());
+    for (int l = 0; l < d.n_layers; ++l) {
+        LayerW& L = ctx->layers[l];
+        L.norm_w = (const float*)(db + w.take(4 * dm));
+        L.in_sign = (const uint32_t*)(db + w.take(4 * dip * (dm / 32)));
+        L.in_row_scale = (const __half*)(db + w.take(2 * dip));
+        L.in_A = (const int8_t*)(db + w.take(r * dm));
+        L.in_a_s = (const float*)(db + w.take(4 * r));
+        L.in_B = (const int8_t*)(db + w.take(dip * r));
+        L.in_b_s = (const float*)(db + w.take(4 * dip));
+        L.conv_w = (const float*)(db + w.take(16 * cd));
+        L.conv_b = (const float*)(db + w.take(4 * cd));
+        L.A_log = (const float*)(db + w.take(4 * nh));
+        L.dt_bias = (const float*)(db + w.take(4 * nh));
+        L.D = (const float*)(db + w.take(4 * nh));
+        L.gnorm_w = (const float*)(db + w.take(4 * di));
+        L.out_sign = (const uint32_t*)(db + w.take(4 * dm * (di / 32)));
+        L.out_row_scale = (const __half*)(db + w.take(2 * dm));
+        L.out_A = (const int8_t*)(db + w.take(r * di));
+        L.out_a_s = (const float*)(db + w.take(4 * r));
+        L.out_B = (const int8_t*)(db + w.take(dm * r));
+        L.out_b_s = (const float*)(db + w.take(4 * dm));
+    }
+    ctx->emb = (const int8_t*)(db + w.take((size_t)d.vocab * dm));
+    ctx->emb_s = (const float*)(db + w.take(4 * (size_t)d.vocab));
+    ctx->normf_w = (const float*)(db + w.take(4 * dm));
+    CK(cudaStreamSynchronize(ctx->stream));
+    for (auto& e : ctx->graphs) cudaGraphExecDestroy(e.exec);
+    ctx->graphs.clear();
+    ctx->blob_bytes = nbytes;
+    ctx->loaded = true;
+    return DFSSM_OK;
+}
+
+int dfssm_reset_state(dfssm_ctx* ctx, int seq)
+{
+    if (!ctx) return DFSSM_E_ARG;
+    if (seq >= ctx->cfg.max_batch) return fail(ctx, DFSSM_E_ARG, "seq_index out of range");
+    const Dims& d = ctx->dm;
+    const Carve& v = ctx->cv;
+    const size_t B = ctx->cfg.max_batch, nl = d.n_layers > 0 ? d.n_layers : 1;
+    if (seq < 0) {
+        CK(cudaMemsetAsync(ctx->arena + v.ssm, 0, nl * B * v.ssm_elems * 4, ctx->stream));
+        CK(cudaMemsetAsync(ctx->arena + v.conv, 0, nl * B * (size_t)d.conv_dim * 16, ctx->stream));
+        return DFSSM_OK;
+    }
+    // one sequence of every layer: strided 2-D memsets (rows = layers)
+    CK(cudaMemset2DAsync(ctx->arena + v.ssm + (size_t)seq * v.ssm_elems * 4, B * v.ssm_elems * 4, 0,
+                         v.ssm_elems * 4, nl, ctx->stream));
+    CK(cudaMemset2DAsync(ctx->arena + v.conv + (size_t)seq * d.conv_dim * 16, B * (size_t)d.conv_dim * 16, 0,
+                         (size_t)d.conv_dim * 16, nl, ctx->stream));
+    return DFSSM_OK;
+}
+
+int dfssm_step(dfssm_ctx* ctx, const int32_t* tokens_dev, int batch)
+{
+    if (!ctx || !tokens_dev) return DFSSM_E_ARG;
+    if (!ctx->loaded) return fail(ctx, DFSSM_E_STATE, "dfssm_step before dfssm_load_weights");
+    if (batch < 1 || batch > ctx->cfg.max_batch) return fail(ctx, DFSSM_E_ARG, "batch %d outside [1, %d]", batch, ctx->cfg.max_batch);
+    // the step reads its tokens from the arena's token buffer.  After a step that buffer already
+    // holds the greedy tokens, so feeding dfssm_next_tokens' pointer back costs no copy at all.
+    int32_t* tok = at<int32_t>(ctx, ctx->cv.tok);
+    const int32_t* next = at<int32_t>(ctx, ctx->cv.next);
+    const bool resident = tokens_dev == tok || (tokens_dev == next && batch <= ctx->last_batch);
+    if (!resident)
+        CK(cudaMemcpyAsync(tok, tokens_dev, sizeof(int32_t) * (size_t)batch, cudaMemcpyDeviceToDevice, ctx->stream));
+    ctx->last_batch = batch;
+    if (ctx->cfg.flags & (DFSSM_FLAG_NO_GRAPH | DFSSM_FLAG_TAPS)) return enqueue_step(ctx, batch, nullptr, nullptr);
+    cudaGraphExec_t exec;
+    const int rc = get_graph(ctx, batch, &exec);
+    if (rc != DFSSM_OK) return rc;
+    CK(cudaGraphLaunch(exec, ctx->stream));
+    return DFSSM_OK;
+}
+
+int dfssm_step_host(dfssm_ctx* ctx, const int32_t* tokens_host, int batch, int32_t* next_host, float* logits_host)
+{
+    if (!ctx || !tokens_host || !next_host) return DFSSM_E_ARG;
+    if (batch < 1 || batch > ctx->cfg.max_batch) return fail(ctx, DFSSM_E_ARG, "batch %d outside [1, %d]", batch, ctx->cfg.max_batch);
+    int32_t* tok_dev = at<int32_t>(ctx, ctx->cv.tok);
+    memcpy(ctx->pinned_tok, tokens_host, sizeof(int32_t) * (size_t)batch);
+    CK(cudaMemcpyAsync(tok_dev, ctx->pinned_tok, sizeof(int32_t) * (size_t)batch, cudaMemcpyHostToDevice, ctx->stream));
+    const int rc = dfssm_step(ctx, tok_dev, batch);
+    if (rc != DFSSM_OK) return rc;
+    int32_t* stage = ctx->pinned_tok + ctx->cfg.max_batch;
+    CK(cudaMemcpyAsync(stage, at<int32_t>(ctx, ctx->cv.next), sizeof(int32_t) * (size_t)batch, cudaMemcpyDeviceToHost, ctx->stream));
+    if (logits_host)
+        CK(cudaMemcpyAsync(logits_host, at<float>(ctx, ctx->cv.logits), sizeof(float) * (size_t)batch * ctx->dm.vocab,
+                           cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    memcpy(next_host, stage, sizeof(int32_t) * (size_t)batch);
+    return DFSSM_OK;
+}
+
+int dfssm_logits(dfssm_ctx* ctx, const float** p)
+{
+    if (!ctx || !p) return DFSSM_E_ARG;
+    *p = at<float>(ctx, ctx->cv.logits);
+    return DFSSM_OK;
+}
+
+int dfssm_next_tokens(dfssm_ctx* ctx, const int32_t** p)
+{
+    if (!ctx || !p) return DFSSM_E_ARG;
+    *p = at<int32_t>(ctx, ctx->cv.next);
+    return DFSSM_OK;
+}
+
+int dfssm_hidden(dfssm_ctx* ctx, const float** p)
+{
+    if (!ctx || !p) return DFSSM_E_ARG;
+    *p = at<float>(ctx, ctx->cv.u);
+    return DFSSM_OK;
+}
+
+int dfssm_debug_tensor(dfssm_ctx* ctx, int layer, int which, int seq, const void** dev, size_t* nbytes)
+{
+    if (!ctx || !dev) return DFSSM_E_ARG;
+    if (!(ctx->cfg.flags & DFSSM_FLAG_TAPS)) return fail(ctx, DFSSM_E_STATE, "context created without DFSSM_FLAG_TAPS");
+    if (layer < 0 || layer >= ctx->dm.n_layers || which < 0 || which >= DFSSM_TAP_COUNT || seq < 0 || seq >= ctx->cfg.max_batch)
+        return fail(ctx, DFSSM_E_ARG, "tap index out of range");
+    const Carve& v = ctx->cv;
+    *dev = ctx->arena + v.taps + ((size_t)layer * ctx->cfg.max_batch + seq) * v.tap_stride + v.tl.off[which];
+    if (nbytes) *nbytes = tap_bytes(ctx->dm, which);
+    return DFSSM_OK;
+}
+
+static int state_copy(dfssm_ctx* ctx, int layer, int seq, float* ssm_h, size_t ssm_bytes, float* conv_h,
+                      size_t conv_bytes, bool to_host)
+{
+    if (!ctx) return DFSSM_E_ARG;
+    const Dims& d = ctx->dm;
+    const Carve& v = ctx->cv;
+    if (layer < 0 || layer >= d.n_layers || seq < 0 || seq >= ctx->cfg.max_batch) return fail(ctx, DFSSM_E_ARG, "state index out of range");
+    const size_t B = ctx->cfg.max_batch;
+    if (ssm_h && ssm_bytes != v.ssm_elems * 4) return fail(ctx, DFSSM_E_SIZE, "ssm state is %zu bytes", v.ssm_elems * 4);
+    if (conv_h && conv_bytes != (size_t)d.conv_dim * 12) return fail(ctx, DFSSM_E_SIZE, "conv state is %zu bytes", (size_t)d.conv_dim * 12);
+    CK(cudaStreamSynchronize(ctx->stream));
+    float* ssm_d = at<float>(ctx, v.ssm) + ((size_t)layer * B + seq) * v.ssm_elems;
+    float* ring_d = at<float>(ctx, v.conv) + ((size_t)layer * B + seq) * (size_t)d.conv_dim * 4;
+    if (ssm_h) {
+        if (to_host) CK(cudaMemcpy(ssm_h, ssm_d, ssm_bytes, cudaMemcpyDeviceToHost));
+        else CK(cudaMemcpy(ssm_d, ssm_h, ssm_bytes, cudaMemcpyHostToDevice));
+    }
+    if (conv_h) {
+        // ring <-> canonical [conv_dim][3] oldest first: the next step writes slot pos, so the three
+        // live samples are slots pos+1, pos+2, pos+3 (mod 4), oldest first
+        int32_t pos = 0;
+        CK(cudaMemcpy(&pos, at<int32_t>(ctx, v.pos) + seq, 4, cudaMemcpyDeviceToHost));
+        pos &= 3;
+        std::vector<float> ring((size_t)d.conv_dim * 4);
+        if (to_host) {
+            CK(cudaMemcpy(ring.data(), ring_d, ring.size() * 4, cudaMemcpyDeviceToHost));
+            for (int c = 0; c < d.conv_dim; ++c)
+                for (int j = 0; j < 3; ++j) conv_h[3 * (size_t)c + j] = ring[4 * (size_t)c + ((pos + 1 + j) & 3)];
+        } else {
+            for (int c = 0; c < d.conv_dim; ++c) {
+                ring[4 * (size_t)c + pos] = 0.0f;
+                for (int j = 0; j < 3; ++j) ring[4 * (size_t)c + ((pos + 1 + j) & 3)] = conv_h[3 * (size_t)c + j];
+            }
+            CK(cudaMemcpy(ring_d, ring.data(), ring.size() * 4, cudaMemcpyHostToDevice));
+        }
+    }
+    return DFSSM_OK;
+}
+
+int dfssm_get_state(dfssm_ctx* ctx, int layer, int seq, float* ssm_host, size_t ssm_bytes, float* conv_host, size_t conv_bytes)
+{
+    return state_copy(ctx, layer, seq, ssm_host, ssm_bytes, conv_host, conv_bytes, true);
+}
+
+int dfssm_set_state(dfssm_ctx* ctx, int layer, int seq, const float* ssm_host, size_t ssm_bytes, const float* conv_host, size_t conv_bytes)
+{
+    return state_copy(ctx, layer, seq, const_cast<float*>(ssm_host), ssm_bytes, const_cast<float*>(conv_host), conv_bytes, false);
+}
+
+int dfssm_sync(dfssm_ctx* ctx)
+{
+    if (!ctx) return DFSSM_E_ARG;
+    int* err_d = at<int>(ctx, ctx->cv.err);
+    CK(cudaMemcpyAsync(ctx->pinned_err, err_d, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    if (*ctx->pinned_err) {
+        CK(cudaMemsetAsync(err_d, 0, sizeof(int), ctx->stream));
+        return fail(ctx, DFSSM_E_TOKEN, "a token id outside [0, vocab) was clamped");
+    }
+    return DFSSM_OK;
+}
+
+int dfssm_launches_per_step(dfssm_ctx* ctx, int batch)
+{
+    if (!ctx || batch < 1) return DFSSM_E_ARG;
+    const int per_layer = (ctx->cfg.flags & DFSSM_FLAG_TAPS) ? 10 : 6;
+    return 1 + ctx->dm.n_layers * per_layer + 3;
+}
+
+int dfssm_time_kernels(dfssm_ctx* ctx, const int32_t* tokens_dev, int batch, int iters, float* out_us)
+{
+    if (!ctx || !tokens_dev || !out_us || iters < 1) return DFSSM_E_ARG;
+    if (!ctx->loaded) return fail(ctx, DFSSM_E_STATE, "dfssm_time_kernels before dfssm_load_weights");
+    if (batch < 1 || batch > ctx->cfg.max_batch) return fail(ctx, DFSSM_E_ARG, "batch out of range");
+    double sum[DFSSM_KCLASS_COUNT] = { 0 };
+    for (int it = 0; it < iters; ++it) {
+        KTimer tm;
+        tm.on = true;
+        tm.st = ctx->stream;
+        CK(cudaMemcpyAsync(at<int32_t>(ctx, ctx->cv.tok), tokens_dev, sizeof(int32_t) * (size_t)batch,
+                           cudaMemcpyDeviceToDevice, ctx->stream));
+        const int rc = enqueue_step(ctx, batch, &tm, nullptr);
+        cudaError_t e = cudaStreamSynchronize(ctx->stream);
+        if (rc == DFSSM_OK && e == cudaSuccess)
+            for (size_t i = 0; i < tm.cls.size(); ++i) {
+                float ms = 0.f;
+                cudaEventElapsedTime(&ms, tm.ev[2 * i], tm.ev[2 * i + 1]);
+                sum[tm.cls[i]] += 1e3 * ms;
+            }
+        for (auto ev : tm.ev) cudaEventDestroy(ev);
+        if (rc != DFSSM_OK) return rc;
+        if (e != cudaSuccess) return fail(ctx, DFSSM_E_CUDA, "sync failed: %s", cudaGetErrorString(e));
+    }
+    for (int k = 0; k < DFSSM_KCLASS_COUNT; ++k) out_us[k] = (float)(sum[k] / iters);
+    return DFSSM_OK;
+}
+
+const char* dfssm_last_error(const dfssm_ctx* ctx) { return ctx ? ctx->err : ""; }
+
+void dfssm_destroy(dfssm_ctx* ctx)
+{
+    if (!ctx) return;
+    for (auto& e : ctx->graphs) cudaGraphExecDestroy(e.exec);
+    if (ctx->pinned_tok) cudaFreeHost(ctx->pinned_tok);
+    if (ctx->pinned_err) cudaFreeHost(ctx->pinned_err);
+    delete ctx;
+}
+
+}  // extern "C"

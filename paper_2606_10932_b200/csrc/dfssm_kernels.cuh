@@ -1,0 +1,487 @@
+// Kernel-chain implementation of the DF-SSM decode step ("chain" path): one kernel per row of
+// the step list in include/dfssm.h, replayed as one CUDA graph.  Works for any batch.
+// The fused persistent kernel for small batches lives in dfssm_mega.cuh.
+#pragma once
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "dfssm_math.cuh"
+
+namespace dfssm {
+
+// ---- device-side view of one layer's weights (pointers into the arena copy of the blob) ----
+struct LayerW {
+    const float* norm_w;
+    const uint32_t* in_sign; const __half* in_row_scale;
+    const int8_t* in_A; const float* in_a_s; const int8_t* in_B; const float* in_b_s;
+    const float* conv_w; const float* conv_b;
+    const float* A_log; const float* dt_bias; const float* D;
+    const float* gnorm_w;
+    const uint32_t* out_sign; const __half* out_row_scale;
+    const int8_t* out_A; const float* out_a_s; const int8_t* out_B; const float* out_b_s;
+};
+
+struct Dims {
+    int n_layers, d_model, d_inner, headdim, d_state, ngroups, vocab, r;
+    int nheads, d_in_proj, conv_dim;
+    float eps;
+};
+
+// debug taps: byte offsets inside one (layer, seq) record; stride = off[DFSSM_TAP_COUNT]
+struct TapLayout { uint32_t off[16]; };
+
+constexpr int T_STRIDE = 64;      // ints per sequence in the LoRA stage-1 buffer t
+constexpr int PROJ_BT = 8;        // sequences per CTA tile in the projection kernels
+constexpr int SSM_PB = 16;        // (head, p) rows per CTA in the SSM kernel
+
+// =============================================================================================
+// S0  embedding: u = e_s[tok] * float(E[tok,:])
+// =============================================================================================
+__global__ void k_embed(const int32_t* __restrict__ tokens, const int8_t* __restrict__ E,
+                        const float* __restrict__ e_s, int vocab, int d, float* __restrict__ u,
+                        int* __restrict__ err)
+{
+    const int b = blockIdx.y;
+    int tok = tokens[b];
+    if (tok < 0 || tok >= vocab) {
+        if (threadIdx.x == 0 && blockIdx.x == 0) atomicOr(err, 1);
+        tok = tok < 0 ? 0 : vocab - 1;
+    }
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < d) u[(size_t)b * d + k] = fmul(e_s[tok], (float)E[(size_t)tok * d + k]);
+}
+
+// =============================================================================================
+// S1 / S6(b) / S8(a)  RMSNorm + per-token absmax int8 quantiser (R4, R13)
+//   rstd = 1/sqrt(mean(v^2)+eps); t_k = v_k*w_k; amax = max|t_k|; q_k = clamp(rint(t_k*(127/amax)));
+//   s = (amax*rstd)/127.  Writes the codes twice: canonical order (xq) and the bit-plane order
+//   (xqp) the masked-dp4a sign dot product reads: inside each group of 32, canonical position
+//   8j+i goes to position 4i+j.  Also writes sum_k q_k (the sign dot needs 2*P - sum q).
+//   One CTA per sequence.
+// =============================================================================================
+constexpr int NQ_THREADS = 512;
+
+__global__ void __launch_bounds__(NQ_THREADS)
+k_normquant(const float* __restrict__ v, int ldv, const float* __restrict__ w, int d, float eps,
+            int8_t* __restrict__ xq, int8_t* __restrict__ xqp, int ldq, float* __restrict__ s_out,
+            int32_t* __restrict__ qsum_out, uint8_t* __restrict__ taps, uint32_t tap_stride,
+            uint32_t tap_q_off, uint32_t tap_s_off)
+{
+    __shared__ double sh_d[NQ_THREADS / 32];
+    __shared__ float sh_f[NQ_THREADS / 32];
+    __shared__ int sh_i[NQ_THREADS / 32];
+    __shared__ float sh_bcast[2];
+    const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const float* vb = v + (size_t)b * ldv;
+
+    double ss = 0.0;
+    float amax = 0.0f;
+    for (int k = tid; k < d; k += NQ_THREADS) {
+        const float x = vb[k];
+        ss = dacc(ss, x, x);
+        amax = fmaxf(amax, fabsf(fmul(x, w[k])));
+    }
+    ss = warp_sum(ss);
+    amax = warp_max(amax);
+    if (lane == 0) { sh_d[wid] = ss; sh_f[wid] = amax; }
+    __syncthreads();
+    if (wid == 0) {
+        double s2 = lane < NQ_THREADS / 32 ? sh_d[lane] : 0.0;
+        float m2 = lane < NQ_THREADS / 32 ? sh_f[lane] : 0.0f;
+        s2 = warp_sum(s2);
+        m2 = warp_max(m2);
+        if (lane == 0) {
+            const float ms = (float)(s2 / (double)d);
+            const float rstd = fdiv(1.0f, __fsqrt_rn(fadd(ms, eps)));
+            sh_bcast[0] = m2;
+            sh_bcast[1] = rstd;
+        }
+    }
+    __syncthreads();
+    amax = sh_bcast[0];
+    const float rstd = sh_bcast[1];
+    const float inv = amax == 0.0f ? 0.0f : fdiv(127.0f, amax);
+    const float s = amax == 0.0f ? 0.0f : fdiv(fmul(amax, rstd), 127.0f);
+    int qs = 0;
+    int8_t* qb = xq + (size_t)b * ldq;
+    int8_t* qpb = xqp + (size_t)b * ldq;
+    uint8_t* tp = taps ? taps + (size_t)b * tap_stride : nullptr;
+    for (int k = tid; k < d; k += NQ_THREADS) {
+        const int q = amax == 0.0f ? 0 : quant_code(fmul(vb[k], w[k]), inv);
+        qs += q;
+        qb[k] = (int8_t)q;
+        const int p = k & 31;
+        qpb[(k & ~31) + 4 * (p & 7) + (p >> 3)] = (int8_t)q;
+        if (tp) ((int8_t*)(tp + tap_q_off))[k] = (int8_t)q;
+    }
+    qs = warp_sum_i(qs);
+    if (lane == 0) sh_i[wid] = qs;
+    __syncthreads();
+    if (tid == 0) {
+        int tot = 0;
+        for (int i = 0; i < NQ_THREADS / 32; ++i) tot += sh_i[i];
+        qsum_out[b] = tot;
+        s_out[b] = s;
+        if (tp) *(float*)(tp + tap_s_off) = s;
+    }
+}
+
+// =============================================================================================
+// S2 + S3 stage 1 (and S7): bit-packed sign matvec + int8 LoRA down-projection, exact int32.
+//   rows [0, rows)      : acc_i = sum_k sign_ik * q_k = 2 * sum_{bit_ik = 1} q_k - sum_k q_k
+//   rows [rows, rows+r) : t_j   = sum_k A_jk * q_k
+//   One warp per row; a lane takes whole 32-bit sign words.  For each word the eight masks
+//   0x01010101 << i pick bit i of every byte; dp4a(u8 mask bytes, s8 codes) against the codes
+//   stored in bit-plane order gives 2^i * (partial sum); the eight partial sums are recombined
+//   exactly as sum_i a_i * 2^(7-i) = 128 * P.
+//   grid = (row blocks, batch tiles of PROJ_BT); dynamic smem = PROJ_BT * 2 * K bytes.
+// =============================================================================================
+constexpr int PROJ_THREADS = 256;
+
+__global__ void __launch_bounds__(PROJ_THREADS)
+k_proj(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int rows, int r, int K,
+       const int8_t* __restrict__ xq, const int8_t* __restrict__ xqp, int ldq,
+       const int32_t* __restrict__ qsum, int batch, int32_t* __restrict__ acc, int ld_acc,
+       int32_t* __restrict__ t)
+{
+    extern __shared__ __align__(16) uint8_t smem[];
+    const int b0 = blockIdx.y * PROJ_BT;
+    const int nb = min(PROJ_BT, batch - b0);
+    int8_t* sq = (int8_t*)smem;                    // [nb][K] canonical
+    int8_t* sqp = sq + (size_t)PROJ_BT * K;        // [nb][K] bit-plane order
+    for (int i = threadIdx.x; i < nb * (K / 16); i += PROJ_THREADS) {
+        const int bb = i / (K / 16), c = i % (K / 16);
+        ((int4*)sq)[bb * (K / 16) + c] = ((const int4*)(xq + (size_t)(b0 + bb) * ldq))[c];
+        ((int4*)sqp)[bb * (K / 16) + c] = ((const int4*)(xqp + (size_t)(b0 + bb) * ldq))[c];
+    }
+    __syncthreads();
+
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int W = K / 32;
+    const int rows_total = rows + r;
+    for (int row = blockIdx.x * (PROJ_THREADS / 32) + wid; row < rows_total;
+         row += gridDim.x * (PROJ_THREADS / 32)) {
+        if (row < rows) {
+            const uint32_t* wrow = sign + (size_t)row * W;
+            int p128[PROJ_BT];
+#pragma unroll
+            for (int bb = 0; bb < PROJ_BT; ++bb) p128[bb] = 0;
+            for (int w = lane; w < W; w += 32) {
+                const uint32_t bits = __ldg(wrow + w);
+#pragma unroll
+                for (int bb = 0; bb < PROJ_BT; ++bb) {
+                    if (bb < nb) {
+                        const int4 qa = *(const int4*)(sqp + (size_t)bb * K + 32 * w);
+                        const int4 qb = *(const int4*)(sqp + (size_t)bb * K + 32 * w + 16);
+                        int a;
+                        a = dp4a_us(bits & 0x01010101u, qa.x, 0) * 128;
+                        a += dp4a_us(bits & 0x02020202u, qa.y, 0) * 64;
+                        a += dp4a_us(bits & 0x04040404u, qa.z, 0) * 32;
+                        a += dp4a_us(bits & 0x08080808u, qa.w, 0) * 16;
+                        a += dp4a_us(bits & 0x10101010u, qb.x, 0) * 8;
+                        a += dp4a_us(bits & 0x20202020u, qb.y, 0) * 4;
+                        a += dp4a_us(bits & 0x40404040u, qb.z, 0) * 2;
+                        a += dp4a_us(bits & 0x80808080u, qb.w, 0);
+                        p128[bb] += a;
+                    }
+                }
+            }
+#pragma unroll
+            for (int bb = 0; bb < PROJ_BT; ++bb) {
+                if (bb < nb) {
+                    const int p = warp_sum_i(p128[bb]) / 128;    // exact: every term is a multiple of 128
+                    if (lane == 0) acc[(size_t)(b0 + bb) * ld_acc + row] = 2 * p - qsum[b0 + bb];
+                }
+            }
+        } else {
+            const int j = row - rows;
+            const int4* arow = (const int4*)(A + (size_t)j * K);
+            int s[PROJ_BT];
+#pragma unroll
+            for (int bb = 0; bb < PROJ_BT; ++bb) s[bb] = 0;
+            for (int c = lane; c < K / 16; c += 32) {
+                const int4 a4 = __ldg(arow + c);
+#pragma unroll
+                for (int bb = 0; bb < PROJ_BT; ++bb) {
+                    if (bb < nb) {
+                        const int4 q4 = *(const int4*)(sq + (size_t)bb * K + 16 * c);
+                        int a = s[bb];
+                        a = dp4a_ss(a4.x, q4.x, a);
+                        a = dp4a_ss(a4.y, q4.y, a);
+                        a = dp4a_ss(a4.z, q4.z, a);
+                        a = dp4a_ss(a4.w, q4.w, a);
+                        s[bb] = a;
+                    }
+                }
+            }
+#pragma unroll
+            for (int bb = 0; bb < PROJ_BT; ++bb) {
+                if (bb < nb) {
+                    const int tot = warp_sum_i(s[bb]);
+                    if (lane == 0) t[(size_t)(b0 + bb) * T_STRIDE + j] = tot;
+                }
+            }
+        }
+    }
+}
+
+// S3 stage 2 + dequantisation for one output row (Eq. 3; R6, R7):
+//   out = s_x * ( w_s[i]*float(acc_i) + b_s[i]*float( sum_j float(B_ij) * v_j ) ),  v_j = a_s[j]*float(t_j)
+// the sum over j runs in binary64, in index order, and is rounded once.
+__device__ __forceinline__ float proj_epilogue_row(int acc_i, const __half* __restrict__ row_scale,
+                                                   const int8_t* __restrict__ B,
+                                                   const float* __restrict__ b_s, int i, int r,
+                                                   const float* v_sh, float s_x)
+{
+    double lo = 0.0;
+    const int8_t* brow = B + (size_t)i * r;
+    for (int j = 0; j < r; ++j) lo = dacc(lo, (float)brow[j], v_sh[j]);
+    const float lo_f = (float)lo;
+    const float m1 = fmul(__half2float(row_scale[i]), (float)acc_i);
+    const float m2 = fmul(b_s[i], lo_f);
+    return fmul(s_x, fadd(m1, m2));
+}
+
+// =============================================================================================
+// S3 stage 2 (for the rows a head needs) + S4 conv step + S5 state update/readout + S6 gate.
+//   grid = (nheads * headdim/SSM_PB, batch); one CTA owns SSM_PB (head, p) rows of the state.
+//   The B and C rows are recomputed by every CTA of the group (256 rows of 32 fp64 FMAs: cheap);
+//   only the first CTA of a group stores their new conv sample.
+//   Conv state is a 4-slot ring per channel: the sample of step t lives in slot t%4, so the
+//   readers of a step never touch the slot its owner writes.
+// =============================================================================================
+constexpr int SSM_THREADS = 256;
+
+__global__ void __launch_bounds__(SSM_THREADS)
+k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int32_t* __restrict__ t,
+      const float* __restrict__ s_x, float* __restrict__ conv_ring /* [batch][conv_dim][4] */,
+      const int32_t* __restrict__ pos /* [batch] */, float* __restrict__ ssm /* [batch][h][p][n] */,
+      float* __restrict__ g /* [batch][d_inner] */, uint8_t* __restrict__ taps, uint32_t tap_stride,
+      TapLayout tl)
+{
+    extern __shared__ __align__(16) uint8_t smem[];
+    float* v_sh = (float*)smem;                    // [64]
+    float* Bc = v_sh + 64;                         // [d_state]
+    float* Cc = Bc + dm.d_state;                   // [d_state]
+    float* xs = Cc + dm.d_state;                   // [SSM_PB]
+    float* zs = xs + SSM_PB;                       // [SSM_PB]
+    float* dts = zs + SSM_PB;                      // [1] (+pad)
+
+    const int b = blockIdx.y;
+    const int pblocks = dm.headdim / SSM_PB;
+    const int h = blockIdx.x / pblocks, pblk = blockIdx.x % pblocks;
+    const int p0 = pblk * SSM_PB;
+    const int hpg = dm.nheads / dm.ngroups;
+    const int grp = h / hpg;
+    const bool bc_owner = (h % hpg == 0) && pblk == 0;
+    const int tid = threadIdx.x;
+    const int32_t* accb = acc + (size_t)b * ld_acc;
+    const float sx = s_x[b];
+    const int ps = pos[b] & 3;
+    uint8_t* tp = taps ? taps + (size_t)b * tap_stride : nullptr;
+
+    if (tid < dm.r) v_sh[tid] = fmul(L.in_a_s[tid], (float)t[(size_t)b * T_STRIDE + tid]);
+    __syncthreads();
+
+    const int gs = dm.ngroups * dm.d_state;
+    const int n_rows = 2 * SSM_PB + 2 * dm.d_state + 1;
+    for (int i = tid; i < n_rows; i += SSM_THREADS) {
+        int row, kind, idx;      // kind 0 z, 1 x, 2 B, 3 C, 4 dt
+        if (i < SSM_PB) { kind = 0; idx = i; row = h * dm.headdim + p0 + idx; }
+        else if (i < 2 * SSM_PB) { kind = 1; idx = i - SSM_PB; row = dm.d_inner + h * dm.headdim + p0 + idx; }
+        else if (i < 2 * SSM_PB + dm.d_state) { kind = 2; idx = i - 2 * SSM_PB; row = 2 * dm.d_inner + grp * dm.d_state + idx; }
+        else if (i < 2 * SSM_PB + 2 * dm.d_state) { kind = 3; idx = i - 2 * SSM_PB - dm.d_state; row = 2 * dm.d_inner + gs + grp * dm.d_state + idx; }
+        else { kind = 4; idx = 0; row = 2 * dm.d_inner + 2 * gs + h; }
+        const float val = proj_epilogue_row(accb[row], L.in_row_scale, L.in_B, L.in_b_s, row, dm.r, v_sh, sx);
+        const bool owner = (kind == 0 || kind == 1) || (kind == 4 && pblk == 0) || bc_owner;
+        if (tp && owner) ((float*)(tp + tl.off[4]))[row] = val;                    // ZXBCDT
+        if (kind == 0) {
+            zs[idx] = val;
+        } else if (kind == 4) {
+            const float dtv = sp_softplusf(fadd(val, L.dt_bias[h]));
+            dts[0] = dtv;
+            if (tp && pblk == 0) ((float*)(tp + tl.off[6]))[h] = dtv;              // DT
+        } else {
+            const int c = row - dm.d_inner;                                        // conv channel
+            float* ring = conv_ring + ((size_t)b * dm.conv_dim + c) * 4;
+            const float4 rg = *(const float4*)ring;
+            const float sl[4] = { rg.x, rg.y, rg.z, rg.w };
+            const float s0 = sl[(ps + 1) & 3], s1 = sl[(ps + 2) & 3], s2 = sl[(ps + 3) & 3];
+            const float4 cw = *(const float4*)(L.conv_w + 4 * (size_t)c);
+            float o = L.conv_b[c];
+            o = ffma(cw.x, s0, o);
+            o = ffma(cw.y, s1, o);
+            o = ffma(cw.z, s2, o);
+            o = ffma(cw.w, val, o);
+            const float cv = siluf(o);
+            if (kind == 1 || bc_owner) {
+                ring[ps] = val;
+                if (tp) ((float*)(tp + tl.off[5]))[c] = cv;                        // XBC_CONV
+            }
+            if (kind == 1) xs[idx] = cv; else if (kind == 2) Bc[idx] = cv; else Cc[idx] = cv;
+        }
+    }
+    __syncthreads();
+
+    const float dtv = dts[0];
+    const float An = -sp_expf(L.A_log[h]);
+    const float dA = sp_expf(fmul(dtv, An));
+    const int p = tid >> 4, l16 = tid & 15;       // 16 rows x 16 lanes
+    const float xv = xs[p];
+    const float dtx = fmul(dtv, xv);
+    float* Hr = ssm + (((size_t)b * dm.nheads + h) * dm.headdim + p0 + p) * dm.d_state;
+    double a = 0.0;
+    for (int n4 = l16; n4 < dm.d_state / 4; n4 += 16) {
+        float4 hv = *(const float4*)(Hr + 4 * n4);
+        const float4 bv = *(const float4*)(Bc + 4 * n4);
+        const float4 cv = *(const float4*)(Cc + 4 * n4);
+        hv.x = ffma(dA, hv.x, fmul(dtx, bv.x));
+        hv.y = ffma(dA, hv.y, fmul(dtx, bv.y));
+        hv.z = ffma(dA, hv.z, fmul(dtx, bv.z));
+        hv.w = ffma(dA, hv.w, fmul(dtx, bv.w));
+        *(float4*)(Hr + 4 * n4) = hv;
+        a = dacc(a, cv.x, hv.x);
+        a = dacc(a, cv.y, hv.y);
+        a = dacc(a, cv.z, hv.z);
+        a = dacc(a, cv.w, hv.w);
+    }
+#pragma unroll
+    for (int o = 8; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o, 16);
+    if (l16 == 0) {
+        a = dacc(a, L.D[h], xv);
+        const float y = (float)a;
+        const float gv = fmul(y, siluf(zs[p]));
+        const int ch = h * dm.headdim + p0 + p;
+        g[(size_t)b * dm.d_inner + ch] = gv;
+        if (tp) { ((float*)(tp + tl.off[7]))[ch] = y; ((float*)(tp + tl.off[8]))[ch] = gv; }
+    }
+}
+
+// =============================================================================================
+// S7 epilogue + residual: u_i <- u_i + s_g*( w_s[i]*acc_i + b_s[i]*lo_i )
+// =============================================================================================
+constexpr int EPI_THREADS = 128;
+
+__global__ void __launch_bounds__(EPI_THREADS)
+k_epi_out(LayerW L, int d_model, int r, const int32_t* __restrict__ acc, int ld_acc,
+          const int32_t* __restrict__ t, const float* __restrict__ s_g, float* __restrict__ u,
+          uint8_t* __restrict__ taps, uint32_t tap_stride, uint32_t tap_hidden_off)
+{
+    __shared__ float v_sh[64];
+    const int b = blockIdx.y;
+    if (threadIdx.x < r) v_sh[threadIdx.x] = fmul(L.out_a_s[threadIdx.x], (float)t[(size_t)b * T_STRIDE + threadIdx.x]);
+    __syncthreads();
+    const int i = blockIdx.x * EPI_THREADS + threadIdx.x;
+    if (i >= d_model) return;
+    const float o = proj_epilogue_row(acc[(size_t)b * ld_acc + i], L.out_row_scale, L.out_B, L.out_b_s, i, r,
+                                      v_sh, s_g[b]);
+    const float un = fadd(u[(size_t)b * d_model + i], o);
+    u[(size_t)b * d_model + i] = un;
+    if (taps) ((float*)(taps + (size_t)b * tap_stride + tap_hidden_off))[i] = un;
+}
+
+// debug-only: copy int32 vectors into the taps (acc, t)
+__global__ void k_tap_copy_i32(const int32_t* __restrict__ src, int ld_src, int n, uint8_t* __restrict__ taps,
+                               uint32_t tap_stride, uint32_t off)
+{
+    const int b = blockIdx.y;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) ((int32_t*)(taps + (size_t)b * tap_stride + off))[i] = src[(size_t)b * ld_src + i];
+}
+
+// =============================================================================================
+// S8  tied int8 LM head on the quantised final hidden (R16):
+//   logit_v = float( sum_k E_vk * hq_k ) * (s_h * e_s[v]);  one warp per vocabulary row.
+// =============================================================================================
+constexpr int LM_THREADS = 256;
+
+__global__ void __launch_bounds__(LM_THREADS)
+k_lmhead(const int8_t* __restrict__ E, const float* __restrict__ e_s, int vocab, int K,
+         const int8_t* __restrict__ xq, int ldq, const float* __restrict__ s_h, int batch,
+         float* __restrict__ logits)
+{
+    extern __shared__ __align__(16) uint8_t smem[];
+    const int b0 = blockIdx.y * PROJ_BT;
+    const int nb = min(PROJ_BT, batch - b0);
+    int8_t* sq = (int8_t*)smem;
+    for (int i = threadIdx.x; i < nb * (K / 16); i += LM_THREADS) {
+        const int bb = i / (K / 16), c = i % (K / 16);
+        ((int4*)sq)[bb * (K / 16) + c] = ((const int4*)(xq + (size_t)(b0 + bb) * ldq))[c];
+    }
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (int row = blockIdx.x * (LM_THREADS / 32) + wid; row < vocab; row += gridDim.x * (LM_THREADS / 32)) {
+        const int4* erow = (const int4*)(E + (size_t)row * K);
+        int s[PROJ_BT];
+#pragma unroll
+        for (int bb = 0; bb < PROJ_BT; ++bb) s[bb] = 0;
+        for (int c = lane; c < K / 16; c += 32) {
+            const int4 a4 = __ldg(erow + c);
+#pragma unroll
+            for (int bb = 0; bb < PROJ_BT; ++bb) {
+                if (bb < nb) {
+                    const int4 q4 = *(const int4*)(sq + (size_t)bb * K + 16 * c);
+                    int a = s[bb];
+                    a = dp4a_ss(a4.x, q4.x, a);
+                    a = dp4a_ss(a4.y, q4.y, a);
+                    a = dp4a_ss(a4.z, q4.z, a);
+                    a = dp4a_ss(a4.w, q4.w, a);
+                    s[bb] = a;
+                }
+            }
+        }
+        const float es = e_s[row];
+#pragma unroll
+        for (int bb = 0; bb < PROJ_BT; ++bb) {
+            if (bb < nb) {
+                const int tot = warp_sum_i(s[bb]);
+                if (lane == 0) logits[(size_t)(b0 + bb) * vocab + row] = fmul((float)tot, fmul(s_h[b0 + bb], es));
+            }
+        }
+    }
+}
+
+// greedy token: argmax with the lowest index on ties; also advances the conv ring position
+constexpr int AM_THREADS = 1024;
+
+__global__ void __launch_bounds__(AM_THREADS)
+k_argmax(const float* __restrict__ logits, int vocab, int32_t* __restrict__ next, int32_t* __restrict__ tok,
+         int32_t* __restrict__ pos)
+{
+    __shared__ float sv[AM_THREADS / 32];
+    __shared__ int si[AM_THREADS / 32];
+    const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const float* lg = logits + (size_t)b * vocab;
+    float best = -INFINITY;
+    int bi = 0x7fffffff;
+    for (int i = tid; i < vocab; i += AM_THREADS) {
+        const float x = lg[i];
+        if (x > best || (x == best && i < bi)) { best = x; bi = i; }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const float ov = __shfl_xor_sync(0xffffffffu, best, o);
+        const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+        if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+    }
+    if (lane == 0) { sv[wid] = best; si[wid] = bi; }
+    __syncthreads();
+    if (wid == 0) {
+        best = sv[lane];
+        bi = si[lane];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const float ov = __shfl_xor_sync(0xffffffffu, best, o);
+            const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+        }
+        if (lane == 0) {
+            next[b] = bi == 0x7fffffff ? 0 : bi;
+            tok[b] = next[b];                      // the next step's input if the caller decodes greedily
+            pos[b] = (pos[b] + 1) & 3;
+        }
+    }
+}
+
+}  // namespace dfssm
