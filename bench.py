@@ -209,3 +209,175 @@ def workload_name(cfg_idx: int, batch: int) -> str:
              2: "cfg2 Mamba-2-1.3B-shape DF-SSM (48 layers, d_model 2048, d_state 128, LoRA r32)",
              3: "cfg3 Mamba-2-1.3B-shape DF-SSM batch sweep", 4: "cfg4 Mamba-2-2.7B-shape DF-SSM"}
     return f"{names.get(cfg_idx, f'cfg{cfg_idx}')}, batch {batch}, greedy decode after a uniform-random prompt"
+
+
+# ---------------------------------------------------------------------------------------------
+# own arm: the CUDA path through the C ABI
+# ---------------------------------------------------------------------------------------------
+def run_ours(args, s, blob):
+    import torch
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the DF-SSM step has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    from paper_2606_10932_b200 import build
+    build.build()
+    import paper_2606_10932_b200 as pk
+
+    B = args.batch
+    m = pk.Model(pk.Config.from_shape(s, max_batch=B), blob, device=f"cuda:{local}")
+    # every rank is an independent replica with its own token streams ("replicas only")
+    prompt = ds.token_batch(s.vocab, max(args.warmup, 1), seed=1000 * rank + args.config, batch=B)
+    prompt_dev = [torch.from_numpy(prompt[t]).cuda() for t in range(prompt.shape[0])]
+    nxt = m.next_tokens()[:B]
+
+    def barrier():
+        m.sync()
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- device-resident leg: W prompt steps (untimed), then K greedy steps (timed) ----
+    for t in range(args.warmup):
+        m.step(prompt_dev[t])
+    if args.warmup == 0:
+        m.step(prompt_dev[0])
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.15)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    with torch.cuda.stream(m.stream):
+        e0.record()
+        for _ in range(args.steps):
+            m.step(nxt)
+        e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = m.launches_per_step(B) * args.steps
+
+    # ---- end-to-end leg: host buffers through dfssm_step_host, copies inside the timed region ----
+    tok_h = np.ascontiguousarray(m.next_tokens()[:B].cpu().numpy(), np.int32)
+    nxt_h = np.zeros(B, np.int32)
+    e2e_steps = max(8, min(args.steps, 256))
+    for _ in range(3):
+        m.step_host(tok_h, nxt_h)
+        tok_h[:] = nxt_h
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        m.step_host(tok_h, nxt_h)
+        tok_h[:] = nxt_h
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+
+    # ---- per-kernel-class device times (CUDA events on the library's stream, eager chain) ----
+    kt = m.time_kernels(nxt, iters=8)
+    barrier()
+
+    if dist is not None:
+        tt = torch.tensor([ms, e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms, e2e_s = float(tt[0]), float(tt[1])
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    ab = algorithmic_bytes(s, B)
+    value = world * B * args.steps / (ms * 1e-3)
+    e2e_val = world * B * e2e_steps / e2e_s
+    peak, peak_src = measured_peak()
+    step_gbs = ab["total"] * (args.steps / (ms * 1e-3)) / 1e9
+    kb = kernel_class_bytes(s, B)
+    L = s.n_layers
+    counts = {"embed": 1, "normquant": 2 * L + 1, "proj_in": L, "ssm": L, "proj_out": L, "epi_out": L,
+              "lmhead": 1, "argmax": 1}
+    # dominant kernel class = the one with the largest share of the step's device time
+    dom = max(kt, key=lambda k: kt[k])
+    per_launch_us = kt[dom] / max(1, counts.get(dom, 1))
+    achieved = kb[dom] / (per_launch_us * 1e-6) / 1e9 if per_launch_us > 0 else 0.0
+    roofline = {
+        "bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+        "frac": achieved / peak, "traffic": TRAFFIC_NCU.get(dom), "peak_source": peak_src,
+        "bytes_per_launch": kb[dom], "us_per_launch": per_launch_us,
+        "whole_step": {"algorithmic_bytes_per_step": ab["total"], "bj_formula_bytes_per_step": ab["bj_formula"],
+                       "achieved_GBps": step_gbs, "frac_of_measured": step_gbs / peak,
+                       "frac_of_nominal_8TBps": step_gbs / NOMINAL_HBM_GBS,
+                       "bj_formula_frac_of_nominal_8TBps": ab["bj_formula"] * (args.steps / (ms * 1e-3)) / 1e9 / NOMINAL_HBM_GBS},
+        "kernel_us_per_step": kt,
+    }
+
+    cpu_baseline = None
+    if world == 1 and not args.no_cpu_baseline:
+        v, n, dt, thr = time_oracle(s, blob, args.config, B, budget_s=15.0, max_steps=64)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": thr, "kind": "oracle",
+                        "sample": f"{n} greedy decode steps of the same workload after 2 prompt steps ({dt:.1f} s)"}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int8 x {-1,+1} -> int32; fp32 state", "data": "synthetic",
+        "config": {"workload": workload_name(args.config, B), "seed": args.config, "batch_per_gpu": B,
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": f"inputs larger than L2: {ab['total'] / 1e6:.0f} MB streamed per step vs ~126 MB L2"},
+        "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 4 * B, "d2h_bytes_per_step": 4 * B,
+                "steps": e2e_steps, "call": "dfssm_step_host (host token in, host greedy token out)"},
+        "gpu_launches": launches,
+        "clocks": clocks,
+        "roofline": roofline,
+        "cpu_baseline": cpu_baseline,
+    }
+    print(json.dumps(out), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of each kernel class, from the committed
+# `ncu --set full` capture of this command (profiles/); None until captured
+TRAFFIC_NCU = {}
+try:
+    _t = ROOT / "profiles" / "traffic.json"
+    if _t.exists():
+        TRAFFIC_NCU = json.loads(_t.read_text())
+except Exception:
+    TRAFFIC_NCU = {}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=512)
+    ap.add_argument("--warmup", type=int, default=128)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--batch", type=int, default=1)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference" and int(os.environ.get("RANK", "0")) != 0:
+        return
+    s = ds.shape_for_config(args.config)
+    blob = ds.make_blob(s, args.config)
+    if args.impl == "reference":
+        run_reference(args, s, blob)
+    else:
+        run_ours(args, s, blob)
+
+
+if __name__ == "__main__":
+    main()
