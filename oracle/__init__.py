@@ -213,6 +213,10 @@ def set_threads(n: int) -> int:
     return int(lib().dfo_get_threads())
 
 
+def get_threads() -> int:
+    return int(lib().dfo_get_threads())
+
+
 # ------------------------------------ whole-model wrapper ------------------------------------
 class OracleModel:
     _TAP_DTYPES = {0: np.int8, 1: np.float32, 2: np.int32, 3: np.int32, 4: np.float32, 5: np.float32,

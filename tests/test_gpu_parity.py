@@ -150,7 +150,8 @@ def test_cfg2_1p3b_full_run_sampled(env):
             if check and t in samples:
                 compare_step(gpu, orc, 0, st, t, "cfg2-sampled")
             if t >= 128:
-                toks.append(gpu.next_tokens()[:1].clone())
+                with torch.cuda.stream(gpu.stream):          # the library's stream orders this copy after the step
+                    toks.append(gpu.next_tokens()[:1].clone())
         gpu.sync()
         return torch.cat(toks).cpu().numpy(), gpu.logits()[0].cpu().numpy().copy(), st
 
