@@ -89,6 +89,7 @@ def kernel_class_bytes(s, batch: int) -> dict:
         "epi_out": 2 * dm + dm * r + 4 * dm + B * (4 * dm + 8 * dm),
         "lmhead": s.vocab * dm + 4 * s.vocab + B * (dm + 4 * s.vocab),
         "argmax": B * 4 * s.vocab,
+        "mega": algorithmic_bytes(s, B)["total"],      # the whole step is one kernel
     }
 
 
@@ -307,7 +308,7 @@ def run_ours(args, s, blob):
     kb = kernel_class_bytes(s, B)
     L = s.n_layers
     counts = {"embed": 1, "normquant": 2 * L + 1, "proj_in": L, "ssm": L, "proj_out": L, "epi_out": L,
-              "lmhead": 1, "argmax": 1}
+              "lmhead": 1, "argmax": 1, "mega": 1}
     # dominant kernel class = the one with the largest share of the step's device time
     dom = max(kt, key=lambda k: kt[k])
     per_launch_us = kt[dom] / max(1, counts.get(dom, 1))

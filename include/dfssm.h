@@ -60,6 +60,7 @@ enum {
 /* dfssm_config.flags */
 #define DFSSM_FLAG_TAPS      1u  /* allocate per-layer debug taps and record them every step (slower)   */
 #define DFSSM_FLAG_NO_GRAPH  2u  /* launch the step's kernels one by one instead of one CUDA-graph launch */
+#define DFSSM_FLAG_NO_MEGA   4u  /* never use the single persistent kernel ("mega" path) for batch-1 steps    */
 
 /* Shape of the model (the paper's Mamba-2-shaped student, Table 1) + capacity.
  * nheads = d_inner/headdim ; d_in_proj = 2*d_inner + 2*ngroups*d_state + nheads ;
@@ -118,8 +119,11 @@ DFSSM_API int dfssm_reset_state(dfssm_ctx* ctx, int seq_index);
 
 /* One decode step for sequences 0..batch-1: tokens_dev[s] is the input token of sequence s
  * (device int32[batch]; it may be the pointer returned by dfssm_next_tokens -- greedy decode
- * without leaving the device).  Async: exactly one launch (a CUDA graph) unless
- * DFSSM_FLAG_NO_GRAPH or DFSSM_FLAG_TAPS is set.  Token ids outside [0, vocab) are clamped on the
+ * without leaving the device).  Async: exactly one launch -- for batch 1 one persistent cooperative
+ * kernel (the "mega" path: 148 co-resident CTAs, weights and state prefetched ahead of the layer
+ * dependencies), otherwise one CUDA graph of the kernel chain -- unless DFSSM_FLAG_NO_GRAPH or
+ * DFSSM_FLAG_TAPS asks for the chain's kernels one by one.  The two paths share the state layout
+ * and compute bit-identical results.  Token ids outside [0, vocab) are clamped on the
  * device and a sticky error is raised, reported as DFSSM_E_TOKEN by the next dfssm_sync. */
 DFSSM_API int dfssm_step(dfssm_ctx* ctx, const int32_t* tokens_dev, int batch);
 
@@ -163,6 +167,7 @@ DFSSM_API int dfssm_launches_per_step(dfssm_ctx* ctx, int batch);
 enum {
     DFSSM_KCLASS_EMBED = 0, DFSSM_KCLASS_NORMQUANT, DFSSM_KCLASS_PROJ_IN, DFSSM_KCLASS_SSM,
     DFSSM_KCLASS_PROJ_OUT, DFSSM_KCLASS_EPI_OUT, DFSSM_KCLASS_LMHEAD, DFSSM_KCLASS_ARGMAX,
+    DFSSM_KCLASS_MEGA,     /* the whole step as one persistent kernel (batch 1); the others are then 0 */
     DFSSM_KCLASS_COUNT
 };
 DFSSM_API int dfssm_time_kernels(dfssm_ctx* ctx, const int32_t* tokens_dev, int batch, int iters,

@@ -18,13 +18,14 @@ _HERE = Path(__file__).resolve().parent
 ABI_VERSION = 1
 FLAG_TAPS = 1
 FLAG_NO_GRAPH = 2
+FLAG_NO_MEGA = 4
 
 TAPS = dict(XQ_IN=0, S_IN=1, ACC_IN=2, T_IN=3, ZXBCDT=4, XBC_CONV=5, DT=6, Y=7, G=8, GQ=9,
             S_G=10, ACC_OUT=11, T_OUT=12, HIDDEN=13)
 _TAP_DTYPES = {0: np.int8, 1: np.float32, 2: np.int32, 3: np.int32, 4: np.float32, 5: np.float32,
                6: np.float32, 7: np.float32, 8: np.float32, 9: np.int8, 10: np.float32, 11: np.int32,
                12: np.int32, 13: np.float32}
-KCLASSES = ("embed", "normquant", "proj_in", "ssm", "proj_out", "epi_out", "lmhead", "argmax")
+KCLASSES = ("embed", "normquant", "proj_in", "ssm", "proj_out", "epi_out", "lmhead", "argmax", "mega")
 
 # every symbol include/dfssm.h declares (tests check the .so exports exactly these)
 EXPORTED_SYMBOLS = (

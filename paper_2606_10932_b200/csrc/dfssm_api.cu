@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "dfssm_kernels.cuh"
+#include "dfssm_mega_host.cuh"
 
 using namespace dfssm;
 
@@ -23,6 +24,8 @@ inline size_t up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Carve {                 // byte offsets inside the arena
     size_t blob, ssm, conv, pos, u, xq, xqp, sx, qsum, acc, t, g, logits, next, tok, err, taps, total;
+    size_t m_chunks, m_Ain, m_Aout, m_x, m_am;      // mega path regions (valid if mega_fit)
+    bool mega_fit;
     size_t ssm_elems, ldq, ld_acc;
     uint32_t tap_stride;
     TapLayout tl;
@@ -44,6 +47,9 @@ struct dfssm_ctx {
     const int8_t* emb; const float* emb_s; const float* normf_w;
     std::vector<GraphEntry> graphs;
     int last_batch;
+    mega::Params mp;           // layout + pointers of the mega path (batch 1)
+    bool mega_ok;              // the device can co-schedule the mega grid and the shape fits
+    uint64_t epoch;            // steps taken by the mega path: makes every exchange flag unique
     int32_t* pinned_tok;       // page-locked staging for dfssm_step_host
     int* pinned_err;
     char err[512];
@@ -153,6 +159,16 @@ Carve carve(const dfssm_config& c)
     v.tl.off[DFSSM_TAP_COUNT] = (uint32_t)to;
     v.tap_stride = (uint32_t)to;
     v.taps = (c.flags & DFSSM_FLAG_TAPS) ? put(nl * B * to) : 0;
+    mega::Params mp;
+    v.mega_fit = !(c.flags & DFSSM_FLAG_NO_MEGA) && mega::plan(d, mega::GRID, mp);
+    if (v.mega_fit) {
+        const mega::Regions rg = mega::regions(mp);
+        v.m_chunks = put(rg.chunks);
+        v.m_Ain = put(rg.A_in);
+        v.m_Aout = put(rg.A_out);
+        v.m_x = put(rg.xbuf);
+        v.m_am = put(rg.am);
+    }
     v.total = up(o, ARENA_ALIGN);
     return v;
 }
@@ -349,6 +365,106 @@ int get_graph(dfssm_ctx* c, int batch, cudaGraphExec_t* out)
 
 }  // namespace
 
+
+// =================================================================================================
+// mega path: one persistent cooperative kernel per batch-1 step
+// =================================================================================================
+namespace {
+
+bool use_mega(const dfssm_ctx* c, int batch) { return batch == 1 && c->mega_ok; }
+
+int mega_setup(dfssm_ctx* ctx)                      // at create: can this device run the mega grid?
+{
+    ctx->mega_ok = false;
+    if (!ctx->cv.mega_fit) return DFSSM_OK;
+    mega::plan(ctx->dm, mega::GRID, ctx->mp);
+    int dev = 0, sms = 0, coop = 0, per_sm = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+    if (!coop || sms < mega::GRID) return DFSSM_OK;
+    CK(cudaFuncSetAttribute(mega::k_mega, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->mp.smem_bytes));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mega::k_mega, mega::THREADS, ctx->mp.smem_bytes));
+    if (per_sm < 1) return DFSSM_OK;
+    ctx->mega_ok = true;
+    return DFSSM_OK;
+}
+
+// at load: repack the canonical blob into per-(layer, CTA) chunks and plane-ordered LoRA-down rows
+int mega_load(dfssm_ctx* ctx, const std::vector<mega::HostLayer>& HL, const float* normf_w)
+{
+    if (!ctx->cv.mega_fit) return DFSSM_OK;
+    mega::Params& P = ctx->mp;
+    const Carve& v = ctx->cv;
+    const Dims& d = ctx->dm;
+    {
+        std::vector<uint8_t> buf((size_t)P.G * P.chunk_bytes);
+        for (int l = 0; l < d.n_layers; ++l) {
+            const float* nn = l + 1 < d.n_layers ? HL[l + 1].norm_w : normf_w;
+            for (int c = 0; c < P.G; ++c) mega::pack_chunk(P, HL[l], nn, c, buf.data() + (size_t)c * P.chunk_bytes);
+            CK(cudaMemcpyAsync(ctx->arena + v.m_chunks + (size_t)l * buf.size(), buf.data(), buf.size(), cudaMemcpyHostToDevice, ctx->stream));
+            CK(cudaStreamSynchronize(ctx->stream));
+        }
+    }
+    {
+        std::vector<int8_t> a((size_t)d.r * d.d_model), b((size_t)d.r * d.d_inner);
+        for (int l = 0; l < d.n_layers; ++l) {
+            mega::permute_A(HL[l].in_A, d.r, d.d_model, a.data());
+            mega::permute_A(HL[l].out_A, d.r, d.d_inner, b.data());
+            CK(cudaMemcpyAsync(ctx->arena + v.m_Ain + (size_t)l * a.size(), a.data(), a.size(), cudaMemcpyHostToDevice, ctx->stream));
+            CK(cudaMemcpyAsync(ctx->arena + v.m_Aout + (size_t)l * b.size(), b.data(), b.size(), cudaMemcpyHostToDevice, ctx->stream));
+            CK(cudaStreamSynchronize(ctx->stream));
+        }
+    }
+    // pointers
+    const size_t B = ctx->cfg.max_batch;
+    P.chunks = ctx->arena + v.m_chunks;
+    P.A_in = (const int8_t*)(ctx->arena + v.m_Ain);
+    P.A_out = (const int8_t*)(ctx->arena + v.m_Aout);
+    P.ssm = at<float>(ctx, v.ssm);
+    P.conv = at<float>(ctx, v.conv);
+    P.ssm_lstride = B * v.ssm_elems;
+    P.conv_lstride = B * (size_t)d.conv_dim * 4;
+    P.emb = ctx->emb; P.emb_s = ctx->emb_s;
+    P.first_norm_w = d.n_layers > 0 ? ctx->layers[0].norm_w : ctx->normf_w;
+    P.tokens = at<int32_t>(ctx, v.tok);
+    P.next = at<int32_t>(ctx, v.next);
+    P.tok_out = at<int32_t>(ctx, v.tok);
+    P.pos = at<int32_t>(ctx, v.pos);
+    P.logits = at<float>(ctx, v.logits);
+    P.u_out = at<float>(ctx, v.u);
+    uint64_t* xb = at<uint64_t>(ctx, v.m_x);
+    P.x_stat1 = xb; xb += 3 * P.G;
+    P.x_stat3 = xb; xb += 3 * P.G;
+    P.x_code1 = xb; xb += (size_t)P.G * P.wpc1;
+    P.x_code3 = xb; xb += (size_t)P.G * P.wpc3;
+    P.x_t = xb; xb += 64;
+    P.x_t4 = xb; xb += 64;
+    P.x_bc = xb;
+    P.am_val = at<float>(ctx, v.m_am);
+    P.am_idx = (int*)(P.am_val + P.G);
+    P.am_count = (unsigned*)(P.am_idx + P.G);
+    P.err = at<int>(ctx, v.err);
+    const bool taps_on = (ctx->cfg.flags & DFSSM_FLAG_TAPS) != 0;
+    P.taps = taps_on ? at<uint8_t>(ctx, v.taps) : nullptr;
+    P.tap_lstride = B * (size_t)v.tap_stride;
+    P.tl = v.tl;
+    return DFSSM_OK;
+}
+
+int mega_launch(dfssm_ctx* ctx)
+{
+    mega::Params P = ctx->mp;
+    ctx->epoch += 1;
+    P.base32 = (uint32_t)(ctx->epoch * (uint64_t)(8 * (P.L + 1)));
+    P.e255 = (uint32_t)(ctx->epoch % 255u);
+    void* args[] = { &P };
+    CK(cudaLaunchCooperativeKernel((const void*)mega::k_mega, dim3(P.G), dim3(mega::THREADS), args, P.smem_bytes, ctx->stream));
+    return DFSSM_OK;
+}
+
+}  // namespace
+
 // =================================================================================================
 // exported C ABI
 // =================================================================================================
@@ -381,6 +497,8 @@ int dfssm_create(const dfssm_config* cfg, void* dev_arena, size_t arena_bytes, v
     ctx->pinned_tok = nullptr;
     ctx->pinned_err = nullptr;
     ctx->err[0] = 0;
+    ctx->mega_ok = false;
+    ctx->epoch = 0;
     *out = ctx;                       // handed out even on failure below so last_error can be read
     if (arena_bytes < ctx->cv.total)
         return fail(ctx, DFSSM_E_SIZE, "arena too small: %zu < %zu", arena_bytes, ctx->cv.total);
@@ -388,6 +506,10 @@ int dfssm_create(const dfssm_config* cfg, void* dev_arena, size_t arena_bytes, v
     CK(cudaMallocHost((void**)&ctx->pinned_err, sizeof(int)));
     CK(cudaFuncSetAttribute(k_proj, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)proj_smem(8192)));
     CK(cudaFuncSetAttribute(k_lmhead, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lm_smem(8192)));
+    {
+        const int rc = mega_setup(ctx);
+        if (rc != DFSSM_OK) return rc;
+    }
     // zero everything behind the weights: state, ring positions, activations, error flag
     CK(cudaMemsetAsync(ctx->arena + ctx->cv.ssm, 0, ctx->cv.total - ctx->cv.ssm, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
@@ -417,6 +539,7 @@ int dfssm_load_weights(dfssm_ctx* ctx, const void* host_blob, size_t nbytes)
     BlobWalk w;
     const size_t dm = d.d_model, di = d.d_inner, dip = d.d_in_proj, r = d.r, cd = d.conv_dim, nh = d.nheads;
     ctx->layers.assign((size_t)d.n_layers, LayerW());
+    std::vector<mega::HostLayer> HL((size_t)d.n_layers);
     for (int l = 0; l < d.n_layers; ++l) {
         LayerW& L = ctx->layers[l];
         L.norm_w = (const float*)(db + w.take(4 * dm));
@@ -438,11 +561,28 @@ int dfssm_load_weights(dfssm_ctx* ctx, const void* host_blob, size_t nbytes)
         L.out_a_s = (const float*)(db + w.take(4 * r));
         L.out_B = (const int8_t*)(db + w.take(dm * r));
         L.out_b_s = (const float*)(db + w.take(4 * dm));
+        // the same tensors in the host blob (for the mega repack)
+        mega::HostLayer& H = HL[l];
+        auto hp = [&](const void* dev_ptr) { return hb + ((const uint8_t*)dev_ptr - db); };
+        H.norm_w = (const float*)hp(L.norm_w);
+        H.in_sign = (const uint32_t*)hp(L.in_sign); H.in_row_scale = (const uint16_t*)hp(L.in_row_scale);
+        H.in_A = (const int8_t*)hp(L.in_A); H.in_a_s = (const float*)hp(L.in_a_s);
+        H.in_B = (const int8_t*)hp(L.in_B); H.in_b_s = (const float*)hp(L.in_b_s);
+        H.conv_w = (const float*)hp(L.conv_w); H.conv_b = (const float*)hp(L.conv_b);
+        H.A_log = (const float*)hp(L.A_log); H.dt_bias = (const float*)hp(L.dt_bias); H.D = (const float*)hp(L.D);
+        H.gnorm_w = (const float*)hp(L.gnorm_w);
+        H.out_sign = (const uint32_t*)hp(L.out_sign); H.out_row_scale = (const uint16_t*)hp(L.out_row_scale);
+        H.out_A = (const int8_t*)hp(L.out_A); H.out_a_s = (const float*)hp(L.out_a_s);
+        H.out_B = (const int8_t*)hp(L.out_B); H.out_b_s = (const float*)hp(L.out_b_s);
     }
     ctx->emb = (const int8_t*)(db + w.take((size_t)d.vocab * dm));
     ctx->emb_s = (const float*)(db + w.take(4 * (size_t)d.vocab));
     ctx->normf_w = (const float*)(db + w.take(4 * dm));
     CK(cudaStreamSynchronize(ctx->stream));
+    {
+        const int rc = mega_load(ctx, HL, (const float*)(hb + ((const uint8_t*)ctx->normf_w - db)));
+        if (rc != DFSSM_OK) return rc;
+    }
     for (auto& e : ctx->graphs) cudaGraphExecDestroy(e.exec);
     ctx->graphs.clear();
     ctx->blob_bytes = nbytes;
@@ -483,6 +623,7 @@ int dfssm_step(dfssm_ctx* ctx, const int32_t* tokens_dev, int batch)
     if (!resident)
         CK(cudaMemcpyAsync(tok, tokens_dev, sizeof(int32_t) * (size_t)batch, cudaMemcpyDeviceToDevice, ctx->stream));
     ctx->last_batch = batch;
+    if (use_mega(ctx, batch)) return mega_launch(ctx);
     if (ctx->cfg.flags & (DFSSM_FLAG_NO_GRAPH | DFSSM_FLAG_TAPS)) return enqueue_step(ctx, batch, nullptr, nullptr);
     cudaGraphExec_t exec;
     const int rc = get_graph(ctx, batch, &exec);
@@ -599,7 +740,9 @@ int dfssm_sync(dfssm_ctx* ctx)
     CK(cudaMemcpyAsync(ctx->pinned_err, err_d, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     if (*ctx->pinned_err) {
+        const int bits = *ctx->pinned_err;
         CK(cudaMemsetAsync(err_d, 0, sizeof(int), ctx->stream));
+        if (bits & 2) return fail(ctx, DFSSM_E_CUDA, "the persistent step kernel timed out waiting for an exchange between CTAs");
         return fail(ctx, DFSSM_E_TOKEN, "a token id outside [0, vocab) was clamped");
     }
     return DFSSM_OK;
@@ -608,6 +751,7 @@ int dfssm_sync(dfssm_ctx* ctx)
 int dfssm_launches_per_step(dfssm_ctx* ctx, int batch)
 {
     if (!ctx || batch < 1) return DFSSM_E_ARG;
+    if (use_mega(ctx, batch)) return 1;
     const int per_layer = (ctx->cfg.flags & DFSSM_FLAG_TAPS) ? 10 : 6;
     return 1 + ctx->dm.n_layers * per_layer + 3;
 }
@@ -618,6 +762,25 @@ int dfssm_time_kernels(dfssm_ctx* ctx, const int32_t* tokens_dev, int batch, int
     if (!ctx->loaded) return fail(ctx, DFSSM_E_STATE, "dfssm_time_kernels before dfssm_load_weights");
     if (batch < 1 || batch > ctx->cfg.max_batch) return fail(ctx, DFSSM_E_ARG, "batch out of range");
     double sum[DFSSM_KCLASS_COUNT] = { 0 };
+    if (use_mega(ctx, batch)) {                  // one kernel: time it with events on the library's stream
+        cudaEvent_t a, b;
+        CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
+        CK(cudaMemcpyAsync(at<int32_t>(ctx, ctx->cv.tok), tokens_dev, sizeof(int32_t), cudaMemcpyDeviceToDevice, ctx->stream));
+        for (int k = 0; k < DFSSM_KCLASS_COUNT; ++k) out_us[k] = 0.0f;
+        for (int it = 0; it < iters; ++it) {
+            CK(cudaEventRecord(a, ctx->stream));
+            const int rc = mega_launch(ctx);
+            if (rc != DFSSM_OK) return rc;
+            CK(cudaEventRecord(b, ctx->stream));
+            CK(cudaEventSynchronize(b));
+            float ms = 0.f;
+            CK(cudaEventElapsedTime(&ms, a, b));
+            sum[DFSSM_KCLASS_MEGA] += 1e3 * ms;
+        }
+        cudaEventDestroy(a); cudaEventDestroy(b);
+        out_us[DFSSM_KCLASS_MEGA] = (float)(sum[DFSSM_KCLASS_MEGA] / iters);
+        return DFSSM_OK;
+    }
     for (int it = 0; it < iters; ++it) {
         KTimer tm;
         tm.on = true;

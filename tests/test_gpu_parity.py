@@ -316,3 +316,26 @@ def test_graph_equals_eager_chain(env):
         a.sync(); b.sync()
         assert n_diff_bits(a.logits().cpu().numpy(), b.logits().cpu().numpy()) == 0
         assert torch.equal(a.next_tokens(), b.next_tokens())
+
+
+def test_mega_path_is_the_batch1_path_and_equals_chain(env):
+    """Batch 1 runs as ONE persistent cooperative kernel; it must be bit-identical to the kernel chain
+    (DFSSM_FLAG_NO_MEGA), step after step, including the recurrent state, and they share the state layout."""
+    pk, torch = env["pk"], env["torch"]
+    s, blob = blob_for(0)
+    toks = ds.token_batch(s.vocab, 10, seed=12, batch=1)
+    a = pk.Model(pk.Config.from_shape(s, max_batch=1), blob)
+    b = pk.Model(pk.Config.from_shape(s, max_batch=1, flags=pk.binding.FLAG_NO_MEGA), blob)
+    assert a.launches_per_step(1) == 1, "the mega path is not active on this device"
+    assert b.launches_per_step(1) > 1
+    for t in range(10):
+        tk = dev_tokens(torch, toks[t])
+        a.step(tk); b.step(tk)
+        a.sync(); b.sync()
+        assert n_diff_bits(a.logits().cpu().numpy(), b.logits().cpu().numpy()) == 0, f"logits differ at step {t}"
+        assert n_diff_bits(a.hidden().cpu().numpy(), b.hidden().cpu().numpy()) == 0, f"hidden differs at step {t}"
+        assert torch.equal(a.next_tokens(), b.next_tokens())
+    for l in range(s.n_layers):
+        sa, ca = a.get_state(l, 0)
+        sb, cb = b.get_state(l, 0)
+        assert n_diff_bits(sa, sb) == 0 and n_diff_bits(ca, cb) == 0
