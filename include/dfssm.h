@@ -61,6 +61,7 @@ enum {
 #define DFSSM_FLAG_TAPS      1u  /* allocate per-layer debug taps and record them every step (slower)   */
 #define DFSSM_FLAG_NO_GRAPH  2u  /* launch the step's kernels one by one instead of one CUDA-graph launch */
 #define DFSSM_FLAG_NO_MEGA   4u  /* never use the single persistent kernel ("mega" path) for batch-1 steps    */
+#define DFSSM_FLAG_PROF      8u  /* persistent kernel: thread 0 of every CTA stamps its SM clock at every phase */
 
 /* Shape of the model (the paper's Mamba-2-shaped student, Table 1) + capacity.
  * nheads = d_inner/headdim ; d_in_proj = 2*d_inner + 2*ngroups*d_state + nheads ;
@@ -153,6 +154,13 @@ DFSSM_API int dfssm_get_state(dfssm_ctx* ctx, int layer, int seq, float* ssm_hos
                     float* conv_host, size_t conv_bytes);
 DFSSM_API int dfssm_set_state(dfssm_ctx* ctx, int layer, int seq, const float* ssm_host, size_t ssm_bytes,
                     const float* conv_host, size_t conv_bytes);
+
+/* In-kernel phase profile of the LAST persistent-kernel step (needs DFSSM_FLAG_PROF; a tracing aid, not
+ * part of the method).  dims[3] receives {CTAs, layers + 1, stamps per (CTA, layer)}; if stamps_host is
+ * non-null it must hold exactly CTAs*(layers+1)*stamps uint64 (nbytes), filled with the SM-clock value
+ * (clock64) thread 0 of each CTA read at each phase boundary of each layer; stamp 15 is %globaltimer (ns) at
+ * the start of the layer; row `layers` is the LM head (stamps 0, 1).  Synchronises the stream. */
+DFSSM_API int dfssm_debug_profile(dfssm_ctx* ctx, uint64_t* stamps_host, size_t nbytes, int32_t* dims);
 
 /* Wait for the stream; returns DFSSM_E_TOKEN once if a bad token id was clamped since the last
  * call, DFSSM_E_CUDA on a device fault. */

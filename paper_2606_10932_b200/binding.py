@@ -19,6 +19,7 @@ ABI_VERSION = 1
 FLAG_TAPS = 1
 FLAG_NO_GRAPH = 2
 FLAG_NO_MEGA = 4
+FLAG_PROF = 8
 
 TAPS = dict(XQ_IN=0, S_IN=1, ACC_IN=2, T_IN=3, ZXBCDT=4, XBC_CONV=5, DT=6, Y=7, G=8, GQ=9,
             S_G=10, ACC_OUT=11, T_OUT=12, HIDDEN=13)
@@ -31,7 +32,7 @@ KCLASSES = ("embed", "normquant", "proj_in", "ssm", "proj_out", "epi_out", "lmhe
 EXPORTED_SYMBOLS = (
     "dfssm_arena_bytes", "dfssm_create", "dfssm_load_weights", "dfssm_reset_state", "dfssm_step",
     "dfssm_step_host", "dfssm_logits", "dfssm_next_tokens", "dfssm_hidden", "dfssm_debug_tensor",
-    "dfssm_get_state", "dfssm_set_state", "dfssm_sync", "dfssm_launches_per_step",
+    "dfssm_get_state", "dfssm_set_state", "dfssm_debug_profile", "dfssm_sync", "dfssm_launches_per_step",
     "dfssm_time_kernels", "dfssm_last_error", "dfssm_destroy",
 )
 
@@ -123,6 +124,7 @@ def lib() -> C.CDLL:
         "dfssm_debug_tensor": (C.c_int, [vp, C.c_int, C.c_int, C.c_int, C.POINTER(vp), C.POINTER(C.c_size_t)]),
         "dfssm_get_state": (C.c_int, [vp, C.c_int, C.c_int, f32p, C.c_size_t, f32p, C.c_size_t]),
         "dfssm_set_state": (C.c_int, [vp, C.c_int, C.c_int, f32p, C.c_size_t, f32p, C.c_size_t]),
+        "dfssm_debug_profile": (C.c_int, [vp, C.POINTER(C.c_uint64), C.c_size_t, i32p]),
         "dfssm_sync": (C.c_int, [vp]),
         "dfssm_launches_per_step": (C.c_int, [vp, C.c_int]),
         "dfssm_time_kernels": (C.c_int, [vp, vp, C.c_int, C.c_int, f32p]),
@@ -267,6 +269,14 @@ class Model:
         conv = np.ascontiguousarray(conv, np.float32) if conv is not None else None
         self._check(self._L.dfssm_set_state(self._h, int(layer), int(seq), _f32p(ssm), ssm.nbytes if ssm is not None else 0,
                                             _f32p(conv), conv.nbytes if conv is not None else 0))
+
+    def debug_profile(self) -> np.ndarray:
+        """uint64 [CTAs][layers + 1][stamps] phase stamps of the last persistent-kernel step (FLAG_PROF)."""
+        dims = (C.c_int32 * 3)()
+        self._check(self._L.dfssm_debug_profile(self._h, None, 0, dims))
+        out = np.zeros(tuple(int(d) for d in dims), np.uint64)
+        self._check(self._L.dfssm_debug_profile(self._h, out.ctypes.data_as(C.POINTER(C.c_uint64)), out.nbytes, dims))
+        return out
 
     def sync(self):
         self._check(self._L.dfssm_sync(self._h))

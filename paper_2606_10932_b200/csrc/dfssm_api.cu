@@ -24,7 +24,7 @@ inline size_t up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Carve {                 // byte offsets inside the arena
     size_t blob, ssm, conv, pos, u, xq, xqp, sx, qsum, acc, t, g, logits, next, tok, err, taps, total;
-    size_t m_chunks, m_Ain, m_Aout, m_x, m_am;      // mega path regions (valid if mega_fit)
+    size_t m_chunks, m_Ain, m_Aout, m_x, m_am, m_prof;      // mega path regions (valid if mega_fit)
     bool mega_fit;
     size_t ssm_elems, ldq, ld_acc;
     uint32_t tap_stride;
@@ -168,6 +168,7 @@ Carve carve(const dfssm_config& c)
         v.m_Aout = put(rg.A_out);
         v.m_x = put(rg.xbuf);
         v.m_am = put(rg.am);
+        v.m_prof = (c.flags & DFSSM_FLAG_PROF) ? put((size_t)mp.G * (mp.L + 1) * mega::PROF_NPH * 8) : 0;
     }
     v.total = up(o, ARENA_ALIGN);
     return v;
@@ -449,6 +450,7 @@ int mega_load(dfssm_ctx* ctx, const std::vector<mega::HostLayer>& HL, const floa
     P.taps = taps_on ? at<uint8_t>(ctx, v.taps) : nullptr;
     P.tap_lstride = B * (size_t)v.tap_stride;
     P.tl = v.tl;
+    P.prof = (ctx->cfg.flags & DFSSM_FLAG_PROF) ? at<unsigned long long>(ctx, v.m_prof) : nullptr;
     return DFSSM_OK;
 }
 
@@ -731,6 +733,20 @@ int dfssm_get_state(dfssm_ctx* ctx, int layer, int seq, float* ssm_host, size_t 
 int dfssm_set_state(dfssm_ctx* ctx, int layer, int seq, const float* ssm_host, size_t ssm_bytes, const float* conv_host, size_t conv_bytes)
 {
     return state_copy(ctx, layer, seq, const_cast<float*>(ssm_host), ssm_bytes, const_cast<float*>(conv_host), conv_bytes, false);
+}
+
+int dfssm_debug_profile(dfssm_ctx* ctx, uint64_t* stamps_host, size_t nbytes, int32_t* dims)
+{
+    if (!ctx || !dims) return DFSSM_E_ARG;
+    if (!(ctx->cfg.flags & DFSSM_FLAG_PROF) || !ctx->mega_ok || !ctx->loaded)
+        return fail(ctx, DFSSM_E_STATE, "no profile: context created without DFSSM_FLAG_PROF, or the persistent kernel is not in use");
+    dims[0] = ctx->mp.G; dims[1] = ctx->mp.L + 1; dims[2] = mega::PROF_NPH;
+    const size_t need = (size_t)dims[0] * dims[1] * dims[2] * 8;
+    if (!stamps_host) return DFSSM_OK;
+    if (nbytes != need) return fail(ctx, DFSSM_E_SIZE, "profile is %zu bytes", need);
+    CK(cudaStreamSynchronize(ctx->stream));
+    CK(cudaMemcpy(stamps_host, ctx->arena + ctx->cv.m_prof, need, cudaMemcpyDeviceToHost));
+    return DFSSM_OK;
 }
 
 int dfssm_sync(dfssm_ctx* ctx)

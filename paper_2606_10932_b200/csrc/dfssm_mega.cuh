@@ -35,6 +35,7 @@ constexpr int NWARPS = THREADS / 32;
 constexpr int MAX_STAGES = 8;
 constexpr uint32_t SPIN_LIMIT = 1u << 21;     // ~0.5 s of polling, then the step aborts with an error flag
 constexpr int CODES_PER_WORD = 7;
+constexpr int PROF_NPH = 16;                  // phase stamps per (CTA, layer) of the in-kernel profiler
 
 struct Params {
     // ---- shape ----
@@ -68,6 +69,7 @@ struct Params {
     int* err;
     uint32_t base32, e255;
     uint8_t* taps; size_t tap_lstride; TapLayout tl;
+    unsigned long long* prof;    // [G][L+1][PROF_NPH] SM-clock stamps of thread 0 (DFSSM_FLAG_PROF), else null
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -141,6 +143,18 @@ struct Ctx {
     int tid, lane, wid, c;
     volatile int* dead;          // shared flag: a poll timed out -> stop spinning everywhere
 };
+
+__device__ __forceinline__ unsigned long long globaltimer_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
+// in-kernel profiler: thread 0 of every CTA stamps its SM clock at phase k of layer l
+#define DFSSM_STAMP(l_, k_)                                                                            \
+    do {                                                                                               \
+        if (P.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + (l_)) * PROF_NPH + (k_)] = clock64();  \
+    } while (0)
 
 __device__ __forceinline__ void poll_fail(const Ctx& x)
 {
@@ -497,6 +511,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         uint8_t* stage = sm + P.s_ring + (size_t)(l % P.stages) * P.stage_bytes;
         uint8_t* tp = taps_on ? P.taps + (size_t)l * P.tap_lstride : nullptr;
         float* conv_l = P.conv + (size_t)l * P.conv_lstride;
+        DFSSM_STAMP(l, 0);
+        if (P.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + 15] = globaltimer_ns();
 
         if (tp && c == 0) {
             for (int k = tid; k < P.d_model; k += THREADS) ((int8_t*)(tp + P.tl.off[0]))[k] = (int8_t)xq[plane_pos(k, P.d_model)];
@@ -515,7 +531,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 }
             }
         }
+        DFSSM_STAMP(l, 1);
         wait_item(x, l);
+        DFSSM_STAMP(l, 2);
 
         // ---- S2: sign rows of this CTA (early rows first, then z, then x), 4 rows per warp pass ----
         {
@@ -537,6 +555,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 if ((lane & 7) == 0 && r < nrows) s_acc_in[slot[r]] = acc;
             }
         }
+        DFSSM_STAMP(l, 3);
         // ---- gather t_in, v_j = a_s[j] * float(t_j) ----
         {
             const float* a_s = (const float*)(stage + P.c_as_in);
@@ -544,6 +563,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         }
         __syncthreads();
 
+        DFSSM_STAMP(l, 4);
         // ---- S3 stage 2 + S4 conv + dt softplus: 4 lanes per row ----
         {
             const int n_rows = 2 * nch + nb;
@@ -610,10 +630,12 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 }
             }
         }
+        DFSSM_STAMP(l, 5);
         // ---- gather B' | C' | dt ----
         poll_words<32>(x, P.x_bc, P.n_bcdt, f32 + 1, [&](int e, uint64_t v) { s_bc[e] = __uint_as_float((uint32_t)v); });
         __syncthreads();
 
+        DFSSM_STAMP(l, 6);
         // ---- S5 state update + readout, S6 gate: 16 lanes per channel ----
         double ss_own = 0.0;
         float amax_own = 0.0f;
@@ -663,6 +685,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             fence_proxy_async();               // the updated state is about to be read by the async proxy
             block_sum_max(x, ss_own, amax_own);
         }
+        DFSSM_STAMP(l, 7);
         // ---- write the state slice back (async), while the exchanges go on ----
         if (tid == 0 && nch > 0) {
             bulk_s2g(P.ssm + (size_t)l * P.ssm_lstride + (size_t)ch0 * P.d_state, stage + P.st_ssm, (uint32_t)nch * P.d_state * 4);
@@ -676,12 +699,14 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         // ---- S6 norm + quantise of g: stats hop, codes hop ----
         float inv_g, s_g;
         exchange_stats(x, P.x_stat3, f32 + 2, ss_own, amax_own, P.d_inner, inv_g, s_g);
+        DFSSM_STAMP(l, 8);
         const int qsum_g = exchange_codes(x, P.x_code3, f8g, s_tq, nch, inv_g, chs, P.wpc3, P.d_inner, false);
         if (tp && c == 0) {
             for (int k = tid; k < P.d_inner; k += THREADS) ((int8_t*)(tp + P.tl.off[9]))[k] = (int8_t)xq[plane_pos(k, P.d_inner)];
             if (tid == 0) *(float*)(tp + P.tl.off[10]) = s_g;
         }
 
+        DFSSM_STAMP(l, 9);
         // ---- S7: t_out rows (last warp) and the out_proj sign rows of this CTA ----
         if (wid == NWARPS - 1) {
             for (int j = jt0; j < P.r; j += P.G) {
@@ -707,12 +732,14 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 if ((lane & 7) == 0 && r < nrows) s_acc_out[4 * q + r] = acc;
             }
         }
+        DFSSM_STAMP(l, 10);
         {
             const float* a_s = (const float*)(stage + P.c_as_out);
             poll_words<32>(x, P.x_t4, P.r, f32 + 3, [&](int j, uint64_t v) { s_vout[j] = fmul(a_s[j], (float)(int32_t)(uint32_t)v); });
         }
         __syncthreads();
 
+        DFSSM_STAMP(l, 11);
         // ---- S7 epilogue + residual; stats of the new u for the next norm ----
         double ss_u = 0.0;
         float amax_u = 0.0f;
@@ -743,6 +770,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             }
             block_sum_max(x, ss_u, amax_u);     // also: every thread is done with this stage's weights
         }
+        DFSSM_STAMP(l, 12);
         // ---- refill this ring stage with the item `stages` ahead ----
         if (tid == 0) {
             bulk_wait_read0();                  // the state write-back has finished reading the stage
@@ -753,11 +781,15 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         // ---- S1 of the next layer (or S8's norm): stats hop, codes hop ----
         float inv_u;
         exchange_stats(x, P.x_stat1, f32 + 4, ss_u, amax_u, P.d_model, inv_u, s_act);
+        DFSSM_STAMP(l, 13);
         qsum = exchange_codes(x, P.x_code1, f8, s_tq, nor, inv_u, ors, P.wpc1, P.d_model, l == P.L - 1);
+        DFSSM_STAMP(l, 14);
     }
 
     // =============================================== S8 LM head ===============================================
     for (int i = tid; i < nor; i += THREADS) P.u_out[or0 + i] = s_u[i];
+    DFSSM_STAMP(P.L, 0);
+    if (P.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + P.L) * PROF_NPH + 15] = globaltimer_ns();
     float best = -INFINITY;
     int besti = 0x7fffffff;
     for (int it = 0; it < n_lm_items; ++it) {
@@ -803,6 +835,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         __syncthreads();
         if (tid == 0 && item + P.stages < n_items) issue_item(x, item + P.stages, v0, v1);
     }
+    DFSSM_STAMP(P.L, 1);
     // ---- greedy token: CTA argmax -> global partials -> the last CTA to arrive finishes (lowest index on ties) ----
     {
 #pragma unroll
