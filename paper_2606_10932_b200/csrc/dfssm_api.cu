@@ -24,7 +24,7 @@ inline size_t up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Carve {                 // byte offsets inside the arena
     size_t blob, ssm, conv, pos, u, xq, xqp, sx, qsum, acc, t, g, logits, next, tok, err, taps, total;
-    size_t m_chunks, m_Ain, m_Aout, m_x, m_am, m_prof;      // mega path regions (valid if mega_fit)
+    size_t m_chunks, m_blocks, m_Ain, m_Aout, m_x, m_xbytes, m_am, m_prof;      // mega path regions (valid if mega_fit)
     bool mega_fit;
     size_t ssm_elems, ldq, ld_acc;
     uint32_t tap_stride;
@@ -164,9 +164,11 @@ Carve carve(const dfssm_config& c)
     if (v.mega_fit) {
         const mega::Regions rg = mega::regions(mp);
         v.m_chunks = put(rg.chunks);
+        v.m_blocks = put(rg.blocks);
         v.m_Ain = put(rg.A_in);
         v.m_Aout = put(rg.A_out);
         v.m_x = put(rg.xbuf);
+        v.m_xbytes = rg.xbuf;
         v.m_am = put(rg.am);
         v.m_prof = (c.flags & DFSSM_FLAG_PROF) ? put((size_t)mp.G * (mp.L + 1) * mega::PROF_NPH * 8) : 0;
     }
@@ -408,6 +410,16 @@ int mega_load(dfssm_ctx* ctx, const std::vector<mega::HostLayer>& HL, const floa
         }
     }
     {
+        std::vector<uint8_t> buf((size_t)P.blk_bytes);
+        for (int l = 0; l < d.n_layers; ++l) {
+            mega::pack_block(P, HL[l], buf.data());
+            CK(cudaMemcpyAsync(ctx->arena + v.m_blocks + (size_t)l * buf.size(), buf.data(), buf.size(), cudaMemcpyHostToDevice, ctx->stream));
+            CK(cudaStreamSynchronize(ctx->stream));
+        }
+        // every exchange word starts as "not written" (mega::SENT)
+        CK(cudaMemsetAsync(ctx->arena + v.m_x, 0xff, v.m_xbytes, ctx->stream));
+    }
+    {
         std::vector<int8_t> a((size_t)d.r * d.d_model), b((size_t)d.r * d.d_inner);
         for (int l = 0; l < d.n_layers; ++l) {
             mega::permute_A(HL[l].in_A, d.r, d.d_model, a.data());
@@ -434,14 +446,8 @@ int mega_load(dfssm_ctx* ctx, const std::vector<mega::HostLayer>& HL, const floa
     P.pos = at<int32_t>(ctx, v.pos);
     P.logits = at<float>(ctx, v.logits);
     P.u_out = at<float>(ctx, v.u);
-    uint64_t* xb = at<uint64_t>(ctx, v.m_x);
-    P.x_stat1 = xb; xb += 3 * P.G;
-    P.x_stat3 = xb; xb += 3 * P.G;
-    P.x_code1 = xb; xb += (size_t)P.G * P.wpc1;
-    P.x_code3 = xb; xb += (size_t)P.G * P.wpc3;
-    P.x_t = xb; xb += 64;
-    P.x_t4 = xb; xb += 64;
-    P.x_bc = xb;
+    P.xbuf = at<uint32_t>(ctx, v.m_x);
+    P.blocks = ctx->arena + v.m_blocks;
     P.am_val = at<float>(ctx, v.m_am);
     P.am_idx = (int*)(P.am_val + P.G);
     P.am_count = (unsigned*)(P.am_idx + P.G);
@@ -458,8 +464,7 @@ int mega_launch(dfssm_ctx* ctx)
 {
     mega::Params P = ctx->mp;
     ctx->epoch += 1;
-    P.base32 = (uint32_t)(ctx->epoch * (uint64_t)(8 * (P.L + 1)));
-    P.e255 = (uint32_t)(ctx->epoch % 255u);
+    P.rec0 = (uint32_t)(((ctx->epoch - 1) * (uint64_t)P.L) & 3u);      // global layer counter mod 4
     void* args[] = { &P };
     CK(cudaLaunchCooperativeKernel((const void*)mega::k_mega, dim3(P.G), dim3(mega::THREADS), args, P.smem_bytes, ctx->stream));
     return DFSSM_OK;

@@ -6,18 +6,31 @@
 //   * Ownership.  CTA c owns d_inner channels [chs[c], chs[c+1]) -- their z and x in_proj rows, their conv
 //     and SSM state, their gate -- and out_proj rows [ors[c], ors[c+1]) together with that slice of the
 //     residual stream u (kept in shared memory for the whole step).  The B|C|dt in_proj rows and the
-//     LoRA down-projection rows (t = A.xq) are dealt round-robin: row e belongs to CTA e % G.
+//     LoRA down-projection rows (t = A.xq) are "early tasks" dealt round-robin: task e belongs to CTA e % G.
 //   * Weights.  dfssm_load_weights repacks every layer into one contiguous chunk per (layer, CTA)
-//     (sign rows, LoRA-up rows, scales, conv taps, per-channel constants).  A chunk plus the CTA's slice
-//     of the SSM / conv state is one pipeline item, fetched by bulk async copies (cp.async.bulk ->
-//     mbarrier) into a ring of shared-memory stages several layers AHEAD of the dependency chain:
-//     addresses never depend on activations, so HBM stays busy while CTAs wait on each other.
-//     The LM head streams the int8 embedding through the same ring.
-//   * Exchange.  All-gathers between CTAs use flag-in-data 64-bit words in global memory (L2):
-//     {payload32, flag32} or {7 int8 codes, flag8}, written with st.relaxed.gpu.b64 and polled with
-//     ld.relaxed.gpu.b64 -- a 64-bit scalar access is single-copy atomic, so a matching flag proves the
-//     payload; no fence, no separate barrier, one L2 round trip per hop.  Flags are unique per use.
-//     Per layer: stats(u) -> codes(u) -> t_in -> B'|C'|dt -> stats(g) -> codes(g) -> t_out.
+//     (sign rows, LoRA-up rows, scales, conv taps, per-channel constants) plus one block per layer that
+//     every CTA reads (the LoRA-up rows / scales / conv taps of the B|C|dt rows).  Chunk + block + the CTA's
+//     slice of the SSM / conv state form one pipeline item, fetched by bulk async copies
+//     (cp.async.bulk -> mbarrier) into a ring of shared-memory stages several layers AHEAD of the
+//     dependency chain: addresses never depend on activations, so HBM stays busy while CTAs wait on
+//     each other.  The LM head streams the int8 embedding through the same ring.
+//   * Exchange.  Measured on B200: one store -> poll hop between CTAs through L2 costs >= ~0.9 us, so the
+//     layer is built around FOUR all-gathers, two of them hidden behind sign-row work:
+//       U : t_k = u_k * w_k (fp32) of the owned out rows + the CTA's partial sum of u^2 (fp64)
+//           -> every CTA derives rstd / amax / the int8 codes of the WHOLE vector itself (S1)
+//       A : raw int32 accumulators of the B|C|dt rows + t_in        (hidden behind the z|x sign rows)
+//           -> every CTA finishes the B|C|dt epilogue, conv and softplus redundantly (S3, S4)
+//       G : t_k = g_k * w_k (fp32) of the owned channels + partial sum of g^2  -> S6 everywhere
+//       T : partial LoRA-down sums of out_proj                     (hidden behind the out_proj sign rows)
+//     Buffers are self-validating ("Lamport" style): every 32-bit word is either the sentinel 0xffffffff
+//     or payload (fp32 values are never that NaN; int32 values are stored with the sign bit flipped;
+//     fp64 partials are 8-byte stores validated by their high word), so a hop is one store and one
+//     successful poll, with no flag, fence or barrier.  Measured: when all 148 CTAs poll the SAME lines the
+//     L2 serialises them (3-6 us per hop), so every payload is PUSHED into M mailboxes (G/M CTAs poll each);
+//     the U / G payload of a CTA is one 64 / 128-byte slot written with 16-byte stores.  Records rotate
+//     over 4 (global layer counter mod 4): at layer l a CTA resets its own slots of the record that layer
+//     l+2 will use (last used by layer l-2, which every CTA has finished reading: it has since published
+//     for layer l-1), so the buffers stay L2-resident and a reset is at least two hops old when reused.
 //   * Arithmetic: identical to the chain path (dfssm_math.cuh; contract of DESIGN.md section 5).
 #pragma once
 #include <cooperative_groups.h>
@@ -33,8 +46,9 @@ namespace mega {
 constexpr int THREADS = 512;
 constexpr int NWARPS = THREADS / 32;
 constexpr int MAX_STAGES = 8;
-constexpr uint32_t SPIN_LIMIT = 1u << 21;     // ~0.5 s of polling, then the step aborts with an error flag
-constexpr int CODES_PER_WORD = 7;
+constexpr uint32_t SPIN_LIMIT = 1u << 20;     // ~0.3 s of polling, then the step aborts with an error flag
+constexpr uint32_t SENT = 0xffffffffu;        // "not written yet"
+constexpr uint32_t IBIAS = 0x80000000u;       // int32 payloads are stored xor IBIAS (|value| < 2^30)
 constexpr int PROF_NPH = 16;                  // phase stamps per (CTA, layer) of the in-kernel profiler
 
 struct Params {
@@ -44,18 +58,26 @@ struct Params {
     int G;                       // grid size (CTAs), all co-resident
     int nch_max, nor_max, nb_max, n_slots, r_pad;
     int Win, Wout;               // sign words per row of in_proj / out_proj
-    int wpc1, wpc3;              // code words per CTA in the u / g code exchanges
+    int n_early;                 // early tasks: n_bcdt sign rows + r LoRA-down rows
+    int tsplit, n_ttask;         // out_proj LoRA-down rows are split into tsplit partial tasks each
     // ---- chunk layout (byte offsets inside one (layer, CTA) chunk) ----
     uint32_t c_in_bits, c_out_bits, c_in_B, c_out_B, c_in_scale, c_in_bs, c_out_scale, c_out_bs, c_conv_w, c_conv_b,
-        c_e_conv_w, c_e_conv_b, c_e_dtb, c_alog, c_D, c_gnorm, c_nnorm, c_as_in, c_as_out, chunk_bytes;
+        c_alog, c_D, c_gnorm, c_nnorm, chunk_bytes;
+    // ---- per-layer block read by every CTA (byte offsets) ----
+    uint32_t b_eB, b_escale, b_ebs, b_econv_w, b_econv_b, b_dtb, b_as_in, b_as_out, blk_bytes;
     // ---- pipeline stage ----
-    uint32_t st_ssm, st_conv, stage_bytes;
+    uint32_t st_blk, st_ssm, st_conv, st_econv, stage_bytes;
     int stages, lm_rows_item;
+    // ---- exchange: M mailboxes x 4 rotating records; 32-bit word offsets inside one (record, mailbox) ----
+    int M, gsz;                  // mailboxes, CTAs polling each (G = M * gsz); CTA c polls mailbox c / gsz
+    int u_slot, u_dpos, g_slot, g_dpos;      // words per CTA slot of U / G, position of the fp64 partial inside it
+    uint32_t x_U, x_A, x_G, x_T, x_words;
     // ---- shared memory carve ----
-    uint32_t s_ring, s_mbar, s_xq, s_bc, s_u, s_z, s_x, s_tq, s_vin, s_vout, s_acc_in, s_acc_out, s_chs, s_ors,
-        s_stats, s_red, smem_bytes;
+    uint32_t s_ring, s_mbar, s_xq, s_bc, s_u, s_z, s_x, s_dt, s_tq, s_v, s_eacc, s_acc_in, s_acc_out, s_chs, s_ors,
+        s_part, s_red, s_slot, smem_bytes;
     // ---- device pointers ----
     const uint8_t* chunks;       // [L][G][chunk_bytes]
+    const uint8_t* blocks;       // [L][blk_bytes]
     const int8_t* A_in;          // [L][r][d_model]  plane-permuted
     const int8_t* A_out;         // [L][r][d_inner]  plane-permuted
     float* ssm;                  // sequence 0 of layer 0; layer stride ssm_lstride floats
@@ -64,10 +86,10 @@ struct Params {
     const int8_t* emb; const float* emb_s; const float* first_norm_w;
     const int32_t* tokens; int32_t* next; int32_t* tok_out; int32_t* pos;
     float* logits; float* u_out;
-    uint64_t *x_stat1, *x_code1, *x_t, *x_bc, *x_stat3, *x_code3, *x_t4;
+    uint32_t* xbuf;              // [4 records][M][x_words]
     float* am_val; int* am_idx; unsigned* am_count;
     int* err;
-    uint32_t base32, e255;
+    uint32_t rec0;               // record of layer 0 of this step (global layer counter mod 4)
     uint8_t* taps; size_t tap_lstride; TapLayout tl;
     unsigned long long* prof;    // [G][L+1][PROF_NPH] SM-clock stamps of thread 0 (DFSSM_FLAG_PROF), else null
 };
@@ -110,17 +132,27 @@ __device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
-__device__ __forceinline__ void ll_store(uint64_t* p, uint64_t v)
+// exchange words: relaxed gpu-scope accesses (served by L2; a 32-bit / 64-bit scalar access is single-copy atomic)
+__device__ __forceinline__ void x_st32(uint32_t* p, uint32_t v)
+{
+    asm volatile("st.relaxed.gpu.global.b32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void x_st64(uint32_t* p, uint64_t v)
 {
     asm volatile("st.relaxed.gpu.global.b64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
-__device__ __forceinline__ uint64_t ll_load(const uint64_t* p)
+// 16 bytes as TWO 64-bit elements, each single-copy atomic (a float pair, or one fp64)
+__device__ __forceinline__ uint4 x_ld128(const uint32_t* p)
 {
-    uint64_t v;
-    asm volatile("ld.relaxed.gpu.global.b64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
-    return v;
+    uint64_t a, b;
+    asm volatile("ld.relaxed.gpu.global.v2.b64 {%0,%1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
+    return make_uint4((uint32_t)a, (uint32_t)(a >> 32), (uint32_t)b, (uint32_t)(b >> 32));
 }
-__device__ __forceinline__ uint64_t ll_pack32(uint32_t payload, uint32_t flag) { return ((uint64_t)flag << 32) | payload; }
+__device__ __forceinline__ void x_st128(uint32_t* p, uint4 v)
+{
+    const uint64_t a = ((uint64_t)v.y << 32) | v.x, b = ((uint64_t)v.w << 32) | v.z;
+    asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1,%2};" ::"l"(p), "l"(a), "l"(b) : "memory");
+}
 
 __device__ __forceinline__ int4 ldg_nc16(const void* p)
 {
@@ -162,53 +194,39 @@ __device__ __forceinline__ void poll_fail(const Ctx& x)
     atomicExch(x.P.err, 2);
 }
 
-// Poll n flag-in-data words; consume(idx, word) is called once per word by the thread that polled it.
-// Each thread keeps up to 4 loads in flight.  flag is compared with the top `fbits` bits (32 or 8).
-template <int FBITS, typename F>
-__device__ __forceinline__ void poll_words(const Ctx& x, const uint64_t* buf, int n, uint32_t flag, F consume)
+// ------------------------------------------------------------------------------------------------
+// exchange: gather a self-validating buffer
+// ------------------------------------------------------------------------------------------------
+// Thread t owns the 16-byte chunks t, t + THREADS, ... (at most NJ) of the nw 32-bit words at buf.  Words
+// behind nw count as valid.  If slot_w > 0 the buffer is a sequence of slots of slot_w words whose word dpos is
+// the low half of an fp64 (any bit pattern: exempt; its high half at dpos + 1 validates it).
+// Spins until every owned word has been written; the raw words come back in v[].
+template <int NJ>
+__device__ __forceinline__ void hop_gather(const Ctx& x, const uint32_t* buf, int nw, int slot_w, int dpos, uint4 (&v)[NJ])
 {
-    for (int base = x.tid; base < n; base += THREADS * 4) {
-        uint64_t v[4];
-        bool ok[4];
+    const int nchunk = (nw + 3) >> 2;
+    bool need[NJ];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) ok[j] = (base + j * THREADS) >= n;
-        uint32_t spins = 0;
-        for (;;) {
-            bool all = true;
+    for (int j = 0; j < NJ; ++j) need[j] = x.tid + j * THREADS < nchunk;
+    uint32_t spins = 0;
+    for (;;) {
 #pragma unroll
-            for (int j = 0; j < 4; ++j)
-                if (!ok[j]) v[j] = ll_load(buf + base + j * THREADS);
+        for (int j = 0; j < NJ; ++j)
+            if (need[j]) v[j] = x_ld128(buf + 4 * (x.tid + j * THREADS));
+        bool all = true;
 #pragma unroll
-            for (int j = 0; j < 4; ++j)
-                if (!ok[j]) {
-                    ok[j] = (uint32_t)(v[j] >> (64 - FBITS)) == flag;
-                    all = all && ok[j];
-                }
-            if (all) break;
-            if (++spins > SPIN_LIMIT || *x.dead) { poll_fail(x); break; }
-        }
-#pragma unroll
-        for (int j = 0; j < 4; ++j)
-            if (base + j * THREADS < n) consume(base + j * THREADS, v[j]);
+        for (int j = 0; j < NJ; ++j)
+            if (need[j]) {
+                const int base = 4 * (x.tid + j * THREADS);
+                const int ex = slot_w > 0 ? dpos - base % slot_w : -1;      // index of the exempt word inside this chunk
+                const bool ok = (v[j].x != SENT || ex == 0) && (base + 1 >= nw || v[j].y != SENT) &&
+                                (base + 2 >= nw || v[j].z != SENT || ex == 2) && (base + 3 >= nw || v[j].w != SENT);
+                need[j] = !ok;
+                all = all && ok;
+            }
+        if (all) break;
+        if (++spins > SPIN_LIMIT || *x.dead) { poll_fail(x); break; }
     }
-}
-
-// block-wide (sum of doubles, max of floats); result to every thread.  Two __syncthreads.
-__device__ __forceinline__ void block_sum_max(const Ctx& x, double& s, float& m)
-{
-    double* rd = (double*)(x.sm + x.P.s_red);             // [NWARPS]
-    float* rf = (float*)(rd + NWARPS);                    // [NWARPS]
-    s = warp_sum(s);
-    m = warp_max(m);
-    if (x.lane == 0) { rd[x.wid] = s; rf[x.wid] = m; }
-    __syncthreads();
-    double s2 = 0.0;
-    float m2 = 0.0f;
-#pragma unroll
-    for (int i = 0; i < NWARPS; ++i) { s2 += rd[i]; m2 = fmaxf(m2, rf[i]); }
-    __syncthreads();
-    s = s2;
-    m = m2;
 }
 
 // quantiser constants from (sum of squares, amax) of a vector of length d (R4, R13)
@@ -220,23 +238,125 @@ __device__ __forceinline__ void quant_consts(double ss, float amax, int d, float
     s = amax == 0.0f ? 0.0f : fdiv(fmul(amax, rstd), 127.0f);
 }
 
-// Sign dot products of up to 4 rows against the plane-ordered codes in shared memory (S2 / S7):
-// returns in lane 8*r the value sum_k sign_rk * q_k of row r.  rowp[r] points at the row's packed words.
-__device__ __forceinline__ int sign_dot4(const uint32_t* (&rowp)[4], int nrows, int W, const uint8_t* xq, int K,
-                                         int qsum, int lane)
+// scratch inside s_red: [0,16) floats warp maxima | [16,32) ints warp code sums | doubles [8,24) warp sums (byte 64..)
+__device__ __forceinline__ float* red_f(const Ctx& x) { return (float*)(x.sm + x.P.s_red); }
+__device__ __forceinline__ int* red_i(const Ctx& x) { return (int*)(x.sm + x.P.s_red) + NWARPS; }
+__device__ __forceinline__ double* red_d(const Ctx& x) { return (double*)(x.sm + x.P.s_red + 8 * NWARPS); }
+
+// S1 / S6 / S8 norm + quantise of a whole vector in every CTA.  `en(f)` calls f(k, bits) for every element this
+// thread holds: bits = fp32 t_k = value_k * w_k.  The caller has stored the partial sums of squares (one per
+// CTA, or per warp for the embedding) into part[0..G) (zeros where unused).  Every CTA derives the same
+// rstd / amax / codes.  Writes the codes to xq (plane order unless `canonical`), returns the sum of the codes
+// and the activation scale s.  Two __syncthreads.
+template <typename Enum>
+__device__ __forceinline__ int norm_quant(const Ctx& x, Enum en, int K, bool canonical, float& s_out, int8_t* tap_codes)
 {
-    int a[4][8];
+    const Params& P = x.P;
+    uint8_t* xq = x.sm + P.s_xq;
+    const double* part = (const double*)(x.sm + P.s_part);
+    float am = 0.0f;
+    en([&](int, uint32_t w) { am = fmaxf(am, fabsf(__uint_as_float(w))); });
+    am = warp_max(am);
+    if (x.lane == 0) red_f(x)[x.wid] = am;
+    __syncthreads();
+    // every warp derives the constants itself
+    float amax = x.lane < NWARPS ? red_f(x)[x.lane] : 0.0f;
+    amax = warp_max(amax);
+    double ss = 0.0;
+    for (int g = x.lane; g < P.G; g += 32) ss += part[g];
+    ss = warp_sum(ss);
+    float inv;
+    quant_consts(ss, amax, K, P.eps, inv, s_out);
+    int qs = 0;
+    en([&](int k, uint32_t w) {
+        const int q = quant_code(__uint_as_float(w), inv);          // inv == 0 -> code 0
+        xq[canonical ? k : plane_pos(k, K)] = (uint8_t)q;
+        if (tap_codes) tap_codes[k] = (int8_t)q;
+        qs += q;
+    });
+    qs = warp_sum_i(qs);
+    if (x.lane == 0) red_i(x)[x.wid] = qs;
+    __syncthreads();
+    const int tot = x.lane < NWARPS ? red_i(x)[x.lane] : 0;
+    return warp_sum_i(tot);
+}
+
+// the elements a thread holds after gathering a slot-structured mailbox part (U or G): chunk ci = tid + j*THREADS is
+// piece ci % pps of slot ci / pps; slot g carries elements starts[g] .. starts[g+1]-1 and its fp64 partial at dpos
+template <int NJ>
+struct SlotEnum {
+    const uint4 (&v)[NJ];
+    const int* starts;
+    int tid, nslots, pps;
+    template <typename F>
+    __device__ __forceinline__ void operator()(F f) const
+    {
 #pragma unroll
-    for (int r = 0; r < 4; ++r)
+        for (int j = 0; j < NJ; ++j) {
+            const int ci = tid + j * THREADS;
+            if (ci < nslots * pps) {
+                const int g = ci / pps, piece = ci - g * pps;
+                const int k0 = starts[g] + 4 * piece, n = starts[g + 1] - starts[g] - 4 * piece;
+                if (n > 0) f(k0, v[j].x);
+                if (n > 1) f(k0 + 1, v[j].y);
+                if (n > 2) f(k0 + 2, v[j].z);
+                if (n > 3) f(k0 + 3, v[j].w);
+            }
+        }
+    }
+};
+// store the fp64 partials found in the gathered chunks into part[slot]
+template <int NJ>
+__device__ __forceinline__ void slot_partials(const Ctx& x, const uint4 (&v)[NJ], int nslots, int slot_w, int dpos)
+{
+    double* part = (double*)(x.sm + x.P.s_part);
+    const int pps = slot_w >> 2;
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+        const int ci = x.tid + j * THREADS;
+        if (ci < nslots * pps) {
+            const int g = ci / pps, ex = dpos - 4 * (ci - g * pps);
+            if (ex == 0) part[g] = __hiloint2double((int)v[j].y, (int)v[j].x);
+            else if (ex == 2) part[g] = __hiloint2double((int)v[j].w, (int)v[j].z);
+        }
+    }
+}
+
+// block-wide sum of doubles held by some lanes (others pass 0); result valid in thread 0 only.  One __syncthreads.
+__device__ __forceinline__ double block_sum_t0(const Ctx& x, double s)
+{
+    s = warp_sum(s);
+    if (x.lane == 0) red_d(x)[x.wid] = s;
+    __syncthreads();
+    double t = 0.0;
+    if (x.tid == 0)
+#pragma unroll
+        for (int i = 0; i < NWARPS; ++i) t += red_d(x)[i];
+    return t;
+}
+
+// ------------------------------------------------------------------------------------------------
+// integer dot products
+// ------------------------------------------------------------------------------------------------
+// Sign dot products of up to NR rows against the plane-ordered codes in shared memory (S2 / S7) over the sign
+// words [w0, w1) of each row: returns, in every lane, 128 * sum_{bit=1} q_k of row r in p[r] AFTER the caller
+// reduces across lanes.  (dp4a of the mask 0x01010101 << i against plane i gives 2^i * partial sum.)
+template <int NR>
+__device__ __forceinline__ void sign_partial(const uint32_t* const (&rowp)[NR], int nrows, int w0, int w1, const uint8_t* xq, int K,
+                                             int lane, int (&p)[NR])
+{
+    int a[NR][8];
+#pragma unroll
+    for (int r = 0; r < NR; ++r)
 #pragma unroll
         for (int i = 0; i < 8; ++i) a[r][i] = 0;
     const uint8_t* xlo = xq;
     const uint8_t* xhi = xq + (K >> 1);
-    for (int w = lane; w < W; w += 32) {
+    for (int w = w0 + lane; w < w1; w += 32) {
         const int4 lo = *(const int4*)(xlo + 16 * w);
         const int4 hi = *(const int4*)(xhi + 16 * w);
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
+        for (int r = 0; r < NR; ++r) {
             if (r < nrows) {
                 const uint32_t b = rowp[r][w];
                 a[r][0] = dp4a_us(b & 0x01010101u, lo.x, a[r][0]);
@@ -250,15 +370,18 @@ __device__ __forceinline__ int sign_dot4(const uint32_t* (&rowp)[4], int nrows, 
             }
         }
     }
-    int p[4];
 #pragma unroll
-    for (int r = 0; r < 4; ++r)       // a[r][i] = 2^i * S_i  ->  128 * sum_i S_i
+    for (int r = 0; r < NR; ++r)       // a[r][i] = 2^i * S_i  ->  128 * sum_i S_i
         p[r] = (a[r][0] << 7) + (a[r][1] << 6) + (a[r][2] << 5) + (a[r][3] << 4) + (a[r][4] << 3) + (a[r][5] << 2) +
                (a[r][6] << 1) + a[r][7];
-    // transposing reduction: 4 values x 32 lanes -> lane 8r holds the total of row r
+}
+
+// transposing reduction of 4 per-lane values: lane 8r ends up with the warp total of p[r]
+__device__ __forceinline__ int reduce4(const int (&p)[4], int lane)
+{
     const bool up16 = (lane & 16) != 0, up8 = (lane & 8) != 0;
     int k0 = up16 ? p[2] : p[0], k1 = up16 ? p[3] : p[1];
-    int s0 = up16 ? p[0] : p[2], s1 = up16 ? p[1] : p[3];
+    const int s0 = up16 ? p[0] : p[2], s1 = up16 ? p[1] : p[3];
     k0 += __shfl_xor_sync(0xffffffffu, s0, 16);
     k1 += __shfl_xor_sync(0xffffffffu, s1, 16);
     int v = up8 ? k1 : k0;
@@ -267,24 +390,38 @@ __device__ __forceinline__ int sign_dot4(const uint32_t* (&rowp)[4], int nrows, 
     v += __shfl_xor_sync(0xffffffffu, v, 4);
     v += __shfl_xor_sync(0xffffffffu, v, 2);
     v += __shfl_xor_sync(0xffffffffu, v, 1);
-    return 2 * (v / 128) - qsum;      // exact: every term is a multiple of 128
+    return v;
+}
+// same for 2 values: lane 16r ends up with the warp total of p[r]
+__device__ __forceinline__ int reduce2(const int (&p)[2], int lane)
+{
+    const bool up16 = (lane & 16) != 0;
+    int v = up16 ? p[1] : p[0];
+    const int sv = up16 ? p[0] : p[1];
+    v += __shfl_xor_sync(0xffffffffu, sv, 16);
+    v += __shfl_xor_sync(0xffffffffu, v, 8);
+    v += __shfl_xor_sync(0xffffffffu, v, 4);
+    v += __shfl_xor_sync(0xffffffffu, v, 2);
+    v += __shfl_xor_sync(0xffffffffu, v, 1);
+    return v;
 }
 
-// int8 x int8 dot of a plane-permuted LoRA-down row (global memory) with the codes in shared memory.
-// pre[] holds the row's first 8*32 16-byte chunks, loaded earlier so their latency is off the critical path.
-constexpr int T_PRE = 8;
-__device__ __forceinline__ void trow_prefetch(const int8_t* row, int K, int lane, int4 (&pre)[T_PRE])
+// int8 x int8 dot of `nbytes` plane-permuted LoRA-down weights (global memory) with the codes at the same
+// positions in shared memory.  pre[] holds the first T_PRE*32 16-byte chunks, loaded a phase earlier so that
+// their latency is off the critical path.
+constexpr int T_PRE = 4;
+__device__ __forceinline__ void trow_prefetch(const int8_t* row, int nbytes, int lane, int4 (&pre)[T_PRE])
 {
-    const int nch = K >> 4;
+    const int nch = nbytes >> 4;
 #pragma unroll
     for (int i = 0; i < T_PRE; ++i) {
         const int ch = lane + 32 * i;
         if (ch < nch) pre[i] = ldg_nc16(row + 16 * ch);
     }
 }
-__device__ __forceinline__ int trow_dot(const int8_t* row, int K, const uint8_t* xq, int lane, const int4 (&pre)[T_PRE])
+__device__ __forceinline__ int trow_dot(const int8_t* row, int nbytes, const uint8_t* xq, int lane, const int4 (&pre)[T_PRE])
 {
-    const int nch = K >> 4;
+    const int nch = nbytes >> 4;
     int s = 0;
 #pragma unroll
     for (int i = 0; i < T_PRE; ++i) {
@@ -303,6 +440,9 @@ __device__ __forceinline__ int trow_dot(const int8_t* row, int K, const uint8_t*
     return warp_sum_i(s);
 }
 
+// ------------------------------------------------------------------------------------------------
+// weight / state pipeline
+// ------------------------------------------------------------------------------------------------
 // issue the bulk copies of pipeline item `item` into its ring stage (one thread)
 __device__ __forceinline__ void issue_item(const Ctx& x, int item, int v0, int v1)
 {
@@ -313,9 +453,11 @@ __device__ __forceinline__ void issue_item(const Ctx& x, int item, int v0, int v
     if (item < P.L) {
         const int* chs = (const int*)(x.sm + P.s_chs);
         const int ch0 = chs[x.c], nch = chs[x.c + 1] - ch0;
-        const uint32_t ssm_b = (uint32_t)nch * P.d_state * 4, conv_b = (uint32_t)nch * 16;
-        mbar_expect_tx(bar, P.chunk_bytes + ssm_b + conv_b);
+        const uint32_t ssm_b = (uint32_t)nch * P.d_state * 4, conv_b = (uint32_t)nch * 16, econv_b = (uint32_t)P.gs * 32;
+        mbar_expect_tx(bar, P.chunk_bytes + P.blk_bytes + ssm_b + conv_b + econv_b);
         bulk_g2s(stage, P.chunks + ((size_t)item * P.G + x.c) * P.chunk_bytes, P.chunk_bytes, bar);
+        bulk_g2s(stage + P.st_blk, P.blocks + (size_t)item * P.blk_bytes, P.blk_bytes, bar);
+        bulk_g2s(stage + P.st_econv, P.conv + (size_t)item * P.conv_lstride + (size_t)P.d_inner * 4, econv_b, bar);
         if (nch > 0) {
             bulk_g2s(stage + P.st_ssm, P.ssm + (size_t)item * P.ssm_lstride + (size_t)ch0 * P.d_state, ssm_b, bar);
             bulk_g2s(stage + P.st_conv, P.conv + (size_t)item * P.conv_lstride + (size_t)ch0 * 4, conv_b, bar);
@@ -340,78 +482,24 @@ __device__ __forceinline__ void wait_item(const Ctx& x, int item)
     }
 }
 
-// ---- hop (a): publish this CTA's (sum of squares, amax), gather all, derive the quantiser constants ----
-__device__ __forceinline__ void exchange_stats(const Ctx& x, uint64_t* buf, uint32_t flag, double ss_own, float amax_own,
-                                               int d, float& inv, float& s)
+// The stores of one CTA into the M mailboxes of a record.  publish and reset use the SAME thread -> address map, so
+// a reset and the later publish of a word are ordered by program order of one thread.
+//   slot (U / G): thread t < M * pps writes 16-byte piece t % pps of its slot in mailbox t / pps
+template <typename F>
+__device__ __forceinline__ void slot_store(const Ctx& x, uint32_t* rec, uint32_t part_off, int slot_w, F piece_value)
 {
     const Params& P = x.P;
-    if (x.tid == 0) {
-        const long long b = __double_as_longlong(ss_own);
-        ll_store(buf + 3 * x.c + 0, ll_pack32((uint32_t)((unsigned long long)b >> 32), flag));
-        ll_store(buf + 3 * x.c + 1, ll_pack32((uint32_t)b, flag));
-        ll_store(buf + 3 * x.c + 2, ll_pack32(__float_as_uint(amax_own), flag));
+    const int pps = slot_w >> 2;
+    for (int t = x.tid; t < P.M * pps; t += THREADS) {
+        const int m = t / pps, piece = t - m * pps;
+        x_st128(rec + (size_t)m * P.x_words + part_off + (size_t)x.c * slot_w + 4 * piece, piece_value(piece));
     }
-    uint32_t* st = (uint32_t*)(x.sm + P.s_stats);
-    poll_words<32>(x, buf, 3 * P.G, flag, [&](int idx, uint64_t v) { st[idx] = (uint32_t)v; });
-    __syncthreads();
-    float* bc = (float*)(x.sm + P.s_red) + 3 * NWARPS;   // behind block_sum_max's scratch
-    if (x.wid == 0) {
-        double ss = 0.0;
-        float am = 0.0f;
-        for (int g = x.lane; g < P.G; g += 32) {
-            ss += __hiloint2double((int)st[3 * g], (int)st[3 * g + 1]);
-            am = fmaxf(am, __uint_as_float(st[3 * g + 2]));
-        }
-        ss = warp_sum(ss);
-        am = warp_max(am);
-        if (x.lane == 0) {
-            float i_, s_;
-            quant_consts(ss, am, d, P.eps, i_, s_);
-            bc[0] = i_; bc[1] = s_;
-        }
-    }
-    __syncthreads();
-    inv = bc[0];
-    s = bc[1];
 }
-
-// ---- hop (b): quantise the own slice, publish the codes, gather everyone's codes into xq; returns sum q ----
-__device__ __forceinline__ int exchange_codes(const Ctx& x, uint64_t* buf, uint32_t flag8, const float* tq_own, int n_own,
-                                              float inv, const int* starts, int wpc, int K, bool canonical)
+//   word (A / T): the lanes of one warp write the word to all mailboxes
+__device__ __forceinline__ void word_store(const Ctx& x, uint32_t* rec, uint32_t part_off, int idx, uint32_t value)
 {
     const Params& P = x.P;
-    uint8_t* xq = x.sm + P.s_xq;
-    if (x.tid < wpc) {
-        uint64_t v = (uint64_t)flag8 << 56;
-#pragma unroll
-        for (int b = 0; b < CODES_PER_WORD; ++b) {
-            const int i = CODES_PER_WORD * x.tid + b;
-            if (i < n_own) v |= (uint64_t)(uint8_t)(int8_t)quant_code(tq_own[i], inv) << (8 * b);   // inv == 0 -> code 0
-        }
-        ll_store(buf + (size_t)x.c * wpc + x.tid, v);
-    }
-    int qs = 0;
-    poll_words<8>(x, buf, P.G * wpc, flag8, [&](int idx, uint64_t v) {
-        const int g = idx / wpc, j = idx - g * wpc;
-        const int k0 = starts[g], n = starts[g + 1] - k0;
-#pragma unroll
-        for (int b = 0; b < CODES_PER_WORD; ++b) {
-            const int i = CODES_PER_WORD * j + b;
-            if (i < n) {
-                const int q = (int)(int8_t)(uint8_t)(v >> (8 * b));
-                const int k = k0 + i;
-                xq[canonical ? k : plane_pos(k, K)] = (uint8_t)q;
-                qs += q;
-            }
-        }
-    });
-    int* qsum = (int*)((float*)(x.sm + P.s_red) + 3 * NWARPS + 4);
-    if (x.tid == 0) *qsum = 0;
-    __syncthreads();
-    qs = warp_sum_i(qs);
-    if (x.lane == 0 && qs != 0) atomicAdd(qsum, qs);
-    __syncthreads();
-    return *qsum;
+    for (int m = x.lane; m < P.M; m += 32) x_st32(rec + (size_t)m * P.x_words + part_off + idx, value);
 }
 
 __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
@@ -429,9 +517,10 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
     float* s_u = (float*)(sm + P.s_u);
     float* s_z = (float*)(sm + P.s_z);
     float* s_x = (float*)(sm + P.s_x);
-    float* s_tq = (float*)(sm + P.s_tq);
-    float* s_vin = (float*)(sm + P.s_vin);
-    float* s_vout = (float*)(sm + P.s_vout);
+    float* s_dt = (float*)(sm + P.s_dt);
+    double* s_vin = (double*)(sm + P.s_v);
+    double* s_vout = s_vin + P.r_pad;
+    int* s_eacc = (int*)(sm + P.s_eacc);
     int* s_acc_in = (int*)(sm + P.s_acc_in);
     int* s_acc_out = (int*)(sm + P.s_acc_out);
 
@@ -439,6 +528,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         chs[g] = (int)(((long long)g * P.d_inner) / P.G);
         ors[g] = (int)(((long long)g * P.d_model) / P.G);
     }
+    if (tid < 2 * P.r_pad) s_vin[tid] = 0.0;
     if (tid == 0) {
         s_dead = 0;
         for (int s = 0; s < P.stages; ++s) mbar_init(mbar + s, 1);
@@ -454,15 +544,22 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         for (int it = 0; it < P.stages && it < n_items; ++it) issue_item(x, it, v0, v1);
 
     const int ps = P.pos[0] & 3;                     // conv ring slot this step writes
-    const int nb = c < P.n_bcdt ? (P.n_bcdt - c + P.G - 1) / P.G : 0;      // early (B|C|dt) rows of this CTA
+    const int nb_tasks = c < P.n_early ? (P.n_early - c + P.G - 1) / P.G : 0;      // early tasks of this CTA
+    const int h0 = nch > 0 ? ch0 / P.headdim : 0, h1 = nch > 0 ? (ch0 + nch - 1) / P.headdim : -1;
     const bool taps_on = P.taps != nullptr;
+    const size_t rec_words = (size_t)P.M * P.x_words;
+    const int mbox = c / P.gsz;                      // the mailbox this CTA polls
+    uint32_t* s_slotU = (uint32_t*)(sm + P.s_slot);
+    uint32_t* s_slotG = s_slotU + P.u_slot;
+    if (tid < P.u_slot + P.g_slot) s_slotU[tid] = 0u;      // pad words of the slots are published as 0
+    const int KS = P.Wout >= 64 ? 2 : 1;             // K-split of the out_proj sign rows
+    const int tbytes = P.d_inner / P.tsplit;         // bytes of one out_proj LoRA-down partial task
 
-    // LoRA-down rows of this CTA (t = A.xq): row j of t_in belongs to CTA (n_bcdt + j) % G, row j of t_out to
-    // CTA (n_bcdt + r + j) % G.  The last warp fetches its row into registers one phase before it is needed.
-    const int jt_in = (c - P.n_bcdt % P.G + P.G) % P.G;
-    const int jt0 = (c - (P.n_bcdt + P.r) % P.G + 2 * P.G) % P.G;
+    // warp k takes early task k (e = c + k G); if that is a LoRA-down row it fetches the row a phase ahead
+    const int e_first = c + wid * P.G;
+    const bool t_first = wid < nb_tasks && e_first >= P.n_bcdt;
     int4 pre_in[T_PRE];
-    if (wid == NWARPS - 1 && jt_in < P.r && P.L > 0) trow_prefetch(P.A_in + (size_t)jt_in * P.d_model, P.d_model, lane, pre_in);
+    if (t_first && P.L > 0) trow_prefetch(P.A_in + (size_t)(e_first - P.n_bcdt) * P.d_model, P.d_model, lane, pre_in);
 
     // ---------------- S0 embedding + the first norm/quantise, redundantly in every CTA ----------------
     float s_act;                                     // scale of the current activation codes
@@ -475,119 +572,156 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         }
         const int8_t* erow = P.emb + (size_t)tok * P.d_model;
         const float es = P.emb_s[tok];
+        uint4 v[4];
         double ss = 0.0;
-        float amax = 0.0f;
-        for (int k = tid; k < P.d_model; k += THREADS) {
-            const float u = fmul(es, (float)erow[k]);
-            ss = dacc(ss, u, u);
-            amax = fmaxf(amax, fabsf(fmul(u, P.first_norm_w[k])));
-            if (k >= or0 && k < or0 + nor) s_u[k - or0] = u;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int k0 = 4 * (tid + j * THREADS);
+            if (k0 < P.d_model) {
+                uint32_t w[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const float u = fmul(es, (float)erow[k0 + e]);
+                    ss = dacc(ss, u, u);
+                    w[e] = __float_as_uint(fmul(u, P.first_norm_w[k0 + e]));
+                    if (k0 + e >= or0 && k0 + e < or0 + nor) s_u[k0 + e - or0] = u;
+                }
+                v[j] = make_uint4(w[0], w[1], w[2], w[3]);
+            }
         }
-        block_sum_max(x, ss, amax);
-        float inv;
-        quant_consts(ss, amax, P.d_model, P.eps, inv, s_act);
-        int qs = 0;
-        const bool canon = P.L == 0;
-        for (int k = tid; k < P.d_model; k += THREADS) {
-            const float u = fmul(es, (float)erow[k]);
-            const int q = amax == 0.0f ? 0 : quant_code(fmul(u, P.first_norm_w[k]), inv);
-            xq[canon ? k : plane_pos(k, P.d_model)] = (uint8_t)q;
-            qs += q;
-        }
-        int* qsp = (int*)((float*)(sm + P.s_red) + 3 * NWARPS + 4);
-        if (tid == 0) *qsp = 0;
-        __syncthreads();
-        qs = warp_sum_i(qs);
-        if (lane == 0 && qs != 0) atomicAdd(qsp, qs);
-        __syncthreads();
-        qsum = *qsp;
+        // the per-CTA partial sums of the exchange are replaced by the per-warp partial sums of this CTA
+        double* part = (double*)(sm + P.s_part);
+        ss = warp_sum(ss);
+        for (int g = tid; g < P.G; g += THREADS)
+            if (g >= NWARPS) part[g] = 0.0;
+        if (lane == 0) part[wid] = ss;
+        uint8_t* tp0 = (taps_on && c == 0 && P.L > 0) ? P.taps : nullptr;
+        auto en = [&](auto f) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int k0 = 4 * (tid + j * THREADS);
+                if (k0 < P.d_model) { f(k0, v[j].x); f(k0 + 1, v[j].y); f(k0 + 2, v[j].z); f(k0 + 3, v[j].w); }
+            }
+        };
+        qsum = norm_quant(x, en, P.d_model, P.L == 0, s_act, tp0 ? (int8_t*)(tp0 + P.tl.off[0]) : nullptr);
+        if (tp0 && tid == 0) *(float*)(tp0 + P.tl.off[1]) = s_act;
     }
 
     // =============================================== layers ===============================================
     for (int l = 0; l < P.L; ++l) {
-        const uint32_t f32 = P.base32 + 8u * (uint32_t)l;                   // 32-bit flags of this layer: f32 + hop
-        const uint32_t f8 = (uint32_t)((P.e255 * (uint32_t)(P.L + 1) + (uint32_t)l + 1u) % 255u) + 1u;   // codes(u) after layer l
-        const uint32_t f8g = (uint32_t)((P.e255 * (uint32_t)(P.L + 1) + (uint32_t)l) % 255u) + 1u;       // codes(g) of layer l
         uint8_t* stage = sm + P.s_ring + (size_t)(l % P.stages) * P.stage_bytes;
+        const uint8_t* blk = stage + P.st_blk;
         uint8_t* tp = taps_on ? P.taps + (size_t)l * P.tap_lstride : nullptr;
         float* conv_l = P.conv + (size_t)l * P.conv_lstride;
+        uint32_t* rec = P.xbuf + (size_t)((P.rec0 + (uint32_t)l) & 3u) * rec_words;          // published into (all mailboxes)
+        const uint32_t* mine = rec + (size_t)mbox * P.x_words;                                 // polled
+        uint32_t* recc = P.xbuf + (size_t)((P.rec0 + (uint32_t)l + 2u) & 3u) * rec_words;     // reset for layer l + 2
         DFSSM_STAMP(l, 0);
         if (P.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + 15] = globaltimer_ns();
-
-        if (tp && c == 0) {
-            for (int k = tid; k < P.d_model; k += THREADS) ((int8_t*)(tp + P.tl.off[0]))[k] = (int8_t)xq[plane_pos(k, P.d_model)];
-            if (tid == 0) *(float*)(tp + P.tl.off[1]) = s_act;
+        {   // reset own slots of the record two layers ahead (same thread -> address map as the publishes below)
+            slot_store(x, recc, P.x_U, P.u_slot, [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
+            slot_store(x, recc, P.x_G, P.g_slot, [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
+            for (int k = wid; k < nb_tasks; k += NWARPS) word_store(x, recc, P.x_A, c + k * P.G, SENT);
+            if (wid == 0)
+                for (int e = c; e < P.n_ttask; e += P.G) word_store(x, recc, P.x_T, e, SENT);
         }
 
-        // ---- t_in rows owned by this CTA (warp NWARPS-1): LoRA down-projection on the int8 codes ----
-        if (wid == NWARPS - 1) {
-            for (int j = jt_in; j < P.r; j += P.G) {
-                const int8_t* arow = P.A_in + ((size_t)l * P.r + j) * P.d_model;
-                if (j != jt_in) trow_prefetch(arow, P.d_model, lane, pre_in);
-                const int t = trow_dot(arow, P.d_model, xq, lane, pre_in);
-                if (lane == 0) {
-                    ll_store(P.x_t + j, ll_pack32((uint32_t)t, f32 + 0));
-                    if (tp) ((int32_t*)(tp + P.tl.off[3]))[j] = t;
-                }
-            }
-        }
-        DFSSM_STAMP(l, 1);
         wait_item(x, l);
-        DFSSM_STAMP(l, 2);
-
-        // ---- S2: sign rows of this CTA (early rows first, then z, then x), 4 rows per warp pass ----
+        DFSSM_STAMP(l, 1);
+        // ---- early tasks: B|C|dt sign rows and LoRA-down rows of this CTA; raw int32 results are published ----
         {
             const uint32_t* bits = (const uint32_t*)(stage + P.c_in_bits);
-            const int n_tasks = nb + 2 * nch;
-            for (int q0 = 4 * wid; q0 < n_tasks; q0 += 4 * NWARPS) {
-                const uint32_t* rowp[4];
-                int slot[4];
-                const int nrows = min(4, n_tasks - q0);
-#pragma unroll
-                for (int r = 0; r < 4; ++r) {
-                    const int t = q0 + r;
-                    slot[r] = t < nb ? 2 * P.nch_max + t : (t < nb + nch ? t - nb : P.nch_max + (t - nb - nch));
-                    if (r >= nrows) slot[r] = 0;
-                    rowp[r] = bits + (size_t)slot[r] * P.Win;
+            for (int k = wid; k < nb_tasks; k += NWARPS) {
+                const int e = c + k * P.G;
+                int val;
+                if (e < P.n_bcdt) {
+                    const uint32_t* const rowp[1] = { bits + (size_t)(2 * P.nch_max + k) * P.Win };
+                    int p[1];
+                    sign_partial<1>(rowp, 1, 0, P.Win, xq, P.d_model, lane, p);
+                    val = 2 * (warp_sum_i(p[0]) / 128) - qsum;       // exact: every term is a multiple of 128
+                } else {
+                    const int8_t* arow = P.A_in + ((size_t)l * P.r + (e - P.n_bcdt)) * P.d_model;
+                    if (k != wid) trow_prefetch(arow, P.d_model, lane, pre_in);
+                    val = trow_dot(arow, P.d_model, xq, lane, pre_in);
                 }
-                const int acc = sign_dot4(rowp, nrows, P.Win, xq, P.d_model, qsum, lane);
-                const int r = lane >> 3;
-                if ((lane & 7) == 0 && r < nrows) s_acc_in[slot[r]] = acc;
+                word_store(x, rec, P.x_A, e, (uint32_t)val ^ IBIAS);
+                if (lane == 0 && tp && e >= P.n_bcdt) ((int32_t*)(tp + P.tl.off[3]))[e - P.n_bcdt] = val;
             }
         }
-        DFSSM_STAMP(l, 3);
-        // ---- gather t_in, v_j = a_s[j] * float(t_j) ----
+        // ---- S2: z and x sign rows of this CTA, 4 rows per warp pass, dealt from the top warp down ----
         {
-            const float* a_s = (const float*)(stage + P.c_as_in);
-            poll_words<32>(x, P.x_t, P.r, f32 + 0, [&](int j, uint64_t v) { s_vin[j] = fmul(a_s[j], (float)(int32_t)(uint32_t)v); });
+            const uint32_t* bits = (const uint32_t*)(stage + P.c_in_bits);
+            const int n_tasks = 2 * nch;
+            for (int q = NWARPS - 1 - wid; 4 * q < n_tasks; q += NWARPS) {
+                const uint32_t* rowp[4];
+                int slot[4];
+                const int nrows = min(4, n_tasks - 4 * q);
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const int t = 4 * q + r;
+                    slot[r] = r < nrows ? (t < nch ? t : P.nch_max + (t - nch)) : 0;
+                    rowp[r] = bits + (size_t)slot[r] * P.Win;
+                }
+                int p[4];
+                sign_partial<4>(rowp, nrows, 0, P.Win, xq, P.d_model, lane, p);
+                const int v = reduce4(p, lane);
+                const int r = lane >> 3;
+                if ((lane & 7) == 0 && r < nrows) s_acc_in[slot[r]] = 2 * (v / 128) - qsum;
+            }
+        }
+        DFSSM_STAMP(l, 2);
+        // ---- gather A: accumulators of all B|C|dt rows and t_in;  v_j = a_s[j] * float(t_j) ----
+        {
+            uint4 va[2];
+            hop_gather<2>(x, mine + P.x_A, P.n_early, 0, 0, va);
+            const float* a_s = (const float*)(blk + P.b_as_in);
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const int e0 = 4 * (tid + j * THREADS);
+                const uint32_t w[4] = { va[j].x, va[j].y, va[j].z, va[j].w };
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const int e = e0 + i;
+                    if (e < P.n_early) {
+                        const int val = (int)(w[i] ^ IBIAS);
+                        if (e < P.n_bcdt) s_eacc[e] = val;
+                        else s_vin[e - P.n_bcdt] = (double)fmul(a_s[e - P.n_bcdt], (float)val);
+                    }
+                }
+            }
         }
         __syncthreads();
-
-        DFSSM_STAMP(l, 4);
-        // ---- S3 stage 2 + S4 conv + dt softplus: 4 lanes per row ----
+        DFSSM_STAMP(l, 3);
+        // ---- S3 stage 2 + S4 conv + dt softplus: one thread per row; own z|x rows and ALL B|C rows (+ own dt) ----
         {
-            const int n_rows = 2 * nch + nb;
-            const int8_t* Bm = (const int8_t*)(stage + P.c_in_B);
-            const float* scale = (const float*)(stage + P.c_in_scale);
-            const float* bsv = (const float*)(stage + P.c_in_bs);
+            const int n_dt = tp ? P.nheads : (h1 - h0 + 1);
+            const int n_rows = 2 * nch + 2 * P.gs + n_dt;
             float* ring = (float*)(stage + P.st_conv);
-            for (int ib = 0; ib < n_rows; ib += THREADS / 4) {       // warp-uniform trip count (shuffles inside)
-                const int i = ib + (tid >> 2), sub = tid & 3;
-                const bool valid = i < n_rows;
-                int slot = 0, kind = 0, e = 0;     // kind 0 z, 1 x, 2 early
+            const float* ering = (const float*)(stage + P.st_econv);
+            for (int i = tid; i < n_rows; i += THREADS) {
+                int kind, slot = 0, e = 0;         // kind 0 z, 1 x, 2 B|C, 3 dt
                 if (i < nch) { kind = 0; slot = i; }
                 else if (i < 2 * nch) { kind = 1; slot = P.nch_max + (i - nch); }
-                else if (valid) { kind = 2; slot = 2 * P.nch_max + (i - 2 * nch); e = c + (i - 2 * nch) * P.G; }
-                double lo = 0.0;
-                const int8_t* brow = Bm + (size_t)slot * P.r_pad;
-                if (valid)
-                    for (int j = sub; j < P.r; j += 4) lo = dacc(lo, (float)brow[j], s_vin[j]);
-                lo += __shfl_xor_sync(0xffffffffu, lo, 1);
-                lo += __shfl_xor_sync(0xffffffffu, lo, 2);
-                if (sub != 0 || !valid) continue;
-                const int acc = s_acc_in[slot];
-                const float val = fmul(s_act, fadd(fmul(scale[slot], (float)acc), fmul(bsv[slot], (float)lo)));
-                int row;                   // canonical in_proj row (for the taps)
+                else if (i < 2 * nch + 2 * P.gs) { kind = 2; e = i - 2 * nch; }
+                else { kind = 3; e = 2 * P.gs + (tp ? 0 : h0) + (i - 2 * nch - 2 * P.gs); }
+                const bool own = kind < 2;
+                const int8_t* brow = own ? (const int8_t*)(stage + P.c_in_B) + (size_t)slot * P.r_pad
+                                         : (const int8_t*)(blk + P.b_eB) + (size_t)e * P.r_pad;
+                const float scale = own ? ((const float*)(stage + P.c_in_scale))[slot] : ((const float*)(blk + P.b_escale))[e];
+                const float bsv = own ? ((const float*)(stage + P.c_in_bs))[slot] : ((const float*)(blk + P.b_ebs))[e];
+                const int acc = own ? s_acc_in[slot] : s_eacc[e];
+                double lo0 = 0.0, lo1 = 0.0;
+                for (int j4 = 0; j4 < P.r_pad; j4 += 4) {         // pad entries of B are 0, pad entries of v are 0
+                    const int w = *(const int*)(brow + j4);
+                    lo0 = __fma_rn((double)((int)((unsigned)w << 24) >> 24), s_vin[j4], lo0);
+                    lo1 = __fma_rn((double)((int)((unsigned)w << 16) >> 24), s_vin[j4 + 1], lo1);
+                    lo0 = __fma_rn((double)((int)((unsigned)w << 8) >> 24), s_vin[j4 + 2], lo0);
+                    lo1 = __fma_rn((double)(w >> 24), s_vin[j4 + 3], lo1);
+                }
+                const float lo = (float)(lo0 + lo1);
+                const float val = fmul(s_act, fadd(fmul(scale, (float)acc), fmul(bsv, lo)));
+                int row;                       // canonical in_proj row (for the taps)
+                bool tap_owner = true;
                 if (kind == 0) {
                     s_z[i] = val;
                     row = ch0 + i;
@@ -603,43 +737,45 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     s_x[ic] = cv;
                     row = P.d_inner + ch0 + ic;
                     if (tp) ((float*)(tp + P.tl.off[5]))[ch0 + ic] = cv;
-                } else {
-                    const int ie = i - 2 * nch;
+                } else if (kind == 2) {
+                    const float* rg = ering + 4 * e;
+                    const float s0 = rg[(ps + 1) & 3], s1 = rg[(ps + 2) & 3], s2 = rg[(ps + 3) & 3];
+                    const float4 cw = *(const float4*)(blk + P.b_econv_w + 16 * e);
+                    float o = ((const float*)(blk + P.b_econv_b))[e];
+                    o = ffma(cw.x, s0, o); o = ffma(cw.y, s1, o); o = ffma(cw.z, s2, o); o = ffma(cw.w, val, o);
+                    tap_owner = e % P.G == c;
+                    if (tap_owner) conv_l[4 * (size_t)(P.d_inner + e) + ps] = val;      // the early-task owner keeps the state
+                    const float cv = siluf(o);
+                    s_bc[e] = cv;
                     row = 2 * P.d_inner + e;
-                    float outv;
-                    if (e < 2 * P.gs) {        // B or C channel: conv state lives in global memory (4-slot ring)
-                        float* rg = conv_l + 4 * (size_t)(P.d_inner + e);
-                        const float4 rv = *(const float4*)rg;
-                        const float sl[4] = { rv.x, rv.y, rv.z, rv.w };
-                        const float s0 = sl[(ps + 1) & 3], s1 = sl[(ps + 2) & 3], s2 = sl[(ps + 3) & 3];
-                        const float4 cw = *(const float4*)(stage + P.c_e_conv_w + 16 * ie);
-                        float o = ((const float*)(stage + P.c_e_conv_b))[ie];
-                        o = ffma(cw.x, s0, o); o = ffma(cw.y, s1, o); o = ffma(cw.z, s2, o); o = ffma(cw.w, val, o);
-                        rg[ps] = val;
-                        outv = siluf(o);
-                        if (tp) ((float*)(tp + P.tl.off[5]))[P.d_inner + e] = outv;
-                    } else {                   // dt
-                        outv = sp_softplusf(fadd(val, ((const float*)(stage + P.c_e_dtb))[ie]));
-                        if (tp) ((float*)(tp + P.tl.off[6]))[e - 2 * P.gs] = outv;
-                    }
-                    ll_store(P.x_bc + e, ll_pack32(__float_as_uint(outv), f32 + 1));
+                    if (tp && tap_owner) ((float*)(tp + P.tl.off[5]))[P.d_inner + e] = cv;
+                } else {
+                    const int h = e - 2 * P.gs;
+                    const float dtv = sp_softplusf(fadd(val, ((const float*)(blk + P.b_dtb))[h]));
+                    s_dt[h] = dtv;
+                    row = 2 * P.d_inner + e;
+                    tap_owner = e % P.G == c;
+                    if (tp && tap_owner) ((float*)(tp + P.tl.off[6]))[h] = dtv;
                 }
-                if (tp) {
+                if (tp && tap_owner) {
                     ((float*)(tp + P.tl.off[4]))[row] = val;
                     ((int32_t*)(tp + P.tl.off[2]))[row] = acc;
                 }
             }
         }
-        DFSSM_STAMP(l, 5);
-        // ---- gather B' | C' | dt ----
-        poll_words<32>(x, P.x_bc, P.n_bcdt, f32 + 1, [&](int e, uint64_t v) { s_bc[e] = __uint_as_float((uint32_t)v); });
         __syncthreads();
+        DFSSM_STAMP(l, 4);
 
-        DFSSM_STAMP(l, 6);
-        // ---- S5 state update + readout, S6 gate: 16 lanes per channel ----
-        double ss_own = 0.0;
-        float amax_own = 0.0f;
+        // out_proj LoRA-down partial task of this CTA (warp 0): fetch the weights now, use them after gather G
+        const int et_first = c;
+        const bool tt_first = wid == 0 && et_first < P.n_ttask;
+        int4 pre_out[T_PRE];
+        if (tt_first)
+            trow_prefetch(P.A_out + ((size_t)l * P.r + et_first / P.tsplit) * P.d_inner + (size_t)(et_first % P.tsplit) * tbytes, tbytes, lane, pre_out);
+
+        // ---- S5 state update + readout, S6 gate: 16 lanes per channel; t = g*w is published as it is produced ----
         {
+            double ss_own = 0.0;
             const int hpg = P.nheads / P.ngroups;
             const float* alog = (const float*)(stage + P.c_alog);
             const float* Dv = (const float*)(stage + P.c_D);
@@ -649,7 +785,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 const int i = min(ib + (tid >> 4), nch - 1);
                 const bool valid = ib + (tid >> 4) < nch;
                 const int ch = ch0 + i, h = ch / P.headdim, grp = h / hpg;
-                const float dtv = s_bc[2 * P.gs + h];
+                const float dtv = s_dt[h];
                 const float An = -sp_expf(alog[i]);
                 const float dA = sp_expf(fmul(dtv, An));
                 const float xv = s_x[i];
@@ -675,75 +811,95 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     a = dacc(a, Dv[i], xv);
                     const float y = (float)a;
                     const float gv = fmul(y, siluf(s_z[i]));
-                    const float tq = fmul(gv, gw[i]);
-                    s_tq[i] = tq;
+                    s_slotG[i] = __float_as_uint(fmul(gv, gw[i]));
                     ss_own = dacc(ss_own, gv, gv);
-                    amax_own = fmaxf(amax_own, fabsf(tq));
                     if (tp) { ((float*)(tp + P.tl.off[7]))[ch] = y; ((float*)(tp + P.tl.off[8]))[ch] = gv; }
                 }
             }
             fence_proxy_async();               // the updated state is about to be read by the async proxy
-            block_sum_max(x, ss_own, amax_own);
+            ss_own = warp_sum(ss_own);
+            if (lane == 0) red_d(x)[wid] = ss_own;
+            __syncthreads();
+            slot_store(x, rec, P.x_G, P.g_slot, [&](int piece) {
+                uint4 w = *(const uint4*)(s_slotG + 4 * piece);
+                const int ex = P.g_dpos - 4 * piece;
+                if (ex == 0 || ex == 2) {
+                    double tot = 0.0;
+#pragma unroll
+                    for (int i = 0; i < NWARPS; ++i) tot += red_d(x)[i];
+                    const uint32_t lo = (uint32_t)__double2loint(tot), hi = (uint32_t)__double2hiint(tot);
+                    if (ex == 0) { w.x = lo; w.y = hi; } else { w.z = lo; w.w = hi; }
+                }
+                return w;
+            });
+            if (tid == 0 && nch > 0) {         // write the state slice back (async), while the exchange goes on
+                bulk_s2g(P.ssm + (size_t)l * P.ssm_lstride + (size_t)ch0 * P.d_state, stage + P.st_ssm, (uint32_t)nch * P.d_state * 4);
+                bulk_s2g(conv_l + (size_t)ch0 * 4, stage + P.st_conv, (uint32_t)nch * 16);
+                bulk_commit();
+            }
+        }
+        DFSSM_STAMP(l, 5);
+
+        // ---- gather G, S6 norm + quantise of the whole gated vector in every CTA ----
+        float s_g;
+        int qsum_g;
+        {
+            uint4 vg[4];
+            hop_gather<4>(x, mine + P.x_G, P.G * P.g_slot, P.g_slot, P.g_dpos, vg);
+            DFSSM_STAMP(l, 6);
+            slot_partials<4>(x, vg, P.G, P.g_slot, P.g_dpos);
+            qsum_g = norm_quant(x, SlotEnum<4>{ vg, chs, tid, P.G, P.g_slot >> 2 }, P.d_inner, false, s_g,
+                                (tp && c == 0) ? (int8_t*)(tp + P.tl.off[9]) : nullptr);
+            if (tp && c == 0 && tid == 0) *(float*)(tp + P.tl.off[10]) = s_g;
         }
         DFSSM_STAMP(l, 7);
-        // ---- write the state slice back (async), while the exchanges go on ----
-        if (tid == 0 && nch > 0) {
-            bulk_s2g(P.ssm + (size_t)l * P.ssm_lstride + (size_t)ch0 * P.d_state, stage + P.st_ssm, (uint32_t)nch * P.d_state * 4);
-            bulk_s2g(conv_l + (size_t)ch0 * 4, stage + P.st_conv, (uint32_t)nch * 16);
-            bulk_commit();
+        // ---- S7: LoRA-down partial tasks (warp 0, published) and the out_proj sign rows (other warps) ----
+        if (wid == 0) {
+            for (int e = c; e < P.n_ttask; e += P.G) {
+                const int j = e / P.tsplit, part = e % P.tsplit;
+                const int8_t* arow = P.A_out + ((size_t)l * P.r + j) * P.d_inner + (size_t)part * tbytes;
+                if (e != c) trow_prefetch(arow, tbytes, lane, pre_out);
+                const int t = trow_dot(arow, tbytes, xq + (size_t)part * tbytes, lane, pre_out);
+                word_store(x, rec, P.x_T, e, (uint32_t)t ^ IBIAS);
+            }
+        } else {
+            const uint32_t* bits = (const uint32_t*)(stage + P.c_out_bits);
+            const int npair = (nor + 1) >> 1, wspan = P.Wout / KS;
+            for (int id = wid - 1; id < npair * KS; id += NWARPS - 1) {
+                const int pair = id / KS, half = id - pair * KS;
+                const int nrows = min(2, nor - 2 * pair);
+                const uint32_t* const rowp[2] = { bits + (size_t)(2 * pair) * P.Wout, bits + (size_t)(2 * pair + (nrows > 1 ? 1 : 0)) * P.Wout };
+                int p[2];
+                sign_partial<2>(rowp, nrows, half * wspan, half == KS - 1 ? P.Wout : (half + 1) * wspan, xq, P.d_inner, lane, p);
+                const int v = reduce2(p, lane);
+                const int r = lane >> 4;
+                if ((lane & 15) == 0 && r < nrows) s_acc_out[half * P.nor_max + 2 * pair + r] = v;
+            }
         }
-        // t_out row of this CTA: start fetching the LoRA-down row now, use it after the codes arrive
-        int4 pre_out[T_PRE];
-        if (wid == NWARPS - 1 && jt0 < P.r) trow_prefetch(P.A_out + ((size_t)l * P.r + jt0) * P.d_inner, P.d_inner, lane, pre_out);
-
-        // ---- S6 norm + quantise of g: stats hop, codes hop ----
-        float inv_g, s_g;
-        exchange_stats(x, P.x_stat3, f32 + 2, ss_own, amax_own, P.d_inner, inv_g, s_g);
         DFSSM_STAMP(l, 8);
-        const int qsum_g = exchange_codes(x, P.x_code3, f8g, s_tq, nch, inv_g, chs, P.wpc3, P.d_inner, false);
-        if (tp && c == 0) {
-            for (int k = tid; k < P.d_inner; k += THREADS) ((int8_t*)(tp + P.tl.off[9]))[k] = (int8_t)xq[plane_pos(k, P.d_inner)];
-            if (tid == 0) *(float*)(tp + P.tl.off[10]) = s_g;
-        }
-
-        DFSSM_STAMP(l, 9);
-        // ---- S7: t_out rows (last warp) and the out_proj sign rows of this CTA ----
-        if (wid == NWARPS - 1) {
-            for (int j = jt0; j < P.r; j += P.G) {
-                const int8_t* arow = P.A_out + ((size_t)l * P.r + j) * P.d_inner;
-                if (j != jt0) trow_prefetch(arow, P.d_inner, lane, pre_out);
-                const int t = trow_dot(arow, P.d_inner, xq, lane, pre_out);
-                if (lane == 0) {
-                    ll_store(P.x_t4 + j, ll_pack32((uint32_t)t, f32 + 3));
-                    if (tp) ((int32_t*)(tp + P.tl.off[12]))[j] = t;
+        // ---- gather T: t_out = sum of the partial sums;  v_j = a_s[j] * float(t_j) ----
+        {
+            uint4 vt[1];
+            hop_gather<1>(x, mine + P.x_T, P.n_ttask, 0, 0, vt);
+            const float* a_s = (const float*)(blk + P.b_as_out);
+            const uint32_t w[4] = { vt[0].x, vt[0].y, vt[0].z, vt[0].w };
+            const int rows_per_chunk = 4 / P.tsplit;
+#pragma unroll
+            for (int jj = 0; jj < 4; ++jj) {
+                const int j = tid * rows_per_chunk + jj;
+                if (jj < rows_per_chunk && j < P.r) {
+                    int t = 0;
+                    for (int q = 0; q < P.tsplit; ++q) t += (int)(w[jj * P.tsplit + q] ^ IBIAS);
+                    s_vout[j] = (double)fmul(a_s[j], (float)t);
+                    if (tp && c == 0) ((int32_t*)(tp + P.tl.off[12]))[j] = t;
                 }
             }
         }
-        {
-            const uint32_t* bits = (const uint32_t*)(stage + P.c_out_bits);
-            // the last warp is busy with t_out when it owns one: the other warps take the quads first
-            for (int q = (wid + 1) % NWARPS; 4 * q < nor; q += NWARPS) {
-                const uint32_t* rowp[4];
-                const int nrows = min(4, nor - 4 * q);
-#pragma unroll
-                for (int r = 0; r < 4; ++r) rowp[r] = bits + (size_t)(r < nrows ? 4 * q + r : 0) * P.Wout;
-                const int acc = sign_dot4(rowp, nrows, P.Wout, xq, P.d_inner, qsum_g, lane);
-                const int r = lane >> 3;
-                if ((lane & 7) == 0 && r < nrows) s_acc_out[4 * q + r] = acc;
-            }
-        }
-        DFSSM_STAMP(l, 10);
-        {
-            const float* a_s = (const float*)(stage + P.c_as_out);
-            poll_words<32>(x, P.x_t4, P.r, f32 + 3, [&](int j, uint64_t v) { s_vout[j] = fmul(a_s[j], (float)(int32_t)(uint32_t)v); });
-        }
         __syncthreads();
-
-        DFSSM_STAMP(l, 11);
-        // ---- S7 epilogue + residual; stats of the new u for the next norm ----
-        double ss_u = 0.0;
-        float amax_u = 0.0f;
+        DFSSM_STAMP(l, 9);
+        // ---- S7 epilogue + residual; t = u*w of the next norm is published as it is produced ----
         {
+            double ss_u = 0.0;
             const int8_t* Bm = (const int8_t*)(stage + P.c_out_B);
             const float* scale = (const float*)(stage + P.c_out_scale);
             const float* bsv = (const float*)(stage + P.c_out_bs);
@@ -754,36 +910,54 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 double lo = 0.0;
                 const int8_t* brow = Bm + (size_t)(valid ? i : 0) * P.r_pad;
                 if (valid)
-                    for (int j = sub; j < P.r; j += 4) lo = dacc(lo, (float)brow[j], s_vout[j]);
+                    for (int j = sub; j < P.r; j += 4) lo = __fma_rn((double)brow[j], s_vout[j], lo);
                 lo += __shfl_xor_sync(0xffffffffu, lo, 1);
                 lo += __shfl_xor_sync(0xffffffffu, lo, 2);
                 if (sub != 0 || !valid) continue;
-                const int acc = s_acc_out[i];
+                const int p128 = s_acc_out[i] + (KS > 1 ? s_acc_out[P.nor_max + i] : 0);
+                const int acc = 2 * (p128 / 128) - qsum_g;       // exact: every term is a multiple of 128
                 const float o = fmul(s_g, fadd(fmul(scale[i], (float)acc), fmul(bsv[i], (float)lo)));
                 const float un = fadd(s_u[i], o);
                 s_u[i] = un;
-                const float tq = fmul(un, nw[i]);
-                s_tq[i] = tq;
+                s_slotU[i] = __float_as_uint(fmul(un, nw[i]));
                 ss_u = dacc(ss_u, un, un);
-                amax_u = fmaxf(amax_u, fabsf(tq));
                 if (tp) { ((float*)(tp + P.tl.off[13]))[or0 + i] = un; ((int32_t*)(tp + P.tl.off[11]))[or0 + i] = acc; }
             }
-            block_sum_max(x, ss_u, amax_u);     // also: every thread is done with this stage's weights
+            ss_u = warp_sum(ss_u);
+            if (lane == 0) red_d(x)[wid] = ss_u;
+            __syncthreads();                        // also: every thread is done with this stage's weights
+            slot_store(x, rec, P.x_U, P.u_slot, [&](int piece) {
+                uint4 w = *(const uint4*)(s_slotU + 4 * piece);
+                const int ex = P.u_dpos - 4 * piece;
+                if (ex == 0 || ex == 2) {
+                    double tot = 0.0;
+#pragma unroll
+                    for (int i = 0; i < NWARPS; ++i) tot += red_d(x)[i];
+                    const uint32_t lo = (uint32_t)__double2loint(tot), hi = (uint32_t)__double2hiint(tot);
+                    if (ex == 0) { w.x = lo; w.y = hi; } else { w.z = lo; w.w = hi; }
+                }
+                return w;
+            });
+            if (tid == 0) {
+                bulk_wait_read0();                  // the state write-back has finished reading the stage
+                if (l + P.stages < n_items) issue_item(x, l + P.stages, v0, v1);
+            }
+        }
+        if (t_first && l + 1 < P.L)
+            trow_prefetch(P.A_in + ((size_t)(l + 1) * P.r + (e_first - P.n_bcdt)) * P.d_model, P.d_model, lane, pre_in);
+        DFSSM_STAMP(l, 10);
+        // ---- gather U, S1 of the next layer (or S8's norm) in every CTA ----
+        {
+            uint4 vu[2];
+            hop_gather<2>(x, mine + P.x_U, P.G * P.u_slot, P.u_slot, P.u_dpos, vu);
+            DFSSM_STAMP(l, 11);
+            slot_partials<2>(x, vu, P.G, P.u_slot, P.u_dpos);
+            uint8_t* tpn = (taps_on && c == 0 && l + 1 < P.L) ? P.taps + (size_t)(l + 1) * P.tap_lstride : nullptr;
+            qsum = norm_quant(x, SlotEnum<2>{ vu, ors, tid, P.G, P.u_slot >> 2 }, P.d_model, l == P.L - 1, s_act,
+                              tpn ? (int8_t*)(tpn + P.tl.off[0]) : nullptr);
+            if (tpn && tid == 0) *(float*)(tpn + P.tl.off[1]) = s_act;
         }
         DFSSM_STAMP(l, 12);
-        // ---- refill this ring stage with the item `stages` ahead ----
-        if (tid == 0) {
-            bulk_wait_read0();                  // the state write-back has finished reading the stage
-            if (l + P.stages < n_items) issue_item(x, l + P.stages, v0, v1);
-        }
-        if (wid == NWARPS - 1 && jt_in < P.r && l + 1 < P.L)
-            trow_prefetch(P.A_in + ((size_t)(l + 1) * P.r + jt_in) * P.d_model, P.d_model, lane, pre_in);
-        // ---- S1 of the next layer (or S8's norm): stats hop, codes hop ----
-        float inv_u;
-        exchange_stats(x, P.x_stat1, f32 + 4, ss_u, amax_u, P.d_model, inv_u, s_act);
-        DFSSM_STAMP(l, 13);
-        qsum = exchange_codes(x, P.x_code1, f8, s_tq, nor, inv_u, ors, P.wpc1, P.d_model, l == P.L - 1);
-        DFSSM_STAMP(l, 14);
     }
 
     // =============================================== S8 LM head ===============================================
@@ -813,17 +987,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     }
                 }
             }
-            const bool up16 = (lane & 16) != 0, up8 = (lane & 8) != 0;
-            int k0 = up16 ? s[2] : s[0], k1 = up16 ? s[3] : s[1];
-            const int t0 = up16 ? s[0] : s[2], t1 = up16 ? s[1] : s[3];
-            k0 += __shfl_xor_sync(0xffffffffu, t0, 16);
-            k1 += __shfl_xor_sync(0xffffffffu, t1, 16);
-            int v = up8 ? k1 : k0;
-            const int sv = up8 ? k0 : k1;
-            v += __shfl_xor_sync(0xffffffffu, sv, 8);
-            v += __shfl_xor_sync(0xffffffffu, v, 4);
-            v += __shfl_xor_sync(0xffffffffu, v, 2);
-            v += __shfl_xor_sync(0xffffffffu, v, 1);
+            const int v = reduce4(s, lane);
             const int r = lane >> 3;
             if ((lane & 7) == 0 && r < nr) {
                 const int row = row0 + q0 + r;
@@ -844,8 +1008,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             const int oi = __shfl_xor_sync(0xffffffffu, besti, o);
             if (ov > best || (ov == best && oi < besti)) { best = ov; besti = oi; }
         }
-        float* rv = (float*)(sm + P.s_red);
-        int* ri = (int*)(rv + NWARPS);
+        float* rv = red_f(x);
+        int* ri = red_i(x);
         __shared__ int s_last;
         if (lane == 0) { rv[wid] = best; ri[wid] = besti; }
         __syncthreads();

@@ -1,6 +1,7 @@
 // Host side of the mega path: the per-(layer, CTA) chunk layout, the shared-memory plan, and the
 // load-time repack of the canonical blob (DESIGN.md sections 3 and 6) into that layout.
 #pragma once
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -25,7 +26,8 @@ inline bool plan(const Dims& d, int G, Params& P)
     P.n_bcdt = 2 * P.gs + d.nheads;
     P.eps = d.eps;
     P.G = G;
-    if (d.d_state % 4 || d.d_model % 32 || d.d_inner % 32 || d.r > 64) return false;
+    if (d.d_state % 4 || d.d_model % 32 || d.d_inner % 32 || d.r > 64 || (G & 1)) return false;
+    if (d.d_model > 16 * THREADS || d.d_inner > 16 * THREADS) return false;       // 4 chunks of 4 words per thread
     P.nch_max = (d.d_inner + G - 1) / G;
     P.nor_max = (d.d_model + G - 1) / G;
     P.nb_max = (P.n_bcdt + G - 1) / G;
@@ -33,49 +35,81 @@ inline bool plan(const Dims& d, int G, Params& P)
     P.r_pad = (d.r + 3) / 4 * 4;
     P.Win = d.d_model / 32;
     P.Wout = d.d_inner / 32;
-    P.wpc1 = (P.nor_max + CODES_PER_WORD - 1) / CODES_PER_WORD;
-    P.wpc3 = (P.nch_max + CODES_PER_WORD - 1) / CODES_PER_WORD;
-    if (P.wpc1 > THREADS || P.wpc3 > THREADS) return false;
+    P.n_early = P.n_bcdt + d.r;
+    if (P.n_early > 8 * THREADS || P.n_early > 64 * G) return false;
+    P.tsplit = (d.d_inner % 64 == 0 && 4 * d.r <= G) ? 4 : (2 * d.r <= G ? 2 : 1);
+    P.n_ttask = d.r * P.tsplit;
+    if (P.nch_max > 128 || P.nor_max > 128 || d.d_inner < G || d.d_model < G) return false;
 
     uint32_t off = 0;
     auto take = [&](size_t bytes) { off = up32(off, 16); const uint32_t at = off; off += (uint32_t)bytes; return at; };
     P.c_in_bits = take((size_t)P.n_slots * P.Win * 4);
     P.c_out_bits = take((size_t)P.nor_max * P.Wout * 4);
-    P.c_in_B = take((size_t)P.n_slots * P.r_pad);
+    P.c_in_B = take((size_t)2 * P.nch_max * P.r_pad);
     P.c_out_B = take((size_t)P.nor_max * P.r_pad);
-    P.c_in_scale = take((size_t)P.n_slots * 4);
-    P.c_in_bs = take((size_t)P.n_slots * 4);
+    P.c_in_scale = take((size_t)2 * P.nch_max * 4);
+    P.c_in_bs = take((size_t)2 * P.nch_max * 4);
     P.c_out_scale = take((size_t)P.nor_max * 4);
     P.c_out_bs = take((size_t)P.nor_max * 4);
     P.c_conv_w = take((size_t)P.nch_max * 16);
     P.c_conv_b = take((size_t)P.nch_max * 4);
-    P.c_e_conv_w = take((size_t)P.nb_max * 16);
-    P.c_e_conv_b = take((size_t)P.nb_max * 4);
-    P.c_e_dtb = take((size_t)P.nb_max * 4);
     P.c_alog = take((size_t)P.nch_max * 4);
     P.c_D = take((size_t)P.nch_max * 4);
     P.c_gnorm = take((size_t)P.nch_max * 4);
     P.c_nnorm = take((size_t)P.nor_max * 4);
-    P.c_as_in = take((size_t)P.r_pad * 4);
-    P.c_as_out = take((size_t)P.r_pad * 4);
     P.chunk_bytes = up32(off, 128);
 
-    P.st_ssm = P.chunk_bytes;
+    off = 0;
+    P.b_eB = take((size_t)P.n_bcdt * P.r_pad);
+    P.b_escale = take((size_t)P.n_bcdt * 4);
+    P.b_ebs = take((size_t)P.n_bcdt * 4);
+    P.b_econv_w = take((size_t)2 * P.gs * 16);
+    P.b_econv_b = take((size_t)2 * P.gs * 4);
+    P.b_dtb = take((size_t)d.nheads * 4);
+    P.b_as_in = take((size_t)P.r_pad * 4);
+    P.b_as_out = take((size_t)P.r_pad * 4);
+    P.blk_bytes = up32(off, 128);
+
+    P.st_blk = P.chunk_bytes;
+    P.st_ssm = P.st_blk + P.blk_bytes;
     P.st_conv = up32(P.st_ssm + (uint32_t)P.nch_max * d.d_state * 4, 128);
-    P.stage_bytes = up32(P.st_conv + (uint32_t)P.nch_max * 16, 128);
+    P.st_econv = up32(P.st_conv + (uint32_t)P.nch_max * 16, 128);
+    P.stage_bytes = up32(P.st_econv + (uint32_t)P.gs * 32, 128);
     if (P.stage_bytes < 4u * d.d_model) P.stage_bytes = up32(4u * d.d_model, 128);      // an LM item holds >= 4 rows
     P.lm_rows_item = (int)(P.stage_bytes / d.d_model);
+
+    // exchange: one (record, mailbox) part list, 32-bit word offsets, every part 128-byte aligned
+    P.M = 37;                                       // mailboxes (tunable: DFSSM_MEGA_M, must divide G)
+    if (const char* e = getenv("DFSSM_MEGA_M")) {
+        const int m = atoi(e);
+        if (m >= 1 && m <= G && G % m == 0) P.M = m;
+    }
+    if (G % P.M) P.M = G;
+    P.gsz = G / P.M;
+    P.u_dpos = (P.nor_max + 1) / 2 * 2;
+    P.u_slot = (P.u_dpos + 2 + 3) / 4 * 4;
+    P.g_dpos = (P.nch_max + 1) / 2 * 2;
+    P.g_slot = (P.g_dpos + 2 + 3) / 4 * 4;
+    if (G * P.u_slot / 4 > 2 * THREADS || G * P.g_slot / 4 > 4 * THREADS) return false;
+    if (P.u_slot + P.g_slot > THREADS) return false;
+    uint32_t xo = 0;
+    auto xtake = [&](size_t words) { xo = up32(xo, 32); const uint32_t at = xo; xo += (uint32_t)words; return at; };
+    P.x_U = xtake((size_t)G * P.u_slot);
+    P.x_A = xtake(P.n_early);
+    P.x_G = xtake((size_t)G * P.g_slot);
+    P.x_T = xtake(P.n_ttask);
+    P.x_words = up32(xo, 32);
 
     // shared memory behind the ring
     uint32_t so = 0;
     auto stake = [&](size_t bytes) { so = up32(so, 16); const uint32_t at = so; so += (uint32_t)bytes; return at; };
     const int kmax = d.d_model > d.d_inner ? d.d_model : d.d_inner;
-    const int nmax = P.nch_max > P.nor_max ? P.nch_max : P.nor_max;
-    const uint32_t x_xq = stake(kmax), x_bc = stake((size_t)P.n_bcdt * 4), x_u = stake((size_t)P.nor_max * 4),
-                   x_z = stake((size_t)P.nch_max * 4), x_x = stake((size_t)P.nch_max * 4), x_tq = stake((size_t)nmax * 4),
-                   x_vin = stake((size_t)P.r_pad * 4), x_vout = stake((size_t)P.r_pad * 4), x_ai = stake((size_t)P.n_slots * 4),
-                   x_ao = stake((size_t)P.nor_max * 4), x_chs = stake((size_t)(G + 1) * 4), x_ors = stake((size_t)(G + 1) * 4),
-                   x_stats = stake((size_t)3 * G * 4), x_red = stake(256), x_mbar = stake(8 * MAX_STAGES);
+    const uint32_t x_xq = stake(kmax), x_bc = stake((size_t)2 * P.gs * 4), x_u = stake((size_t)P.nor_max * 4),
+                   x_z = stake((size_t)P.nch_max * 4), x_x = stake((size_t)P.nch_max * 4), x_dt = stake((size_t)d.nheads * 4),
+                   x_v = stake((size_t)2 * P.r_pad * 8), x_ea = stake((size_t)P.n_bcdt * 4), x_ai = stake((size_t)P.n_slots * 4),
+                   x_ao = stake((size_t)2 * P.nor_max * 4), x_chs = stake((size_t)(G + 1) * 4), x_ors = stake((size_t)(G + 1) * 4),
+                   x_part = stake((size_t)(G + 2) * 8), x_red = stake(256), x_slot = stake((size_t)(P.u_slot + P.g_slot) * 4),
+                   x_mbar = stake(8 * MAX_STAGES);
     const uint32_t fixed = up32(so, 128);
     if (fixed + 2 * (size_t)P.stage_bytes > SMEM_LIMIT) return false;
     int stages = (int)((SMEM_LIMIT - fixed) / P.stage_bytes);
@@ -83,26 +117,26 @@ inline bool plan(const Dims& d, int G, Params& P)
     P.stages = stages;
     const uint32_t ring = (uint32_t)stages * P.stage_bytes;
     P.s_ring = 0;
-    P.s_xq = ring + x_xq; P.s_bc = ring + x_bc; P.s_u = ring + x_u; P.s_z = ring + x_z; P.s_x = ring + x_x;
-    P.s_tq = ring + x_tq; P.s_vin = ring + x_vin; P.s_vout = ring + x_vout; P.s_acc_in = ring + x_ai;
-    P.s_acc_out = ring + x_ao; P.s_chs = ring + x_chs; P.s_ors = ring + x_ors; P.s_stats = ring + x_stats;
-    P.s_red = ring + x_red; P.s_mbar = ring + x_mbar;
+    P.s_xq = ring + x_xq; P.s_bc = ring + x_bc; P.s_u = ring + x_u; P.s_z = ring + x_z; P.s_x = ring + x_x; P.s_dt = ring + x_dt;
+    P.s_v = ring + x_v; P.s_eacc = ring + x_ea; P.s_acc_in = ring + x_ai; P.s_acc_out = ring + x_ao;
+    P.s_chs = ring + x_chs; P.s_ors = ring + x_ors; P.s_part = ring + x_part; P.s_red = ring + x_red; P.s_slot = ring + x_slot; P.s_mbar = ring + x_mbar;
     P.smem_bytes = ring + fixed;
     return true;
 }
 
 // arena regions of the mega path (byte sizes)
 struct Regions {
-    size_t chunks, A_in, A_out, xbuf, am;
+    size_t chunks, blocks, A_in, A_out, xbuf, am;
 };
 inline Regions regions(const Params& P)
 {
     Regions r;
-    r.chunks = (size_t)(P.L > 0 ? P.L : 1) * P.G * P.chunk_bytes;
-    r.A_in = (size_t)(P.L > 0 ? P.L : 1) * P.r * P.d_model;
-    r.A_out = (size_t)(P.L > 0 ? P.L : 1) * P.r * P.d_inner;
-    // exchange words: stats x2 (3G each), codes (G*wpc1, G*wpc3), t x2 (64 each), bc (n_bcdt)
-    r.xbuf = 8 * ((size_t)6 * P.G + (size_t)P.G * (P.wpc1 + P.wpc3) + 128 + P.n_bcdt + 64);
+    const size_t nl = (size_t)(P.L > 0 ? P.L : 1);
+    r.chunks = nl * P.G * P.chunk_bytes;
+    r.blocks = nl * P.blk_bytes;
+    r.A_in = nl * P.r * P.d_model;
+    r.A_out = nl * P.r * P.d_inner;
+    r.xbuf = (size_t)4 * P.M * P.x_words * 4;       // four rotating records of M mailboxes
     r.am = (size_t)P.G * 8 + 64;
     return r;
 }
@@ -168,15 +202,8 @@ inline void pack_chunk(const Params& P, const HostLayer& H, const float* next_no
         ((float*)(out + P.c_D))[i] = H.D[h];
         ((float*)(out + P.c_gnorm))[i] = H.gnorm_w[ch];
     }
-    for (int k = 0, e = c; e < P.n_bcdt; ++k, e += G) {      // early rows: B | C | dt
-        put_in_row(2 * P.nch_max + k, 2 * P.d_inner + e);
-        if (e < 2 * P.gs) {
-            memcpy(out + P.c_e_conv_w + 16 * (size_t)k, H.conv_w + 4 * (size_t)(P.d_inner + e), 16);
-            ((float*)(out + P.c_e_conv_b))[k] = H.conv_b[P.d_inner + e];
-        } else {
-            ((float*)(out + P.c_e_dtb))[k] = H.dt_bias[e - 2 * P.gs];
-        }
-    }
+    for (int k = 0, e = c; e < P.n_bcdt; ++k, e += G)        // early sign rows: B | C | dt (their epilogue data is in the block)
+        memcpy(out + P.c_in_bits + (size_t)(2 * P.nch_max + k) * P.Win * 4, H.in_sign + (size_t)(2 * P.d_inner + e) * P.Win, (size_t)P.Win * 4);
     for (int i = 0; i < nor; ++i) {
         const int row = or0 + i;
         memcpy(out + P.c_out_bits + (size_t)i * P.Wout * 4, H.out_sign + (size_t)row * P.Wout, (size_t)P.Wout * 4);
@@ -185,9 +212,27 @@ inline void pack_chunk(const Params& P, const HostLayer& H, const float* next_no
         ((float*)(out + P.c_out_bs))[i] = H.out_b_s[row];
         ((float*)(out + P.c_nnorm))[i] = next_norm_w[row];
     }
+}
+
+// block of a layer: what every CTA needs to finish the B | C | dt rows itself
+inline void pack_block(const Params& P, const HostLayer& H, uint8_t* out)
+{
+    memset(out, 0, P.blk_bytes);
+    for (int e = 0; e < P.n_bcdt; ++e) {
+        const int row = 2 * P.d_inner + e;
+        memcpy(out + P.b_eB + (size_t)e * P.r_pad, H.in_B + (size_t)row * P.r, P.r);
+        ((float*)(out + P.b_escale))[e] = half_bits_to_float(H.in_row_scale[row]);
+        ((float*)(out + P.b_ebs))[e] = H.in_b_s[row];
+        if (e < 2 * P.gs) {
+            memcpy(out + P.b_econv_w + 16 * (size_t)e, H.conv_w + 4 * (size_t)(P.d_inner + e), 16);
+            ((float*)(out + P.b_econv_b))[e] = H.conv_b[P.d_inner + e];
+        } else {
+            ((float*)(out + P.b_dtb))[e - 2 * P.gs] = H.dt_bias[e - 2 * P.gs];
+        }
+    }
     for (int j = 0; j < P.r; ++j) {
-        ((float*)(out + P.c_as_in))[j] = H.in_a_s[j];
-        ((float*)(out + P.c_as_out))[j] = H.out_a_s[j];
+        ((float*)(out + P.b_as_in))[j] = H.in_a_s[j];
+        ((float*)(out + P.b_as_out))[j] = H.out_a_s[j];
     }
 }
 
