@@ -48,6 +48,7 @@ struct dfssm_ctx {
     std::vector<GraphEntry> graphs;
     int last_batch;
     mega::Params mp;           // layout + pointers of the mega path (batch 1)
+    mega::KernelFn mega_fn;    // the instantiation of the persistent kernel that serves this shape
     bool mega_ok;              // the device can co-schedule the mega grid and the shape fits
     uint64_t epoch;            // steps taken by the mega path: makes every exchange flag unique
     int32_t* pinned_tok;       // page-locked staging for dfssm_step_host
@@ -386,8 +387,9 @@ int mega_setup(dfssm_ctx* ctx)                      // at create: can this devic
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
     if (!coop || sms < mega::GRID) return DFSSM_OK;
-    CK(cudaFuncSetAttribute(mega::k_mega, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->mp.smem_bytes));
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mega::k_mega, mega::THREADS, ctx->mp.smem_bytes));
+    ctx->mega_fn = mega::pick_kernel(ctx->dm, (ctx->cfg.flags & DFSSM_FLAG_TAPS) != 0);
+    CK(cudaFuncSetAttribute((const void*)ctx->mega_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->mp.smem_bytes));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)ctx->mega_fn, mega::THREADS, ctx->mp.smem_bytes));
     if (per_sm < 1) return DFSSM_OK;
     ctx->mega_ok = true;
     return DFSSM_OK;
@@ -466,7 +468,7 @@ int mega_launch(dfssm_ctx* ctx)
     ctx->epoch += 1;
     P.rec0 = (uint32_t)(((ctx->epoch - 1) * (uint64_t)P.L) & 3u);      // global layer counter mod 4
     void* args[] = { &P };
-    CK(cudaLaunchCooperativeKernel((const void*)mega::k_mega, dim3(P.G), dim3(mega::THREADS), args, P.smem_bytes, ctx->stream));
+    CK(cudaLaunchCooperativeKernel((const void*)ctx->mega_fn, dim3(P.G), dim3(mega::THREADS), args, P.smem_bytes, ctx->stream));
     return DFSSM_OK;
 }
 

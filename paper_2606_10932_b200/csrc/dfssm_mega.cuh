@@ -169,11 +169,44 @@ __device__ __forceinline__ int plane_pos(int k, int K)
     return (i < 4 ? 0 : (K >> 1)) + 16 * w + 4 * (i & 3) + j;
 }
 
+// Shape of the model as the kernel sees it: compile-time constants for the shapes of BASELINE.json's configs (every
+// index computation, division and loop bound folds), or the run-time values of Params (any other shape).
+struct ShapeRT { static constexpr bool kStatic = false; static constexpr int d_model = 0, d_inner = 0, headdim = 0, d_state = 0, ngroups = 0, r = 0; };
+template <int DM, int DI, int HD, int DS, int NG, int R>
+struct ShapeCT { static constexpr bool kStatic = true; static constexpr int d_model = DM, d_inner = DI, headdim = HD, d_state = DS, ngroups = NG, r = R; };
+
+constexpr int GRID = 148;                       // one CTA per B200 SM
+constexpr int MBOX = 37;                        // mailboxes of the exchange (4 CTAs poll each)
+
+template <class S>
 struct Ctx {
     const Params& P;
     uint8_t* sm;
     int tid, lane, wid, c;
     volatile int* dead;          // shared flag: a poll timed out -> stop spinning everywhere
+#define DFSSM_DIM(n_) __device__ __forceinline__ int n_() const { return S::kStatic ? S::n_ : P.n_; }
+    DFSSM_DIM(d_model) DFSSM_DIM(d_inner) DFSSM_DIM(headdim) DFSSM_DIM(d_state) DFSSM_DIM(ngroups) DFSSM_DIM(r)
+#undef DFSSM_DIM
+    __device__ __forceinline__ constexpr int G() const { return GRID; }
+    __device__ __forceinline__ constexpr int M() const { return MBOX; }
+    __device__ __forceinline__ constexpr int gsz() const { return GRID / MBOX; }
+    __device__ __forceinline__ int nheads() const { return d_inner() / headdim(); }
+    __device__ __forceinline__ int gs() const { return ngroups() * d_state(); }
+    __device__ __forceinline__ int n_bcdt() const { return 2 * gs() + nheads(); }
+    __device__ __forceinline__ int nch_max() const { return (d_inner() + GRID - 1) / GRID; }
+    __device__ __forceinline__ int nor_max() const { return (d_model() + GRID - 1) / GRID; }
+    __device__ __forceinline__ int nb_max() const { return (n_bcdt() + GRID - 1) / GRID; }
+    __device__ __forceinline__ int n_slots() const { return 2 * nch_max() + nb_max(); }
+    __device__ __forceinline__ int r_pad() const { return (r() + 3) / 4 * 4; }
+    __device__ __forceinline__ int Win() const { return d_model() / 32; }
+    __device__ __forceinline__ int Wout() const { return d_inner() / 32; }
+    __device__ __forceinline__ int n_early() const { return n_bcdt() + r(); }
+    __device__ __forceinline__ int tsplit() const { return (d_inner() % 64 == 0 && 4 * r() <= GRID) ? 4 : (2 * r() <= GRID ? 2 : 1); }
+    __device__ __forceinline__ int n_ttask() const { return r() * tsplit(); }
+    __device__ __forceinline__ int u_dpos() const { return (nor_max() + 1) / 2 * 2; }
+    __device__ __forceinline__ int u_slot() const { return (u_dpos() + 2 + 3) / 4 * 4; }
+    __device__ __forceinline__ int g_dpos() const { return (nch_max() + 1) / 2 * 2; }
+    __device__ __forceinline__ int g_slot() const { return (g_dpos() + 2 + 3) / 4 * 4; }
 };
 
 __device__ __forceinline__ unsigned long long globaltimer_ns()
@@ -188,7 +221,8 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
         if (P.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + (l_)) * PROF_NPH + (k_)] = clock64();  \
     } while (0)
 
-__device__ __forceinline__ void poll_fail(const Ctx& x)
+template <class S>
+__device__ __forceinline__ void poll_fail(const Ctx<S>& x)
 {
     *x.dead = 1;
     atomicExch(x.P.err, 2);
@@ -201,8 +235,8 @@ __device__ __forceinline__ void poll_fail(const Ctx& x)
 // behind nw count as valid.  If slot_w > 0 the buffer is a sequence of slots of slot_w words whose word dpos is
 // the low half of an fp64 (any bit pattern: exempt; its high half at dpos + 1 validates it).
 // Spins until every owned word has been written; the raw words come back in v[].
-template <int NJ>
-__device__ __forceinline__ void hop_gather(const Ctx& x, const uint32_t* buf, int nw, int slot_w, int dpos, uint4 (&v)[NJ])
+template <int NJ, class S>
+__device__ __forceinline__ void hop_gather(const Ctx<S>& x, const uint32_t* buf, int nw, int slot_w, int dpos, uint4 (&v)[NJ])
 {
     const int nchunk = (nw + 3) >> 2;
     bool need[NJ];
@@ -239,17 +273,20 @@ __device__ __forceinline__ void quant_consts(double ss, float amax, int d, float
 }
 
 // scratch inside s_red: [0,16) floats warp maxima | [16,32) ints warp code sums | doubles [8,24) warp sums (byte 64..)
-__device__ __forceinline__ float* red_f(const Ctx& x) { return (float*)(x.sm + x.P.s_red); }
-__device__ __forceinline__ int* red_i(const Ctx& x) { return (int*)(x.sm + x.P.s_red) + NWARPS; }
-__device__ __forceinline__ double* red_d(const Ctx& x) { return (double*)(x.sm + x.P.s_red + 8 * NWARPS); }
+template <class S>
+__device__ __forceinline__ float* red_f(const Ctx<S>& x) { return (float*)(x.sm + x.P.s_red); }
+template <class S>
+__device__ __forceinline__ int* red_i(const Ctx<S>& x) { return (int*)(x.sm + x.P.s_red) + NWARPS; }
+template <class S>
+__device__ __forceinline__ double* red_d(const Ctx<S>& x) { return (double*)(x.sm + x.P.s_red + 8 * NWARPS); }
 
 // S1 / S6 / S8 norm + quantise of a whole vector in every CTA.  `en(f)` calls f(k, bits) for every element this
 // thread holds: bits = fp32 t_k = value_k * w_k.  The caller has stored the partial sums of squares (one per
 // CTA, or per warp for the embedding) into part[0..G) (zeros where unused).  Every CTA derives the same
 // rstd / amax / codes.  Writes the codes to xq (plane order unless `canonical`), returns the sum of the codes
 // and the activation scale s.  Two __syncthreads.
-template <typename Enum>
-__device__ __forceinline__ int norm_quant(const Ctx& x, Enum en, int K, bool canonical, float& s_out, int8_t* tap_codes)
+template <class S, typename Enum>
+__device__ __forceinline__ int norm_quant(const Ctx<S>& x, Enum en, int K, bool canonical, float& s_out, int8_t* tap_codes)
 {
     const Params& P = x.P;
     uint8_t* xq = x.sm + P.s_xq;
@@ -263,7 +300,7 @@ __device__ __forceinline__ int norm_quant(const Ctx& x, Enum en, int K, bool can
     float amax = x.lane < NWARPS ? red_f(x)[x.lane] : 0.0f;
     amax = warp_max(amax);
     double ss = 0.0;
-    for (int g = x.lane; g < P.G; g += 32) ss += part[g];
+    for (int g = x.lane; g < x.G(); g += 32) ss += part[g];
     ss = warp_sum(ss);
     float inv;
     quant_consts(ss, amax, K, P.eps, inv, s_out);
@@ -306,8 +343,8 @@ struct SlotEnum {
     }
 };
 // store the fp64 partials found in the gathered chunks into part[slot]
-template <int NJ>
-__device__ __forceinline__ void slot_partials(const Ctx& x, const uint4 (&v)[NJ], int nslots, int slot_w, int dpos)
+template <int NJ, class S>
+__device__ __forceinline__ void slot_partials(const Ctx<S>& x, const uint4 (&v)[NJ], int nslots, int slot_w, int dpos)
 {
     double* part = (double*)(x.sm + x.P.s_part);
     const int pps = slot_w >> 2;
@@ -323,7 +360,8 @@ __device__ __forceinline__ void slot_partials(const Ctx& x, const uint4 (&v)[NJ]
 }
 
 // block-wide sum of doubles held by some lanes (others pass 0); result valid in thread 0 only.  One __syncthreads.
-__device__ __forceinline__ double block_sum_t0(const Ctx& x, double s)
+template <class S>
+__device__ __forceinline__ double block_sum_t0(const Ctx<S>& x, double s)
 {
     s = warp_sum(s);
     if (x.lane == 0) red_d(x)[x.wid] = s;
@@ -444,7 +482,8 @@ __device__ __forceinline__ int trow_dot(const int8_t* row, int nbytes, const uin
 // weight / state pipeline
 // ------------------------------------------------------------------------------------------------
 // issue the bulk copies of pipeline item `item` into its ring stage (one thread)
-__device__ __forceinline__ void issue_item(const Ctx& x, int item, int v0, int v1)
+template <class S>
+__device__ __forceinline__ void issue_item(const Ctx<S>& x, int item, int v0, int v1)
 {
     const Params& P = x.P;
     const int st = item % P.stages;
@@ -453,25 +492,26 @@ __device__ __forceinline__ void issue_item(const Ctx& x, int item, int v0, int v
     if (item < P.L) {
         const int* chs = (const int*)(x.sm + P.s_chs);
         const int ch0 = chs[x.c], nch = chs[x.c + 1] - ch0;
-        const uint32_t ssm_b = (uint32_t)nch * P.d_state * 4, conv_b = (uint32_t)nch * 16, econv_b = (uint32_t)P.gs * 32;
+        const uint32_t ssm_b = (uint32_t)nch * x.d_state() * 4, conv_b = (uint32_t)nch * 16, econv_b = (uint32_t)x.gs() * 32;
         mbar_expect_tx(bar, P.chunk_bytes + P.blk_bytes + ssm_b + conv_b + econv_b);
-        bulk_g2s(stage, P.chunks + ((size_t)item * P.G + x.c) * P.chunk_bytes, P.chunk_bytes, bar);
+        bulk_g2s(stage, P.chunks + ((size_t)item * x.G() + x.c) * P.chunk_bytes, P.chunk_bytes, bar);
         bulk_g2s(stage + P.st_blk, P.blocks + (size_t)item * P.blk_bytes, P.blk_bytes, bar);
-        bulk_g2s(stage + P.st_econv, P.conv + (size_t)item * P.conv_lstride + (size_t)P.d_inner * 4, econv_b, bar);
+        bulk_g2s(stage + P.st_econv, P.conv + (size_t)item * P.conv_lstride + (size_t)x.d_inner() * 4, econv_b, bar);
         if (nch > 0) {
-            bulk_g2s(stage + P.st_ssm, P.ssm + (size_t)item * P.ssm_lstride + (size_t)ch0 * P.d_state, ssm_b, bar);
+            bulk_g2s(stage + P.st_ssm, P.ssm + (size_t)item * P.ssm_lstride + (size_t)ch0 * x.d_state(), ssm_b, bar);
             bulk_g2s(stage + P.st_conv, P.conv + (size_t)item * P.conv_lstride + (size_t)ch0 * 4, conv_b, bar);
         }
     } else {
         const int row0 = v0 + (item - P.L) * P.lm_rows_item;
         const int nrows = min(P.lm_rows_item, v1 - row0);
-        const uint32_t bytes = (uint32_t)nrows * P.d_model;
+        const uint32_t bytes = (uint32_t)nrows * x.d_model();
         mbar_expect_tx(bar, bytes);
-        bulk_g2s(stage, P.emb + (size_t)row0 * P.d_model, bytes, bar);
+        bulk_g2s(stage, P.emb + (size_t)row0 * x.d_model(), bytes, bar);
     }
 }
 
-__device__ __forceinline__ void wait_item(const Ctx& x, int item)
+template <class S>
+__device__ __forceinline__ void wait_item(const Ctx<S>& x, int item)
 {
     const int st = item % x.P.stages;
     uint64_t* bar = (uint64_t*)(x.sm + x.P.s_mbar) + st;
@@ -485,29 +525,31 @@ __device__ __forceinline__ void wait_item(const Ctx& x, int item)
 // The stores of one CTA into the M mailboxes of a record.  publish and reset use the SAME thread -> address map, so
 // a reset and the later publish of a word are ordered by program order of one thread.
 //   slot (U / G): thread t < M * pps writes 16-byte piece t % pps of its slot in mailbox t / pps
-template <typename F>
-__device__ __forceinline__ void slot_store(const Ctx& x, uint32_t* rec, uint32_t part_off, int slot_w, F piece_value)
+template <class S, typename F>
+__device__ __forceinline__ void slot_store(const Ctx<S>& x, uint32_t* rec, uint32_t part_off, int slot_w, F piece_value)
 {
     const Params& P = x.P;
     const int pps = slot_w >> 2;
-    for (int t = x.tid; t < P.M * pps; t += THREADS) {
+    for (int t = x.tid; t < x.M() * pps; t += THREADS) {
         const int m = t / pps, piece = t - m * pps;
         x_st128(rec + (size_t)m * P.x_words + part_off + (size_t)x.c * slot_w + 4 * piece, piece_value(piece));
     }
 }
 //   word (A / T): the lanes of one warp write the word to all mailboxes
-__device__ __forceinline__ void word_store(const Ctx& x, uint32_t* rec, uint32_t part_off, int idx, uint32_t value)
+template <class S>
+__device__ __forceinline__ void word_store(const Ctx<S>& x, uint32_t* rec, uint32_t part_off, int idx, uint32_t value)
 {
     const Params& P = x.P;
-    for (int m = x.lane; m < P.M; m += 32) x_st32(rec + (size_t)m * P.x_words + part_off + idx, value);
+    for (int m = x.lane; m < x.M(); m += 32) x_st32(rec + (size_t)m * P.x_words + part_off + idx, value);
 }
 
+template <class S, bool TAPS>
 __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
 {
     extern __shared__ __align__(128) uint8_t sm[];
     __shared__ int s_dead;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, c = blockIdx.x;
-    Ctx x{ P, sm, tid, lane, wid, c, &s_dead };
+    Ctx<S> x{ P, sm, tid, lane, wid, c, &s_dead };
 
     int* chs = (int*)(sm + P.s_chs);
     int* ors = (int*)(sm + P.s_ors);
@@ -519,16 +561,16 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
     float* s_x = (float*)(sm + P.s_x);
     float* s_dt = (float*)(sm + P.s_dt);
     double* s_vin = (double*)(sm + P.s_v);
-    double* s_vout = s_vin + P.r_pad;
+    double* s_vout = s_vin + x.r_pad();
     int* s_eacc = (int*)(sm + P.s_eacc);
     int* s_acc_in = (int*)(sm + P.s_acc_in);
     int* s_acc_out = (int*)(sm + P.s_acc_out);
 
-    for (int g = tid; g <= P.G; g += THREADS) {
-        chs[g] = (int)(((long long)g * P.d_inner) / P.G);
-        ors[g] = (int)(((long long)g * P.d_model) / P.G);
+    for (int g = tid; g <= x.G(); g += THREADS) {
+        chs[g] = (int)(((long long)g * x.d_inner()) / x.G());
+        ors[g] = (int)(((long long)g * x.d_model()) / x.G());
     }
-    if (tid < 2 * P.r_pad) s_vin[tid] = 0.0;
+    if (tid < 2 * x.r_pad()) s_vin[tid] = 0.0;
     if (tid == 0) {
         s_dead = 0;
         for (int s = 0; s < P.stages; ++s) mbar_init(mbar + s, 1);
@@ -537,29 +579,29 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
     __syncthreads();
     const int ch0 = chs[c], nch = chs[c + 1] - ch0;
     const int or0 = ors[c], nor = ors[c + 1] - or0;
-    const int v0 = (int)(((long long)c * P.vocab) / P.G), v1 = (int)(((long long)(c + 1) * P.vocab) / P.G);
+    const int v0 = (int)(((long long)c * P.vocab) / x.G()), v1 = (int)(((long long)(c + 1) * P.vocab) / x.G());
     const int n_lm_items = (v1 - v0 + P.lm_rows_item - 1) / P.lm_rows_item;
     const int n_items = P.L + n_lm_items;
     if (tid == 0)
         for (int it = 0; it < P.stages && it < n_items; ++it) issue_item(x, it, v0, v1);
 
     const int ps = P.pos[0] & 3;                     // conv ring slot this step writes
-    const int nb_tasks = c < P.n_early ? (P.n_early - c + P.G - 1) / P.G : 0;      // early tasks of this CTA
-    const int h0 = nch > 0 ? ch0 / P.headdim : 0, h1 = nch > 0 ? (ch0 + nch - 1) / P.headdim : -1;
-    const bool taps_on = P.taps != nullptr;
-    const size_t rec_words = (size_t)P.M * P.x_words;
-    const int mbox = c / P.gsz;                      // the mailbox this CTA polls
+    const int nb_tasks = c < x.n_early() ? (x.n_early() - c + x.G() - 1) / x.G() : 0;      // early tasks of this CTA
+    const int h0 = nch > 0 ? ch0 / x.headdim() : 0, h1 = nch > 0 ? (ch0 + nch - 1) / x.headdim() : -1;
+    const bool taps_on = TAPS && P.taps != nullptr;
+    const size_t rec_words = (size_t)x.M() * P.x_words;
+    const int mbox = c / x.gsz();                      // the mailbox this CTA polls
     uint32_t* s_slotU = (uint32_t*)(sm + P.s_slot);
-    uint32_t* s_slotG = s_slotU + P.u_slot;
-    if (tid < P.u_slot + P.g_slot) s_slotU[tid] = 0u;      // pad words of the slots are published as 0
-    const int KS = P.Wout >= 64 ? 2 : 1;             // K-split of the out_proj sign rows
-    const int tbytes = P.d_inner / P.tsplit;         // bytes of one out_proj LoRA-down partial task
+    uint32_t* s_slotG = s_slotU + x.u_slot();
+    if (tid < x.u_slot() + x.g_slot()) s_slotU[tid] = 0u;      // pad words of the slots are published as 0
+    const int KS = x.Wout() >= 64 ? 2 : 1;             // K-split of the out_proj sign rows
+    const int tbytes = x.d_inner() / x.tsplit();         // bytes of one out_proj LoRA-down partial task
 
     // warp k takes early task k (e = c + k G); if that is a LoRA-down row it fetches the row a phase ahead
-    const int e_first = c + wid * P.G;
-    const bool t_first = wid < nb_tasks && e_first >= P.n_bcdt;
+    const int e_first = c + wid * x.G();
+    const bool t_first = wid < nb_tasks && e_first >= x.n_bcdt();
     int4 pre_in[T_PRE];
-    if (t_first && P.L > 0) trow_prefetch(P.A_in + (size_t)(e_first - P.n_bcdt) * P.d_model, P.d_model, lane, pre_in);
+    if (t_first && P.L > 0) trow_prefetch(P.A_in + (size_t)(e_first - x.n_bcdt()) * x.d_model(), x.d_model(), lane, pre_in);
 
     // ---------------- S0 embedding + the first norm/quantise, redundantly in every CTA ----------------
     float s_act;                                     // scale of the current activation codes
@@ -570,14 +612,14 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             if (tid == 0 && c == 0) atomicOr(P.err, 1);
             tok = tok < 0 ? 0 : P.vocab - 1;
         }
-        const int8_t* erow = P.emb + (size_t)tok * P.d_model;
+        const int8_t* erow = P.emb + (size_t)tok * x.d_model();
         const float es = P.emb_s[tok];
         uint4 v[4];
         double ss = 0.0;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const int k0 = 4 * (tid + j * THREADS);
-            if (k0 < P.d_model) {
+            if (k0 < x.d_model()) {
                 uint32_t w[4];
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
@@ -592,7 +634,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         // the per-CTA partial sums of the exchange are replaced by the per-warp partial sums of this CTA
         double* part = (double*)(sm + P.s_part);
         ss = warp_sum(ss);
-        for (int g = tid; g < P.G; g += THREADS)
+        for (int g = tid; g < x.G(); g += THREADS)
             if (g >= NWARPS) part[g] = 0.0;
         if (lane == 0) part[wid] = ss;
         uint8_t* tp0 = (taps_on && c == 0 && P.L > 0) ? P.taps : nullptr;
@@ -600,10 +642,10 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const int k0 = 4 * (tid + j * THREADS);
-                if (k0 < P.d_model) { f(k0, v[j].x); f(k0 + 1, v[j].y); f(k0 + 2, v[j].z); f(k0 + 3, v[j].w); }
+                if (k0 < x.d_model()) { f(k0, v[j].x); f(k0 + 1, v[j].y); f(k0 + 2, v[j].z); f(k0 + 3, v[j].w); }
             }
         };
-        qsum = norm_quant(x, en, P.d_model, P.L == 0, s_act, tp0 ? (int8_t*)(tp0 + P.tl.off[0]) : nullptr);
+        qsum = norm_quant(x, en, x.d_model(), P.L == 0, s_act, tp0 ? (int8_t*)(tp0 + P.tl.off[0]) : nullptr);
         if (tp0 && tid == 0) *(float*)(tp0 + P.tl.off[1]) = s_act;
     }
 
@@ -619,11 +661,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         DFSSM_STAMP(l, 0);
         if (P.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + 15] = globaltimer_ns();
         {   // reset own slots of the record two layers ahead (same thread -> address map as the publishes below)
-            slot_store(x, recc, P.x_U, P.u_slot, [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
-            slot_store(x, recc, P.x_G, P.g_slot, [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
-            for (int k = wid; k < nb_tasks; k += NWARPS) word_store(x, recc, P.x_A, c + k * P.G, SENT);
+            slot_store(x, recc, P.x_U, x.u_slot(), [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
+            slot_store(x, recc, P.x_G, x.g_slot(), [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
+            for (int k = wid; k < nb_tasks; k += NWARPS) word_store(x, recc, P.x_A, c + k * x.G(), SENT);
             if (wid == 0)
-                for (int e = c; e < P.n_ttask; e += P.G) word_store(x, recc, P.x_T, e, SENT);
+                for (int e = c; e < x.n_ttask(); e += x.G()) word_store(x, recc, P.x_T, e, SENT);
         }
 
         wait_item(x, l);
@@ -632,20 +674,20 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         {
             const uint32_t* bits = (const uint32_t*)(stage + P.c_in_bits);
             for (int k = wid; k < nb_tasks; k += NWARPS) {
-                const int e = c + k * P.G;
+                const int e = c + k * x.G();
                 int val;
-                if (e < P.n_bcdt) {
-                    const uint32_t* const rowp[1] = { bits + (size_t)(2 * P.nch_max + k) * P.Win };
+                if (e < x.n_bcdt()) {
+                    const uint32_t* const rowp[1] = { bits + (size_t)(2 * x.nch_max() + k) * x.Win() };
                     int p[1];
-                    sign_partial<1>(rowp, 1, 0, P.Win, xq, P.d_model, lane, p);
+                    sign_partial<1>(rowp, 1, 0, x.Win(), xq, x.d_model(), lane, p);
                     val = 2 * (warp_sum_i(p[0]) / 128) - qsum;       // exact: every term is a multiple of 128
                 } else {
-                    const int8_t* arow = P.A_in + ((size_t)l * P.r + (e - P.n_bcdt)) * P.d_model;
-                    if (k != wid) trow_prefetch(arow, P.d_model, lane, pre_in);
-                    val = trow_dot(arow, P.d_model, xq, lane, pre_in);
+                    const int8_t* arow = P.A_in + ((size_t)l * x.r() + (e - x.n_bcdt())) * x.d_model();
+                    if (k != wid) trow_prefetch(arow, x.d_model(), lane, pre_in);
+                    val = trow_dot(arow, x.d_model(), xq, lane, pre_in);
                 }
                 word_store(x, rec, P.x_A, e, (uint32_t)val ^ IBIAS);
-                if (lane == 0 && tp && e >= P.n_bcdt) ((int32_t*)(tp + P.tl.off[3]))[e - P.n_bcdt] = val;
+                if (lane == 0 && tp && e >= x.n_bcdt()) ((int32_t*)(tp + P.tl.off[3]))[e - x.n_bcdt()] = val;
             }
         }
         // ---- S2: z and x sign rows of this CTA, 4 rows per warp pass, dealt from the top warp down ----
@@ -659,11 +701,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
 #pragma unroll
                 for (int r = 0; r < 4; ++r) {
                     const int t = 4 * q + r;
-                    slot[r] = r < nrows ? (t < nch ? t : P.nch_max + (t - nch)) : 0;
-                    rowp[r] = bits + (size_t)slot[r] * P.Win;
+                    slot[r] = r < nrows ? (t < nch ? t : x.nch_max() + (t - nch)) : 0;
+                    rowp[r] = bits + (size_t)slot[r] * x.Win();
                 }
                 int p[4];
-                sign_partial<4>(rowp, nrows, 0, P.Win, xq, P.d_model, lane, p);
+                sign_partial<4>(rowp, nrows, 0, x.Win(), xq, x.d_model(), lane, p);
                 const int v = reduce4(p, lane);
                 const int r = lane >> 3;
                 if ((lane & 7) == 0 && r < nrows) s_acc_in[slot[r]] = 2 * (v / 128) - qsum;
@@ -673,7 +715,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         // ---- gather A: accumulators of all B|C|dt rows and t_in;  v_j = a_s[j] * float(t_j) ----
         {
             uint4 va[2];
-            hop_gather<2>(x, mine + P.x_A, P.n_early, 0, 0, va);
+            hop_gather<2>(x, mine + P.x_A, x.n_early(), 0, 0, va);
             const float* a_s = (const float*)(blk + P.b_as_in);
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
@@ -682,10 +724,10 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
 #pragma unroll
                 for (int i = 0; i < 4; ++i) {
                     const int e = e0 + i;
-                    if (e < P.n_early) {
+                    if (e < x.n_early()) {
                         const int val = (int)(w[i] ^ IBIAS);
-                        if (e < P.n_bcdt) s_eacc[e] = val;
-                        else s_vin[e - P.n_bcdt] = (double)fmul(a_s[e - P.n_bcdt], (float)val);
+                        if (e < x.n_bcdt()) s_eacc[e] = val;
+                        else s_vin[e - x.n_bcdt()] = (double)fmul(a_s[e - x.n_bcdt()], (float)val);
                     }
                 }
             }
@@ -694,24 +736,24 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         DFSSM_STAMP(l, 3);
         // ---- S3 stage 2 + S4 conv + dt softplus: one thread per row; own z|x rows and ALL B|C rows (+ own dt) ----
         {
-            const int n_dt = tp ? P.nheads : (h1 - h0 + 1);
-            const int n_rows = 2 * nch + 2 * P.gs + n_dt;
+            const int n_dt = tp ? x.nheads() : (h1 - h0 + 1);
+            const int n_rows = 2 * nch + 2 * x.gs() + n_dt;
             float* ring = (float*)(stage + P.st_conv);
             const float* ering = (const float*)(stage + P.st_econv);
             for (int i = tid; i < n_rows; i += THREADS) {
                 int kind, slot = 0, e = 0;         // kind 0 z, 1 x, 2 B|C, 3 dt
                 if (i < nch) { kind = 0; slot = i; }
-                else if (i < 2 * nch) { kind = 1; slot = P.nch_max + (i - nch); }
-                else if (i < 2 * nch + 2 * P.gs) { kind = 2; e = i - 2 * nch; }
-                else { kind = 3; e = 2 * P.gs + (tp ? 0 : h0) + (i - 2 * nch - 2 * P.gs); }
+                else if (i < 2 * nch) { kind = 1; slot = x.nch_max() + (i - nch); }
+                else if (i < 2 * nch + 2 * x.gs()) { kind = 2; e = i - 2 * nch; }
+                else { kind = 3; e = 2 * x.gs() + (tp ? 0 : h0) + (i - 2 * nch - 2 * x.gs()); }
                 const bool own = kind < 2;
-                const int8_t* brow = own ? (const int8_t*)(stage + P.c_in_B) + (size_t)slot * P.r_pad
-                                         : (const int8_t*)(blk + P.b_eB) + (size_t)e * P.r_pad;
+                const int8_t* brow = own ? (const int8_t*)(stage + P.c_in_B) + (size_t)slot * x.r_pad()
+                                         : (const int8_t*)(blk + P.b_eB) + (size_t)e * x.r_pad();
                 const float scale = own ? ((const float*)(stage + P.c_in_scale))[slot] : ((const float*)(blk + P.b_escale))[e];
                 const float bsv = own ? ((const float*)(stage + P.c_in_bs))[slot] : ((const float*)(blk + P.b_ebs))[e];
                 const int acc = own ? s_acc_in[slot] : s_eacc[e];
                 double lo0 = 0.0, lo1 = 0.0;
-                for (int j4 = 0; j4 < P.r_pad; j4 += 4) {         // pad entries of B are 0, pad entries of v are 0
+                for (int j4 = 0; j4 < x.r_pad(); j4 += 4) {         // pad entries of B are 0, pad entries of v are 0
                     const int w = *(const int*)(brow + j4);
                     lo0 = __fma_rn((double)((int)((unsigned)w << 24) >> 24), s_vin[j4], lo0);
                     lo1 = __fma_rn((double)((int)((unsigned)w << 16) >> 24), s_vin[j4 + 1], lo1);
@@ -735,7 +777,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     rg[ps] = val;
                     const float cv = siluf(o);
                     s_x[ic] = cv;
-                    row = P.d_inner + ch0 + ic;
+                    row = x.d_inner() + ch0 + ic;
                     if (tp) ((float*)(tp + P.tl.off[5]))[ch0 + ic] = cv;
                 } else if (kind == 2) {
                     const float* rg = ering + 4 * e;
@@ -743,18 +785,18 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     const float4 cw = *(const float4*)(blk + P.b_econv_w + 16 * e);
                     float o = ((const float*)(blk + P.b_econv_b))[e];
                     o = ffma(cw.x, s0, o); o = ffma(cw.y, s1, o); o = ffma(cw.z, s2, o); o = ffma(cw.w, val, o);
-                    tap_owner = e % P.G == c;
-                    if (tap_owner) conv_l[4 * (size_t)(P.d_inner + e) + ps] = val;      // the early-task owner keeps the state
+                    tap_owner = e % x.G() == c;
+                    if (tap_owner) conv_l[4 * (size_t)(x.d_inner() + e) + ps] = val;      // the early-task owner keeps the state
                     const float cv = siluf(o);
                     s_bc[e] = cv;
-                    row = 2 * P.d_inner + e;
-                    if (tp && tap_owner) ((float*)(tp + P.tl.off[5]))[P.d_inner + e] = cv;
+                    row = 2 * x.d_inner() + e;
+                    if (tp && tap_owner) ((float*)(tp + P.tl.off[5]))[x.d_inner() + e] = cv;
                 } else {
-                    const int h = e - 2 * P.gs;
+                    const int h = e - 2 * x.gs();
                     const float dtv = sp_softplusf(fadd(val, ((const float*)(blk + P.b_dtb))[h]));
                     s_dt[h] = dtv;
-                    row = 2 * P.d_inner + e;
-                    tap_owner = e % P.G == c;
+                    row = 2 * x.d_inner() + e;
+                    tap_owner = e % x.G() == c;
                     if (tp && tap_owner) ((float*)(tp + P.tl.off[6]))[h] = dtv;
                 }
                 if (tp && tap_owner) {
@@ -768,15 +810,15 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
 
         // out_proj LoRA-down partial task of this CTA (warp 0): fetch the weights now, use them after gather G
         const int et_first = c;
-        const bool tt_first = wid == 0 && et_first < P.n_ttask;
+        const bool tt_first = wid == 0 && et_first < x.n_ttask();
         int4 pre_out[T_PRE];
         if (tt_first)
-            trow_prefetch(P.A_out + ((size_t)l * P.r + et_first / P.tsplit) * P.d_inner + (size_t)(et_first % P.tsplit) * tbytes, tbytes, lane, pre_out);
+            trow_prefetch(P.A_out + ((size_t)l * x.r() + et_first / x.tsplit()) * x.d_inner() + (size_t)(et_first % x.tsplit()) * tbytes, tbytes, lane, pre_out);
 
         // ---- S5 state update + readout, S6 gate: 16 lanes per channel; t = g*w is published as it is produced ----
         {
             double ss_own = 0.0;
-            const int hpg = P.nheads / P.ngroups;
+            const int hpg = x.nheads() / x.ngroups();
             const float* alog = (const float*)(stage + P.c_alog);
             const float* Dv = (const float*)(stage + P.c_D);
             const float* gw = (const float*)(stage + P.c_gnorm);
@@ -784,17 +826,17 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             for (int ib = 0; ib < nch; ib += THREADS / 16) {         // warp-uniform trip count (shuffles inside)
                 const int i = min(ib + (tid >> 4), nch - 1);
                 const bool valid = ib + (tid >> 4) < nch;
-                const int ch = ch0 + i, h = ch / P.headdim, grp = h / hpg;
+                const int ch = ch0 + i, h = ch / x.headdim(), grp = h / hpg;
                 const float dtv = s_dt[h];
                 const float An = -sp_expf(alog[i]);
                 const float dA = sp_expf(fmul(dtv, An));
                 const float xv = s_x[i];
                 const float dtx = fmul(dtv, xv);
-                float* Hr = (float*)(stage + P.st_ssm) + (size_t)i * P.d_state;
-                const float* Bc = s_bc + grp * P.d_state;
-                const float* Cc = s_bc + P.gs + grp * P.d_state;
+                float* Hr = (float*)(stage + P.st_ssm) + (size_t)i * x.d_state();
+                const float* Bc = s_bc + grp * x.d_state();
+                const float* Cc = s_bc + x.gs() + grp * x.d_state();
                 double a = 0.0;
-                for (int n4 = l16; valid && n4 < P.d_state / 4; n4 += 16) {
+                for (int n4 = l16; valid && n4 < x.d_state() / 4; n4 += 16) {
                     float4 hv = *(const float4*)(Hr + 4 * n4);
                     const float4 bv = *(const float4*)(Bc + 4 * n4);
                     const float4 cv = *(const float4*)(Cc + 4 * n4);
@@ -820,9 +862,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             ss_own = warp_sum(ss_own);
             if (lane == 0) red_d(x)[wid] = ss_own;
             __syncthreads();
-            slot_store(x, rec, P.x_G, P.g_slot, [&](int piece) {
+            slot_store(x, rec, P.x_G, x.g_slot(), [&](int piece) {
                 uint4 w = *(const uint4*)(s_slotG + 4 * piece);
-                const int ex = P.g_dpos - 4 * piece;
+                const int ex = x.g_dpos() - 4 * piece;
                 if (ex == 0 || ex == 2) {
                     double tot = 0.0;
 #pragma unroll
@@ -833,7 +875,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 return w;
             });
             if (tid == 0 && nch > 0) {         // write the state slice back (async), while the exchange goes on
-                bulk_s2g(P.ssm + (size_t)l * P.ssm_lstride + (size_t)ch0 * P.d_state, stage + P.st_ssm, (uint32_t)nch * P.d_state * 4);
+                bulk_s2g(P.ssm + (size_t)l * P.ssm_lstride + (size_t)ch0 * x.d_state(), stage + P.st_ssm, (uint32_t)nch * x.d_state() * 4);
                 bulk_s2g(conv_l + (size_t)ch0 * 4, stage + P.st_conv, (uint32_t)nch * 16);
                 bulk_commit();
             }
@@ -845,51 +887,51 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         int qsum_g;
         {
             uint4 vg[4];
-            hop_gather<4>(x, mine + P.x_G, P.G * P.g_slot, P.g_slot, P.g_dpos, vg);
+            hop_gather<4>(x, mine + P.x_G, x.G() * x.g_slot(), x.g_slot(), x.g_dpos(), vg);
             DFSSM_STAMP(l, 6);
-            slot_partials<4>(x, vg, P.G, P.g_slot, P.g_dpos);
-            qsum_g = norm_quant(x, SlotEnum<4>{ vg, chs, tid, P.G, P.g_slot >> 2 }, P.d_inner, false, s_g,
+            slot_partials<4>(x, vg, x.G(), x.g_slot(), x.g_dpos());
+            qsum_g = norm_quant(x, SlotEnum<4>{ vg, chs, tid, x.G(), x.g_slot() >> 2 }, x.d_inner(), false, s_g,
                                 (tp && c == 0) ? (int8_t*)(tp + P.tl.off[9]) : nullptr);
             if (tp && c == 0 && tid == 0) *(float*)(tp + P.tl.off[10]) = s_g;
         }
         DFSSM_STAMP(l, 7);
         // ---- S7: LoRA-down partial tasks (warp 0, published) and the out_proj sign rows (other warps) ----
         if (wid == 0) {
-            for (int e = c; e < P.n_ttask; e += P.G) {
-                const int j = e / P.tsplit, part = e % P.tsplit;
-                const int8_t* arow = P.A_out + ((size_t)l * P.r + j) * P.d_inner + (size_t)part * tbytes;
+            for (int e = c; e < x.n_ttask(); e += x.G()) {
+                const int j = e / x.tsplit(), part = e % x.tsplit();
+                const int8_t* arow = P.A_out + ((size_t)l * x.r() + j) * x.d_inner() + (size_t)part * tbytes;
                 if (e != c) trow_prefetch(arow, tbytes, lane, pre_out);
                 const int t = trow_dot(arow, tbytes, xq + (size_t)part * tbytes, lane, pre_out);
                 word_store(x, rec, P.x_T, e, (uint32_t)t ^ IBIAS);
             }
         } else {
             const uint32_t* bits = (const uint32_t*)(stage + P.c_out_bits);
-            const int npair = (nor + 1) >> 1, wspan = P.Wout / KS;
+            const int npair = (nor + 1) >> 1, wspan = x.Wout() / KS;
             for (int id = wid - 1; id < npair * KS; id += NWARPS - 1) {
                 const int pair = id / KS, half = id - pair * KS;
                 const int nrows = min(2, nor - 2 * pair);
-                const uint32_t* const rowp[2] = { bits + (size_t)(2 * pair) * P.Wout, bits + (size_t)(2 * pair + (nrows > 1 ? 1 : 0)) * P.Wout };
+                const uint32_t* const rowp[2] = { bits + (size_t)(2 * pair) * x.Wout(), bits + (size_t)(2 * pair + (nrows > 1 ? 1 : 0)) * x.Wout() };
                 int p[2];
-                sign_partial<2>(rowp, nrows, half * wspan, half == KS - 1 ? P.Wout : (half + 1) * wspan, xq, P.d_inner, lane, p);
+                sign_partial<2>(rowp, nrows, half * wspan, half == KS - 1 ? x.Wout() : (half + 1) * wspan, xq, x.d_inner(), lane, p);
                 const int v = reduce2(p, lane);
                 const int r = lane >> 4;
-                if ((lane & 15) == 0 && r < nrows) s_acc_out[half * P.nor_max + 2 * pair + r] = v;
+                if ((lane & 15) == 0 && r < nrows) s_acc_out[half * x.nor_max() + 2 * pair + r] = v;
             }
         }
         DFSSM_STAMP(l, 8);
         // ---- gather T: t_out = sum of the partial sums;  v_j = a_s[j] * float(t_j) ----
         {
             uint4 vt[1];
-            hop_gather<1>(x, mine + P.x_T, P.n_ttask, 0, 0, vt);
+            hop_gather<1>(x, mine + P.x_T, x.n_ttask(), 0, 0, vt);
             const float* a_s = (const float*)(blk + P.b_as_out);
             const uint32_t w[4] = { vt[0].x, vt[0].y, vt[0].z, vt[0].w };
-            const int rows_per_chunk = 4 / P.tsplit;
+            const int rows_per_chunk = 4 / x.tsplit();
 #pragma unroll
             for (int jj = 0; jj < 4; ++jj) {
                 const int j = tid * rows_per_chunk + jj;
-                if (jj < rows_per_chunk && j < P.r) {
+                if (jj < rows_per_chunk && j < x.r()) {
                     int t = 0;
-                    for (int q = 0; q < P.tsplit; ++q) t += (int)(w[jj * P.tsplit + q] ^ IBIAS);
+                    for (int q = 0; q < x.tsplit(); ++q) t += (int)(w[jj * x.tsplit() + q] ^ IBIAS);
                     s_vout[j] = (double)fmul(a_s[j], (float)t);
                     if (tp && c == 0) ((int32_t*)(tp + P.tl.off[12]))[j] = t;
                 }
@@ -908,13 +950,13 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 const int i = ib + (tid >> 2), sub = tid & 3;
                 const bool valid = i < nor;
                 double lo = 0.0;
-                const int8_t* brow = Bm + (size_t)(valid ? i : 0) * P.r_pad;
+                const int8_t* brow = Bm + (size_t)(valid ? i : 0) * x.r_pad();
                 if (valid)
-                    for (int j = sub; j < P.r; j += 4) lo = __fma_rn((double)brow[j], s_vout[j], lo);
+                    for (int j = sub; j < x.r(); j += 4) lo = __fma_rn((double)brow[j], s_vout[j], lo);
                 lo += __shfl_xor_sync(0xffffffffu, lo, 1);
                 lo += __shfl_xor_sync(0xffffffffu, lo, 2);
                 if (sub != 0 || !valid) continue;
-                const int p128 = s_acc_out[i] + (KS > 1 ? s_acc_out[P.nor_max + i] : 0);
+                const int p128 = s_acc_out[i] + (KS > 1 ? s_acc_out[x.nor_max() + i] : 0);
                 const int acc = 2 * (p128 / 128) - qsum_g;       // exact: every term is a multiple of 128
                 const float o = fmul(s_g, fadd(fmul(scale[i], (float)acc), fmul(bsv[i], (float)lo)));
                 const float un = fadd(s_u[i], o);
@@ -926,9 +968,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             ss_u = warp_sum(ss_u);
             if (lane == 0) red_d(x)[wid] = ss_u;
             __syncthreads();                        // also: every thread is done with this stage's weights
-            slot_store(x, rec, P.x_U, P.u_slot, [&](int piece) {
+            slot_store(x, rec, P.x_U, x.u_slot(), [&](int piece) {
                 uint4 w = *(const uint4*)(s_slotU + 4 * piece);
-                const int ex = P.u_dpos - 4 * piece;
+                const int ex = x.u_dpos() - 4 * piece;
                 if (ex == 0 || ex == 2) {
                     double tot = 0.0;
 #pragma unroll
@@ -944,16 +986,16 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             }
         }
         if (t_first && l + 1 < P.L)
-            trow_prefetch(P.A_in + ((size_t)(l + 1) * P.r + (e_first - P.n_bcdt)) * P.d_model, P.d_model, lane, pre_in);
+            trow_prefetch(P.A_in + ((size_t)(l + 1) * x.r() + (e_first - x.n_bcdt())) * x.d_model(), x.d_model(), lane, pre_in);
         DFSSM_STAMP(l, 10);
         // ---- gather U, S1 of the next layer (or S8's norm) in every CTA ----
         {
             uint4 vu[2];
-            hop_gather<2>(x, mine + P.x_U, P.G * P.u_slot, P.u_slot, P.u_dpos, vu);
+            hop_gather<2>(x, mine + P.x_U, x.G() * x.u_slot(), x.u_slot(), x.u_dpos(), vu);
             DFSSM_STAMP(l, 11);
-            slot_partials<2>(x, vu, P.G, P.u_slot, P.u_dpos);
+            slot_partials<2>(x, vu, x.G(), x.u_slot(), x.u_dpos());
             uint8_t* tpn = (taps_on && c == 0 && l + 1 < P.L) ? P.taps + (size_t)(l + 1) * P.tap_lstride : nullptr;
-            qsum = norm_quant(x, SlotEnum<2>{ vu, ors, tid, P.G, P.u_slot >> 2 }, P.d_model, l == P.L - 1, s_act,
+            qsum = norm_quant(x, SlotEnum<2>{ vu, ors, tid, x.G(), x.u_slot() >> 2 }, x.d_model(), l == P.L - 1, s_act,
                               tpn ? (int8_t*)(tpn + P.tl.off[0]) : nullptr);
             if (tpn && tid == 0) *(float*)(tpn + P.tl.off[1]) = s_act;
         }
@@ -972,7 +1014,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         const uint8_t* stage = sm + P.s_ring + (size_t)(item % P.stages) * P.stage_bytes;
         const int row0 = v0 + it * P.lm_rows_item;
         const int nrows_it = min(P.lm_rows_item, v1 - row0);
-        const int nchunk = P.d_model >> 4;
+        const int nchunk = x.d_model() >> 4;
         for (int q0 = 4 * wid; q0 < nrows_it; q0 += 4 * NWARPS) {
             const int nr = min(4, nrows_it - q0);
             int s[4] = { 0, 0, 0, 0 };
@@ -981,7 +1023,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
 #pragma unroll
                 for (int r = 0; r < 4; ++r) {
                     if (r < nr) {
-                        const int4 a4 = *(const int4*)(stage + (size_t)(q0 + r) * P.d_model + 16 * ch);
+                        const int4 a4 = *(const int4*)(stage + (size_t)(q0 + r) * x.d_model() + 16 * ch);
                         s[r] = dp4a_ss(a4.x, q4.x, s[r]); s[r] = dp4a_ss(a4.y, q4.y, s[r]);
                         s[r] = dp4a_ss(a4.z, q4.z, s[r]); s[r] = dp4a_ss(a4.w, q4.w, s[r]);
                     }
@@ -1020,7 +1062,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             P.am_idx[c] = besti;
             __threadfence();
             const unsigned prev = atomicAdd(P.am_count, 1u);
-            s_last = prev == (unsigned)P.G - 1;
+            s_last = prev == (unsigned)x.G() - 1;
             bulk_wait0();                       // all state write-backs of this CTA are complete
         }
         __syncthreads();
@@ -1028,7 +1070,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             __threadfence();
             float b = -INFINITY;
             int bi = 0x7fffffff;
-            for (int g = lane; g < P.G; g += 32) {
+            for (int g = lane; g < x.G(); g += 32) {
                 const float ov = __ldcg(P.am_val + g);
                 const int oi = __ldcg(P.am_idx + g);
                 if (ov > b || (ov == b && oi < bi)) { b = ov; bi = oi; }

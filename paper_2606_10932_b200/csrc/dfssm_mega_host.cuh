@@ -10,7 +10,6 @@
 namespace dfssm {
 namespace mega {
 
-constexpr int GRID = 148;                       // one CTA per B200 SM
 constexpr size_t SMEM_LIMIT = 232448 - 1024;    // 227 KB opt-in maximum minus the kernel's static shared memory
 
 inline uint32_t up32(uint32_t x, uint32_t a) { return (x + a - 1) / a * a; }
@@ -79,12 +78,8 @@ inline bool plan(const Dims& d, int G, Params& P)
     P.lm_rows_item = (int)(P.stage_bytes / d.d_model);
 
     // exchange: one (record, mailbox) part list, 32-bit word offsets, every part 128-byte aligned
-    P.M = 37;                                       // mailboxes (tunable: DFSSM_MEGA_M, must divide G)
-    if (const char* e = getenv("DFSSM_MEGA_M")) {
-        const int m = atoi(e);
-        if (m >= 1 && m <= G && G % m == 0) P.M = m;
-    }
-    if (G % P.M) P.M = G;
+    if (G != GRID) return false;
+    P.M = MBOX;
     P.gsz = G / P.M;
     P.u_dpos = (P.nor_max + 1) / 2 * 2;
     P.u_slot = (P.u_dpos + 2 + 3) / 4 * 4;
@@ -240,6 +235,38 @@ inline void permute_A(const int8_t* A, int r, int K, int8_t* out)
 {
     for (int j = 0; j < r; ++j)
         for (int k = 0; k < K; ++k) out[(size_t)j * K + plane_pos_host(k, K)] = A[(size_t)j * K + k];
+}
+
+}  // namespace mega
+}  // namespace dfssm
+
+namespace dfssm {
+namespace mega {
+
+// the shapes of BASELINE.json's configs get a kernel with compile-time dimensions; taps or any other shape use
+// the run-time-shape kernel
+using Shape0 = ShapeCT<256, 512, 64, 64, 1, 8>;
+using Shape1 = ShapeCT<768, 1536, 64, 128, 1, 16>;
+using Shape2 = ShapeCT<2048, 4096, 64, 128, 1, 32>;
+using Shape4 = ShapeCT<2560, 5120, 64, 128, 1, 32>;
+
+template <class S>
+inline bool shape_is(const Dims& d)
+{
+    return d.d_model == S::d_model && d.d_inner == S::d_inner && d.headdim == S::headdim && d.d_state == S::d_state &&
+           d.ngroups == S::ngroups && d.r == S::r;
+}
+
+typedef void (*KernelFn)(const Params);
+inline KernelFn pick_kernel(const Dims& d, bool taps)
+{
+    if (!taps) {
+        if (shape_is<Shape0>(d)) return k_mega<Shape0, false>;
+        if (shape_is<Shape1>(d)) return k_mega<Shape1, false>;
+        if (shape_is<Shape2>(d)) return k_mega<Shape2, false>;
+        if (shape_is<Shape4>(d)) return k_mega<Shape4, false>;
+    }
+    return k_mega<ShapeRT, true>;
 }
 
 }  // namespace mega
