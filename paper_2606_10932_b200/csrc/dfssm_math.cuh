@@ -23,7 +23,8 @@ __device__ __forceinline__ float sp_expf(float x)
 {
     if (x < -87.0f) return 0.0f;
     if (x > 88.0f) x = 88.0f;
-    const float n = rintf(fmul(x, 0x1.715476p+0f));
+    const float nr = fadd(fmul(x, 0x1.715476p+0f), 12582912.0f);    // rint by magic-number addition (|n| <= 127)
+    const float n = fadd(nr, -12582912.0f);
     float r = ffma(n, -0x1.63p-1f, x);
     r = ffma(n, 0x1.bd0106p-13f, r);               // -LN2_LO with LN2_LO = -0x1.bd0106p-13
     float p = 0x1.a01a02p-13f;                     // 1/7!
@@ -34,7 +35,7 @@ __device__ __forceinline__ float sp_expf(float x)
     p = ffma(p, r, 0x1p-1f);                       // 1/2!
     p = ffma(p, r, 1.0f);
     p = ffma(p, r, 1.0f);
-    const int ni = (int)n;                         // in [-126, 127]
+    const int ni = __float_as_int(nr) - 0x4b400000;   // in [-126, 127]
     return fmul(p, __uint_as_float((uint32_t)(ni + 127) << 23));
 }
 
@@ -88,12 +89,14 @@ __device__ __forceinline__ int dp4a_us(uint32_t a, int b, int c)
 // signed x signed
 __device__ __forceinline__ int dp4a_ss(int a, int b, int c) { return __dp4a(a, b, c); }
 
-// per-token absmax quantiser (R4): codes from t = v*w, inv = 127/amax, ties to even, clamp +-127
+// per-token absmax quantiser (R4): codes from t = v*w, inv = 127/amax, ties to even, clamp +-127.
+// rint by the magic-number addition (exact ties-to-even for |x| < 2^22; here |t*inv| <= 127(1 + 2^-23)): the
+// FRND / F2I conversions run at a quarter of the fp32 rate and the quantiser is on the critical path.
 __device__ __forceinline__ int quant_code(float t, float inv)
 {
-    float f = rintf(fmul(t, inv));
-    f = fminf(fmaxf(f, -127.0f), 127.0f);
-    return (int)f;
+    const float r = fadd(fmul(t, inv), 12582912.0f);            // 1.5 * 2^23
+    const int q = __float_as_int(r) - 0x4b400000;
+    return max(-127, min(127, q));
 }
 
 // ---- warp / block reductions (any tree is allowed: sums are binary64, max is exact) ----

@@ -43,13 +43,20 @@
 namespace dfssm {
 namespace mega {
 
-constexpr int THREADS = 512;
+constexpr int THREADS = 512;                  // 16 warps (measured: 32 warps only add issue pressure to the short phases)
 constexpr int NWARPS = THREADS / 32;
+constexpr int NJ_G = 2048 / THREADS;          // 16-byte chunks per thread when gathering G / U / A (plan() checks the sizes)
+constexpr int NJ_U = 1024 / THREADS;
+constexpr int NJ_A = 1024 / THREADS;
+constexpr int NR_IN = THREADS >= 1024 ? 2 : 4;     // in_proj sign rows per warp pass
+constexpr int LPR = THREADS / 512;            // lanes per row in the in_proj epilogue
+constexpr int LPC = 16;                       // lanes per channel in the state update
+constexpr int KS_MAX = 4;                     // largest K-split of the out_proj sign rows
 constexpr int MAX_STAGES = 8;
 constexpr uint32_t SPIN_LIMIT = 1u << 20;     // ~0.3 s of polling, then the step aborts with an error flag
 constexpr uint32_t SENT = 0xffffffffu;        // "not written yet"
 constexpr uint32_t IBIAS = 0x80000000u;       // int32 payloads are stored xor IBIAS (|value| < 2^30)
-constexpr int PROF_NPH = 16;                  // phase stamps per (CTA, layer) of the in-kernel profiler
+constexpr int PROF_NPH = 32;                  // phase stamps per (CTA, layer) of the in-kernel profiler
 
 struct Params {
     // ---- shape ----
@@ -66,7 +73,7 @@ struct Params {
     // ---- per-layer block read by every CTA (byte offsets) ----
     uint32_t b_eB, b_escale, b_ebs, b_econv_w, b_econv_b, b_dtb, b_as_in, b_as_out, blk_bytes;
     // ---- pipeline stage ----
-    uint32_t st_blk, st_ssm, st_conv, st_econv, stage_bytes;
+    uint32_t st_blk, st_ssm, st_conv, st_econv, st_tin, st_tout, stage_bytes;
     int stages, lm_rows_item;
     // ---- exchange: M mailboxes x 4 rotating records; 32-bit word offsets inside one (record, mailbox) ----
     int M, gsz;                  // mailboxes, CTAs polling each (G = M * gsz); CTA c polls mailbox c / gsz
@@ -161,12 +168,13 @@ __device__ __forceinline__ int4 ldg_nc16(const void* p)
     return r;
 }
 
-// position of canonical element k inside a plane-ordered code vector of length K: word w = k/32, in-word
-// p = 8j + i; planes 0..3 live in the first half (16 B per word), planes 4..7 in the second half.
+// Code layout for the masked-dp4a sign dot: a 32-block of codes is eight 4-byte words ("planes"), plane i = elements
+// 4i .. 4i+3 of the block; the load-time repack moves the sign bit of element 4i + j to bit 8j + i of the sign word,
+// so dp4a(bits & (0x01010101 << i), plane i) sums plane i.  Planes 0..3 of all blocks form the first half of
+// the vector (16 B per block), planes 4..7 the second half: position of canonical element k in a vector of length K.
 __device__ __forceinline__ int plane_pos(int k, int K)
 {
-    const int w = k >> 5, p = k & 31, j = p >> 3, i = p & 7;
-    return (i < 4 ? 0 : (K >> 1)) + 16 * w + 4 * (i & 3) + j;
+    return ((k & 16) ? (K >> 1) : 0) + ((k >> 5) << 4) + (k & 15);
 }
 
 // Shape of the model as the kernel sees it: compile-time constants for the shapes of BASELINE.json's configs (every
@@ -187,6 +195,10 @@ struct Ctx {
 #define DFSSM_DIM(n_) __device__ __forceinline__ int n_() const { return S::kStatic ? S::n_ : P.n_; }
     DFSSM_DIM(d_model) DFSSM_DIM(d_inner) DFSSM_DIM(headdim) DFSSM_DIM(d_state) DFSSM_DIM(ngroups) DFSSM_DIM(r)
 #undef DFSSM_DIM
+    __device__ __forceinline__ void stamp(int l, int k) const
+    {
+        if (P.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + k] = clock64();
+    }
     __device__ __forceinline__ constexpr int G() const { return GRID; }
     __device__ __forceinline__ constexpr int M() const { return MBOX; }
     __device__ __forceinline__ constexpr int gsz() const { return GRID / MBOX; }
@@ -203,6 +215,13 @@ struct Ctx {
     __device__ __forceinline__ int n_early() const { return n_bcdt() + r(); }
     __device__ __forceinline__ int tsplit() const { return (d_inner() % 64 == 0 && 4 * r() <= GRID) ? 4 : (2 * r() <= GRID ? 2 : 1); }
     __device__ __forceinline__ int n_ttask() const { return r() * tsplit(); }
+    // early task e = c + k G of this CTA that is a LoRA-down row (at most one: r <= G), or -1
+    __device__ __forceinline__ int t_in_task() const
+    {
+        const int k = c >= n_bcdt() ? 0 : (n_bcdt() - c + GRID - 1) / GRID;
+        const int e = c + k * GRID;
+        return e < n_early() ? e : -1;
+    }
     __device__ __forceinline__ int u_dpos() const { return (nor_max() + 1) / 2 * 2; }
     __device__ __forceinline__ int u_slot() const { return (u_dpos() + 2 + 3) / 4 * 4; }
     __device__ __forceinline__ int g_dpos() const { return (nch_max() + 1) / 2 * 2; }
@@ -281,29 +300,39 @@ template <class S>
 __device__ __forceinline__ double* red_d(const Ctx<S>& x) { return (double*)(x.sm + x.P.s_red + 8 * NWARPS); }
 
 // S1 / S6 / S8 norm + quantise of a whole vector in every CTA.  `en(f)` calls f(k, bits) for every element this
-// thread holds: bits = fp32 t_k = value_k * w_k.  The caller has stored the partial sums of squares (one per
-// CTA, or per warp for the embedding) into part[0..G) (zeros where unused).  Every CTA derives the same
-// rstd / amax / codes.  Writes the codes to xq (plane order unless `canonical`), returns the sum of the codes
-// and the activation scale s.  Two __syncthreads.
+// thread holds: bits = fp32 t_k = value_k * w_k;  ss_local = the partial sums of squares this thread holds (the
+// per-CTA partials it gathered, or its own elements' squares for the embedding).  Warp 0 reduces the warp
+// results and derives rstd / amax / scale once; every thread then quantises its elements.  Writes the codes to
+// xq (plane order unless `canonical`), returns the sum of the codes and the activation scale s.
+// Three __syncthreads.
 template <class S, typename Enum>
-__device__ __forceinline__ int norm_quant(const Ctx<S>& x, Enum en, int K, bool canonical, float& s_out, int8_t* tap_codes)
+__device__ __forceinline__ int norm_quant(const Ctx<S>& x, Enum en, double ss_local, int K, bool canonical, float& s_out, int8_t* tap_codes,
+                                          int pl = 0, int pk = -1)
 {
     const Params& P = x.P;
     uint8_t* xq = x.sm + P.s_xq;
-    const double* part = (const double*)(x.sm + P.s_part);
+    float* bc = (float*)(x.sm + P.s_part);
     float am = 0.0f;
     en([&](int, uint32_t w) { am = fmaxf(am, fabsf(__uint_as_float(w))); });
     am = warp_max(am);
-    if (x.lane == 0) red_f(x)[x.wid] = am;
+    ss_local = warp_sum(ss_local);
+    if (x.lane == 0) { red_f(x)[x.wid] = am; red_d(x)[x.wid] = ss_local; }
+    if (pk >= 0) x.stamp(pl, pk);
     __syncthreads();
-    // every warp derives the constants itself
-    float amax = x.lane < NWARPS ? red_f(x)[x.lane] : 0.0f;
-    amax = warp_max(amax);
-    double ss = 0.0;
-    for (int g = x.lane; g < x.G(); g += 32) ss += part[g];
-    ss = warp_sum(ss);
-    float inv;
-    quant_consts(ss, amax, K, P.eps, inv, s_out);
+    if (pk >= 0) x.stamp(pl, pk + 1);
+    if (x.wid == 0) {
+        float amax = x.lane < NWARPS ? red_f(x)[x.lane] : 0.0f;
+        double ss = x.lane < NWARPS ? red_d(x)[x.lane] : 0.0;
+        amax = warp_max(amax);
+        ss = warp_sum(ss);
+        float inv, sc;
+        quant_consts(ss, amax, K, P.eps, inv, sc);
+        if (x.lane == 0) { bc[0] = inv; bc[1] = sc; }
+    }
+    __syncthreads();
+    const float inv = bc[0];
+    s_out = bc[1];
+    if (pk >= 0) x.stamp(pl, pk + 2);
     int qs = 0;
     en([&](int k, uint32_t w) {
         const int q = quant_code(__uint_as_float(w), inv);          // inv == 0 -> code 0
@@ -313,6 +342,7 @@ __device__ __forceinline__ int norm_quant(const Ctx<S>& x, Enum en, int K, bool 
     });
     qs = warp_sum_i(qs);
     if (x.lane == 0) red_i(x)[x.wid] = qs;
+    if (pk >= 0) x.stamp(pl, pk + 3);
     __syncthreads();
     const int tot = x.lane < NWARPS ? red_i(x)[x.lane] : 0;
     return warp_sum_i(tot);
@@ -342,21 +372,22 @@ struct SlotEnum {
         }
     }
 };
-// store the fp64 partials found in the gathered chunks into part[slot]
+// sum of the fp64 partials found in this thread's gathered chunks
 template <int NJ, class S>
-__device__ __forceinline__ void slot_partials(const Ctx<S>& x, const uint4 (&v)[NJ], int nslots, int slot_w, int dpos)
+__device__ __forceinline__ double slot_partials(const Ctx<S>& x, const uint4 (&v)[NJ], int nslots, int slot_w, int dpos)
 {
-    double* part = (double*)(x.sm + x.P.s_part);
     const int pps = slot_w >> 2;
+    double s = 0.0;
 #pragma unroll
     for (int j = 0; j < NJ; ++j) {
         const int ci = x.tid + j * THREADS;
         if (ci < nslots * pps) {
             const int g = ci / pps, ex = dpos - 4 * (ci - g * pps);
-            if (ex == 0) part[g] = __hiloint2double((int)v[j].y, (int)v[j].x);
-            else if (ex == 2) part[g] = __hiloint2double((int)v[j].w, (int)v[j].z);
+            if (ex == 0) s += __hiloint2double((int)v[j].y, (int)v[j].x);
+            else if (ex == 2) s += __hiloint2double((int)v[j].w, (int)v[j].z);
         }
     }
+    return s;
 }
 
 // block-wide sum of doubles held by some lanes (others pass 0); result valid in thread 0 only.  One __syncthreads.
@@ -444,34 +475,18 @@ __device__ __forceinline__ int reduce2(const int (&p)[2], int lane)
     return v;
 }
 
-// int8 x int8 dot of `nbytes` plane-permuted LoRA-down weights (global memory) with the codes at the same
-// positions in shared memory.  pre[] holds the first T_PRE*32 16-byte chunks, loaded a phase earlier so that
-// their latency is off the critical path.
-constexpr int T_PRE = 4;
-__device__ __forceinline__ void trow_prefetch(const int8_t* row, int nbytes, int lane, int4 (&pre)[T_PRE])
-{
-    const int nch = nbytes >> 4;
-#pragma unroll
-    for (int i = 0; i < T_PRE; ++i) {
-        const int ch = lane + 32 * i;
-        if (ch < nch) pre[i] = ldg_nc16(row + 16 * ch);
-    }
-}
-__device__ __forceinline__ int trow_dot(const int8_t* row, int nbytes, const uint8_t* xq, int lane, const int4 (&pre)[T_PRE])
+template <int NR> struct RowReduce;       // lane (32 / NR) * r ends up with the warp total of p[r]
+template <> struct RowReduce<4> { static __device__ __forceinline__ int run(const int (&p)[4], int lane) { return reduce4(p, lane); } };
+template <> struct RowReduce<2> { static __device__ __forceinline__ int run(const int (&p)[2], int lane) { return reduce2(p, lane); } };
+
+// int8 x int8 dot of `nbytes` plane-permuted LoRA-down weights (fetched into the stage with the rest of the item)
+// with the codes at the same positions
+__device__ __forceinline__ int trow_dot(const uint8_t* row, int nbytes, const uint8_t* xq, int lane)
 {
     const int nch = nbytes >> 4;
     int s = 0;
-#pragma unroll
-    for (int i = 0; i < T_PRE; ++i) {
-        const int ch = lane + 32 * i;
-        if (ch < nch) {
-            const int4 q = *(const int4*)(xq + 16 * ch);
-            s = dp4a_ss(pre[i].x, q.x, s); s = dp4a_ss(pre[i].y, q.y, s);
-            s = dp4a_ss(pre[i].z, q.z, s); s = dp4a_ss(pre[i].w, q.w, s);
-        }
-    }
-    for (int ch = lane + 32 * T_PRE; ch < nch; ch += 32) {
-        const int4 a = ldg_nc16(row + 16 * ch);
+    for (int ch = lane; ch < nch; ch += 32) {
+        const int4 a = *(const int4*)(row + 16 * ch);
         const int4 q = *(const int4*)(xq + 16 * ch);
         s = dp4a_ss(a.x, q.x, s); s = dp4a_ss(a.y, q.y, s); s = dp4a_ss(a.z, q.z, s); s = dp4a_ss(a.w, q.w, s);
     }
@@ -493,7 +508,13 @@ __device__ __forceinline__ void issue_item(const Ctx<S>& x, int item, int v0, in
         const int* chs = (const int*)(x.sm + P.s_chs);
         const int ch0 = chs[x.c], nch = chs[x.c + 1] - ch0;
         const uint32_t ssm_b = (uint32_t)nch * x.d_state() * 4, conv_b = (uint32_t)nch * 16, econv_b = (uint32_t)x.gs() * 32;
-        mbar_expect_tx(bar, P.chunk_bytes + P.blk_bytes + ssm_b + conv_b + econv_b);
+        const int e_t = x.t_in_task();                                      // LoRA-down row of in_proj this CTA owns (or -1)
+        const uint32_t tin_b = e_t >= 0 ? (uint32_t)x.d_model() : 0u;
+        const uint32_t tout_b = x.c < x.n_ttask() ? (uint32_t)(x.d_inner() / x.tsplit()) : 0u;
+        mbar_expect_tx(bar, P.chunk_bytes + P.blk_bytes + ssm_b + conv_b + econv_b + tin_b + tout_b);
+        if (tin_b) bulk_g2s(stage + P.st_tin, P.A_in + ((size_t)item * x.r() + (e_t - x.n_bcdt())) * x.d_model(), tin_b, bar);
+        if (tout_b)
+            bulk_g2s(stage + P.st_tout, P.A_out + ((size_t)item * x.r() + x.c / x.tsplit()) * x.d_inner() + (size_t)(x.c % x.tsplit()) * tout_b, tout_b, bar);
         bulk_g2s(stage, P.chunks + ((size_t)item * x.G() + x.c) * P.chunk_bytes, P.chunk_bytes, bar);
         bulk_g2s(stage + P.st_blk, P.blocks + (size_t)item * P.blk_bytes, P.blk_bytes, bar);
         bulk_g2s(stage + P.st_econv, P.conv + (size_t)item * P.conv_lstride + (size_t)x.d_inner() * 4, econv_b, bar);
@@ -594,14 +615,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
     uint32_t* s_slotU = (uint32_t*)(sm + P.s_slot);
     uint32_t* s_slotG = s_slotU + x.u_slot();
     if (tid < x.u_slot() + x.g_slot()) s_slotU[tid] = 0u;      // pad words of the slots are published as 0
-    const int KS = x.Wout() >= 64 ? 2 : 1;             // K-split of the out_proj sign rows
+    // K-split of the out_proj sign rows: every (row pair, K part) is one warp task
+    const int KS = (THREADS >= 1024 && x.Wout() >= 128) ? 4 : (x.Wout() >= 64 ? 2 : 1);
     const int tbytes = x.d_inner() / x.tsplit();         // bytes of one out_proj LoRA-down partial task
-
-    // warp k takes early task k (e = c + k G); if that is a LoRA-down row it fetches the row a phase ahead
-    const int e_first = c + wid * x.G();
-    const bool t_first = wid < nb_tasks && e_first >= x.n_bcdt();
-    int4 pre_in[T_PRE];
-    if (t_first && P.L > 0) trow_prefetch(P.A_in + (size_t)(e_first - x.n_bcdt()) * x.d_model(), x.d_model(), lane, pre_in);
 
     // ---------------- S0 embedding + the first norm/quantise, redundantly in every CTA ----------------
     float s_act;                                     // scale of the current activation codes
@@ -614,10 +630,10 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         }
         const int8_t* erow = P.emb + (size_t)tok * x.d_model();
         const float es = P.emb_s[tok];
-        uint4 v[4];
+        uint4 v[NJ_G];
         double ss = 0.0;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
+        for (int j = 0; j < NJ_G; ++j) {
             const int k0 = 4 * (tid + j * THREADS);
             if (k0 < x.d_model()) {
                 uint32_t w[4];
@@ -631,21 +647,15 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 v[j] = make_uint4(w[0], w[1], w[2], w[3]);
             }
         }
-        // the per-CTA partial sums of the exchange are replaced by the per-warp partial sums of this CTA
-        double* part = (double*)(sm + P.s_part);
-        ss = warp_sum(ss);
-        for (int g = tid; g < x.G(); g += THREADS)
-            if (g >= NWARPS) part[g] = 0.0;
-        if (lane == 0) part[wid] = ss;
         uint8_t* tp0 = (taps_on && c == 0 && P.L > 0) ? P.taps : nullptr;
         auto en = [&](auto f) {
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
+            for (int j = 0; j < NJ_G; ++j) {
                 const int k0 = 4 * (tid + j * THREADS);
                 if (k0 < x.d_model()) { f(k0, v[j].x); f(k0 + 1, v[j].y); f(k0 + 2, v[j].z); f(k0 + 3, v[j].w); }
             }
         };
-        qsum = norm_quant(x, en, x.d_model(), P.L == 0, s_act, tp0 ? (int8_t*)(tp0 + P.tl.off[0]) : nullptr);
+        qsum = norm_quant(x, en, ss, x.d_model(), P.L == 0, s_act, tp0 ? (int8_t*)(tp0 + P.tl.off[0]) : nullptr);
         if (tp0 && tid == 0) *(float*)(tp0 + P.tl.off[1]) = s_act;
     }
 
@@ -659,13 +669,12 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         const uint32_t* mine = rec + (size_t)mbox * P.x_words;                                 // polled
         uint32_t* recc = P.xbuf + (size_t)((P.rec0 + (uint32_t)l + 2u) & 3u) * rec_words;     // reset for layer l + 2
         DFSSM_STAMP(l, 0);
-        if (P.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + 15] = globaltimer_ns();
+        if (P.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + 31] = globaltimer_ns();
         {   // reset own slots of the record two layers ahead (same thread -> address map as the publishes below)
             slot_store(x, recc, P.x_U, x.u_slot(), [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
             slot_store(x, recc, P.x_G, x.g_slot(), [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
             for (int k = wid; k < nb_tasks; k += NWARPS) word_store(x, recc, P.x_A, c + k * x.G(), SENT);
-            if (wid == 0)
-                for (int e = c; e < x.n_ttask(); e += x.G()) word_store(x, recc, P.x_T, e, SENT);
+            if (wid == 0 && c < x.n_ttask()) word_store(x, recc, P.x_T, c, SENT);
         }
 
         wait_item(x, l);
@@ -682,43 +691,41 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     sign_partial<1>(rowp, 1, 0, x.Win(), xq, x.d_model(), lane, p);
                     val = 2 * (warp_sum_i(p[0]) / 128) - qsum;       // exact: every term is a multiple of 128
                 } else {
-                    const int8_t* arow = P.A_in + ((size_t)l * x.r() + (e - x.n_bcdt())) * x.d_model();
-                    if (k != wid) trow_prefetch(arow, x.d_model(), lane, pre_in);
-                    val = trow_dot(arow, x.d_model(), xq, lane, pre_in);
+                    val = trow_dot(stage + P.st_tin, x.d_model(), xq, lane);
                 }
                 word_store(x, rec, P.x_A, e, (uint32_t)val ^ IBIAS);
                 if (lane == 0 && tp && e >= x.n_bcdt()) ((int32_t*)(tp + P.tl.off[3]))[e - x.n_bcdt()] = val;
             }
         }
-        // ---- S2: z and x sign rows of this CTA, 4 rows per warp pass, dealt from the top warp down ----
+        // ---- S2: z and x sign rows of this CTA, NR_IN rows per warp pass, dealt from the top warp down ----
         {
             const uint32_t* bits = (const uint32_t*)(stage + P.c_in_bits);
             const int n_tasks = 2 * nch;
-            for (int q = NWARPS - 1 - wid; 4 * q < n_tasks; q += NWARPS) {
-                const uint32_t* rowp[4];
-                int slot[4];
-                const int nrows = min(4, n_tasks - 4 * q);
+            for (int q = NWARPS - 1 - wid; NR_IN * q < n_tasks; q += NWARPS) {
+                const uint32_t* rowp[NR_IN];
+                int slot[NR_IN];
+                const int nrows = min(NR_IN, n_tasks - NR_IN * q);
 #pragma unroll
-                for (int r = 0; r < 4; ++r) {
-                    const int t = 4 * q + r;
+                for (int r = 0; r < NR_IN; ++r) {
+                    const int t = NR_IN * q + r;
                     slot[r] = r < nrows ? (t < nch ? t : x.nch_max() + (t - nch)) : 0;
                     rowp[r] = bits + (size_t)slot[r] * x.Win();
                 }
-                int p[4];
-                sign_partial<4>(rowp, nrows, 0, x.Win(), xq, x.d_model(), lane, p);
-                const int v = reduce4(p, lane);
-                const int r = lane >> 3;
-                if ((lane & 7) == 0 && r < nrows) s_acc_in[slot[r]] = 2 * (v / 128) - qsum;
+                int p[NR_IN];
+                sign_partial<NR_IN>(rowp, nrows, 0, x.Win(), xq, x.d_model(), lane, p);
+                const int v = RowReduce<NR_IN>::run(p, lane);
+                const int r = lane / (32 / NR_IN);
+                if (lane % (32 / NR_IN) == 0 && r < nrows) s_acc_in[slot[r]] = 2 * (v / 128) - qsum;
             }
         }
         DFSSM_STAMP(l, 2);
         // ---- gather A: accumulators of all B|C|dt rows and t_in;  v_j = a_s[j] * float(t_j) ----
         {
-            uint4 va[2];
-            hop_gather<2>(x, mine + P.x_A, x.n_early(), 0, 0, va);
+            uint4 va[NJ_A];
+            hop_gather<NJ_A>(x, mine + P.x_A, x.n_early(), 0, 0, va);
             const float* a_s = (const float*)(blk + P.b_as_in);
 #pragma unroll
-            for (int j = 0; j < 2; ++j) {
+            for (int j = 0; j < NJ_A; ++j) {
                 const int e0 = 4 * (tid + j * THREADS);
                 const uint32_t w[4] = { va[j].x, va[j].y, va[j].z, va[j].w };
 #pragma unroll
@@ -734,13 +741,15 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         }
         __syncthreads();
         DFSSM_STAMP(l, 3);
-        // ---- S3 stage 2 + S4 conv + dt softplus: one thread per row; own z|x rows and ALL B|C rows (+ own dt) ----
+        // ---- S3 stage 2 + S4 conv + dt softplus: LPR lanes per row; own z|x rows and ALL B|C rows (+ own dt) ----
         {
             const int n_dt = tp ? x.nheads() : (h1 - h0 + 1);
             const int n_rows = 2 * nch + 2 * x.gs() + n_dt;
             float* ring = (float*)(stage + P.st_conv);
             const float* ering = (const float*)(stage + P.st_econv);
-            for (int i = tid; i < n_rows; i += THREADS) {
+            for (int ib = 0; ib < n_rows; ib += THREADS / LPR) {      // warp-uniform trip count (shuffles inside)
+                const int i = min(ib + tid / LPR, n_rows - 1), sub = tid % LPR;
+                const bool valid = ib + tid / LPR < n_rows;
                 int kind, slot = 0, e = 0;         // kind 0 z, 1 x, 2 B|C, 3 dt
                 if (i < nch) { kind = 0; slot = i; }
                 else if (i < 2 * nch) { kind = 1; slot = x.nch_max() + (i - nch); }
@@ -749,18 +758,21 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 const bool own = kind < 2;
                 const int8_t* brow = own ? (const int8_t*)(stage + P.c_in_B) + (size_t)slot * x.r_pad()
                                          : (const int8_t*)(blk + P.b_eB) + (size_t)e * x.r_pad();
+                double lo0 = 0.0, lo1 = 0.0;
+                for (int j4 = 4 * sub; j4 < x.r_pad(); j4 += 4 * LPR) {         // pad entries of B are 0, pad entries of v are 0
+                    const int w = *(const int*)(brow + j4);
+                    lo0 = __fma_rn((double)(int8_t)w, s_vin[j4], lo0);
+                    lo1 = __fma_rn((double)(int8_t)(w >> 8), s_vin[j4 + 1], lo1);
+                    lo0 = __fma_rn((double)(int8_t)(w >> 16), s_vin[j4 + 2], lo0);
+                    lo1 = __fma_rn((double)(w >> 24), s_vin[j4 + 3], lo1);
+                }
+                lo0 += lo1;
+                if (LPR > 1) lo0 += __shfl_xor_sync(0xffffffffu, lo0, 1);
+                if (sub != 0 || !valid) continue;
                 const float scale = own ? ((const float*)(stage + P.c_in_scale))[slot] : ((const float*)(blk + P.b_escale))[e];
                 const float bsv = own ? ((const float*)(stage + P.c_in_bs))[slot] : ((const float*)(blk + P.b_ebs))[e];
                 const int acc = own ? s_acc_in[slot] : s_eacc[e];
-                double lo0 = 0.0, lo1 = 0.0;
-                for (int j4 = 0; j4 < x.r_pad(); j4 += 4) {         // pad entries of B are 0, pad entries of v are 0
-                    const int w = *(const int*)(brow + j4);
-                    lo0 = __fma_rn((double)((int)((unsigned)w << 24) >> 24), s_vin[j4], lo0);
-                    lo1 = __fma_rn((double)((int)((unsigned)w << 16) >> 24), s_vin[j4 + 1], lo1);
-                    lo0 = __fma_rn((double)((int)((unsigned)w << 8) >> 24), s_vin[j4 + 2], lo0);
-                    lo1 = __fma_rn((double)(w >> 24), s_vin[j4 + 3], lo1);
-                }
-                const float lo = (float)(lo0 + lo1);
+                const float lo = (float)lo0;
                 const float val = fmul(s_act, fadd(fmul(scale, (float)acc), fmul(bsv, lo)));
                 int row;                       // canonical in_proj row (for the taps)
                 bool tap_owner = true;
@@ -808,24 +820,17 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         __syncthreads();
         DFSSM_STAMP(l, 4);
 
-        // out_proj LoRA-down partial task of this CTA (warp 0): fetch the weights now, use them after gather G
-        const int et_first = c;
-        const bool tt_first = wid == 0 && et_first < x.n_ttask();
-        int4 pre_out[T_PRE];
-        if (tt_first)
-            trow_prefetch(P.A_out + ((size_t)l * x.r() + et_first / x.tsplit()) * x.d_inner() + (size_t)(et_first % x.tsplit()) * tbytes, tbytes, lane, pre_out);
-
-        // ---- S5 state update + readout, S6 gate: 16 lanes per channel; t = g*w is published as it is produced ----
+        // ---- S5 state update + readout, S6 gate: LPC lanes per channel; t = g*w is published as it is produced ----
         {
             double ss_own = 0.0;
             const int hpg = x.nheads() / x.ngroups();
             const float* alog = (const float*)(stage + P.c_alog);
             const float* Dv = (const float*)(stage + P.c_D);
             const float* gw = (const float*)(stage + P.c_gnorm);
-            const int l16 = tid & 15;
-            for (int ib = 0; ib < nch; ib += THREADS / 16) {         // warp-uniform trip count (shuffles inside)
-                const int i = min(ib + (tid >> 4), nch - 1);
-                const bool valid = ib + (tid >> 4) < nch;
+            const int l16 = tid % LPC;
+            for (int ib = 0; ib < nch; ib += THREADS / LPC) {        // warp-uniform trip count (shuffles inside)
+                const int i = min(ib + tid / LPC, nch - 1);
+                const bool valid = ib + tid / LPC < nch;
                 const int ch = ch0 + i, h = ch / x.headdim(), grp = h / hpg;
                 const float dtv = s_dt[h];
                 const float An = -sp_expf(alog[i]);
@@ -836,7 +841,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 const float* Bc = s_bc + grp * x.d_state();
                 const float* Cc = s_bc + x.gs() + grp * x.d_state();
                 double a = 0.0;
-                for (int n4 = l16; valid && n4 < x.d_state() / 4; n4 += 16) {
+                for (int n4 = l16; valid && n4 < x.d_state() / 4; n4 += LPC) {
                     float4 hv = *(const float4*)(Hr + 4 * n4);
                     const float4 bv = *(const float4*)(Bc + 4 * n4);
                     const float4 cv = *(const float4*)(Cc + 4 * n4);
@@ -848,7 +853,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     a = dacc(a, cv.x, hv.x); a = dacc(a, cv.y, hv.y); a = dacc(a, cv.z, hv.z); a = dacc(a, cv.w, hv.w);
                 }
 #pragma unroll
-                for (int o = 8; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o, 16);
+                for (int o = LPC / 2; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o, LPC);
                 if (l16 == 0 && valid) {
                     a = dacc(a, Dv[i], xv);
                     const float y = (float)a;
@@ -858,22 +863,27 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     if (tp) { ((float*)(tp + P.tl.off[7]))[ch] = y; ((float*)(tp + P.tl.off[8]))[ch] = gv; }
                 }
             }
+            x.stamp(l, 24);
             fence_proxy_async();               // the updated state is about to be read by the async proxy
+            x.stamp(l, 25);
             ss_own = warp_sum(ss_own);
             if (lane == 0) red_d(x)[wid] = ss_own;
             __syncthreads();
+            x.stamp(l, 26);
             slot_store(x, rec, P.x_G, x.g_slot(), [&](int piece) {
                 uint4 w = *(const uint4*)(s_slotG + 4 * piece);
                 const int ex = x.g_dpos() - 4 * piece;
                 if (ex == 0 || ex == 2) {
-                    double tot = 0.0;
+                    double t4[4] = { 0.0, 0.0, 0.0, 0.0 };
 #pragma unroll
-                    for (int i = 0; i < NWARPS; ++i) tot += red_d(x)[i];
+                    for (int i = 0; i < NWARPS; ++i) t4[i & 3] += red_d(x)[i];
+                    const double tot = (t4[0] + t4[1]) + (t4[2] + t4[3]);
                     const uint32_t lo = (uint32_t)__double2loint(tot), hi = (uint32_t)__double2hiint(tot);
                     if (ex == 0) { w.x = lo; w.y = hi; } else { w.z = lo; w.w = hi; }
                 }
                 return w;
             });
+            x.stamp(l, 27);
             if (tid == 0 && nch > 0) {         // write the state slice back (async), while the exchange goes on
                 bulk_s2g(P.ssm + (size_t)l * P.ssm_lstride + (size_t)ch0 * x.d_state(), stage + P.st_ssm, (uint32_t)nch * x.d_state() * 4);
                 bulk_s2g(conv_l + (size_t)ch0 * 4, stage + P.st_conv, (uint32_t)nch * 16);
@@ -886,23 +896,21 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         float s_g;
         int qsum_g;
         {
-            uint4 vg[4];
-            hop_gather<4>(x, mine + P.x_G, x.G() * x.g_slot(), x.g_slot(), x.g_dpos(), vg);
+            uint4 vg[NJ_G];
+            hop_gather<NJ_G>(x, mine + P.x_G, x.G() * x.g_slot(), x.g_slot(), x.g_dpos(), vg);
             DFSSM_STAMP(l, 6);
-            slot_partials<4>(x, vg, x.G(), x.g_slot(), x.g_dpos());
-            qsum_g = norm_quant(x, SlotEnum<4>{ vg, chs, tid, x.G(), x.g_slot() >> 2 }, x.d_inner(), false, s_g,
-                                (tp && c == 0) ? (int8_t*)(tp + P.tl.off[9]) : nullptr);
+            const double ssl = slot_partials<NJ_G>(x, vg, x.G(), x.g_slot(), x.g_dpos());
+            qsum_g = norm_quant(x, SlotEnum<NJ_G>{ vg, chs, tid, x.G(), x.g_slot() >> 2 }, ssl, x.d_inner(), false, s_g,
+                                (tp && c == 0) ? (int8_t*)(tp + P.tl.off[9]) : nullptr, l, 16);
             if (tp && c == 0 && tid == 0) *(float*)(tp + P.tl.off[10]) = s_g;
         }
         DFSSM_STAMP(l, 7);
-        // ---- S7: LoRA-down partial tasks (warp 0, published) and the out_proj sign rows (other warps) ----
+        // ---- S7: LoRA-down partial task (warp 0, published) and the out_proj sign rows (other warps) ----
         if (wid == 0) {
-            for (int e = c; e < x.n_ttask(); e += x.G()) {
-                const int j = e / x.tsplit(), part = e % x.tsplit();
-                const int8_t* arow = P.A_out + ((size_t)l * x.r() + j) * x.d_inner() + (size_t)part * tbytes;
-                if (e != c) trow_prefetch(arow, tbytes, lane, pre_out);
-                const int t = trow_dot(arow, tbytes, xq + (size_t)part * tbytes, lane, pre_out);
-                word_store(x, rec, P.x_T, e, (uint32_t)t ^ IBIAS);
+            if (c < x.n_ttask()) {
+                const int part = c % x.tsplit();
+                const int t = trow_dot(stage + P.st_tout, tbytes, xq + (size_t)part * tbytes, lane);
+                word_store(x, rec, P.x_T, c, (uint32_t)t ^ IBIAS);
             }
         } else {
             const uint32_t* bits = (const uint32_t*)(stage + P.c_out_bits);
@@ -956,7 +964,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 lo += __shfl_xor_sync(0xffffffffu, lo, 1);
                 lo += __shfl_xor_sync(0xffffffffu, lo, 2);
                 if (sub != 0 || !valid) continue;
-                const int p128 = s_acc_out[i] + (KS > 1 ? s_acc_out[x.nor_max() + i] : 0);
+                int p128 = s_acc_out[i];
+                for (int hh = 1; hh < KS; ++hh) p128 += s_acc_out[hh * x.nor_max() + i];
                 const int acc = 2 * (p128 / 128) - qsum_g;       // exact: every term is a multiple of 128
                 const float o = fmul(s_g, fadd(fmul(scale[i], (float)acc), fmul(bsv[i], (float)lo)));
                 const float un = fadd(s_u[i], o);
@@ -972,9 +981,10 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 uint4 w = *(const uint4*)(s_slotU + 4 * piece);
                 const int ex = x.u_dpos() - 4 * piece;
                 if (ex == 0 || ex == 2) {
-                    double tot = 0.0;
+                    double t4[4] = { 0.0, 0.0, 0.0, 0.0 };
 #pragma unroll
-                    for (int i = 0; i < NWARPS; ++i) tot += red_d(x)[i];
+                    for (int i = 0; i < NWARPS; ++i) t4[i & 3] += red_d(x)[i];
+                    const double tot = (t4[0] + t4[1]) + (t4[2] + t4[3]);
                     const uint32_t lo = (uint32_t)__double2loint(tot), hi = (uint32_t)__double2hiint(tot);
                     if (ex == 0) { w.x = lo; w.y = hi; } else { w.z = lo; w.w = hi; }
                 }
@@ -985,18 +995,16 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 if (l + P.stages < n_items) issue_item(x, l + P.stages, v0, v1);
             }
         }
-        if (t_first && l + 1 < P.L)
-            trow_prefetch(P.A_in + ((size_t)(l + 1) * x.r() + (e_first - x.n_bcdt())) * x.d_model(), x.d_model(), lane, pre_in);
         DFSSM_STAMP(l, 10);
         // ---- gather U, S1 of the next layer (or S8's norm) in every CTA ----
         {
-            uint4 vu[2];
-            hop_gather<2>(x, mine + P.x_U, x.G() * x.u_slot(), x.u_slot(), x.u_dpos(), vu);
+            uint4 vu[NJ_U];
+            hop_gather<NJ_U>(x, mine + P.x_U, x.G() * x.u_slot(), x.u_slot(), x.u_dpos(), vu);
             DFSSM_STAMP(l, 11);
-            slot_partials<2>(x, vu, x.G(), x.u_slot(), x.u_dpos());
+            const double ssl = slot_partials<NJ_U>(x, vu, x.G(), x.u_slot(), x.u_dpos());
             uint8_t* tpn = (taps_on && c == 0 && l + 1 < P.L) ? P.taps + (size_t)(l + 1) * P.tap_lstride : nullptr;
-            qsum = norm_quant(x, SlotEnum<2>{ vu, ors, tid, x.G(), x.u_slot() >> 2 }, x.d_model(), l == P.L - 1, s_act,
-                              tpn ? (int8_t*)(tpn + P.tl.off[0]) : nullptr);
+            qsum = norm_quant(x, SlotEnum<NJ_U>{ vu, ors, tid, x.G(), x.u_slot() >> 2 }, ssl, x.d_model(), l == P.L - 1, s_act,
+                              tpn ? (int8_t*)(tpn + P.tl.off[0]) : nullptr, l, 20);
             if (tpn && tid == 0) *(float*)(tpn + P.tl.off[1]) = s_act;
         }
         DFSSM_STAMP(l, 12);
@@ -1005,7 +1013,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
     // =============================================== S8 LM head ===============================================
     for (int i = tid; i < nor; i += THREADS) P.u_out[or0 + i] = s_u[i];
     DFSSM_STAMP(P.L, 0);
-    if (P.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + P.L) * PROF_NPH + 15] = globaltimer_ns();
+    if (P.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + P.L) * PROF_NPH + 31] = globaltimer_ns();
     float best = -INFINITY;
     int besti = 0x7fffffff;
     for (int it = 0; it < n_lm_items; ++it) {

@@ -26,7 +26,7 @@ inline bool plan(const Dims& d, int G, Params& P)
     P.eps = d.eps;
     P.G = G;
     if (d.d_state % 4 || d.d_model % 32 || d.d_inner % 32 || d.r > 64 || (G & 1)) return false;
-    if (d.d_model > 16 * THREADS || d.d_inner > 16 * THREADS) return false;       // 4 chunks of 4 words per thread
+    if (d.d_model > 8192 || d.d_inner > 8192) return false;
     P.nch_max = (d.d_inner + G - 1) / G;
     P.nor_max = (d.d_model + G - 1) / G;
     P.nb_max = (P.n_bcdt + G - 1) / G;
@@ -35,7 +35,7 @@ inline bool plan(const Dims& d, int G, Params& P)
     P.Win = d.d_model / 32;
     P.Wout = d.d_inner / 32;
     P.n_early = P.n_bcdt + d.r;
-    if (P.n_early > 8 * THREADS || P.n_early > 64 * G) return false;
+    if (P.n_early > 4096 || P.n_early > 64 * G || d.r > G) return false;
     P.tsplit = (d.d_inner % 64 == 0 && 4 * d.r <= G) ? 4 : (2 * d.r <= G ? 2 : 1);
     P.n_ttask = d.r * P.tsplit;
     if (P.nch_max > 128 || P.nor_max > 128 || d.d_inner < G || d.d_model < G) return false;
@@ -73,7 +73,9 @@ inline bool plan(const Dims& d, int G, Params& P)
     P.st_ssm = P.st_blk + P.blk_bytes;
     P.st_conv = up32(P.st_ssm + (uint32_t)P.nch_max * d.d_state * 4, 128);
     P.st_econv = up32(P.st_conv + (uint32_t)P.nch_max * 16, 128);
-    P.stage_bytes = up32(P.st_econv + (uint32_t)P.gs * 32, 128);
+    P.st_tin = up32(P.st_econv + (uint32_t)P.gs * 32, 128);
+    P.st_tout = up32(P.st_tin + (uint32_t)d.d_model, 128);
+    P.stage_bytes = up32(P.st_tout + (uint32_t)(d.d_inner / P.tsplit), 128);
     if (P.stage_bytes < 4u * d.d_model) P.stage_bytes = up32(4u * d.d_model, 128);      // an LM item holds >= 4 rows
     P.lm_rows_item = (int)(P.stage_bytes / d.d_model);
 
@@ -85,7 +87,7 @@ inline bool plan(const Dims& d, int G, Params& P)
     P.u_slot = (P.u_dpos + 2 + 3) / 4 * 4;
     P.g_dpos = (P.nch_max + 1) / 2 * 2;
     P.g_slot = (P.g_dpos + 2 + 3) / 4 * 4;
-    if (G * P.u_slot / 4 > 2 * THREADS || G * P.g_slot / 4 > 4 * THREADS) return false;
+    if (G * P.u_slot / 4 > NJ_U * THREADS || G * P.g_slot / 4 > NJ_G * THREADS) return false;
     if (P.u_slot + P.g_slot > THREADS) return false;
     uint32_t xo = 0;
     auto xtake = [&](size_t words) { xo = up32(xo, 32); const uint32_t at = xo; xo += (uint32_t)words; return at; };
@@ -102,8 +104,8 @@ inline bool plan(const Dims& d, int G, Params& P)
     const uint32_t x_xq = stake(kmax), x_bc = stake((size_t)2 * P.gs * 4), x_u = stake((size_t)P.nor_max * 4),
                    x_z = stake((size_t)P.nch_max * 4), x_x = stake((size_t)P.nch_max * 4), x_dt = stake((size_t)d.nheads * 4),
                    x_v = stake((size_t)2 * P.r_pad * 8), x_ea = stake((size_t)P.n_bcdt * 4), x_ai = stake((size_t)P.n_slots * 4),
-                   x_ao = stake((size_t)2 * P.nor_max * 4), x_chs = stake((size_t)(G + 1) * 4), x_ors = stake((size_t)(G + 1) * 4),
-                   x_part = stake((size_t)(G + 2) * 8), x_red = stake(256), x_slot = stake((size_t)(P.u_slot + P.g_slot) * 4),
+                   x_ao = stake((size_t)KS_MAX * P.nor_max * 4), x_chs = stake((size_t)(G + 1) * 4), x_ors = stake((size_t)(G + 1) * 4),
+                   x_part = stake((size_t)(G + 2) * 8), x_red = stake(16 * NWARPS), x_slot = stake((size_t)(P.u_slot + P.g_slot) * 4),
                    x_mbar = stake(8 * MAX_STAGES);
     const uint32_t fixed = up32(so, 128);
     if (fixed + 2 * (size_t)P.stage_bytes > SMEM_LIMIT) return false;
@@ -158,8 +160,30 @@ inline float half_bits_to_float(uint16_t h)     // exact binary16 -> binary32 (h
 
 inline int plane_pos_host(int k, int K)
 {
-    const int w = k >> 5, p = k & 31, j = p >> 3, i = p & 7;
-    return (i < 4 ? 0 : (K >> 1)) + 16 * w + 4 * (i & 3) + j;
+    return ((k & 16) ? (K >> 1) : 0) + ((k >> 5) << 4) + (k & 15);
+}
+
+// canonical sign word (bit p = element p of the 32-block) -> kernel sign word (bit 8j + i = element 4i + j)
+inline uint32_t permute_sign_word(uint32_t w)
+{
+    uint32_t o = 0;
+    for (int p = 0; p < 32; ++p)
+        if ((w >> p) & 1u) o |= 1u << (8 * (p & 3) + (p >> 2));
+    return o;
+}
+struct SignLut {
+    uint32_t t[4][256];
+    SignLut()
+    {
+        for (int b = 0; b < 4; ++b)
+            for (int v = 0; v < 256; ++v) t[b][v] = permute_sign_word((uint32_t)v << (8 * b));
+    }
+    uint32_t operator()(uint32_t w) const { return t[0][w & 255u] | t[1][(w >> 8) & 255u] | t[2][(w >> 16) & 255u] | t[3][w >> 24]; }
+};
+inline void copy_sign_row(uint32_t* dst, const uint32_t* src, int W)
+{
+    static const SignLut lut;
+    for (int w = 0; w < W; ++w) dst[w] = lut(src[w]);
 }
 
 // host pointers to one layer of the canonical blob
@@ -182,7 +206,7 @@ inline void pack_chunk(const Params& P, const HostLayer& H, const float* next_no
     const int ch0 = (int)(((long long)c * P.d_inner) / G), nch = (int)(((long long)(c + 1) * P.d_inner) / G) - ch0;
     const int or0 = (int)(((long long)c * P.d_model) / G), nor = (int)(((long long)(c + 1) * P.d_model) / G) - or0;
     auto put_in_row = [&](int slot, int row) {
-        memcpy(out + P.c_in_bits + (size_t)slot * P.Win * 4, H.in_sign + (size_t)row * P.Win, (size_t)P.Win * 4);
+        copy_sign_row((uint32_t*)(out + P.c_in_bits + (size_t)slot * P.Win * 4), H.in_sign + (size_t)row * P.Win, P.Win);
         memcpy(out + P.c_in_B + (size_t)slot * P.r_pad, H.in_B + (size_t)row * P.r, P.r);
         ((float*)(out + P.c_in_scale))[slot] = half_bits_to_float(H.in_row_scale[row]);
         ((float*)(out + P.c_in_bs))[slot] = H.in_b_s[row];
@@ -198,10 +222,10 @@ inline void pack_chunk(const Params& P, const HostLayer& H, const float* next_no
         ((float*)(out + P.c_gnorm))[i] = H.gnorm_w[ch];
     }
     for (int k = 0, e = c; e < P.n_bcdt; ++k, e += G)        // early sign rows: B | C | dt (their epilogue data is in the block)
-        memcpy(out + P.c_in_bits + (size_t)(2 * P.nch_max + k) * P.Win * 4, H.in_sign + (size_t)(2 * P.d_inner + e) * P.Win, (size_t)P.Win * 4);
+        copy_sign_row((uint32_t*)(out + P.c_in_bits + (size_t)(2 * P.nch_max + k) * P.Win * 4), H.in_sign + (size_t)(2 * P.d_inner + e) * P.Win, P.Win);
     for (int i = 0; i < nor; ++i) {
         const int row = or0 + i;
-        memcpy(out + P.c_out_bits + (size_t)i * P.Wout * 4, H.out_sign + (size_t)row * P.Wout, (size_t)P.Wout * 4);
+        copy_sign_row((uint32_t*)(out + P.c_out_bits + (size_t)i * P.Wout * 4), H.out_sign + (size_t)row * P.Wout, P.Wout);
         memcpy(out + P.c_out_B + (size_t)i * P.r_pad, H.out_B + (size_t)row * P.r, P.r);
         ((float*)(out + P.c_out_scale))[i] = half_bits_to_float(H.out_row_scale[row]);
         ((float*)(out + P.c_out_bs))[i] = H.out_b_s[row];
