@@ -37,6 +37,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 #include "dfssm_kernels.cuh"
 #include "dfssm_math.cuh"
 
@@ -253,24 +255,25 @@ __device__ __forceinline__ void poll_fail(const Ctx<S>& x)
 // Thread t owns the 16-byte chunks t, t + THREADS, ... (at most NJ) of the nw 32-bit words at buf.  Words
 // behind nw count as valid.  If slot_w > 0 the buffer is a sequence of slots of slot_w words whose word dpos is
 // the low half of an fp64 (any bit pattern: exempt; its high half at dpos + 1 validates it).
-// Spins until every owned word has been written; the raw words come back in v[].
+// Spins until every owned word has been written; the raw words come back in v[].  tix = the thread's index for
+// the chunk ownership (tid, or reversed so that the small gathers are polled by the warps that have nothing else to do).
 template <int NJ, class S>
-__device__ __forceinline__ void hop_gather(const Ctx<S>& x, const uint32_t* buf, int nw, int slot_w, int dpos, uint4 (&v)[NJ])
+__device__ __forceinline__ void hop_gather(const Ctx<S>& x, const uint32_t* buf, int nw, int slot_w, int dpos, uint4 (&v)[NJ], int tix)
 {
     const int nchunk = (nw + 3) >> 2;
     bool need[NJ];
 #pragma unroll
-    for (int j = 0; j < NJ; ++j) need[j] = x.tid + j * THREADS < nchunk;
+    for (int j = 0; j < NJ; ++j) need[j] = tix + j * THREADS < nchunk;
     uint32_t spins = 0;
     for (;;) {
 #pragma unroll
         for (int j = 0; j < NJ; ++j)
-            if (need[j]) v[j] = x_ld128(buf + 4 * (x.tid + j * THREADS));
+            if (need[j]) v[j] = x_ld128(buf + 4 * (tix + j * THREADS));
         bool all = true;
 #pragma unroll
         for (int j = 0; j < NJ; ++j)
             if (need[j]) {
-                const int base = 4 * (x.tid + j * THREADS);
+                const int base = 4 * (tix + j * THREADS);
                 const int ex = slot_w > 0 ? dpos - base % slot_w : -1;      // index of the exempt word inside this chunk
                 const bool ok = (v[j].x != SENT || ex == 0) && (base + 1 >= nw || v[j].y != SENT) &&
                                 (base + 2 >= nw || v[j].z != SENT || ex == 2) && (base + 3 >= nw || v[j].w != SENT);
@@ -612,6 +615,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
     const bool taps_on = TAPS && P.taps != nullptr;
     const size_t rec_words = (size_t)x.M() * P.x_words;
     const int mbox = c / x.gsz();                      // the mailbox this CTA polls
+    const int rtid = THREADS - 1 - tid;              // the small gathers (A, T) are polled from the last warp down
     uint32_t* s_slotU = (uint32_t*)(sm + P.s_slot);
     uint32_t* s_slotG = s_slotU + x.u_slot();
     if (tid < x.u_slot() + x.g_slot()) s_slotU[tid] = 0u;      // pad words of the slots are published as 0
@@ -670,13 +674,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         uint32_t* recc = P.xbuf + (size_t)((P.rec0 + (uint32_t)l + 2u) & 3u) * rec_words;     // reset for layer l + 2
         DFSSM_STAMP(l, 0);
         if (P.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + 31] = globaltimer_ns();
-        {   // reset own slots of the record two layers ahead (same thread -> address map as the publishes below)
-            slot_store(x, recc, P.x_U, x.u_slot(), [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
-            slot_store(x, recc, P.x_G, x.g_slot(), [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
-            for (int k = wid; k < nb_tasks; k += NWARPS) word_store(x, recc, P.x_A, c + k * x.G(), SENT);
-            if (wid == 0 && c < x.n_ttask()) word_store(x, recc, P.x_T, c, SENT);
-        }
-
         wait_item(x, l);
         DFSSM_STAMP(l, 1);
         // ---- early tasks: B|C|dt sign rows and LoRA-down rows of this CTA; raw int32 results are published ----
@@ -719,14 +716,22 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             }
         }
         DFSSM_STAMP(l, 2);
+        {   // reset own slots of the record two layers ahead (same thread -> address map as the publishes); the warps
+            // that do it are not the ones polling A, so this costs nothing on the critical path
+            slot_store(x, recc, P.x_U, x.u_slot(), [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
+            slot_store(x, recc, P.x_G, x.g_slot(), [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
+            for (int k = wid; k < nb_tasks; k += NWARPS) word_store(x, recc, P.x_A, c + k * x.G(), SENT);
+            if (wid == 0 && c < x.n_ttask()) word_store(x, recc, P.x_T, c, SENT);
+        }
+
         // ---- gather A: accumulators of all B|C|dt rows and t_in;  v_j = a_s[j] * float(t_j) ----
         {
             uint4 va[NJ_A];
-            hop_gather<NJ_A>(x, mine + P.x_A, x.n_early(), 0, 0, va);
+            hop_gather<NJ_A>(x, mine + P.x_A, x.n_early(), 0, 0, va, rtid);
             const float* a_s = (const float*)(blk + P.b_as_in);
 #pragma unroll
             for (int j = 0; j < NJ_A; ++j) {
-                const int e0 = 4 * (tid + j * THREADS);
+                const int e0 = 4 * (rtid + j * THREADS);
                 const uint32_t w[4] = { va[j].x, va[j].y, va[j].z, va[j].w };
 #pragma unroll
                 for (int i = 0; i < 4; ++i) {
@@ -747,9 +752,15 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             const int n_rows = 2 * nch + 2 * x.gs() + n_dt;
             float* ring = (float*)(stage + P.st_conv);
             const float* ering = (const float*)(stage + P.st_econv);
-            for (int ib = 0; ib < n_rows; ib += THREADS / LPR) {      // warp-uniform trip count (shuffles inside)
-                const int i = min(ib + tid / LPR, n_rows - 1), sub = tid % LPR;
-                const bool valid = ib + tid / LPR < n_rows;
+            // rows [first, first + count) of the index space (z | x | B|C | dt), skipping skip_len rows from skip_from on;
+            // LP lanes share a row's LoRA sum
+            auto epi = [&](auto lp_tag, int first, int count, int skip_from, int skip_len) {
+              constexpr int LP = decltype(lp_tag)::value;
+              for (int ib = 0; ib < count; ib += THREADS / LP) {       // warp-uniform trip count (shuffles inside)
+                int i = first + min(ib + tid / LP, count - 1);
+                if (i >= skip_from) i += skip_len;
+                const int sub = tid % LP;
+                const bool valid = ib + tid / LP < count;
                 int kind, slot = 0, e = 0;         // kind 0 z, 1 x, 2 B|C, 3 dt
                 if (i < nch) { kind = 0; slot = i; }
                 else if (i < 2 * nch) { kind = 1; slot = x.nch_max() + (i - nch); }
@@ -759,7 +770,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 const int8_t* brow = own ? (const int8_t*)(stage + P.c_in_B) + (size_t)slot * x.r_pad()
                                          : (const int8_t*)(blk + P.b_eB) + (size_t)e * x.r_pad();
                 double lo0 = 0.0, lo1 = 0.0;
-                for (int j4 = 4 * sub; j4 < x.r_pad(); j4 += 4 * LPR) {         // pad entries of B are 0, pad entries of v are 0
+                for (int j4 = 4 * sub; j4 < x.r_pad(); j4 += 4 * LP) {         // pad entries of B are 0, pad entries of v are 0
                     const int w = *(const int*)(brow + j4);
                     lo0 = __fma_rn((double)(int8_t)w, s_vin[j4], lo0);
                     lo1 = __fma_rn((double)(int8_t)(w >> 8), s_vin[j4 + 1], lo1);
@@ -767,7 +778,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     lo1 = __fma_rn((double)(w >> 24), s_vin[j4 + 3], lo1);
                 }
                 lo0 += lo1;
-                if (LPR > 1) lo0 += __shfl_xor_sync(0xffffffffu, lo0, 1);
+#pragma unroll
+                for (int o = LP / 2; o > 0; o >>= 1) lo0 += __shfl_xor_sync(0xffffffffu, lo0, o);
                 if (sub != 0 || !valid) continue;
                 const float scale = own ? ((const float*)(stage + P.c_in_scale))[slot] : ((const float*)(blk + P.b_escale))[e];
                 const float bsv = own ? ((const float*)(stage + P.c_in_bs))[slot] : ((const float*)(blk + P.b_ebs))[e];
@@ -815,7 +827,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     ((float*)(tp + P.tl.off[4]))[row] = val;
                     ((int32_t*)(tp + P.tl.off[2]))[row] = acc;
                 }
-            }
+              }
+            };
+            // the 2 gs B|C rows with 2 lanes each, then the few own rows (z, x, dt) with 8 lanes each
+            epi(std::integral_constant<int, 2>{}, 2 * nch, 2 * x.gs(), 1 << 30, 0);
+            epi(std::integral_constant<int, 8>{}, 0, 2 * nch + n_dt, 2 * nch, 2 * x.gs());
         }
         __syncthreads();
         DFSSM_STAMP(l, 4);
@@ -897,7 +913,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         int qsum_g;
         {
             uint4 vg[NJ_G];
-            hop_gather<NJ_G>(x, mine + P.x_G, x.G() * x.g_slot(), x.g_slot(), x.g_dpos(), vg);
+            hop_gather<NJ_G>(x, mine + P.x_G, x.G() * x.g_slot(), x.g_slot(), x.g_dpos(), vg, tid);
             DFSSM_STAMP(l, 6);
             const double ssl = slot_partials<NJ_G>(x, vg, x.G(), x.g_slot(), x.g_dpos());
             qsum_g = norm_quant(x, SlotEnum<NJ_G>{ vg, chs, tid, x.G(), x.g_slot() >> 2 }, ssl, x.d_inner(), false, s_g,
@@ -930,13 +946,13 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         // ---- gather T: t_out = sum of the partial sums;  v_j = a_s[j] * float(t_j) ----
         {
             uint4 vt[1];
-            hop_gather<1>(x, mine + P.x_T, x.n_ttask(), 0, 0, vt);
+            hop_gather<1>(x, mine + P.x_T, x.n_ttask(), 0, 0, vt, rtid);
             const float* a_s = (const float*)(blk + P.b_as_out);
             const uint32_t w[4] = { vt[0].x, vt[0].y, vt[0].z, vt[0].w };
             const int rows_per_chunk = 4 / x.tsplit();
 #pragma unroll
             for (int jj = 0; jj < 4; ++jj) {
-                const int j = tid * rows_per_chunk + jj;
+                const int j = rtid * rows_per_chunk + jj;
                 if (jj < rows_per_chunk && j < x.r()) {
                     int t = 0;
                     for (int q = 0; q < x.tsplit(); ++q) t += (int)(w[jj * x.tsplit() + q] ^ IBIAS);
@@ -999,7 +1015,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         // ---- gather U, S1 of the next layer (or S8's norm) in every CTA ----
         {
             uint4 vu[NJ_U];
-            hop_gather<NJ_U>(x, mine + P.x_U, x.G() * x.u_slot(), x.u_slot(), x.u_dpos(), vu);
+            hop_gather<NJ_U>(x, mine + P.x_U, x.G() * x.u_slot(), x.u_slot(), x.u_dpos(), vu, tid);
             DFSSM_STAMP(l, 11);
             const double ssl = slot_partials<NJ_U>(x, vu, x.G(), x.u_slot(), x.u_dpos());
             uint8_t* tpn = (taps_on && c == 0 && l + 1 < P.L) ? P.taps + (size_t)(l + 1) * P.tap_lstride : nullptr;
