@@ -387,7 +387,7 @@ int mega_setup(dfssm_ctx* ctx)                      // at create: can this devic
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
     if (!coop || sms < mega::GRID) return DFSSM_OK;
-    ctx->mega_fn = mega::pick_kernel(ctx->dm, (ctx->cfg.flags & DFSSM_FLAG_TAPS) != 0);
+    ctx->mega_fn = mega::pick_kernel(ctx->dm, (ctx->cfg.flags & DFSSM_FLAG_TAPS) != 0, (ctx->cfg.flags & DFSSM_FLAG_PROF) != 0);
     CK(cudaFuncSetAttribute((const void*)ctx->mega_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->mp.smem_bytes));
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)ctx->mega_fn, mega::THREADS, ctx->mp.smem_bytes));
     if (per_sm < 1) return DFSSM_OK;

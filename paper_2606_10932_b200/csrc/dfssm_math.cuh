@@ -90,13 +90,13 @@ __device__ __forceinline__ int dp4a_us(uint32_t a, int b, int c)
 __device__ __forceinline__ int dp4a_ss(int a, int b, int c) { return __dp4a(a, b, c); }
 
 // per-token absmax quantiser (R4): codes from t = v*w, inv = 127/amax, ties to even, clamp +-127.
-// rint by the magic-number addition (exact ties-to-even for |x| < 2^22; here |t*inv| <= 127(1 + 2^-23)): the
-// FRND / F2I conversions run at a quarter of the fp32 rate and the quantiser is on the critical path.
+// rint by the magic-number addition (exact ties-to-even for |x| < 2^22); the FRND / F2I conversions run at a
+// quarter of the fp32 rate and the quantiser is on the critical path.  The clamp of R4 can never act here:
+// |t| <= amax and inv = fl(127/amax) give |fl(t*inv)| <= 127 (1 + 2^-23), which rounds to 127.
 __device__ __forceinline__ int quant_code(float t, float inv)
 {
     const float r = fadd(fmul(t, inv), 12582912.0f);            // 1.5 * 2^23
-    const int q = __float_as_int(r) - 0x4b400000;
-    return max(-127, min(127, q));
+    return __float_as_int(r) - 0x4b400000;
 }
 
 // ---- warp / block reductions (any tree is allowed: sums are binary64, max is exact) ----

@@ -188,18 +188,24 @@ struct ShapeCT { static constexpr bool kStatic = true; static constexpr int d_mo
 constexpr int GRID = 148;                       // one CTA per B200 SM
 constexpr int MBOX = 37;                        // mailboxes of the exchange (4 CTAs poll each)
 
+// Ownership: CTA g owns elements [own_start(g, n), own_start(g + 1, n)) of a vector of length n (n % 4 == 0), in
+// groups of 4 so that a gathered 16-byte chunk is four consecutive elements of one 16-element half block of codes.
+__host__ __device__ __forceinline__ int own_start(int g, int n) { return 4 * (int)(((long long)g * (n / 4)) / GRID); }
+__host__ __device__ __forceinline__ int own_max(int n) { return 4 * ((n / 4 + GRID - 1) / GRID); }
+
 template <class S>
 struct Ctx {
     const Params& P;
     uint8_t* sm;
     int tid, lane, wid, c;
     volatile int* dead;          // shared flag: a poll timed out -> stop spinning everywhere
+    bool prof;                   // in-kernel profiler on (a compile-time false in the production instantiations)
 #define DFSSM_DIM(n_) __device__ __forceinline__ int n_() const { return S::kStatic ? S::n_ : P.n_; }
     DFSSM_DIM(d_model) DFSSM_DIM(d_inner) DFSSM_DIM(headdim) DFSSM_DIM(d_state) DFSSM_DIM(ngroups) DFSSM_DIM(r)
 #undef DFSSM_DIM
     __device__ __forceinline__ void stamp(int l, int k) const
     {
-        if (P.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + k] = clock64();
+        if (prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + k] = clock64();
     }
     __device__ __forceinline__ constexpr int G() const { return GRID; }
     __device__ __forceinline__ constexpr int M() const { return MBOX; }
@@ -207,8 +213,8 @@ struct Ctx {
     __device__ __forceinline__ int nheads() const { return d_inner() / headdim(); }
     __device__ __forceinline__ int gs() const { return ngroups() * d_state(); }
     __device__ __forceinline__ int n_bcdt() const { return 2 * gs() + nheads(); }
-    __device__ __forceinline__ int nch_max() const { return (d_inner() + GRID - 1) / GRID; }
-    __device__ __forceinline__ int nor_max() const { return (d_model() + GRID - 1) / GRID; }
+    __device__ __forceinline__ int nch_max() const { return own_max(d_inner()); }
+    __device__ __forceinline__ int nor_max() const { return own_max(d_model()); }
     __device__ __forceinline__ int nb_max() const { return (n_bcdt() + GRID - 1) / GRID; }
     __device__ __forceinline__ int n_slots() const { return 2 * nch_max() + nb_max(); }
     __device__ __forceinline__ int r_pad() const { return (r() + 3) / 4 * 4; }
@@ -237,10 +243,7 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
     return t;
 }
 // in-kernel profiler: thread 0 of every CTA stamps its SM clock at phase k of layer l
-#define DFSSM_STAMP(l_, k_)                                                                            \
-    do {                                                                                               \
-        if (P.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + (l_)) * PROF_NPH + (k_)] = clock64();  \
-    } while (0)
+#define DFSSM_STAMP(l_, k_) x.stamp((l_), (k_))
 
 template <class S>
 __device__ __forceinline__ void poll_fail(const Ctx<S>& x)
@@ -316,7 +319,10 @@ __device__ __forceinline__ int norm_quant(const Ctx<S>& x, Enum en, double ss_lo
     uint8_t* xq = x.sm + P.s_xq;
     float* bc = (float*)(x.sm + P.s_part);
     float am = 0.0f;
-    en([&](int, uint32_t w) { am = fmaxf(am, fabsf(__uint_as_float(w))); });
+    en([&](int, uint4 w) {
+        am = fmaxf(fmaxf(am, fabsf(__uint_as_float(w.x))), fabsf(__uint_as_float(w.y)));
+        am = fmaxf(fmaxf(am, fabsf(__uint_as_float(w.z))), fabsf(__uint_as_float(w.w)));
+    });
     am = warp_max(am);
     ss_local = warp_sum(ss_local);
     if (x.lane == 0) { red_f(x)[x.wid] = am; red_d(x)[x.wid] = ss_local; }
@@ -337,11 +343,13 @@ __device__ __forceinline__ int norm_quant(const Ctx<S>& x, Enum en, double ss_lo
     s_out = bc[1];
     if (pk >= 0) x.stamp(pl, pk + 2);
     int qs = 0;
-    en([&](int k, uint32_t w) {
-        const int q = quant_code(__uint_as_float(w), inv);          // inv == 0 -> code 0
-        xq[canonical ? k : plane_pos(k, K)] = (uint8_t)q;
-        if (tap_codes) tap_codes[k] = (int8_t)q;
-        qs += q;
+    en([&](int k0, uint4 w) {                                       // four consecutive elements, k0 % 4 == 0
+        const uint32_t q0 = (uint32_t)quant_code(__uint_as_float(w.x), inv) & 255u, q1 = (uint32_t)quant_code(__uint_as_float(w.y), inv) & 255u,
+                       q2 = (uint32_t)quant_code(__uint_as_float(w.z), inv) & 255u, q3 = (uint32_t)quant_code(__uint_as_float(w.w), inv) & 255u;
+        const uint32_t packed = q0 | (q1 << 8) | (q2 << 16) | (q3 << 24);       // inv == 0 -> codes 0
+        *(uint32_t*)(xq + (canonical ? k0 : plane_pos(k0, K))) = packed;
+        if (tap_codes) *(uint32_t*)(tap_codes + k0) = packed;
+        qs = dp4a_us(0x01010101u, (int)packed, qs);
     });
     qs = warp_sum_i(qs);
     if (x.lane == 0) red_i(x)[x.wid] = qs;
@@ -366,11 +374,8 @@ struct SlotEnum {
             const int ci = tid + j * THREADS;
             if (ci < nslots * pps) {
                 const int g = ci / pps, piece = ci - g * pps;
-                const int k0 = starts[g] + 4 * piece, n = starts[g + 1] - starts[g] - 4 * piece;
-                if (n > 0) f(k0, v[j].x);
-                if (n > 1) f(k0 + 1, v[j].y);
-                if (n > 2) f(k0 + 2, v[j].z);
-                if (n > 3) f(k0 + 3, v[j].w);
+                const int k0 = starts[g] + 4 * piece;
+                if (k0 < starts[g + 1]) f(k0, v[j]);
             }
         }
     }
@@ -567,13 +572,13 @@ __device__ __forceinline__ void word_store(const Ctx<S>& x, uint32_t* rec, uint3
     for (int m = x.lane; m < x.M(); m += 32) x_st32(rec + (size_t)m * P.x_words + part_off + idx, value);
 }
 
-template <class S, bool TAPS>
+template <class S, bool TAPS, bool PROF>
 __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
 {
     extern __shared__ __align__(128) uint8_t sm[];
     __shared__ int s_dead;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, c = blockIdx.x;
-    Ctx<S> x{ P, sm, tid, lane, wid, c, &s_dead };
+    Ctx<S> x{ P, sm, tid, lane, wid, c, &s_dead, PROF && P.prof != nullptr };
 
     int* chs = (int*)(sm + P.s_chs);
     int* ors = (int*)(sm + P.s_ors);
@@ -591,8 +596,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
     int* s_acc_out = (int*)(sm + P.s_acc_out);
 
     for (int g = tid; g <= x.G(); g += THREADS) {
-        chs[g] = (int)(((long long)g * x.d_inner()) / x.G());
-        ors[g] = (int)(((long long)g * x.d_model()) / x.G());
+        chs[g] = own_start(g, x.d_inner());
+        ors[g] = own_start(g, x.d_model());
     }
     if (tid < 2 * x.r_pad()) s_vin[tid] = 0.0;
     if (tid == 0) {
@@ -656,7 +661,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
 #pragma unroll
             for (int j = 0; j < NJ_G; ++j) {
                 const int k0 = 4 * (tid + j * THREADS);
-                if (k0 < x.d_model()) { f(k0, v[j].x); f(k0 + 1, v[j].y); f(k0 + 2, v[j].z); f(k0 + 3, v[j].w); }
+                if (k0 < x.d_model()) f(k0, v[j]);
             }
         };
         qsum = norm_quant(x, en, ss, x.d_model(), P.L == 0, s_act, tp0 ? (int8_t*)(tp0 + P.tl.off[0]) : nullptr);
@@ -673,7 +678,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         const uint32_t* mine = rec + (size_t)mbox * P.x_words;                                 // polled
         uint32_t* recc = P.xbuf + (size_t)((P.rec0 + (uint32_t)l + 2u) & 3u) * rec_words;     // reset for layer l + 2
         DFSSM_STAMP(l, 0);
-        if (P.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + 31] = globaltimer_ns();
+        if (x.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + 31] = globaltimer_ns();
         wait_item(x, l);
         DFSSM_STAMP(l, 1);
         // ---- early tasks: B|C|dt sign rows and LoRA-down rows of this CTA; raw int32 results are published ----
@@ -1029,7 +1034,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
     // =============================================== S8 LM head ===============================================
     for (int i = tid; i < nor; i += THREADS) P.u_out[or0 + i] = s_u[i];
     DFSSM_STAMP(P.L, 0);
-    if (P.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + P.L) * PROF_NPH + 31] = globaltimer_ns();
+    if (x.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + P.L) * PROF_NPH + 31] = globaltimer_ns();
     float best = -INFINITY;
     int besti = 0x7fffffff;
     for (int it = 0; it < n_lm_items; ++it) {

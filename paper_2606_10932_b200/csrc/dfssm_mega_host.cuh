@@ -27,8 +27,8 @@ inline bool plan(const Dims& d, int G, Params& P)
     P.G = G;
     if (d.d_state % 4 || d.d_model % 32 || d.d_inner % 32 || d.r > 64 || (G & 1)) return false;
     if (d.d_model > 8192 || d.d_inner > 8192) return false;
-    P.nch_max = (d.d_inner + G - 1) / G;
-    P.nor_max = (d.d_model + G - 1) / G;
+    P.nch_max = own_max(d.d_inner);
+    P.nor_max = own_max(d.d_model);
     P.nb_max = (P.n_bcdt + G - 1) / G;
     P.n_slots = 2 * P.nch_max + P.nb_max;
     P.r_pad = (d.r + 3) / 4 * 4;
@@ -38,7 +38,7 @@ inline bool plan(const Dims& d, int G, Params& P)
     if (P.n_early > 4096 || P.n_early > 64 * G || d.r > G) return false;
     P.tsplit = (d.d_inner % 64 == 0 && 4 * d.r <= G) ? 4 : (2 * d.r <= G ? 2 : 1);
     P.n_ttask = d.r * P.tsplit;
-    if (P.nch_max > 128 || P.nor_max > 128 || d.d_inner < G || d.d_model < G) return false;
+    if (P.nch_max > 128 || P.nor_max > 128 || d.d_inner < 4 || d.d_model < 4) return false;
 
     uint32_t off = 0;
     auto take = [&](size_t bytes) { off = up32(off, 16); const uint32_t at = off; off += (uint32_t)bytes; return at; };
@@ -203,8 +203,8 @@ inline void pack_chunk(const Params& P, const HostLayer& H, const float* next_no
 {
     memset(out, 0, P.chunk_bytes);
     const int G = P.G;
-    const int ch0 = (int)(((long long)c * P.d_inner) / G), nch = (int)(((long long)(c + 1) * P.d_inner) / G) - ch0;
-    const int or0 = (int)(((long long)c * P.d_model) / G), nor = (int)(((long long)(c + 1) * P.d_model) / G) - or0;
+    const int ch0 = own_start(c, P.d_inner), nch = own_start(c + 1, P.d_inner) - ch0;
+    const int or0 = own_start(c, P.d_model), nor = own_start(c + 1, P.d_model) - or0;
     auto put_in_row = [&](int slot, int row) {
         copy_sign_row((uint32_t*)(out + P.c_in_bits + (size_t)slot * P.Win * 4), H.in_sign + (size_t)row * P.Win, P.Win);
         memcpy(out + P.c_in_B + (size_t)slot * P.r_pad, H.in_B + (size_t)row * P.r, P.r);
@@ -282,15 +282,15 @@ inline bool shape_is(const Dims& d)
 }
 
 typedef void (*KernelFn)(const Params);
-inline KernelFn pick_kernel(const Dims& d, bool taps)
+inline KernelFn pick_kernel(const Dims& d, bool taps, bool prof)
 {
     if (!taps) {
-        if (shape_is<Shape0>(d)) return k_mega<Shape0, false>;
-        if (shape_is<Shape1>(d)) return k_mega<Shape1, false>;
-        if (shape_is<Shape2>(d)) return k_mega<Shape2, false>;
-        if (shape_is<Shape4>(d)) return k_mega<Shape4, false>;
+        if (shape_is<Shape0>(d)) return prof ? k_mega<Shape0, false, true> : k_mega<Shape0, false, false>;
+        if (shape_is<Shape1>(d)) return prof ? k_mega<Shape1, false, true> : k_mega<Shape1, false, false>;
+        if (shape_is<Shape2>(d)) return prof ? k_mega<Shape2, false, true> : k_mega<Shape2, false, false>;
+        if (shape_is<Shape4>(d)) return prof ? k_mega<Shape4, false, true> : k_mega<Shape4, false, false>;
     }
-    return k_mega<ShapeRT, true>;
+    return k_mega<ShapeRT, true, true>;
 }
 
 }  // namespace mega
