@@ -411,6 +411,12 @@ int mega_load(dfssm_ctx* ctx, const std::vector<mega::HostLayer>& HL, const floa
             CK(cudaStreamSynchronize(ctx->stream));
         }
     }
+    if (d.n_layers > 0) {      // A_log -> A = -exp(A_log) inside the chunks, with the kernel's own exp
+        const size_t n = (size_t)d.n_layers * P.G * P.nch_max;
+        mega::k_mega_prepare<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(ctx->arena + v.m_chunks, (size_t)d.n_layers * P.G,
+                                                                                   P.chunk_bytes, P.c_alog, P.nch_max);
+        CK(cudaGetLastError());
+    }
     {
         std::vector<uint8_t> buf((size_t)P.blk_bytes);
         for (int l = 0; l < d.n_layers; ++l) {

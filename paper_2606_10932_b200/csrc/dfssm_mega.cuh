@@ -329,18 +329,19 @@ __device__ __forceinline__ int norm_quant(const Ctx<S>& x, Enum en, double ss_lo
     if (pk >= 0) x.stamp(pl, pk);
     __syncthreads();
     if (pk >= 0) x.stamp(pl, pk + 1);
-    if (x.wid == 0) {
-        float amax = x.lane < NWARPS ? red_f(x)[x.lane] : 0.0f;
+    if (x.wid == 0) {                      // warp 0: sum of squares -> rstd
         double ss = x.lane < NWARPS ? red_d(x)[x.lane] : 0.0;
-        amax = warp_max(amax);
         ss = warp_sum(ss);
-        float inv, sc;
-        quant_consts(ss, amax, K, P.eps, inv, sc);
-        if (x.lane == 0) { bc[0] = inv; bc[1] = sc; }
+        const float ms = (float)(ss / (double)K);
+        if (x.lane == 0) bc[1] = fdiv(1.0f, __fsqrt_rn(fadd(ms, P.eps)));
+    } else if (x.wid == 1) {               // warp 1: amax -> inv
+        float amax = x.lane < NWARPS ? red_f(x)[x.lane] : 0.0f;
+        amax = warp_max(amax);
+        if (x.lane == 0) { bc[0] = amax == 0.0f ? 0.0f : fdiv(127.0f, amax); bc[2] = amax; }
     }
     __syncthreads();
     const float inv = bc[0];
-    s_out = bc[1];
+    s_out = bc[2] == 0.0f ? 0.0f : fdiv(fmul(bc[2], bc[1]), 127.0f);
     if (pk >= 0) x.stamp(pl, pk + 2);
     int qs = 0;
     en([&](int k0, uint4 w) {                                       // four consecutive elements, k0 % 4 == 0
@@ -570,6 +571,15 @@ __device__ __forceinline__ void word_store(const Ctx<S>& x, uint32_t* rec, uint3
 {
     const Params& P = x.P;
     for (int m = x.lane; m < x.M(); m += 32) x_st32(rec + (size_t)m * P.x_words + part_off + idx, value);
+}
+
+// load time: replace A_log by A = -exp(A_log) inside every chunk (same sp_expf as the step would use; R10)
+__global__ void k_mega_prepare(uint8_t* chunks, size_t n_chunks, uint32_t chunk_bytes, uint32_t c_alog, int nch_max)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_chunks * (size_t)nch_max) return;
+    float* p = (float*)(chunks + (i / nch_max) * chunk_bytes + c_alog) + (i % nch_max);
+    *p = -sp_expf(*p);
 }
 
 template <class S, bool TAPS, bool PROF>
@@ -845,7 +855,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         {
             double ss_own = 0.0;
             const int hpg = x.nheads() / x.ngroups();
-            const float* alog = (const float*)(stage + P.c_alog);
+            const float* Aneg = (const float*)(stage + P.c_alog);      // A = -exp(A_log), made by k_mega_prepare at load
             const float* Dv = (const float*)(stage + P.c_D);
             const float* gw = (const float*)(stage + P.c_gnorm);
             const int l16 = tid % LPC;
@@ -854,10 +864,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 const bool valid = ib + tid / LPC < nch;
                 const int ch = ch0 + i, h = ch / x.headdim(), grp = h / hpg;
                 const float dtv = s_dt[h];
-                const float An = -sp_expf(alog[i]);
+                const float An = Aneg[i];
                 const float dA = sp_expf(fmul(dtv, An));
                 const float xv = s_x[i];
                 const float dtx = fmul(dtv, xv);
+                const float sz = siluf(s_z[i]);             // all lanes: free in SIMT, and off the tail of the reduction
                 float* Hr = (float*)(stage + P.st_ssm) + (size_t)i * x.d_state();
                 const float* Bc = s_bc + grp * x.d_state();
                 const float* Cc = s_bc + x.gs() + grp * x.d_state();
@@ -878,7 +889,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 if (l16 == 0 && valid) {
                     a = dacc(a, Dv[i], xv);
                     const float y = (float)a;
-                    const float gv = fmul(y, siluf(s_z[i]));
+                    const float gv = fmul(y, sz);
                     s_slotG[i] = __float_as_uint(fmul(gv, gw[i]));
                     ss_own = dacc(ss_own, gv, gv);
                     if (tp) { ((float*)(tp + P.tl.off[7]))[ch] = y; ((float*)(tp + P.tl.off[8]))[ch] = gv; }
