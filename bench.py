@@ -205,6 +205,29 @@ def run_reference(args, s, blob):
     print(json.dumps(out), flush=True)
 
 
+# ---------------------------------------------------------------------------------------------
+# N > 1: independent replicas ("replicas only") -- the host-side logic, also run on CPU/gloo by tests
+# ---------------------------------------------------------------------------------------------
+def replica_seed(rank: int, cfg_idx: int) -> int:
+    """Every rank decodes its own sequences: the token-stream seed of a replica."""
+    return 1000 * rank + cfg_idx
+
+
+def max_over_ranks(values, dist=None, device="cpu"):
+    """Element-wise MAX of per-rank durations over all ranks (the job is as slow as its slowest replica)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return [float(v) for v in values]
+    import torch
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.cpu()]
+
+
+def whole_job_rate(world: int, batch: int, steps: int, seconds: float) -> float:
+    """Tokens of ALL replicas divided by the max-over-ranks time."""
+    return world * batch * steps / seconds
+
+
 def workload_name(cfg_idx: int, batch: int) -> str:
     names = {0: "cfg0 tiny DF-SSM (2 layers, d_model 256)", 1: "cfg1 Mamba-2-130M-shape DF-SSM",
              2: "cfg2 Mamba-2-1.3B-shape DF-SSM (48 layers, d_model 2048, d_state 128, LoRA r32)",
@@ -237,7 +260,7 @@ def run_ours(args, s, blob):
     B = args.batch
     m = pk.Model(pk.Config.from_shape(s, max_batch=B), blob, device=f"cuda:{local}")
     # every rank is an independent replica with its own token streams ("replicas only")
-    prompt = ds.token_batch(s.vocab, max(args.warmup, 1), seed=1000 * rank + args.config, batch=B)
+    prompt = ds.token_batch(s.vocab, max(args.warmup, 1), seed=replica_seed(rank, args.config), batch=B)
     prompt_dev = [torch.from_numpy(prompt[t]).cuda() for t in range(prompt.shape[0])]
     nxt = m.next_tokens()[:B]
 
@@ -290,10 +313,7 @@ def run_ours(args, s, blob):
     kt = m.time_kernels(nxt, iters=8)
     barrier()
 
-    if dist is not None:
-        tt = torch.tensor([ms, e2e_s], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms, e2e_s = float(tt[0]), float(tt[1])
+    ms, e2e_s = max_over_ranks([ms, e2e_s], dist, "cuda")
 
     if rank != 0:
         if dist is not None:
@@ -301,8 +321,8 @@ def run_ours(args, s, blob):
         return
 
     ab = algorithmic_bytes(s, B)
-    value = world * B * args.steps / (ms * 1e-3)
-    e2e_val = world * B * e2e_steps / e2e_s
+    value = whole_job_rate(world, B, args.steps, ms * 1e-3)
+    e2e_val = whole_job_rate(world, B, e2e_steps, e2e_s)
     peak, peak_src = measured_peak()
     step_gbs = ab["total"] * (args.steps / (ms * 1e-3)) / 1e9
     kb = kernel_class_bytes(s, B)
