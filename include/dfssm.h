@@ -61,6 +61,7 @@ enum {
 #define DFSSM_FLAG_TAPS      1u  /* allocate per-layer debug taps and record them every step (slower)   */
 #define DFSSM_FLAG_NO_GRAPH  2u  /* launch the step's kernels one by one instead of one CUDA-graph launch */
 #define DFSSM_FLAG_NO_MEGA   4u  /* never use the single persistent kernel ("mega" path) for batch-1 steps    */
+#define DFSSM_FLAG_NO_MMA   16u  /* batch >= 16: keep the projections on the dp4a path instead of tcgen05 kind::i8 tiles  */
 #define DFSSM_FLAG_PROF      8u  /* persistent kernel: thread 0 of every CTA stamps its SM clock at every phase */
 
 /* Shape of the model (the paper's Mamba-2-shaped student, Table 1) + capacity.

@@ -14,6 +14,7 @@
 
 #include "dfssm_kernels.cuh"
 #include "dfssm_mega_host.cuh"
+#include "dfssm_mma.cuh"
 
 using namespace dfssm;
 
@@ -234,6 +235,12 @@ int proj_grid(int rows_total)
     return g < cap ? g : cap;
 }
 
+// batch >= 16: the projections run on the tensor cores (tcgen05 kind::i8 on +-1 tiles unpacked in shared memory)
+bool use_mma(const dfssm_ctx* c, int batch, int K)
+{
+    return batch >= 16 && K % mma::KC == 0 && !(c->cfg.flags & DFSSM_FLAG_NO_MMA);
+}
+
 // Enqueue S0, L x (S1..S7), S8 for `batch` sequences on the context's stream.  The input tokens are
 // read from the arena's own token buffer (cv.tok), which the argmax kernel also refreshes with the
 // greedy tokens -- so a graph captured once per batch size serves every caller pointer.
@@ -280,6 +287,10 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         tm->end(); ++nl;
 
         tm->begin(DFSSM_KCLASS_PROJ_IN);
+        if (use_mma(c, batch, d.d_model))
+            mma::k_proj_mma<<<dim3((d.d_in_proj + d.r + mma::TM - 1) / mma::TM, (batch + mma::TN - 1) / mma::TN), mma::THREADS, 0, st>>>(
+                L.in_sign, L.in_A, d.d_in_proj, d.r, d.d_model, xq, ldq, batch, acc, ld_acc, t, err);
+        else
         k_proj<<<dim3(proj_grid(d.d_in_proj + d.r), (batch + PROJ_BT - 1) / PROJ_BT), PROJ_THREADS,
                  proj_smem(d.d_model), st>>>(L.in_sign, L.in_A, d.d_in_proj, d.r, d.d_model, xq, xqp, ldq, qsum,
                                              batch, acc, ld_acc, t);
@@ -302,6 +313,10 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         tm->end(); ++nl;
 
         tm->begin(DFSSM_KCLASS_PROJ_OUT);
+        if (use_mma(c, batch, d.d_inner))
+            mma::k_proj_mma<<<dim3((d.d_model + d.r + mma::TM - 1) / mma::TM, (batch + mma::TN - 1) / mma::TN), mma::THREADS, 0, st>>>(
+                L.out_sign, L.out_A, d.d_model, d.r, d.d_inner, xq, ldq, batch, acc, ld_acc, t, err);
+        else
         k_proj<<<dim3(proj_grid(d.d_model + d.r), (batch + PROJ_BT - 1) / PROJ_BT), PROJ_THREADS,
                  proj_smem(d.d_inner), st>>>(L.out_sign, L.out_A, d.d_model, d.r, d.d_inner, xq, xqp, ldq, qsum,
                                              batch, acc, ld_acc, t);
@@ -772,6 +787,7 @@ int dfssm_sync(dfssm_ctx* ctx)
         const int bits = *ctx->pinned_err;
         CK(cudaMemsetAsync(err_d, 0, sizeof(int), ctx->stream));
         if (bits & 2) return fail(ctx, DFSSM_E_CUDA, "the persistent step kernel timed out waiting for an exchange between CTAs");
+        if (bits & 4) return fail(ctx, DFSSM_E_CUDA, "a tensor-core projection timed out waiting for its MMAs");
         return fail(ctx, DFSSM_E_TOKEN, "a token id outside [0, vocab) was clamped");
     }
     return DFSSM_OK;

@@ -1,0 +1,166 @@
+// Batched projections (batch >= 16) on the 5th-generation tensor cores: S2 + S3 stage 1 (and S7) as
+//   [rows + r] x K   times   K x batch      int8 x int8 -> int32      (BJ north_star; S.8(a) last row)
+// The +-1 scaffold tile is unpacked from its sign bits into int8 in shared memory (never in HBM), the LoRA-down rows are
+// appended as further int8 rows of the same tile, the activation codes are the N operand, and the int32 accumulators
+// live in TMEM: tcgen05.mma.kind::i8, M = 128, N = 64, K = 32 per instruction, issued by one thread; tcgen05.commit ->
+// mbarrier tells the CTA that the shared-memory tile may be overwritten; tcgen05.ld brings the accumulators back.
+// Integer arithmetic: exact, so the results are bit-identical to the dp4a path (k_proj) and to the oracle.
+//
+// Shared-memory operand layout (K-major, no swizzle; "core matrix" = 8 rows x 16 bytes, stored contiguously):
+//   offset(row m, byte k) = (k / 16) * LBO + (m / 8) * 128 + (m % 8) * 16 + k % 16,   LBO = (tile rows / 8) * 128, SBO = 128
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "dfssm_kernels.cuh"
+
+namespace dfssm {
+namespace mma {
+
+constexpr int TM = 128;            // rows of the weight tile (MMA M)
+constexpr int TN = 64;             // sequences per tile (MMA N)
+constexpr int KC = 128;            // bytes of K per shared-memory stage (4 MMAs of K = 32)
+constexpr int THREADS = 128;
+constexpr uint32_t LBO_A = (TM / 8) * 128, LBO_B = (TN / 8) * 128, SBO = 128;
+constexpr uint32_t SPIN_LIMIT = 1u << 22;
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// shared-memory matrix descriptor (sm_100): start address, leading / stride byte offsets in 16-byte units, version 1, no swizzle
+__device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo, uint32_t sbo)
+{
+    return (uint64_t)((addr >> 4) & 0x3fffu) | ((uint64_t)((lbo >> 4) & 0x3fffu) << 16) | ((uint64_t)((sbo >> 4) & 0x3fffu) << 32) |
+           (1ull << 46);
+}
+// instruction descriptor of kind::i8: D = s32, A = B = signed 8-bit, both K-major, N >> 3 at bit 17, M >> 4 at bit 24
+constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TN >> 3) << 17) | ((uint32_t)(TM >> 4) << 24);
+
+// 4 sign bits -> 4 bytes of +1 (bit 1) / -1 (bit 0)
+__device__ __forceinline__ uint32_t signs4(uint32_t bits)
+{
+    const uint32_t spread = ((bits & 0xfu) * 0x00204081u) & 0x01010101u;
+    return 0xffffffffu ^ (spread * 0xfeu);
+}
+
+// grid = (ceil((rows + r) / 128), ceil(batch / 64)); 128 threads; K % 128 == 0
+__global__ void __launch_bounds__(THREADS)
+k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int rows, int r, int K,
+           const int8_t* __restrict__ xq, int ldq, int batch, int32_t* __restrict__ acc, int ld_acc,
+           int32_t* __restrict__ t, int* __restrict__ err)
+{
+    __shared__ __align__(128) uint8_t sA[TM * KC];
+    __shared__ __align__(128) uint8_t sB[TN * KC];
+    __shared__ __align__(8) uint64_t mbar;
+    __shared__ uint32_t tmem_base;
+    const int tid = threadIdx.x, wid = tid >> 5;
+    const int row0 = blockIdx.x * TM, b0 = blockIdx.y * TN;
+    const int rows_total = rows + r;
+    const int W = K / 32;
+
+    if (wid == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base)), "r"((uint32_t)TN) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&mbar)) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem = tmem_base;
+
+    const int grow = row0 + tid;                      // the weight row this thread unpacks
+    const int bn = tid >> 1, bhalf = tid & 1;          // the sequence / half chunk of codes this thread stages
+    const bool b_valid = b0 + bn < batch;
+    uint8_t* a_dst = sA + (tid >> 3) * 128 + (tid & 7) * 16;
+    uint8_t* b_dst = sB + (bn >> 3) * 128 + (bn & 7) * 16;
+    bool dead = false;
+
+    for (int kc = 0; kc < K / KC; ++kc) {
+        // ---- A: 128 weights of this row -> int8 ----
+        if (grow < rows) {
+            const uint4 w = *(const uint4*)(sign + (size_t)grow * W + kc * (KC / 32));
+            const uint32_t ww[4] = { w.x, w.y, w.z, w.w };
+#pragma unroll
+            for (int c = 0; c < KC / 16; ++c) {                       // 16 weights per 16-byte K column
+                const uint32_t b16 = (ww[c >> 1] >> (16 * (c & 1))) & 0xffffu;
+                *(uint4*)(a_dst + c * LBO_A) = make_uint4(signs4(b16), signs4(b16 >> 4), signs4(b16 >> 8), signs4(b16 >> 12));
+            }
+        } else if (grow < rows_total) {
+            const uint4* src = (const uint4*)(A + (size_t)(grow - rows) * K + kc * KC);
+#pragma unroll
+            for (int c = 0; c < KC / 16; ++c) *(uint4*)(a_dst + c * LBO_A) = src[c];
+        } else {
+#pragma unroll
+            for (int c = 0; c < KC / 16; ++c) *(uint4*)(a_dst + c * LBO_A) = make_uint4(0, 0, 0, 0);
+        }
+        // ---- B: 64 codes of one sequence ----
+        {
+            const uint4* src = (const uint4*)(xq + (size_t)(b0 + bn) * ldq + kc * KC + bhalf * (KC / 2));
+#pragma unroll
+            for (int c = 0; c < KC / 32; ++c)
+                *(uint4*)(b_dst + (bhalf * (KC / 32) + c) * LBO_B) = b_valid ? src[c] : make_uint4(0, 0, 0, 0);
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the tensor core
+        __syncthreads();
+        if (tid == 0) {
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+            for (int j = 0; j < KC / 32; ++j) {
+                const uint64_t da = smem_desc(smem_u32(sA) + j * 2 * LBO_A, LBO_A, SBO);
+                const uint64_t db = smem_desc(smem_u32(sB) + j * 2 * LBO_B, LBO_B, SBO);
+                const uint32_t accumulate = (kc > 0 || j > 0) ? 1u : 0u;
+                asm volatile(
+                    "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                    "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, {%5, %6, %7, %8}, p;\n\t}"
+                    ::"r"(tmem), "l"(da), "l"(db), "r"(IDESC), "r"(accumulate), "r"(0u), "r"(0u), "r"(0u), "r"(0u) : "memory");
+            }
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(&mbar)) : "memory");
+        }
+        // ---- wait until the MMAs of this stage have read shared memory ----
+        {
+            const uint32_t parity = (uint32_t)kc & 1u;
+            uint32_t spins = 0, ok = 0;
+            while (!ok) {
+                asm volatile(
+                    "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                    : "=r"(ok) : "r"(smem_u32(&mbar)), "r"(parity) : "memory");
+                if (!ok && ++spins > SPIN_LIMIT) { dead = true; break; }
+            }
+            if (dead) break;
+        }
+    }
+    if (dead && tid == 0) atomicOr(err, 4);
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+
+    // ---- epilogue: TMEM lane = row of the tile, column = sequence ----
+    if (!__syncthreads_or(dead ? 1 : 0)) {
+        const bool is_acc = grow < rows, is_t = !is_acc && grow < rows_total;
+#pragma unroll
+        for (int q = 0; q < TN / 16; ++q) {
+            uint32_t v[16];
+            const uint32_t taddr = tmem + ((uint32_t)(wid * 32) << 16) + (uint32_t)(q * 16);
+            asm volatile(
+                "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+                  "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                : "r"(taddr) : "memory");
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                const int b = b0 + q * 16 + i;
+                if (b < batch) {
+                    if (is_acc) acc[(size_t)b * ld_acc + grow] = (int32_t)v[i];
+                    else if (is_t) t[(size_t)b * T_STRIDE + (grow - rows)] = (int32_t)v[i];
+                }
+            }
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (wid == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"((uint32_t)TN) : "memory");
+}
+
+}  // namespace mma
+}  // namespace dfssm

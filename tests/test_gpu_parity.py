@@ -339,3 +339,55 @@ def test_mega_path_is_the_batch1_path_and_equals_chain(env):
         sa, ca = a.get_state(l, 0)
         sb, cb = b.get_state(l, 0)
         assert n_diff_bits(sa, sb) == 0 and n_diff_bits(ca, cb) == 0
+
+
+# ------------------------------------------------------------------------------------------------
+# batch >= 16: the projections run as tcgen05 kind::i8 tiles (+-1 unpacked in shared memory, int32 in TMEM)
+# ------------------------------------------------------------------------------------------------
+MMA_SHAPES = [
+    dict(n_layers=2, d_model=128, d_inner=256, headdim=32, d_state=16, lora_rank=3, vocab=211),       # 1 K chunk, ragged M tile
+    dict(n_layers=2, d_model=256, d_inner=512, headdim=64, d_state=64, ngroups=2, lora_rank=64, vocab=300),
+    dict(n_layers=1, d_model=384, d_inner=640, headdim=32, d_state=32, lora_rank=17, vocab=97),       # 3 / 5 K chunks
+]
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("kw", MMA_SHAPES, ids=[f"mma{i}" for i in range(len(MMA_SHAPES))])
+@pytest.mark.parametrize("batch", [17, 70])
+def test_tensor_core_projection_taps_bit_exact(env, kw, batch):
+    """int32 scaffold / LoRA accumulators (and everything downstream) of the tcgen05 path against the oracle, every tap,
+    with a ragged last row tile, a ragged sequence tile (17) and two sequence tiles (70)."""
+    pk, oracle, torch = env["pk"], env["oracle"], env["torch"]
+    s = ds.tiny_shape(**kw)
+    blob = ds.make_blob(s, seed=300 + len(kw), variant="varied")
+    T = 3
+    toks = ds.token_batch(s.vocab, T, seed=9, batch=batch)
+    gpu = pk.Model(pk.Config.from_shape(s, max_batch=batch, flags=pk.binding.FLAG_TAPS), blob)
+    check = sorted(set([0, 1, 15, 16, batch // 2, batch - 1]))
+    orcs = {b: oracle.OracleModel(blob, 1, taps=True) for b in check}
+    st = Stats()
+    for t in range(T):
+        gpu.step(dev_tokens(torch, toks[t]))
+        for b in check:
+            orcs[b].step(toks[t, b:b + 1])
+            for l in range(s.n_layers):
+                compare_taps(gpu, orcs[b], l, b, t, exact_float=True)
+            compare_step(gpu, orcs[b], b, st, t, "mma")
+    assert st.diff_hidden == 0 and st.diff_logits == 0, st
+
+
+@pytest.mark.gpu
+def test_tensor_core_path_equals_dp4a_path(env):
+    """Same model, batch 32, with and without DFSSM_FLAG_NO_MMA: logits, hidden states and greedy tokens identical."""
+    pk, torch = env["pk"], env["torch"]
+    s, blob = blob_for(1)
+    B, T = 32, 6
+    toks = ds.token_batch(s.vocab, T, seed=21, batch=B)
+    a = pk.Model(pk.Config.from_shape(s, max_batch=B), blob)
+    b = pk.Model(pk.Config.from_shape(s, max_batch=B, flags=pk.binding.FLAG_NO_MMA), blob)
+    for t in range(T):
+        a.step(dev_tokens(torch, toks[t]))
+        b.step(dev_tokens(torch, toks[t]))
+        a.sync(); b.sync()
+        assert torch.equal(a.logits(), b.logits()) and torch.equal(a.hidden(), b.hidden())
+        assert torch.equal(a.next_tokens(), b.next_tokens())
