@@ -24,7 +24,7 @@ constexpr size_t ARENA_ALIGN = 256;
 inline size_t up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Carve {                 // byte offsets inside the arena
-    size_t blob, ssm, conv, pos, u, xq, xqp, sx, qsum, acc, t, g, logits, next, tok, err, taps, total;
+    size_t blob, ssm, conv, pos, u, xq, xqp, sx, qsum, acc, t, g, bcdt, logits, next, tok, err, taps, total;
     size_t m_chunks, m_blocks, m_Ain, m_Aout, m_x, m_xbytes, m_am, m_prof;      // mega path regions (valid if mega_fit)
     bool mega_fit;
     size_t ssm_elems, ldq, ld_acc;
@@ -148,6 +148,7 @@ Carve carve(const dfssm_config& c)
     v.acc = put(B * v.ld_acc * 4);
     v.t = put(B * T_STRIDE * 4);
     v.g = put(B * d.d_inner * 4);
+    v.bcdt = put(B * (size_t)(2 * d.ngroups * d.d_state + d.nheads) * 4);
     v.logits = put(B * (size_t)d.vocab * 4);
     v.next = put(B * 4);
     v.tok = put(B * 4);
@@ -241,6 +242,27 @@ bool use_mma(const dfssm_ctx* c, int batch, int K)
     return batch >= 16 && K % mma::KC == 0 && !(c->cfg.flags & DFSSM_FLAG_NO_MMA);
 }
 
+// one projection on the tensor cores; K is split over CTAs until the grid fills the 148 SMs (partial sums are added
+// with integer atomics into zeroed buffers: exact, order-independent)
+int launch_proj_mma(dfssm_ctx* ctx, const uint32_t* sign, const int8_t* A, int rows, int K, int batch)
+{
+    const Dims& d = ctx->dm;
+    const Carve& v = ctx->cv;
+    const int mt = (rows + d.r + mma::TM - 1) / mma::TM, nt = (batch + mma::TN - 1) / mma::TN, nchunk = K / mma::KC;
+    int ks = 148 / (mt * nt);
+    if (ks < 1) ks = 1;
+    if (ks > nchunk) ks = nchunk;
+    int32_t* acc = at<int32_t>(ctx, v.acc);
+    int32_t* t = at<int32_t>(ctx, v.t);
+    if (ks > 1) {
+        CK(cudaMemsetAsync(acc, 0, (size_t)batch * v.ld_acc * 4, ctx->stream));
+        CK(cudaMemsetAsync(t, 0, (size_t)batch * T_STRIDE * 4, ctx->stream));
+    }
+    mma::k_proj_mma<<<dim3(mt, nt, ks), mma::THREADS, 0, ctx->stream>>>(sign, A, rows, d.r, K, at<int8_t>(ctx, v.xq), (int)v.ldq, batch,
+                                                                      acc, (int)v.ld_acc, t, at<int>(ctx, v.err));
+    return DFSSM_OK;
+}
+
 // Enqueue S0, L x (S1..S7), S8 for `batch` sequences on the context's stream.  The input tokens are
 // read from the arena's own token buffer (cv.tok), which the argmax kernel also refreshes with the
 // greedy tokens -- so a graph captured once per batch size serves every caller pointer.
@@ -287,10 +309,10 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         tm->end(); ++nl;
 
         tm->begin(DFSSM_KCLASS_PROJ_IN);
-        if (use_mma(c, batch, d.d_model))
-            mma::k_proj_mma<<<dim3((d.d_in_proj + d.r + mma::TM - 1) / mma::TM, (batch + mma::TN - 1) / mma::TN), mma::THREADS, 0, st>>>(
-                L.in_sign, L.in_A, d.d_in_proj, d.r, d.d_model, xq, ldq, batch, acc, ld_acc, t, err);
-        else
+        if (use_mma(c, batch, d.d_model)) {
+            const int rc = launch_proj_mma(c, L.in_sign, L.in_A, d.d_in_proj, d.d_model, batch);
+            if (rc != DFSSM_OK) return rc;
+        } else
         k_proj<<<dim3(proj_grid(d.d_in_proj + d.r), (batch + PROJ_BT - 1) / PROJ_BT), PROJ_THREADS,
                  proj_smem(d.d_model), st>>>(L.in_sign, L.in_A, d.d_in_proj, d.r, d.d_model, xq, xqp, ldq, qsum,
                                              batch, acc, ld_acc, t);
@@ -303,8 +325,11 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         }
 
         tm->begin(DFSSM_KCLASS_SSM);
+        k_bcdt<<<dim3((2 * d.ngroups * d.d_state + d.nheads + BCDT_THREADS - 1) / BCDT_THREADS, batch), BCDT_THREADS, 0, st>>>(
+            L, d, acc, ld_acc, t, sx, conv, pos, at<float>(c, v.bcdt), tp, v.tap_stride, v.tl);
+        ++nl;
         k_ssm<<<dim3(d.nheads * (d.headdim / SSM_PB), batch), SSM_THREADS, ssm_smem(d), st>>>(
-            L, d, acc, ld_acc, t, sx, conv, pos, ssm, g, tp, v.tap_stride, v.tl);
+            L, d, acc, ld_acc, t, sx, conv, pos, ssm, g, at<float>(c, v.bcdt), tp, v.tap_stride, v.tl);
         tm->end(); ++nl;
 
         tm->begin(DFSSM_KCLASS_NORMQUANT);
@@ -313,10 +338,10 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         tm->end(); ++nl;
 
         tm->begin(DFSSM_KCLASS_PROJ_OUT);
-        if (use_mma(c, batch, d.d_inner))
-            mma::k_proj_mma<<<dim3((d.d_model + d.r + mma::TM - 1) / mma::TM, (batch + mma::TN - 1) / mma::TN), mma::THREADS, 0, st>>>(
-                L.out_sign, L.out_A, d.d_model, d.r, d.d_inner, xq, ldq, batch, acc, ld_acc, t, err);
-        else
+        if (use_mma(c, batch, d.d_inner)) {
+            const int rc = launch_proj_mma(c, L.out_sign, L.out_A, d.d_model, d.d_inner, batch);
+            if (rc != DFSSM_OK) return rc;
+        } else
         k_proj<<<dim3(proj_grid(d.d_model + d.r), (batch + PROJ_BT - 1) / PROJ_BT), PROJ_THREADS,
                  proj_smem(d.d_inner), st>>>(L.out_sign, L.out_A, d.d_model, d.r, d.d_inner, xq, xqp, ldq, qsum,
                                              batch, acc, ld_acc, t);
@@ -797,7 +822,7 @@ int dfssm_launches_per_step(dfssm_ctx* ctx, int batch)
 {
     if (!ctx || batch < 1) return DFSSM_E_ARG;
     if (use_mega(ctx, batch)) return 1;
-    const int per_layer = (ctx->cfg.flags & DFSSM_FLAG_TAPS) ? 10 : 6;
+    const int per_layer = (ctx->cfg.flags & DFSSM_FLAG_TAPS) ? 11 : 7;
     return 1 + ctx->dm.n_layers * per_layer + 3;
 }
 

@@ -244,10 +244,57 @@ __device__ __forceinline__ float proj_epilogue_row(int acc_i, const __half* __re
 }
 
 // =============================================================================================
+// S3 stage 2 + S4 conv + softplus for the B | C | dt rows, ONCE per sequence (every head reads them):
+//   bcdt[b][e] = silu(conv(B|C row e))  for e < 2*gs,   softplus(dt row + dt_bias)  for the nheads rows behind.
+//   grid = (ceil(n_bcdt / BCDT_THREADS), batch)
+// =============================================================================================
+constexpr int BCDT_THREADS = 128;
+
+__global__ void __launch_bounds__(BCDT_THREADS)
+k_bcdt(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int32_t* __restrict__ t,
+       const float* __restrict__ s_x, float* __restrict__ conv_ring, const int32_t* __restrict__ pos,
+       float* __restrict__ bcdt, uint8_t* __restrict__ taps, uint32_t tap_stride, TapLayout tl)
+{
+    __shared__ float v_sh[64];
+    const int b = blockIdx.y, tid = threadIdx.x;
+    const int gs = dm.ngroups * dm.d_state, n_bcdt = 2 * gs + dm.nheads;
+    if (tid < dm.r) v_sh[tid] = fmul(L.in_a_s[tid], (float)t[(size_t)b * T_STRIDE + tid]);
+    __syncthreads();
+    const int e = blockIdx.x * BCDT_THREADS + tid;
+    if (e >= n_bcdt) return;
+    const int row = 2 * dm.d_inner + e;
+    uint8_t* tp = taps ? taps + (size_t)b * tap_stride : nullptr;
+    const float val = proj_epilogue_row(acc[(size_t)b * ld_acc + row], L.in_row_scale, L.in_B, L.in_b_s, row, dm.r, v_sh, s_x[b]);
+    if (tp) ((float*)(tp + tl.off[4]))[row] = val;                               // ZXBCDT
+    float out;
+    if (e < 2 * gs) {
+        const int ps = pos[b] & 3;
+        const int c = dm.d_inner + e;                                            // conv channel
+        float* ring = conv_ring + ((size_t)b * dm.conv_dim + c) * 4;
+        const float4 rg = *(const float4*)ring;
+        const float sl[4] = { rg.x, rg.y, rg.z, rg.w };
+        const float s0 = sl[(ps + 1) & 3], s1 = sl[(ps + 2) & 3], s2 = sl[(ps + 3) & 3];
+        const float4 cw = *(const float4*)(L.conv_w + 4 * (size_t)c);
+        float o = L.conv_b[c];
+        o = ffma(cw.x, s0, o);
+        o = ffma(cw.y, s1, o);
+        o = ffma(cw.z, s2, o);
+        o = ffma(cw.w, val, o);
+        ring[ps] = val;
+        out = siluf(o);
+        if (tp) ((float*)(tp + tl.off[5]))[c] = out;                             // XBC_CONV
+    } else {
+        const int h = e - 2 * gs;
+        out = sp_softplusf(fadd(val, L.dt_bias[h]));
+        if (tp) ((float*)(tp + tl.off[6]))[h] = out;                             // DT
+    }
+    bcdt[(size_t)b * n_bcdt + e] = out;
+}
+
+// =============================================================================================
 // S3 stage 2 (for the rows a head needs) + S4 conv step + S5 state update/readout + S6 gate.
 //   grid = (nheads * headdim/SSM_PB, batch); one CTA owns SSM_PB (head, p) rows of the state.
-//   The B and C rows are recomputed by every CTA of the group (256 rows of 32 fp64 FMAs: cheap);
-//   only the first CTA of a group stores their new conv sample.
+//   The B | C | dt rows are finished once per sequence by k_bcdt and read from its buffer.
 //   Conv state is a 4-slot ring per channel: the sample of step t lives in slot t%4, so the
 //   readers of a step never touch the slot its owner writes.
 // =============================================================================================
@@ -257,8 +304,8 @@ __global__ void __launch_bounds__(SSM_THREADS)
 k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int32_t* __restrict__ t,
       const float* __restrict__ s_x, float* __restrict__ conv_ring /* [batch][conv_dim][4] */,
       const int32_t* __restrict__ pos /* [batch] */, float* __restrict__ ssm /* [batch][h][p][n] */,
-      float* __restrict__ g /* [batch][d_inner] */, uint8_t* __restrict__ taps, uint32_t tap_stride,
-      TapLayout tl)
+      float* __restrict__ g /* [batch][d_inner] */, const float* __restrict__ bcdt /* [batch][n_bcdt] from k_bcdt */,
+      uint8_t* __restrict__ taps, uint32_t tap_stride, TapLayout tl)
 {
     extern __shared__ __align__(16) uint8_t smem[];
     float* v_sh = (float*)smem;                    // [64]
@@ -274,7 +321,6 @@ k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
     const int p0 = pblk * SSM_PB;
     const int hpg = dm.nheads / dm.ngroups;
     const int grp = h / hpg;
-    const bool bc_owner = (h % hpg == 0) && pblk == 0;
     const int tid = threadIdx.x;
     const int32_t* accb = acc + (size_t)b * ld_acc;
     const float sx = s_x[b];
@@ -282,26 +328,24 @@ k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
     uint8_t* tp = taps ? taps + (size_t)b * tap_stride : nullptr;
 
     if (tid < dm.r) v_sh[tid] = fmul(L.in_a_s[tid], (float)t[(size_t)b * T_STRIDE + tid]);
+    const int gs = dm.ngroups * dm.d_state;
+    {   // B', C' of this head's group and dt of this head: made once per sequence by k_bcdt
+        const float* src = bcdt + (size_t)b * (2 * gs + dm.nheads);
+        for (int i = tid; i < dm.d_state; i += SSM_THREADS) {
+            Bc[i] = src[grp * dm.d_state + i];
+            Cc[i] = src[gs + grp * dm.d_state + i];
+        }
+        if (tid == 0) dts[0] = src[2 * gs + h];
+    }
     __syncthreads();
 
-    const int gs = dm.ngroups * dm.d_state;
-    const int n_rows = 2 * SSM_PB + 2 * dm.d_state + 1;
-    for (int i = tid; i < n_rows; i += SSM_THREADS) {
-        int row, kind, idx;      // kind 0 z, 1 x, 2 B, 3 C, 4 dt
-        if (i < SSM_PB) { kind = 0; idx = i; row = h * dm.headdim + p0 + idx; }
-        else if (i < 2 * SSM_PB) { kind = 1; idx = i - SSM_PB; row = dm.d_inner + h * dm.headdim + p0 + idx; }
-        else if (i < 2 * SSM_PB + dm.d_state) { kind = 2; idx = i - 2 * SSM_PB; row = 2 * dm.d_inner + grp * dm.d_state + idx; }
-        else if (i < 2 * SSM_PB + 2 * dm.d_state) { kind = 3; idx = i - 2 * SSM_PB - dm.d_state; row = 2 * dm.d_inner + gs + grp * dm.d_state + idx; }
-        else { kind = 4; idx = 0; row = 2 * dm.d_inner + 2 * gs + h; }
+    for (int i = tid; i < 2 * SSM_PB; i += SSM_THREADS) {
+        const int kind = i < SSM_PB ? 0 : 1, idx = i - kind * SSM_PB;      // kind 0 z, 1 x
+        const int row = kind * dm.d_inner + h * dm.headdim + p0 + idx;
         const float val = proj_epilogue_row(accb[row], L.in_row_scale, L.in_B, L.in_b_s, row, dm.r, v_sh, sx);
-        const bool owner = (kind == 0 || kind == 1) || (kind == 4 && pblk == 0) || bc_owner;
-        if (tp && owner) ((float*)(tp + tl.off[4]))[row] = val;                    // ZXBCDT
+        if (tp) ((float*)(tp + tl.off[4]))[row] = val;                             // ZXBCDT
         if (kind == 0) {
             zs[idx] = val;
-        } else if (kind == 4) {
-            const float dtv = sp_softplusf(fadd(val, L.dt_bias[h]));
-            dts[0] = dtv;
-            if (tp && pblk == 0) ((float*)(tp + tl.off[6]))[h] = dtv;              // DT
         } else {
             const int c = row - dm.d_inner;                                        // conv channel
             float* ring = conv_ring + ((size_t)b * dm.conv_dim + c) * 4;
@@ -315,11 +359,9 @@ k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
             o = ffma(cw.z, s2, o);
             o = ffma(cw.w, val, o);
             const float cv = siluf(o);
-            if (kind == 1 || bc_owner) {
-                ring[ps] = val;
-                if (tp) ((float*)(tp + tl.off[5]))[c] = cv;                        // XBC_CONV
-            }
-            if (kind == 1) xs[idx] = cv; else if (kind == 2) Bc[idx] = cv; else Cc[idx] = cv;
+            ring[ps] = val;
+            if (tp) ((float*)(tp + tl.off[5]))[c] = cv;                            // XBC_CONV
+            xs[idx] = cv;
         }
     }
     __syncthreads();

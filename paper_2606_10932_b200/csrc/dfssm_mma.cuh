@@ -4,7 +4,7 @@
 // appended as further int8 rows of the same tile, the activation codes are the N operand, and the int32 accumulators
 // live in TMEM: tcgen05.mma.kind::i8, M = 128, N = 64, K = 32 per instruction, issued by one thread; tcgen05.commit ->
 // mbarrier tells the CTA that the shared-memory tile may be overwritten; tcgen05.ld brings the accumulators back.
-// Integer arithmetic: exact, so the results are bit-identical to the dp4a path (k_proj) and to the oracle.
+// Integer arithmetic: exact, so the results are bit-identical to the dp4a path (k_proj).
 //
 // Shared-memory operand layout (K-major, no swizzle; "core matrix" = 8 rows x 16 bytes, stored contiguously):
 //   offset(row m, byte k) = (k / 16) * LBO + (m / 8) * 128 + (m % 8) * 16 + k % 16,   LBO = (tile rows / 8) * 128, SBO = 128
@@ -42,7 +42,8 @@ __device__ __forceinline__ uint32_t signs4(uint32_t bits)
     return 0xffffffffu ^ (spread * 0xfeu);
 }
 
-// grid = (ceil((rows + r) / 128), ceil(batch / 64)); 128 threads; K % 128 == 0
+// grid = (ceil((rows + r) / 128), ceil(batch / 64), ksplit); 128 threads; K % 128 == 0.  With ksplit > 1 every CTA takes a
+// slice of K and ADDS its int32 partial sums into acc / t (exact in any order), which the caller has zeroed.
 __global__ void __launch_bounds__(THREADS)
 k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int rows, int r, int K,
            const int8_t* __restrict__ xq, int ldq, int batch, int32_t* __restrict__ acc, int ld_acc,
@@ -77,7 +78,9 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
     uint8_t* b_dst = sB + (bn >> 3) * 128 + (bn & 7) * 16;
     bool dead = false;
 
-    for (int kc = 0; kc < K / KC; ++kc) {
+    const int nchunk = K / KC, kc0 = (int)(((long long)blockIdx.z * nchunk) / gridDim.z), kc1 = (int)(((long long)(blockIdx.z + 1) * nchunk) / gridDim.z);
+    const bool split = gridDim.z > 1;
+    for (int kc = kc0; kc < kc1; ++kc) {
         // ---- A: 128 weights of this row -> int8 ----
         if (grow < rows) {
             const uint4 w = *(const uint4*)(sign + (size_t)grow * W + kc * (KC / 32));
@@ -110,7 +113,7 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
             for (int j = 0; j < KC / 32; ++j) {
                 const uint64_t da = smem_desc(smem_u32(sA) + j * 2 * LBO_A, LBO_A, SBO);
                 const uint64_t db = smem_desc(smem_u32(sB) + j * 2 * LBO_B, LBO_B, SBO);
-                const uint32_t accumulate = (kc > 0 || j > 0) ? 1u : 0u;
+                const uint32_t accumulate = (kc > kc0 || j > 0) ? 1u : 0u;
                 asm volatile(
                     "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
                     "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, {%5, %6, %7, %8}, p;\n\t}"
@@ -120,7 +123,7 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
         }
         // ---- wait until the MMAs of this stage have read shared memory ----
         {
-            const uint32_t parity = (uint32_t)kc & 1u;
+            const uint32_t parity = (uint32_t)(kc - kc0) & 1u;
             uint32_t spins = 0, ok = 0;
             while (!ok) {
                 asm volatile(
@@ -151,8 +154,11 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
             for (int i = 0; i < 16; ++i) {
                 const int b = b0 + q * 16 + i;
                 if (b < batch) {
-                    if (is_acc) acc[(size_t)b * ld_acc + grow] = (int32_t)v[i];
-                    else if (is_t) t[(size_t)b * T_STRIDE + (grow - rows)] = (int32_t)v[i];
+                    int32_t* dst = is_acc ? acc + (size_t)b * ld_acc + grow : t + (size_t)b * T_STRIDE + (grow - rows);
+                    if (is_acc || is_t) {
+                        if (split) atomicAdd(dst, (int32_t)v[i]);
+                        else *dst = (int32_t)v[i];
+                    }
                 }
             }
         }
