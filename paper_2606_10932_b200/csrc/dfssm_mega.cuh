@@ -33,7 +33,6 @@
 //     for layer l-1), so the buffers stay L2-resident and a reset is at least two hops old when reused.
 //   * Arithmetic: identical to the chain path (dfssm_math.cuh; contract of DESIGN.md section 5).
 #pragma once
-#include <cooperative_groups.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -146,10 +145,6 @@ __device__ __forceinline__ void x_st32(uint32_t* p, uint32_t v)
 {
     asm volatile("st.relaxed.gpu.global.b32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
-__device__ __forceinline__ void x_st64(uint32_t* p, uint64_t v)
-{
-    asm volatile("st.relaxed.gpu.global.b64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-}
 // 16 bytes as TWO 64-bit elements, each single-copy atomic (a float pair, or one fp64)
 __device__ __forceinline__ uint4 x_ld128(const uint32_t* p)
 {
@@ -161,13 +156,6 @@ __device__ __forceinline__ void x_st128(uint32_t* p, uint4 v)
 {
     const uint64_t a = ((uint64_t)v.y << 32) | v.x, b = ((uint64_t)v.w << 32) | v.z;
     asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1,%2};" ::"l"(p), "l"(a), "l"(b) : "memory");
-}
-
-__device__ __forceinline__ int4 ldg_nc16(const void* p)
-{
-    int4 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
-    return r;
 }
 
 // Code layout for the masked-dp4a sign dot: a 32-block of codes is eight 4-byte words ("planes"), plane i = elements
@@ -288,16 +276,7 @@ __device__ __forceinline__ void hop_gather(const Ctx<S>& x, const uint32_t* buf,
     }
 }
 
-// quantiser constants from (sum of squares, amax) of a vector of length d (R4, R13)
-__device__ __forceinline__ void quant_consts(double ss, float amax, int d, float eps, float& inv, float& s)
-{
-    const float ms = (float)(ss / (double)d);
-    const float rstd = fdiv(1.0f, __fsqrt_rn(fadd(ms, eps)));
-    inv = amax == 0.0f ? 0.0f : fdiv(127.0f, amax);
-    s = amax == 0.0f ? 0.0f : fdiv(fmul(amax, rstd), 127.0f);
-}
-
-// scratch inside s_red: [0,16) floats warp maxima | [16,32) ints warp code sums | doubles [8,24) warp sums (byte 64..)
+// scratch inside s_red: NWARPS floats (warp maxima) | NWARPS ints (warp code sums) | NWARPS doubles (warp sums)
 template <class S>
 __device__ __forceinline__ float* red_f(const Ctx<S>& x) { return (float*)(x.sm + x.P.s_red); }
 template <class S>
@@ -397,20 +376,6 @@ __device__ __forceinline__ double slot_partials(const Ctx<S>& x, const uint4 (&v
         }
     }
     return s;
-}
-
-// block-wide sum of doubles held by some lanes (others pass 0); result valid in thread 0 only.  One __syncthreads.
-template <class S>
-__device__ __forceinline__ double block_sum_t0(const Ctx<S>& x, double s)
-{
-    s = warp_sum(s);
-    if (x.lane == 0) red_d(x)[x.wid] = s;
-    __syncthreads();
-    double t = 0.0;
-    if (x.tid == 0)
-#pragma unroll
-        for (int i = 0; i < NWARPS; ++i) t += red_d(x)[i];
-    return t;
 }
 
 // ------------------------------------------------------------------------------------------------
