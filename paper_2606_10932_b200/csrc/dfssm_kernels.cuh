@@ -327,6 +327,17 @@ k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
     const int ps = pos[b] & 3;
     uint8_t* tp = taps ? taps + (size_t)b * tap_stride : nullptr;
 
+    // this thread's slice of the state is requested first, so that HBM works while the rows below are finished
+    const int p = tid >> 4, l16 = tid & 15;       // 16 rows x 16 lanes
+    float* Hr = ssm + (((size_t)b * dm.nheads + h) * dm.headdim + p0 + p) * dm.d_state;
+    constexpr int H_PRE = 2;                      // chunks held in registers (all of d_state = 128); further ones are loaded late
+    float4 hpre[H_PRE];
+#pragma unroll
+    for (int j = 0; j < H_PRE; ++j) {
+        const int n4 = l16 + 16 * j;
+        if (n4 < dm.d_state / 4) hpre[j] = *(const float4*)(Hr + 4 * n4);
+    }
+
     if (tid < dm.r) v_sh[tid] = fmul(L.in_a_s[tid], (float)t[(size_t)b * T_STRIDE + tid]);
     const int gs = dm.ngroups * dm.d_state;
     {   // B', C' of this head's group and dt of this head: made once per sequence by k_bcdt
@@ -339,29 +350,42 @@ k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
     }
     __syncthreads();
 
-    for (int i = tid; i < 2 * SSM_PB; i += SSM_THREADS) {
+    // the 2 * SSM_PB own rows (z, x): 8 lanes share a row's LoRA sum (fp64, any tree: DESIGN.md 5.3)
+    static_assert(SSM_THREADS == 8 * 2 * SSM_PB, "8 lanes per own row");
+    {
+        const int i = tid >> 3, sub = tid & 7;
         const int kind = i < SSM_PB ? 0 : 1, idx = i - kind * SSM_PB;      // kind 0 z, 1 x
         const int row = kind * dm.d_inner + h * dm.headdim + p0 + idx;
-        const float val = proj_epilogue_row(accb[row], L.in_row_scale, L.in_B, L.in_b_s, row, dm.r, v_sh, sx);
-        if (tp) ((float*)(tp + tl.off[4]))[row] = val;                             // ZXBCDT
-        if (kind == 0) {
-            zs[idx] = val;
-        } else {
-            const int c = row - dm.d_inner;                                        // conv channel
-            float* ring = conv_ring + ((size_t)b * dm.conv_dim + c) * 4;
-            const float4 rg = *(const float4*)ring;
-            const float sl[4] = { rg.x, rg.y, rg.z, rg.w };
-            const float s0 = sl[(ps + 1) & 3], s1 = sl[(ps + 2) & 3], s2 = sl[(ps + 3) & 3];
-            const float4 cw = *(const float4*)(L.conv_w + 4 * (size_t)c);
-            float o = L.conv_b[c];
-            o = ffma(cw.x, s0, o);
-            o = ffma(cw.y, s1, o);
-            o = ffma(cw.z, s2, o);
-            o = ffma(cw.w, val, o);
-            const float cv = siluf(o);
-            ring[ps] = val;
-            if (tp) ((float*)(tp + tl.off[5]))[c] = cv;                            // XBC_CONV
-            xs[idx] = cv;
+        const int8_t* brow = L.in_B + (size_t)row * dm.r;
+        double lo = 0.0;
+        for (int j = sub; j < dm.r; j += 8) lo = dacc(lo, (float)brow[j], v_sh[j]);
+        lo += __shfl_xor_sync(0xffffffffu, lo, 1);
+        lo += __shfl_xor_sync(0xffffffffu, lo, 2);
+        lo += __shfl_xor_sync(0xffffffffu, lo, 4);
+        if (sub == 0) {
+            const float m1 = fmul(__half2float(L.in_row_scale[row]), (float)accb[row]);
+            const float m2 = fmul(L.in_b_s[row], (float)lo);
+            const float val = fmul(sx, fadd(m1, m2));
+            if (tp) ((float*)(tp + tl.off[4]))[row] = val;                         // ZXBCDT
+            if (kind == 0) {
+                zs[idx] = val;
+            } else {
+                const int c = row - dm.d_inner;                                    // conv channel
+                float* ring = conv_ring + ((size_t)b * dm.conv_dim + c) * 4;
+                const float4 rg = *(const float4*)ring;
+                const float sl[4] = { rg.x, rg.y, rg.z, rg.w };
+                const float s0 = sl[(ps + 1) & 3], s1 = sl[(ps + 2) & 3], s2 = sl[(ps + 3) & 3];
+                const float4 cw = *(const float4*)(L.conv_w + 4 * (size_t)c);
+                float o = L.conv_b[c];
+                o = ffma(cw.x, s0, o);
+                o = ffma(cw.y, s1, o);
+                o = ffma(cw.z, s2, o);
+                o = ffma(cw.w, val, o);
+                const float cv = siluf(o);
+                ring[ps] = val;
+                if (tp) ((float*)(tp + tl.off[5]))[c] = cv;                        // XBC_CONV
+                xs[idx] = cv;
+            }
         }
     }
     __syncthreads();
@@ -369,12 +393,27 @@ k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
     const float dtv = dts[0];
     const float An = -sp_expf(L.A_log[h]);
     const float dA = sp_expf(fmul(dtv, An));
-    const int p = tid >> 4, l16 = tid & 15;       // 16 rows x 16 lanes
     const float xv = xs[p];
     const float dtx = fmul(dtv, xv);
-    float* Hr = ssm + (((size_t)b * dm.nheads + h) * dm.headdim + p0 + p) * dm.d_state;
     double a = 0.0;
-    for (int n4 = l16; n4 < dm.d_state / 4; n4 += 16) {
+#pragma unroll
+    for (int j = 0; j < H_PRE; ++j) {
+        const int n4 = l16 + 16 * j;
+        if (n4 >= dm.d_state / 4) break;
+        float4 hv = hpre[j];
+        const float4 bv = *(const float4*)(Bc + 4 * n4);
+        const float4 cv = *(const float4*)(Cc + 4 * n4);
+        hv.x = ffma(dA, hv.x, fmul(dtx, bv.x));
+        hv.y = ffma(dA, hv.y, fmul(dtx, bv.y));
+        hv.z = ffma(dA, hv.z, fmul(dtx, bv.z));
+        hv.w = ffma(dA, hv.w, fmul(dtx, bv.w));
+        *(float4*)(Hr + 4 * n4) = hv;
+        a = dacc(a, cv.x, hv.x);
+        a = dacc(a, cv.y, hv.y);
+        a = dacc(a, cv.z, hv.z);
+        a = dacc(a, cv.w, hv.w);
+    }
+    for (int n4 = l16 + 16 * H_PRE; n4 < dm.d_state / 4; n4 += 16) {
         float4 hv = *(const float4*)(Hr + 4 * n4);
         const float4 bv = *(const float4*)(Bc + 4 * n4);
         const float4 cv = *(const float4*)(Cc + 4 * n4);
