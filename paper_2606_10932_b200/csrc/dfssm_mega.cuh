@@ -52,6 +52,7 @@ constexpr int NJ_A = 1024 / THREADS;
 constexpr int NR_IN = THREADS >= 1024 ? 2 : 4;     // in_proj sign rows per warp pass
 constexpr int LPR = THREADS / 512;            // lanes per row in the in_proj epilogue
 constexpr int LPC = 16;                       // lanes per channel in the state update
+constexpr int DMA_TID = 96;                   // the thread that issues the state write-back and the ring refills (a warp off the publish paths)
 constexpr int KS_MAX = 4;                     // largest K-split of the out_proj sign rows
 constexpr int MAX_STAGES = 8;
 constexpr uint32_t SPIN_LIMIT = 1u << 20;     // ~0.3 s of polling, then the step aborts with an error flag
@@ -881,7 +882,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 return w;
             });
             x.stamp(l, 27);
-            if (tid == 0 && nch > 0) {         // write the state slice back (async), while the exchange goes on
+            if (tid == DMA_TID && nch > 0) {   // write the state slice back (async), while the exchange goes on
                 bulk_s2g(P.ssm + (size_t)l * P.ssm_lstride + (size_t)ch0 * x.d_state(), stage + P.st_ssm, (uint32_t)nch * x.d_state() * 4);
                 bulk_s2g(conv_l + (size_t)ch0 * 4, stage + P.st_conv, (uint32_t)nch * 16);
                 bulk_commit();
@@ -987,10 +988,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 }
                 return w;
             });
-            if (tid == 0) {
-                bulk_wait_read0();                  // the state write-back has finished reading the stage
-                if (l + P.stages < n_items) issue_item(x, l + P.stages, v0, v1);
-            }
         }
         DFSSM_STAMP(l, 10);
         // ---- gather U, S1 of the next layer (or S8's norm) in every CTA ----
@@ -1003,6 +1000,12 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             qsum = norm_quant(x, SlotEnum<NJ_U>{ vu, ors, tid, x.G(), x.u_slot() >> 2 }, ssl, x.d_model(), l == P.L - 1, s_act,
                               tpn ? (int8_t*)(tpn + P.tl.off[0]) : nullptr, l, 20);
             if (tpn && tid == 0) *(float*)(tpn + P.tl.off[1]) = s_act;
+        }
+        // ---- refill this layer's ring stage with the item `stages` ahead: after the gather, so that the bulk copies do
+        //      not sit in front of its polls in the memory pipeline ----
+        if (tid == DMA_TID) {
+            bulk_wait_read0();                      // the state write-back has finished reading the stage
+            if (l + P.stages < n_items) issue_item(x, l + P.stages, v0, v1);
         }
         DFSSM_STAMP(l, 12);
     }
@@ -1068,8 +1071,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             __threadfence();
             const unsigned prev = atomicAdd(P.am_count, 1u);
             s_last = prev == (unsigned)x.G() - 1;
-            bulk_wait0();                       // all state write-backs of this CTA are complete
         }
+        if (tid == DMA_TID) bulk_wait0();       // all state write-backs of this CTA are complete
         __syncthreads();
         if (s_last && wid == 0) {
             __threadfence();
