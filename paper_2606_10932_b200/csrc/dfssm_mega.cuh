@@ -131,6 +131,23 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src, uint32
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(smem_u32(dst_smem)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
+// the same copies with an L2 evict-first policy: weights and state are touched once per token and must not push the
+// exchange mailboxes (polled every layer) or the per-layer shared blocks out of L2
+__device__ __forceinline__ uint64_t policy_evict_first()
+{
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void bulk_g2s_stream(void* dst_smem, const void* src, uint32_t bytes, uint64_t* bar, uint64_t pol)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                 ::"r"(smem_u32(dst_smem)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g_stream(void* dst, const void* src_smem, uint32_t bytes, uint64_t pol)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(dst), "r"(smem_u32(src_smem)), "r"(bytes), "l"(pol) : "memory");
+}
 __device__ __forceinline__ void bulk_s2g(void* dst, const void* src_smem, uint32_t bytes)
 {
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src_smem)), "r"(bytes) : "memory");
@@ -479,6 +496,7 @@ __device__ __forceinline__ void issue_item(const Ctx<S>& x, int item, int v0, in
     const int st = item % P.stages;
     uint8_t* stage = x.sm + P.s_ring + (size_t)st * P.stage_bytes;
     uint64_t* bar = (uint64_t*)(x.sm + P.s_mbar) + st;
+    const uint64_t pol = policy_evict_first();
     if (item < P.L) {
         const int* chs = (const int*)(x.sm + P.s_chs);
         const int ch0 = chs[x.c], nch = chs[x.c + 1] - ch0;
@@ -487,14 +505,14 @@ __device__ __forceinline__ void issue_item(const Ctx<S>& x, int item, int v0, in
         const uint32_t tin_b = e_t >= 0 ? (uint32_t)x.d_model() : 0u;
         const uint32_t tout_b = x.c < x.n_ttask() ? (uint32_t)(x.d_inner() / x.tsplit()) : 0u;
         mbar_expect_tx(bar, P.chunk_bytes + P.blk_bytes + ssm_b + conv_b + econv_b + tin_b + tout_b);
-        if (tin_b) bulk_g2s(stage + P.st_tin, P.A_in + ((size_t)item * x.r() + (e_t - x.n_bcdt())) * x.d_model(), tin_b, bar);
+        if (tin_b) bulk_g2s_stream(stage + P.st_tin, P.A_in + ((size_t)item * x.r() + (e_t - x.n_bcdt())) * x.d_model(), tin_b, bar, pol);
         if (tout_b)
-            bulk_g2s(stage + P.st_tout, P.A_out + ((size_t)item * x.r() + x.c / x.tsplit()) * x.d_inner() + (size_t)(x.c % x.tsplit()) * tout_b, tout_b, bar);
-        bulk_g2s(stage, P.chunks + ((size_t)item * x.G() + x.c) * P.chunk_bytes, P.chunk_bytes, bar);
+            bulk_g2s_stream(stage + P.st_tout, P.A_out + ((size_t)item * x.r() + x.c / x.tsplit()) * x.d_inner() + (size_t)(x.c % x.tsplit()) * tout_b, tout_b, bar, pol);
+        bulk_g2s_stream(stage, P.chunks + ((size_t)item * x.G() + x.c) * P.chunk_bytes, P.chunk_bytes, bar, pol);
         bulk_g2s(stage + P.st_blk, P.blocks + (size_t)item * P.blk_bytes, P.blk_bytes, bar);
         bulk_g2s(stage + P.st_econv, P.conv + (size_t)item * P.conv_lstride + (size_t)x.d_inner() * 4, econv_b, bar);
         if (nch > 0) {
-            bulk_g2s(stage + P.st_ssm, P.ssm + (size_t)item * P.ssm_lstride + (size_t)ch0 * x.d_state(), ssm_b, bar);
+            bulk_g2s_stream(stage + P.st_ssm, P.ssm + (size_t)item * P.ssm_lstride + (size_t)ch0 * x.d_state(), ssm_b, bar, pol);
             bulk_g2s(stage + P.st_conv, P.conv + (size_t)item * P.conv_lstride + (size_t)ch0 * 4, conv_b, bar);
         }
     } else {
@@ -502,7 +520,7 @@ __device__ __forceinline__ void issue_item(const Ctx<S>& x, int item, int v0, in
         const int nrows = min(P.lm_rows_item, v1 - row0);
         const uint32_t bytes = (uint32_t)nrows * x.d_model();
         mbar_expect_tx(bar, bytes);
-        bulk_g2s(stage, P.emb + (size_t)row0 * x.d_model(), bytes, bar);
+        bulk_g2s_stream(stage, P.emb + (size_t)row0 * x.d_model(), bytes, bar, pol);
     }
 }
 
@@ -883,7 +901,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             });
             x.stamp(l, 27);
             if (tid == DMA_TID && nch > 0) {   // write the state slice back (async), while the exchange goes on
-                bulk_s2g(P.ssm + (size_t)l * P.ssm_lstride + (size_t)ch0 * x.d_state(), stage + P.st_ssm, (uint32_t)nch * x.d_state() * 4);
+                bulk_s2g_stream(P.ssm + (size_t)l * P.ssm_lstride + (size_t)ch0 * x.d_state(), stage + P.st_ssm, (uint32_t)nch * x.d_state() * 4,
+                                policy_evict_first());
                 bulk_s2g(conv_l + (size_t)ch0 * 4, stage + P.st_conv, (uint32_t)nch * 16);
                 bulk_commit();
             }
