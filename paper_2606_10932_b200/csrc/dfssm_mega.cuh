@@ -47,7 +47,7 @@ namespace mega {
 constexpr int THREADS = 512;                  // 16 warps (measured: 32 warps only add issue pressure to the short phases)
 constexpr int NWARPS = THREADS / 32;
 constexpr int NJ_G = 2048 / THREADS;          // 16-byte chunks per thread when gathering G / U / A (plan() checks the sizes)
-constexpr int NJ_U = 1024 / THREADS;
+constexpr int NJ_U = 1536 / THREADS;
 constexpr int NJ_A = 1024 / THREADS;
 constexpr int NR_IN = THREADS >= 1024 ? 2 : 4;     // in_proj sign rows per warp pass
 constexpr int LPR = THREADS / 512;            // lanes per row in the in_proj epilogue
@@ -198,6 +198,9 @@ constexpr int MBOX = 37;                        // mailboxes of the exchange (4 
 // groups of 4 so that a gathered 16-byte chunk is four consecutive elements of one 16-element half block of codes.
 __host__ __device__ __forceinline__ int own_start(int g, int n) { return 4 * (int)(((long long)g * (n / 4)) / GRID); }
 __host__ __device__ __forceinline__ int own_max(int n) { return 4 * ((n / 4 + GRID - 1) / GRID); }
+// words of one CTA's slot in a U / G mailbox: a power of two (16, 32, 64 ...), so that a slot never straddles a 128-byte
+// line (measured: 80-byte slots cost ~1000 clocks per hop more than 64- or 128-byte ones)
+__host__ __device__ __forceinline__ int slot_words(int need) { int w = 4; while (w < need) w *= 2; return w; }
 
 template <class S>
 struct Ctx {
@@ -237,9 +240,9 @@ struct Ctx {
         return e < n_early() ? e : -1;
     }
     __device__ __forceinline__ int u_dpos() const { return (nor_max() + 1) / 2 * 2; }
-    __device__ __forceinline__ int u_slot() const { return (u_dpos() + 2 + 3) / 4 * 4; }
+    __device__ __forceinline__ int u_slot() const { return slot_words(u_dpos() + 2); }
     __device__ __forceinline__ int g_dpos() const { return (nch_max() + 1) / 2 * 2; }
-    __device__ __forceinline__ int g_slot() const { return (g_dpos() + 2 + 3) / 4 * 4; }
+    __device__ __forceinline__ int g_slot() const { return slot_words(g_dpos() + 2); }
 };
 
 __device__ __forceinline__ unsigned long long globaltimer_ns()

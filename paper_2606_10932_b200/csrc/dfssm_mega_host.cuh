@@ -84,9 +84,9 @@ inline bool plan(const Dims& d, int G, Params& P)
     P.M = MBOX;
     P.gsz = G / P.M;
     P.u_dpos = (P.nor_max + 1) / 2 * 2;
-    P.u_slot = (P.u_dpos + 2 + 3) / 4 * 4;
+    P.u_slot = slot_words(P.u_dpos + 2);
     P.g_dpos = (P.nch_max + 1) / 2 * 2;
-    P.g_slot = (P.g_dpos + 2 + 3) / 4 * 4;
+    P.g_slot = slot_words(P.g_dpos + 2);
     if (G * P.u_slot / 4 > NJ_U * THREADS || G * P.g_slot / 4 > NJ_G * THREADS) return false;
     if (P.u_slot + P.g_slot > THREADS) return false;
     uint32_t xo = 0;
