@@ -192,7 +192,16 @@ template <int DM, int DI, int HD, int DS, int NG, int R>
 struct ShapeCT { static constexpr bool kStatic = true; static constexpr int d_model = DM, d_inner = DI, headdim = HD, d_state = DS, ngroups = NG, r = R; };
 
 constexpr int GRID = 148;                       // one CTA per B200 SM
-constexpr int MBOX = 37;                        // mailboxes of the exchange (4 CTAs poll each)
+constexpr int MBOX = 37;                        // mailboxes allocated per record
+// mailboxes actually used by each part (each must divide GRID and be <= MBOX): with M the payload is pushed M times and
+// GRID / M CTAs poll each copy.  Tuned on the B200 (us per step, cfg 2): see DESIGN.md 6.2
+#ifndef DFSSM_MU
+#define DFSSM_MU 1
+#define DFSSM_MG 1
+#define DFSSM_MA 1
+#define DFSSM_MT 37
+#endif
+constexpr int M_U = DFSSM_MU, M_G = DFSSM_MG, M_A = DFSSM_MA, M_T = DFSSM_MT;
 
 // Ownership: CTA g owns elements [own_start(g, n), own_start(g + 1, n)) of a vector of length n (n % 4 == 0), in
 // groups of 4 so that a gathered 16-byte chunk is four consecutive elements of one 16-element half block of codes.
@@ -543,21 +552,21 @@ __device__ __forceinline__ void wait_item(const Ctx<S>& x, int item)
 // a reset and the later publish of a word are ordered by program order of one thread.
 //   slot (U / G): thread t < M * pps writes 16-byte piece t % pps of its slot in mailbox t / pps
 template <class S, typename F>
-__device__ __forceinline__ void slot_store(const Ctx<S>& x, uint32_t* rec, uint32_t part_off, int slot_w, F piece_value)
+__device__ __forceinline__ void slot_store(const Ctx<S>& x, uint32_t* rec, uint32_t part_off, int slot_w, int M, F piece_value)
 {
     const Params& P = x.P;
     const int pps = slot_w >> 2;
-    for (int t = x.tid; t < x.M() * pps; t += THREADS) {
+    for (int t = x.tid; t < M * pps; t += THREADS) {
         const int m = t / pps, piece = t - m * pps;
         x_st128(rec + (size_t)m * P.x_words + part_off + (size_t)x.c * slot_w + 4 * piece, piece_value(piece));
     }
 }
 //   word (A / T): the lanes of one warp write the word to all mailboxes
 template <class S>
-__device__ __forceinline__ void word_store(const Ctx<S>& x, uint32_t* rec, uint32_t part_off, int idx, uint32_t value)
+__device__ __forceinline__ void word_store(const Ctx<S>& x, uint32_t* rec, uint32_t part_off, int idx, int M, uint32_t value)
 {
     const Params& P = x.P;
-    for (int m = x.lane; m < x.M(); m += 32) x_st32(rec + (size_t)m * P.x_words + part_off + idx, value);
+    for (int m = x.lane; m < M; m += 32) x_st32(rec + (size_t)m * P.x_words + part_off + idx, value);
 }
 
 // load time: replace A_log by A = -exp(A_log) inside every chunk (same sp_expf as the step would use; R10)
@@ -616,7 +625,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
     const int h0 = nch > 0 ? ch0 / x.headdim() : 0, h1 = nch > 0 ? (ch0 + nch - 1) / x.headdim() : -1;
     const bool taps_on = TAPS && P.taps != nullptr;
     const size_t rec_words = (size_t)x.M() * P.x_words;
-    const int mbox = c / x.gsz();                      // the mailbox this CTA polls
+    auto mbox = [&](int M) { return (size_t)(c / (GRID / M)) * P.x_words; };      // offset of the mailbox this CTA polls of a part pushed M times
     const int rtid = THREADS - 1 - tid;              // the small gathers (A, T) are polled from the last warp down
     uint32_t* s_slotU = (uint32_t*)(sm + P.s_slot);
     uint32_t* s_slotG = s_slotU + x.u_slot();
@@ -672,7 +681,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         uint8_t* tp = taps_on ? P.taps + (size_t)l * P.tap_lstride : nullptr;
         float* conv_l = P.conv + (size_t)l * P.conv_lstride;
         uint32_t* rec = P.xbuf + (size_t)((P.rec0 + (uint32_t)l) & 3u) * rec_words;          // published into (all mailboxes)
-        const uint32_t* mine = rec + (size_t)mbox * P.x_words;                                 // polled
         uint32_t* recc = P.xbuf + (size_t)((P.rec0 + (uint32_t)l + 2u) & 3u) * rec_words;     // reset for layer l + 2
         DFSSM_STAMP(l, 0);
         if (x.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + 31] = globaltimer_ns();
@@ -692,7 +700,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 } else {
                     val = trow_dot(stage + P.st_tin, x.d_model(), xq, lane);
                 }
-                word_store(x, rec, P.x_A, e, (uint32_t)val ^ IBIAS);
+                word_store(x, rec, P.x_A, e, M_A, (uint32_t)val ^ IBIAS);
                 if (lane == 0 && tp && e >= x.n_bcdt()) ((int32_t*)(tp + P.tl.off[3]))[e - x.n_bcdt()] = val;
             }
         }
@@ -720,16 +728,16 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         DFSSM_STAMP(l, 2);
         {   // reset own slots of the record two layers ahead (same thread -> address map as the publishes); the warps
             // that do it are not the ones polling A, so this costs nothing on the critical path
-            slot_store(x, recc, P.x_U, x.u_slot(), [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
-            slot_store(x, recc, P.x_G, x.g_slot(), [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
-            for (int k = wid; k < nb_tasks; k += NWARPS) word_store(x, recc, P.x_A, c + k * x.G(), SENT);
-            if (wid == 0 && c < x.n_ttask()) word_store(x, recc, P.x_T, c, SENT);
+            slot_store(x, recc, P.x_U, x.u_slot(), M_U, [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
+            slot_store(x, recc, P.x_G, x.g_slot(), M_G, [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
+            for (int k = wid; k < nb_tasks; k += NWARPS) word_store(x, recc, P.x_A, c + k * x.G(), M_A, SENT);
+            if (wid == 0 && c < x.n_ttask()) word_store(x, recc, P.x_T, c, M_T, SENT);
         }
 
         // ---- gather A: accumulators of all B|C|dt rows and t_in;  v_j = a_s[j] * float(t_j) ----
         {
             uint4 va[NJ_A];
-            hop_gather<NJ_A>(x, mine + P.x_A, x.n_early(), 0, 0, va, rtid);
+            hop_gather<NJ_A>(x, rec + mbox(M_A) + P.x_A, x.n_early(), 0, 0, va, rtid);
             const float* a_s = (const float*)(blk + P.b_as_in);
 #pragma unroll
             for (int j = 0; j < NJ_A; ++j) {
@@ -889,7 +897,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             if (lane == 0) red_d(x)[wid] = ss_own;
             __syncthreads();
             x.stamp(l, 26);
-            slot_store(x, rec, P.x_G, x.g_slot(), [&](int piece) {
+            slot_store(x, rec, P.x_G, x.g_slot(), M_G, [&](int piece) {
                 uint4 w = *(const uint4*)(s_slotG + 4 * piece);
                 const int ex = x.g_dpos() - 4 * piece;
                 if (ex == 0 || ex == 2) {
@@ -917,7 +925,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         int qsum_g;
         {
             uint4 vg[NJ_G];
-            hop_gather<NJ_G>(x, mine + P.x_G, x.G() * x.g_slot(), x.g_slot(), x.g_dpos(), vg, tid);
+            hop_gather<NJ_G>(x, rec + mbox(M_G) + P.x_G, x.G() * x.g_slot(), x.g_slot(), x.g_dpos(), vg, tid);
             DFSSM_STAMP(l, 6);
             const double ssl = slot_partials<NJ_G>(x, vg, x.G(), x.g_slot(), x.g_dpos());
             qsum_g = norm_quant(x, SlotEnum<NJ_G>{ vg, chs, tid, x.G(), x.g_slot() >> 2 }, ssl, x.d_inner(), false, s_g,
@@ -930,7 +938,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             if (c < x.n_ttask()) {
                 const int part = c % x.tsplit();
                 const int t = trow_dot(stage + P.st_tout, tbytes, xq + (size_t)part * tbytes, lane);
-                word_store(x, rec, P.x_T, c, (uint32_t)t ^ IBIAS);
+                word_store(x, rec, P.x_T, c, M_T, (uint32_t)t ^ IBIAS);
             }
         } else {
             const uint32_t* bits = (const uint32_t*)(stage + P.c_out_bits);
@@ -950,7 +958,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         // ---- gather T: t_out = sum of the partial sums;  v_j = a_s[j] * float(t_j) ----
         {
             uint4 vt[1];
-            hop_gather<1>(x, mine + P.x_T, x.n_ttask(), 0, 0, vt, rtid);
+            hop_gather<1>(x, rec + mbox(M_T) + P.x_T, x.n_ttask(), 0, 0, vt, rtid);
             const float* a_s = (const float*)(blk + P.b_as_out);
             const uint32_t w[4] = { vt[0].x, vt[0].y, vt[0].z, vt[0].w };
             const int rows_per_chunk = 4 / x.tsplit();
@@ -997,7 +1005,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             ss_u = warp_sum(ss_u);
             if (lane == 0) red_d(x)[wid] = ss_u;
             __syncthreads();                        // also: every thread is done with this stage's weights
-            slot_store(x, rec, P.x_U, x.u_slot(), [&](int piece) {
+            slot_store(x, rec, P.x_U, x.u_slot(), M_U, [&](int piece) {
                 uint4 w = *(const uint4*)(s_slotU + 4 * piece);
                 const int ex = x.u_dpos() - 4 * piece;
                 if (ex == 0 || ex == 2) {
@@ -1015,7 +1023,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         // ---- gather U, S1 of the next layer (or S8's norm) in every CTA ----
         {
             uint4 vu[NJ_U];
-            hop_gather<NJ_U>(x, mine + P.x_U, x.G() * x.u_slot(), x.u_slot(), x.u_dpos(), vu, tid);
+            hop_gather<NJ_U>(x, rec + mbox(M_U) + P.x_U, x.G() * x.u_slot(), x.u_slot(), x.u_dpos(), vu, tid);
             DFSSM_STAMP(l, 11);
             const double ssl = slot_partials<NJ_U>(x, vu, x.G(), x.u_slot(), x.u_dpos());
             uint8_t* tpn = (taps_on && c == 0 && l + 1 < P.L) ? P.taps + (size_t)(l + 1) * P.tap_lstride : nullptr;
