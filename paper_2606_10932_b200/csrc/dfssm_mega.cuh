@@ -25,12 +25,14 @@
 //     Buffers are self-validating ("Lamport" style): every 32-bit word is either the sentinel 0xffffffff
 //     or payload (fp32 values are never that NaN; int32 values are stored with the sign bit flipped;
 //     fp64 partials are 8-byte stores validated by their high word), so a hop is one store and one
-//     successful poll, with no flag, fence or barrier.  Measured: when all 148 CTAs poll the SAME lines the
-//     L2 serialises them (3-6 us per hop), so every payload is PUSHED into M mailboxes (G/M CTAs poll each);
-//     the U / G payload of a CTA is one 64 / 128-byte slot written with 16-byte stores.  Records rotate
-//     over 4 (global layer counter mod 4): at layer l a CTA resets its own slots of the record that layer
-//     l+2 will use (last used by layer l-2, which every CTA has finished reading: it has since published
-//     for layer l-1), so the buffers stay L2-resident and a reset is at least two hops old when reused.
+//     successful poll, with no flag, fence or barrier.  A part can be PUSHED into M mailboxes (GRID / M CTAs poll each
+//     copy).  Measured on the B200: U, G and A are fastest pulled from ONE copy; T, which every CTA
+//     starts polling before it is written, is 2x faster pushed into 37 copies (polls delay stores to the same
+//     lines).  The U / G payload of a CTA is one 128-byte slot written with 16-byte stores (a slot that straddles
+//     a line costs ~1000 clocks per hop).  Records rotate over 4 (global layer counter mod 4): at layer l a CTA
+//     resets its own slots of the record that layer l+2 will use (last used by layer l-2, which every CTA has
+//     finished reading: it has since published for layer l-1), so the buffers stay L2-resident and a reset is at
+//     least two hops old when the word is written or polled again.
 //   * Arithmetic: identical to the chain path (dfssm_math.cuh; contract of DESIGN.md section 5).
 #pragma once
 #include <cuda_runtime.h>
@@ -316,10 +318,10 @@ __device__ __forceinline__ double* red_d(const Ctx<S>& x) { return (double*)(x.s
 
 // S1 / S6 / S8 norm + quantise of a whole vector in every CTA.  `en(f)` calls f(k, bits) for every element this
 // thread holds: bits = fp32 t_k = value_k * w_k;  ss_local = the partial sums of squares this thread holds (the
-// per-CTA partials it gathered, or its own elements' squares for the embedding).  Warp 0 reduces the warp
-// results and derives rstd / amax / scale once; every thread then quantises its elements.  Writes the codes to
+// per-CTA partials it gathered, or its own elements' squares for the embedding).  Every warp reduces the 16 warp
+// results and derives rstd / amax / scale itself; every thread then quantises its elements.  Writes the codes to
 // xq (plane order unless `canonical`), returns the sum of the codes and the activation scale s.
-// Three __syncthreads.
+// Two __syncthreads.
 template <class S, typename Enum>
 __device__ __forceinline__ int norm_quant(const Ctx<S>& x, Enum en, double ss_local, int K, bool canonical, float& s_out, int8_t* tap_codes,
                                           int pl = 0, int pk = -1)
@@ -338,19 +340,26 @@ __device__ __forceinline__ int norm_quant(const Ctx<S>& x, Enum en, double ss_lo
     if (pk >= 0) x.stamp(pl, pk);
     __syncthreads();
     if (pk >= 0) x.stamp(pl, pk + 1);
-    if (x.wid == 0) {                      // warp 0: sum of squares -> rstd
-        double ss = x.lane < NWARPS ? red_d(x)[x.lane] : 0.0;
-        ss = warp_sum(ss);
-        const float ms = (float)(ss / (double)K);
-        if (x.lane == 0) bc[1] = fdiv(1.0f, __fsqrt_rn(fadd(ms, P.eps)));
-    } else if (x.wid == 1) {               // warp 1: amax -> inv
-        float amax = x.lane < NWARPS ? red_f(x)[x.lane] : 0.0f;
-        amax = warp_max(amax);
-        if (x.lane == 0) { bc[0] = amax == 0.0f ? 0.0f : fdiv(127.0f, amax); bc[2] = amax; }
+    // every warp derives the constants itself from the NWARPS warp results (cheaper than a second barrier)
+    static_assert(NWARPS == 16, "the reductions below read 16 warp results");
+    float amax;
+    double ss;
+    {
+        const float4* rf = (const float4*)red_f(x);
+        const float4 a0 = rf[0], a1 = rf[1], a2 = rf[2], a3 = rf[3];
+        amax = fmaxf(fmaxf(fmaxf(fmaxf(a0.x, a0.y), fmaxf(a0.z, a0.w)), fmaxf(fmaxf(a1.x, a1.y), fmaxf(a1.z, a1.w))),
+                     fmaxf(fmaxf(fmaxf(a2.x, a2.y), fmaxf(a2.z, a2.w)), fmaxf(fmaxf(a3.x, a3.y), fmaxf(a3.z, a3.w))));
+        const double2* rd = (const double2*)red_d(x);
+        double2 d[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) d[i] = rd[i];
+        ss = (((d[0].x + d[0].y) + (d[1].x + d[1].y)) + ((d[2].x + d[2].y) + (d[3].x + d[3].y))) +
+             (((d[4].x + d[4].y) + (d[5].x + d[5].y)) + ((d[6].x + d[6].y) + (d[7].x + d[7].y)));
     }
-    __syncthreads();
-    const float inv = bc[0];
-    s_out = bc[2] == 0.0f ? 0.0f : fdiv(fmul(bc[2], bc[1]), 127.0f);
+    const float ms = (float)(ss / (double)K);
+    const float rstd = fdiv(1.0f, __fsqrt_rn(fadd(ms, P.eps)));
+    const float inv = amax == 0.0f ? 0.0f : fdiv(127.0f, amax);
+    s_out = amax == 0.0f ? 0.0f : fdiv(fmul(amax, rstd), 127.0f);
     if (pk >= 0) x.stamp(pl, pk + 2);
     int qs = 0;
     en([&](int k0, uint4 w) {                                       // four consecutive elements, k0 % 4 == 0
@@ -365,8 +374,9 @@ __device__ __forceinline__ int norm_quant(const Ctx<S>& x, Enum en, double ss_lo
     if (x.lane == 0) red_i(x)[x.wid] = qs;
     if (pk >= 0) x.stamp(pl, pk + 3);
     __syncthreads();
-    const int tot = x.lane < NWARPS ? red_i(x)[x.lane] : 0;
-    return warp_sum_i(tot);
+    const int4* ri = (const int4*)red_i(x);
+    const int4 q0 = ri[0], q1 = ri[1], q2 = ri[2], q3 = ri[3];
+    return ((q0.x + q0.y) + (q0.z + q0.w)) + ((q1.x + q1.y) + (q1.z + q1.w)) + ((q2.x + q2.y) + (q2.z + q2.w)) + ((q3.x + q3.y) + (q3.z + q3.w));
 }
 
 // the elements a thread holds after gathering a slot-structured mailbox part (U or G): chunk ci = tid + j*THREADS is
