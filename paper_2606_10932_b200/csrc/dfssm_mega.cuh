@@ -48,9 +48,8 @@ namespace mega {
 
 constexpr int THREADS = 512;                  // 16 warps (measured: 32 warps only add issue pressure to the short phases)
 constexpr int NWARPS = THREADS / 32;
-constexpr int NJ_G = 2048 / THREADS;          // 16-byte chunks per thread when gathering G / U / A (plan() checks the sizes)
-constexpr int NJ_U = 1536 / THREADS;
-constexpr int NJ_A = 1024 / THREADS;
+constexpr int NJ_MAX = 3072 / THREADS;        // 16-byte chunks per thread when gathering U / G with run-time shapes (plan() checks)
+constexpr int NJ_A = 1024 / THREADS;          // ... when gathering A
 constexpr int NR_IN = THREADS >= 1024 ? 2 : 4;     // in_proj sign rows per warp pass
 constexpr int LPR = THREADS / 512;            // lanes per row in the in_proj epilogue
 constexpr int LPC = 16;                       // lanes per channel in the state update
@@ -207,11 +206,13 @@ constexpr int M_U = DFSSM_MU, M_G = DFSSM_MG, M_A = DFSSM_MA, M_T = DFSSM_MT;
 
 // Ownership: CTA g owns elements [own_start(g, n), own_start(g + 1, n)) of a vector of length n (n % 4 == 0), in
 // groups of 4 so that a gathered 16-byte chunk is four consecutive elements of one 16-element half block of codes.
-__host__ __device__ __forceinline__ int own_start(int g, int n) { return 4 * (int)(((long long)g * (n / 4)) / GRID); }
-__host__ __device__ __forceinline__ int own_max(int n) { return 4 * ((n / 4 + GRID - 1) / GRID); }
+__host__ __device__ constexpr int own_start(int g, int n) { return 4 * (int)(((long long)g * (n / 4)) / GRID); }
+__host__ __device__ constexpr int own_max(int n) { return 4 * ((n / 4 + GRID - 1) / GRID); }
 // words of one CTA's slot in a U / G mailbox: a power of two (16, 32, 64 ...), so that a slot never straddles a 128-byte
 // line (measured: 80-byte slots cost ~1000 clocks per hop more than 64- or 128-byte ones)
-__host__ __device__ __forceinline__ int slot_words(int need) { int w = 4; while (w < need) w *= 2; return w; }
+__host__ __device__ constexpr int slot_words(int need) { int w = 4; while (w < need) w *= 2; return w; }
+// 16-byte chunks per thread needed to gather the slots of a vector of length n (or to hold n / 4 chunks: n_flat)
+__host__ __device__ constexpr int nj_slots(int n) { return (GRID * slot_words((own_max(n) + 1) / 2 * 2 + 2) / 4 + THREADS - 1) / THREADS; }
 
 template <class S>
 struct Ctx {
@@ -220,6 +221,9 @@ struct Ctx {
     int tid, lane, wid, c;
     volatile int* dead;          // shared flag: a poll timed out -> stop spinning everywhere
     bool prof;                   // in-kernel profiler on (a compile-time false in the production instantiations)
+    static constexpr int NJG = S::kStatic ? nj_slots(S::d_inner) : NJ_MAX;     // chunks per thread: gather G, gather U, embedding
+    static constexpr int NJU = S::kStatic ? nj_slots(S::d_model) : NJ_MAX;
+    static constexpr int NJ0 = S::kStatic ? (S::d_model / 4 + THREADS - 1) / THREADS : 8192 / 4 / THREADS;
 #define DFSSM_DIM(n_) __device__ __forceinline__ int n_() const { return S::kStatic ? S::n_ : P.n_; }
     DFSSM_DIM(d_model) DFSSM_DIM(d_inner) DFSSM_DIM(headdim) DFSSM_DIM(d_state) DFSSM_DIM(ngroups) DFSSM_DIM(r)
 #undef DFSSM_DIM
@@ -595,6 +599,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
     __shared__ int s_dead;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, c = blockIdx.x;
     Ctx<S> x{ P, sm, tid, lane, wid, c, &s_dead, PROF && P.prof != nullptr };
+    constexpr int NJ_G = Ctx<S>::NJG, NJ_U = Ctx<S>::NJU, NJ_0 = Ctx<S>::NJ0;
 
     int* chs = (int*)(sm + P.s_chs);
     int* ors = (int*)(sm + P.s_ors);
@@ -655,10 +660,10 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         }
         const int8_t* erow = P.emb + (size_t)tok * x.d_model();
         const float es = P.emb_s[tok];
-        uint4 v[NJ_G];
+        uint4 v[NJ_0];
         double ss = 0.0;
 #pragma unroll
-        for (int j = 0; j < NJ_G; ++j) {
+        for (int j = 0; j < NJ_0; ++j) {
             const int k0 = 4 * (tid + j * THREADS);
             if (k0 < x.d_model()) {
                 uint32_t w[4];
@@ -675,7 +680,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         uint8_t* tp0 = (taps_on && c == 0 && P.L > 0) ? P.taps : nullptr;
         auto en = [&](auto f) {
 #pragma unroll
-            for (int j = 0; j < NJ_G; ++j) {
+            for (int j = 0; j < NJ_0; ++j) {
                 const int k0 = 4 * (tid + j * THREADS);
                 if (k0 < x.d_model()) f(k0, v[j]);
             }

@@ -87,7 +87,7 @@ inline bool plan(const Dims& d, int G, Params& P)
     P.u_slot = slot_words(P.u_dpos + 2);
     P.g_dpos = (P.nch_max + 1) / 2 * 2;
     P.g_slot = slot_words(P.g_dpos + 2);
-    if (G * P.u_slot / 4 > NJ_U * THREADS || G * P.g_slot / 4 > NJ_G * THREADS) return false;
+    if (G * P.u_slot / 4 > NJ_MAX * THREADS || G * P.g_slot / 4 > NJ_MAX * THREADS) return false;
     if (P.u_slot + P.g_slot > THREADS) return false;
     uint32_t xo = 0;
     auto xtake = [&](size_t words) { xo = up32(xo, 32); const uint32_t at = xo; xo += (uint32_t)words; return at; };

@@ -391,3 +391,15 @@ def test_tensor_core_path_equals_dp4a_path(env):
         a.sync(); b.sync()
         assert torch.equal(a.logits(), b.logits()) and torch.equal(a.hidden(), b.hidden())
         assert torch.equal(a.next_tokens(), b.next_tokens())
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg_idx", [0, 1, 2, 4])
+def test_every_baseline_shape_runs_the_persistent_kernel_at_batch_1(env, cfg_idx):
+    """A shape that silently falls back to the 300-launch chain at batch 1 is a performance regression, not a parity one:
+    every BASELINE.json shape must fit the one-launch persistent kernel."""
+    pk = env["pk"]
+    s = ds.shape_for_config(cfg_idx)
+    m = pk.Model(pk.Config.from_shape(s, max_batch=1))
+    assert m.launches_per_step(1) == 1
+    m.close()
