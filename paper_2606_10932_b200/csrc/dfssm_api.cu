@@ -365,7 +365,10 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
     tm->end(); ++nl;
 
     tm->begin(DFSSM_KCLASS_LMHEAD);
-    {
+    if (use_mma(c, batch, d.d_model)) {
+        mma::k_proj_mma<<<dim3((d.vocab + mma::TM - 1) / mma::TM, (batch + mma::TN - 1) / mma::TN, 1), mma::THREADS, 0, st>>>(
+            nullptr, c->emb, 0, d.vocab, d.d_model, xq, ldq, batch, nullptr, 0, nullptr, err, logits, sx, c->emb_s);
+    } else {
         const int per = LM_THREADS / 32;
         int gx = (d.vocab + per - 1) / per;
         if (gx > 148 * 16) gx = 148 * 16;
@@ -655,6 +658,9 @@ int dfssm_reset_state(dfssm_ctx* ctx, int seq)
     if (seq < 0) {
         CK(cudaMemsetAsync(ctx->arena + v.ssm, 0, nl * B * v.ssm_elems * 4, ctx->stream));
         CK(cudaMemsetAsync(ctx->arena + v.conv, 0, nl * B * (size_t)d.conv_dim * 16, ctx->stream));
+        // the exchange records of the persistent kernel go back to "nothing written" too (matters only after a step that
+        // was aborted by a poll time-out and left half-written records behind)
+        if (v.mega_fit) CK(cudaMemsetAsync(ctx->arena + v.m_x, 0xff, v.m_xbytes, ctx->stream));
         return DFSSM_OK;
     }
     // one sequence of every layer: strided 2-D memsets (rows = layers)

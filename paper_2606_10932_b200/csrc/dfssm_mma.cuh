@@ -4,6 +4,7 @@
 // appended as further int8 rows of the same tile, the activation codes are the N operand, and the int32 accumulators
 // live in TMEM: tcgen05.mma.kind::i8, M = 128, N = 64, K = 32 per instruction, issued by one thread; tcgen05.commit ->
 // mbarrier tells the CTA that the shared-memory tile may be overwritten; tcgen05.ld brings the accumulators back.
+// The tied int8 LM head (S8) is the same contraction with the embedding rows as the int8 rows and a float epilogue.
 // Integer arithmetic: exact, so the results are bit-identical to the dp4a path (k_proj).
 //
 // Shared-memory operand layout (K-major, no swizzle; "core matrix" = 8 rows x 16 bytes, stored contiguously):
@@ -42,12 +43,14 @@ __device__ __forceinline__ uint32_t signs4(uint32_t bits)
     return 0xffffffffu ^ (spread * 0xfeu);
 }
 
-// grid = (ceil((rows + r) / 128), ceil(batch / 64), ksplit); 128 threads; K % 128 == 0.  With ksplit > 1 every CTA takes a
+// grid = (ceil((rows + r) / 128), ceil(batch / 64), ksplit); 128 threads; K % 128 == 0.  LM head: rows = 0, r = vocab,
+// A = the embedding, ksplit = 1, logits / s_h / e_s given.  With ksplit > 1 every CTA takes a
 // slice of K and ADDS its int32 partial sums into acc / t (exact in any order), which the caller has zeroed.
 __global__ void __launch_bounds__(THREADS)
 k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int rows, int r, int K,
            const int8_t* __restrict__ xq, int ldq, int batch, int32_t* __restrict__ acc, int ld_acc,
-           int32_t* __restrict__ t, int* __restrict__ err)
+           int32_t* __restrict__ t, int* __restrict__ err,
+           float* __restrict__ logits = nullptr, const float* __restrict__ s_h = nullptr, const float* __restrict__ e_s = nullptr)
 {
     __shared__ __align__(128) uint8_t sA[TM * KC];
     __shared__ __align__(128) uint8_t sB[TN * KC];
@@ -154,6 +157,10 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
             for (int i = 0; i < 16; ++i) {
                 const int b = b0 + q * 16 + i;
                 if (b < batch) {
+                    if (logits) {          // S8: logit_v = float(acc_v) * (s_h * e_s[v])   (R16); rows == 0, r == vocab
+                        if (is_t) logits[(size_t)b * r + grow] = fmul((float)(int32_t)v[i], fmul(s_h[b], e_s[grow]));
+                        continue;
+                    }
                     int32_t* dst = is_acc ? acc + (size_t)b * ld_acc + grow : t + (size_t)b * T_STRIDE + (grow - rows);
                     if (is_acc || is_t) {
                         if (split) atomicAdd(dst, (int32_t)v[i]);
