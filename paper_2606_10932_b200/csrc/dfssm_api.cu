@@ -226,7 +226,7 @@ struct KTimer {                       // optional per-kernel-class device timing
 
 size_t proj_smem(int K) { return (size_t)PROJ_BT * 2 * K; }
 size_t lm_smem(int K) { return (size_t)PROJ_BT * K; }
-size_t ssm_smem(const Dims& d) { return sizeof(float) * (64 + 2 * (size_t)d.d_state + 2 * SSM_PB + 4); }
+size_t ssm_smem(const Dims& d) { return sizeof(float) * (64 + 2 * (size_t)d.d_state + 2 * 32 + 4); }
 
 int proj_grid(int rows_total)
 {
@@ -328,8 +328,12 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         k_bcdt<<<dim3((2 * d.ngroups * d.d_state + d.nheads + BCDT_THREADS - 1) / BCDT_THREADS, batch), BCDT_THREADS, 0, st>>>(
             L, d, acc, ld_acc, t, sx, conv, pos, at<float>(c, v.bcdt), tp, v.tap_stride, v.tl);
         ++nl;
-        k_ssm<<<dim3(d.nheads * (d.headdim / SSM_PB), batch), SSM_THREADS, ssm_smem(d), st>>>(
-            L, d, acc, ld_acc, t, sx, conv, pos, ssm, g, at<float>(c, v.bcdt), tp, v.tap_stride, v.tl);
+        if (d.headdim % 32 == 0)
+            k_ssm<32><<<dim3(d.nheads * (d.headdim / 32), batch), SSM_THREADS, ssm_smem(d), st>>>(
+                L, d, acc, ld_acc, t, sx, conv, pos, ssm, g, at<float>(c, v.bcdt), tp, v.tap_stride, v.tl);
+        else
+            k_ssm<16><<<dim3(d.nheads * (d.headdim / 16), batch), SSM_THREADS, ssm_smem(d), st>>>(
+                L, d, acc, ld_acc, t, sx, conv, pos, ssm, g, at<float>(c, v.bcdt), tp, v.tap_stride, v.tl);
         tm->end(); ++nl;
 
         tm->begin(DFSSM_KCLASS_NORMQUANT);

@@ -293,13 +293,15 @@ k_bcdt(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int
 
 // =============================================================================================
 // S3 stage 2 (for the rows a head needs) + S4 conv step + S5 state update/readout + S6 gate.
-//   grid = (nheads * headdim/SSM_PB, batch); one CTA owns SSM_PB (head, p) rows of the state.
+//   grid = (nheads * headdim/PB, batch); one CTA owns PB (head, p) rows of the state: PB = 32 when headdim allows
+//   (16 KB of state per CTA: the kernel is bound by per-CTA latency x occupancy, so more state per CTA is faster), else 16.
 //   The B | C | dt rows are finished once per sequence by k_bcdt and read from its buffer.
 //   Conv state is a 4-slot ring per channel: the sample of step t lives in slot t%4, so the
 //   readers of a step never touch the slot its owner writes.
 // =============================================================================================
 constexpr int SSM_THREADS = 256;
 
+template <int PB>
 __global__ void __launch_bounds__(SSM_THREADS)
 k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int32_t* __restrict__ t,
       const float* __restrict__ s_x, float* __restrict__ conv_ring /* [batch][conv_dim][4] */,
@@ -311,14 +313,16 @@ k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
     float* v_sh = (float*)smem;                    // [64]
     float* Bc = v_sh + 64;                         // [d_state]
     float* Cc = Bc + dm.d_state;                   // [d_state]
-    float* xs = Cc + dm.d_state;                   // [SSM_PB]
-    float* zs = xs + SSM_PB;                       // [SSM_PB]
-    float* dts = zs + SSM_PB;                      // [1] (+pad)
+    float* xs = Cc + dm.d_state;                   // [PB]
+    float* zs = xs + PB;                           // [PB]
+    float* dts = zs + PB;                          // [1] (+pad)
+    constexpr int LANES = SSM_THREADS / PB;        // lanes per state row (16 or 8)
+    constexpr int ROWL = SSM_THREADS / (2 * PB);   // lanes per own in_proj row (8 or 4)
 
     const int b = blockIdx.y;
-    const int pblocks = dm.headdim / SSM_PB;
+    const int pblocks = dm.headdim / PB;
     const int h = blockIdx.x / pblocks, pblk = blockIdx.x % pblocks;
-    const int p0 = pblk * SSM_PB;
+    const int p0 = pblk * PB;
     const int hpg = dm.nheads / dm.ngroups;
     const int grp = h / hpg;
     const int tid = threadIdx.x;
@@ -328,13 +332,13 @@ k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
     uint8_t* tp = taps ? taps + (size_t)b * tap_stride : nullptr;
 
     // this thread's slice of the state is requested first, so that HBM works while the rows below are finished
-    const int p = tid >> 4, l16 = tid & 15;       // 16 rows x 16 lanes
+    const int p = tid / LANES, l16 = tid % LANES;  // PB rows x LANES lanes
     float* Hr = ssm + (((size_t)b * dm.nheads + h) * dm.headdim + p0 + p) * dm.d_state;
-    constexpr int H_PRE = 2;                      // chunks held in registers (all of d_state = 128); further ones are loaded late
+    constexpr int H_PRE = 32 / LANES;             // chunks held in registers (all of d_state = 128); further ones are loaded late
     float4 hpre[H_PRE];
 #pragma unroll
     for (int j = 0; j < H_PRE; ++j) {
-        const int n4 = l16 + 16 * j;
+        const int n4 = l16 + LANES * j;
         if (n4 < dm.d_state / 4) hpre[j] = *(const float4*)(Hr + 4 * n4);
     }
 
@@ -350,18 +354,16 @@ k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
     }
     __syncthreads();
 
-    // the 2 * SSM_PB own rows (z, x): 8 lanes share a row's LoRA sum (fp64, any tree: DESIGN.md 5.3)
-    static_assert(SSM_THREADS == 8 * 2 * SSM_PB, "8 lanes per own row");
+    // the 2 * PB own rows (z, x): ROWL lanes share a row's LoRA sum (fp64, any tree: DESIGN.md 5.3)
     {
-        const int i = tid >> 3, sub = tid & 7;
-        const int kind = i < SSM_PB ? 0 : 1, idx = i - kind * SSM_PB;      // kind 0 z, 1 x
+        const int i = tid / ROWL, sub = tid % ROWL;
+        const int kind = i < PB ? 0 : 1, idx = i - kind * PB;              // kind 0 z, 1 x
         const int row = kind * dm.d_inner + h * dm.headdim + p0 + idx;
         const int8_t* brow = L.in_B + (size_t)row * dm.r;
         double lo = 0.0;
-        for (int j = sub; j < dm.r; j += 8) lo = dacc(lo, (float)brow[j], v_sh[j]);
-        lo += __shfl_xor_sync(0xffffffffu, lo, 1);
-        lo += __shfl_xor_sync(0xffffffffu, lo, 2);
-        lo += __shfl_xor_sync(0xffffffffu, lo, 4);
+        for (int j = sub; j < dm.r; j += ROWL) lo = dacc(lo, (float)brow[j], v_sh[j]);
+#pragma unroll
+        for (int o = 1; o < ROWL; o <<= 1) lo += __shfl_xor_sync(0xffffffffu, lo, o);
         if (sub == 0) {
             const float m1 = fmul(__half2float(L.in_row_scale[row]), (float)accb[row]);
             const float m2 = fmul(L.in_b_s[row], (float)lo);
@@ -398,7 +400,7 @@ k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
     double a = 0.0;
 #pragma unroll
     for (int j = 0; j < H_PRE; ++j) {
-        const int n4 = l16 + 16 * j;
+        const int n4 = l16 + LANES * j;
         if (n4 >= dm.d_state / 4) break;
         float4 hv = hpre[j];
         const float4 bv = *(const float4*)(Bc + 4 * n4);
@@ -413,7 +415,7 @@ k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
         a = dacc(a, cv.z, hv.z);
         a = dacc(a, cv.w, hv.w);
     }
-    for (int n4 = l16 + 16 * H_PRE; n4 < dm.d_state / 4; n4 += 16) {
+    for (int n4 = l16 + LANES * H_PRE; n4 < dm.d_state / 4; n4 += LANES) {
         float4 hv = *(const float4*)(Hr + 4 * n4);
         const float4 bv = *(const float4*)(Bc + 4 * n4);
         const float4 cv = *(const float4*)(Cc + 4 * n4);
@@ -428,7 +430,7 @@ k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
         a = dacc(a, cv.w, hv.w);
     }
 #pragma unroll
-    for (int o = 8; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o, 16);
+    for (int o = LANES / 2; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o, LANES);
     if (l16 == 0) {
         a = dacc(a, L.D[h], xv);
         const float y = (float)a;
