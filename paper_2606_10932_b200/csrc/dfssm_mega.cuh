@@ -779,13 +779,16 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             const float* ering = (const float*)(stage + P.st_econv);
             // rows [first, first + count) of the index space (z | x | B|C | dt), skipping skip_len rows from skip_from on;
             // LP lanes share a row's LoRA sum
-            auto epi = [&](auto lp_tag, int first, int count, int skip_from, int skip_len) {
+            // done by the threads [t0, t0 + nthr) (whole warps)
+            auto epi = [&](auto lp_tag, int first, int count, int skip_from, int skip_len, int t0, int nthr) {
               constexpr int LP = decltype(lp_tag)::value;
-              for (int ib = 0; ib < count; ib += THREADS / LP) {       // warp-uniform trip count (shuffles inside)
-                int i = first + min(ib + tid / LP, count - 1);
+              const int lt = tid - t0;
+              if (lt < 0 || lt >= nthr) return;
+              for (int ib = 0; ib < count; ib += nthr / LP) {          // warp-uniform trip count (shuffles inside)
+                int i = first + min(ib + lt / LP, count - 1);
                 if (i >= skip_from) i += skip_len;
-                const int sub = tid % LP;
-                const bool valid = ib + tid / LP < count;
+                const int sub = lt % LP;
+                const bool valid = ib + lt / LP < count;
                 int kind, slot = 0, e = 0;         // kind 0 z, 1 x, 2 B|C, 3 dt
                 if (i < nch) { kind = 0; slot = i; }
                 else if (i < 2 * nch) { kind = 1; slot = x.nch_max() + (i - nch); }
@@ -854,9 +857,10 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 }
               }
             };
-            // the 2 gs B|C rows with 2 lanes each, then the few own rows (z, x, dt) with 8 lanes each
-            epi(std::integral_constant<int, 2>{}, 2 * nch, 2 * x.gs(), 1 << 30, 0);
-            epi(std::integral_constant<int, 8>{}, 0, 2 * nch + n_dt, 2 * nch, 2 * x.gs());
+            // first half of the CTA: the 2 gs B|C rows, one thread per row (dense tails); second half, at the same time: the
+            // few own rows (z, x, dt) with 4 lanes each
+            epi(std::integral_constant<int, 1>{}, 2 * nch, 2 * x.gs(), 1 << 30, 0, 0, THREADS / 2);
+            epi(std::integral_constant<int, 4>{}, 0, 2 * nch + n_dt, 2 * nch, 2 * x.gs(), THREADS / 2, THREADS / 2);
         }
         __syncthreads();
         DFSSM_STAMP(l, 4);
