@@ -463,34 +463,19 @@ __device__ __forceinline__ void sign_partial(const uint32_t* const (&rowp)[NR], 
                (a[r][6] << 1) + a[r][7];
 }
 
-// transposing reduction of 4 per-lane values: lane 8r ends up with the warp total of p[r]
+// reduction of 4 per-lane values: lane 8r ends up with the warp total of p[r] (one REDUX per value)
 __device__ __forceinline__ int reduce4(const int (&p)[4], int lane)
 {
-    const bool up16 = (lane & 16) != 0, up8 = (lane & 8) != 0;
-    int k0 = up16 ? p[2] : p[0], k1 = up16 ? p[3] : p[1];
-    const int s0 = up16 ? p[0] : p[2], s1 = up16 ? p[1] : p[3];
-    k0 += __shfl_xor_sync(0xffffffffu, s0, 16);
-    k1 += __shfl_xor_sync(0xffffffffu, s1, 16);
-    int v = up8 ? k1 : k0;
-    const int sv = up8 ? k0 : k1;
-    v += __shfl_xor_sync(0xffffffffu, sv, 8);
-    v += __shfl_xor_sync(0xffffffffu, v, 4);
-    v += __shfl_xor_sync(0xffffffffu, v, 2);
-    v += __shfl_xor_sync(0xffffffffu, v, 1);
-    return v;
+    const int t0 = __reduce_add_sync(0xffffffffu, p[0]), t1 = __reduce_add_sync(0xffffffffu, p[1]);
+    const int t2 = __reduce_add_sync(0xffffffffu, p[2]), t3 = __reduce_add_sync(0xffffffffu, p[3]);
+    const int r = lane >> 3;
+    return r == 0 ? t0 : r == 1 ? t1 : r == 2 ? t2 : t3;
 }
 // same for 2 values: lane 16r ends up with the warp total of p[r]
 __device__ __forceinline__ int reduce2(const int (&p)[2], int lane)
 {
-    const bool up16 = (lane & 16) != 0;
-    int v = up16 ? p[1] : p[0];
-    const int sv = up16 ? p[0] : p[1];
-    v += __shfl_xor_sync(0xffffffffu, sv, 16);
-    v += __shfl_xor_sync(0xffffffffu, v, 8);
-    v += __shfl_xor_sync(0xffffffffu, v, 4);
-    v += __shfl_xor_sync(0xffffffffu, v, 2);
-    v += __shfl_xor_sync(0xffffffffu, v, 1);
-    return v;
+    const int t0 = __reduce_add_sync(0xffffffffu, p[0]), t1 = __reduce_add_sync(0xffffffffu, p[1]);
+    return (lane & 16) ? t1 : t0;
 }
 
 template <int NR> struct RowReduce;       // lane (32 / NR) * r ends up with the warp total of p[r]
