@@ -106,6 +106,13 @@ __device__ __forceinline__ double warp_sum(double v)
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
 }
+// sum over the lanes {k, k + stride, k + 2 stride, ...} (stride a power of two; the other lanes hold 0): the result is
+// valid in those lanes.  Saves log2(stride) of the five fp64 shuffle steps when only every stride-th lane has a value.
+__device__ __forceinline__ double warp_sum_strided(double v, int stride)
+{
+    for (int o = stride; o < 32; o <<= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
 // max of NON-NEGATIVE floats (all uses: |x| maxima): their bit patterns order like unsigned integers, so one REDUX does it
 __device__ __forceinline__ float warp_max(float v)
 {

@@ -327,8 +327,8 @@ __device__ __forceinline__ double* red_d(const Ctx<S>& x) { return (double*)(x.s
 // xq (plane order unless `canonical`), returns the sum of the codes and the activation scale s.
 // Two __syncthreads.
 template <class S, typename Enum>
-__device__ __forceinline__ int norm_quant(const Ctx<S>& x, Enum en, double ss_local, int K, bool canonical, float& s_out, int8_t* tap_codes,
-                                          int pl = 0, int pk = -1)
+__device__ __forceinline__ int norm_quant(const Ctx<S>& x, Enum en, double ss_local, int dstride, int dlane, int K, bool canonical, float& s_out,
+                                          int8_t* tap_codes, int pl = 0, int pk = -1)
 {
     const Params& P = x.P;
     uint8_t* xq = x.sm + P.s_xq;
@@ -339,8 +339,9 @@ __device__ __forceinline__ int norm_quant(const Ctx<S>& x, Enum en, double ss_lo
         am = fmaxf(fmaxf(am, fabsf(__uint_as_float(w.z))), fabsf(__uint_as_float(w.w)));
     });
     am = warp_max(am);
-    ss_local = warp_sum(ss_local);
-    if (x.lane == 0) { red_f(x)[x.wid] = am; red_d(x)[x.wid] = ss_local; }
+    ss_local = warp_sum_strided(ss_local, dstride);      // only the lanes dlane + k * dstride hold partial sums
+    if (x.lane == 0) red_f(x)[x.wid] = am;
+    if (x.lane == dlane) red_d(x)[x.wid] = ss_local;
     if (pk >= 0) x.stamp(pl, pk);
     __syncthreads();
     if (pk >= 0) x.stamp(pl, pk + 1);
@@ -670,7 +671,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 if (k0 < x.d_model()) f(k0, v[j]);
             }
         };
-        qsum = norm_quant(x, en, ss, x.d_model(), P.L == 0, s_act, tp0 ? (int8_t*)(tp0 + P.tl.off[0]) : nullptr);
+        qsum = norm_quant(x, en, ss, 1, 0, x.d_model(), P.L == 0, s_act, tp0 ? (int8_t*)(tp0 + P.tl.off[0]) : nullptr);
         if (tp0 && tid == 0) *(float*)(tp0 + P.tl.off[1]) = s_act;
     }
 
@@ -897,7 +898,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             x.stamp(l, 24);
             fence_proxy_async();               // the updated state is about to be read by the async proxy
             x.stamp(l, 25);
-            ss_own = warp_sum(ss_own);
+            ss_own = warp_sum_strided(ss_own, LPC);     // only lanes 0 and 16 hold a value
             if (lane == 0) red_d(x)[wid] = ss_own;
             __syncthreads();
             x.stamp(l, 26);
@@ -932,7 +933,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             hop_gather<NJ_G>(x, rec + mbox(M_G) + P.x_G, x.G() * x.g_slot(), x.g_slot(), x.g_dpos(), vg, tid);
             DFSSM_STAMP(l, 6);
             const double ssl = slot_partials<NJ_G>(x, vg, x.G(), x.g_slot(), x.g_dpos());
-            qsum_g = norm_quant(x, SlotEnum<NJ_G>{ vg, chs, tid, x.G(), x.g_slot() >> 2 }, ssl, x.d_inner(), false, s_g,
+            const int gpps = x.g_slot() >> 2;            // the fp64 partials sit in the lanes (g_dpos / 4) mod pps
+            qsum_g = norm_quant(x, SlotEnum<NJ_G>{ vg, chs, tid, x.G(), gpps }, ssl, gpps < 32 ? gpps : 1, gpps < 32 ? (x.g_dpos() >> 2) % gpps : 0,
+                                x.d_inner(), false, s_g,
                                 (tp && c == 0) ? (int8_t*)(tp + P.tl.off[9]) : nullptr, l, 16);
             if (tp && c == 0 && tid == 0) *(float*)(tp + P.tl.off[10]) = s_g;
         }
@@ -1006,7 +1009,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 ss_u = dacc(ss_u, un, un);
                 if (tp) { ((float*)(tp + P.tl.off[13]))[or0 + i] = un; ((int32_t*)(tp + P.tl.off[11]))[or0 + i] = acc; }
             }
-            ss_u = warp_sum(ss_u);
+            ss_u = warp_sum_strided(ss_u, 4);           // only every fourth lane holds a value
             if (lane == 0) red_d(x)[wid] = ss_u;
             __syncthreads();                        // also: every thread is done with this stage's weights
             slot_store(x, rec, P.x_U, x.u_slot(), M_U, [&](int piece) {
@@ -1031,7 +1034,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             DFSSM_STAMP(l, 11);
             const double ssl = slot_partials<NJ_U>(x, vu, x.G(), x.u_slot(), x.u_dpos());
             uint8_t* tpn = (taps_on && c == 0 && l + 1 < P.L) ? P.taps + (size_t)(l + 1) * P.tap_lstride : nullptr;
-            qsum = norm_quant(x, SlotEnum<NJ_U>{ vu, ors, tid, x.G(), x.u_slot() >> 2 }, ssl, x.d_model(), l == P.L - 1, s_act,
+            const int upps = x.u_slot() >> 2;
+            qsum = norm_quant(x, SlotEnum<NJ_U>{ vu, ors, tid, x.G(), upps }, ssl, upps < 32 ? upps : 1, upps < 32 ? (x.u_dpos() >> 2) % upps : 0,
+                              x.d_model(), l == P.L - 1, s_act,
                               tpn ? (int8_t*)(tpn + P.tl.off[0]) : nullptr, l, 20);
             if (tpn && tid == 0) *(float*)(tpn + P.tl.off[1]) = s_act;
         }
