@@ -781,11 +781,13 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 else if (i < 2 * nch + 2 * x.gs()) { kind = 2; e = i - 2 * nch; }
                 else { kind = 3; e = 2 * x.gs() + (tp ? 0 : h0) + (i - 2 * nch - 2 * x.gs()); }
                 const bool own = kind < 2;
-                const int8_t* brow = own ? (const int8_t*)(stage + P.c_in_B) + (size_t)slot * x.r_pad()
-                                         : (const int8_t*)(blk + P.b_eB) + (size_t)e * x.r_pad();
+                // LoRA-up row as 4-byte words: own rows are [slot][r_pad]; the B|C|dt rows of the shared block are stored word-major
+                // ([r_pad / 4][n_bcdt]) so that one thread per row reads shared memory without bank conflicts
+                const int* bw = own ? (const int*)(stage + P.c_in_B + (size_t)slot * x.r_pad()) : (const int*)(blk + P.b_eB) + e;
+                const int bstep = own ? 1 : x.n_bcdt();
                 double lo0 = 0.0, lo1 = 0.0;
                 for (int j4 = 4 * sub; j4 < x.r_pad(); j4 += 4 * LP) {         // pad entries of B are 0, pad entries of v are 0
-                    const int w = *(const int*)(brow + j4);
+                    const int w = bw[(j4 >> 2) * bstep];
                     lo0 = __fma_rn((double)(int8_t)w, s_vin[j4], lo0);
                     lo1 = __fma_rn((double)(int8_t)(w >> 8), s_vin[j4 + 1], lo1);
                     lo0 = __fma_rn((double)(int8_t)(w >> 16), s_vin[j4 + 2], lo0);

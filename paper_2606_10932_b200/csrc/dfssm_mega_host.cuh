@@ -239,7 +239,11 @@ inline void pack_block(const Params& P, const HostLayer& H, uint8_t* out)
     memset(out, 0, P.blk_bytes);
     for (int e = 0; e < P.n_bcdt; ++e) {
         const int row = 2 * P.d_inner + e;
-        memcpy(out + P.b_eB + (size_t)e * P.r_pad, H.in_B + (size_t)row * P.r, P.r);
+        {   // word-major: word g of row e (its LoRA-up bytes 4g .. 4g+3, zero padded) at [g][e]
+            uint8_t rowb[64] = { 0 };
+            memcpy(rowb, H.in_B + (size_t)row * P.r, P.r);
+            for (int g = 0; g < P.r_pad / 4; ++g) memcpy(out + P.b_eB + ((size_t)g * P.n_bcdt + e) * 4, rowb + 4 * g, 4);
+        }
         ((float*)(out + P.b_escale))[e] = half_bits_to_float(H.in_row_scale[row]);
         ((float*)(out + P.b_ebs))[e] = H.in_b_s[row];
         if (e < 2 * P.gs) {
