@@ -202,6 +202,12 @@ constexpr int MBOX = 37;                        // mailboxes allocated per recor
 #define DFSSM_MA 1
 #define DFSSM_MT 37
 #endif
+// clocks a CTA waits after publishing G / U before its first poll: polls that reach a line before the data delay the
+// stores to it (measured: 0 -> 0.501 ms/step, 300..700 -> 0.488)
+#ifndef DFSSM_WG
+#define DFSSM_WG 500
+#define DFSSM_WU 500
+#endif
 constexpr int M_U = DFSSM_MU, M_G = DFSSM_MG, M_A = DFSSM_MA, M_T = DFSSM_MT;
 
 // Ownership: CTA g owns elements [own_start(g, n), own_start(g + 1, n)) of a vector of length n (n % 4 == 0), in
@@ -285,8 +291,12 @@ __device__ __forceinline__ void poll_fail(const Ctx<S>& x)
 // Spins until every owned word has been written; the raw words come back in v[].  tix = the thread's index for
 // the chunk ownership (tid, or reversed so that the small gathers are polled by the warps that have nothing else to do).
 template <int NJ, class S>
-__device__ __forceinline__ void hop_gather(const Ctx<S>& x, const uint32_t* buf, int nw, int slot_w, int dpos, uint4 (&v)[NJ], int tix)
+__device__ __forceinline__ void hop_gather(const Ctx<S>& x, const uint32_t* buf, int nw, int slot_w, int dpos, uint4 (&v)[NJ], int tix, int first_wait = 0)
 {
+    if (first_wait > 0) {                          // polls that arrive before the data delay the stores to the same lines
+        const long long t0 = clock64();
+        while (clock64() - t0 < first_wait) {}
+    }
     const int nchunk = (nw + 3) >> 2;
     bool need[NJ];
 #pragma unroll
@@ -932,7 +942,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         int qsum_g;
         {
             uint4 vg[NJ_G];
-            hop_gather<NJ_G>(x, rec + mbox(M_G) + P.x_G, x.G() * x.g_slot(), x.g_slot(), x.g_dpos(), vg, tid);
+            hop_gather<NJ_G>(x, rec + mbox(M_G) + P.x_G, x.G() * x.g_slot(), x.g_slot(), x.g_dpos(), vg, tid, DFSSM_WG);
             DFSSM_STAMP(l, 6);
             const double ssl = slot_partials<NJ_G>(x, vg, x.G(), x.g_slot(), x.g_dpos());
             const int gpps = x.g_slot() >> 2;            // the fp64 partials sit in the lanes (g_dpos / 4) mod pps
@@ -1032,7 +1042,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         // ---- gather U, S1 of the next layer (or S8's norm) in every CTA ----
         {
             uint4 vu[NJ_U];
-            hop_gather<NJ_U>(x, rec + mbox(M_U) + P.x_U, x.G() * x.u_slot(), x.u_slot(), x.u_dpos(), vu, tid);
+            hop_gather<NJ_U>(x, rec + mbox(M_U) + P.x_U, x.G() * x.u_slot(), x.u_slot(), x.u_dpos(), vu, tid, DFSSM_WU);
             DFSSM_STAMP(l, 11);
             const double ssl = slot_partials<NJ_U>(x, vu, x.G(), x.u_slot(), x.u_dpos());
             uint8_t* tpn = (taps_on && c == 0 && l + 1 < P.L) ? P.taps + (size_t)(l + 1) * P.tap_lstride : nullptr;
