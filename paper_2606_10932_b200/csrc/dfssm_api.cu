@@ -244,12 +244,16 @@ bool use_mma(const dfssm_ctx* c, int batch, int K)
 
 // one projection on the tensor cores; K is split over CTAs until the grid fills the 148 SMs (partial sums are added
 // with integer atomics into zeroed buffers: exact, order-independent)
+// K is split until this many CTAs share an SM: a CTA is 4 warps that unpack, issue and wait in turn, so co-resident CTAs are
+// what hides its latencies (measured, cfg 3, ms/step at batch 64 / 16: 1 CTA 5.72 / 3.52, 2 CTAs 5.46 / 3.24, 3 CTAs 5.49 / 3.29,
+// 4 CTAs 5.53 / 3.23)
+constexpr int MMA_CTAS_PER_SM = 2;
 int launch_proj_mma(dfssm_ctx* ctx, const uint32_t* sign, const int8_t* A, int rows, int K, int batch)
 {
     const Dims& d = ctx->dm;
     const Carve& v = ctx->cv;
     const int mt = (rows + d.r + mma::TM - 1) / mma::TM, nt = (batch + mma::TN - 1) / mma::TN, nchunk = K / mma::KC;
-    int ks = 148 / (mt * nt);
+    int ks = (148 * MMA_CTAS_PER_SM) / (mt * nt);
     if (ks < 1) ks = 1;
     if (ks > nchunk) ks = nchunk;
     int32_t* acc = at<int32_t>(ctx, v.acc);

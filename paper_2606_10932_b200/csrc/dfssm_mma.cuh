@@ -83,11 +83,22 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
 
     const int nchunk = K / KC, kc0 = (int)(((long long)blockIdx.z * nchunk) / gridDim.z), kc1 = (int)(((long long)(blockIdx.z + 1) * nchunk) / gridDim.z);
     const bool split = gridDim.z > 1;
+    // the sign words and the codes of a chunk are requested one chunk ahead (registers), so that their latency runs under the
+    // MMAs and the wait of the chunk before; the few LoRA-down rows (last tile only) are read directly
+    const bool is_sign = grow < rows;
+    const uint32_t* sign_row = sign + (size_t)(is_sign ? grow : 0) * W;
+    const int8_t* x_row = xq + (size_t)(b_valid ? b0 + bn : 0) * ldq + bhalf * (KC / 2);
+    uint4 w_next = make_uint4(0, 0, 0, 0), x_next[KC / 32];
+    auto request = [&](int kc) {
+        if (is_sign) w_next = *(const uint4*)(sign_row + kc * (KC / 32));
+#pragma unroll
+        for (int c = 0; c < KC / 32; ++c) x_next[c] = b_valid ? ((const uint4*)(x_row + kc * KC))[c] : make_uint4(0, 0, 0, 0);
+    };
+    if (kc0 < kc1) request(kc0);
     for (int kc = kc0; kc < kc1; ++kc) {
         // ---- A: 128 weights of this row -> int8 ----
-        if (grow < rows) {
-            const uint4 w = *(const uint4*)(sign + (size_t)grow * W + kc * (KC / 32));
-            const uint32_t ww[4] = { w.x, w.y, w.z, w.w };
+        if (is_sign) {
+            const uint32_t ww[4] = { w_next.x, w_next.y, w_next.z, w_next.w };
 #pragma unroll
             for (int c = 0; c < KC / 16; ++c) {                       // 16 weights per 16-byte K column
                 const uint32_t b16 = (ww[c >> 1] >> (16 * (c & 1))) & 0xffffu;
@@ -102,12 +113,8 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
             for (int c = 0; c < KC / 16; ++c) *(uint4*)(a_dst + c * LBO_A) = make_uint4(0, 0, 0, 0);
         }
         // ---- B: 64 codes of one sequence ----
-        {
-            const uint4* src = (const uint4*)(xq + (size_t)(b0 + bn) * ldq + kc * KC + bhalf * (KC / 2));
 #pragma unroll
-            for (int c = 0; c < KC / 32; ++c)
-                *(uint4*)(b_dst + (bhalf * (KC / 32) + c) * LBO_B) = b_valid ? src[c] : make_uint4(0, 0, 0, 0);
-        }
+        for (int c = 0; c < KC / 32; ++c) *(uint4*)(b_dst + (bhalf * (KC / 32) + c) * LBO_B) = x_next[c];
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the tensor core
         __syncthreads();
         if (tid == 0) {
@@ -124,6 +131,7 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
             }
             asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(&mbar)) : "memory");
         }
+        if (kc + 1 < kc1) request(kc + 1);
         // ---- wait until the MMAs of this stage have read shared memory ----
         {
             const uint32_t parity = (uint32_t)(kc - kc0) & 1u;
