@@ -335,7 +335,7 @@ def run_ours(args, s, blob):
     achieved = kb[dom] / (per_launch_us * 1e-6) / 1e9 if per_launch_us > 0 else 0.0
     roofline = {
         "bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-        "frac": achieved / peak, "traffic": TRAFFIC_NCU.get(dom), "peak_source": peak_src,
+        "frac": achieved / peak, "traffic": TRAFFIC_NCU.get((args.config, B, dom)), "peak_source": peak_src,
         "bytes_per_launch": kb[dom], "us_per_launch": per_launch_us,
         "whole_step": {"algorithmic_bytes_per_step": ab["total"], "bj_formula_bytes_per_step": ab["bj_formula"],
                        "achieved_GBps": step_gbs, "frac_of_measured": step_gbs / peak,
@@ -369,13 +369,16 @@ def run_ours(args, s, blob):
         dist.destroy_process_group()
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of each kernel class, from the committed
-# `ncu --set full` capture of this command (profiles/); None until captured
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
+# captures (profiles/r01_traffic.csv: config,batch,kernel,dram_bytes_per_launch); None for a workload that was not captured
 TRAFFIC_NCU = {}
 try:
-    _t = ROOT / "profiles" / "traffic.json"
+    _t = ROOT / "profiles" / "r01_traffic.csv"
     if _t.exists():
-        TRAFFIC_NCU = json.loads(_t.read_text())
+        for _line in _t.read_text().splitlines()[1:]:
+            _f = _line.split(",")
+            if len(_f) >= 4:
+                TRAFFIC_NCU[(int(_f[0]), int(_f[1]), _f[2].strip())] = int(_f[3])
 except Exception:
     TRAFFIC_NCU = {}
 
