@@ -258,10 +258,7 @@ int launch_proj_mma(dfssm_ctx* ctx, const uint32_t* sign, const int8_t* A, int r
     if (ks > nchunk) ks = nchunk;
     int32_t* acc = at<int32_t>(ctx, v.acc);
     int32_t* t = at<int32_t>(ctx, v.t);
-    if (ks > 1) {
-        CK(cudaMemsetAsync(acc, 0, (size_t)batch * v.ld_acc * 4, ctx->stream));
-        CK(cudaMemsetAsync(t, 0, (size_t)batch * T_STRIDE * 4, ctx->stream));
-    }
+    // ks > 1: acc / t were zeroed by the k_normquant launch in front of this projection
     mma::k_proj_mma<<<dim3(mt, nt, ks), mma::THREADS, 0, ctx->stream>>>(sign, A, rows, d.r, K, at<int8_t>(ctx, v.xq), (int)v.ldq, batch,
                                                                       acc, (int)v.ld_acc, t, at<int>(ctx, v.err));
     return DFSSM_OK;
@@ -309,7 +306,8 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
 
         tm->begin(DFSSM_KCLASS_NORMQUANT);
         k_normquant<<<batch, NQ_THREADS, 0, st>>>(u, d.d_model, L.norm_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum,
-                                                  tp, v.tap_stride, v.tl.off[DFSSM_TAP_XQ_IN], v.tl.off[DFSSM_TAP_S_IN]);
+                                                  tp, v.tap_stride, v.tl.off[DFSSM_TAP_XQ_IN], v.tl.off[DFSSM_TAP_S_IN],
+                                                  use_mma(c, batch, d.d_model) ? acc : nullptr, (int)ld_acc, t);
         tm->end(); ++nl;
 
         tm->begin(DFSSM_KCLASS_PROJ_IN);
@@ -342,7 +340,8 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
 
         tm->begin(DFSSM_KCLASS_NORMQUANT);
         k_normquant<<<batch, NQ_THREADS, 0, st>>>(g, d.d_inner, L.gnorm_w, d.d_inner, d.eps, xq, xqp, ldq, sx, qsum,
-                                                  tp, v.tap_stride, v.tl.off[DFSSM_TAP_GQ], v.tl.off[DFSSM_TAP_S_G]);
+                                                  tp, v.tap_stride, v.tl.off[DFSSM_TAP_GQ], v.tl.off[DFSSM_TAP_S_G],
+                                                  use_mma(c, batch, d.d_inner) ? acc : nullptr, (int)ld_acc, t);
         tm->end(); ++nl;
 
         tm->begin(DFSSM_KCLASS_PROJ_OUT);

@@ -66,8 +66,16 @@ __global__ void __launch_bounds__(NQ_THREADS)
 k_normquant(const float* __restrict__ v, int ldv, const float* __restrict__ w, int d, float eps,
             int8_t* __restrict__ xq, int8_t* __restrict__ xqp, int ldq, float* __restrict__ s_out,
             int32_t* __restrict__ qsum_out, uint8_t* __restrict__ taps, uint32_t tap_stride,
-            uint32_t tap_q_off, uint32_t tap_s_off)
+            uint32_t tap_q_off, uint32_t tap_s_off,
+            int32_t* __restrict__ zero_acc = nullptr, int ld_acc = 0, int32_t* __restrict__ zero_t = nullptr)
 {
+    // the split-K tensor-core projection that follows adds into acc / t: this sequence's rows are zeroed here (their last
+    // reader ran before this kernel) instead of by two memset nodes per projection
+    if (zero_acc) {
+        int32_t* za = zero_acc + (size_t)blockIdx.x * ld_acc;
+        for (int k = threadIdx.x; k < ld_acc; k += NQ_THREADS) za[k] = 0;
+        if (threadIdx.x < T_STRIDE) zero_t[(size_t)blockIdx.x * T_STRIDE + threadIdx.x] = 0;
+    }
     __shared__ double sh_d[NQ_THREADS / 32];
     __shared__ float sh_f[NQ_THREADS / 32];
     __shared__ int sh_i[NQ_THREADS / 32];
