@@ -25,7 +25,7 @@ inline size_t up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Carve {                 // byte offsets inside the arena
     size_t blob, ssm, conv, pos, u, xq, xqp, sx, qsum, acc, t, g, bcdt, logits, next, tok, err, taps, total;
-    size_t m_chunks, m_blocks, m_Ain, m_Aout, m_x, m_xbytes, m_am, m_prof;      // mega path regions (valid if mega_fit)
+    size_t m_chunks, m_schunks, m_blocks, m_x, m_xbytes, m_am, m_prof;      // mega path regions (valid if mega_fit)
     bool mega_fit;
     size_t ssm_elems, ldq, ld_acc;
     uint32_t tap_stride;
@@ -167,9 +167,8 @@ Carve carve(const dfssm_config& c)
     if (v.mega_fit) {
         const mega::Regions rg = mega::regions(mp);
         v.m_chunks = put(rg.chunks);
+        v.m_schunks = put(rg.schunks);
         v.m_blocks = put(rg.blocks);
-        v.m_Ain = put(rg.A_in);
-        v.m_Aout = put(rg.A_out);
         v.m_x = put(rg.xbuf);
         v.m_xbytes = rg.xbuf;
         v.m_am = put(rg.am);
@@ -453,17 +452,20 @@ int mega_load(dfssm_ctx* ctx, const std::vector<mega::HostLayer>& HL, const floa
     const Carve& v = ctx->cv;
     const Dims& d = ctx->dm;
     {
-        std::vector<uint8_t> buf((size_t)P.G * P.chunk_bytes);
+        std::vector<uint8_t> buf((size_t)P.NW * P.chunk_bytes), sbuf((size_t)P.NS * P.schunk_bytes);
+        std::vector<int8_t> tmp;
         for (int l = 0; l < d.n_layers; ++l) {
             const float* nn = l + 1 < d.n_layers ? HL[l + 1].norm_w : normf_w;
-            for (int c = 0; c < P.G; ++c) mega::pack_chunk(P, HL[l], nn, c, buf.data() + (size_t)c * P.chunk_bytes);
+            for (int c = 0; c < P.NW; ++c) mega::pack_chunk(P, HL[l], nn, c, buf.data() + (size_t)c * P.chunk_bytes);
+            for (int s = 0; s < P.NS; ++s) mega::pack_schunk(P, HL[l], s, sbuf.data() + (size_t)s * P.schunk_bytes, tmp);
             CK(cudaMemcpyAsync(ctx->arena + v.m_chunks + (size_t)l * buf.size(), buf.data(), buf.size(), cudaMemcpyHostToDevice, ctx->stream));
+            CK(cudaMemcpyAsync(ctx->arena + v.m_schunks + (size_t)l * sbuf.size(), sbuf.data(), sbuf.size(), cudaMemcpyHostToDevice, ctx->stream));
             CK(cudaStreamSynchronize(ctx->stream));
         }
     }
     if (d.n_layers > 0) {      // A_log -> A = -exp(A_log) inside the chunks, with the kernel's own exp
-        const size_t n = (size_t)d.n_layers * P.G * P.nch_max;
-        mega::k_mega_prepare<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(ctx->arena + v.m_chunks, (size_t)d.n_layers * P.G,
+        const size_t n = (size_t)d.n_layers * P.NW * P.nch_max;
+        mega::k_mega_prepare<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(ctx->arena + v.m_chunks, (size_t)d.n_layers * P.NW,
                                                                                    P.chunk_bytes, P.c_alog, P.nch_max);
         CK(cudaGetLastError());
     }
@@ -477,21 +479,10 @@ int mega_load(dfssm_ctx* ctx, const std::vector<mega::HostLayer>& HL, const floa
         // every exchange word starts as "not written" (mega::SENT)
         CK(cudaMemsetAsync(ctx->arena + v.m_x, 0xff, v.m_xbytes, ctx->stream));
     }
-    {
-        std::vector<int8_t> a((size_t)d.r * d.d_model), b((size_t)d.r * d.d_inner);
-        for (int l = 0; l < d.n_layers; ++l) {
-            mega::permute_A(HL[l].in_A, d.r, d.d_model, a.data());
-            mega::permute_A(HL[l].out_A, d.r, d.d_inner, b.data());
-            CK(cudaMemcpyAsync(ctx->arena + v.m_Ain + (size_t)l * a.size(), a.data(), a.size(), cudaMemcpyHostToDevice, ctx->stream));
-            CK(cudaMemcpyAsync(ctx->arena + v.m_Aout + (size_t)l * b.size(), b.data(), b.size(), cudaMemcpyHostToDevice, ctx->stream));
-            CK(cudaStreamSynchronize(ctx->stream));
-        }
-    }
     // pointers
     const size_t B = ctx->cfg.max_batch;
     P.chunks = ctx->arena + v.m_chunks;
-    P.A_in = (const int8_t*)(ctx->arena + v.m_Ain);
-    P.A_out = (const int8_t*)(ctx->arena + v.m_Aout);
+    P.schunks = ctx->arena + v.m_schunks;
     P.ssm = at<float>(ctx, v.ssm);
     P.conv = at<float>(ctx, v.conv);
     P.ssm_lstride = B * v.ssm_elems;
@@ -522,7 +513,7 @@ int mega_launch(dfssm_ctx* ctx)
 {
     mega::Params P = ctx->mp;
     ctx->epoch += 1;
-    P.rec0 = (uint32_t)(((ctx->epoch - 1) * (uint64_t)P.L) & 3u);      // global layer counter mod 4
+    P.set = (uint32_t)(ctx->epoch & 1u);       // this step's record set; the kernel resets the other one for the next step
     void* args[] = { &P };
     CK(cudaLaunchCooperativeKernel((const void*)ctx->mega_fn, dim3(P.G), dim3(mega::THREADS), args, P.smem_bytes, ctx->stream));
     return DFSSM_OK;

@@ -3,36 +3,45 @@
 // here the step is a single launch and the per-layer dependencies are resolved inside the kernel.)
 //
 // Design:
-//   * Ownership.  CTA c owns d_inner channels [chs[c], chs[c+1]) -- their z and x in_proj rows, their conv
-//     and SSM state, their gate -- and out_proj rows [ors[c], ors[c+1]) together with that slice of the
-//     residual stream u (kept in shared memory for the whole step).  The B|C|dt in_proj rows and the
-//     LoRA down-projection rows (t = A.xq) are "early tasks" dealt round-robin: task e belongs to CTA e % G.
-//   * Weights.  dfssm_load_weights repacks every layer into one contiguous chunk per (layer, CTA)
-//     (sign rows, LoRA-up rows, scales, conv taps, per-channel constants) plus one block per layer that
-//     every CTA reads (the LoRA-up rows / scales / conv taps of the B|C|dt rows).  Chunk + block + the CTA's
-//     slice of the SSM / conv state form one pipeline item, fetched by bulk async copies
-//     (cp.async.bulk -> mbarrier) into a ring of shared-memory stages several layers AHEAD of the
-//     dependency chain: addresses never depend on activations, so HBM stays busy while CTAs wait on
-//     each other.  The LM head streams the int8 embedding through the same ring.
-//   * Exchange.  Measured on B200: one store -> poll hop between CTAs through L2 costs >= ~0.9 us, so the
-//     layer is built around FOUR all-gathers, two of them hidden behind sign-row work:
-//       U : t_k = u_k * w_k (fp32) of the owned out rows + the CTA's partial sum of u^2 (fp64)
-//           -> every CTA derives rstd / amax / the int8 codes of the WHOLE vector itself (S1)
-//       A : raw int32 accumulators of the B|C|dt rows + t_in        (hidden behind the z|x sign rows)
-//           -> every CTA finishes the B|C|dt epilogue, conv and softplus redundantly (S3, S4)
-//       G : t_k = g_k * w_k (fp32) of the owned channels + partial sum of g^2  -> S6 everywhere
-//       T : partial LoRA-down sums of out_proj                     (hidden behind the out_proj sign rows)
-//     Buffers are self-validating ("Lamport" style): every 32-bit word is either the sentinel 0xffffffff
-//     or payload (fp32 values are never that NaN; int32 values are stored with the sign bit flipped;
-//     fp64 partials are 8-byte stores validated by their high word), so a hop is one store and one
-//     successful poll, with no flag, fence or barrier.  A part can be PUSHED into M mailboxes (GRID / M CTAs poll each
-//     copy).  Measured on the B200: U, G and A are fastest pulled from ONE copy; T, which every CTA
-//     starts polling before it is written, is 2x faster pushed into 37 copies (polls delay stores to the same
-//     lines).  The U / G payload of a CTA is one 128-byte slot written with 16-byte stores (a slot that straddles
-//     a line costs ~1000 clocks per hop).  Records rotate over 4 (global layer counter mod 4): at layer l a CTA
-//     resets its own slots of the record that layer l+2 will use (last used by layer l-2, which every CTA has
-//     finished reading: it has since published for layer l-1), so the buffers stay L2-resident and a reset is at
-//     least two hops old when the word is written or polled again.
+//   * Roles.  The 148 CTAs are NW "workers" (CTAs 0 .. NW-1) and NS = 148 - NW "service" CTAs.
+//     Worker c owns d_inner channels [chs[c], chs[c+1]) -- their z and x in_proj rows, their conv and SSM
+//     state, their gate -- and out_proj rows [ors[c], ors[c+1]) with that slice of the residual stream u (kept
+//     in shared memory for the whole step).  The service CTAs own the rows whose result EVERY worker needs and
+//     that need the whole activation vector: the B|C|dt in_proj rows and the LoRA down-projections t = A.xq of
+//     both projections.  They own no state and stream almost no weights, so they are always waiting when an
+//     activation vector completes and publish their few int32 words while the workers are still busy with
+//     their own sign rows: the two small exchanges (A, T) overlap with the workers' integer work instead of
+//     following it (round 1 dealt these rows round-robin over all CTAs: every worker then waited for the
+//     slowest of 148 publishers, 2.5 k + 1.7 k clocks per layer).
+//   * Weights.  dfssm_load_weights repacks every layer into one contiguous chunk per (layer, worker)
+//     (sign rows, LoRA-up rows, scales, conv taps, per-channel constants), one chunk per (layer, service CTA)
+//     (its sign rows and LoRA-down rows) plus one block per layer that every worker reads (the LoRA-up rows /
+//     scales / conv taps of the B|C|dt rows).  Chunk + block + the CTA's slice of the SSM / conv state form one
+//     pipeline item, fetched by bulk async copies (cp.async.bulk -> mbarrier) into a ring of shared-memory
+//     stages several layers AHEAD of the dependency chain: addresses never depend on activations, so HBM stays
+//     busy while CTAs wait on each other.  The LM head streams the int8 embedding through the same ring.
+//   * Exchange.  Four self-validating all-gathers per layer through L2:
+//       U : t_k = u_k * w_k (fp32) of the owned out rows (+ the worker's partial sum of u^2, fp64, in its own array)
+//           -> every CTA derives amax and the int8 codes of the WHOLE vector itself (S1)
+//       A : raw int32 accumulators of the B|C|dt rows + t_in   (service -> workers)
+//           -> every worker finishes the B|C|dt epilogue, conv and softplus itself (S3, S4)
+//       G : t_k = g_k * w_k (fp32) of the owned channels (+ partial sum of g^2)  -> S6 everywhere
+//       T : partial LoRA-down sums of out_proj                 (service -> workers)
+//     Every 32-bit word is either the sentinel 0xffffffff or payload (fp32 values are never that NaN; int32
+//     values are stored with the sign bit flipped; fp64 partials are 8-byte stores validated by their high
+//     word), so a hop is one store and one successful poll: no flag, no fence.
+//   * Memory ordering (PTX model).  There are 2 x L records: step n publishes layer l into record (n & 1, l) and
+//     resets its own words of record (~n & 1, l) to the sentinel.  Inside one launch a word is therefore written
+//     ONCE and never reset, and a word that is reset is never polled: every reset is ordered against the polls
+//     that need it, and against the reads that precede it, by a KERNEL BOUNDARY (the record was last read by
+//     the previous launch and is next polled by the following one).  All exchange accesses are relaxed gpu-scope
+//     64-bit accesses (single-copy atomic, "morally strong": no data race); a poll accepts only a non-sentinel
+//     value, which can only be this launch's payload.  No ordering rests on elapsed time, and no fence is needed
+//     (round 1 rotated 4 records inside a launch and relied on a reset being "at least two hops old";
+//     fence.acq_rel.gpu around every publish and gather was measured at ~1000 clocks per fence, +55 % step time).
+//   * Critical path.  Only amax -> 127/amax -> codes is on it; the fp64 sum of squares, rstd and the activation
+//     scale are made by one warp from the partial array while the sign rows run (they are first needed in the
+//     projection epilogue).
 //   * Arithmetic: identical to the chain path (dfssm_math.cuh; contract of DESIGN.md section 5).
 #pragma once
 #include <cuda_runtime.h>
@@ -46,13 +55,16 @@
 namespace dfssm {
 namespace mega {
 
-constexpr int THREADS = 512;                  // 16 warps (measured: 32 warps only add issue pressure to the short phases)
+#ifndef DFSSM_THREADS
+#define DFSSM_THREADS 512
+#endif
+constexpr int THREADS = DFSSM_THREADS;        // 16 or 32 warps
 constexpr int NWARPS = THREADS / 32;
 constexpr int NJ_MAX = 3072 / THREADS;        // 16-byte chunks per thread when gathering U / G with run-time shapes (plan() checks)
 constexpr int NJ_A = 1024 / THREADS;          // ... when gathering A
 constexpr int NR_IN = THREADS >= 1024 ? 2 : 4;     // in_proj sign rows per warp pass
-constexpr int LPR = THREADS / 512;            // lanes per row in the in_proj epilogue
-constexpr int LPC = 16;                       // lanes per channel in the state update
+constexpr int LPC = THREADS / 32;             // lanes per channel in the state update (32 channels per pass)
+constexpr int LPB = THREADS / 512;            // lanes per B|C row in the in_proj epilogue
 constexpr int DMA_TID = 96;                   // the thread that issues the state write-back and the ring refills (a warp off the publish paths)
 constexpr int KS_MAX = 4;                     // largest K-split of the out_proj sign rows
 constexpr int MAX_STAGES = 8;
@@ -61,45 +73,69 @@ constexpr uint32_t SENT = 0xffffffffu;        // "not written yet"
 constexpr uint32_t IBIAS = 0x80000000u;       // int32 payloads are stored xor IBIAS (|value| < 2^30)
 constexpr int PROF_NPH = 32;                  // phase stamps per (CTA, layer) of the in-kernel profiler
 
+constexpr int GRID = 148;                     // one CTA per B200 SM
+constexpr int NW_CT = 128;                    // workers of the compile-time-shape kernels (the rest are service CTAs)
+constexpr int MBOX = 37;                      // mailboxes allocated per record
+
+// mailboxes of the small parts A and T (each must divide GRID and be <= MBOX): the payload is pushed M times and GRID / M
+// workers poll each copy (polls that reach a line before the data delay the stores to it).  U and G have one copy.
+#ifndef DFSSM_MA
+#define DFSSM_MA 37
+#endif
+#ifndef DFSSM_MT
+#define DFSSM_MT 37
+#endif
+// clocks a worker waits after publishing G / U before its first poll: polls that reach a line before the data delay the
+// stores to it
+#ifndef DFSSM_WG
+#define DFSSM_WG 500
+#endif
+#ifndef DFSSM_WU
+#define DFSSM_WU 500
+#endif
+constexpr int M_A = DFSSM_MA, M_T = DFSSM_MT;
+
 struct Params {
     // ---- shape ----
     int L, d_model, d_inner, headdim, d_state, ngroups, nheads, r, vocab, n_bcdt, gs;
     float eps;
-    int G;                       // grid size (CTAs), all co-resident
-    int nch_max, nor_max, nb_max, n_slots, r_pad;
+    int G, NW, NS;               // grid size (all co-resident), workers, service CTAs
+    int nch_max, nor_max, r_pad;
     int Win, Wout;               // sign words per row of in_proj / out_proj
-    int n_early;                 // early tasks: n_bcdt sign rows + r LoRA-down rows
+    int n_early;                 // service results of in_proj: n_bcdt sign rows + r LoRA-down rows
     int tsplit, n_ttask;         // out_proj LoRA-down rows are split into tsplit partial tasks each
-    // ---- chunk layout (byte offsets inside one (layer, CTA) chunk) ----
+    int ns_sig, ns_lin, ns_tt;   // most sign rows / in_proj LoRA-down rows / out_proj partial tasks one service CTA holds
+    // ---- worker chunk layout (byte offsets inside one (layer, worker) chunk) ----
     uint32_t c_in_bits, c_out_bits, c_in_B, c_out_B, c_in_scale, c_in_bs, c_out_scale, c_out_bs, c_conv_w, c_conv_b,
         c_alog, c_D, c_gnorm, c_nnorm, chunk_bytes;
-    // ---- per-layer block read by every CTA (byte offsets) ----
+    // ---- service chunk layout (byte offsets inside one (layer, service CTA) chunk) ----
+    uint32_t sc_sign, sc_tin, sc_tout, schunk_bytes;
+    // ---- per-layer block read by every worker (byte offsets) ----
     uint32_t b_eB, b_escale, b_ebs, b_econv_w, b_econv_b, b_dtb, b_as_in, b_as_out, blk_bytes;
     // ---- pipeline stage ----
-    uint32_t st_blk, st_ssm, st_conv, st_econv, st_tin, st_tout, stage_bytes;
+    uint32_t st_blk, st_ssm, st_conv, st_econv, stage_bytes;
     int stages, lm_rows_item;
-    // ---- exchange: M mailboxes x 4 rotating records; 32-bit word offsets inside one (record, mailbox) ----
-    int M, gsz;                  // mailboxes, CTAs polling each (G = M * gsz); CTA c polls mailbox c / gsz
-    int u_slot, u_dpos, g_slot, g_dpos;      // words per CTA slot of U / G, position of the fp64 partial inside it
-    uint32_t x_U, x_A, x_G, x_T, x_words;
+    // ---- exchange: 2 sets x L records; a record = main part (U, PU, G, PG: one copy) + MBOX small mailboxes (A, T);
+    //      32-bit word offsets inside the main part / inside one small mailbox ----
+    int u_slot, g_slot;          // words per worker slot of U / G (a power of two >= the owned elements)
+    uint32_t x_U, x_PU, x_G, x_PG, x_main, x_A, x_T, x_small;
     // ---- shared memory carve ----
-    uint32_t s_ring, s_mbar, s_xq, s_bc, s_u, s_z, s_x, s_dt, s_tq, s_v, s_eacc, s_acc_in, s_acc_out, s_chs, s_ors,
-        s_part, s_red, s_slot, smem_bytes;
+    uint32_t s_ring, s_mbar, s_xq, s_bc, s_cd, s_u, s_z, s_x, s_dt, s_v, s_eacc, s_acc_in, s_acc_out, s_chs, s_ors,
+        s_red, s_slot, s_scal, smem_bytes;
     // ---- device pointers ----
-    const uint8_t* chunks;       // [L][G][chunk_bytes]
+    const uint8_t* chunks;       // [L][NW][chunk_bytes]
+    const uint8_t* schunks;      // [L][NS][schunk_bytes]
     const uint8_t* blocks;       // [L][blk_bytes]
-    const int8_t* A_in;          // [L][r][d_model]  plane-permuted
-    const int8_t* A_out;         // [L][r][d_inner]  plane-permuted
     float* ssm;                  // sequence 0 of layer 0; layer stride ssm_lstride floats
     float* conv;                 // [conv_dim][4] ring of sequence 0 of layer 0; layer stride conv_lstride floats
     size_t ssm_lstride, conv_lstride;
     const int8_t* emb; const float* emb_s; const float* first_norm_w;
     const int32_t* tokens; int32_t* next; int32_t* tok_out; int32_t* pos;
     float* logits; float* u_out;
-    uint32_t* xbuf;              // [4 records][M][x_words]
+    uint32_t* xbuf;              // [2 sets][L][x_main + MBOX * x_small]
     float* am_val; int* am_idx; unsigned* am_count;
     int* err;
-    uint32_t rec0;               // record of layer 0 of this step (global layer counter mod 4)
+    uint32_t set;                // record set this step publishes into (step counter & 1); it resets the other one
     uint8_t* taps; size_t tap_lstride; TapLayout tl;
     unsigned long long* prof;    // [G][L+1][PROF_NPH] SM-clock stamps of thread 0 (DFSSM_FLAG_PROF), else null
 };
@@ -159,10 +195,15 @@ __device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
-// exchange words: relaxed gpu-scope accesses (served by L2; a 32-bit / 64-bit scalar access is single-copy atomic)
+// exchange words: relaxed gpu-scope accesses (served by L2; a 32-bit / 64-bit scalar access is single-copy atomic).
 __device__ __forceinline__ void x_st32(uint32_t* p, uint32_t v)
 {
     asm volatile("st.relaxed.gpu.global.b32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void x_st64(uint32_t* p, uint32_t lo, uint32_t hi)
+{
+    const uint64_t a = ((uint64_t)hi << 32) | lo;
+    asm volatile("st.relaxed.gpu.global.b64 [%0], %1;" ::"l"(p), "l"(a) : "memory");
 }
 // 16 bytes as TWO 64-bit elements, each single-copy atomic (a float pair, or one fp64)
 __device__ __forceinline__ uint4 x_ld128(const uint32_t* p)
@@ -176,7 +217,6 @@ __device__ __forceinline__ void x_st128(uint32_t* p, uint4 v)
     const uint64_t a = ((uint64_t)v.y << 32) | v.x, b = ((uint64_t)v.w << 32) | v.z;
     asm volatile("st.relaxed.gpu.global.v2.b64 [%0], {%1,%2};" ::"l"(p), "l"(a), "l"(b) : "memory");
 }
-
 // Code layout for the masked-dp4a sign dot: a 32-block of codes is eight 4-byte words ("planes"), plane i = elements
 // 4i .. 4i+3 of the block; the load-time repack moves the sign bit of element 4i + j to bit 8j + i of the sign word,
 // so dp4a(bits & (0x01010101 << i), plane i) sums plane i.  Planes 0..3 of all blocks form the first half of
@@ -188,37 +228,21 @@ __device__ __forceinline__ int plane_pos(int k, int K)
 
 // Shape of the model as the kernel sees it: compile-time constants for the shapes of BASELINE.json's configs (every
 // index computation, division and loop bound folds), or the run-time values of Params (any other shape).
-struct ShapeRT { static constexpr bool kStatic = false; static constexpr int d_model = 0, d_inner = 0, headdim = 0, d_state = 0, ngroups = 0, r = 0; };
+struct ShapeRT { static constexpr bool kStatic = false; static constexpr int d_model = 0, d_inner = 0, headdim = 0, d_state = 0, ngroups = 0, r = 0, NW = 0; };
 template <int DM, int DI, int HD, int DS, int NG, int R>
-struct ShapeCT { static constexpr bool kStatic = true; static constexpr int d_model = DM, d_inner = DI, headdim = HD, d_state = DS, ngroups = NG, r = R; };
+struct ShapeCT { static constexpr bool kStatic = true; static constexpr int d_model = DM, d_inner = DI, headdim = HD, d_state = DS, ngroups = NG, r = R, NW = NW_CT; };
 
-constexpr int GRID = 148;                       // one CTA per B200 SM
-constexpr int MBOX = 37;                        // mailboxes allocated per record
-// mailboxes actually used by each part (each must divide GRID and be <= MBOX): with M the payload is pushed M times and
-// GRID / M CTAs poll each copy.  Tuned on the B200 (us per step, cfg 2): see DESIGN.md 6.2
-#ifndef DFSSM_MU
-#define DFSSM_MU 1
-#define DFSSM_MG 1
-#define DFSSM_MA 1
-#define DFSSM_MT 37
-#endif
-// clocks a CTA waits after publishing G / U before its first poll: polls that reach a line before the data delay the
-// stores to it (measured: 0 -> 0.501 ms/step, 300..700 -> 0.488)
-#ifndef DFSSM_WG
-#define DFSSM_WG 500
-#define DFSSM_WU 500
-#endif
-constexpr int M_U = DFSSM_MU, M_G = DFSSM_MG, M_A = DFSSM_MA, M_T = DFSSM_MT;
-
-// Ownership: CTA g owns elements [own_start(g, n), own_start(g + 1, n)) of a vector of length n (n % 4 == 0), in
-// groups of 4 so that a gathered 16-byte chunk is four consecutive elements of one 16-element half block of codes.
-__host__ __device__ constexpr int own_start(int g, int n) { return 4 * (int)(((long long)g * (n / 4)) / GRID); }
-__host__ __device__ constexpr int own_max(int n) { return 4 * ((n / 4 + GRID - 1) / GRID); }
-// words of one CTA's slot in a U / G mailbox: a power of two (16, 32, 64 ...), so that a slot never straddles a 128-byte
+// Ownership: worker g owns elements [own_start(g, n, NW), own_start(g + 1, n, NW)) of a vector of length n (n % 4 == 0),
+// in groups of 4 so that a gathered 16-byte chunk is four consecutive elements of one 16-element half block of codes.
+__host__ __device__ constexpr int own_start(int g, int n, int NW) { return 4 * (int)(((long long)g * (n / 4)) / NW); }
+__host__ __device__ constexpr int own_max(int n, int NW) { return 4 * ((n / 4 + NW - 1) / NW); }
+// words of one worker's slot in a U / G mailbox: a power of two (4, 8, 16 ...), so that a slot never straddles a 128-byte
 // line (measured: 80-byte slots cost ~1000 clocks per hop more than 64- or 128-byte ones)
 __host__ __device__ constexpr int slot_words(int need) { int w = 4; while (w < need) w *= 2; return w; }
-// 16-byte chunks per thread needed to gather the slots of a vector of length n (or to hold n / 4 chunks: n_flat)
-__host__ __device__ constexpr int nj_slots(int n) { return (GRID * slot_words((own_max(n) + 1) / 2 * 2 + 2) / 4 + THREADS - 1) / THREADS; }
+// 16-byte chunks per thread needed to gather the NW slots of a vector of length n
+__host__ __device__ constexpr int nj_slots(int n, int NW) { return (NW * slot_words(own_max(n, NW)) / 4 + THREADS - 1) / THREADS; }
+// service CTA s holds the items s, s + NS, s + 2 NS ... of a list of n
+__host__ __device__ constexpr int dealt(int n, int s, int NS) { return s < n ? (n - s + NS - 1) / NS : 0; }
 
 template <class S>
 struct Ctx {
@@ -227,43 +251,37 @@ struct Ctx {
     int tid, lane, wid, c;
     volatile int* dead;          // shared flag: a poll timed out -> stop spinning everywhere
     bool prof;                   // in-kernel profiler on (a compile-time false in the production instantiations)
-    static constexpr int NJG = S::kStatic ? nj_slots(S::d_inner) : NJ_MAX;     // chunks per thread: gather G, gather U, embedding
-    static constexpr int NJU = S::kStatic ? nj_slots(S::d_model) : NJ_MAX;
-    static constexpr int NJ0 = S::kStatic ? (S::d_model / 4 + THREADS - 1) / THREADS : 8192 / 4 / THREADS;
+    static constexpr int NJG = S::kStatic ? nj_slots(S::d_inner, S::NW) : NJ_MAX;     // chunks per thread: gather G, gather U
+    static constexpr int NJU = S::kStatic ? nj_slots(S::d_model, S::NW) : NJ_MAX;
+    static constexpr int NJ0 = S::kStatic ? (S::d_model / 4 + THREADS - 1) / THREADS : 8192 / 4 / THREADS;   // embedding
 #define DFSSM_DIM(n_) __device__ __forceinline__ int n_() const { return S::kStatic ? S::n_ : P.n_; }
-    DFSSM_DIM(d_model) DFSSM_DIM(d_inner) DFSSM_DIM(headdim) DFSSM_DIM(d_state) DFSSM_DIM(ngroups) DFSSM_DIM(r)
+    DFSSM_DIM(d_model) DFSSM_DIM(d_inner) DFSSM_DIM(headdim) DFSSM_DIM(d_state) DFSSM_DIM(ngroups) DFSSM_DIM(r) DFSSM_DIM(NW)
 #undef DFSSM_DIM
     __device__ __forceinline__ void stamp(int l, int k) const
     {
-        if (prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + k] = clock64();
+        if (prof && tid == 0) {     // the clock is read behind a shared-memory load: a stamp after a barrier is the RELEASE time
+            const int v = *dead;
+            unsigned long long t;
+            asm volatile("mov.u64 %0, %%clock64;" : "=l"(t) : "r"(v) : "memory");
+            P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + k] = t;
+        }
     }
     __device__ __forceinline__ constexpr int G() const { return GRID; }
-    __device__ __forceinline__ constexpr int M() const { return MBOX; }
-    __device__ __forceinline__ constexpr int gsz() const { return GRID / MBOX; }
+    __device__ __forceinline__ int NS() const { return GRID - NW(); }
+    __device__ __forceinline__ bool service() const { return c >= NW(); }
     __device__ __forceinline__ int nheads() const { return d_inner() / headdim(); }
     __device__ __forceinline__ int gs() const { return ngroups() * d_state(); }
     __device__ __forceinline__ int n_bcdt() const { return 2 * gs() + nheads(); }
-    __device__ __forceinline__ int nch_max() const { return own_max(d_inner()); }
-    __device__ __forceinline__ int nor_max() const { return own_max(d_model()); }
-    __device__ __forceinline__ int nb_max() const { return (n_bcdt() + GRID - 1) / GRID; }
-    __device__ __forceinline__ int n_slots() const { return 2 * nch_max() + nb_max(); }
+    __device__ __forceinline__ int nch_max() const { return own_max(d_inner(), NW()); }
+    __device__ __forceinline__ int nor_max() const { return own_max(d_model(), NW()); }
     __device__ __forceinline__ int r_pad() const { return (r() + 3) / 4 * 4; }
     __device__ __forceinline__ int Win() const { return d_model() / 32; }
     __device__ __forceinline__ int Wout() const { return d_inner() / 32; }
     __device__ __forceinline__ int n_early() const { return n_bcdt() + r(); }
-    __device__ __forceinline__ int tsplit() const { return (d_inner() % 64 == 0 && 4 * r() <= GRID) ? 4 : (2 * r() <= GRID ? 2 : 1); }
+    __device__ __forceinline__ int tsplit() const { return d_inner() % 64 == 0 ? 4 : 2; }
     __device__ __forceinline__ int n_ttask() const { return r() * tsplit(); }
-    // early task e = c + k G of this CTA that is a LoRA-down row (at most one: r <= G), or -1
-    __device__ __forceinline__ int t_in_task() const
-    {
-        const int k = c >= n_bcdt() ? 0 : (n_bcdt() - c + GRID - 1) / GRID;
-        const int e = c + k * GRID;
-        return e < n_early() ? e : -1;
-    }
-    __device__ __forceinline__ int u_dpos() const { return (nor_max() + 1) / 2 * 2; }
-    __device__ __forceinline__ int u_slot() const { return slot_words(u_dpos() + 2); }
-    __device__ __forceinline__ int g_dpos() const { return (nch_max() + 1) / 2 * 2; }
-    __device__ __forceinline__ int g_slot() const { return slot_words(g_dpos() + 2); }
+    __device__ __forceinline__ int u_slot() const { return slot_words(nor_max()); }
+    __device__ __forceinline__ int g_slot() const { return slot_words(nch_max()); }
 };
 
 __device__ __forceinline__ unsigned long long globaltimer_ns()
@@ -279,28 +297,33 @@ template <class S>
 __device__ __forceinline__ void poll_fail(const Ctx<S>& x)
 {
     *x.dead = 1;
-    atomicExch(x.P.err, 2);
+    atomicOr(x.P.err, 2);
 }
+
+// mailbox (of a part pushed M times) that CTA c polls, and the number of mailboxes the CTAs [0, n) poll
+__device__ __forceinline__ constexpr int mbox_of(int c, int M) { return c / (GRID / M); }
+__device__ __forceinline__ constexpr int mbox_count(int n, int M) { return (n + GRID / M - 1) / (GRID / M); }
 
 // ------------------------------------------------------------------------------------------------
 // exchange: gather a self-validating buffer
 // ------------------------------------------------------------------------------------------------
 // Thread t owns the 16-byte chunks t, t + THREADS, ... (at most NJ) of the nw 32-bit words at buf.  Words
-// behind nw count as valid.  If slot_w > 0 the buffer is a sequence of slots of slot_w words whose word dpos is
-// the low half of an fp64 (any bit pattern: exempt; its high half at dpos + 1 validates it).
-// Spins until every owned word has been written; the raw words come back in v[].  tix = the thread's index for
-// the chunk ownership (tid, or reversed so that the small gathers are polled by the warps that have nothing else to do).
+// behind nw count as valid.  Spins until every owned word has been written; the raw words come back in v[].
+// tix = the thread's index for the chunk ownership (tid, or reversed so that the small gathers are polled by the
+// warps that have nothing else to do).
 template <int NJ, class S>
-__device__ __forceinline__ void hop_gather(const Ctx<S>& x, const uint32_t* buf, int nw, int slot_w, int dpos, uint4 (&v)[NJ], int tix, int first_wait = 0)
+__device__ __forceinline__ void hop_gather(const Ctx<S>& x, const uint32_t* buf, int nw, uint4 (&v)[NJ], int tix, int first_wait = 0)
 {
+    const int nchunk = (nw + 3) >> 2;
+    bool need[NJ];
+    bool any = false;
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) { need[j] = tix + j * THREADS < nchunk; any = any || need[j]; }
+    if (!any) return;
     if (first_wait > 0) {                          // polls that arrive before the data delay the stores to the same lines
         const long long t0 = clock64();
         while (clock64() - t0 < first_wait) {}
     }
-    const int nchunk = (nw + 3) >> 2;
-    bool need[NJ];
-#pragma unroll
-    for (int j = 0; j < NJ; ++j) need[j] = tix + j * THREADS < nchunk;
     uint32_t spins = 0;
     for (;;) {
 #pragma unroll
@@ -311,9 +334,8 @@ __device__ __forceinline__ void hop_gather(const Ctx<S>& x, const uint32_t* buf,
         for (int j = 0; j < NJ; ++j)
             if (need[j]) {
                 const int base = 4 * (tix + j * THREADS);
-                const int ex = slot_w > 0 ? dpos - base % slot_w : -1;      // index of the exempt word inside this chunk
-                const bool ok = (v[j].x != SENT || ex == 0) && (base + 1 >= nw || v[j].y != SENT) &&
-                                (base + 2 >= nw || v[j].z != SENT || ex == 2) && (base + 3 >= nw || v[j].w != SENT);
+                const bool ok = v[j].x != SENT && (base + 1 >= nw || v[j].y != SENT) && (base + 2 >= nw || v[j].z != SENT) &&
+                                (base + 3 >= nw || v[j].w != SENT);
                 need[j] = !ok;
                 all = all && ok;
             }
@@ -329,53 +351,44 @@ template <class S>
 __device__ __forceinline__ int* red_i(const Ctx<S>& x) { return (int*)(x.sm + x.P.s_red) + NWARPS; }
 template <class S>
 __device__ __forceinline__ double* red_d(const Ctx<S>& x) { return (double*)(x.sm + x.P.s_red + 8 * NWARPS); }
+// scalars: [0] amax of the last norm_quant, [1] scale of the in_proj / LM-head codes, [2] scale of the out_proj codes
+template <class S>
+__device__ __forceinline__ float* scal(const Ctx<S>& x) { return (float*)(x.sm + x.P.s_scal); }
 
-// S1 / S6 / S8 norm + quantise of a whole vector in every CTA.  `en(f)` calls f(k, bits) for every element this
-// thread holds: bits = fp32 t_k = value_k * w_k;  ss_local = the partial sums of squares this thread holds (the
-// per-CTA partials it gathered, or its own elements' squares for the embedding).  Every warp reduces the 16 warp
-// results and derives rstd / amax / scale itself; every thread then quantises its elements.  Writes the codes to
-// xq (plane order unless `canonical`), returns the sum of the codes and the activation scale s.
+// S1 / S6 / S8 absmax + quantise of a whole vector in every CTA (the critical path of the norm: only amax is needed for
+// the codes, R13).  `en(f)` calls f(k, bits) for every group of four elements this thread holds: bits = fp32 t_k = value_k * w_k.
+// Writes the codes to xq (plane order unless `canonical`), leaves amax in scal[0] and returns the sum of the codes.
 // Two __syncthreads.
 template <class S, typename Enum>
-__device__ __forceinline__ int norm_quant(const Ctx<S>& x, Enum en, double ss_local, int dstride, int dlane, int K, bool canonical, float& s_out,
-                                          int8_t* tap_codes, int pl = 0, int pk = -1)
+__device__ __forceinline__ int absmax_quant(const Ctx<S>& x, Enum en, int K, bool canonical, int8_t* tap_codes, int pl = 0, int pk = -1)
 {
     const Params& P = x.P;
     uint8_t* xq = x.sm + P.s_xq;
-    float* bc = (float*)(x.sm + P.s_part);
     float am = 0.0f;
     en([&](int, uint4 w) {
         am = fmaxf(fmaxf(am, fabsf(__uint_as_float(w.x))), fabsf(__uint_as_float(w.y)));
         am = fmaxf(fmaxf(am, fabsf(__uint_as_float(w.z))), fabsf(__uint_as_float(w.w)));
     });
     am = warp_max(am);
-    ss_local = warp_sum_strided(ss_local, dstride);      // only the lanes dlane + k * dstride hold partial sums
     if (x.lane == 0) red_f(x)[x.wid] = am;
-    if (x.lane == dlane) red_d(x)[x.wid] = ss_local;
     if (pk >= 0) x.stamp(pl, pk);
     __syncthreads();
     if (pk >= 0) x.stamp(pl, pk + 1);
-    // every warp derives the constants itself from the NWARPS warp results (cheaper than a second barrier)
-    static_assert(NWARPS == 16, "the reductions below read 16 warp results");
+    static_assert(NWARPS % 8 == 0, "the reductions below read the warp results eight at a time");
     float amax;
-    double ss;
     {
         const float4* rf = (const float4*)red_f(x);
-        const float4 a0 = rf[0], a1 = rf[1], a2 = rf[2], a3 = rf[3];
-        amax = fmaxf(fmaxf(fmaxf(fmaxf(a0.x, a0.y), fmaxf(a0.z, a0.w)), fmaxf(fmaxf(a1.x, a1.y), fmaxf(a1.z, a1.w))),
-                     fmaxf(fmaxf(fmaxf(a2.x, a2.y), fmaxf(a2.z, a2.w)), fmaxf(fmaxf(a3.x, a3.y), fmaxf(a3.z, a3.w))));
-        const double2* rd = (const double2*)red_d(x);
-        double2 d[8];
+        float m[NWARPS / 8];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) d[i] = rd[i];
-        ss = (((d[0].x + d[0].y) + (d[1].x + d[1].y)) + ((d[2].x + d[2].y) + (d[3].x + d[3].y))) +
-             (((d[4].x + d[4].y) + (d[5].x + d[5].y)) + ((d[6].x + d[6].y) + (d[7].x + d[7].y)));
+        for (int i = 0; i < NWARPS / 8; ++i) {
+            const float4 a0 = rf[2 * i], a1 = rf[2 * i + 1];
+            m[i] = fmaxf(fmaxf(fmaxf(a0.x, a0.y), fmaxf(a0.z, a0.w)), fmaxf(fmaxf(a1.x, a1.y), fmaxf(a1.z, a1.w)));
+        }
+        amax = m[0];
+#pragma unroll
+        for (int i = 1; i < NWARPS / 8; ++i) amax = fmaxf(amax, m[i]);
     }
-    const float ms = (float)(ss / (double)K);
-    const float rstd = fdiv(1.0f, __fsqrt_rn(fadd(ms, P.eps)));
     const float inv = amax == 0.0f ? 0.0f : fdiv(127.0f, amax);
-    s_out = amax == 0.0f ? 0.0f : fdiv(fmul(amax, rstd), 127.0f);
-    if (pk >= 0) x.stamp(pl, pk + 2);
     int qs = 0;
     en([&](int k0, uint4 w) {                                       // four consecutive elements, k0 % 4 == 0
         const uint32_t q0 = (uint32_t)quant_code(__uint_as_float(w.x), inv) & 255u, q1 = (uint32_t)quant_code(__uint_as_float(w.y), inv) & 255u,
@@ -387,15 +400,56 @@ __device__ __forceinline__ int norm_quant(const Ctx<S>& x, Enum en, double ss_lo
     });
     qs = warp_sum_i(qs);
     if (x.lane == 0) red_i(x)[x.wid] = qs;
-    if (pk >= 0) x.stamp(pl, pk + 3);
+    if (x.tid == 0) scal(x)[0] = amax;
+    if (pk >= 0) x.stamp(pl, pk + 2);
     __syncthreads();
     const int4* ri = (const int4*)red_i(x);
-    const int4 q0 = ri[0], q1 = ri[1], q2 = ri[2], q3 = ri[3];
-    return ((q0.x + q0.y) + (q0.z + q0.w)) + ((q1.x + q1.y) + (q1.z + q1.w)) + ((q2.x + q2.y) + (q2.z + q2.w)) + ((q3.x + q3.y) + (q3.z + q3.w));
+    int tot = 0;
+#pragma unroll
+    for (int i = 0; i < NWARPS / 4; ++i) {
+        const int4 q = ri[i];
+        tot += (q.x + q.y) + (q.z + q.w);
+    }
+    return tot;
+}
+
+// rstd and the activation scale s = (amax * rstd) / 127 (R13) from a sum of squares; ONE thread's arithmetic
+__device__ __forceinline__ float act_scale(double ss, int K, float eps, float amax)
+{
+    const float ms = (float)(ss / (double)K);
+    const float rstd = fdiv(1.0f, __fsqrt_rn(fadd(ms, eps)));
+    return amax == 0.0f ? 0.0f : fdiv(fmul(amax, rstd), 127.0f);
+}
+
+// Off the critical path, ONE warp: gather the NW fp64 partial sums of squares of a record part (8-byte elements
+// validated by their high word), add them (any tree: DESIGN.md 5.3) and leave the activation scale in scal[which].
+// amax comes from scal[0] (absmax_quant of the same vector; a CTA barrier lies between).
+template <class S>
+__device__ __forceinline__ void scale_side(const Ctx<S>& x, const uint32_t* part, int K, int which, float* tap_scale)
+{
+    double s = 0.0;
+    const int nchunk = (x.NW() + 1) >> 1;
+    for (int ch = x.lane; ch < nchunk; ch += 32) {
+        uint4 v;
+        uint32_t spins = 0;
+        for (;;) {
+            v = x_ld128(part + 4 * ch);
+            if (v.y != SENT && (2 * ch + 1 >= x.NW() || v.w != SENT)) break;
+            if (++spins > SPIN_LIMIT || *x.dead) { poll_fail(x); break; }
+        }
+        s += __hiloint2double((int)v.y, (int)v.x);
+        if (2 * ch + 1 < x.NW()) s += __hiloint2double((int)v.w, (int)v.z);
+    }
+    s = warp_sum(s);
+    if (x.lane == 0) {
+        const float sc = act_scale(s, K, x.P.eps, scal(x)[0]);
+        scal(x)[which] = sc;
+        if (tap_scale) *tap_scale = sc;
+    }
 }
 
 // the elements a thread holds after gathering a slot-structured mailbox part (U or G): chunk ci = tid + j*THREADS is
-// piece ci % pps of slot ci / pps; slot g carries elements starts[g] .. starts[g+1]-1 and its fp64 partial at dpos
+// piece ci % pps of slot ci / pps; slot g carries elements starts[g] .. starts[g+1]-1
 template <int NJ>
 struct SlotEnum {
     const uint4 (&v)[NJ];
@@ -415,23 +469,6 @@ struct SlotEnum {
         }
     }
 };
-// sum of the fp64 partials found in this thread's gathered chunks
-template <int NJ, class S>
-__device__ __forceinline__ double slot_partials(const Ctx<S>& x, const uint4 (&v)[NJ], int nslots, int slot_w, int dpos)
-{
-    const int pps = slot_w >> 2;
-    double s = 0.0;
-#pragma unroll
-    for (int j = 0; j < NJ; ++j) {
-        const int ci = x.tid + j * THREADS;
-        if (ci < nslots * pps) {
-            const int g = ci / pps, ex = dpos - 4 * (ci - g * pps);
-            if (ex == 0) s += __hiloint2double((int)v[j].y, (int)v[j].x);
-            else if (ex == 2) s += __hiloint2double((int)v[j].w, (int)v[j].z);
-        }
-    }
-    return s;
-}
 
 // ------------------------------------------------------------------------------------------------
 // integer dot products
@@ -507,6 +544,12 @@ __device__ __forceinline__ int trow_dot(const uint8_t* row, int nbytes, const ui
     return warp_sum_i(s);
 }
 
+// exact int -> double without the 64-bit conversion unit (16 lanes / clock / SM): bits of 1.5 * 2^52 + b, minus 1.5 * 2^52
+__device__ __forceinline__ double i2d(int b)
+{
+    return __dadd_rn(__hiloint2double(0x43380000 + (b >> 31), b), -6755399441055744.0);
+}
+
 // ------------------------------------------------------------------------------------------------
 // weight / state pipeline
 // ------------------------------------------------------------------------------------------------
@@ -520,17 +563,16 @@ __device__ __forceinline__ void issue_item(const Ctx<S>& x, int item, int v0, in
     uint64_t* bar = (uint64_t*)(x.sm + P.s_mbar) + st;
     const uint64_t pol = policy_evict_first();
     if (item < P.L) {
+        if (x.service()) {
+            mbar_expect_tx(bar, P.schunk_bytes);
+            bulk_g2s_stream(stage, P.schunks + ((size_t)item * x.NS() + (x.c - x.NW())) * P.schunk_bytes, P.schunk_bytes, bar, pol);
+            return;
+        }
         const int* chs = (const int*)(x.sm + P.s_chs);
         const int ch0 = chs[x.c], nch = chs[x.c + 1] - ch0;
         const uint32_t ssm_b = (uint32_t)nch * x.d_state() * 4, conv_b = (uint32_t)nch * 16, econv_b = (uint32_t)x.gs() * 32;
-        const int e_t = x.t_in_task();                                      // LoRA-down row of in_proj this CTA owns (or -1)
-        const uint32_t tin_b = e_t >= 0 ? (uint32_t)x.d_model() : 0u;
-        const uint32_t tout_b = x.c < x.n_ttask() ? (uint32_t)(x.d_inner() / x.tsplit()) : 0u;
-        mbar_expect_tx(bar, P.chunk_bytes + P.blk_bytes + ssm_b + conv_b + econv_b + tin_b + tout_b);
-        if (tin_b) bulk_g2s_stream(stage + P.st_tin, P.A_in + ((size_t)item * x.r() + (e_t - x.n_bcdt())) * x.d_model(), tin_b, bar, pol);
-        if (tout_b)
-            bulk_g2s_stream(stage + P.st_tout, P.A_out + ((size_t)item * x.r() + x.c / x.tsplit()) * x.d_inner() + (size_t)(x.c % x.tsplit()) * tout_b, tout_b, bar, pol);
-        bulk_g2s_stream(stage, P.chunks + ((size_t)item * x.G() + x.c) * P.chunk_bytes, P.chunk_bytes, bar, pol);
+        mbar_expect_tx(bar, P.chunk_bytes + P.blk_bytes + ssm_b + conv_b + econv_b);
+        bulk_g2s_stream(stage, P.chunks + ((size_t)item * x.NW() + x.c) * P.chunk_bytes, P.chunk_bytes, bar, pol);
         bulk_g2s(stage + P.st_blk, P.blocks + (size_t)item * P.blk_bytes, P.blk_bytes, bar);
         bulk_g2s(stage + P.st_econv, P.conv + (size_t)item * P.conv_lstride + (size_t)x.d_inner() * 4, econv_b, bar);
         if (nch > 0) {
@@ -558,25 +600,27 @@ __device__ __forceinline__ void wait_item(const Ctx<S>& x, int item)
     }
 }
 
-// The stores of one CTA into the M mailboxes of a record.  publish and reset use the SAME thread -> address map, so
-// a reset and the later publish of a word are ordered by program order of one thread.
-//   slot (U / G): thread t < M * pps writes 16-byte piece t % pps of its slot in mailbox t / pps
+// The stores of one CTA into a record.  publish and reset use the SAME thread -> address map.
+//   slot (U / G): thread t < pps writes 16-byte piece t of its slot
 template <class S, typename F>
-__device__ __forceinline__ void slot_store(const Ctx<S>& x, uint32_t* rec, uint32_t part_off, int slot_w, int M, F piece_value)
+__device__ __forceinline__ void slot_store(const Ctx<S>& x, uint32_t* rec, uint32_t part_off, int slot_w, F piece_value)
 {
-    const Params& P = x.P;
     const int pps = slot_w >> 2;
-    for (int t = x.tid; t < M * pps; t += THREADS) {
-        const int m = t / pps, piece = t - m * pps;
-        x_st128(rec + (size_t)m * P.x_words + part_off + (size_t)x.c * slot_w + 4 * piece, piece_value(piece));
-    }
+    for (int t = x.tid; t < pps; t += THREADS) x_st128(rec + part_off + (size_t)x.c * slot_w + 4 * t, piece_value(t));
 }
-//   word (A / T): the lanes of one warp write the word to all mailboxes
+//   the worker's fp64 partial of a slot part: the last thread (a warp that publishes no slot piece)
+template <class S>
+__device__ __forceinline__ void partial_store(const Ctx<S>& x, uint32_t* rec, uint32_t part_off, uint32_t lo, uint32_t hi)
+{
+    if (x.tid == THREADS - 1) x_st64(rec + part_off + 2 * (size_t)x.c, lo, hi);
+}
+//   word (A / T): the lanes of one warp write the word to the small mailboxes the workers poll
 template <class S>
 __device__ __forceinline__ void word_store(const Ctx<S>& x, uint32_t* rec, uint32_t part_off, int idx, int M, uint32_t value)
 {
     const Params& P = x.P;
-    for (int m = x.lane; m < M; m += 32) x_st32(rec + (size_t)m * P.x_words + part_off + idx, value);
+    const int nm = mbox_count(x.NW(), M);
+    for (int m = x.lane; m < nm; m += 32) x_st32(rec + P.x_main + (size_t)m * P.x_small + part_off + idx, value);
 }
 
 // load time: replace A_log by A = -exp(A_log) inside every chunk (same sp_expf as the step would use; R10)
@@ -601,7 +645,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
     int* ors = (int*)(sm + P.s_ors);
     uint64_t* mbar = (uint64_t*)(sm + P.s_mbar);
     uint8_t* xq = sm + P.s_xq;
-    float* s_bc = (float*)(sm + P.s_bc);
+    float* s_bc = (float*)(sm + P.s_bc);             // B' [gs] (fp32)
+    double* s_cd = (double*)(sm + P.s_cd);           // C' [gs] as fp64: converted once, read by every channel of the state update
     float* s_u = (float*)(sm + P.s_u);
     float* s_z = (float*)(sm + P.s_z);
     float* s_x = (float*)(sm + P.s_x);
@@ -611,10 +656,13 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
     int* s_eacc = (int*)(sm + P.s_eacc);
     int* s_acc_in = (int*)(sm + P.s_acc_in);
     int* s_acc_out = (int*)(sm + P.s_acc_out);
+    const int NW = x.NW(), NS = x.NS();
+    const bool service = c >= NW;
+    const int sv = c - NW;                           // index among the service CTAs (if service)
 
-    for (int g = tid; g <= x.G(); g += THREADS) {
-        chs[g] = own_start(g, x.d_inner());
-        ors[g] = own_start(g, x.d_model());
+    for (int g = tid; g <= NW; g += THREADS) {
+        chs[g] = own_start(g, x.d_inner(), NW);
+        ors[g] = own_start(g, x.d_model(), NW);
     }
     if (tid < 2 * x.r_pad()) s_vin[tid] = 0.0;
     if (tid == 0) {
@@ -623,8 +671,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         fence_mbar_init();
     }
     __syncthreads();
-    const int ch0 = chs[c], nch = chs[c + 1] - ch0;
-    const int or0 = ors[c], nor = ors[c + 1] - or0;
+    const int ch0 = service ? 0 : chs[c], nch = service ? 0 : chs[c + 1] - ch0;
+    const int or0 = service ? 0 : ors[c], nor = service ? 0 : ors[c + 1] - or0;
     const int v0 = (int)(((long long)c * P.vocab) / x.G()), v1 = (int)(((long long)(c + 1) * P.vocab) / x.G());
     const int n_lm_items = (v1 - v0 + P.lm_rows_item - 1) / P.lm_rows_item;
     const int n_items = P.L + n_lm_items;
@@ -632,11 +680,10 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         for (int it = 0; it < P.stages && it < n_items; ++it) issue_item(x, it, v0, v1);
 
     const int ps = P.pos[0] & 3;                     // conv ring slot this step writes
-    const int nb_tasks = c < x.n_early() ? (x.n_early() - c + x.G() - 1) / x.G() : 0;      // early tasks of this CTA
     const int h0 = nch > 0 ? ch0 / x.headdim() : 0, h1 = nch > 0 ? (ch0 + nch - 1) / x.headdim() : -1;
     const bool taps_on = TAPS && P.taps != nullptr;
-    const size_t rec_words = (size_t)x.M() * P.x_words;
-    auto mbox = [&](int M) { return (size_t)(c / (GRID / M)) * P.x_words; };      // offset of the mailbox this CTA polls of a part pushed M times
+    const size_t rec_words = (size_t)P.x_main + (size_t)MBOX * P.x_small;
+    auto mbox = [&](int M) { return (size_t)P.x_main + (size_t)mbox_of(c, M) * P.x_small; };      // offset of the small mailbox this worker polls
     const int rtid = THREADS - 1 - tid;              // the small gathers (A, T) are polled from the last warp down
     uint32_t* s_slotU = (uint32_t*)(sm + P.s_slot);
     uint32_t* s_slotG = s_slotU + x.u_slot();
@@ -644,9 +691,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
     // K-split of the out_proj sign rows: every (row pair, K part) is one warp task
     const int KS = (THREADS >= 1024 && x.Wout() >= 128) ? 4 : (x.Wout() >= 64 ? 2 : 1);
     const int tbytes = x.d_inner() / x.tsplit();         // bytes of one out_proj LoRA-down partial task
+    // service: what this CTA holds of each dealt list
+    const int n_sig = service ? dealt(x.n_bcdt(), sv, NS) : 0, n_lin = service ? dealt(x.r(), sv, NS) : 0,
+              n_tt = service ? dealt(x.n_ttask(), sv, NS) : 0;
 
     // ---------------- S0 embedding + the first norm/quantise, redundantly in every CTA ----------------
-    float s_act;                                     // scale of the current activation codes
     int qsum;
     {
         int tok = P.tokens[0];
@@ -673,6 +722,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 v[j] = make_uint4(w[0], w[1], w[2], w[3]);
             }
         }
+        ss = warp_sum(ss);
+        if (lane == 0) red_d(x)[wid] = ss;           // read by thread 0 after the barriers of absmax_quant
         uint8_t* tp0 = (taps_on && c == 0 && P.L > 0) ? P.taps : nullptr;
         auto en = [&](auto f) {
 #pragma unroll
@@ -681,8 +732,16 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 if (k0 < x.d_model()) f(k0, v[j]);
             }
         };
-        qsum = norm_quant(x, en, ss, 1, 0, x.d_model(), P.L == 0, s_act, tp0 ? (int8_t*)(tp0 + P.tl.off[0]) : nullptr);
-        if (tp0 && tid == 0) *(float*)(tp0 + P.tl.off[1]) = s_act;
+        qsum = absmax_quant(x, en, x.d_model(), P.L == 0, tp0 ? (int8_t*)(tp0 + P.tl.off[0]) : nullptr);
+        if (tid == 0) {
+            double t4[4] = { 0.0, 0.0, 0.0, 0.0 };
+#pragma unroll
+            for (int i = 0; i < NWARPS; ++i) t4[i & 3] += red_d(x)[i];
+            const float sc = act_scale((t4[0] + t4[1]) + (t4[2] + t4[3]), x.d_model(), P.eps, scal(x)[0]);
+            scal(x)[1] = sc;
+            if (tp0) *(float*)(tp0 + P.tl.off[1]) = sc;
+        }
+        __syncthreads();
     }
 
     // =============================================== layers ===============================================
@@ -691,366 +750,386 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         const uint8_t* blk = stage + P.st_blk;
         uint8_t* tp = taps_on ? P.taps + (size_t)l * P.tap_lstride : nullptr;
         float* conv_l = P.conv + (size_t)l * P.conv_lstride;
-        uint32_t* rec = P.xbuf + (size_t)((P.rec0 + (uint32_t)l) & 3u) * rec_words;          // published into (all mailboxes)
-        uint32_t* recc = P.xbuf + (size_t)((P.rec0 + (uint32_t)l + 2u) & 3u) * rec_words;     // reset for layer l + 2
+        uint32_t* rec = P.xbuf + ((size_t)P.set * P.L + l) * rec_words;                       // this step's record of layer l
+        uint32_t* recp = rec - rec_words;                                                     // ... of layer l - 1 (U partials; l > 0)
+        uint32_t* recc = P.xbuf + ((size_t)(P.set ^ 1u) * P.L + l) * rec_words;               // the next step's: own words are reset here
         DFSSM_STAMP(l, 0);
         if (x.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + 31] = globaltimer_ns();
         wait_item(x, l);
         DFSSM_STAMP(l, 1);
-        // ---- early tasks: B|C|dt sign rows and LoRA-down rows of this CTA; raw int32 results are published ----
-        {
-            const uint32_t* bits = (const uint32_t*)(stage + P.c_in_bits);
-            for (int k = wid; k < nb_tasks; k += NWARPS) {
-                const int e = c + k * x.G();
-                int val;
-                if (e < x.n_bcdt()) {
-                    const uint32_t* const rowp[1] = { bits + (size_t)(2 * x.nch_max() + k) * x.Win() };
-                    int p[1];
-                    sign_partial<1>(rowp, 1, 0, x.Win(), xq, x.d_model(), lane, p);
-                    val = 2 * (warp_sum_i(p[0]) / 128) - qsum;       // exact: every term is a multiple of 128
-                } else {
-                    val = trow_dot(stage + P.st_tin, x.d_model(), xq, lane);
-                }
-                word_store(x, rec, P.x_A, e, M_A, (uint32_t)val ^ IBIAS);
-                if (lane == 0 && tp && e >= x.n_bcdt()) ((int32_t*)(tp + P.tl.off[3]))[e - x.n_bcdt()] = val;
-            }
-        }
-        // ---- S2: z and x sign rows of this CTA, NR_IN rows per warp pass, dealt from the top warp down ----
-        {
-            const uint32_t* bits = (const uint32_t*)(stage + P.c_in_bits);
-            const int n_tasks = 2 * nch;
-            for (int q = NWARPS - 1 - wid; NR_IN * q < n_tasks; q += NWARPS) {
-                const uint32_t* rowp[NR_IN];
-                int slot[NR_IN];
-                const int nrows = min(NR_IN, n_tasks - NR_IN * q);
-#pragma unroll
-                for (int r = 0; r < NR_IN; ++r) {
-                    const int t = NR_IN * q + r;
-                    slot[r] = r < nrows ? (t < nch ? t : x.nch_max() + (t - nch)) : 0;
-                    rowp[r] = bits + (size_t)slot[r] * x.Win();
-                }
-                int p[NR_IN];
-                sign_partial<NR_IN>(rowp, nrows, 0, x.Win(), xq, x.d_model(), lane, p);
-                const int v = RowReduce<NR_IN>::run(p, lane);
-                const int r = lane / (32 / NR_IN);
-                if (lane % (32 / NR_IN) == 0 && r < nrows) s_acc_in[slot[r]] = 2 * (v / 128) - qsum;
-            }
-        }
-        DFSSM_STAMP(l, 2);
-        {   // reset own slots of the record two layers ahead (same thread -> address map as the publishes); the warps
-            // that do it are not the ones polling A, so this costs nothing on the critical path
-            slot_store(x, recc, P.x_U, x.u_slot(), M_U, [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
-            slot_store(x, recc, P.x_G, x.g_slot(), M_G, [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
-            for (int k = wid; k < nb_tasks; k += NWARPS) word_store(x, recc, P.x_A, c + k * x.G(), M_A, SENT);
-            if (wid == 0 && c < x.n_ttask()) word_store(x, recc, P.x_T, c, M_T, SENT);
-        }
 
-        // ---- gather A: accumulators of all B|C|dt rows and t_in;  v_j = a_s[j] * float(t_j) ----
-        {
-            uint4 va[NJ_A];
-            hop_gather<NJ_A>(x, rec + mbox(M_A) + P.x_A, x.n_early(), 0, 0, va, rtid);
-            const float* a_s = (const float*)(blk + P.b_as_in);
+        if (service) {
+            // ================= service CTA: rows whose result every worker needs =================
+            // ---- in_proj: B|C|dt sign rows and LoRA-down rows dealt to this CTA; raw int32 results are published ----
+            {
+                const uint32_t* bits = (const uint32_t*)(stage + P.sc_sign);
+                for (int k = wid; k < n_sig + n_lin; k += NWARPS) {
+                    int val, idx;
+                    if (k < n_sig) {
+                        const uint32_t* const rowp[1] = { bits + (size_t)k * x.Win() };
+                        int p[1];
+                        sign_partial<1>(rowp, 1, 0, x.Win(), xq, x.d_model(), lane, p);
+                        val = 2 * (warp_sum_i(p[0]) / 128) - qsum;       // exact: every term is a multiple of 128
+                        idx = sv + k * NS;
+                    } else {
+                        const int kk = k - n_sig;
+                        val = trow_dot(stage + P.sc_tin + (size_t)kk * x.d_model(), x.d_model(), xq, lane);
+                        idx = x.n_bcdt() + sv + kk * NS;
+                    }
+                    word_store(x, rec, P.x_A, idx, M_A, (uint32_t)val ^ IBIAS);
+                }
+            }
+            DFSSM_STAMP(l, 2);
+            // ---- gather G, codes of the whole gated vector ----
+            int qsum_g;
+            {
+                uint4 vg[NJ_G];
+                hop_gather<NJ_G>(x, rec + P.x_G, NW * x.g_slot(), vg, tid);
+                DFSSM_STAMP(l, 6);
+                qsum_g = absmax_quant(x, SlotEnum<NJ_G>{ vg, chs, tid, NW, x.g_slot() >> 2 }, x.d_inner(), false, nullptr, l, 16);
+            }
+            (void)qsum_g;
+            DFSSM_STAMP(l, 7);
+            // ---- out_proj: LoRA-down partial tasks dealt to this CTA ----
+            for (int k = wid; k < n_tt; k += NWARPS) {
+                const int q = sv + k * NS, part = q % x.tsplit();
+                const int t = trow_dot(stage + P.sc_tout + (size_t)k * tbytes, tbytes, xq + (size_t)part * tbytes, lane);
+                word_store(x, rec, P.x_T, q, M_T, (uint32_t)t ^ IBIAS);
+            }
+            DFSSM_STAMP(l, 8);
+            // ---- reset own words of the next step's record of this layer (this CTA is idle until U arrives) ----
+            for (int k = wid; k < n_sig; k += NWARPS) word_store(x, recc, P.x_A, sv + k * NS, M_A, SENT);
+            for (int k = wid; k < n_lin; k += NWARPS) word_store(x, recc, P.x_A, x.n_bcdt() + sv + k * NS, M_A, SENT);
+            for (int k = wid; k < n_tt; k += NWARPS) word_store(x, recc, P.x_T, sv + k * NS, M_T, SENT);
+            __syncthreads();                        // every thread is done with this stage's weights
+            DFSSM_STAMP(l, 10);
+        } else {
+            // ================= worker CTA =================
+            // ---- S2: z and x sign rows of this CTA, NR_IN rows per warp pass, dealt from the top warp down ----
+            {
+                const uint32_t* bits = (const uint32_t*)(stage + P.c_in_bits);
+                const int n_tasks = 2 * nch;
+                for (int q = NWARPS - 1 - wid; NR_IN * q < n_tasks; q += NWARPS) {
+                    const uint32_t* rowp[NR_IN];
+                    int slot[NR_IN];
+                    const int nrows = min(NR_IN, n_tasks - NR_IN * q);
 #pragma unroll
-            for (int j = 0; j < NJ_A; ++j) {
-                const int e0 = 4 * (rtid + j * THREADS);
-                const uint32_t w[4] = { va[j].x, va[j].y, va[j].z, va[j].w };
+                    for (int r = 0; r < NR_IN; ++r) {
+                        const int t = NR_IN * q + r;
+                        slot[r] = r < nrows ? (t < nch ? t : x.nch_max() + (t - nch)) : 0;
+                        rowp[r] = bits + (size_t)slot[r] * x.Win();
+                    }
+                    int p[NR_IN];
+                    sign_partial<NR_IN>(rowp, nrows, 0, x.Win(), xq, x.d_model(), lane, p);
+                    const int v = RowReduce<NR_IN>::run(p, lane);
+                    const int r = lane / (32 / NR_IN);
+                    if (lane % (32 / NR_IN) == 0 && r < nrows) s_acc_in[slot[r]] = 2 * (v / 128) - qsum;
+                }
+            }
+            DFSSM_STAMP(l, 2);
+            {   // reset own slots of the next step's record of this layer (same thread -> address map as the publishes)
+                slot_store(x, recc, P.x_U, x.u_slot(), [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
+                slot_store(x, recc, P.x_G, x.g_slot(), [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
+                partial_store(x, recc, P.x_PU, SENT, SENT);
+                partial_store(x, recc, P.x_PG, SENT, SENT);
+            }
+            // ---- warp 0: scale of the in_proj codes from the U partials of layer l - 1 (layer 0: made with the embedding) ----
+            if (wid == 0 && l > 0)
+                scale_side(x, recp + P.x_PU, x.d_model(), 1, (tp && c == 0) ? (float*)(tp + P.tl.off[1]) : nullptr);
+            // ---- gather A: accumulators of all B|C|dt rows and t_in;  v_j = a_s[j] * float(t_j) ----
+            {
+                uint4 va[NJ_A];
+                hop_gather<NJ_A>(x, rec + mbox(M_A) + P.x_A, x.n_early(), va, rtid);
+                const float* a_s = (const float*)(blk + P.b_as_in);
 #pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    const int e = e0 + i;
-                    if (e < x.n_early()) {
-                        const int val = (int)(w[i] ^ IBIAS);
-                        if (e < x.n_bcdt()) s_eacc[e] = val;
-                        else s_vin[e - x.n_bcdt()] = (double)fmul(a_s[e - x.n_bcdt()], (float)val);
+                for (int j = 0; j < NJ_A; ++j) {
+                    const int e0 = 4 * (rtid + j * THREADS);
+                    const uint32_t w[4] = { va[j].x, va[j].y, va[j].z, va[j].w };
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const int e = e0 + i;
+                        if (e < x.n_early()) {
+                            const int val = (int)(w[i] ^ IBIAS);
+                            if (e < x.n_bcdt()) s_eacc[e] = val;
+                            else {
+                                s_vin[e - x.n_bcdt()] = (double)fmul(a_s[e - x.n_bcdt()], (float)val);
+                                if (tp && c == 0) ((int32_t*)(tp + P.tl.off[3]))[e - x.n_bcdt()] = val;
+                            }
+                        }
                     }
                 }
             }
-        }
-        __syncthreads();
-        DFSSM_STAMP(l, 3);
-        // ---- S3 stage 2 + S4 conv + dt softplus: LPR lanes per row; own z|x rows and ALL B|C rows (+ own dt) ----
-        {
-            const int n_dt = tp ? x.nheads() : (h1 - h0 + 1);
-            const int n_rows = 2 * nch + 2 * x.gs() + n_dt;
-            float* ring = (float*)(stage + P.st_conv);
-            const float* ering = (const float*)(stage + P.st_econv);
-            // rows [first, first + count) of the index space (z | x | B|C | dt), skipping skip_len rows from skip_from on;
-            // LP lanes share a row's LoRA sum
-            // done by the threads [t0, t0 + nthr) (whole warps)
-            auto epi = [&](auto lp_tag, int first, int count, int skip_from, int skip_len, int t0, int nthr) {
-              constexpr int LP = decltype(lp_tag)::value;
-              const int lt = tid - t0;
-              if (lt < 0 || lt >= nthr) return;
-              for (int ib = 0; ib < count; ib += nthr / LP) {          // warp-uniform trip count (shuffles inside)
-                int i = first + min(ib + lt / LP, count - 1);
-                if (i >= skip_from) i += skip_len;
-                const int sub = lt % LP;
-                const bool valid = ib + lt / LP < count;
-                int kind, slot = 0, e = 0;         // kind 0 z, 1 x, 2 B|C, 3 dt
-                if (i < nch) { kind = 0; slot = i; }
-                else if (i < 2 * nch) { kind = 1; slot = x.nch_max() + (i - nch); }
-                else if (i < 2 * nch + 2 * x.gs()) { kind = 2; e = i - 2 * nch; }
-                else { kind = 3; e = 2 * x.gs() + (tp ? 0 : h0) + (i - 2 * nch - 2 * x.gs()); }
-                const bool own = kind < 2;
-                // LoRA-up row as 4-byte words: own rows are [slot][r_pad]; the B|C|dt rows of the shared block are stored word-major
-                // ([r_pad / 4][n_bcdt]) so that one thread per row reads shared memory without bank conflicts
-                const int* bw = own ? (const int*)(stage + P.c_in_B + (size_t)slot * x.r_pad()) : (const int*)(blk + P.b_eB) + e;
-                const int bstep = own ? 1 : x.n_bcdt();
-                double lo0 = 0.0, lo1 = 0.0;
-                for (int j4 = 4 * sub; j4 < x.r_pad(); j4 += 4 * LP) {         // pad entries of B are 0, pad entries of v are 0
-                    const int w = bw[(j4 >> 2) * bstep];
-                    lo0 = __fma_rn((double)(int8_t)w, s_vin[j4], lo0);
-                    lo1 = __fma_rn((double)(int8_t)(w >> 8), s_vin[j4 + 1], lo1);
-                    lo0 = __fma_rn((double)(int8_t)(w >> 16), s_vin[j4 + 2], lo0);
-                    lo1 = __fma_rn((double)(w >> 24), s_vin[j4 + 3], lo1);
-                }
-                lo0 += lo1;
-#pragma unroll
-                for (int o = LP / 2; o > 0; o >>= 1) lo0 += __shfl_xor_sync(0xffffffffu, lo0, o);
-                if (sub != 0 || !valid) continue;
-                const float scale = own ? ((const float*)(stage + P.c_in_scale))[slot] : ((const float*)(blk + P.b_escale))[e];
-                const float bsv = own ? ((const float*)(stage + P.c_in_bs))[slot] : ((const float*)(blk + P.b_ebs))[e];
-                const int acc = own ? s_acc_in[slot] : s_eacc[e];
-                const float lo = (float)lo0;
-                const float val = fmul(s_act, fadd(fmul(scale, (float)acc), fmul(bsv, lo)));
-                int row;                       // canonical in_proj row (for the taps)
-                bool tap_owner = true;
-                if (kind == 0) {
-                    s_z[i] = val;
-                    row = ch0 + i;
-                } else if (kind == 1) {
-                    const int ic = i - nch;
-                    float* rg = ring + 4 * ic;
-                    const float s0 = rg[(ps + 1) & 3], s1 = rg[(ps + 2) & 3], s2 = rg[(ps + 3) & 3];
-                    const float4 cw = *(const float4*)(stage + P.c_conv_w + 16 * ic);
-                    float o = ((const float*)(stage + P.c_conv_b))[ic];
-                    o = ffma(cw.x, s0, o); o = ffma(cw.y, s1, o); o = ffma(cw.z, s2, o); o = ffma(cw.w, val, o);
-                    rg[ps] = val;
-                    const float cv = siluf(o);
-                    s_x[ic] = cv;
-                    row = x.d_inner() + ch0 + ic;
-                    if (tp) ((float*)(tp + P.tl.off[5]))[ch0 + ic] = cv;
-                } else if (kind == 2) {
-                    const float* rg = ering + 4 * e;
-                    const float s0 = rg[(ps + 1) & 3], s1 = rg[(ps + 2) & 3], s2 = rg[(ps + 3) & 3];
-                    const float4 cw = *(const float4*)(blk + P.b_econv_w + 16 * e);
-                    float o = ((const float*)(blk + P.b_econv_b))[e];
-                    o = ffma(cw.x, s0, o); o = ffma(cw.y, s1, o); o = ffma(cw.z, s2, o); o = ffma(cw.w, val, o);
-                    tap_owner = e % x.G() == c;
-                    if (tap_owner) conv_l[4 * (size_t)(x.d_inner() + e) + ps] = val;      // the early-task owner keeps the state
-                    const float cv = siluf(o);
-                    s_bc[e] = cv;
-                    row = 2 * x.d_inner() + e;
-                    if (tp && tap_owner) ((float*)(tp + P.tl.off[5]))[x.d_inner() + e] = cv;
-                } else {
-                    const int h = e - 2 * x.gs();
-                    const float dtv = sp_softplusf(fadd(val, ((const float*)(blk + P.b_dtb))[h]));
-                    s_dt[h] = dtv;
-                    row = 2 * x.d_inner() + e;
-                    tap_owner = e % x.G() == c;
-                    if (tp && tap_owner) ((float*)(tp + P.tl.off[6]))[h] = dtv;
-                }
-                if (tp && tap_owner) {
-                    ((float*)(tp + P.tl.off[4]))[row] = val;
-                    ((int32_t*)(tp + P.tl.off[2]))[row] = acc;
-                }
-              }
-            };
-            // first half of the CTA: the 2 gs B|C rows, one thread per row (dense tails); second half, at the same time: the
-            // few own rows (z, x, dt) with 4 lanes each
-            epi(std::integral_constant<int, 1>{}, 2 * nch, 2 * x.gs(), 1 << 30, 0, 0, THREADS / 2);
-            epi(std::integral_constant<int, 4>{}, 0, 2 * nch + n_dt, 2 * nch, 2 * x.gs(), THREADS / 2, THREADS / 2);
-        }
-        __syncthreads();
-        DFSSM_STAMP(l, 4);
-
-        // ---- S5 state update + readout, S6 gate: LPC lanes per channel; t = g*w is published as it is produced ----
-        {
-            double ss_own = 0.0;
-            const int hpg = x.nheads() / x.ngroups();
-            const float* Aneg = (const float*)(stage + P.c_alog);      // A = -exp(A_log), made by k_mega_prepare at load
-            const float* Dv = (const float*)(stage + P.c_D);
-            const float* gw = (const float*)(stage + P.c_gnorm);
-            const int l16 = tid % LPC;
-            for (int ib = 0; ib < nch; ib += THREADS / LPC) {        // warp-uniform trip count (shuffles inside)
-                const int i = min(ib + tid / LPC, nch - 1);
-                const bool valid = ib + tid / LPC < nch;
-                const int ch = ch0 + i, h = ch / x.headdim(), grp = h / hpg;
-                const float dtv = s_dt[h];
-                const float An = Aneg[i];
-                const float dA = sp_expf(fmul(dtv, An));
-                const float xv = s_x[i];
-                const float dtx = fmul(dtv, xv);
-                const float sz = siluf(s_z[i]);             // all lanes: free in SIMT, and off the tail of the reduction
-                float* Hr = (float*)(stage + P.st_ssm) + (size_t)i * x.d_state();
-                const float* Bc = s_bc + grp * x.d_state();
-                const float* Cc = s_bc + x.gs() + grp * x.d_state();
-                double a = 0.0;
-                for (int n4 = l16; valid && n4 < x.d_state() / 4; n4 += LPC) {
-                    float4 hv = *(const float4*)(Hr + 4 * n4);
-                    const float4 bv = *(const float4*)(Bc + 4 * n4);
-                    const float4 cv = *(const float4*)(Cc + 4 * n4);
-                    hv.x = ffma(dA, hv.x, fmul(dtx, bv.x));
-                    hv.y = ffma(dA, hv.y, fmul(dtx, bv.y));
-                    hv.z = ffma(dA, hv.z, fmul(dtx, bv.z));
-                    hv.w = ffma(dA, hv.w, fmul(dtx, bv.w));
-                    *(float4*)(Hr + 4 * n4) = hv;
-                    a = dacc(a, cv.x, hv.x); a = dacc(a, cv.y, hv.y); a = dacc(a, cv.z, hv.z); a = dacc(a, cv.w, hv.w);
-                }
-#pragma unroll
-                for (int o = LPC / 2; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o, LPC);
-                if (l16 == 0 && valid) {
-                    a = dacc(a, Dv[i], xv);
-                    const float y = (float)a;
-                    const float gv = fmul(y, sz);
-                    s_slotG[i] = __float_as_uint(fmul(gv, gw[i]));
-                    ss_own = dacc(ss_own, gv, gv);
-                    if (tp) { ((float*)(tp + P.tl.off[7]))[ch] = y; ((float*)(tp + P.tl.off[8]))[ch] = gv; }
-                }
-            }
-            x.stamp(l, 24);
-            fence_proxy_async();               // the updated state is about to be read by the async proxy
-            x.stamp(l, 25);
-            ss_own = warp_sum_strided(ss_own, LPC);     // only lanes 0 and 16 hold a value
-            if (lane == 0) red_d(x)[wid] = ss_own;
             __syncthreads();
-            x.stamp(l, 26);
-            slot_store(x, rec, P.x_G, x.g_slot(), M_G, [&](int piece) {
-                uint4 w = *(const uint4*)(s_slotG + 4 * piece);
-                const int ex = x.g_dpos() - 4 * piece;
-                if (ex == 0 || ex == 2) {
-                    double t4[4] = { 0.0, 0.0, 0.0, 0.0 };
+            DFSSM_STAMP(l, 3);
+            const float s_act = scal(x)[1];
+            // ---- S3 stage 2 + S4 conv + dt softplus: own z|x rows and ALL B|C rows (+ own dt) ----
+            {
+                const int n_dt = (tp && c == 0) ? x.nheads() : (h1 - h0 + 1);
+                float* ring = (float*)(stage + P.st_conv);
+                const float* ering = (const float*)(stage + P.st_econv);
+                // rows [first, first + count) of the index space (z | x | B|C | dt), skipping skip_len rows from skip_from on;
+                // LP lanes share a row's LoRA sum; done by the threads [t0, t0 + nthr) (whole warps)
+                auto epi = [&](auto lp_tag, int first, int count, int skip_from, int skip_len, int t0, int nthr) {
+                  constexpr int LP = decltype(lp_tag)::value;
+                  const int lt = tid - t0;
+                  if (lt < 0 || lt >= nthr) return;
+                  for (int ib = 0; ib < count; ib += nthr / LP) {          // warp-uniform trip count (shuffles inside)
+                    int i = first + min(ib + lt / LP, count - 1);
+                    if (i >= skip_from) i += skip_len;
+                    const int sub = lt % LP;
+                    const bool valid = ib + lt / LP < count;
+                    int kind, slot = 0, e = 0;         // kind 0 z, 1 x, 2 B|C, 3 dt
+                    if (i < nch) { kind = 0; slot = i; }
+                    else if (i < 2 * nch) { kind = 1; slot = x.nch_max() + (i - nch); }
+                    else if (i < 2 * nch + 2 * x.gs()) { kind = 2; e = i - 2 * nch; }
+                    else { kind = 3; e = 2 * x.gs() + ((tp && c == 0) ? 0 : h0) + (i - 2 * nch - 2 * x.gs()); }
+                    const bool own = kind < 2;
+                    // LoRA-up row as 4-byte words: own rows are [slot][r_pad]; the B|C|dt rows of the shared block are stored word-major
+                    // ([r_pad / 4][n_bcdt]) so that one thread per row reads shared memory without bank conflicts
+                    const int* bw = own ? (const int*)(stage + P.c_in_B + (size_t)slot * x.r_pad()) : (const int*)(blk + P.b_eB) + e;
+                    const int bstep = own ? 1 : x.n_bcdt();
+                    double lo0 = 0.0, lo1 = 0.0;
+                    for (int j4 = 4 * sub; j4 < x.r_pad(); j4 += 4 * LP) {         // pad entries of B are 0, pad entries of v are 0
+                        const int w = bw[(j4 >> 2) * bstep];
+                        lo0 = __fma_rn(i2d((int)(int8_t)w), s_vin[j4], lo0);
+                        lo1 = __fma_rn(i2d((int)(int8_t)(w >> 8)), s_vin[j4 + 1], lo1);
+                        lo0 = __fma_rn(i2d((int)(int8_t)(w >> 16)), s_vin[j4 + 2], lo0);
+                        lo1 = __fma_rn(i2d(w >> 24), s_vin[j4 + 3], lo1);
+                    }
+                    lo0 += lo1;
 #pragma unroll
-                    for (int i = 0; i < NWARPS; ++i) t4[i & 3] += red_d(x)[i];
-                    const double tot = (t4[0] + t4[1]) + (t4[2] + t4[3]);
-                    const uint32_t lo = (uint32_t)__double2loint(tot), hi = (uint32_t)__double2hiint(tot);
-                    if (ex == 0) { w.x = lo; w.y = hi; } else { w.z = lo; w.w = hi; }
-                }
-                return w;
-            });
-            x.stamp(l, 27);
-            if (tid == DMA_TID && nch > 0) {   // write the state slice back (async), while the exchange goes on
-                bulk_s2g_stream(P.ssm + (size_t)l * P.ssm_lstride + (size_t)ch0 * x.d_state(), stage + P.st_ssm, (uint32_t)nch * x.d_state() * 4,
-                                policy_evict_first());
-                bulk_s2g(conv_l + (size_t)ch0 * 4, stage + P.st_conv, (uint32_t)nch * 16);
-                bulk_commit();
+                    for (int o = LP / 2; o > 0; o >>= 1) lo0 += __shfl_xor_sync(0xffffffffu, lo0, o);
+                    if (sub != 0 || !valid) continue;
+                    const float scale = own ? ((const float*)(stage + P.c_in_scale))[slot] : ((const float*)(blk + P.b_escale))[e];
+                    const float bsv = own ? ((const float*)(stage + P.c_in_bs))[slot] : ((const float*)(blk + P.b_ebs))[e];
+                    const int acc = own ? s_acc_in[slot] : s_eacc[e];
+                    const float lo = (float)lo0;
+                    const float val = fmul(s_act, fadd(fmul(scale, (float)acc), fmul(bsv, lo)));
+                    int row;                       // canonical in_proj row (for the taps)
+                    bool tap_owner = true;
+                    if (kind == 0) {
+                        s_z[i] = val;
+                        row = ch0 + i;
+                    } else if (kind == 1) {
+                        const int ic = i - nch;
+                        float* rg = ring + 4 * ic;
+                        const float s0 = rg[(ps + 1) & 3], s1 = rg[(ps + 2) & 3], s2 = rg[(ps + 3) & 3];
+                        const float4 cw = *(const float4*)(stage + P.c_conv_w + 16 * ic);
+                        float o = ((const float*)(stage + P.c_conv_b))[ic];
+                        o = ffma(cw.x, s0, o); o = ffma(cw.y, s1, o); o = ffma(cw.z, s2, o); o = ffma(cw.w, val, o);
+                        rg[ps] = val;
+                        const float cv = siluf(o);
+                        s_x[ic] = cv;
+                        row = x.d_inner() + ch0 + ic;
+                        if (tp) ((float*)(tp + P.tl.off[5]))[ch0 + ic] = cv;
+                    } else if (kind == 2) {
+                        const float* rg = ering + 4 * e;
+                        const float s0 = rg[(ps + 1) & 3], s1 = rg[(ps + 2) & 3], s2 = rg[(ps + 3) & 3];
+                        const float4 cw = *(const float4*)(blk + P.b_econv_w + 16 * e);
+                        float o = ((const float*)(blk + P.b_econv_b))[e];
+                        o = ffma(cw.x, s0, o); o = ffma(cw.y, s1, o); o = ffma(cw.z, s2, o); o = ffma(cw.w, val, o);
+                        if (e % NW == c) conv_l[4 * (size_t)(x.d_inner() + e) + ps] = val;      // one worker keeps the state of this channel
+                        const float cv = siluf(o);
+                        if (e < x.gs()) s_bc[e] = cv;
+                        else s_cd[e - x.gs()] = (double)cv;
+                        row = 2 * x.d_inner() + e;
+                        tap_owner = c == 0;
+                        if (tp && tap_owner) ((float*)(tp + P.tl.off[5]))[x.d_inner() + e] = cv;
+                    } else {
+                        const int h = e - 2 * x.gs();
+                        const float dtv = sp_softplusf(fadd(val, ((const float*)(blk + P.b_dtb))[h]));
+                        s_dt[h] = dtv;
+                        row = 2 * x.d_inner() + e;
+                        tap_owner = c == 0;
+                        if (tp && tap_owner) ((float*)(tp + P.tl.off[6]))[h] = dtv;
+                    }
+                    if (tp && tap_owner) {
+                        ((float*)(tp + P.tl.off[4]))[row] = val;
+                        ((int32_t*)(tp + P.tl.off[2]))[row] = acc;
+                    }
+                  }
+                };
+                // first half of the CTA: the 2 gs B|C rows, one thread per row (dense tails); second half, at the same time: the
+                // few own rows (dt first: the longest tail; then x, z) with 4 lanes each if they fit one pass, else 2
+                epi(std::integral_constant<int, LPB>{}, 2 * nch, 2 * x.gs(), 1 << 30, 0, 0, THREADS / 2);
+                if (4 * (2 * nch + n_dt) <= THREADS / 2)
+                    epi(std::integral_constant<int, 4>{}, 0, 2 * nch + n_dt, 2 * nch, 2 * x.gs(), THREADS / 2, THREADS / 2);
+                else
+                    epi(std::integral_constant<int, 2>{}, 0, 2 * nch + n_dt, 2 * nch, 2 * x.gs(), THREADS / 2, THREADS / 2);
             }
-        }
-        DFSSM_STAMP(l, 5);
+            __syncthreads();
+            DFSSM_STAMP(l, 4);
 
-        // ---- gather G, S6 norm + quantise of the whole gated vector in every CTA ----
-        float s_g;
-        int qsum_g;
-        {
-            uint4 vg[NJ_G];
-            hop_gather<NJ_G>(x, rec + mbox(M_G) + P.x_G, x.G() * x.g_slot(), x.g_slot(), x.g_dpos(), vg, tid, DFSSM_WG);
-            DFSSM_STAMP(l, 6);
-            const double ssl = slot_partials<NJ_G>(x, vg, x.G(), x.g_slot(), x.g_dpos());
-            const int gpps = x.g_slot() >> 2;            // the fp64 partials sit in the lanes (g_dpos / 4) mod pps
-            qsum_g = norm_quant(x, SlotEnum<NJ_G>{ vg, chs, tid, x.G(), gpps }, ssl, gpps < 32 ? gpps : 1, gpps < 32 ? (x.g_dpos() >> 2) % gpps : 0,
-                                x.d_inner(), false, s_g,
-                                (tp && c == 0) ? (int8_t*)(tp + P.tl.off[9]) : nullptr, l, 16);
-            if (tp && c == 0 && tid == 0) *(float*)(tp + P.tl.off[10]) = s_g;
-        }
-        DFSSM_STAMP(l, 7);
-        // ---- S7: LoRA-down partial task (warp 0, published) and the out_proj sign rows (other warps) ----
-        if (wid == 0) {
-            if (c < x.n_ttask()) {
-                const int part = c % x.tsplit();
-                const int t = trow_dot(stage + P.st_tout, tbytes, xq + (size_t)part * tbytes, lane);
-                word_store(x, rec, P.x_T, c, M_T, (uint32_t)t ^ IBIAS);
-            }
-        } else {
-            const uint32_t* bits = (const uint32_t*)(stage + P.c_out_bits);
-            const int npair = (nor + 1) >> 1, wspan = x.Wout() / KS;
-            for (int id = wid - 1; id < npair * KS; id += NWARPS - 1) {
-                const int pair = id / KS, half = id - pair * KS;
-                const int nrows = min(2, nor - 2 * pair);
-                const uint32_t* const rowp[2] = { bits + (size_t)(2 * pair) * x.Wout(), bits + (size_t)(2 * pair + (nrows > 1 ? 1 : 0)) * x.Wout() };
-                int p[2];
-                sign_partial<2>(rowp, nrows, half * wspan, half == KS - 1 ? x.Wout() : (half + 1) * wspan, xq, x.d_inner(), lane, p);
-                const int v = reduce2(p, lane);
-                const int r = lane >> 4;
-                if ((lane & 15) == 0 && r < nrows) s_acc_out[half * x.nor_max() + 2 * pair + r] = v;
-            }
-        }
-        DFSSM_STAMP(l, 8);
-        // ---- gather T: t_out = sum of the partial sums;  v_j = a_s[j] * float(t_j) ----
-        {
-            uint4 vt[1];
-            hop_gather<1>(x, rec + mbox(M_T) + P.x_T, x.n_ttask(), 0, 0, vt, rtid);
-            const float* a_s = (const float*)(blk + P.b_as_out);
-            const uint32_t w[4] = { vt[0].x, vt[0].y, vt[0].z, vt[0].w };
-            const int rows_per_chunk = 4 / x.tsplit();
+            // ---- S5 state update + readout, S6 gate: LPC lanes per channel; t = g*w is published as it is produced ----
+            {
+                double ss_own = 0.0;
+                const int hpg = x.nheads() / x.ngroups();
+                const float* Aneg = (const float*)(stage + P.c_alog);      // A = -exp(A_log), made by k_mega_prepare at load
+                const float* Dv = (const float*)(stage + P.c_D);
+                const float* gw = (const float*)(stage + P.c_gnorm);
+                const int l16 = tid % LPC;
+                for (int ib = 0; ib < nch; ib += THREADS / LPC) {        // warp-uniform trip count (shuffles inside)
+                    const int i = min(ib + tid / LPC, nch - 1);
+                    const bool valid = ib + tid / LPC < nch;
+                    const int ch = ch0 + i, h = ch / x.headdim(), grp = h / hpg;
+                    const float dtv = s_dt[h];
+                    const float An = Aneg[i];
+                    const float dA = sp_expf(fmul(dtv, An));
+                    const float xv = s_x[i];
+                    const float dtx = fmul(dtv, xv);
+                    const float sz = siluf(s_z[i]);             // all lanes: free in SIMT, and off the tail of the reduction
+                    float* Hr = (float*)(stage + P.st_ssm) + (size_t)i * x.d_state();
+                    const float* Bc = s_bc + grp * x.d_state();
+                    const double* Cc = s_cd + grp * x.d_state();
+                    double a0 = 0.0, a1 = 0.0;
+                    for (int n4 = l16; valid && n4 < x.d_state() / 4; n4 += LPC) {
+                        float4 hv = *(const float4*)(Hr + 4 * n4);
+                        const float4 bv = *(const float4*)(Bc + 4 * n4);
+                        const double2 c01 = *(const double2*)(Cc + 4 * n4), c23 = *(const double2*)(Cc + 4 * n4 + 2);
+                        hv.x = ffma(dA, hv.x, fmul(dtx, bv.x));
+                        hv.y = ffma(dA, hv.y, fmul(dtx, bv.y));
+                        hv.z = ffma(dA, hv.z, fmul(dtx, bv.z));
+                        hv.w = ffma(dA, hv.w, fmul(dtx, bv.w));
+                        *(float4*)(Hr + 4 * n4) = hv;
+                        a0 = __fma_rn(c01.x, (double)hv.x, a0); a1 = __fma_rn(c01.y, (double)hv.y, a1);
+                        a0 = __fma_rn(c23.x, (double)hv.z, a0); a1 = __fma_rn(c23.y, (double)hv.w, a1);
+                    }
+                    double a = a0 + a1;
 #pragma unroll
-            for (int jj = 0; jj < 4; ++jj) {
-                const int j = rtid * rows_per_chunk + jj;
-                if (jj < rows_per_chunk && j < x.r()) {
-                    int t = 0;
-                    for (int q = 0; q < x.tsplit(); ++q) t += (int)(w[jj * x.tsplit() + q] ^ IBIAS);
-                    s_vout[j] = (double)fmul(a_s[j], (float)t);
-                    if (tp && c == 0) ((int32_t*)(tp + P.tl.off[12]))[j] = t;
+                    for (int o = LPC / 2; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o, LPC);
+                    if (l16 == 0 && valid) {
+                        a = dacc(a, Dv[i], xv);
+                        const float y = (float)a;
+                        const float gv = fmul(y, sz);
+                        s_slotG[i] = __float_as_uint(fmul(gv, gw[i]));
+                        ss_own = dacc(ss_own, gv, gv);
+                        if (tp) { ((float*)(tp + P.tl.off[7]))[ch] = y; ((float*)(tp + P.tl.off[8]))[ch] = gv; }
+                    }
                 }
-            }
-        }
-        __syncthreads();
-        DFSSM_STAMP(l, 9);
-        // ---- S7 epilogue + residual; t = u*w of the next norm is published as it is produced ----
-        {
-            double ss_u = 0.0;
-            const int8_t* Bm = (const int8_t*)(stage + P.c_out_B);
-            const float* scale = (const float*)(stage + P.c_out_scale);
-            const float* bsv = (const float*)(stage + P.c_out_bs);
-            const float* nw = (const float*)(stage + P.c_nnorm);
-            for (int ib = 0; ib < nor; ib += THREADS / 4) {
-                const int i = ib + (tid >> 2), sub = tid & 3;
-                const bool valid = i < nor;
-                double lo = 0.0;
-                const int8_t* brow = Bm + (size_t)(valid ? i : 0) * x.r_pad();
-                if (valid)
-                    for (int j = sub; j < x.r(); j += 4) lo = __fma_rn((double)brow[j], s_vout[j], lo);
-                lo += __shfl_xor_sync(0xffffffffu, lo, 1);
-                lo += __shfl_xor_sync(0xffffffffu, lo, 2);
-                if (sub != 0 || !valid) continue;
-                int p128 = s_acc_out[i];
-                for (int hh = 1; hh < KS; ++hh) p128 += s_acc_out[hh * x.nor_max() + i];
-                const int acc = 2 * (p128 / 128) - qsum_g;       // exact: every term is a multiple of 128
-                const float o = fmul(s_g, fadd(fmul(scale[i], (float)acc), fmul(bsv[i], (float)lo)));
-                const float un = fadd(s_u[i], o);
-                s_u[i] = un;
-                s_slotU[i] = __float_as_uint(fmul(un, nw[i]));
-                ss_u = dacc(ss_u, un, un);
-                if (tp) { ((float*)(tp + P.tl.off[13]))[or0 + i] = un; ((int32_t*)(tp + P.tl.off[11]))[or0 + i] = acc; }
-            }
-            ss_u = warp_sum_strided(ss_u, 4);           // only every fourth lane holds a value
-            if (lane == 0) red_d(x)[wid] = ss_u;
-            __syncthreads();                        // also: every thread is done with this stage's weights
-            slot_store(x, rec, P.x_U, x.u_slot(), M_U, [&](int piece) {
-                uint4 w = *(const uint4*)(s_slotU + 4 * piece);
-                const int ex = x.u_dpos() - 4 * piece;
-                if (ex == 0 || ex == 2) {
+                x.stamp(l, 24);
+                fence_proxy_async();               // the updated state is about to be read by the async proxy
+                if (LPC < 32) ss_own = warp_sum_strided(ss_own, LPC);     // only the lanes 0, LPC, ... hold a value
+                if (lane == 0) red_d(x)[wid] = ss_own;
+                __syncthreads();
+                x.stamp(l, 26);
+                slot_store(x, rec, P.x_G, x.g_slot(), [&](int piece) { return *(const uint4*)(s_slotG + 4 * piece); });
+                if (rtid == 0) {
                     double t4[4] = { 0.0, 0.0, 0.0, 0.0 };
 #pragma unroll
                     for (int i = 0; i < NWARPS; ++i) t4[i & 3] += red_d(x)[i];
                     const double tot = (t4[0] + t4[1]) + (t4[2] + t4[3]);
-                    const uint32_t lo = (uint32_t)__double2loint(tot), hi = (uint32_t)__double2hiint(tot);
-                    if (ex == 0) { w.x = lo; w.y = hi; } else { w.z = lo; w.w = hi; }
+                    partial_store(x, rec, P.x_PG, (uint32_t)__double2loint(tot), (uint32_t)__double2hiint(tot));
                 }
-                return w;
-            });
+                x.stamp(l, 27);
+                if (tid == DMA_TID && nch > 0) {   // write the state slice back (async), while the exchange goes on
+                    bulk_s2g_stream(P.ssm + (size_t)l * P.ssm_lstride + (size_t)ch0 * x.d_state(), stage + P.st_ssm, (uint32_t)nch * x.d_state() * 4,
+                                    policy_evict_first());
+                    bulk_s2g(conv_l + (size_t)ch0 * 4, stage + P.st_conv, (uint32_t)nch * 16);
+                    bulk_commit();
+                }
+            }
+            DFSSM_STAMP(l, 5);
+
+            // ---- gather G, S6 absmax + quantise of the whole gated vector in every CTA ----
+            int qsum_g;
+            {
+                uint4 vg[NJ_G];
+                hop_gather<NJ_G>(x, rec + P.x_G, NW * x.g_slot(), vg, tid, DFSSM_WG);
+                DFSSM_STAMP(l, 6);
+                qsum_g = absmax_quant(x, SlotEnum<NJ_G>{ vg, chs, tid, NW, x.g_slot() >> 2 }, x.d_inner(), false,
+                                      (tp && c == 0) ? (int8_t*)(tp + P.tl.off[9]) : nullptr, l, 16);
+            }
+            DFSSM_STAMP(l, 7);
+            // ---- S7: warp 0 makes the scale of the gated codes; the other warps do the out_proj sign rows ----
+            if (wid == 0) {
+                scale_side(x, rec + P.x_PG, x.d_inner(), 2, (tp && c == 0) ? (float*)(tp + P.tl.off[10]) : nullptr);
+            } else {
+                const uint32_t* bits = (const uint32_t*)(stage + P.c_out_bits);
+                const int npair = (nor + 1) >> 1, wspan = x.Wout() / KS;
+                for (int id = wid - 1; id < npair * KS; id += NWARPS - 1) {
+                    const int pair = id / KS, half = id - pair * KS;
+                    const int nrows = min(2, nor - 2 * pair);
+                    const uint32_t* const rowp[2] = { bits + (size_t)(2 * pair) * x.Wout(), bits + (size_t)(2 * pair + (nrows > 1 ? 1 : 0)) * x.Wout() };
+                    int p[2];
+                    sign_partial<2>(rowp, nrows, half * wspan, half == KS - 1 ? x.Wout() : (half + 1) * wspan, xq, x.d_inner(), lane, p);
+                    const int v = reduce2(p, lane);
+                    const int r = lane >> 4;
+                    if ((lane & 15) == 0 && r < nrows) s_acc_out[half * x.nor_max() + 2 * pair + r] = v;
+                }
+            }
+            DFSSM_STAMP(l, 8);
+            // ---- gather T: t_out = sum of the partial sums;  v_j = a_s[j] * float(t_j) ----
+            {
+                uint4 vt[1];
+                hop_gather<1>(x, rec + mbox(M_T) + P.x_T, x.n_ttask(), vt, rtid);
+                if (rtid < (x.n_ttask() + 3) / 4) {
+                    const float* a_s = (const float*)(blk + P.b_as_out);
+                    const uint32_t w[4] = { vt[0].x, vt[0].y, vt[0].z, vt[0].w };
+                    const int rows_per_chunk = 4 / x.tsplit();
+#pragma unroll
+                    for (int jj = 0; jj < 4; ++jj) {
+                        const int j = rtid * rows_per_chunk + jj;
+                        if (jj < rows_per_chunk && j < x.r()) {
+                            int t = 0;
+                            for (int q = 0; q < x.tsplit(); ++q) t += (int)(w[jj * x.tsplit() + q] ^ IBIAS);
+                            s_vout[j] = (double)fmul(a_s[j], (float)t);
+                            if (tp && c == 0) ((int32_t*)(tp + P.tl.off[12]))[j] = t;
+                        }
+                    }
+                }
+            }
+            __syncthreads();
+            DFSSM_STAMP(l, 9);
+            const float s_g = scal(x)[2];
+            // ---- S7 epilogue + residual; t = u*w of the next norm is published as it is produced ----
+            {
+                double ss_u = 0.0;
+                const int8_t* Bm = (const int8_t*)(stage + P.c_out_B);
+                const float* scale = (const float*)(stage + P.c_out_scale);
+                const float* bsv = (const float*)(stage + P.c_out_bs);
+                const float* nw = (const float*)(stage + P.c_nnorm);
+                for (int ib = 0; ib < nor; ib += THREADS / 4) {
+                    const int i = ib + (tid >> 2), sub = tid & 3;
+                    const bool valid = i < nor;
+                    double lo = 0.0;
+                    const int8_t* brow = Bm + (size_t)(valid ? i : 0) * x.r_pad();
+                    if (valid)
+                        for (int j = sub; j < x.r(); j += 4) lo = __fma_rn(i2d((int)brow[j]), s_vout[j], lo);
+                    lo += __shfl_xor_sync(0xffffffffu, lo, 1);
+                    lo += __shfl_xor_sync(0xffffffffu, lo, 2);
+                    if (sub != 0 || !valid) continue;
+                    int p128 = s_acc_out[i];
+                    for (int hh = 1; hh < KS; ++hh) p128 += s_acc_out[hh * x.nor_max() + i];
+                    const int acc = 2 * (p128 / 128) - qsum_g;       // exact: every term is a multiple of 128
+                    const float o = fmul(s_g, fadd(fmul(scale[i], (float)acc), fmul(bsv[i], (float)lo)));
+                    const float un = fadd(s_u[i], o);
+                    s_u[i] = un;
+                    s_slotU[i] = __float_as_uint(fmul(un, nw[i]));
+                    ss_u = dacc(ss_u, un, un);
+                    if (tp) { ((float*)(tp + P.tl.off[13]))[or0 + i] = un; ((int32_t*)(tp + P.tl.off[11]))[or0 + i] = acc; }
+                }
+                ss_u = warp_sum_strided(ss_u, 4);           // only every fourth lane holds a value
+                if (lane == 0) red_d(x)[wid] = ss_u;
+                __syncthreads();                        // also: every thread is done with this stage's weights
+                slot_store(x, rec, P.x_U, x.u_slot(), [&](int piece) { return *(const uint4*)(s_slotU + 4 * piece); });
+                if (rtid == 0) {
+                    double t4[4] = { 0.0, 0.0, 0.0, 0.0 };
+#pragma unroll
+                    for (int i = 0; i < NWARPS; ++i) t4[i & 3] += red_d(x)[i];
+                    const double tot = (t4[0] + t4[1]) + (t4[2] + t4[3]);
+                    partial_store(x, rec, P.x_PU, (uint32_t)__double2loint(tot), (uint32_t)__double2hiint(tot));
+                }
+            }
+            DFSSM_STAMP(l, 10);
         }
-        DFSSM_STAMP(l, 10);
         // ---- gather U, S1 of the next layer (or S8's norm) in every CTA ----
         {
             uint4 vu[NJ_U];
-            hop_gather<NJ_U>(x, rec + mbox(M_U) + P.x_U, x.G() * x.u_slot(), x.u_slot(), x.u_dpos(), vu, tid, DFSSM_WU);
+            hop_gather<NJ_U>(x, rec + P.x_U, NW * x.u_slot(), vu, tid, service ? 0 : DFSSM_WU);
             DFSSM_STAMP(l, 11);
-            const double ssl = slot_partials<NJ_U>(x, vu, x.G(), x.u_slot(), x.u_dpos());
             uint8_t* tpn = (taps_on && c == 0 && l + 1 < P.L) ? P.taps + (size_t)(l + 1) * P.tap_lstride : nullptr;
-            const int upps = x.u_slot() >> 2;
-            qsum = norm_quant(x, SlotEnum<NJ_U>{ vu, ors, tid, x.G(), upps }, ssl, upps < 32 ? upps : 1, upps < 32 ? (x.u_dpos() >> 2) % upps : 0,
-                              x.d_model(), l == P.L - 1, s_act,
-                              tpn ? (int8_t*)(tpn + P.tl.off[0]) : nullptr, l, 20);
-            if (tpn && tid == 0) *(float*)(tpn + P.tl.off[1]) = s_act;
+            qsum = absmax_quant(x, SlotEnum<NJ_U>{ vu, ors, tid, NW, x.u_slot() >> 2 }, x.d_model(), l == P.L - 1,
+                                tpn ? (int8_t*)(tpn + P.tl.off[0]) : nullptr, l, 20);
         }
         // ---- refill this layer's ring stage with the item `stages` ahead: after the gather, so that the bulk copies do
         //      not sit in front of its polls in the memory pipeline ----
@@ -1062,6 +1141,12 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
     }
 
     // =============================================== S8 LM head ===============================================
+    if (P.L > 0) {      // scale of the final codes from the U partials of the last layer (L == 0: made with the embedding)
+        uint32_t* recl = P.xbuf + ((size_t)P.set * P.L + (P.L - 1)) * rec_words;
+        if (wid == 0) scale_side(x, recl + P.x_PU, x.d_model(), 1, nullptr);
+        __syncthreads();
+    }
+    const float s_act = scal(x)[1];
     for (int i = tid; i < nor; i += THREADS) P.u_out[or0 + i] = s_u[i];
     DFSSM_STAMP(P.L, 0);
     if (x.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + P.L) * PROF_NPH + 31] = globaltimer_ns();

@@ -14,6 +14,20 @@ constexpr size_t SMEM_LIMIT = 232448 - 1024;    // 227 KB opt-in maximum minus t
 
 inline uint32_t up32(uint32_t x, uint32_t a) { return (x + a - 1) / a * a; }
 
+// workers of a shape: 128 whenever that deals whole groups of 4 to every worker (all BASELINE shapes), else the count in
+// [116, 132] with the least sign-row work on the busiest worker
+inline int pick_workers(const Dims& d)
+{
+    if ((d.d_inner / 4) % NW_CT == 0 || d.d_inner / 4 < NW_CT) return NW_CT;
+    int best = NW_CT;
+    long long best_cost = -1;
+    for (int nw = 132; nw >= 116; nw -= 4) {
+        const long long cost = (long long)own_max(d.d_inner, nw) * 2 * (d.d_model / 32) + (long long)own_max(d.d_model, nw) * (d.d_inner / 32);
+        if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = nw; }
+    }
+    return best;
+}
+
 // Fills every shape / layout field of P (no pointers).  Returns false if the shape does not fit the
 // mega path (the chain path then serves it).
 inline bool plan(const Dims& d, int G, Params& P)
@@ -25,24 +39,28 @@ inline bool plan(const Dims& d, int G, Params& P)
     P.n_bcdt = 2 * P.gs + d.nheads;
     P.eps = d.eps;
     P.G = G;
-    if (d.d_state % 4 || d.d_model % 32 || d.d_inner % 32 || d.r > 64 || (G & 1)) return false;
+    if (G != GRID) return false;
+    if (d.d_state % 4 || d.d_model % 32 || d.d_inner % 32 || d.r > 64) return false;
     if (d.d_model > 8192 || d.d_inner > 8192) return false;
-    P.nch_max = own_max(d.d_inner);
-    P.nor_max = own_max(d.d_model);
-    P.nb_max = (P.n_bcdt + G - 1) / G;
-    P.n_slots = 2 * P.nch_max + P.nb_max;
+    P.NW = pick_workers(d);
+    P.NS = G - P.NW;
+    P.nch_max = own_max(d.d_inner, P.NW);
+    P.nor_max = own_max(d.d_model, P.NW);
     P.r_pad = (d.r + 3) / 4 * 4;
     P.Win = d.d_model / 32;
     P.Wout = d.d_inner / 32;
     P.n_early = P.n_bcdt + d.r;
-    if (P.n_early > 4096 || P.n_early > 64 * G || d.r > G) return false;
-    P.tsplit = (d.d_inner % 64 == 0 && 4 * d.r <= G) ? 4 : (2 * d.r <= G ? 2 : 1);
+    if (P.n_early > NJ_A * THREADS * 4) return false;
+    P.tsplit = d.d_inner % 64 == 0 ? 4 : 2;
     P.n_ttask = d.r * P.tsplit;
     if (P.nch_max > 128 || P.nor_max > 128 || d.d_inner < 4 || d.d_model < 4) return false;
+    P.ns_sig = dealt(P.n_bcdt, 0, P.NS);
+    P.ns_lin = dealt(d.r, 0, P.NS);
+    P.ns_tt = dealt(P.n_ttask, 0, P.NS);
 
     uint32_t off = 0;
     auto take = [&](size_t bytes) { off = up32(off, 16); const uint32_t at = off; off += (uint32_t)bytes; return at; };
-    P.c_in_bits = take((size_t)P.n_slots * P.Win * 4);
+    P.c_in_bits = take((size_t)2 * P.nch_max * P.Win * 4);
     P.c_out_bits = take((size_t)P.nor_max * P.Wout * 4);
     P.c_in_B = take((size_t)2 * P.nch_max * P.r_pad);
     P.c_out_B = take((size_t)P.nor_max * P.r_pad);
@@ -59,6 +77,12 @@ inline bool plan(const Dims& d, int G, Params& P)
     P.chunk_bytes = up32(off, 128);
 
     off = 0;
+    P.sc_sign = take((size_t)P.ns_sig * P.Win * 4);
+    P.sc_tin = take((size_t)P.ns_lin * d.d_model);
+    P.sc_tout = take((size_t)P.ns_tt * (d.d_inner / P.tsplit));
+    P.schunk_bytes = up32(off, 128);
+
+    off = 0;
     P.b_eB = take((size_t)P.n_bcdt * P.r_pad);
     P.b_escale = take((size_t)P.n_bcdt * 4);
     P.b_ebs = take((size_t)P.n_bcdt * 4);
@@ -73,39 +97,37 @@ inline bool plan(const Dims& d, int G, Params& P)
     P.st_ssm = P.st_blk + P.blk_bytes;
     P.st_conv = up32(P.st_ssm + (uint32_t)P.nch_max * d.d_state * 4, 128);
     P.st_econv = up32(P.st_conv + (uint32_t)P.nch_max * 16, 128);
-    P.st_tin = up32(P.st_econv + (uint32_t)P.gs * 32, 128);
-    P.st_tout = up32(P.st_tin + (uint32_t)d.d_model, 128);
-    P.stage_bytes = up32(P.st_tout + (uint32_t)(d.d_inner / P.tsplit), 128);
+    P.stage_bytes = up32(P.st_econv + (uint32_t)P.gs * 32, 128);
+    if (P.stage_bytes < P.schunk_bytes) P.stage_bytes = P.schunk_bytes;
     if (P.stage_bytes < 4u * d.d_model) P.stage_bytes = up32(4u * d.d_model, 128);      // an LM item holds >= 4 rows
     P.lm_rows_item = (int)(P.stage_bytes / d.d_model);
 
-    // exchange: one (record, mailbox) part list, 32-bit word offsets, every part 128-byte aligned
-    if (G != GRID) return false;
-    P.M = MBOX;
-    P.gsz = G / P.M;
-    P.u_dpos = (P.nor_max + 1) / 2 * 2;
-    P.u_slot = slot_words(P.u_dpos + 2);
-    P.g_dpos = (P.nch_max + 1) / 2 * 2;
-    P.g_slot = slot_words(P.g_dpos + 2);
-    if (G * P.u_slot / 4 > NJ_MAX * THREADS || G * P.g_slot / 4 > NJ_MAX * THREADS) return false;
+    // exchange: part lists of a record's main part and of one small mailbox, 32-bit word offsets, every part 128-byte aligned
+    P.u_slot = slot_words(P.nor_max);
+    P.g_slot = slot_words(P.nch_max);
+    if (P.NW * P.u_slot / 4 > NJ_MAX * THREADS || P.NW * P.g_slot / 4 > NJ_MAX * THREADS) return false;
     if (P.u_slot + P.g_slot > THREADS) return false;
     uint32_t xo = 0;
     auto xtake = [&](size_t words) { xo = up32(xo, 32); const uint32_t at = xo; xo += (uint32_t)words; return at; };
-    P.x_U = xtake((size_t)G * P.u_slot);
+    P.x_U = xtake((size_t)P.NW * P.u_slot);
+    P.x_PU = xtake((size_t)2 * P.NW);
+    P.x_G = xtake((size_t)P.NW * P.g_slot);
+    P.x_PG = xtake((size_t)2 * P.NW);
+    P.x_main = up32(xo, 32);
+    xo = 0;
     P.x_A = xtake(P.n_early);
-    P.x_G = xtake((size_t)G * P.g_slot);
     P.x_T = xtake(P.n_ttask);
-    P.x_words = up32(xo, 32);
+    P.x_small = up32(xo, 32);
 
     // shared memory behind the ring
     uint32_t so = 0;
     auto stake = [&](size_t bytes) { so = up32(so, 16); const uint32_t at = so; so += (uint32_t)bytes; return at; };
     const int kmax = d.d_model > d.d_inner ? d.d_model : d.d_inner;
-    const uint32_t x_xq = stake(kmax), x_bc = stake((size_t)2 * P.gs * 4), x_u = stake((size_t)P.nor_max * 4),
+    const uint32_t x_xq = stake(kmax), x_bc = stake((size_t)P.gs * 4), x_cd = stake((size_t)P.gs * 8), x_u = stake((size_t)P.nor_max * 4),
                    x_z = stake((size_t)P.nch_max * 4), x_x = stake((size_t)P.nch_max * 4), x_dt = stake((size_t)d.nheads * 4),
-                   x_v = stake((size_t)2 * P.r_pad * 8), x_ea = stake((size_t)P.n_bcdt * 4), x_ai = stake((size_t)P.n_slots * 4),
+                   x_v = stake((size_t)2 * P.r_pad * 8), x_ea = stake((size_t)P.n_bcdt * 4), x_ai = stake((size_t)2 * P.nch_max * 4),
                    x_ao = stake((size_t)KS_MAX * P.nor_max * 4), x_chs = stake((size_t)(G + 1) * 4), x_ors = stake((size_t)(G + 1) * 4),
-                   x_part = stake((size_t)(G + 2) * 8), x_red = stake(16 * NWARPS), x_slot = stake((size_t)(P.u_slot + P.g_slot) * 4),
+                   x_red = stake(16 * NWARPS), x_slot = stake((size_t)(P.u_slot + P.g_slot) * 4), x_scal = stake(16),
                    x_mbar = stake(8 * MAX_STAGES);
     const uint32_t fixed = up32(so, 128);
     if (fixed + 2 * (size_t)P.stage_bytes > SMEM_LIMIT) return false;
@@ -114,26 +136,26 @@ inline bool plan(const Dims& d, int G, Params& P)
     P.stages = stages;
     const uint32_t ring = (uint32_t)stages * P.stage_bytes;
     P.s_ring = 0;
-    P.s_xq = ring + x_xq; P.s_bc = ring + x_bc; P.s_u = ring + x_u; P.s_z = ring + x_z; P.s_x = ring + x_x; P.s_dt = ring + x_dt;
+    P.s_xq = ring + x_xq; P.s_bc = ring + x_bc; P.s_cd = ring + x_cd; P.s_u = ring + x_u; P.s_z = ring + x_z; P.s_x = ring + x_x; P.s_dt = ring + x_dt;
     P.s_v = ring + x_v; P.s_eacc = ring + x_ea; P.s_acc_in = ring + x_ai; P.s_acc_out = ring + x_ao;
-    P.s_chs = ring + x_chs; P.s_ors = ring + x_ors; P.s_part = ring + x_part; P.s_red = ring + x_red; P.s_slot = ring + x_slot; P.s_mbar = ring + x_mbar;
+    P.s_chs = ring + x_chs; P.s_ors = ring + x_ors; P.s_red = ring + x_red; P.s_slot = ring + x_slot; P.s_scal = ring + x_scal;
+    P.s_mbar = ring + x_mbar;
     P.smem_bytes = ring + fixed;
     return true;
 }
 
 // arena regions of the mega path (byte sizes)
 struct Regions {
-    size_t chunks, blocks, A_in, A_out, xbuf, am;
+    size_t chunks, schunks, blocks, xbuf, am;
 };
 inline Regions regions(const Params& P)
 {
     Regions r;
     const size_t nl = (size_t)(P.L > 0 ? P.L : 1);
-    r.chunks = nl * P.G * P.chunk_bytes;
+    r.chunks = nl * P.NW * P.chunk_bytes;
+    r.schunks = nl * P.NS * P.schunk_bytes;
     r.blocks = nl * P.blk_bytes;
-    r.A_in = nl * P.r * P.d_model;
-    r.A_out = nl * P.r * P.d_inner;
-    r.xbuf = (size_t)4 * P.M * P.x_words * 4;       // four rotating records of M mailboxes
+    r.xbuf = (size_t)2 * nl * ((size_t)P.x_main + (size_t)MBOX * P.x_small) * 4;      // 2 sets x L records
     r.am = (size_t)P.G * 8 + 64;
     return r;
 }
@@ -198,13 +220,12 @@ struct HostLayer {
     const int8_t* out_A; const float* out_a_s; const int8_t* out_B; const float* out_b_s;
 };
 
-// chunk of (layer, CTA c): `next_norm_w` is the norm weight applied to u after this layer
+// chunk of (layer, worker c): `next_norm_w` is the norm weight applied to u after this layer
 inline void pack_chunk(const Params& P, const HostLayer& H, const float* next_norm_w, int c, uint8_t* out)
 {
     memset(out, 0, P.chunk_bytes);
-    const int G = P.G;
-    const int ch0 = own_start(c, P.d_inner), nch = own_start(c + 1, P.d_inner) - ch0;
-    const int or0 = own_start(c, P.d_model), nor = own_start(c + 1, P.d_model) - or0;
+    const int ch0 = own_start(c, P.d_inner, P.NW), nch = own_start(c + 1, P.d_inner, P.NW) - ch0;
+    const int or0 = own_start(c, P.d_model, P.NW), nor = own_start(c + 1, P.d_model, P.NW) - or0;
     auto put_in_row = [&](int slot, int row) {
         copy_sign_row((uint32_t*)(out + P.c_in_bits + (size_t)slot * P.Win * 4), H.in_sign + (size_t)row * P.Win, P.Win);
         memcpy(out + P.c_in_B + (size_t)slot * P.r_pad, H.in_B + (size_t)row * P.r, P.r);
@@ -221,8 +242,6 @@ inline void pack_chunk(const Params& P, const HostLayer& H, const float* next_no
         ((float*)(out + P.c_D))[i] = H.D[h];
         ((float*)(out + P.c_gnorm))[i] = H.gnorm_w[ch];
     }
-    for (int k = 0, e = c; e < P.n_bcdt; ++k, e += G)        // early sign rows: B | C | dt (their epilogue data is in the block)
-        copy_sign_row((uint32_t*)(out + P.c_in_bits + (size_t)(2 * P.nch_max + k) * P.Win * 4), H.in_sign + (size_t)(2 * P.d_inner + e) * P.Win, P.Win);
     for (int i = 0; i < nor; ++i) {
         const int row = or0 + i;
         copy_sign_row((uint32_t*)(out + P.c_out_bits + (size_t)i * P.Wout * 4), H.out_sign + (size_t)row * P.Wout, P.Wout);
@@ -230,6 +249,28 @@ inline void pack_chunk(const Params& P, const HostLayer& H, const float* next_no
         ((float*)(out + P.c_out_scale))[i] = half_bits_to_float(H.out_row_scale[row]);
         ((float*)(out + P.c_out_bs))[i] = H.out_b_s[row];
         ((float*)(out + P.c_nnorm))[i] = next_norm_w[row];
+    }
+}
+
+inline void permute_row(const int8_t* A, int K, int8_t* out)
+{
+    for (int k = 0; k < K; ++k) out[plane_pos_host(k, K)] = A[k];
+}
+
+// chunk of (layer, service CTA s): the B|C|dt sign rows s, s + NS, ..., the in_proj LoRA-down rows s, s + NS, ... and the
+// out_proj LoRA-down partial tasks s, s + NS, ... (task q = row q / tsplit, part q % tsplit of the plane-permuted row)
+inline void pack_schunk(const Params& P, const HostLayer& H, int s, uint8_t* out, std::vector<int8_t>& tmp)
+{
+    memset(out, 0, P.schunk_bytes);
+    for (int k = 0, e = s; e < P.n_bcdt; ++k, e += P.NS)
+        copy_sign_row((uint32_t*)(out + P.sc_sign + (size_t)k * P.Win * 4), H.in_sign + (size_t)(2 * P.d_inner + e) * P.Win, P.Win);
+    for (int k = 0, j = s; j < P.r; ++k, j += P.NS)
+        permute_row(H.in_A + (size_t)j * P.d_model, P.d_model, (int8_t*)(out + P.sc_tin + (size_t)k * P.d_model));
+    const int tbytes = P.d_inner / P.tsplit;
+    tmp.resize((size_t)P.d_inner);
+    for (int k = 0, q = s; q < P.n_ttask; ++k, q += P.NS) {
+        permute_row(H.out_A + (size_t)(q / P.tsplit) * P.d_inner, P.d_inner, tmp.data());
+        memcpy(out + P.sc_tout + (size_t)k * tbytes, tmp.data() + (size_t)(q % P.tsplit) * tbytes, tbytes);
     }
 }
 
@@ -259,20 +300,14 @@ inline void pack_block(const Params& P, const HostLayer& H, uint8_t* out)
     }
 }
 
-inline void permute_A(const int8_t* A, int r, int K, int8_t* out)
-{
-    for (int j = 0; j < r; ++j)
-        for (int k = 0; k < K; ++k) out[(size_t)j * K + plane_pos_host(k, K)] = A[(size_t)j * K + k];
-}
-
 }  // namespace mega
 }  // namespace dfssm
 
 namespace dfssm {
 namespace mega {
 
-// the shapes of BASELINE.json's configs get a kernel with compile-time dimensions; taps or any other shape use
-// the run-time-shape kernel
+// the shapes of BASELINE.json's configs get a kernel with compile-time dimensions; any other shape uses the run-time-shape
+// kernel (with the taps / profiler code compiled in only when asked for)
 using Shape0 = ShapeCT<256, 512, 64, 64, 1, 8>;
 using Shape1 = ShapeCT<768, 1536, 64, 128, 1, 16>;
 using Shape2 = ShapeCT<2048, 4096, 64, 128, 1, 32>;
@@ -294,7 +329,8 @@ inline KernelFn pick_kernel(const Dims& d, bool taps, bool prof)
         if (shape_is<Shape2>(d)) return prof ? k_mega<Shape2, false, true> : k_mega<Shape2, false, false>;
         if (shape_is<Shape4>(d)) return prof ? k_mega<Shape4, false, true> : k_mega<Shape4, false, false>;
     }
-    return k_mega<ShapeRT, true, true>;
+    if (taps || prof) return k_mega<ShapeRT, true, true>;
+    return k_mega<ShapeRT, false, false>;
 }
 
 }  // namespace mega
