@@ -444,6 +444,18 @@ int mega_setup(dfssm_ctx* ctx)                      // at create: can this devic
     return DFSSM_OK;
 }
 
+// the exchange records of the persistent kernel: everything "not written" (at load, and after a step that was aborted by a
+// poll time-out and left half-written records behind)
+int mega_init_x(dfssm_ctx* ctx)
+{
+    const mega::Params& P = ctx->mp;
+    const size_t nrec = 2 * (size_t)(P.L > 0 ? P.L : 1);
+    mega::k_mega_init_x<<<592, 256, 0, ctx->stream>>>((uint32_t*)(ctx->arena + ctx->cv.m_x), nrec, P.x_main, P.x_small, P.x_A, P.n_early + 1,
+                                                      P.x_T, P.n_ttask, (P.n_ttask + 3) / 4 * 4, (P.n_ttask + 3) / 4 * 4 + 4);
+    CK(cudaGetLastError());
+    return DFSSM_OK;
+}
+
 // at load: repack the canonical blob into per-(layer, CTA) chunks and plane-ordered LoRA-down rows
 int mega_load(dfssm_ctx* ctx, const std::vector<mega::HostLayer>& HL, const float* normf_w)
 {
@@ -452,12 +464,12 @@ int mega_load(dfssm_ctx* ctx, const std::vector<mega::HostLayer>& HL, const floa
     const Carve& v = ctx->cv;
     const Dims& d = ctx->dm;
     {
-        std::vector<uint8_t> buf((size_t)P.NW * P.chunk_bytes), sbuf((size_t)P.NS * P.schunk_bytes);
+        std::vector<uint8_t> buf((size_t)P.NW * P.chunk_bytes), sbuf((size_t)P.NT * P.schunk_bytes);
         std::vector<int8_t> tmp;
         for (int l = 0; l < d.n_layers; ++l) {
             const float* nn = l + 1 < d.n_layers ? HL[l + 1].norm_w : normf_w;
             for (int c = 0; c < P.NW; ++c) mega::pack_chunk(P, HL[l], nn, c, buf.data() + (size_t)c * P.chunk_bytes);
-            for (int s = 0; s < P.NS; ++s) mega::pack_schunk(P, HL[l], s, sbuf.data() + (size_t)s * P.schunk_bytes, tmp);
+            for (int s = 0; s < P.NT; ++s) mega::pack_schunk(P, HL[l], s, sbuf.data() + (size_t)s * P.schunk_bytes, tmp);
             CK(cudaMemcpyAsync(ctx->arena + v.m_chunks + (size_t)l * buf.size(), buf.data(), buf.size(), cudaMemcpyHostToDevice, ctx->stream));
             CK(cudaMemcpyAsync(ctx->arena + v.m_schunks + (size_t)l * sbuf.size(), sbuf.data(), sbuf.size(), cudaMemcpyHostToDevice, ctx->stream));
             CK(cudaStreamSynchronize(ctx->stream));
@@ -476,8 +488,8 @@ int mega_load(dfssm_ctx* ctx, const std::vector<mega::HostLayer>& HL, const floa
             CK(cudaMemcpyAsync(ctx->arena + v.m_blocks + (size_t)l * buf.size(), buf.data(), buf.size(), cudaMemcpyHostToDevice, ctx->stream));
             CK(cudaStreamSynchronize(ctx->stream));
         }
-        // every exchange word starts as "not written" (mega::SENT)
-        CK(cudaMemsetAsync(ctx->arena + v.m_x, 0xff, v.m_xbytes, ctx->stream));
+        const int rc = mega_init_x(ctx);        // every exchange word starts as "not written"
+        if (rc != DFSSM_OK) return rc;
     }
     // pointers
     const size_t B = ctx->cfg.max_batch;
@@ -658,7 +670,10 @@ int dfssm_reset_state(dfssm_ctx* ctx, int seq)
         CK(cudaMemsetAsync(ctx->arena + v.conv, 0, nl * B * (size_t)d.conv_dim * 16, ctx->stream));
         // the exchange records of the persistent kernel go back to "nothing written" too (matters only after a step that
         // was aborted by a poll time-out and left half-written records behind)
-        if (v.mega_fit) CK(cudaMemsetAsync(ctx->arena + v.m_x, 0xff, v.m_xbytes, ctx->stream));
+        if (v.mega_fit && ctx->loaded) {
+            const int rc = mega_init_x(ctx);
+            if (rc != DFSSM_OK) return rc;
+        }
         return DFSSM_OK;
     }
     // one sequence of every layer: strided 2-D memsets (rows = layers)

@@ -65,6 +65,7 @@ constexpr int NJ_A = 1024 / THREADS;          // ... when gathering A
 constexpr int NR_IN = THREADS >= 1024 ? 2 : 4;     // in_proj sign rows per warp pass
 constexpr int LPC = THREADS / 32;             // lanes per channel in the state update (32 channels per pass)
 constexpr int LPB = THREADS / 512;            // lanes per B|C row in the in_proj epilogue
+constexpr int SCALE_WARP = 2;                 // the warp of service CTA 0 that makes the activation scales (it has one early task, not two)
 constexpr int DMA_TID = 96;                   // the thread that issues the state write-back and the ring refills (a warp off the publish paths)
 constexpr int KS_MAX = 4;                     // largest K-split of the out_proj sign rows
 constexpr int MAX_STAGES = 8;
@@ -75,31 +76,31 @@ constexpr int PROF_NPH = 32;                  // phase stamps per (CTA, layer) o
 
 constexpr int GRID = 148;                     // one CTA per B200 SM
 constexpr int NW_CT = 128;                    // workers of the compile-time-shape kernels (the rest are service CTAs)
-constexpr int MBOX = 37;                      // mailboxes allocated per record
 
 // mailboxes of the small parts A and T (each must divide GRID and be <= MBOX): the payload is pushed M times and GRID / M
 // workers poll each copy (polls that reach a line before the data delay the stores to it).  U and G have one copy.
 #ifndef DFSSM_MA
-#define DFSSM_MA 37
+#define DFSSM_MA 1
 #endif
 #ifndef DFSSM_MT
-#define DFSSM_MT 37
+#define DFSSM_MT 1
 #endif
 // clocks a worker waits after publishing G / U before its first poll: polls that reach a line before the data delay the
 // stores to it
 #ifndef DFSSM_WG
-#define DFSSM_WG 500
+#define DFSSM_WG 250
 #endif
 #ifndef DFSSM_WU
-#define DFSSM_WU 500
+#define DFSSM_WU 250
 #endif
+constexpr int MBOX = DFSSM_MA > DFSSM_MT ? DFSSM_MA : DFSSM_MT;      // small mailboxes allocated per record
 constexpr int M_A = DFSSM_MA, M_T = DFSSM_MT;
 
 struct Params {
     // ---- shape ----
     int L, d_model, d_inner, headdim, d_state, ngroups, nheads, r, vocab, n_bcdt, gs;
     float eps;
-    int G, NW, NS;               // grid size (all co-resident), workers, service CTAs
+    int G, NW, NS, NT;           // grid size (all co-resident), workers, service CTAs, of which NT = NS - 1 hold row tasks
     int nch_max, nor_max, r_pad;
     int Win, Wout;               // sign words per row of in_proj / out_proj
     int n_early;                 // service results of in_proj: n_bcdt sign rows + r LoRA-down rows
@@ -124,7 +125,7 @@ struct Params {
         s_red, s_slot, s_scal, smem_bytes;
     // ---- device pointers ----
     const uint8_t* chunks;       // [L][NW][chunk_bytes]
-    const uint8_t* schunks;      // [L][NS][schunk_bytes]
+    const uint8_t* schunks;      // [L][NT][schunk_bytes]
     const uint8_t* blocks;       // [L][blk_bytes]
     float* ssm;                  // sequence 0 of layer 0; layer stride ssm_lstride floats
     float* conv;                 // [conv_dim][4] ring of sequence 0 of layer 0; layer stride conv_lstride floats
@@ -280,6 +281,10 @@ struct Ctx {
     __device__ __forceinline__ int n_early() const { return n_bcdt() + r(); }
     __device__ __forceinline__ int tsplit() const { return d_inner() % 64 == 0 ? 4 : 2; }
     __device__ __forceinline__ int n_ttask() const { return r() * tsplit(); }
+    // words of the A / T part: the service results plus the activation scale(s) made by service CTA 0
+    __device__ __forceinline__ int n_A() const { return n_early() + 1; }          // [n_early]: scale of this layer's in_proj codes
+    __device__ __forceinline__ int i_sg() const { return (n_ttask() + 3) / 4 * 4; }   // T word: scale of this layer's out_proj codes (own chunk)
+    __device__ __forceinline__ int i_slm() const { return i_sg() + 4; }               // T word: scale of the LM-head codes (last layer only; own chunk)
     __device__ __forceinline__ int u_slot() const { return slot_words(nor_max()); }
     __device__ __forceinline__ int g_slot() const { return slot_words(nch_max()); }
 };
@@ -307,14 +312,16 @@ __device__ __forceinline__ constexpr int mbox_count(int n, int M) { return (n + 
 // ------------------------------------------------------------------------------------------------
 // exchange: gather a self-validating buffer
 // ------------------------------------------------------------------------------------------------
-// Thread t owns the 16-byte chunks t, t + THREADS, ... (at most NJ) of the nw 32-bit words at buf.  Words
-// behind nw count as valid.  Spins until every owned word has been written; the raw words come back in v[].
-// tix = the thread's index for the chunk ownership (tid, or reversed so that the small gathers are polled by the
-// warps that have nothing else to do).
+// a 16-byte chunk is complete when none of its four words is the sentinel (every part is padded to whole chunks and
+// pad words hold 0 from load time on)
+__device__ __forceinline__ bool chunk_ok(uint4 v) { return max(max(v.x, v.y), max(v.z, v.w)) != SENT; }
+
+// Thread t owns the 16-byte chunks t, t + THREADS, ... (at most NJ) of the nchunk chunks at buf.  Spins until every owned
+// word has been written; the raw words come back in v[].  tix = the thread's index for the chunk ownership (tid, or
+// reversed so that the small gathers are polled by the warps that have nothing else to do).
 template <int NJ, class S>
-__device__ __forceinline__ void hop_gather(const Ctx<S>& x, const uint32_t* buf, int nw, uint4 (&v)[NJ], int tix, int first_wait = 0)
+__device__ __forceinline__ void hop_gather(const Ctx<S>& x, const uint32_t* buf, int nchunk, uint4 (&v)[NJ], int tix, int first_wait = 0)
 {
-    const int nchunk = (nw + 3) >> 2;
     bool need[NJ];
     bool any = false;
 #pragma unroll
@@ -332,62 +339,43 @@ __device__ __forceinline__ void hop_gather(const Ctx<S>& x, const uint32_t* buf,
         bool all = true;
 #pragma unroll
         for (int j = 0; j < NJ; ++j)
-            if (need[j]) {
-                const int base = 4 * (tix + j * THREADS);
-                const bool ok = v[j].x != SENT && (base + 1 >= nw || v[j].y != SENT) && (base + 2 >= nw || v[j].z != SENT) &&
-                                (base + 3 >= nw || v[j].w != SENT);
-                need[j] = !ok;
-                all = all && ok;
-            }
+            if (need[j]) { need[j] = !chunk_ok(v[j]); all = all && !need[j]; }
         if (all) break;
         if (++spins > SPIN_LIMIT || *x.dead) { poll_fail(x); break; }
     }
 }
 
-// scratch inside s_red: NWARPS floats (warp maxima) | NWARPS ints (warp code sums) | NWARPS doubles (warp sums)
+// scratch inside s_red: NWARPS doubles (warp sums of squares)
 template <class S>
-__device__ __forceinline__ float* red_f(const Ctx<S>& x) { return (float*)(x.sm + x.P.s_red); }
-template <class S>
-__device__ __forceinline__ int* red_i(const Ctx<S>& x) { return (int*)(x.sm + x.P.s_red) + NWARPS; }
-template <class S>
-__device__ __forceinline__ double* red_d(const Ctx<S>& x) { return (double*)(x.sm + x.P.s_red + 8 * NWARPS); }
-// scalars: [0] amax of the last norm_quant, [1] scale of the in_proj / LM-head codes, [2] scale of the out_proj codes
+__device__ __forceinline__ double* red_d(const Ctx<S>& x) { return (double*)(x.sm + x.P.s_red); }
+// scalars: [0] amax of the last absmax_quant, [1] scale of the in_proj / LM-head codes, [2] scale of the out_proj codes;
+// behind them the accumulators of the CTA-wide reductions, double-buffered by call parity: uint amax bits [2], int code sums [2]
 template <class S>
 __device__ __forceinline__ float* scal(const Ctx<S>& x) { return (float*)(x.sm + x.P.s_scal); }
+template <class S>
+__device__ __forceinline__ unsigned* acc_amax(const Ctx<S>& x) { return (unsigned*)(x.sm + x.P.s_scal) + 4; }
+template <class S>
+__device__ __forceinline__ int* acc_qs(const Ctx<S>& x) { return (int*)(x.sm + x.P.s_scal) + 6; }
 
 // S1 / S6 / S8 absmax + quantise of a whole vector in every CTA (the critical path of the norm: only amax is needed for
 // the codes, R13).  `en(f)` calls f(k, bits) for every group of four elements this thread holds: bits = fp32 t_k = value_k * w_k.
 // Writes the codes to xq (plane order unless `canonical`), leaves amax in scal[0] and returns the sum of the codes.
-// Two __syncthreads.
+// The two CTA-wide reductions (max, integer sum: exact in any order) are shared-memory atomics into accumulators that
+// alternate with the call parity `par`; thread 0 clears the other pair between the two barriers.  Two __syncthreads.
 template <class S, typename Enum>
-__device__ __forceinline__ int absmax_quant(const Ctx<S>& x, Enum en, int K, bool canonical, int8_t* tap_codes, int pl = 0, int pk = -1)
+__device__ __forceinline__ int absmax_quant(const Ctx<S>& x, Enum en, int K, bool canonical, int8_t* tap_codes, unsigned& par,
+                                          int pl = 0, int pk = -1)
 {
     const Params& P = x.P;
     uint8_t* xq = x.sm + P.s_xq;
-    float am = 0.0f;
-    en([&](int, uint4 w) {
-        am = fmaxf(fmaxf(am, fabsf(__uint_as_float(w.x))), fabsf(__uint_as_float(w.y)));
-        am = fmaxf(fmaxf(am, fabsf(__uint_as_float(w.z))), fabsf(__uint_as_float(w.w)));
-    });
-    am = warp_max(am);
-    if (x.lane == 0) red_f(x)[x.wid] = am;
+    unsigned am = 0u;                  // |t| as bits: non-negative floats order like unsigned integers
+    en([&](int, uint4 w) { am = max(max(am, w.x & 0x7fffffffu), max(max(w.y & 0x7fffffffu, w.z & 0x7fffffffu), w.w & 0x7fffffffu)); });
+    am = __reduce_max_sync(0xffffffffu, am);
+    if (x.lane == 0) atomicMax(acc_amax(x) + par, am);
     if (pk >= 0) x.stamp(pl, pk);
     __syncthreads();
     if (pk >= 0) x.stamp(pl, pk + 1);
-    static_assert(NWARPS % 8 == 0, "the reductions below read the warp results eight at a time");
-    float amax;
-    {
-        const float4* rf = (const float4*)red_f(x);
-        float m[NWARPS / 8];
-#pragma unroll
-        for (int i = 0; i < NWARPS / 8; ++i) {
-            const float4 a0 = rf[2 * i], a1 = rf[2 * i + 1];
-            m[i] = fmaxf(fmaxf(fmaxf(a0.x, a0.y), fmaxf(a0.z, a0.w)), fmaxf(fmaxf(a1.x, a1.y), fmaxf(a1.z, a1.w)));
-        }
-        amax = m[0];
-#pragma unroll
-        for (int i = 1; i < NWARPS / 8; ++i) amax = fmaxf(amax, m[i]);
-    }
+    const float amax = __uint_as_float(acc_amax(x)[par]);
     const float inv = amax == 0.0f ? 0.0f : fdiv(127.0f, amax);
     int qs = 0;
     en([&](int k0, uint4 w) {                                       // four consecutive elements, k0 % 4 == 0
@@ -399,17 +387,16 @@ __device__ __forceinline__ int absmax_quant(const Ctx<S>& x, Enum en, int K, boo
         qs = dp4a_us(0x01010101u, (int)packed, qs);
     });
     qs = warp_sum_i(qs);
-    if (x.lane == 0) red_i(x)[x.wid] = qs;
-    if (x.tid == 0) scal(x)[0] = amax;
+    if (x.lane == 0) atomicAdd(acc_qs(x) + par, qs);
+    if (x.tid == 0) {
+        scal(x)[0] = amax;
+        acc_amax(x)[par ^ 1u] = 0u;        // last read behind the second barrier of the previous call
+        acc_qs(x)[par ^ 1u] = 0;
+    }
     if (pk >= 0) x.stamp(pl, pk + 2);
     __syncthreads();
-    const int4* ri = (const int4*)red_i(x);
-    int tot = 0;
-#pragma unroll
-    for (int i = 0; i < NWARPS / 4; ++i) {
-        const int4 q = ri[i];
-        tot += (q.x + q.y) + (q.z + q.w);
-    }
+    const int tot = acc_qs(x)[par];
+    par ^= 1u;
     return tot;
 }
 
@@ -421,31 +408,44 @@ __device__ __forceinline__ float act_scale(double ss, int K, float eps, float am
     return amax == 0.0f ? 0.0f : fdiv(fmul(amax, rstd), 127.0f);
 }
 
-// Off the critical path, ONE warp: gather the NW fp64 partial sums of squares of a record part (8-byte elements
-// validated by their high word), add them (any tree: DESIGN.md 5.3) and leave the activation scale in scal[which].
-// amax comes from scal[0] (absmax_quant of the same vector; a CTA barrier lies between).
+// ONE warp: the activation scale of the vector whose amax is in scal[0], from the NWARPS warp sums of squares in red_d
+// (the embedding: every CTA has the whole vector).  Valid in lane 0.
 template <class S>
-__device__ __forceinline__ void scale_side(const Ctx<S>& x, const uint32_t* part, int K, int which, float* tap_scale)
+__device__ __forceinline__ float scale_from_warps(const Ctx<S>& x, int K)
+{
+    double s = x.lane < NWARPS ? red_d(x)[x.lane] : 0.0;
+#pragma unroll
+    for (int o = NWARPS / 2; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    return act_scale(s, K, x.P.eps, scal(x)[0]);
+}
+
+// ONE warp of service CTA 0, off the critical path: gather the NW fp64 partial sums of squares the workers published beside
+// their U / G slots (8-byte elements validated by their high word), add them (any tree: DESIGN.md 5.3) and return the
+// activation scale (valid in lane 0); amax comes from scal[0] (absmax_quant of the same vector; a CTA barrier lies between).
+// The scale travels to the workers as one more word of the A / T part.
+template <class S>
+__device__ __forceinline__ float scale_side(const Ctx<S>& x, const uint32_t* part, int K)
 {
     double s = 0.0;
     const int nchunk = (x.NW() + 1) >> 1;
-    for (int ch = x.lane; ch < nchunk; ch += 32) {
-        uint4 v;
+    for (int ch0 = 0; ch0 < nchunk; ch0 += 64) {          // two chunks per lane in flight
+        const int ca = ch0 + x.lane, cb = ch0 + 32 + x.lane;
+        uint4 va = make_uint4(0u, 0u, 0u, 0u), vb = va;
+        bool na = ca < nchunk, nb = cb < nchunk;
+        const bool ha = na, hb = nb;
         uint32_t spins = 0;
-        for (;;) {
-            v = x_ld128(part + 4 * ch);
-            if (v.y != SENT && (2 * ch + 1 >= x.NW() || v.w != SENT)) break;
+        while (na || nb) {
+            if (na) va = x_ld128(part + 4 * ca);
+            if (nb) vb = x_ld128(part + 4 * cb);
+            if (na) na = va.y == SENT || (2 * ca + 1 < x.NW() && va.w == SENT);
+            if (nb) nb = vb.y == SENT || (2 * cb + 1 < x.NW() && vb.w == SENT);
             if (++spins > SPIN_LIMIT || *x.dead) { poll_fail(x); break; }
         }
-        s += __hiloint2double((int)v.y, (int)v.x);
-        if (2 * ch + 1 < x.NW()) s += __hiloint2double((int)v.w, (int)v.z);
+        if (ha) { s += __hiloint2double((int)va.y, (int)va.x); if (2 * ca + 1 < x.NW()) s += __hiloint2double((int)va.w, (int)va.z); }
+        if (hb) { s += __hiloint2double((int)vb.y, (int)vb.x); if (2 * cb + 1 < x.NW()) s += __hiloint2double((int)vb.w, (int)vb.z); }
     }
     s = warp_sum(s);
-    if (x.lane == 0) {
-        const float sc = act_scale(s, K, x.P.eps, scal(x)[0]);
-        scal(x)[which] = sc;
-        if (tap_scale) *tap_scale = sc;
-    }
+    return act_scale(s, K, x.P.eps, scal(x)[0]);
 }
 
 // the elements a thread holds after gathering a slot-structured mailbox part (U or G): chunk ci = tid + j*THREADS is
@@ -487,6 +487,7 @@ __device__ __forceinline__ void sign_partial(const uint32_t* const (&rowp)[NR], 
         for (int i = 0; i < 8; ++i) a[r][i] = 0;
     const uint8_t* xlo = xq;
     const uint8_t* xhi = xq + (K >> 1);
+#pragma unroll 2
     for (int w = w0 + lane; w < w1; w += 32) {
         const int4 lo = *(const int4*)(xlo + 16 * w);
         const int4 hi = *(const int4*)(xhi + 16 * w);
@@ -544,12 +545,6 @@ __device__ __forceinline__ int trow_dot(const uint8_t* row, int nbytes, const ui
     return warp_sum_i(s);
 }
 
-// exact int -> double without the 64-bit conversion unit (16 lanes / clock / SM): bits of 1.5 * 2^52 + b, minus 1.5 * 2^52
-__device__ __forceinline__ double i2d(int b)
-{
-    return __dadd_rn(__hiloint2double(0x43380000 + (b >> 31), b), -6755399441055744.0);
-}
-
 // ------------------------------------------------------------------------------------------------
 // weight / state pipeline
 // ------------------------------------------------------------------------------------------------
@@ -564,8 +559,9 @@ __device__ __forceinline__ void issue_item(const Ctx<S>& x, int item, int v0, in
     const uint64_t pol = policy_evict_first();
     if (item < P.L) {
         if (x.service()) {
-            mbar_expect_tx(bar, P.schunk_bytes);
-            bulk_g2s_stream(stage, P.schunks + ((size_t)item * x.NS() + (x.c - x.NW())) * P.schunk_bytes, P.schunk_bytes, bar, pol);
+            const int ts = x.c - x.NW() - 1;          // task index of this service CTA; -1: the scale CTA streams nothing
+            mbar_expect_tx(bar, ts >= 0 ? P.schunk_bytes : 0u);
+            if (ts >= 0) bulk_g2s_stream(stage, P.schunks + ((size_t)item * (x.NS() - 1) + ts) * P.schunk_bytes, P.schunk_bytes, bar, pol);
             return;
         }
         const int* chs = (const int*)(x.sm + P.s_chs);
@@ -615,11 +611,12 @@ __device__ __forceinline__ void partial_store(const Ctx<S>& x, uint32_t* rec, ui
     if (x.tid == THREADS - 1) x_st64(rec + part_off + 2 * (size_t)x.c, lo, hi);
 }
 //   word (A / T): the lanes of one warp write the word to the small mailboxes the workers poll
+//   ncta = how many CTAs (0 .. ncta-1) poll the word: the workers, or everybody (0 = the workers)
 template <class S>
-__device__ __forceinline__ void word_store(const Ctx<S>& x, uint32_t* rec, uint32_t part_off, int idx, int M, uint32_t value)
+__device__ __forceinline__ void word_store(const Ctx<S>& x, uint32_t* rec, uint32_t part_off, int idx, int M, uint32_t value, int ncta = 0)
 {
     const Params& P = x.P;
-    const int nm = mbox_count(x.NW(), M);
+    const int nm = mbox_count(ncta > 0 ? ncta : x.NW(), M);
     for (int m = x.lane; m < nm; m += 32) x_st32(rec + P.x_main + (size_t)m * P.x_small + part_off + idx, value);
 }
 
@@ -630,6 +627,26 @@ __global__ void k_mega_prepare(uint8_t* chunks, size_t n_chunks, uint32_t chunk_
     if (i >= n_chunks * (size_t)nch_max) return;
     float* p = (float*)(chunks + (i / nch_max) * chunk_bytes + c_alog) + (i % nch_max);
     *p = -sp_expf(*p);
+}
+
+// every exchange word starts as "not written" (SENT); the words of a small mailbox that are never written (the pads that
+// round the A and T parts up to whole 16-byte chunks: hop_gather tests whole chunks) hold 0 for good
+__global__ void k_mega_init_x(uint32_t* xbuf, size_t n_records, uint32_t x_main, uint32_t x_small, uint32_t x_A, int n_A, uint32_t x_T,
+                              int n_ttask, int i_sg, int i_slm)
+{
+    const size_t rec_words = (size_t)x_main + (size_t)MBOX * x_small;
+    const size_t n = n_records * rec_words;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t w = i % rec_words;
+        uint32_t v = SENT;
+        if (w >= x_main) {
+            const uint32_t o = (uint32_t)((w - x_main) % x_small);
+            const bool used = (o >= x_A && o < x_A + (uint32_t)n_A) || (o >= x_T && o < x_T + (uint32_t)n_ttask) || o == x_T + (uint32_t)i_sg ||
+                              o == x_T + (uint32_t)i_slm;
+            if (!used) v = 0u;
+        }
+        xbuf[i] = v;
+    }
 }
 
 template <class S, bool TAPS, bool PROF>
@@ -658,7 +675,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
     int* s_acc_out = (int*)(sm + P.s_acc_out);
     const int NW = x.NW(), NS = x.NS();
     const bool service = c >= NW;
-    const int sv = c - NW;                           // index among the service CTAs (if service)
+    const int sv = c - NW;                           // index among the service CTAs (if service): 0 = the scale CTA, 1 .. NS-1 hold row tasks
+    const int ts = sv - 1, NT = NS - 1;              // task index / number of task CTAs
 
     for (int g = tid; g <= NW; g += THREADS) {
         chs[g] = own_start(g, x.d_inner(), NW);
@@ -692,11 +710,15 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
     const int KS = (THREADS >= 1024 && x.Wout() >= 128) ? 4 : (x.Wout() >= 64 ? 2 : 1);
     const int tbytes = x.d_inner() / x.tsplit();         // bytes of one out_proj LoRA-down partial task
     // service: what this CTA holds of each dealt list
-    const int n_sig = service ? dealt(x.n_bcdt(), sv, NS) : 0, n_lin = service ? dealt(x.r(), sv, NS) : 0,
-              n_tt = service ? dealt(x.n_ttask(), sv, NS) : 0;
+    const bool tasks = service && ts >= 0;
+    const int n_sig = tasks ? dealt(x.n_bcdt(), ts, NT) : 0, n_lin = tasks ? dealt(x.r(), ts, NT) : 0,
+              n_tt = tasks ? dealt(x.n_ttask(), ts, NT) : 0;
 
     // ---------------- S0 embedding + the first norm/quantise, redundantly in every CTA ----------------
     int qsum;
+    unsigned par = 0u;                               // call parity of absmax_quant (its accumulators alternate)
+    if (tid < 4) acc_amax(x)[tid] = 0u;              // acc_amax[2] | acc_qs[2]
+    __syncthreads();
     {
         int tok = P.tokens[0];
         if (tok < 0 || tok >= P.vocab) {
@@ -723,7 +745,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             }
         }
         ss = warp_sum(ss);
-        if (lane == 0) red_d(x)[wid] = ss;           // read by thread 0 after the barriers of absmax_quant
+        if (lane == 0) red_d(x)[wid] = ss;           // read by warp 0 behind the barriers of absmax_quant
         uint8_t* tp0 = (taps_on && c == 0 && P.L > 0) ? P.taps : nullptr;
         auto en = [&](auto f) {
 #pragma unroll
@@ -732,14 +754,10 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 if (k0 < x.d_model()) f(k0, v[j]);
             }
         };
-        qsum = absmax_quant(x, en, x.d_model(), P.L == 0, tp0 ? (int8_t*)(tp0 + P.tl.off[0]) : nullptr);
-        if (tid == 0) {
-            double t4[4] = { 0.0, 0.0, 0.0, 0.0 };
-#pragma unroll
-            for (int i = 0; i < NWARPS; ++i) t4[i & 3] += red_d(x)[i];
-            const float sc = act_scale((t4[0] + t4[1]) + (t4[2] + t4[3]), x.d_model(), P.eps, scal(x)[0]);
-            scal(x)[1] = sc;
-            if (tp0) *(float*)(tp0 + P.tl.off[1]) = sc;
+        qsum = absmax_quant(x, en, x.d_model(), P.L == 0, tp0 ? (int8_t*)(tp0 + P.tl.off[0]) : nullptr, par);
+        if (wid == 0) {
+            const float sc = scale_from_warps(x, x.d_model());
+            if (lane == 0) scal(x)[1] = sc;          // scale of the layer-0 in_proj codes (L == 0: of the LM-head codes)
         }
         __syncthreads();
     }
@@ -751,7 +769,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         uint8_t* tp = taps_on ? P.taps + (size_t)l * P.tap_lstride : nullptr;
         float* conv_l = P.conv + (size_t)l * P.conv_lstride;
         uint32_t* rec = P.xbuf + ((size_t)P.set * P.L + l) * rec_words;                       // this step's record of layer l
-        uint32_t* recp = rec - rec_words;                                                     // ... of layer l - 1 (U partials; l > 0)
         uint32_t* recc = P.xbuf + ((size_t)(P.set ^ 1u) * P.L + l) * rec_words;               // the next step's: own words are reset here
         DFSSM_STAMP(l, 0);
         if (x.prof && tid == 0) P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + 31] = globaltimer_ns();
@@ -770,76 +787,73 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                         int p[1];
                         sign_partial<1>(rowp, 1, 0, x.Win(), xq, x.d_model(), lane, p);
                         val = 2 * (warp_sum_i(p[0]) / 128) - qsum;       // exact: every term is a multiple of 128
-                        idx = sv + k * NS;
+                        idx = ts + k * NT;
                     } else {
                         const int kk = k - n_sig;
                         val = trow_dot(stage + P.sc_tin + (size_t)kk * x.d_model(), x.d_model(), xq, lane);
-                        idx = x.n_bcdt() + sv + kk * NS;
+                        idx = x.n_bcdt() + ts + kk * NT;
                     }
                     word_store(x, rec, P.x_A, idx, M_A, (uint32_t)val ^ IBIAS);
                 }
             }
+            // ---- the scale CTA: the scale of the layer-0 in_proj codes (made with the embedding) travels with A; the later
+            //      layers' scales are published as soon as their U has been gathered (end of the loop body) ----
+            if (sv == 0 && wid == SCALE_WARP && l == 0) word_store(x, rec, P.x_A, x.n_early(), M_A, __float_as_uint(scal(x)[1]));
             DFSSM_STAMP(l, 2);
             // ---- gather G, codes of the whole gated vector ----
             int qsum_g;
             {
                 uint4 vg[NJ_G];
-                hop_gather<NJ_G>(x, rec + P.x_G, NW * x.g_slot(), vg, tid);
+                hop_gather<NJ_G>(x, rec + P.x_G, NW * x.g_slot() / 4, vg, tid);
                 DFSSM_STAMP(l, 6);
-                qsum_g = absmax_quant(x, SlotEnum<NJ_G>{ vg, chs, tid, NW, x.g_slot() >> 2 }, x.d_inner(), false, nullptr, l, 16);
+                qsum_g = absmax_quant(x, SlotEnum<NJ_G>{ vg, chs, tid, NW, x.g_slot() >> 2 }, x.d_inner(), false, nullptr, par, l, 16);
             }
             (void)qsum_g;
             DFSSM_STAMP(l, 7);
             // ---- out_proj: LoRA-down partial tasks dealt to this CTA ----
             for (int k = wid; k < n_tt; k += NWARPS) {
-                const int q = sv + k * NS, part = q % x.tsplit();
+                const int q = ts + k * NT, part = q % x.tsplit();
                 const int t = trow_dot(stage + P.sc_tout + (size_t)k * tbytes, tbytes, xq + (size_t)part * tbytes, lane);
                 word_store(x, rec, P.x_T, q, M_T, (uint32_t)t ^ IBIAS);
             }
+            if (sv == 0 && wid == SCALE_WARP) {     // the scale of the gated codes travels with T
+                const float sc = scale_side(x, rec + P.x_PG, x.d_inner());
+                word_store(x, rec, P.x_T, x.i_sg(), M_T, __float_as_uint(sc));
+            }
             DFSSM_STAMP(l, 8);
             // ---- reset own words of the next step's record of this layer (this CTA is idle until U arrives) ----
-            for (int k = wid; k < n_sig; k += NWARPS) word_store(x, recc, P.x_A, sv + k * NS, M_A, SENT);
-            for (int k = wid; k < n_lin; k += NWARPS) word_store(x, recc, P.x_A, x.n_bcdt() + sv + k * NS, M_A, SENT);
-            for (int k = wid; k < n_tt; k += NWARPS) word_store(x, recc, P.x_T, sv + k * NS, M_T, SENT);
+            if (sv == 0 && wid == SCALE_WARP) {
+                word_store(x, recc, P.x_A, x.n_early(), M_A, SENT);
+                word_store(x, recc, P.x_T, x.i_sg(), M_T, SENT);
+                if (l == P.L - 1) word_store(x, recc, P.x_T, x.i_slm(), M_T, SENT, GRID);
+            }
+            for (int k = wid; k < n_sig; k += NWARPS) word_store(x, recc, P.x_A, ts + k * NT, M_A, SENT);
+            for (int k = wid; k < n_lin; k += NWARPS) word_store(x, recc, P.x_A, x.n_bcdt() + ts + k * NT, M_A, SENT);
+            for (int k = wid; k < n_tt; k += NWARPS) word_store(x, recc, P.x_T, ts + k * NT, M_T, SENT);
             __syncthreads();                        // every thread is done with this stage's weights
             DFSSM_STAMP(l, 10);
         } else {
             // ================= worker CTA =================
-            // ---- S2: z and x sign rows of this CTA, NR_IN rows per warp pass, dealt from the top warp down ----
+            // ---- S2: z and x sign rows of this CTA (slots 0 .. 2 nch - 1: z rows, then x rows; the chunk pads them with zero rows
+            //      to whole groups of NR_IN), NR_IN rows per warp pass, dealt from the top warp down ----
             {
                 const uint32_t* bits = (const uint32_t*)(stage + P.c_in_bits);
-                const int n_tasks = 2 * nch;
-                for (int q = NWARPS - 1 - wid; NR_IN * q < n_tasks; q += NWARPS) {
+                const int n_groups = (2 * nch + NR_IN - 1) / NR_IN;
+                for (int q = NWARPS - 1 - wid; q < n_groups; q += NWARPS) {
                     const uint32_t* rowp[NR_IN];
-                    int slot[NR_IN];
-                    const int nrows = min(NR_IN, n_tasks - NR_IN * q);
 #pragma unroll
-                    for (int r = 0; r < NR_IN; ++r) {
-                        const int t = NR_IN * q + r;
-                        slot[r] = r < nrows ? (t < nch ? t : x.nch_max() + (t - nch)) : 0;
-                        rowp[r] = bits + (size_t)slot[r] * x.Win();
-                    }
+                    for (int r = 0; r < NR_IN; ++r) rowp[r] = bits + (size_t)(NR_IN * q + r) * x.Win();
                     int p[NR_IN];
-                    sign_partial<NR_IN>(rowp, nrows, 0, x.Win(), xq, x.d_model(), lane, p);
+                    sign_partial<NR_IN>(rowp, NR_IN, 0, x.Win(), xq, x.d_model(), lane, p);
                     const int v = RowReduce<NR_IN>::run(p, lane);
-                    const int r = lane / (32 / NR_IN);
-                    if (lane % (32 / NR_IN) == 0 && r < nrows) s_acc_in[slot[r]] = 2 * (v / 128) - qsum;
+                    if (lane % (32 / NR_IN) == 0) s_acc_in[NR_IN * q + lane / (32 / NR_IN)] = 2 * (v / 128) - qsum;
                 }
             }
             DFSSM_STAMP(l, 2);
-            {   // reset own slots of the next step's record of this layer (same thread -> address map as the publishes)
-                slot_store(x, recc, P.x_U, x.u_slot(), [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
-                slot_store(x, recc, P.x_G, x.g_slot(), [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
-                partial_store(x, recc, P.x_PU, SENT, SENT);
-                partial_store(x, recc, P.x_PG, SENT, SENT);
-            }
-            // ---- warp 0: scale of the in_proj codes from the U partials of layer l - 1 (layer 0: made with the embedding) ----
-            if (wid == 0 && l > 0)
-                scale_side(x, recp + P.x_PU, x.d_model(), 1, (tp && c == 0) ? (float*)(tp + P.tl.off[1]) : nullptr);
             // ---- gather A: accumulators of all B|C|dt rows and t_in;  v_j = a_s[j] * float(t_j) ----
             {
                 uint4 va[NJ_A];
-                hop_gather<NJ_A>(x, rec + mbox(M_A) + P.x_A, x.n_early(), va, rtid);
+                hop_gather<NJ_A>(x, rec + mbox(M_A) + P.x_A, (x.n_A() + 3) / 4, va, rtid);
                 const float* a_s = (const float*)(blk + P.b_as_in);
 #pragma unroll
                 for (int j = 0; j < NJ_A; ++j) {
@@ -848,6 +862,10 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
                         const int e = e0 + i;
+                        if (e == x.n_early()) {                   // scale of this layer's in_proj codes (made by service CTA 0)
+                            scal(x)[1] = __uint_as_float(w[i]);
+                            if (tp && c == 0) *(float*)(tp + P.tl.off[1]) = __uint_as_float(w[i]);
+                        }
                         if (e < x.n_early()) {
                             const int val = (int)(w[i] ^ IBIAS);
                             if (e < x.n_bcdt()) s_eacc[e] = val;
@@ -880,7 +898,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     const bool valid = ib + lt / LP < count;
                     int kind, slot = 0, e = 0;         // kind 0 z, 1 x, 2 B|C, 3 dt
                     if (i < nch) { kind = 0; slot = i; }
-                    else if (i < 2 * nch) { kind = 1; slot = x.nch_max() + (i - nch); }
+                    else if (i < 2 * nch) { kind = 1; slot = i; }
                     else if (i < 2 * nch + 2 * x.gs()) { kind = 2; e = i - 2 * nch; }
                     else { kind = 3; e = 2 * x.gs() + ((tp && c == 0) ? 0 : h0) + (i - 2 * nch - 2 * x.gs()); }
                     const bool own = kind < 2;
@@ -891,10 +909,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     double lo0 = 0.0, lo1 = 0.0;
                     for (int j4 = 4 * sub; j4 < x.r_pad(); j4 += 4 * LP) {         // pad entries of B are 0, pad entries of v are 0
                         const int w = bw[(j4 >> 2) * bstep];
-                        lo0 = __fma_rn(i2d((int)(int8_t)w), s_vin[j4], lo0);
-                        lo1 = __fma_rn(i2d((int)(int8_t)(w >> 8)), s_vin[j4 + 1], lo1);
-                        lo0 = __fma_rn(i2d((int)(int8_t)(w >> 16)), s_vin[j4 + 2], lo0);
-                        lo1 = __fma_rn(i2d(w >> 24), s_vin[j4 + 3], lo1);
+                        const double2 v01 = *(const double2*)(s_vin + j4), v23 = *(const double2*)(s_vin + j4 + 2);
+                        lo0 = __fma_rn((double)(int8_t)w, v01.x, lo0);
+                        lo1 = __fma_rn((double)(int8_t)(w >> 8), v01.y, lo1);
+                        lo0 = __fma_rn((double)(int8_t)(w >> 16), v23.x, lo0);
+                        lo1 = __fma_rn((double)(w >> 24), v23.y, lo1);
                     }
                     lo0 += lo1;
 #pragma unroll
@@ -908,7 +927,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     int row;                       // canonical in_proj row (for the taps)
                     bool tap_owner = true;
                     if (kind == 0) {
-                        s_z[i] = val;
+                        s_z[i] = siluf(val);           // the gate's factor
                         row = ch0 + i;
                     } else if (kind == 1) {
                         const int ic = i - nch;
@@ -977,7 +996,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     const float dA = sp_expf(fmul(dtv, An));
                     const float xv = s_x[i];
                     const float dtx = fmul(dtv, xv);
-                    const float sz = siluf(s_z[i]);             // all lanes: free in SIMT, and off the tail of the reduction
                     float* Hr = (float*)(stage + P.st_ssm) + (size_t)i * x.d_state();
                     const float* Bc = s_bc + grp * x.d_state();
                     const double* Cc = s_cd + grp * x.d_state();
@@ -1000,7 +1018,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     if (l16 == 0 && valid) {
                         a = dacc(a, Dv[i], xv);
                         const float y = (float)a;
-                        const float gv = fmul(y, sz);
+                        const float gv = fmul(y, s_z[i]);
                         s_slotG[i] = __float_as_uint(fmul(gv, gw[i]));
                         ss_own = dacc(ss_own, gv, gv);
                         if (tp) { ((float*)(tp + P.tl.off[7]))[ch] = y; ((float*)(tp + P.tl.off[8]))[ch] = gv; }
@@ -1028,25 +1046,31 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     bulk_commit();
                 }
             }
+            // reset own slots of the next step's record of this layer (same thread -> address map as the publishes), in the
+            // shadow of the G exchange
+            {
+                slot_store(x, recc, P.x_U, x.u_slot(), [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
+                slot_store(x, recc, P.x_G, x.g_slot(), [](int) { return make_uint4(SENT, SENT, SENT, SENT); });
+                partial_store(x, recc, P.x_PU, SENT, SENT);
+                partial_store(x, recc, P.x_PG, SENT, SENT);
+            }
             DFSSM_STAMP(l, 5);
 
             // ---- gather G, S6 absmax + quantise of the whole gated vector in every CTA ----
             int qsum_g;
             {
                 uint4 vg[NJ_G];
-                hop_gather<NJ_G>(x, rec + P.x_G, NW * x.g_slot(), vg, tid, DFSSM_WG);
+                hop_gather<NJ_G>(x, rec + P.x_G, NW * x.g_slot() / 4, vg, tid, DFSSM_WG);
                 DFSSM_STAMP(l, 6);
                 qsum_g = absmax_quant(x, SlotEnum<NJ_G>{ vg, chs, tid, NW, x.g_slot() >> 2 }, x.d_inner(), false,
-                                      (tp && c == 0) ? (int8_t*)(tp + P.tl.off[9]) : nullptr, l, 16);
+                                      (tp && c == 0) ? (int8_t*)(tp + P.tl.off[9]) : nullptr, par, l, 16);
             }
             DFSSM_STAMP(l, 7);
-            // ---- S7: warp 0 makes the scale of the gated codes; the other warps do the out_proj sign rows ----
-            if (wid == 0) {
-                scale_side(x, rec + P.x_PG, x.d_inner(), 2, (tp && c == 0) ? (float*)(tp + P.tl.off[10]) : nullptr);
-            } else {
+            // ---- S7: the out_proj sign rows ----
+            {
                 const uint32_t* bits = (const uint32_t*)(stage + P.c_out_bits);
                 const int npair = (nor + 1) >> 1, wspan = x.Wout() / KS;
-                for (int id = wid - 1; id < npair * KS; id += NWARPS - 1) {
+                for (int id = wid; id < npair * KS; id += NWARPS) {
                     const int pair = id / KS, half = id - pair * KS;
                     const int nrows = min(2, nor - 2 * pair);
                     const uint32_t* const rowp[2] = { bits + (size_t)(2 * pair) * x.Wout(), bits + (size_t)(2 * pair + (nrows > 1 ? 1 : 0)) * x.Wout() };
@@ -1061,8 +1085,12 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             // ---- gather T: t_out = sum of the partial sums;  v_j = a_s[j] * float(t_j) ----
             {
                 uint4 vt[1];
-                hop_gather<1>(x, rec + mbox(M_T) + P.x_T, x.n_ttask(), vt, rtid);
-                if (rtid < (x.n_ttask() + 3) / 4) {
+                hop_gather<1>(x, rec + mbox(M_T) + P.x_T, x.i_sg() / 4 + 1, vt, rtid);
+                if (rtid == x.i_sg() / 4) {                   // scale of the gated codes (made by service CTA 0)
+                    scal(x)[2] = __uint_as_float(vt[0].x);
+                    if (tp && c == 0) *(float*)(tp + P.tl.off[10]) = __uint_as_float(vt[0].x);
+                }
+                if (rtid < x.i_sg() / 4) {
                     const float* a_s = (const float*)(blk + P.b_as_out);
                     const uint32_t w[4] = { vt[0].x, vt[0].y, vt[0].z, vt[0].w };
                     const int rows_per_chunk = 4 / x.tsplit();
@@ -1094,7 +1122,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     double lo = 0.0;
                     const int8_t* brow = Bm + (size_t)(valid ? i : 0) * x.r_pad();
                     if (valid)
-                        for (int j = sub; j < x.r(); j += 4) lo = __fma_rn(i2d((int)brow[j]), s_vout[j], lo);
+                        for (int j = sub; j < x.r(); j += 4) lo = __fma_rn((double)brow[j], s_vout[j], lo);
                     lo += __shfl_xor_sync(0xffffffffu, lo, 1);
                     lo += __shfl_xor_sync(0xffffffffu, lo, 2);
                     if (sub != 0 || !valid) continue;
@@ -1125,11 +1153,17 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         // ---- gather U, S1 of the next layer (or S8's norm) in every CTA ----
         {
             uint4 vu[NJ_U];
-            hop_gather<NJ_U>(x, rec + P.x_U, NW * x.u_slot(), vu, tid, service ? 0 : DFSSM_WU);
+            hop_gather<NJ_U>(x, rec + P.x_U, NW * x.u_slot() / 4, vu, tid, service ? 0 : DFSSM_WU);
             DFSSM_STAMP(l, 11);
             uint8_t* tpn = (taps_on && c == 0 && l + 1 < P.L) ? P.taps + (size_t)(l + 1) * P.tap_lstride : nullptr;
             qsum = absmax_quant(x, SlotEnum<NJ_U>{ vu, ors, tid, NW, x.u_slot() >> 2 }, x.d_model(), l == P.L - 1,
-                                tpn ? (int8_t*)(tpn + P.tl.off[0]) : nullptr, l, 20);
+                                tpn ? (int8_t*)(tpn + P.tl.off[0]) : nullptr, par, l, 20);
+            // the scale of these codes is made by the scale CTA and travels with the next layer's A; the LM head gets it through T
+            if (service && sv == 0 && wid == SCALE_WARP) {
+                const float sc = scale_side(x, rec + P.x_PU, x.d_model());
+                if (l == P.L - 1) word_store(x, rec, P.x_T, x.i_slm(), M_T, __float_as_uint(sc), GRID);     // every CTA reads it
+                else word_store(x, rec + rec_words, P.x_A, x.n_early(), M_A, __float_as_uint(sc));
+            }
         }
         // ---- refill this layer's ring stage with the item `stages` ahead: after the gather, so that the bulk copies do
         //      not sit in front of its polls in the memory pipeline ----
@@ -1141,11 +1175,18 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
     }
 
     // =============================================== S8 LM head ===============================================
-    if (P.L > 0) {      // scale of the final codes from the U partials of the last layer (L == 0: made with the embedding)
-        uint32_t* recl = P.xbuf + ((size_t)P.set * P.L + (P.L - 1)) * rec_words;
-        if (wid == 0) scale_side(x, recl + P.x_PU, x.d_model(), 1, nullptr);
-        __syncthreads();
+    if (P.L > 0 && tid == 0) {                       // scale of the final codes: word i_slm of the last layer's T part
+        const uint32_t* w = P.xbuf + ((size_t)P.set * P.L + (P.L - 1)) * rec_words + P.x_main + (size_t)mbox_of(c, M_T) * P.x_small + P.x_T +
+                            x.i_slm();
+        uint32_t v, spins = 0;
+        for (;;) {
+            asm volatile("ld.relaxed.gpu.global.b32 %0, [%1];" : "=r"(v) : "l"(w) : "memory");
+            if (v != SENT) break;
+            if (++spins > SPIN_LIMIT || *x.dead) { poll_fail(x); break; }
+        }
+        scal(x)[1] = __uint_as_float(v);
     }
+    __syncthreads();
     const float s_act = scal(x)[1];
     for (int i = tid; i < nor; i += THREADS) P.u_out[or0 + i] = s_u[i];
     DFSSM_STAMP(P.L, 0);
@@ -1194,8 +1235,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             const int oi = __shfl_xor_sync(0xffffffffu, besti, o);
             if (ov > best || (ov == best && oi < besti)) { best = ov; besti = oi; }
         }
-        float* rv = red_f(x);
-        int* ri = red_i(x);
+        float* rv = (float*)red_d(x);               // scratch: NWARPS floats | NWARPS ints
+        int* ri = (int*)rv + NWARPS;
         __shared__ int s_last;
         if (lane == 0) { rv[wid] = best; ri[wid] = besti; }
         __syncthreads();

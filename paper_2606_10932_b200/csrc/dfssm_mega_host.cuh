@@ -44,23 +44,24 @@ inline bool plan(const Dims& d, int G, Params& P)
     if (d.d_model > 8192 || d.d_inner > 8192) return false;
     P.NW = pick_workers(d);
     P.NS = G - P.NW;
+    P.NT = P.NS - 1;                            // service CTA 0 makes the activation scales, the others hold the row tasks
     P.nch_max = own_max(d.d_inner, P.NW);
     P.nor_max = own_max(d.d_model, P.NW);
     P.r_pad = (d.r + 3) / 4 * 4;
     P.Win = d.d_model / 32;
     P.Wout = d.d_inner / 32;
     P.n_early = P.n_bcdt + d.r;
-    if (P.n_early > NJ_A * THREADS * 4) return false;
+    if (P.n_early + 1 > NJ_A * THREADS * 4) return false;
     P.tsplit = d.d_inner % 64 == 0 ? 4 : 2;
     P.n_ttask = d.r * P.tsplit;
     if (P.nch_max > 128 || P.nor_max > 128 || d.d_inner < 4 || d.d_model < 4) return false;
-    P.ns_sig = dealt(P.n_bcdt, 0, P.NS);
-    P.ns_lin = dealt(d.r, 0, P.NS);
-    P.ns_tt = dealt(P.n_ttask, 0, P.NS);
+    P.ns_sig = dealt(P.n_bcdt, 0, P.NT);
+    P.ns_lin = dealt(d.r, 0, P.NT);
+    P.ns_tt = dealt(P.n_ttask, 0, P.NT);
 
     uint32_t off = 0;
     auto take = [&](size_t bytes) { off = up32(off, 16); const uint32_t at = off; off += (uint32_t)bytes; return at; };
-    P.c_in_bits = take((size_t)2 * P.nch_max * P.Win * 4);
+    P.c_in_bits = take((size_t)up32(2 * P.nch_max, 4) * P.Win * 4);     // zero rows pad the z | x rows to whole groups of NR_IN
     P.c_out_bits = take((size_t)P.nor_max * P.Wout * 4);
     P.c_in_B = take((size_t)2 * P.nch_max * P.r_pad);
     P.c_out_B = take((size_t)P.nor_max * P.r_pad);
@@ -115,8 +116,8 @@ inline bool plan(const Dims& d, int G, Params& P)
     P.x_PG = xtake((size_t)2 * P.NW);
     P.x_main = up32(xo, 32);
     xo = 0;
-    P.x_A = xtake(P.n_early);
-    P.x_T = xtake(P.n_ttask);
+    P.x_A = xtake(up32(P.n_early + 1, 4));      // + the scale word(s) made by service CTA 0
+    P.x_T = xtake(up32(P.n_ttask, 4) + 8);      // + two scale words, each in a chunk of its own
     P.x_small = up32(xo, 32);
 
     // shared memory behind the ring
@@ -125,9 +126,9 @@ inline bool plan(const Dims& d, int G, Params& P)
     const int kmax = d.d_model > d.d_inner ? d.d_model : d.d_inner;
     const uint32_t x_xq = stake(kmax), x_bc = stake((size_t)P.gs * 4), x_cd = stake((size_t)P.gs * 8), x_u = stake((size_t)P.nor_max * 4),
                    x_z = stake((size_t)P.nch_max * 4), x_x = stake((size_t)P.nch_max * 4), x_dt = stake((size_t)d.nheads * 4),
-                   x_v = stake((size_t)2 * P.r_pad * 8), x_ea = stake((size_t)P.n_bcdt * 4), x_ai = stake((size_t)2 * P.nch_max * 4),
+                   x_v = stake((size_t)2 * P.r_pad * 8), x_ea = stake((size_t)P.n_bcdt * 4), x_ai = stake((size_t)up32(2 * P.nch_max, 4) * 4),
                    x_ao = stake((size_t)KS_MAX * P.nor_max * 4), x_chs = stake((size_t)(G + 1) * 4), x_ors = stake((size_t)(G + 1) * 4),
-                   x_red = stake(16 * NWARPS), x_slot = stake((size_t)(P.u_slot + P.g_slot) * 4), x_scal = stake(16),
+                   x_red = stake(8 * NWARPS), x_slot = stake((size_t)(P.u_slot + P.g_slot) * 4), x_scal = stake(32),
                    x_mbar = stake(8 * MAX_STAGES);
     const uint32_t fixed = up32(so, 128);
     if (fixed + 2 * (size_t)P.stage_bytes > SMEM_LIMIT) return false;
@@ -153,7 +154,7 @@ inline Regions regions(const Params& P)
     Regions r;
     const size_t nl = (size_t)(P.L > 0 ? P.L : 1);
     r.chunks = nl * P.NW * P.chunk_bytes;
-    r.schunks = nl * P.NS * P.schunk_bytes;
+    r.schunks = nl * P.NT * P.schunk_bytes;
     r.blocks = nl * P.blk_bytes;
     r.xbuf = (size_t)2 * nl * ((size_t)P.x_main + (size_t)MBOX * P.x_small) * 4;      // 2 sets x L records
     r.am = (size_t)P.G * 8 + 64;
@@ -235,7 +236,7 @@ inline void pack_chunk(const Params& P, const HostLayer& H, const float* next_no
     for (int i = 0; i < nch; ++i) {
         const int ch = ch0 + i, h = ch / P.headdim;
         put_in_row(i, ch);                                   // z row
-        put_in_row(P.nch_max + i, P.d_inner + ch);           // x row
+        put_in_row(nch + i, P.d_inner + ch);                 // x row
         memcpy(out + P.c_conv_w + 16 * (size_t)i, H.conv_w + 4 * (size_t)ch, 16);
         ((float*)(out + P.c_conv_b))[i] = H.conv_b[ch];
         ((float*)(out + P.c_alog))[i] = H.A_log[h];
@@ -257,18 +258,18 @@ inline void permute_row(const int8_t* A, int K, int8_t* out)
     for (int k = 0; k < K; ++k) out[plane_pos_host(k, K)] = A[k];
 }
 
-// chunk of (layer, service CTA s): the B|C|dt sign rows s, s + NS, ..., the in_proj LoRA-down rows s, s + NS, ... and the
-// out_proj LoRA-down partial tasks s, s + NS, ... (task q = row q / tsplit, part q % tsplit of the plane-permuted row)
+// chunk of (layer, task CTA s): the B|C|dt sign rows s, s + NT, ..., the in_proj LoRA-down rows s, s + NT, ... and the
+// out_proj LoRA-down partial tasks s, s + NT, ... (task q = row q / tsplit, part q % tsplit of the plane-permuted row)
 inline void pack_schunk(const Params& P, const HostLayer& H, int s, uint8_t* out, std::vector<int8_t>& tmp)
 {
     memset(out, 0, P.schunk_bytes);
-    for (int k = 0, e = s; e < P.n_bcdt; ++k, e += P.NS)
+    for (int k = 0, e = s; e < P.n_bcdt; ++k, e += P.NT)
         copy_sign_row((uint32_t*)(out + P.sc_sign + (size_t)k * P.Win * 4), H.in_sign + (size_t)(2 * P.d_inner + e) * P.Win, P.Win);
-    for (int k = 0, j = s; j < P.r; ++k, j += P.NS)
+    for (int k = 0, j = s; j < P.r; ++k, j += P.NT)
         permute_row(H.in_A + (size_t)j * P.d_model, P.d_model, (int8_t*)(out + P.sc_tin + (size_t)k * P.d_model));
     const int tbytes = P.d_inner / P.tsplit;
     tmp.resize((size_t)P.d_inner);
-    for (int k = 0, q = s; q < P.n_ttask; ++k, q += P.NS) {
+    for (int k = 0, q = s; q < P.n_ttask; ++k, q += P.NT) {
         permute_row(H.out_A + (size_t)(q / P.tsplit) * P.d_inner, P.d_inner, tmp.data());
         memcpy(out + P.sc_tout + (size_t)k * tbytes, tmp.data() + (size_t)(q % P.tsplit) * tbytes, tbytes);
     }
