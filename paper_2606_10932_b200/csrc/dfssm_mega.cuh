@@ -65,7 +65,7 @@ constexpr int NJ_A = 1024 / THREADS;          // ... when gathering A
 constexpr int NR_IN = THREADS >= 1024 ? 2 : 4;     // in_proj sign rows per warp pass
 constexpr int LPC = THREADS / 32;             // lanes per channel in the state update (32 channels per pass)
 constexpr int LPB = THREADS / 512;            // lanes per B|C row in the in_proj epilogue
-constexpr int SCALE_WARP = 2;                 // the warp of service CTA 0 that makes the activation scales (it has one early task, not two)
+constexpr int SCALE_WARP = 0;                 // the warp of the scale CTA that finishes the activation scales
 constexpr int DMA_TID = 96;                   // the thread that issues the state write-back and the ring refills (a warp off the publish paths)
 constexpr int KS_MAX = 4;                     // largest K-split of the out_proj sign rows
 constexpr int MAX_STAGES = 8;
@@ -119,7 +119,7 @@ struct Params {
     // ---- exchange: 2 sets x L records; a record = main part (U, PU, G, PG: one copy) + MBOX small mailboxes (A, T);
     //      32-bit word offsets inside the main part / inside one small mailbox ----
     int u_slot, g_slot;          // words per worker slot of U / G (a power of two >= the owned elements)
-    uint32_t x_U, x_PU, x_G, x_PG, x_main, x_A, x_T, x_small;
+    uint32_t x_U, x_PU, x_G, x_PG, x_main, x_A, x_T, x_small;      // PU / PG: the workers' fp64 partial sums of squares
     // ---- shared memory carve ----
     uint32_t s_ring, s_mbar, s_xq, s_bc, s_cd, s_u, s_z, s_x, s_dt, s_v, s_eacc, s_acc_in, s_acc_out, s_chs, s_ors,
         s_red, s_slot, s_scal, smem_bytes;
@@ -255,6 +255,11 @@ struct Ctx {
     static constexpr int NJG = S::kStatic ? nj_slots(S::d_inner, S::NW) : NJ_MAX;     // chunks per thread: gather G, gather U
     static constexpr int NJU = S::kStatic ? nj_slots(S::d_model, S::NW) : NJ_MAX;
     static constexpr int NJ0 = S::kStatic ? (S::d_model / 4 + THREADS - 1) / THREADS : 8192 / 4 / THREADS;   // embedding
+    // every worker owns the same number of channels / out rows (a compile-time constant), and a slot holds exactly that many
+    // words: element k of the gathered vector sits in chunk k / 4 (no ownership tables on the critical path)
+    static constexpr bool kEven = S::kStatic && (S::d_inner / 4) % (S::kStatic ? S::NW : 1) == 0 && (S::d_model / 4) % (S::kStatic ? S::NW : 1) == 0;
+    static constexpr int kNch = kEven ? S::d_inner / (S::kStatic ? S::NW : 1) : 0, kNor = kEven ? S::d_model / (S::kStatic ? S::NW : 1) : 0;
+    static constexpr bool kDenseG = kEven && slot_words(kNch) == kNch, kDenseU = kEven && slot_words(kNor) == kNor;
 #define DFSSM_DIM(n_) __device__ __forceinline__ int n_() const { return S::kStatic ? S::n_ : P.n_; }
     DFSSM_DIM(d_model) DFSSM_DIM(d_inner) DFSSM_DIM(headdim) DFSSM_DIM(d_state) DFSSM_DIM(ngroups) DFSSM_DIM(r) DFSSM_DIM(NW)
 #undef DFSSM_DIM
@@ -264,6 +269,15 @@ struct Ctx {
             const int v = *dead;
             unsigned long long t;
             asm volatile("mov.u64 %0, %%clock64;" : "=l"(t) : "r"(v) : "memory");
+            P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + k] = t;
+        }
+    }
+    __device__ __forceinline__ void gstamp(int l, int k) const      // %globaltimer (ns, one clock for all SMs): cross-CTA timelines
+    {
+        if (prof && tid == 0) {
+            const int v = *dead;
+            unsigned long long t;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t) : "r"(v) : "memory");
             P.prof[((size_t)c * (P.L + 1) + l) * PROF_NPH + k] = t;
         }
     }
@@ -312,6 +326,9 @@ __device__ __forceinline__ constexpr int mbox_count(int n, int M) { return (n + 
 // ------------------------------------------------------------------------------------------------
 // exchange: gather a self-validating buffer
 // ------------------------------------------------------------------------------------------------
+// scratch inside s_red: NWARPS doubles (warp sums of squares)
+template <class S>
+__device__ __forceinline__ double* red_d(const Ctx<S>& x) { return (double*)(x.sm + x.P.s_red); }
 // a 16-byte chunk is complete when none of its four words is the sentinel (every part is padded to whole chunks and
 // pad words hold 0 from load time on)
 __device__ __forceinline__ bool chunk_ok(uint4 v) { return max(max(v.x, v.y), max(v.z, v.w)) != SENT; }
@@ -319,35 +336,56 @@ __device__ __forceinline__ bool chunk_ok(uint4 v) { return max(max(v.x, v.y), ma
 // Thread t owns the 16-byte chunks t, t + THREADS, ... (at most NJ) of the nchunk chunks at buf.  Spins until every owned
 // word has been written; the raw words come back in v[].  tix = the thread's index for the chunk ownership (tid, or
 // reversed so that the small gathers are polled by the warps that have nothing else to do).
+// If `part` is given (the scale CTA gathering U or G), the lanes 0 .. PLN-1 of every warp also poll one chunk (two fp64 partial
+// sums of squares, validated by their high words) of the workers' partial array, and the warp's sum of them is left in
+// red_d[warp] (read by scale_finish behind the barriers of absmax_quant).
+constexpr int PLN = 8;
 template <int NJ, class S>
-__device__ __forceinline__ void hop_gather(const Ctx<S>& x, const uint32_t* buf, int nchunk, uint4 (&v)[NJ], int tix, int first_wait = 0)
+__device__ __forceinline__ void hop_gather(const Ctx<S>& x, const uint32_t* buf, int nchunk, uint4 (&v)[NJ], int tix, int first_wait = 0,
+                                           const uint32_t* part = nullptr)
 {
     bool need[NJ];
     bool any = false;
 #pragma unroll
     for (int j = 0; j < NJ; ++j) { need[j] = tix + j * THREADS < nchunk; any = any || need[j]; }
-    if (!any) return;
-    if (first_wait > 0) {                          // polls that arrive before the data delay the stores to the same lines
-        const long long t0 = clock64();
-        while (clock64() - t0 < first_wait) {}
+    const int pch = x.wid * PLN + x.lane;
+    bool needp = part != nullptr && x.lane < PLN && 2 * pch < x.NW();
+    const bool hasp = needp;
+    uint4 pv = make_uint4(0u, 0u, 0u, 0u);
+    if (any || needp) {
+        if (first_wait > 0) {                          // polls that arrive before the data delay the stores to the same lines
+            const long long t0 = clock64();
+            while (clock64() - t0 < first_wait) {}
+        }
+        uint32_t spins = 0;
+        for (;;) {
+#pragma unroll
+            for (int j = 0; j < NJ; ++j)
+                if (need[j]) v[j] = x_ld128(buf + 4 * (tix + j * THREADS));
+            if (needp) pv = x_ld128(part + 4 * pch);
+            bool all = true;
+#pragma unroll
+            for (int j = 0; j < NJ; ++j)
+                if (need[j]) { need[j] = !chunk_ok(v[j]); all = all && !need[j]; }
+            if (needp) { needp = pv.y == SENT || (2 * pch + 1 < x.NW() && pv.w == SENT); all = all && !needp; }
+            if (all) break;
+            if (++spins > SPIN_LIMIT || *x.dead) { poll_fail(x); break; }
+        }
     }
-    uint32_t spins = 0;
-    for (;;) {
-#pragma unroll
-        for (int j = 0; j < NJ; ++j)
-            if (need[j]) v[j] = x_ld128(buf + 4 * (tix + j * THREADS));
-        bool all = true;
-#pragma unroll
-        for (int j = 0; j < NJ; ++j)
-            if (need[j]) { need[j] = !chunk_ok(v[j]); all = all && !need[j]; }
-        if (all) break;
-        if (++spins > SPIN_LIMIT || *x.dead) { poll_fail(x); break; }
+    if (part != nullptr) {                             // warp-uniform
+        double ps = 0.0;
+        if (hasp) {
+            ps = __hiloint2double((int)pv.y, (int)pv.x);
+            if (2 * pch + 1 < x.NW()) ps += __hiloint2double((int)pv.w, (int)pv.z);
+        }
+        static_assert(PLN == 8, "three shuffle steps");
+        ps += __shfl_xor_sync(0xffffffffu, ps, 1);
+        ps += __shfl_xor_sync(0xffffffffu, ps, 2);
+        ps += __shfl_xor_sync(0xffffffffu, ps, 4);
+        if (x.lane == 0) red_d(x)[x.wid] = ps;
     }
 }
 
-// scratch inside s_red: NWARPS doubles (warp sums of squares)
-template <class S>
-__device__ __forceinline__ double* red_d(const Ctx<S>& x) { return (double*)(x.sm + x.P.s_red); }
 // scalars: [0] amax of the last absmax_quant, [1] scale of the in_proj / LM-head codes, [2] scale of the out_proj codes;
 // behind them the accumulators of the CTA-wide reductions, double-buffered by call parity: uint amax bits [2], int code sums [2]
 template <class S>
@@ -362,6 +400,8 @@ __device__ __forceinline__ int* acc_qs(const Ctx<S>& x) { return (int*)(x.sm + x
 // Writes the codes to xq (plane order unless `canonical`), leaves amax in scal[0] and returns the sum of the codes.
 // The two CTA-wide reductions (max, integer sum: exact in any order) are shared-memory atomics into accumulators that
 // alternate with the call parity `par`; thread 0 clears the other pair between the two barriers.  Two __syncthreads.
+// (Tried: every warp polls a 512-byte array of the workers' own maxima and skips the first barrier -- 2368 warps then hammer
+// four L2 lines and the gathers go from 1.0 k to 9.5 k clocks.)
 template <class S, typename Enum>
 __device__ __forceinline__ int absmax_quant(const Ctx<S>& x, Enum en, int K, bool canonical, int8_t* tap_codes, unsigned& par,
                                           int pl = 0, int pk = -1)
@@ -408,8 +448,10 @@ __device__ __forceinline__ float act_scale(double ss, int K, float eps, float am
     return amax == 0.0f ? 0.0f : fdiv(fmul(amax, rstd), 127.0f);
 }
 
-// ONE warp: the activation scale of the vector whose amax is in scal[0], from the NWARPS warp sums of squares in red_d
-// (the embedding: every CTA has the whole vector).  Valid in lane 0.
+// ONE warp, behind the barriers of absmax_quant: the activation scale of the vector whose amax is in scal[0], from the NWARPS
+// warp sums of squares in red_d (any tree: DESIGN.md 5.3).  The embedding: every CTA holds the whole vector; U and G: the scale
+// CTA gathered the workers' partial sums with the data (hop_gather) and the scale travels on as one word of the A / T part.
+// Valid in lane 0.
 template <class S>
 __device__ __forceinline__ float scale_from_warps(const Ctx<S>& x, int K)
 {
@@ -419,38 +461,10 @@ __device__ __forceinline__ float scale_from_warps(const Ctx<S>& x, int K)
     return act_scale(s, K, x.P.eps, scal(x)[0]);
 }
 
-// ONE warp of service CTA 0, off the critical path: gather the NW fp64 partial sums of squares the workers published beside
-// their U / G slots (8-byte elements validated by their high word), add them (any tree: DESIGN.md 5.3) and return the
-// activation scale (valid in lane 0); amax comes from scal[0] (absmax_quant of the same vector; a CTA barrier lies between).
-// The scale travels to the workers as one more word of the A / T part.
-template <class S>
-__device__ __forceinline__ float scale_side(const Ctx<S>& x, const uint32_t* part, int K)
-{
-    double s = 0.0;
-    const int nchunk = (x.NW() + 1) >> 1;
-    for (int ch0 = 0; ch0 < nchunk; ch0 += 64) {          // two chunks per lane in flight
-        const int ca = ch0 + x.lane, cb = ch0 + 32 + x.lane;
-        uint4 va = make_uint4(0u, 0u, 0u, 0u), vb = va;
-        bool na = ca < nchunk, nb = cb < nchunk;
-        const bool ha = na, hb = nb;
-        uint32_t spins = 0;
-        while (na || nb) {
-            if (na) va = x_ld128(part + 4 * ca);
-            if (nb) vb = x_ld128(part + 4 * cb);
-            if (na) na = va.y == SENT || (2 * ca + 1 < x.NW() && va.w == SENT);
-            if (nb) nb = vb.y == SENT || (2 * cb + 1 < x.NW() && vb.w == SENT);
-            if (++spins > SPIN_LIMIT || *x.dead) { poll_fail(x); break; }
-        }
-        if (ha) { s += __hiloint2double((int)va.y, (int)va.x); if (2 * ca + 1 < x.NW()) s += __hiloint2double((int)va.w, (int)va.z); }
-        if (hb) { s += __hiloint2double((int)vb.y, (int)vb.x); if (2 * cb + 1 < x.NW()) s += __hiloint2double((int)vb.w, (int)vb.z); }
-    }
-    s = warp_sum(s);
-    return act_scale(s, K, x.P.eps, scal(x)[0]);
-}
-
 // the elements a thread holds after gathering a slot-structured mailbox part (U or G): chunk ci = tid + j*THREADS is
 // piece ci % pps of slot ci / pps; slot g carries elements starts[g] .. starts[g+1]-1
-template <int NJ>
+// DENSE: every slot is full and as long as its owner's element count: chunk ci holds the elements 4 ci .. 4 ci + 3
+template <int NJ, bool DENSE>
 struct SlotEnum {
     const uint4 (&v)[NJ];
     const int* starts;
@@ -462,9 +476,13 @@ struct SlotEnum {
         for (int j = 0; j < NJ; ++j) {
             const int ci = tid + j * THREADS;
             if (ci < nslots * pps) {
-                const int g = ci / pps, piece = ci - g * pps;
-                const int k0 = starts[g] + 4 * piece;
-                if (k0 < starts[g + 1]) f(k0, v[j]);
+                if (DENSE) {
+                    f(4 * ci, v[j]);
+                } else {
+                    const int g = ci / pps, piece = ci - g * pps;
+                    const int k0 = starts[g] + 4 * piece;
+                    if (k0 < starts[g + 1]) f(k0, v[j]);
+                }
             }
         }
     }
@@ -689,8 +707,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         fence_mbar_init();
     }
     __syncthreads();
-    const int ch0 = service ? 0 : chs[c], nch = service ? 0 : chs[c + 1] - ch0;
-    const int or0 = service ? 0 : ors[c], nor = service ? 0 : ors[c + 1] - or0;
+    constexpr bool kEven = Ctx<S>::kEven;
+    const int ch0 = service ? 0 : (kEven ? c * Ctx<S>::kNch : chs[c]), nch = service ? 0 : (kEven ? Ctx<S>::kNch : chs[c + 1] - ch0);
+    const int or0 = service ? 0 : (kEven ? c * Ctx<S>::kNor : ors[c]), nor = service ? 0 : (kEven ? Ctx<S>::kNor : ors[c + 1] - or0);
     const int v0 = (int)(((long long)c * P.vocab) / x.G()), v1 = (int)(((long long)(c + 1) * P.vocab) / x.G());
     const int n_lm_items = (v1 - v0 + P.lm_rows_item - 1) / P.lm_rows_item;
     const int n_items = P.L + n_lm_items;
@@ -800,13 +819,18 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             //      layers' scales are published as soon as their U has been gathered (end of the loop body) ----
             if (sv == 0 && wid == SCALE_WARP && l == 0) word_store(x, rec, P.x_A, x.n_early(), M_A, __float_as_uint(scal(x)[1]));
             DFSSM_STAMP(l, 2);
+            x.gstamp(l, 29);
             // ---- gather G, codes of the whole gated vector ----
             int qsum_g;
             {
                 uint4 vg[NJ_G];
-                hop_gather<NJ_G>(x, rec + P.x_G, NW * x.g_slot() / 4, vg, tid);
+                hop_gather<NJ_G>(x, rec + P.x_G, NW * x.g_slot() / 4, vg, tid, 0, sv == 0 ? rec + P.x_PG : nullptr);
                 DFSSM_STAMP(l, 6);
-                qsum_g = absmax_quant(x, SlotEnum<NJ_G>{ vg, chs, tid, NW, x.g_slot() >> 2 }, x.d_inner(), false, nullptr, par, l, 16);
+                qsum_g = absmax_quant(x, SlotEnum<NJ_G, Ctx<S>::kDenseG>{ vg, chs, tid, NW, x.g_slot() >> 2 }, x.d_inner(), false, nullptr, par, l, 16);
+            }
+            if (sv == 0 && wid == SCALE_WARP) {     // the scale of the gated codes travels with T
+                const float sc = scale_from_warps(x, x.d_inner());
+                word_store(x, rec, P.x_T, x.i_sg(), M_T, __float_as_uint(sc));
             }
             (void)qsum_g;
             DFSSM_STAMP(l, 7);
@@ -815,10 +839,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 const int q = ts + k * NT, part = q % x.tsplit();
                 const int t = trow_dot(stage + P.sc_tout + (size_t)k * tbytes, tbytes, xq + (size_t)part * tbytes, lane);
                 word_store(x, rec, P.x_T, q, M_T, (uint32_t)t ^ IBIAS);
-            }
-            if (sv == 0 && wid == SCALE_WARP) {     // the scale of the gated codes travels with T
-                const float sc = scale_side(x, rec + P.x_PG, x.d_inner());
-                word_store(x, rec, P.x_T, x.i_sg(), M_T, __float_as_uint(sc));
             }
             DFSSM_STAMP(l, 8);
             // ---- reset own words of the next step's record of this layer (this CTA is idle until U arrives) ----
@@ -850,6 +870,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 }
             }
             DFSSM_STAMP(l, 2);
+            x.gstamp(l, 30);
             // ---- gather A: accumulators of all B|C|dt rows and t_in;  v_j = a_s[j] * float(t_j) ----
             {
                 uint4 va[NJ_A];
@@ -879,6 +900,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             }
             __syncthreads();
             DFSSM_STAMP(l, 3);
+            x.gstamp(l, 29);
             const float s_act = scal(x)[1];
             // ---- S3 stage 2 + S4 conv + dt softplus: own z|x rows and ALL B|C rows (+ own dt) ----
             {
@@ -1062,7 +1084,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 uint4 vg[NJ_G];
                 hop_gather<NJ_G>(x, rec + P.x_G, NW * x.g_slot() / 4, vg, tid, DFSSM_WG);
                 DFSSM_STAMP(l, 6);
-                qsum_g = absmax_quant(x, SlotEnum<NJ_G>{ vg, chs, tid, NW, x.g_slot() >> 2 }, x.d_inner(), false,
+                qsum_g = absmax_quant(x, SlotEnum<NJ_G, Ctx<S>::kDenseG>{ vg, chs, tid, NW, x.g_slot() >> 2 }, x.d_inner(), false,
                                       (tp && c == 0) ? (int8_t*)(tp + P.tl.off[9]) : nullptr, par, l, 16);
             }
             DFSSM_STAMP(l, 7);
@@ -1153,14 +1175,15 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
         // ---- gather U, S1 of the next layer (or S8's norm) in every CTA ----
         {
             uint4 vu[NJ_U];
-            hop_gather<NJ_U>(x, rec + P.x_U, NW * x.u_slot() / 4, vu, tid, service ? 0 : DFSSM_WU);
+            hop_gather<NJ_U>(x, rec + P.x_U, NW * x.u_slot() / 4, vu, tid, service ? 0 : DFSSM_WU, (service && sv == 0) ? rec + P.x_PU : nullptr);
             DFSSM_STAMP(l, 11);
+            x.gstamp(l, 28);
             uint8_t* tpn = (taps_on && c == 0 && l + 1 < P.L) ? P.taps + (size_t)(l + 1) * P.tap_lstride : nullptr;
-            qsum = absmax_quant(x, SlotEnum<NJ_U>{ vu, ors, tid, NW, x.u_slot() >> 2 }, x.d_model(), l == P.L - 1,
+            qsum = absmax_quant(x, SlotEnum<NJ_U, Ctx<S>::kDenseU>{ vu, ors, tid, NW, x.u_slot() >> 2 }, x.d_model(), l == P.L - 1,
                                 tpn ? (int8_t*)(tpn + P.tl.off[0]) : nullptr, par, l, 20);
             // the scale of these codes is made by the scale CTA and travels with the next layer's A; the LM head gets it through T
             if (service && sv == 0 && wid == SCALE_WARP) {
-                const float sc = scale_side(x, rec + P.x_PU, x.d_model());
+                const float sc = scale_from_warps(x, x.d_model());
                 if (l == P.L - 1) word_store(x, rec, P.x_T, x.i_slm(), M_T, __float_as_uint(sc), GRID);     // every CTA reads it
                 else word_store(x, rec + rec_words, P.x_A, x.n_early(), M_A, __float_as_uint(sc));
             }

@@ -15,13 +15,13 @@ constexpr size_t SMEM_LIMIT = 232448 - 1024;    // 227 KB opt-in maximum minus t
 inline uint32_t up32(uint32_t x, uint32_t a) { return (x + a - 1) / a * a; }
 
 // workers of a shape: 128 whenever that deals whole groups of 4 to every worker (all BASELINE shapes), else the count in
-// [116, 132] with the least sign-row work on the busiest worker
+// [112, 128] with the least sign-row work on the busiest worker
 inline int pick_workers(const Dims& d)
 {
     if ((d.d_inner / 4) % NW_CT == 0 || d.d_inner / 4 < NW_CT) return NW_CT;
     int best = NW_CT;
     long long best_cost = -1;
-    for (int nw = 132; nw >= 116; nw -= 4) {
+    for (int nw = 128; nw >= 112; nw -= 4) {         // <= 128: a warp polls the workers' maxima with one 16-byte chunk per lane
         const long long cost = (long long)own_max(d.d_inner, nw) * 2 * (d.d_model / 32) + (long long)own_max(d.d_model, nw) * (d.d_inner / 32);
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = nw; }
     }
