@@ -149,12 +149,12 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------
 # the oracle, as it stands, on the host cores (cpu_baseline leg and --impl reference)
 # ---------------------------------------------------------------------------------------------
-def time_oracle(s, blob, cfg_idx: int, batch: int, budget_s: float, max_steps: int, n_prompt: int = 2):
+def time_oracle(s, blob, cfg_idx: int, batch: int, budget_s: float, max_steps: int, n_prompt: int = 2, threads: int = 0):
     """Feed `n_prompt` prompt tokens (untimed), then time greedy decode steps until the budget or
     max_steps is reached.  Returns (tokens/s, steps, seconds, threads)."""
     import oracle
     oracle.build()
-    oracle.set_threads(n_cores())
+    oracle.set_threads(threads if threads > 0 else n_cores())
     m = oracle.OracleModel(blob, batch)
     prompt = ds.token_batch(s.vocab, n_prompt, seed=cfg_idx, batch=batch)
     for t in range(n_prompt):
@@ -276,6 +276,10 @@ def run_ours(args, s, blob):
         m.step(prompt_dev[t])
     if args.warmup == 0:
         m.step(prompt_dev[0])
+    # at least 32 warm-up steps before anything is timed (greedy steps beyond the W prompt steps, untimed)
+    extra_warmup = max(0, 32 - max(args.warmup, 1))
+    for _ in range(extra_warmup):
+        m.step(nxt)
     barrier()
     sampler = ClockSampler(local)
     if rank == 0:
@@ -291,6 +295,18 @@ def run_ours(args, s, blob):
     barrier()
     ms = e0.elapsed_time(e1)
     launches = m.launches_per_step(B) * args.steps
+    # best and median of 5 repetitions of the same K steps (the first one is the reported value)
+    rep_ms = [ms]
+    for _ in range(max(0, args.reps - 1)):
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        with torch.cuda.stream(m.stream):
+            r0.record()
+            for _ in range(args.steps):
+                m.step(nxt)
+            r1.record()
+        barrier()
+        rep_ms.append(r0.elapsed_time(r1))
 
     # ---- end-to-end leg: host buffers through dfssm_step_host, copies inside the timed region ----
     tok_h = np.ascontiguousarray(m.next_tokens()[:B].cpu().numpy(), np.int32)
@@ -314,6 +330,7 @@ def run_ours(args, s, blob):
     barrier()
 
     ms, e2e_s = max_over_ranks([ms, e2e_s], dist, "cuda")
+    rep_ms = max_over_ranks(rep_ms, dist, "cuda")
 
     if rank != 0:
         if dist is not None:
@@ -333,9 +350,10 @@ def run_ours(args, s, blob):
     dom = max(kt, key=lambda k: kt[k])
     per_launch_us = kt[dom] / max(1, counts.get(dom, 1))
     achieved = kb[dom] / (per_launch_us * 1e-6) / 1e9 if per_launch_us > 0 else 0.0
+    traffic, traffic_src = ncu_traffic(args.config, B, dom)
     roofline = {
         "bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-        "frac": achieved / peak, "traffic": TRAFFIC_NCU.get((args.config, B, dom)), "peak_source": peak_src,
+        "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
         "bytes_per_launch": kb[dom], "us_per_launch": per_launch_us,
         "whole_step": {"algorithmic_bytes_per_step": ab["total"], "bj_formula_bytes_per_step": ab["bj_formula"],
                        "achieved_GBps": step_gbs, "frac_of_measured": step_gbs / peak,
@@ -347,12 +365,18 @@ def run_ours(args, s, blob):
     cpu_baseline = None
     if world == 1 and not args.no_cpu_baseline:
         v, n, dt, thr = time_oracle(s, blob, args.config, B, budget_s=15.0, max_steps=64)
+        v1, n1, dt1, _ = time_oracle(s, blob, args.config, B, budget_s=6.0, max_steps=8, threads=1)
         cpu_baseline = {"value": v, "unit": UNIT, "cores": thr, "kind": "oracle",
-                        "sample": f"{n} greedy decode steps of the same workload after 2 prompt steps ({dt:.1f} s)"}
+                        "sample": f"{n} greedy decode steps of the same workload after 2 prompt steps ({dt:.1f} s)",
+                        "single_thread": {"value": v1, "unit": UNIT, "cores": 1, "sample": f"{n1} steps ({dt1:.1f} s)"}}
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None,       # BASELINE.md holds no published number for this metric on this workload (the paper's are A100, trained, r16)
+        "repeats": {"n": len(rep_ms), "steps_each": args.steps, "best_ms_per_step": min(rep_ms) / args.steps,
+                    "median_ms_per_step": statistics.median(rep_ms) / args.steps, "extra_warmup_steps": extra_warmup},
+        "speedup_vs_cpu_baseline": (value / cpu_baseline["value"]) if cpu_baseline else None,
         "dtype": "int8 x {-1,+1} -> int32; fp32 state", "data": "synthetic",
         "config": {"workload": workload_name(args.config, B), "seed": args.config, "batch_per_gpu": B,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
@@ -370,17 +394,42 @@ def run_ours(args, s, blob):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
-# captures (profiles/r01_traffic.csv: config,batch,kernel,dram_bytes_per_launch); None for a workload that was not captured
-TRAFFIC_NCU = {}
-try:
-    _t = ROOT / "profiles" / "r01_traffic.csv"
-    if _t.exists():
-        for _line in _t.read_text().splitlines()[1:]:
-            _f = _line.split(",")
-            if len(_f) >= 4:
-                TRAFFIC_NCU[(int(_f[0]), int(_f[1]), _f[2].strip())] = int(_f[3])
-except Exception:
-    TRAFFIC_NCU = {}
+# captures (profiles/r02_traffic.csv: config,batch,kernel,dram_bytes_per_launch,commit).  NOT measured by this run: the
+# value is reported only while no commit after the one it was captured at touches the kernels (csrc/); on a box without
+# the git history (gpurun snapshots) that cannot be checked and the source string says so.
+def ncu_traffic(cfg_idx: int, batch: int, kernel: str):
+    t = ROOT / "profiles" / "r02_traffic.csv"
+    if not t.exists():
+        return None, "no capture committed"
+    row = None
+    for line in t.read_text().splitlines()[1:]:
+        f = [x.strip() for x in line.split(",")]
+        if len(f) >= 5 and (int(f[0]), int(f[1]), f[2]) == (cfg_idx, batch, kernel):
+            row = f
+    if row is None:
+        return None, "no capture of this workload"
+    src = f"profiles/r02_traffic.csv (ncu --set full capture at commit {row[4][:12]}, not this run)"
+    try:
+        res = subprocess.run(["git", "-C", str(ROOT), "rev-list", f"{row[4]}..HEAD", "--", "paper_2606_10932_b200/csrc"],
+                             capture_output=True, text=True, timeout=20)
+        if res.returncode != 0:
+            return int(row[3]), src + "; staleness unchecked (no git history here)"
+        if res.stdout.strip():
+            return None, src + "; STALE: csrc/ changed since, re-capture"
+        return int(row[3]), src
+    except Exception:
+        return int(row[3]), src + "; staleness unchecked (git unavailable)"
+
+
+def respawn_under_torchrun(args) -> int:
+    """`python bench.py --gpus N` without torchrun: start the N replicas ourselves (one process per GPU)."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), str(Path(__file__).resolve()), *sys.argv[1:]]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -392,7 +441,13 @@ def main():
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--batch", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--reps", type=int, default=5, help="repetitions of the K timed steps (the first is the reported value)")
     args = ap.parse_args()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "ours" and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        raise SystemExit(respawn_under_torchrun(args))
+    if args.impl == "ours" and world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: launch with torchrun --nproc-per-node {args.gpus}, or without torchrun")
     if args.impl == "reference" and int(os.environ.get("RANK", "0")) != 0:
         return
     s = ds.shape_for_config(args.config)

@@ -164,7 +164,10 @@ DFSSM_API int dfssm_set_state(dfssm_ctx* ctx, int layer, int seq, const float* s
 DFSSM_API int dfssm_debug_profile(dfssm_ctx* ctx, uint64_t* stamps_host, size_t nbytes, int32_t* dims);
 
 /* Wait for the stream; returns DFSSM_E_TOKEN once if a bad token id was clamped since the last
- * call, DFSSM_E_CUDA on a device fault. */
+ * call, DFSSM_E_CUDA on a device fault or if a step timed out on the device (an exchange between the
+ * CTAs of the persistent kernel, or a tensor-core projection, did not complete within ~0.3 s).  After
+ * such a time-out the recurrent state is half-written: dfssm_step returns DFSSM_E_STATE until
+ * dfssm_reset_state(ctx, -1) has been called. */
 DFSSM_API int dfssm_sync(dfssm_ctx* ctx);
 
 /* Number of kernels of this library that one dfssm_step(batch) launches (graph nodes).  >= 1. */

@@ -65,6 +65,8 @@ def lib() -> C.CDLL:
         "dfo_free": (None, [C.c_void_p]),
         "dfo_set_threads": (None, [C.c_int]),
         "dfo_get_threads": (C.c_int, []),
+        "dfo_set_mode": (None, [C.c_int]),
+        "dfo_get_mode": (C.c_int, []),
         "dfo_enable_taps": (None, [C.c_void_p, C.c_int]),
         "dfo_reset": (None, [C.c_void_p, C.c_int]),
         "dfo_step": (C.c_int, [C.c_void_p, i32p, C.c_int]),
@@ -211,6 +213,20 @@ def argmax(logits):
 def set_threads(n: int) -> int:
     lib().dfo_set_threads(int(n))
     return int(lib().dfo_get_threads())
+
+
+# TEST-ONLY arithmetic modes of the oracle (dfssm_oracle.c): the default is the contract of DESIGN.md section 5
+MODE_CONTRACT, MODE_REVERSED, MODE_F64 = 0, 1, 2
+
+
+def set_mode(mode: int) -> None:
+    """MODE_REVERSED: every binary64 reduction summed in reversed order (must not change a bit);
+    MODE_F64: the "float64 everything" diagnostic (departs from the contract within a few steps)."""
+    lib().dfo_set_mode(int(mode))
+
+
+def get_mode() -> int:
+    return int(lib().dfo_get_mode())
 
 
 def get_threads() -> int:

@@ -20,6 +20,24 @@
 #endif
 
 /* ------------------------------------------------------------------------------------------
+ * Arithmetic mode (TEST-ONLY switch; the default, DFO_MODE_CONTRACT, is the oracle).
+ *   DFO_MODE_CONTRACT  the arithmetic contract of DESIGN.md section 5.
+ *   DFO_MODE_REVERSED  the same contract with every binary64 reduction summed in REVERSED index order:
+ *                      the contract says the result does not depend on the summation tree;
+ *                      tests/test_oracle_model.py checks that on the oracle itself, bit for bit.
+ *   DFO_MODE_F64       diagnostic ("float64 everything"): every expression is evaluated in
+ *                      binary64 with libm transcendentals and rounded once where the contract stores a binary32
+ *                      value (activations, state).  A perfectly reasonable implementation -- and it departs from
+ *                      the contract mode within a few steps because a quantiser input that differs in the last bit
+ *                      eventually rounds the other way.  It exists to show why the contract is needed.
+ * ------------------------------------------------------------------------------------------ */
+static int g_mode = DFO_MODE_CONTRACT;
+void dfo_set_mode(int mode) { g_mode = (mode == DFO_MODE_REVERSED || mode == DFO_MODE_F64) ? mode : DFO_MODE_CONTRACT; }
+int dfo_get_mode(void) { return g_mode; }
+/* index of the i-th term of a reduction over n terms */
+static int red_idx(int i, int n) { return g_mode == DFO_MODE_REVERSED ? n - 1 - i : i; }
+
+/* ------------------------------------------------------------------------------------------
  * Specified transcendentals.  Fixed sequences of binary32 operations.
  * ------------------------------------------------------------------------------------------ */
 
@@ -125,6 +143,12 @@ float dfo_half_to_float(uint16_t h)
  * ------------------------------------------------------------------------------------------ */
 
 /* S0: int8 per-row embedding, "quantized to int8 per-row", tied with the head */
+static float silu_mode(float x)
+{
+    if (g_mode == DFO_MODE_F64) return (float)((double)x / (1.0 + exp(-(double)x)));
+    return dfo_siluf(x);
+}
+
 void dfo_embed(const int8_t* E_row, float e_s, int d, float* u)
 {
     for (int k = 0; k < d; ++k) u[k] = e_s * (float)E_row[k];
@@ -137,9 +161,10 @@ void dfo_norm_quant(const float* v, const float* w, int d, float eps,
                     int8_t* q, float* s, float* rstd_out, float* amax_out)
 {
     double ss = 0.0;
-    for (int k = 0; k < d; ++k) ss += (double)v[k] * (double)v[k];
+    for (int i = 0; i < d; ++i) { const int k = red_idx(i, d); ss += (double)v[k] * (double)v[k]; }
     float ms = (float)(ss / (double)d);
     float rstd = 1.0f / sqrtf(ms + eps);
+    if (g_mode == DFO_MODE_F64) rstd = (float)(1.0 / sqrt(ss / (double)d + (double)eps));
     float amax = 0.0f;
     for (int k = 0; k < d; ++k) {
         float a = fabsf(v[k] * w[k]);
@@ -152,11 +177,13 @@ void dfo_norm_quant(const float* v, const float* w, int d, float eps,
         float inv = 127.0f / amax;
         for (int k = 0; k < d; ++k) {
             float f = rintf((v[k] * w[k]) * inv);     /* ties to even */
+            if (g_mode == DFO_MODE_F64) f = (float)rint((double)v[k] * (double)w[k] * (127.0 / (double)amax));
             if (f > 127.0f) f = 127.0f;
             if (f < -127.0f) f = -127.0f;
             q[k] = (int8_t)f;
         }
         *s = (amax * rstd) / 127.0f;
+        if (g_mode == DFO_MODE_F64) *s = (float)((double)amax * (1.0 / sqrt(ss / (double)d + (double)eps)) / 127.0);
     }
     if (rstd_out) *rstd_out = rstd;
     if (amax_out) *amax_out = amax;
@@ -199,11 +226,16 @@ void dfo_proj_epilogue(const int32_t* acc, const int32_t* t, const uint16_t* row
     for (int j = 0; j < r; ++j) v[j] = a_s[j] * (float)t[j];
     for (int i = 0; i < rows; ++i) {
         double lo = 0.0;
-        for (int j = 0; j < r; ++j) lo += (double)(float)B[(size_t)i * r + j] * (double)v[j];
+        for (int jj = 0; jj < r; ++jj) { const int j = red_idx(jj, r); lo += (double)(float)B[(size_t)i * r + j] * (double)v[j]; }
         float lo_f = (float)lo;
         float m1 = dfo_half_to_float(row_scale_f16[i]) * (float)acc[i];
         float m2 = b_s[i] * lo_f;
         out[i] = s_x * (m1 + m2);
+        if (g_mode == DFO_MODE_F64) {
+            double lod = 0.0;
+            for (int j = 0; j < r; ++j) lod += (double)B[(size_t)i * r + j] * ((double)a_s[j] * (double)t[j]);
+            out[i] = (float)((double)s_x * ((double)dfo_half_to_float(row_scale_f16[i]) * (double)acc[i] + (double)b_s[i] * lod));
+        }
     }
     free(v);
 }
@@ -223,7 +255,9 @@ void dfo_conv_step(float* state, const float* w, const float* bias, const float*
         state[3 * c + 0] = s1;
         state[3 * c + 1] = s2;
         state[3 * c + 2] = xn;
-        out[c] = dfo_siluf(o);
+        if (g_mode == DFO_MODE_F64)
+            o = (float)((double)bias[c] + (double)w[4 * c + 0] * s0 + (double)w[4 * c + 1] * s1 + (double)w[4 * c + 2] * s2 + (double)w[4 * c + 3] * xn);
+        out[c] = silu_mode(o);
     }
 }
 
@@ -236,7 +270,7 @@ void dfo_ssm_step(float* H, const float* x, const float* Bv, const float* Cv, co
     const int hpg = nheads / ngroups;
 #pragma omp parallel for schedule(static)
     for (int h = 0; h < nheads; ++h) {
-        const float dA = dfo_sp_expf(dt[h] * A[h]);
+        const float dA = g_mode == DFO_MODE_F64 ? (float)exp((double)dt[h] * (double)A[h]) : dfo_sp_expf(dt[h] * A[h]);
         const float* Bg = Bv + (size_t)(h / hpg) * d_state;
         const float* Cg = Cv + (size_t)(h / hpg) * d_state;
         for (int p = 0; p < headdim; ++p) {
@@ -244,12 +278,15 @@ void dfo_ssm_step(float* H, const float* x, const float* Bv, const float* Cv, co
             const float dtx = dt[h] * xv;
             float* Hr = H + ((size_t)h * headdim + p) * d_state;
             double a = 0.0;
-            for (int n = 0; n < d_state; ++n) {
+            if (g_mode == DFO_MODE_REVERSED) a += (double)D[h] * (double)xv;      /* the last term first */
+            for (int i = 0; i < d_state; ++i) {
+                const int n = red_idx(i, d_state);
                 float hn = fmaf(dA, Hr[n], dtx * Bg[n]);
+                if (g_mode == DFO_MODE_F64) hn = (float)((double)dA * (double)Hr[n] + (double)dt[h] * (double)xv * (double)Bg[n]);
                 Hr[n] = hn;
                 a += (double)Cg[n] * (double)hn;
             }
-            a += (double)D[h] * (double)xv;
+            if (g_mode != DFO_MODE_REVERSED) a += (double)D[h] * (double)xv;
             y[h * headdim + p] = (float)a;
         }
     }
@@ -258,7 +295,7 @@ void dfo_ssm_step(float* H, const float* x, const float* Bv, const float* Cv, co
 /* S6: norm(y * silu(z)) -- gate first */
 void dfo_gate(const float* y, const float* z, int n, float* g)
 {
-    for (int i = 0; i < n; ++i) g[i] = y[i] * dfo_siluf(z[i]);
+    for (int i = 0; i < n; ++i) g[i] = g_mode == DFO_MODE_F64 ? (float)((double)y[i] * ((double)z[i] / (1.0 + exp(-(double)z[i])))) : y[i] * dfo_siluf(z[i]);
 }
 
 /* S8: tied int8 LM head on the quantised final hidden (R16) */
@@ -513,6 +550,11 @@ static void step_one(dfo_model* m, int s, int32_t tok)
         for (int h = 0; h < m->nheads; ++h) {                                            /* S5 */
             dt[h] = dfo_sp_softplusf(dt_raw[h] + L->dt_bias[h]);
             An[h] = -dfo_sp_expf(L->A_log[h]);
+            if (g_mode == DFO_MODE_F64) {
+                const double xx = (double)dt_raw[h] + (double)L->dt_bias[h];
+                dt[h] = (float)(xx > 20.0 ? xx : log1p(exp(xx)));
+                An[h] = (float)(-exp((double)L->A_log[h]));
+            }
         }
         TAP(DFO_TAP_DT, dt, 4 * (size_t)m->nheads);
         dfo_ssm_step(dfo_ssm_state(m, l, s), xbc, xbc + di, xbc + di + gs, dt, An, L->D,

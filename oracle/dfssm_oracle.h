@@ -110,6 +110,11 @@ float* dfo_ssm_state(dfo_model*, int layer, int seq);   /* [nheads][headdim][d_s
 float* dfo_conv_state(dfo_model*, int layer, int seq);  /* [conv_dim][3] */
 int    dfo_shape(const dfo_model*, int32_t out[12]);    /* the header's 9 ints + nheads,d_in_proj,conv_dim */
 
+/* TEST-ONLY arithmetic mode switch (see dfssm_oracle.c): the default is the contract. */
+enum { DFO_MODE_CONTRACT = 0, DFO_MODE_REVERSED = 1, DFO_MODE_F64 = 2 };
+void dfo_set_mode(int mode);
+int dfo_get_mode(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -216,6 +216,12 @@ class Model:
         else:
             assert tokens_dev.dtype == self._torch.int32 and tokens_dev.is_cuda and tokens_dev.is_contiguous()
             ptr, n = tokens_dev.data_ptr(), (int(batch) if batch is not None else tokens_dev.numel())
+            a0 = self.arena.data_ptr()
+            if not (a0 <= ptr < a0 + self.arena.numel()):
+                # a caller tensor made on torch's current stream: the library copies it on ITS stream, so order that stream
+                # behind the producer and keep the block from being reused before the copy has run
+                self.stream.wait_stream(self._torch.cuda.current_stream(self.device))
+                tokens_dev.record_stream(self.stream)
         self._check(self._L.dfssm_step(self._h, C.c_void_p(ptr), n))
         self.batch = n
 

@@ -326,6 +326,19 @@ __device__ __forceinline__ constexpr int mbox_count(int n, int M) { return (n + 
 // ------------------------------------------------------------------------------------------------
 // exchange: gather a self-validating buffer
 // ------------------------------------------------------------------------------------------------
+// spin on ONE exchange word until it has been written
+template <class S>
+__device__ __forceinline__ uint32_t poll_word(const Ctx<S>& x, const uint32_t* w)
+{
+    uint32_t v, spins = 0;
+    for (;;) {
+        asm volatile("ld.relaxed.gpu.global.b32 %0, [%1];" : "=r"(v) : "l"(w) : "memory");
+        if (v != SENT) break;
+        if (++spins > SPIN_LIMIT || *x.dead) { poll_fail(x); break; }
+    }
+    return v;
+}
+
 // scratch inside s_red: NWARPS doubles (warp sums of squares)
 template <class S>
 __device__ __forceinline__ double* red_d(const Ctx<S>& x) { return (double*)(x.sm + x.P.s_red); }
@@ -799,7 +812,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             // ---- in_proj: B|C|dt sign rows and LoRA-down rows dealt to this CTA; raw int32 results are published ----
             {
                 const uint32_t* bits = (const uint32_t*)(stage + P.sc_sign);
-                for (int k = wid; k < n_sig + n_lin; k += NWARPS) {
+                for (int k0 = wid; k0 < n_sig + n_lin; k0 += NWARPS) {
+                    // the LoRA-down rows go first (the workers need t_in before the accumulators of the B|C|dt rows)
+                    const int k = k0 < n_lin ? n_sig + k0 : k0 - n_lin;
                     int val, idx;
                     if (k < n_sig) {
                         const uint32_t* const rowp[1] = { bits + (size_t)k * x.Win() };
@@ -871,14 +886,18 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
             }
             DFSSM_STAMP(l, 2);
             x.gstamp(l, 30);
-            // ---- gather A: accumulators of all B|C|dt rows and t_in;  v_j = a_s[j] * float(t_j) ----
+            // ---- gather A, first part: t_in and the scale (the chunks from word n_bcdt on; the task CTAs publish them first);
+            //      v_j = a_s[j] * float(t_j).  The accumulators of the B|C|dt rows are polled word by word by the thread that
+            //      finishes the row, behind its LoRA sum: they may arrive a whole epilogue later without anybody waiting ----
+            const uint32_t* recA = rec + mbox(M_A) + P.x_A;
             {
-                uint4 va[NJ_A];
-                hop_gather<NJ_A>(x, rec + mbox(M_A) + P.x_A, (x.n_A() + 3) / 4, va, rtid);
+                uint4 va[1];
+                const int c0 = x.n_bcdt() / 4, nc1 = (x.n_A() + 3) / 4 - c0;
+                hop_gather<1>(x, recA + 4 * c0, nc1, va, rtid);
                 const float* a_s = (const float*)(blk + P.b_as_in);
-#pragma unroll
-                for (int j = 0; j < NJ_A; ++j) {
-                    const int e0 = 4 * (rtid + j * THREADS);
+                if (rtid < nc1) {
+                    const int j = 0;
+                    const int e0 = 4 * (c0 + rtid);
                     const uint32_t w[4] = { va[j].x, va[j].y, va[j].z, va[j].w };
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
@@ -887,13 +906,10 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                             scal(x)[1] = __uint_as_float(w[i]);
                             if (tp && c == 0) *(float*)(tp + P.tl.off[1]) = __uint_as_float(w[i]);
                         }
-                        if (e < x.n_early()) {
+                        if (e >= x.n_bcdt() && e < x.n_early()) {
                             const int val = (int)(w[i] ^ IBIAS);
-                            if (e < x.n_bcdt()) s_eacc[e] = val;
-                            else {
-                                s_vin[e - x.n_bcdt()] = (double)fmul(a_s[e - x.n_bcdt()], (float)val);
-                                if (tp && c == 0) ((int32_t*)(tp + P.tl.off[3]))[e - x.n_bcdt()] = val;
-                            }
+                            s_vin[e - x.n_bcdt()] = (double)fmul(a_s[e - x.n_bcdt()], (float)val);
+                            if (tp && c == 0) ((int32_t*)(tp + P.tl.off[3]))[e - x.n_bcdt()] = val;
                         }
                     }
                 }
@@ -943,7 +959,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     if (sub != 0 || !valid) continue;
                     const float scale = own ? ((const float*)(stage + P.c_in_scale))[slot] : ((const float*)(blk + P.b_escale))[e];
                     const float bsv = own ? ((const float*)(stage + P.c_in_bs))[slot] : ((const float*)(blk + P.b_ebs))[e];
-                    const int acc = own ? s_acc_in[slot] : s_eacc[e];
+                    const int acc = own ? s_acc_in[slot] : (int)(poll_word(x, recA + e) ^ IBIAS);
                     const float lo = (float)lo0;
                     const float val = fmul(s_act, fadd(fmul(scale, (float)acc), fmul(bsv, lo)));
                     int row;                       // canonical in_proj row (for the taps)

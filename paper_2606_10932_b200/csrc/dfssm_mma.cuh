@@ -136,16 +136,15 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
         {
             const uint32_t parity = (uint32_t)(kc - kc0) & 1u;
             uint32_t spins = 0, ok = 0;
-            while (!ok) {
+            while (!ok && !dead) {      // a thread that timed out keeps going through the loop (same barrier count as the others) without waiting
                 asm volatile(
                     "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                     : "=r"(ok) : "r"(smem_u32(&mbar)), "r"(parity) : "memory");
-                if (!ok && ++spins > SPIN_LIMIT) { dead = true; break; }
+                if (!ok && ++spins > SPIN_LIMIT) dead = true;
             }
-            if (dead) break;
         }
     }
-    if (dead && tid == 0) atomicOr(err, 4);
+    if (dead) atomicOr(err, 4);
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 
     // ---- epilogue: TMEM lane = row of the tile, column = sequence ----
