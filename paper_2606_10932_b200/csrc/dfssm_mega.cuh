@@ -85,13 +85,14 @@ constexpr int NW_CT = 128;                    // workers of the compile-time-sha
 #ifndef DFSSM_MT
 #define DFSSM_MT 1
 #endif
-// clocks a worker waits after publishing G / U before its first poll: polls that reach a line before the data delay the
-// stores to it
+// clocks a worker waits after publishing G / U before its first poll (round 1: polls that reach a line before the data delay
+// the stores to it, 500 clocks paid; with 128-byte-aligned full slots and the resets moved behind the publish: 0 / 250 / 500
+// clocks -> 389.6 / 392.7 / 399.0 us per step, so no wait)
 #ifndef DFSSM_WG
-#define DFSSM_WG 250
+#define DFSSM_WG 0
 #endif
 #ifndef DFSSM_WU
-#define DFSSM_WU 250
+#define DFSSM_WU 0
 #endif
 constexpr int MBOX = DFSSM_MA > DFSSM_MT ? DFSSM_MA : DFSSM_MT;      // small mailboxes allocated per record
 constexpr int M_A = DFSSM_MA, M_T = DFSSM_MT;
@@ -1009,7 +1010,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                 // first half of the CTA: the 2 gs B|C rows, one thread per row (dense tails); second half, at the same time: the
                 // few own rows (dt first: the longest tail; then x, z) with 4 lanes each if they fit one pass, else 2
                 epi(std::integral_constant<int, LPB>{}, 2 * nch, 2 * x.gs(), 1 << 30, 0, 0, THREADS / 2);
-                if (4 * (2 * nch + n_dt) <= THREADS / 2)
+                if constexpr (kEven && !TAPS) {          // the lane count is a compile-time choice: one copy of the epilogue code
+                    constexpr int rows_own = 2 * Ctx<S>::kNch + (Ctx<S>::kNch + S::headdim - 1) / S::headdim + 1;
+                    constexpr int LPO = 4 * rows_own <= THREADS / 2 ? 4 : 2;
+                    epi(std::integral_constant<int, LPO>{}, 0, 2 * nch + n_dt, 2 * nch, 2 * x.gs(), THREADS / 2, THREADS / 2);
+                } else if (4 * (2 * nch + n_dt) <= THREADS / 2)
                     epi(std::integral_constant<int, 4>{}, 0, 2 * nch + n_dt, 2 * nch, 2 * x.gs(), THREADS / 2, THREADS / 2);
                 else
                     epi(std::integral_constant<int, 2>{}, 0, 2 * nch + n_dt, 2 * nch, 2 * x.gs(), THREADS / 2, THREADS / 2);
