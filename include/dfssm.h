@@ -121,9 +121,10 @@ DFSSM_API int dfssm_reset_state(dfssm_ctx* ctx, int seq_index);
 
 /* One decode step for sequences 0..batch-1: tokens_dev[s] is the input token of sequence s
  * (device int32[batch]; it may be the pointer returned by dfssm_next_tokens -- greedy decode
- * without leaving the device).  Async: exactly one launch -- for batch 1 one persistent cooperative
+ * without leaving the device).  Async: for batch 1 exactly one launch of the persistent cooperative
  * kernel (the "mega" path: 148 co-resident CTAs, weights and state prefetched ahead of the layer
- * dependencies), otherwise one CUDA graph of the kernel chain (projections on tcgen05 kind::i8 tiles from batch 16 on) -- unless DFSSM_FLAG_NO_GRAPH or
+ * dependencies), for batch 2..4 one such launch per sequence, otherwise one CUDA graph of the kernel chain
+ * (projections on tcgen05 kind::i8 tiles from batch 16 on) -- unless DFSSM_FLAG_NO_GRAPH or
  * DFSSM_FLAG_TAPS asks for the chain's kernels one by one.  The two paths share the state layout
  * and compute bit-identical results.  Token ids outside [0, vocab) are clamped on the
  * device and a sticky error is raised, reported as DFSSM_E_TOKEN by the next dfssm_sync. */
