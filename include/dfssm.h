@@ -130,6 +130,14 @@ DFSSM_API int dfssm_reset_state(dfssm_ctx* ctx, int seq_index);
  * device and a sticky error is raised, reported as DFSSM_E_TOKEN by the next dfssm_sync. */
 DFSSM_API int dfssm_step(dfssm_ctx* ctx, const int32_t* tokens_dev, int batch);
 
+/* Prefill (the paper feeds prompts in chunks): feed n_tokens >= 1 prompt tokens
+ * (device int32[n_tokens]) of ONE sequence `seq` in [0, max_batch).  Equivalent to n_tokens calls of dfssm_step for that
+ * sequence alone -- bit-identical recurrent state, hidden state, logits and greedy token of the LAST position (readable
+ * through dfssm_logits / dfssm_next_tokens / dfssm_hidden at index seq) -- but the projections run over up to 128 positions at a
+ * time with the weights read once per chunk, and only the conv / state recurrence is serial in the position.  Async.
+ * Shapes whose d_state is not a multiple of 16 (and contexts with DFSSM_FLAG_TAPS) are fed token by token instead (max_batch 1 only). */
+DFSSM_API int dfssm_prefill(dfssm_ctx* ctx, const int32_t* tokens_dev, int n_tokens, int seq);
+
 /* Host-buffer form of the same step (the end-to-end call): copies tokens_host[batch] to the
  * device, runs the step, copies the greedy next tokens to next_host[batch] and, if logits_host is
  * non-null, the logits to logits_host[batch*vocab]; synchronises the stream before returning.

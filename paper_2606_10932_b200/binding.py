@@ -31,7 +31,7 @@ KCLASSES = ("embed", "normquant", "proj_in", "ssm", "proj_out", "epi_out", "lmhe
 
 # every symbol include/dfssm.h declares (tests check the .so exports exactly these)
 EXPORTED_SYMBOLS = (
-    "dfssm_arena_bytes", "dfssm_create", "dfssm_load_weights", "dfssm_reset_state", "dfssm_step",
+    "dfssm_arena_bytes", "dfssm_create", "dfssm_load_weights", "dfssm_reset_state", "dfssm_step", "dfssm_prefill",
     "dfssm_step_host", "dfssm_logits", "dfssm_next_tokens", "dfssm_hidden", "dfssm_debug_tensor",
     "dfssm_get_state", "dfssm_set_state", "dfssm_debug_profile", "dfssm_sync", "dfssm_launches_per_step",
     "dfssm_time_kernels", "dfssm_last_error", "dfssm_destroy",
@@ -118,6 +118,7 @@ def lib() -> C.CDLL:
         "dfssm_load_weights": (C.c_int, [vp, vp, C.c_size_t]),
         "dfssm_reset_state": (C.c_int, [vp, C.c_int]),
         "dfssm_step": (C.c_int, [vp, vp, C.c_int]),
+        "dfssm_prefill": (C.c_int, [vp, vp, C.c_int, C.c_int]),
         "dfssm_step_host": (C.c_int, [vp, i32p, C.c_int, i32p, f32p]),
         "dfssm_logits": (C.c_int, [vp, C.POINTER(vp)]),
         "dfssm_next_tokens": (C.c_int, [vp, C.POINTER(vp)]),
@@ -224,6 +225,14 @@ class Model:
                 tokens_dev.record_stream(self.stream)
         self._check(self._L.dfssm_step(self._h, C.c_void_p(ptr), n))
         self.batch = n
+
+    def prefill(self, tokens_dev, seq: int = 0):
+        """tokens_dev: torch int32 CUDA tensor [n_tokens] of sequence `seq` (dfssm_prefill)."""
+        assert tokens_dev.dtype == self._torch.int32 and tokens_dev.is_cuda and tokens_dev.is_contiguous()
+        self.stream.wait_stream(self._torch.cuda.current_stream(self.device))
+        tokens_dev.record_stream(self.stream)
+        self._check(self._L.dfssm_prefill(self._h, C.c_void_p(tokens_dev.data_ptr()), tokens_dev.numel(), int(seq)))
+        self.batch = max(self.batch, int(seq) + 1)
 
     def step_host(self, tokens_host: np.ndarray, next_host: np.ndarray, logits_host: Optional[np.ndarray] = None):
         assert tokens_host.dtype == np.int32 and next_host.dtype == np.int32

@@ -15,6 +15,7 @@
 #include "dfssm_kernels.cuh"
 #include "dfssm_mega_host.cuh"
 #include "dfssm_mma.cuh"
+#include "dfssm_prefill.cuh"
 
 using namespace dfssm;
 
@@ -25,6 +26,7 @@ inline size_t up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Carve {                 // byte offsets inside the arena
     size_t blob, ssm, conv, pos, u, xq, xqp, sx, qsum, acc, t, g, bcdt, logits, next, tok, err, taps, total;
+    size_t p_tok, p_u, p_xq, p_xqp, p_sx, p_qsum, p_acc, p_t, p_zx, p_xbc, p_dt, p_g;      // prefill: activations of one chunk of positions
     size_t m_chunks, m_schunks, m_blocks, m_x, m_xbytes, m_am, m_prof;      // mega path regions (valid if mega_fit)
     bool mega_fit;
     size_t ssm_elems, ldq, ld_acc;
@@ -154,6 +156,12 @@ Carve carve(const dfssm_config& c)
     v.next = put(B * 4);
     v.tok = put(B * 4);
     v.err = put(16);
+    {
+        const size_t C = prefill::CHUNK;
+        v.p_tok = put(C * 4); v.p_u = put(C * d.d_model * 4); v.p_xq = put(C * v.ldq); v.p_xqp = put(C * v.ldq); v.p_sx = put(C * 4);
+        v.p_qsum = put(C * 4); v.p_acc = put(C * v.ld_acc * 4); v.p_t = put(C * T_STRIDE * 4); v.p_zx = put(C * (size_t)d.d_in_proj * 4);
+        v.p_xbc = put(C * (size_t)d.conv_dim * 4); v.p_dt = put(C * (size_t)d.nheads * 4); v.p_g = put(C * d.d_inner * 4);
+    }
     const size_t sizes[DFSSM_TAP_COUNT] = {
         (size_t)d.d_model, 4, 4 * (size_t)d.d_in_proj, 4 * (size_t)d.r, 4 * (size_t)d.d_in_proj,
         4 * (size_t)d.conv_dim, 4 * (size_t)d.nheads, 4 * (size_t)d.d_inner, 4 * (size_t)d.d_inner,
@@ -546,6 +554,84 @@ int mega_launch(dfssm_ctx* ctx, int seq = 0)
 }  // namespace
 
 // =================================================================================================
+// prefill: one chunk of T <= CHUNK prompt positions of sequence `seq`, layer by layer (dfssm_prefill.cuh)
+// =================================================================================================
+namespace {
+
+bool prefill_supported(const Dims& d) { return d.d_state % prefill::SEQ_LANES == 0 && d.d_state / prefill::SEQ_LANES <= prefill::SEQ_NMAX && d.headdim % prefill::SEQ_PB == 0; }
+
+int prefill_chunk(dfssm_ctx* c, const int32_t* tokens_dev, int T, int seq)
+{
+    dfssm_ctx* ctx = c;
+    const Dims& d = c->dm;
+    const Carve& v = c->cv;
+    cudaStream_t st = c->stream;
+    const size_t B = c->cfg.max_batch;
+    int32_t* tok = at<int32_t>(c, v.p_tok);
+    float* u = at<float>(c, v.p_u);
+    int8_t* xq = at<int8_t>(c, v.p_xq);
+    int8_t* xqp = at<int8_t>(c, v.p_xqp);
+    float* sx = at<float>(c, v.p_sx);
+    int32_t* qsum = at<int32_t>(c, v.p_qsum);
+    int32_t* acc = at<int32_t>(c, v.p_acc);
+    int32_t* t = at<int32_t>(c, v.p_t);
+    float* zx = at<float>(c, v.p_zx);
+    float* xbc = at<float>(c, v.p_xbc);
+    float* dtv = at<float>(c, v.p_dt);
+    float* g = at<float>(c, v.p_g);
+    int32_t* pos = at<int32_t>(c, v.pos) + seq;
+    int* err = at<int>(c, v.err);
+    const int ldq = (int)v.ldq, ld_acc = (int)v.ld_acc;
+    auto proj = [&](const uint32_t* sign, const int8_t* A, int rows, int K) {
+        if (use_mma(c, T, K)) {
+            const int mt = (rows + d.r + mma::TM - 1) / mma::TM, nt = (T + mma::TN - 1) / mma::TN, nchunk = K / mma::KC;
+            int ks = (148 * MMA_CTAS_PER_SM) / (mt * nt);
+            if (ks < 1) ks = 1;
+            if (ks > nchunk) ks = nchunk;
+            mma::k_proj_mma<<<dim3(mt, nt, ks), mma::THREADS, 0, st>>>(sign, A, rows, d.r, K, xq, ldq, T, acc, ld_acc, t, err);
+        } else {
+            k_proj<<<dim3(proj_grid(rows + d.r), (T + PROJ_BT - 1) / PROJ_BT), PROJ_THREADS, proj_smem(K), st>>>(sign, A, rows, d.r, K, xq, xqp, ldq, qsum,
+                                                                                                              T, acc, ld_acc, t);
+        }
+    };
+    CK(cudaMemcpyAsync(tok, tokens_dev, sizeof(int32_t) * (size_t)T, cudaMemcpyDeviceToDevice, st));
+    k_embed<<<dim3((d.d_model + 255) / 256, T), 256, 0, st>>>(tok, c->emb, c->emb_s, d.vocab, d.d_model, u, err);
+    for (int l = 0; l < d.n_layers; ++l) {
+        const LayerW& L = c->layers[l];
+        float* ssm = at<float>(c, v.ssm) + ((size_t)l * B + seq) * v.ssm_elems;
+        float* ring = at<float>(c, v.conv) + ((size_t)l * B + seq) * (size_t)d.conv_dim * 4;
+        k_normquant<<<T, NQ_THREADS, 0, st>>>(u, d.d_model, L.norm_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum, nullptr, 0, 0, 0,
+                                              use_mma(c, T, d.d_model) ? acc : nullptr, ld_acc, t);
+        proj(L.in_sign, L.in_A, d.d_in_proj, d.d_model);
+        prefill::k_pf_epi<<<dim3((d.d_in_proj + prefill::EPI_T - 1) / prefill::EPI_T, T), prefill::EPI_T, 0, st>>>(L, d, acc, ld_acc, t, sx, zx);
+        prefill::k_pf_conv<<<dim3((d.conv_dim + d.nheads + prefill::CONV_T - 1) / prefill::CONV_T, T), prefill::CONV_T, 0, st>>>(L, d, zx, T, ring, pos, xbc,
+                                                                                                                               dtv);
+        prefill::k_pf_ring<<<(d.conv_dim + 255) / 256, 256, 0, st>>>(d, zx, T, ring, pos);
+        prefill::k_pf_ssm<<<d.nheads * (d.headdim / prefill::SEQ_PB), prefill::SEQ_T, 0, st>>>(L, d, zx, xbc, dtv, T, ssm, g);
+        k_normquant<<<T, NQ_THREADS, 0, st>>>(g, d.d_inner, L.gnorm_w, d.d_inner, d.eps, xq, xqp, ldq, sx, qsum, nullptr, 0, 0, 0,
+                                              use_mma(c, T, d.d_inner) ? acc : nullptr, ld_acc, t);
+        proj(L.out_sign, L.out_A, d.d_model, d.d_inner);
+        k_epi_out<<<dim3((d.d_model + EPI_THREADS - 1) / EPI_THREADS, T), EPI_THREADS, 0, st>>>(L, d.d_model, d.r, acc, ld_acc, t, sx, u, nullptr, 0, 0);
+    }
+    // the last position: hidden state, logits and greedy token of the sequence; the conv ring position advances by T
+    const float* u_last = u + (size_t)(T - 1) * d.d_model;
+    float* logits = at<float>(c, v.logits) + (size_t)seq * d.vocab;
+    prefill::k_pf_copy_hidden<<<(d.d_model + 255) / 256, 256, 0, st>>>(u_last, at<float>(c, v.u) + (size_t)seq * d.d_model, d.d_model);
+    k_normquant<<<1, NQ_THREADS, 0, st>>>(u_last, d.d_model, c->normf_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum, nullptr, 0, 0, 0);
+    {
+        const int per = LM_THREADS / 32;
+        int gx = (d.vocab + per - 1) / per;
+        if (gx > 148 * 16) gx = 148 * 16;
+        k_lmhead<<<dim3(gx, 1), LM_THREADS, lm_smem(d.d_model), st>>>(c->emb, c->emb_s, d.vocab, d.d_model, xq, ldq, sx, 1, logits);
+    }
+    k_argmax<<<1, AM_THREADS, 0, st>>>(logits, d.vocab, at<int32_t>(c, v.next) + seq, at<int32_t>(c, v.tok) + seq, pos, T);
+    CK(cudaGetLastError());
+    return DFSSM_OK;
+}
+
+}  // namespace
+
+// =================================================================================================
 // exported C ABI
 // =================================================================================================
 extern "C" {
@@ -724,6 +810,31 @@ int dfssm_step(dfssm_ctx* ctx, const int32_t* tokens_dev, int batch)
     const int rc = get_graph(ctx, batch, &exec);
     if (rc != DFSSM_OK) return rc;
     CK(cudaGraphLaunch(exec, ctx->stream));
+    return DFSSM_OK;
+}
+
+int dfssm_prefill(dfssm_ctx* ctx, const int32_t* tokens_dev, int n_tokens, int seq)
+{
+    if (!ctx || !tokens_dev) return DFSSM_E_ARG;
+    if (!ctx->loaded) return fail(ctx, DFSSM_E_STATE, "dfssm_prefill before dfssm_load_weights");
+    if (n_tokens < 1 || seq < 0 || seq >= ctx->cfg.max_batch) return fail(ctx, DFSSM_E_ARG, "n_tokens %d / seq %d out of range", n_tokens, seq);
+    if (ctx->failed) return fail(ctx, DFSSM_E_STATE, "an earlier step timed out on the device: call dfssm_reset_state(ctx, -1) first");
+    if (ctx->last_batch < seq + 1) ctx->last_batch = seq + 1;
+    if (!prefill_supported(ctx->dm) || (ctx->cfg.flags & DFSSM_FLAG_TAPS)) {
+        // shapes the serial-in-t state kernel does not cover (d_state not a multiple of 16), or taps wanted: token by token
+        // through the persistent kernel / chain of the step path (same results by construction)
+        if (seq != 0 || ctx->cfg.max_batch != 1) return fail(ctx, DFSSM_E_ARG, "this shape prefills only through dfssm_step");
+        for (int i = 0; i < n_tokens; ++i) {
+            const int rc = dfssm_step(ctx, tokens_dev + i, 1);
+            if (rc != DFSSM_OK) return rc;
+        }
+        return DFSSM_OK;
+    }
+    for (int i = 0; i < n_tokens; i += prefill::CHUNK) {
+        const int T = n_tokens - i < prefill::CHUNK ? n_tokens - i : prefill::CHUNK;
+        const int rc = prefill_chunk(ctx, tokens_dev + i, T, seq);
+        if (rc != DFSSM_OK) return rc;
+    }
     return DFSSM_OK;
 }
 

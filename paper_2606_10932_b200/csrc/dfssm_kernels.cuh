@@ -539,7 +539,7 @@ constexpr int AM_THREADS = 1024;
 
 __global__ void __launch_bounds__(AM_THREADS)
 k_argmax(const float* __restrict__ logits, int vocab, int32_t* __restrict__ next, int32_t* __restrict__ tok,
-         int32_t* __restrict__ pos)
+         int32_t* __restrict__ pos, int pos_inc = 1)
 {
     __shared__ float sv[AM_THREADS / 32];
     __shared__ int si[AM_THREADS / 32];
@@ -571,7 +571,7 @@ k_argmax(const float* __restrict__ logits, int vocab, int32_t* __restrict__ next
         if (lane == 0) {
             next[b] = bi == 0x7fffffff ? 0 : bi;
             tok[b] = next[b];                      // the next step's input if the caller decodes greedily
-            pos[b] = (pos[b] + 1) & 3;
+            pos[b] = (pos[b] + pos_inc) & 3;
         }
     }
 }
