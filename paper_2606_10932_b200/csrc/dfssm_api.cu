@@ -159,7 +159,7 @@ Carve carve(const dfssm_config& c)
     {
         const size_t C = prefill::CHUNK;
         v.p_tok = put(C * 4); v.p_u = put(C * d.d_model * 4); v.p_xq = put(C * v.ldq); v.p_xqp = put(C * v.ldq); v.p_sx = put(C * 4);
-        v.p_qsum = put(C * 4); v.p_acc = put(C * v.ld_acc * 4); v.p_t = put(C * T_STRIDE * 4); v.p_zx = put(C * (size_t)d.d_in_proj * 4);
+        v.p_qsum = put(C * 4); v.p_acc = put(C * v.ld_acc * 4); v.p_t = put(C * T_STRIDE * 4); v.p_zx = put(C * v.ld_acc * 4);
         v.p_xbc = put(C * (size_t)d.conv_dim * 4); v.p_dt = put(C * (size_t)d.nheads * 4); v.p_g = put(C * d.d_inner * 4);
     }
     const size_t sizes[DFSSM_TAP_COUNT] = {
@@ -558,7 +558,12 @@ int mega_launch(dfssm_ctx* ctx, int seq = 0)
 // =================================================================================================
 namespace {
 
-bool prefill_supported(const Dims& d) { return d.d_state % prefill::SEQ_LANES == 0 && d.d_state / prefill::SEQ_LANES <= prefill::SEQ_NMAX && d.headdim % prefill::SEQ_PB == 0; }
+bool prefill_supported(const Dims& d)
+{
+    const int nper = d.d_state / prefill::SEQ_LANES;
+    return prefill::seq_smem(d) <= 48 * 1024 && d.d_state % prefill::SEQ_LANES == 0 && (nper == 1 || nper == 2 || nper == 4 || nper == 8 || nper == 16) &&
+           d.headdim % prefill::SEQ_PB == 0;
+}
 
 int prefill_chunk(dfssm_ctx* c, const int32_t* tokens_dev, int T, int seq)
 {
@@ -603,11 +608,21 @@ int prefill_chunk(dfssm_ctx* c, const int32_t* tokens_dev, int T, int seq)
         k_normquant<<<T, NQ_THREADS, 0, st>>>(u, d.d_model, L.norm_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum, nullptr, 0, 0, 0,
                                               use_mma(c, T, d.d_model) ? acc : nullptr, ld_acc, t);
         proj(L.in_sign, L.in_A, d.d_in_proj, d.d_model);
-        prefill::k_pf_epi<<<dim3((d.d_in_proj + prefill::EPI_T - 1) / prefill::EPI_T, T), prefill::EPI_T, 0, st>>>(L, d, acc, ld_acc, t, sx, zx);
-        prefill::k_pf_conv<<<dim3((d.conv_dim + d.nheads + prefill::CONV_T - 1) / prefill::CONV_T, T), prefill::CONV_T, 0, st>>>(L, d, zx, T, ring, pos, xbc,
+        prefill::k_pf_epi<<<dim3((d.d_in_proj + prefill::EPI_T - 1) / prefill::EPI_T, T), prefill::EPI_T, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
+        prefill::k_pf_conv<<<dim3((d.conv_dim + d.nheads + prefill::CONV_T - 1) / prefill::CONV_T, T), prefill::CONV_T, 0, st>>>(L, d, zx, ld_acc, T, ring, pos, xbc,
                                                                                                                                dtv);
-        prefill::k_pf_ring<<<(d.conv_dim + 255) / 256, 256, 0, st>>>(d, zx, T, ring, pos);
-        prefill::k_pf_ssm<<<d.nheads * (d.headdim / prefill::SEQ_PB), prefill::SEQ_T, 0, st>>>(L, d, zx, xbc, dtv, T, ssm, g);
+        prefill::k_pf_ring<<<(d.conv_dim + 255) / 256, 256, 0, st>>>(d, zx, ld_acc, T, ring, pos);
+        {
+            const dim3 gr(d.nheads * (d.headdim / prefill::SEQ_PB));
+            const size_t sm = prefill::seq_smem(d);
+            switch (d.d_state / prefill::SEQ_LANES) {
+                case 1: prefill::k_pf_ssm<1><<<gr, prefill::SEQ_T, sm, st>>>(L, d, zx, ld_acc, xbc, dtv, T, ssm, g); break;
+                case 2: prefill::k_pf_ssm<2><<<gr, prefill::SEQ_T, sm, st>>>(L, d, zx, ld_acc, xbc, dtv, T, ssm, g); break;
+                case 4: prefill::k_pf_ssm<4><<<gr, prefill::SEQ_T, sm, st>>>(L, d, zx, ld_acc, xbc, dtv, T, ssm, g); break;
+                case 8: prefill::k_pf_ssm<8><<<gr, prefill::SEQ_T, sm, st>>>(L, d, zx, ld_acc, xbc, dtv, T, ssm, g); break;
+                default: prefill::k_pf_ssm<16><<<gr, prefill::SEQ_T, sm, st>>>(L, d, zx, ld_acc, xbc, dtv, T, ssm, g); break;
+            }
+        }
         k_normquant<<<T, NQ_THREADS, 0, st>>>(g, d.d_inner, L.gnorm_w, d.d_inner, d.eps, xq, xqp, ldq, sx, qsum, nullptr, 0, 0, 0,
                                               use_mma(c, T, d.d_inner) ? acc : nullptr, ld_acc, t);
         proj(L.out_sign, L.out_A, d.d_model, d.d_inner);
