@@ -138,6 +138,14 @@ DFSSM_API int dfssm_step(dfssm_ctx* ctx, const int32_t* tokens_dev, int batch);
  * Shapes whose d_state is not a multiple of 16 (and contexts with DFSSM_FLAG_TAPS) are fed token by token instead (max_batch 1 only). */
 DFSSM_API int dfssm_prefill(dfssm_ctx* ctx, const int32_t* tokens_dev, int n_tokens, int seq);
 
+/* On-device temperature / top-k sampling (the generation loop of P:126; definition: DESIGN.md R23) from the
+ * logits of the last step, for sequences 0..batch-1: the top_k (1..64) largest logits, equal logits by lower index first;
+ * weights sp_expf((l - l_max) / temperature); the token whose running sum (binary64, rank order) first exceeds
+ * uniform_dev[s] * total.  uniform_dev: device f32[batch], each in [0, 1) -- the caller's random numbers (the library draws none).
+ * Overwrites the greedy tokens (dfssm_next_tokens), so feeding that pointer to the next dfssm_step decodes the sampled tokens
+ * without leaving the device.  temperature <= 0 or top_k == 1 is greedy decode.  Async. */
+DFSSM_API int dfssm_sample(dfssm_ctx* ctx, int batch, float temperature, int top_k, const float* uniform_dev);
+
 /* Host-buffer form of the same step (the end-to-end call): copies tokens_host[batch] to the
  * device, runs the step, copies the greedy next tokens to next_host[batch] and, if logits_host is
  * non-null, the logits to logits_host[batch*vocab]; synchronises the stream before returning.

@@ -61,6 +61,7 @@ def lib() -> C.CDLL:
         "dfo_gate": (None, [f32p, f32p, C.c_int, f32p]),
         "dfo_lm_head": (None, [i8p, f32p, C.c_int, C.c_int, i8p, C.c_float, i32p, f32p]),
         "dfo_argmax": (C.c_int, [f32p, C.c_int]),
+        "dfo_sample": (C.c_int, [f32p, C.c_int, C.c_float, C.c_int, C.c_float]),
         "dfo_load": (C.c_void_p, [C.c_void_p, C.c_size_t, C.c_int, C.c_char_p, C.c_size_t]),
         "dfo_free": (None, [C.c_void_p]),
         "dfo_set_threads": (None, [C.c_int]),
@@ -208,6 +209,11 @@ def lm_head(E, e_s, hq, s_h):
 def argmax(logits):
     logits = _c(logits, np.float32)
     return int(lib().dfo_argmax(_p(logits, C.c_float), logits.size))
+
+
+def sample(logits, temperature: float, top_k: int, u: float) -> int:
+    lg = _c(logits, np.float32)
+    return int(lib().dfo_sample(_p(lg, C.c_float), lg.size, float(temperature), int(top_k), float(u)))
 
 
 def set_threads(n: int) -> int:

@@ -312,6 +312,49 @@ void dfo_lm_head(const int8_t* E, const float* e_s, int vocab, int d, const int8
     }
 }
 
+/* Temperature / top-k sampling of one token from a logits vector (the generation loop the paper implies; the paper gives no
+ * sampler: DESIGN.md R23).  Greedy decode is the case top_k == 1 (or temperature <= 0).
+ *   1. the top_k largest logits, equal logits ordered by LOWER index first: ranks 0 .. k-1;
+ *   2. w_r = sp_expf((l_r - l_0) / temperature)        (binary32 operations, the specified exp);
+ *   3. c_r = w_0 + ... + w_r accumulated in binary64 in rank order;
+ *   4. the smallest rank r with c_r > (double)u * c_{k-1} (u in [0,1) is the caller's uniform random number; r = k-1 if none).
+ * Returns the vocabulary index of that rank.  O(k * n): a plain selection, no sort. */
+int dfo_sample(const float* logits, int n, float temperature, int top_k, float u)
+{
+    if (top_k < 1) top_k = 1;
+    if (top_k > n) top_k = n;
+    if (top_k > 64) top_k = 64;
+    if (!(temperature > 0.0f)) top_k = 1;
+    int idx[64];
+    float val[64];
+    int prev_i = -1;
+    float prev_v = 0.0f;
+    for (int r = 0; r < top_k; ++r) {
+        int bi = -1;
+        float bv = 0.0f;
+        for (int i = 0; i < n; ++i) {
+            const float x = logits[i];
+            /* candidates strictly after the previous pick in the order (value descending, index ascending) */
+            if (r > 0 && !(x < prev_v || (x == prev_v && i > prev_i))) continue;
+            if (bi < 0 || x > bv) { bi = i; bv = x; }       /* the first (lowest) index wins among equals */
+        }
+        idx[r] = bi; val[r] = bv;
+        prev_i = bi; prev_v = bv;
+    }
+    if (top_k == 1) return idx[0];
+    double c[64];
+    double run = 0.0;
+    for (int r = 0; r < top_k; ++r) {
+        const float w = dfo_sp_expf((val[r] - val[0]) / temperature);
+        run += (double)w;
+        c[r] = run;
+    }
+    const double thr = (double)u * run;
+    for (int r = 0; r < top_k; ++r)
+        if (c[r] > thr) return idx[r];
+    return idx[top_k - 1];
+}
+
 int dfo_argmax(const float* logits, int n)
 {
     int best = 0;

@@ -110,6 +110,9 @@ float* dfo_ssm_state(dfo_model*, int layer, int seq);   /* [nheads][headdim][d_s
 float* dfo_conv_state(dfo_model*, int layer, int seq);  /* [conv_dim][3] */
 int    dfo_shape(const dfo_model*, int32_t out[12]);    /* the header's 9 ints + nheads,d_in_proj,conv_dim */
 
+/* temperature / top-k sampling of one token (R23); top_k <= 64 */
+int dfo_sample(const float* logits, int n, float temperature, int top_k, float u);
+
 /* TEST-ONLY arithmetic mode switch (see dfssm_oracle.c): the default is the contract. */
 enum { DFO_MODE_CONTRACT = 0, DFO_MODE_REVERSED = 1, DFO_MODE_F64 = 2 };
 void dfo_set_mode(int mode);

@@ -31,7 +31,7 @@ KCLASSES = ("embed", "normquant", "proj_in", "ssm", "proj_out", "epi_out", "lmhe
 
 # every symbol include/dfssm.h declares (tests check the .so exports exactly these)
 EXPORTED_SYMBOLS = (
-    "dfssm_arena_bytes", "dfssm_create", "dfssm_load_weights", "dfssm_reset_state", "dfssm_step", "dfssm_prefill",
+    "dfssm_arena_bytes", "dfssm_create", "dfssm_load_weights", "dfssm_reset_state", "dfssm_step", "dfssm_prefill", "dfssm_sample",
     "dfssm_step_host", "dfssm_logits", "dfssm_next_tokens", "dfssm_hidden", "dfssm_debug_tensor",
     "dfssm_get_state", "dfssm_set_state", "dfssm_debug_profile", "dfssm_sync", "dfssm_launches_per_step",
     "dfssm_time_kernels", "dfssm_last_error", "dfssm_destroy",
@@ -119,6 +119,7 @@ def lib() -> C.CDLL:
         "dfssm_reset_state": (C.c_int, [vp, C.c_int]),
         "dfssm_step": (C.c_int, [vp, vp, C.c_int]),
         "dfssm_prefill": (C.c_int, [vp, vp, C.c_int, C.c_int]),
+        "dfssm_sample": (C.c_int, [vp, C.c_int, C.c_float, C.c_int, vp]),
         "dfssm_step_host": (C.c_int, [vp, i32p, C.c_int, i32p, f32p]),
         "dfssm_logits": (C.c_int, [vp, C.POINTER(vp)]),
         "dfssm_next_tokens": (C.c_int, [vp, C.POINTER(vp)]),
@@ -233,6 +234,14 @@ class Model:
         tokens_dev.record_stream(self.stream)
         self._check(self._L.dfssm_prefill(self._h, C.c_void_p(tokens_dev.data_ptr()), tokens_dev.numel(), int(seq)))
         self.batch = max(self.batch, int(seq) + 1)
+
+    def sample(self, temperature: float, top_k: int, uniform_dev, batch: Optional[int] = None):
+        """uniform_dev: torch float32 CUDA tensor [batch] in [0, 1) (dfssm_sample); the result replaces next_tokens()."""
+        assert uniform_dev.dtype == self._torch.float32 and uniform_dev.is_cuda and uniform_dev.is_contiguous()
+        n = int(batch) if batch is not None else uniform_dev.numel()
+        self.stream.wait_stream(self._torch.cuda.current_stream(self.device))
+        uniform_dev.record_stream(self.stream)
+        self._check(self._L.dfssm_sample(self._h, n, float(temperature), int(top_k), C.c_void_p(uniform_dev.data_ptr())))
 
     def step_host(self, tokens_host: np.ndarray, next_host: np.ndarray, logits_host: Optional[np.ndarray] = None):
         assert tokens_host.dtype == np.int32 and next_host.dtype == np.int32

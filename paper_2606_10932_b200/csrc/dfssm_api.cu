@@ -853,6 +853,18 @@ int dfssm_prefill(dfssm_ctx* ctx, const int32_t* tokens_dev, int n_tokens, int s
     return DFSSM_OK;
 }
 
+int dfssm_sample(dfssm_ctx* ctx, int batch, float temperature, int top_k, const float* uniform_dev)
+{
+    if (!ctx || !uniform_dev) return DFSSM_E_ARG;
+    if (!ctx->loaded) return fail(ctx, DFSSM_E_STATE, "dfssm_sample before dfssm_load_weights");
+    if (batch < 1 || batch > ctx->cfg.max_batch) return fail(ctx, DFSSM_E_ARG, "batch %d outside [1, %d]", batch, ctx->cfg.max_batch);
+    if (top_k < 1 || top_k > SAMPLE_KMAX) return fail(ctx, DFSSM_E_ARG, "top_k %d outside [1, %d]", top_k, SAMPLE_KMAX);
+    k_sample<<<batch, SAMPLE_THREADS, 0, ctx->stream>>>(at<float>(ctx, ctx->cv.logits), ctx->dm.vocab, temperature, top_k, uniform_dev,
+                                                        at<int32_t>(ctx, ctx->cv.next), at<int32_t>(ctx, ctx->cv.tok));
+    CK(cudaGetLastError());
+    return DFSSM_OK;
+}
+
 int dfssm_step_host(dfssm_ctx* ctx, const int32_t* tokens_host, int batch, int32_t* next_host, float* logits_host)
 {
     if (!ctx || !tokens_host || !next_host) return DFSSM_E_ARG;

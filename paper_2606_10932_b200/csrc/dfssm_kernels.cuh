@@ -576,4 +576,80 @@ k_argmax(const float* __restrict__ logits, int vocab, int32_t* __restrict__ next
     }
 }
 
+// =============================================================================================
+// Temperature / top-k sampling of the next token (R23; the generation loop of P:126), one CTA per sequence:
+//   ranks 0 .. k-1 = the k largest logits, equal logits by lower index first (k rounds of a CTA-wide argmax over the
+//   candidates that come strictly after the previous pick in that order); w_r = sp_expf((l_r - l_0) / temperature);
+//   c_r = fp64 running sum in rank order; the pick is the smallest r with c_r > u * c_{k-1}.  u[b] in [0,1) comes from the caller.
+//   Overwrites next[b] and tok[b] (the next dfssm_step's input); the conv ring position is NOT touched (the step did that).
+// =============================================================================================
+constexpr int SAMPLE_THREADS = 1024, SAMPLE_KMAX = 64;
+
+__global__ void __launch_bounds__(SAMPLE_THREADS)
+k_sample(const float* __restrict__ logits, int vocab, float temperature, int top_k, const float* __restrict__ u,
+         int32_t* __restrict__ next, int32_t* __restrict__ tok)
+{
+    __shared__ float sv[SAMPLE_THREADS / 32];
+    __shared__ int si[SAMPLE_THREADS / 32];
+    __shared__ float pick_v[SAMPLE_KMAX];
+    __shared__ int pick_i[SAMPLE_KMAX];
+    const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const float* lg = logits + (size_t)b * vocab;
+    if (top_k < 1) top_k = 1;
+    if (top_k > vocab) top_k = vocab;
+    if (top_k > SAMPLE_KMAX) top_k = SAMPLE_KMAX;
+    if (!(temperature > 0.0f)) top_k = 1;
+    float prev_v = 0.0f;
+    int prev_i = -1;
+    for (int r = 0; r < top_k; ++r) {
+        float best = 0.0f;
+        int bi = 0x7fffffff;
+        for (int i = tid; i < vocab; i += SAMPLE_THREADS) {
+            const float x = lg[i];
+            if (r > 0 && !(x < prev_v || (x == prev_v && i > prev_i))) continue;
+            if (bi == 0x7fffffff || x > best) { best = x; bi = i; }      // ascending i per thread: the lowest index wins among equals
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const float ov = __shfl_xor_sync(0xffffffffu, best, o);
+            const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (oi != 0x7fffffff && (bi == 0x7fffffff || ov > best || (ov == best && oi < bi))) { best = ov; bi = oi; }
+        }
+        if (lane == 0) { sv[wid] = best; si[wid] = bi; }
+        __syncthreads();
+        if (wid == 0) {
+            best = sv[lane];
+            bi = si[lane];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                const float ov = __shfl_xor_sync(0xffffffffu, best, o);
+                const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+                if (oi != 0x7fffffff && (bi == 0x7fffffff || ov > best || (ov == best && oi < bi))) { best = ov; bi = oi; }
+            }
+            if (lane == 0) { pick_v[r] = best; pick_i[r] = bi; }
+        }
+        __syncthreads();
+        prev_v = pick_v[r];
+        prev_i = pick_i[r];
+    }
+    if (tid == 0) {
+        int choice = pick_i[0];
+        if (top_k > 1) {
+            double c[SAMPLE_KMAX];
+            double run = 0.0;
+            for (int r = 0; r < top_k; ++r) {
+                const float w = sp_expf(fdiv(fadd(pick_v[r], -pick_v[0]), temperature));
+                run += (double)w;
+                c[r] = run;
+            }
+            const double thr = (double)u[b] * run;
+            choice = pick_i[top_k - 1];
+            for (int r = 0; r < top_k; ++r)
+                if (c[r] > thr) { choice = pick_i[r]; break; }
+        }
+        next[b] = choice;
+        tok[b] = choice;
+    }
+}
+
 }  // namespace dfssm
