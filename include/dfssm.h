@@ -62,6 +62,10 @@ enum {
 #define DFSSM_FLAG_NO_GRAPH  2u  /* launch the step's kernels one by one instead of one CUDA-graph launch */
 #define DFSSM_FLAG_NO_MEGA   4u  /* never use the single persistent kernel ("mega" path) for batch-1 steps    */
 #define DFSSM_FLAG_NO_MMA   16u  /* batch >= 16: keep the projections on the dp4a path instead of tcgen05 kind::i8 tiles  */
+#define DFSSM_FLAG_STATE_FP16 64u /* SURVEY 8(f) NEXT-2, first step (R24): the SSM state is STORED as binary16 (round to nearest even of each
+                                   * step's binary32 update; the step's own readout uses the unrounded values).  Halves the state bytes (95 % of the
+                                   * traffic at batch 64).  LOSSY against the fp32-state model; bit-identical to the oracle in the same mode.
+                                   * Served by the kernel chain and dfssm_prefill (the persistent batch-1 kernel keeps fp32 state). */
 #define DFSSM_FLAG_PROF      8u  /* persistent kernel: thread 0 of every CTA stamps its SM clock at every phase */
 
 /* Shape of the model (the paper's Mamba-2-shaped student, Table 1) + capacity.

@@ -61,6 +61,8 @@ def lib() -> C.CDLL:
         "dfo_gate": (None, [f32p, f32p, C.c_int, f32p]),
         "dfo_lm_head": (None, [i8p, f32p, C.c_int, C.c_int, i8p, C.c_float, i32p, f32p]),
         "dfo_argmax": (C.c_int, [f32p, C.c_int]),
+        "dfo_float_to_half": (C.c_uint16, [C.c_float]),
+        "dfo_set_state_fp16": (None, [C.c_void_p, C.c_int]),
         "dfo_sample": (C.c_int, [f32p, C.c_int, C.c_float, C.c_int, C.c_float]),
         "dfo_load": (C.c_void_p, [C.c_void_p, C.c_size_t, C.c_int, C.c_char_p, C.c_size_t]),
         "dfo_free": (None, [C.c_void_p]),
@@ -211,6 +213,13 @@ def argmax(logits):
     return int(lib().dfo_argmax(_p(logits, C.c_float), logits.size))
 
 
+def float_to_half(x) -> np.ndarray:
+    """binary32 -> binary16 bit patterns (RN-even), element by element through dfo_float_to_half"""
+    a = np.atleast_1d(np.asarray(x, np.float32))
+    L = lib()
+    return np.array([L.dfo_float_to_half(float(v)) for v in a.ravel()], np.uint16).reshape(a.shape)
+
+
 def sample(logits, temperature: float, top_k: int, u: float) -> int:
     lg = _c(logits, np.float32)
     return int(lib().dfo_sample(_p(lg, C.c_float), lg.size, float(temperature), int(top_k), float(u)))
@@ -263,6 +272,10 @@ class OracleModel:
         self._tap_len = {0: self.d_model, 1: 1, 2: self.d_in_proj, 3: self.lora_rank, 4: self.d_in_proj,
                          5: self.conv_dim, 6: self.nheads, 7: self.d_inner, 8: self.d_inner, 9: self.d_inner,
                          10: 1, 11: self.d_model, 12: self.lora_rank, 13: self.d_model}
+
+    def set_state_fp16(self, on: bool = True):
+        """DESIGN.md R24: store the SSM state as binary16 between steps (rounded after every step)."""
+        self._L.dfo_set_state_fp16(self._h, 1 if on else 0)
 
     def close(self):
         if getattr(self, "_h", None):

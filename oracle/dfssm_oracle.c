@@ -143,6 +143,37 @@ float dfo_half_to_float(uint16_t h)
  * ------------------------------------------------------------------------------------------ */
 
 /* S0: int8 per-row embedding, "quantized to int8 per-row", tied with the head */
+/* binary32 -> binary16, round to nearest even (IEEE 754 convertFormat: subnormals kept, overflow -> infinity, NaN stays NaN);
+ * the inverse of dfo_half_to_float on every binary16 value.  Used by the fp16 state format (R24). */
+uint16_t dfo_float_to_half(float f)
+{
+    uint32_t x;
+    memcpy(&x, &f, 4);
+    const uint32_t sign = (x >> 16) & 0x8000u;
+    const uint32_t ax = x & 0x7fffffffu;
+    if (ax >= 0x7f800000u) return (uint16_t)(sign | 0x7c00u | (ax > 0x7f800000u ? 0x200u : 0u));       /* inf / NaN */
+    if (ax >= 0x477ff000u) return (uint16_t)(sign | 0x7c00u);          /* >= 65520 rounds to infinity */
+    if (ax < 0x33000001u) return (uint16_t)sign;                        /* <= 2^-25: rounds to zero (2^-25 itself ties to even = 0) */
+    int e = (int)(ax >> 23) - 127;                                      /* unbiased exponent */
+    uint32_t m = (ax & 0x7fffffu) | 0x800000u;                          /* 24-bit significand */
+    int shift;                                                          /* bits dropped from the significand */
+    uint32_t he;
+    if (e < -14) { shift = 13 + (-14 - e); he = 0; }                    /* binary16 subnormal */
+    else { shift = 13; he = (uint32_t)(e + 15); }
+    uint32_t q = m >> shift;
+    const uint32_t rem = m & ((1u << shift) - 1u), half = 1u << (shift - 1);
+    if (rem > half || (rem == half && (q & 1u))) ++q;                   /* ties to even; a carry walks into the exponent */
+    uint32_t h = he == 0 ? q : ((he << 10) + (q - 0x400u));
+    return (uint16_t)(sign | h);
+}
+
+/* the fp16 state format (R24): every state value is replaced by float(half(value)) after the step's update and
+ * readout (the readout of the step itself used the unrounded binary32 values) */
+void dfo_round_state_f16(float* H, size_t n)
+{
+    for (size_t i = 0; i < n; ++i) H[i] = dfo_half_to_float(dfo_float_to_half(H[i]));
+}
+
 static float silu_mode(float x)
 {
     if (g_mode == DFO_MODE_F64) return (float)((double)x / (1.0 + exp(-(double)x)));
@@ -392,6 +423,7 @@ struct dfo_model {
     int32_t* next; /* [seq] */
     float* hidden; /* [seq][d_model] */
     int taps_on;
+    int state_fp16;             /* DESIGN.md R24: the SSM state is stored as binary16 between steps */
     uint8_t* taps; /* [layer][seq][tap_stride] */
     size_t tap_off[DFO_TAP_COUNT + 1];
 };
@@ -507,6 +539,8 @@ int dfo_get_threads(void)
 #endif
 }
 
+void dfo_set_state_fp16(dfo_model* m, int on) { m->state_fp16 = on ? 1 : 0; }
+
 void dfo_enable_taps(dfo_model* m, int on)
 {
     m->taps_on = on;
@@ -602,6 +636,7 @@ static void step_one(dfo_model* m, int s, int32_t tok)
         TAP(DFO_TAP_DT, dt, 4 * (size_t)m->nheads);
         dfo_ssm_step(dfo_ssm_state(m, l, s), xbc, xbc + di, xbc + di + gs, dt, An, L->D,
                      m->nheads, m->headdim, m->d_state, m->ngroups, y);
+        if (m->state_fp16) dfo_round_state_f16(dfo_ssm_state(m, l, s), ssm_elems(m));
         TAP(DFO_TAP_Y, y, 4 * (size_t)di);
         dfo_gate(y, z, di, g);                                                           /* S6 */
         TAP(DFO_TAP_G, g, 4 * (size_t)di);

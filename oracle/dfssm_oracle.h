@@ -110,6 +110,11 @@ float* dfo_ssm_state(dfo_model*, int layer, int seq);   /* [nheads][headdim][d_s
 float* dfo_conv_state(dfo_model*, int layer, int seq);  /* [conv_dim][3] */
 int    dfo_shape(const dfo_model*, int32_t out[12]);    /* the header's 9 ints + nheads,d_in_proj,conv_dim */
 
+/* fp16 state format (R24): binary32 -> binary16 RN-even, and the model switch (state rounded after every step) */
+uint16_t dfo_float_to_half(float f);
+void dfo_round_state_f16(float* H, size_t n);
+void dfo_set_state_fp16(dfo_model*, int on);
+
 /* temperature / top-k sampling of one token (R23); top_k <= 64 */
 int dfo_sample(const float* logits, int n, float temperature, int top_k, float u);
 

@@ -21,6 +21,7 @@ FLAG_NO_GRAPH = 2
 FLAG_NO_MEGA = 4
 FLAG_PROF = 8
 FLAG_NO_MMA = 16
+FLAG_STATE_FP16 = 64
 
 TAPS = dict(XQ_IN=0, S_IN=1, ACC_IN=2, T_IN=3, ZXBCDT=4, XBC_CONV=5, DT=6, Y=7, G=8, GQ=9,
             S_G=10, ACC_OUT=11, T_OUT=12, HIDDEN=13)

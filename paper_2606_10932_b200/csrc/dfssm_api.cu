@@ -29,7 +29,7 @@ struct Carve {                 // byte offsets inside the arena
     size_t p_tok, p_u, p_xq, p_xqp, p_sx, p_qsum, p_acc, p_t, p_zx, p_xbc, p_dt, p_g;      // prefill: activations of one chunk of positions
     size_t m_chunks, m_schunks, m_blocks, m_x, m_xbytes, m_am, m_prof;      // mega path regions (valid if mega_fit)
     bool mega_fit;
-    size_t ssm_elems, ldq, ld_acc;
+    size_t ssm_elems, ssm_esize, ldq, ld_acc;      // ssm_esize: bytes per state value (4, or 2 with DFSSM_FLAG_STATE_FP16)
     uint32_t tap_stride;
     TapLayout tl;
 };
@@ -140,7 +140,8 @@ Carve carve(const dfssm_config& c)
     size_t o = 0;
     auto put = [&](size_t bytes) { o = up(o, ARENA_ALIGN); size_t at = o; o += bytes; return at; };
     v.blob = put(blob_bytes_for(d));
-    v.ssm = put(nl * B * v.ssm_elems * 4);
+    v.ssm_esize = (c.flags & DFSSM_FLAG_STATE_FP16) ? 2 : 4;
+    v.ssm = put(nl * B * v.ssm_elems * v.ssm_esize);
     v.conv = put(nl * B * (size_t)d.conv_dim * 16);
     v.pos = put(B * 4);
     v.u = put(B * d.d_model * 4);
@@ -172,7 +173,7 @@ Carve carve(const dfssm_config& c)
     v.tap_stride = (uint32_t)to;
     v.taps = (c.flags & DFSSM_FLAG_TAPS) ? put(nl * B * to) : 0;
     mega::Params mp;
-    v.mega_fit = !(c.flags & DFSSM_FLAG_NO_MEGA) && mega::plan(d, mega::GRID, mp);
+    v.mega_fit = !(c.flags & (DFSSM_FLAG_NO_MEGA | DFSSM_FLAG_STATE_FP16)) && mega::plan(d, mega::GRID, mp);      // the persistent kernel keeps fp32 state
     if (v.mega_fit) {
         const mega::Regions rg = mega::regions(mp);
         v.m_chunks = put(rg.chunks);
@@ -309,7 +310,10 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
     for (int l = 0; l < d.n_layers; ++l) {
         const LayerW& L = c->layers[l];
         uint8_t* tp = taps_on ? at<uint8_t>(c, v.taps) + (size_t)l * B * v.tap_stride : nullptr;
-        float* ssm = at<float>(c, v.ssm) + (size_t)l * B * v.ssm_elems;
+        uint8_t* ssm_b = c->arena + v.ssm + (size_t)l * B * v.ssm_elems * v.ssm_esize;
+        float* ssm = (float*)ssm_b;
+        __half* ssm_h = (__half*)ssm_b;
+        const bool st16 = v.ssm_esize == 2;
         float* conv = at<float>(c, v.conv) + (size_t)l * B * (size_t)d.conv_dim * 4;
 
         tm->begin(DFSSM_KCLASS_NORMQUANT);
@@ -338,12 +342,18 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         k_bcdt<<<dim3((2 * d.ngroups * d.d_state + d.nheads + BCDT_THREADS - 1) / BCDT_THREADS, batch), BCDT_THREADS, 0, st>>>(
             L, d, acc, ld_acc, t, sx, conv, pos, at<float>(c, v.bcdt), tp, v.tap_stride, v.tl);
         ++nl;
-        if (d.headdim % 32 == 0)
-            k_ssm<32><<<dim3(d.nheads * (d.headdim / 32), batch), SSM_THREADS, ssm_smem(d), st>>>(
-                L, d, acc, ld_acc, t, sx, conv, pos, ssm, g, at<float>(c, v.bcdt), tp, v.tap_stride, v.tl);
-        else
-            k_ssm<16><<<dim3(d.nheads * (d.headdim / 16), batch), SSM_THREADS, ssm_smem(d), st>>>(
-                L, d, acc, ld_acc, t, sx, conv, pos, ssm, g, at<float>(c, v.bcdt), tp, v.tap_stride, v.tl);
+        {
+            const dim3 g32(d.nheads * (d.headdim / 32), batch), g16(d.nheads * (d.headdim / 16), batch);
+            float* bc = at<float>(c, v.bcdt);
+            if (d.headdim % 32 == 0 && !st16)
+                k_ssm<32, float><<<g32, SSM_THREADS, ssm_smem(d), st>>>(L, d, acc, ld_acc, t, sx, conv, pos, ssm, g, bc, tp, v.tap_stride, v.tl);
+            else if (d.headdim % 32 == 0)
+                k_ssm<32, __half><<<g32, SSM_THREADS, ssm_smem(d), st>>>(L, d, acc, ld_acc, t, sx, conv, pos, ssm_h, g, bc, tp, v.tap_stride, v.tl);
+            else if (!st16)
+                k_ssm<16, float><<<g16, SSM_THREADS, ssm_smem(d), st>>>(L, d, acc, ld_acc, t, sx, conv, pos, ssm, g, bc, tp, v.tap_stride, v.tl);
+            else
+                k_ssm<16, __half><<<g16, SSM_THREADS, ssm_smem(d), st>>>(L, d, acc, ld_acc, t, sx, conv, pos, ssm_h, g, bc, tp, v.tap_stride, v.tl);
+        }
         tm->end(); ++nl;
 
         tm->begin(DFSSM_KCLASS_NORMQUANT);
@@ -603,7 +613,7 @@ int prefill_chunk(dfssm_ctx* c, const int32_t* tokens_dev, int T, int seq)
     k_embed<<<dim3((d.d_model + 255) / 256, T), 256, 0, st>>>(tok, c->emb, c->emb_s, d.vocab, d.d_model, u, err);
     for (int l = 0; l < d.n_layers; ++l) {
         const LayerW& L = c->layers[l];
-        float* ssm = at<float>(c, v.ssm) + ((size_t)l * B + seq) * v.ssm_elems;
+        uint8_t* ssm_b = c->arena + v.ssm + ((size_t)l * B + seq) * v.ssm_elems * v.ssm_esize;
         float* ring = at<float>(c, v.conv) + ((size_t)l * B + seq) * (size_t)d.conv_dim * 4;
         k_normquant<<<T, NQ_THREADS, 0, st>>>(u, d.d_model, L.norm_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum, nullptr, 0, 0, 0,
                                               use_mma(c, T, d.d_model) ? acc : nullptr, ld_acc, t);
@@ -615,13 +625,17 @@ int prefill_chunk(dfssm_ctx* c, const int32_t* tokens_dev, int T, int seq)
         {
             const dim3 gr(d.nheads * (d.headdim / prefill::SEQ_PB));
             const size_t sm = prefill::seq_smem(d);
+#define DFSSM_PF_SSM(N_)                                                                                                             \
+    if (v.ssm_esize == 2) prefill::k_pf_ssm<N_, __half><<<gr, prefill::SEQ_T, sm, st>>>(L, d, zx, ld_acc, xbc, dtv, T, (__half*)ssm_b, g); \
+    else prefill::k_pf_ssm<N_, float><<<gr, prefill::SEQ_T, sm, st>>>(L, d, zx, ld_acc, xbc, dtv, T, (float*)ssm_b, g)
             switch (d.d_state / prefill::SEQ_LANES) {
-                case 1: prefill::k_pf_ssm<1><<<gr, prefill::SEQ_T, sm, st>>>(L, d, zx, ld_acc, xbc, dtv, T, ssm, g); break;
-                case 2: prefill::k_pf_ssm<2><<<gr, prefill::SEQ_T, sm, st>>>(L, d, zx, ld_acc, xbc, dtv, T, ssm, g); break;
-                case 4: prefill::k_pf_ssm<4><<<gr, prefill::SEQ_T, sm, st>>>(L, d, zx, ld_acc, xbc, dtv, T, ssm, g); break;
-                case 8: prefill::k_pf_ssm<8><<<gr, prefill::SEQ_T, sm, st>>>(L, d, zx, ld_acc, xbc, dtv, T, ssm, g); break;
-                default: prefill::k_pf_ssm<16><<<gr, prefill::SEQ_T, sm, st>>>(L, d, zx, ld_acc, xbc, dtv, T, ssm, g); break;
+                case 1: DFSSM_PF_SSM(1); break;
+                case 2: DFSSM_PF_SSM(2); break;
+                case 4: DFSSM_PF_SSM(4); break;
+                case 8: DFSSM_PF_SSM(8); break;
+                default: DFSSM_PF_SSM(16); break;
             }
+#undef DFSSM_PF_SSM
         }
         k_normquant<<<T, NQ_THREADS, 0, st>>>(g, d.d_inner, L.gnorm_w, d.d_inner, d.eps, xq, xqp, ldq, sx, qsum, nullptr, 0, 0, 0,
                                               use_mma(c, T, d.d_inner) ? acc : nullptr, ld_acc, t);
@@ -780,7 +794,7 @@ int dfssm_reset_state(dfssm_ctx* ctx, int seq)
     const Carve& v = ctx->cv;
     const size_t B = ctx->cfg.max_batch, nl = d.n_layers > 0 ? d.n_layers : 1;
     if (seq < 0) {
-        CK(cudaMemsetAsync(ctx->arena + v.ssm, 0, nl * B * v.ssm_elems * 4, ctx->stream));
+        CK(cudaMemsetAsync(ctx->arena + v.ssm, 0, nl * B * v.ssm_elems * v.ssm_esize, ctx->stream));
         CK(cudaMemsetAsync(ctx->arena + v.conv, 0, nl * B * (size_t)d.conv_dim * 16, ctx->stream));
         // the exchange records of the persistent kernel go back to "nothing written" too (matters only after a step that
         // was aborted by a poll time-out and left half-written records behind)
@@ -792,8 +806,8 @@ int dfssm_reset_state(dfssm_ctx* ctx, int seq)
         return DFSSM_OK;
     }
     // one sequence of every layer: strided 2-D memsets (rows = layers)
-    CK(cudaMemset2DAsync(ctx->arena + v.ssm + (size_t)seq * v.ssm_elems * 4, B * v.ssm_elems * 4, 0,
-                         v.ssm_elems * 4, nl, ctx->stream));
+    CK(cudaMemset2DAsync(ctx->arena + v.ssm + (size_t)seq * v.ssm_elems * v.ssm_esize, B * v.ssm_elems * v.ssm_esize, 0,
+                         v.ssm_elems * v.ssm_esize, nl, ctx->stream));
     CK(cudaMemset2DAsync(ctx->arena + v.conv + (size_t)seq * d.conv_dim * 16, B * (size_t)d.conv_dim * 16, 0,
                          (size_t)d.conv_dim * 16, nl, ctx->stream));
     return DFSSM_OK;
@@ -928,11 +942,22 @@ static int state_copy(dfssm_ctx* ctx, int layer, int seq, float* ssm_h, size_t s
     if (ssm_h && ssm_bytes != v.ssm_elems * 4) return fail(ctx, DFSSM_E_SIZE, "ssm state is %zu bytes", v.ssm_elems * 4);
     if (conv_h && conv_bytes != (size_t)d.conv_dim * 12) return fail(ctx, DFSSM_E_SIZE, "conv state is %zu bytes", (size_t)d.conv_dim * 12);
     CK(cudaStreamSynchronize(ctx->stream));
-    float* ssm_d = at<float>(ctx, v.ssm) + ((size_t)layer * B + seq) * v.ssm_elems;
+    uint8_t* ssm_d = ctx->arena + v.ssm + ((size_t)layer * B + seq) * v.ssm_elems * v.ssm_esize;
     float* ring_d = at<float>(ctx, v.conv) + ((size_t)layer * B + seq) * (size_t)d.conv_dim * 4;
     if (ssm_h) {
-        if (to_host) CK(cudaMemcpy(ssm_h, ssm_d, ssm_bytes, cudaMemcpyDeviceToHost));
-        else CK(cudaMemcpy(ssm_d, ssm_h, ssm_bytes, cudaMemcpyHostToDevice));
+        if (v.ssm_esize == 4) {
+            if (to_host) CK(cudaMemcpy(ssm_h, ssm_d, ssm_bytes, cudaMemcpyDeviceToHost));
+            else CK(cudaMemcpy(ssm_d, ssm_h, ssm_bytes, cudaMemcpyHostToDevice));
+        } else {                               // fp16 state format: the host view stays fp32 (set: rounded to nearest even)
+            std::vector<__half> tmp(v.ssm_elems);
+            if (to_host) {
+                CK(cudaMemcpy(tmp.data(), ssm_d, v.ssm_elems * 2, cudaMemcpyDeviceToHost));
+                for (size_t i = 0; i < v.ssm_elems; ++i) ssm_h[i] = __half2float(tmp[i]);
+            } else {
+                for (size_t i = 0; i < v.ssm_elems; ++i) tmp[i] = __float2half_rn(ssm_h[i]);
+                CK(cudaMemcpy(ssm_d, tmp.data(), v.ssm_elems * 2, cudaMemcpyHostToDevice));
+            }
+        }
     }
     if (conv_h) {
         // ring <-> canonical [conv_dim][3] oldest first: the next step writes slot pos, so the three

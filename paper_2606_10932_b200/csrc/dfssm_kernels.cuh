@@ -309,12 +309,31 @@ k_bcdt(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int
 // =============================================================================================
 constexpr int SSM_THREADS = 256;
 
+// four consecutive state values: fp32 state, or the fp16 state format of DESIGN.md R24 (stored as binary16, RN-even of the
+// binary32 update; the readout of the step uses the unrounded binary32 values)
+__device__ __forceinline__ float4 state_ld4(const float* p) { return *(const float4*)p; }
+__device__ __forceinline__ void state_st4(float* p, float4 v) { *(float4*)p = v; }
+__device__ __forceinline__ float4 state_ld4(const __half* p)
+{
+    const uint2 r = *(const uint2*)p;
+    const __half2 a = *(const __half2*)&r.x, b = *(const __half2*)&r.y;
+    return make_float4(__low2float(a), __high2float(a), __low2float(b), __high2float(b));
+}
+__device__ __forceinline__ void state_st4(__half* p, float4 v)
+{
+    const __half2 a = __halves2half2(__float2half_rn(v.x), __float2half_rn(v.y)), b = __halves2half2(__float2half_rn(v.z), __float2half_rn(v.w));
+    uint2 r;
+    r.x = *(const uint32_t*)&a;
+    r.y = *(const uint32_t*)&b;
+    *(uint2*)p = r;
+}
+
 // 6 CTAs per SM (40 registers): the kernel is latency-bound, 4 CTAs of 58 registers were 11 % slower, 8 of 32 spill
-template <int PB>
+template <int PB, typename ST>
 __global__ void __launch_bounds__(SSM_THREADS, 6)
 k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int32_t* __restrict__ t,
       const float* __restrict__ s_x, float* __restrict__ conv_ring /* [batch][conv_dim][4] */,
-      const int32_t* __restrict__ pos /* [batch] */, float* __restrict__ ssm /* [batch][h][p][n] */,
+      const int32_t* __restrict__ pos /* [batch] */, ST* __restrict__ ssm /* [batch][h][p][n] */,
       float* __restrict__ g /* [batch][d_inner] */, const float* __restrict__ bcdt /* [batch][n_bcdt] from k_bcdt */,
       uint8_t* __restrict__ taps, uint32_t tap_stride, TapLayout tl)
 {
@@ -342,13 +361,13 @@ k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
 
     // this thread's slice of the state is requested first, so that HBM works while the rows below are finished
     const int p = tid / LANES, l16 = tid % LANES;  // PB rows x LANES lanes
-    float* Hr = ssm + (((size_t)b * dm.nheads + h) * dm.headdim + p0 + p) * dm.d_state;
+    ST* Hr = ssm + (((size_t)b * dm.nheads + h) * dm.headdim + p0 + p) * dm.d_state;
     constexpr int H_PRE = 32 / LANES;             // chunks held in registers (all of d_state = 128); further ones are loaded late
     float4 hpre[H_PRE];
 #pragma unroll
     for (int j = 0; j < H_PRE; ++j) {
         const int n4 = l16 + LANES * j;
-        if (n4 < dm.d_state / 4) hpre[j] = *(const float4*)(Hr + 4 * n4);
+        if (n4 < dm.d_state / 4) hpre[j] = state_ld4(Hr + 4 * n4);
     }
 
     if (tid < dm.r) v_sh[tid] = fmul(L.in_a_s[tid], (float)t[(size_t)b * T_STRIDE + tid]);
@@ -418,21 +437,21 @@ k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
         hv.y = ffma(dA, hv.y, fmul(dtx, bv.y));
         hv.z = ffma(dA, hv.z, fmul(dtx, bv.z));
         hv.w = ffma(dA, hv.w, fmul(dtx, bv.w));
-        *(float4*)(Hr + 4 * n4) = hv;
+        state_st4(Hr + 4 * n4, hv);
         a = dacc(a, cv.x, hv.x);
         a = dacc(a, cv.y, hv.y);
         a = dacc(a, cv.z, hv.z);
         a = dacc(a, cv.w, hv.w);
     }
     for (int n4 = l16 + LANES * H_PRE; n4 < dm.d_state / 4; n4 += LANES) {
-        float4 hv = *(const float4*)(Hr + 4 * n4);
+        float4 hv = state_ld4(Hr + 4 * n4);
         const float4 bv = *(const float4*)(Bc + 4 * n4);
         const float4 cv = *(const float4*)(Cc + 4 * n4);
         hv.x = ffma(dA, hv.x, fmul(dtx, bv.x));
         hv.y = ffma(dA, hv.y, fmul(dtx, bv.y));
         hv.z = ffma(dA, hv.z, fmul(dtx, bv.z));
         hv.w = ffma(dA, hv.w, fmul(dtx, bv.w));
-        *(float4*)(Hr + 4 * n4) = hv;
+        state_st4(Hr + 4 * n4, hv);
         a = dacc(a, cv.x, hv.x);
         a = dacc(a, cv.y, hv.y);
         a = dacc(a, cv.z, hv.z);

@@ -84,10 +84,17 @@ __device__ __forceinline__ void cp_async4(void* dst, const void* src)
 }
 inline size_t seq_smem(const Dims& d) { return 2 * sizeof(float) * ((size_t)SEQ_TB * (2 * d.d_state + 2 * SEQ_PB) + SEQ_TB) + sizeof(float) * 3 * SEQ_T; }
 
-template <int NPER>       // state values per lane = d_state / SEQ_LANES
+__device__ __forceinline__ float st_get(const float* p) { return *p; }
+__device__ __forceinline__ float st_get(const __half* p) { return __half2float(*p); }
+__device__ __forceinline__ void st_put(float* p, float v) { *p = v; }
+__device__ __forceinline__ void st_put(__half* p, float v) { *p = __float2half_rn(v); }      // v is already binary16-representable
+__device__ __forceinline__ float st_round(float v, const float*) { return v; }
+__device__ __forceinline__ float st_round(float v, const __half*) { return __half2float(__float2half_rn(v)); }     // R24: rounded after EVERY step
+
+template <int NPER, typename ST>       // state values per lane = d_state / SEQ_LANES; state type (fp32, or the fp16 format of R24)
 __global__ void __launch_bounds__(SEQ_T)
 k_pf_ssm(LayerW L, Dims dm, const float* __restrict__ zx, int ldz, const float* __restrict__ xbc, const float* __restrict__ dtv, int T,
-         float* __restrict__ ssm /* [h][p][n] of the sequence */, float* __restrict__ g /* [T][d_inner] */)
+         ST* __restrict__ ssm /* [h][p][n] of the sequence */, float* __restrict__ g /* [T][d_inner] */)
 {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     const int ds = dm.d_state;
@@ -102,11 +109,11 @@ k_pf_ssm(LayerW L, Dims dm, const float* __restrict__ zx, int ldz, const float* 
     const int tid = threadIdx.x, p = tid / SEQ_LANES, ln = tid % SEQ_LANES;
     const int ch0 = h * dm.headdim + p0, ch = ch0 + p;
     const int gs = dm.ngroups * ds;
-    float* Hr = ssm + (size_t)ch * ds;
+    ST* Hr = ssm + (size_t)ch * ds;
     float hreg[NPER];
     constexpr int nper = NPER;                            // contiguous state values of this lane
 #pragma unroll
-    for (int k = 0; k < NPER; ++k) hreg[k] = Hr[ln * nper + k];
+    for (int k = 0; k < NPER; ++k) hreg[k] = st_get(Hr + ln * nper + k);
     const float An = -sp_expf(L.A_log[h]);
     const float Dh = L.D[h];
 
@@ -177,8 +184,8 @@ k_pf_ssm(LayerW L, Dims dm, const float* __restrict__ zx, int ldz, const float* 
 #pragma unroll
             for (int k = 0; k < NPER; ++k) {
                 const float hn = ffma(dA, hreg[k], fmul(dtx, bv[k]));
-                hreg[k] = hn;
-                a2[k & 1] = dacc(a2[k & 1], cv[k], hn);
+                hreg[k] = st_round(hn, Hr);                // what the next position reads
+                a2[k & 1] = dacc(a2[k & 1], cv[k], hn);   // the readout of this position uses the unrounded value
             }
             double a = a2[0] + a2[1];
 #pragma unroll
@@ -192,7 +199,7 @@ k_pf_ssm(LayerW L, Dims dm, const float* __restrict__ zx, int ldz, const float* 
         __syncthreads();                                  // the stage is refilled two blocks on; s_dA / s_dtx / s_sz by the next block
     }
 #pragma unroll
-    for (int k = 0; k < NPER; ++k) Hr[ln * nper + k] = hreg[k];
+    for (int k = 0; k < NPER; ++k) st_put(Hr + ln * nper + k, hreg[k]);
 }
 
 // the last position's residual stream becomes the sequence's hidden state
