@@ -152,7 +152,7 @@ Carve carve(const dfssm_config& c)
     v.acc = put(B * v.ld_acc * 4);
     v.t = put(B * T_STRIDE * 4);
     v.g = put(B * d.d_inner * 4);
-    v.bcdt = put(B * (size_t)(2 * d.ngroups * d.d_state + d.nheads) * 4);
+    v.bcdt = put(B * (size_t)(d.d_in_proj + d.nheads) * 4);      // k_fin's finished in_proj values (fin)
     v.logits = put(B * (size_t)d.vocab * 4);
     v.next = put(B * 4);
     v.tok = put(B * 4);
@@ -339,6 +339,8 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         }
 
         tm->begin(DFSSM_KCLASS_SSM);
+        static const int ssm_v = getenv("DFSSM_SSM_V") ? atoi(getenv("DFSSM_SSM_V")) : 1;
+        if (ssm_v == 0) {
         k_bcdt<<<dim3((2 * d.ngroups * d.d_state + d.nheads + BCDT_THREADS - 1) / BCDT_THREADS, batch), BCDT_THREADS, 0, st>>>(
             L, d, acc, ld_acc, t, sx, conv, pos, at<float>(c, v.bcdt), tp, v.tap_stride, v.tl);
         ++nl;
@@ -353,6 +355,35 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
                 k_ssm<16, float><<<g16, SSM_THREADS, ssm_smem(d), st>>>(L, d, acc, ld_acc, t, sx, conv, pos, ssm, g, bc, tp, v.tap_stride, v.tl);
             else
                 k_ssm<16, __half><<<g16, SSM_THREADS, ssm_smem(d), st>>>(L, d, acc, ld_acc, t, sx, conv, pos, ssm_h, g, bc, tp, v.tap_stride, v.tl);
+        }
+        } else {
+        float* fin = at<float>(c, v.bcdt);
+        {
+            const dim3 gf((d.d_in_proj + FIN_THREADS - 1) / FIN_THREADS, batch);
+#define DFSSM_FIN_ARGS L, d, acc, ld_acc, t, sx, conv, pos, fin, tp, v.tap_stride, v.tl
+            switch (d.r) {
+                case 8: k_fin4<2><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS); break;
+                case 16: k_fin4<4><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS); break;
+                case 32: k_fin4<8><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS); break;
+                case 64: k_fin4<16><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS); break;
+                default: k_fin<<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS); break;
+            }
+#undef DFSSM_FIN_ARGS
+        }
+        ++nl;
+        {
+            const dim3 g32(d.headdim / 32, d.nheads, batch), g16(d.headdim / 16, d.nheads, batch);
+            const size_t sm = 2 * (size_t)d.d_state * sizeof(float);
+#define DFSSM_SSM_GO(PB_, DS_, G_)                                                                                          \
+    if (st16) k_ssm_stream<PB_, DS_, __half><<<G_, SSM_THREADS, sm, st>>>(L, d, fin, ssm_h, g, tp, v.tap_stride, v.tl);    \
+    else k_ssm_stream<PB_, DS_, float><<<G_, SSM_THREADS, sm, st>>>(L, d, fin, ssm, g, tp, v.tap_stride, v.tl)
+            if (d.headdim % 32 == 0) {
+                if (d.d_state == 128) { DFSSM_SSM_GO(32, 128, g32); }
+                else if (d.d_state == 64) { DFSSM_SSM_GO(32, 64, g32); }
+                else { DFSSM_SSM_GO(32, 0, g32); }
+            } else { DFSSM_SSM_GO(16, 0, g16); }
+#undef DFSSM_SSM_GO
+        }
         }
         tm->end(); ++nl;
 

@@ -470,6 +470,256 @@ k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
 }
 
 // =============================================================================================
+// S3 stage 2 + S4 conv + SiLU / softplus for EVERY in_proj row, once per sequence (the streaming state kernel below reads
+// finished values only):  fin[b] = [ silu(z) : d_inner ][ silu(conv(x | B | C)) : conv_dim ][ dt : nheads ][ dA : nheads ]
+//   grid = (ceil(d_in_proj / FIN_THREADS), batch).  Same arithmetic, value by value, as k_bcdt + the row prologue of k_ssm.
+// =============================================================================================
+constexpr int FIN_THREADS = 128;
+
+__global__ void __launch_bounds__(FIN_THREADS)
+k_fin(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int32_t* __restrict__ t,
+      const float* __restrict__ s_x, float* __restrict__ conv_ring, const int32_t* __restrict__ pos,
+      float* __restrict__ fin, uint8_t* __restrict__ taps, uint32_t tap_stride, TapLayout tl)
+{
+    __shared__ float v_sh[64];
+    const int b = blockIdx.y, tid = threadIdx.x;
+    const int gs = dm.ngroups * dm.d_state, d_in_proj = 2 * dm.d_inner + 2 * gs + dm.nheads;
+    if (tid < dm.r) v_sh[tid] = fmul(L.in_a_s[tid], (float)t[(size_t)b * T_STRIDE + tid]);
+    __syncthreads();
+    const int row = blockIdx.x * FIN_THREADS + tid;
+    if (row >= d_in_proj) return;
+    uint8_t* tp = taps ? taps + (size_t)b * tap_stride : nullptr;
+    float* out = fin + (size_t)b * (d_in_proj + dm.nheads);
+    const float val = proj_epilogue_row(acc[(size_t)b * ld_acc + row], L.in_row_scale, L.in_B, L.in_b_s, row, dm.r, v_sh, s_x[b]);
+    if (tp) ((float*)(tp + tl.off[4]))[row] = val;                               // ZXBCDT
+    if (row < dm.d_inner) {
+        out[row] = siluf(val);                                                   // the gate factor of S6
+    } else if (row < d_in_proj - dm.nheads) {
+        const int ps = pos[b] & 3;
+        const int c = row - dm.d_inner;                                          // conv channel
+        float* ring = conv_ring + ((size_t)b * dm.conv_dim + c) * 4;
+        const float4 rg = *(const float4*)ring;
+        const float sl[4] = { rg.x, rg.y, rg.z, rg.w };
+        const float s0 = sl[(ps + 1) & 3], s1 = sl[(ps + 2) & 3], s2 = sl[(ps + 3) & 3];
+        const float4 cw = *(const float4*)(L.conv_w + 4 * (size_t)c);
+        float o = L.conv_b[c];
+        o = ffma(cw.x, s0, o);
+        o = ffma(cw.y, s1, o);
+        o = ffma(cw.z, s2, o);
+        o = ffma(cw.w, val, o);
+        ring[ps] = val;
+        const float cv = siluf(o);
+        if (tp) ((float*)(tp + tl.off[5]))[c] = cv;                              // XBC_CONV
+        out[row] = cv;
+    } else {
+        const int h = row - (d_in_proj - dm.nheads);
+        const float dtv = sp_softplusf(fadd(val, L.dt_bias[h]));
+        if (tp) ((float*)(tp + tl.off[6]))[h] = dtv;                             // DT
+        out[row] = dtv;
+        out[row + dm.nheads] = sp_expf(fmul(dtv, -sp_expf(L.A_log[h])));         // dA (Eq. 5)
+    }
+}
+
+// k_fin for lora_rank = 4 * JW (JW = 2, 4, 8, 16): four lanes share a row's LoRA sum, each holding its JW values of v in
+// registers and reading its JW bytes of the row with one load (a warp reads 8 x 32 contiguous bytes per pass); a CTA of
+// FIN_THREADS threads finishes FIN_THREADS rows in 4 passes, then lane `sub` of a group finishes the row of pass `sub`, so that
+// the row epilogues (conv, SiLU, softplus) run on every lane and row = base + tid is coalesced.  fp64 sum, tree (p0+p1)+(p2+p3).
+// exact int8 -> binary64 without the conversion unit (I2F.F64 runs at a quarter of the fp64 rate): the byte with its sign bit
+// flipped is b + 128 in [0, 255]; as the low word of 2^52 it makes the double 2^52 + 128 + b, and the subtraction is exact.
+__device__ __forceinline__ double s8_to_double(uint8_t byte)
+{
+    return __hiloint2double(0x43300000, (int)(byte ^ 0x80u)) - 4503599627370624.0;      // 2^52 + 128
+}
+
+#ifndef DFSSM_FIN_MAGIC
+#define DFSSM_FIN_MAGIC 1
+#endif
+template <int JW> struct BytesT;
+template <> struct BytesT<2> { using T = uint16_t; };
+template <> struct BytesT<4> { using T = uint32_t; };
+template <> struct BytesT<8> { using T = uint2; };
+template <> struct BytesT<16> { using T = uint4; };
+
+template <int JW>
+__global__ void __launch_bounds__(FIN_THREADS)
+k_fin4(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int32_t* __restrict__ t,
+       const float* __restrict__ s_x, float* __restrict__ conv_ring, const int32_t* __restrict__ pos,
+       float* __restrict__ fin, uint8_t* __restrict__ taps, uint32_t tap_stride, TapLayout tl)
+{
+    constexpr int R = 4 * JW;
+    const int b = blockIdx.y, tid = threadIdx.x;
+    const int gs = dm.ngroups * dm.d_state, d_in_proj = 2 * dm.d_inner + 2 * gs + dm.nheads;
+    const int q = tid >> 2, sub = tid & 3;
+    const int base = blockIdx.x * FIN_THREADS;
+    const int row = base + tid;                                  // the row this lane finishes
+    const bool own = row < d_in_proj;
+
+    // requested early: everything the row epilogue needs
+    const int rl = own ? row : 0;
+    const int acc_i = acc[(size_t)b * ld_acc + rl];
+    const float rs = __half2float(L.in_row_scale[rl]), bs = L.in_b_s[rl], sx = s_x[b];
+    const bool is_conv = own && row >= dm.d_inner && row < d_in_proj - dm.nheads;
+    const int c = is_conv ? row - dm.d_inner : 0;                // conv channel
+    float* ring = conv_ring + ((size_t)b * dm.conv_dim + c) * 4;
+    float4 rg = make_float4(0.f, 0.f, 0.f, 0.f), cw = rg;
+    float cb = 0.f;
+    if (is_conv) {
+        rg = *(const float4*)ring;
+        cw = *(const float4*)(L.conv_w + 4 * (size_t)c);
+        cb = L.conv_b[c];
+    }
+
+    double v[JW];
+#pragma unroll
+    for (int i = 0; i < JW; ++i) {
+        const int j = sub * JW + i;
+        v[i] = (double)fmul(L.in_a_s[j], (float)t[(size_t)b * T_STRIDE + j]);
+    }
+    double part[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int rk = base + q * 4 + k;
+        double lo = 0.0;
+        if (rk < d_in_proj) {
+            const typename BytesT<JW>::T w = *(const typename BytesT<JW>::T*)(L.in_B + (size_t)rk * R + sub * JW);
+            const uint8_t* wb = (const uint8_t*)&w;
+#pragma unroll
+#if DFSSM_FIN_MAGIC
+            for (int i = 0; i < JW; ++i) lo = __fma_rn(s8_to_double(wb[i]), v[i], lo);
+#else
+            for (int i = 0; i < JW; ++i) lo = __fma_rn((double)(int)(int8_t)wb[i], v[i], lo);
+#endif
+        }
+        lo += __shfl_xor_sync(0xffffffffu, lo, 1);
+        lo += __shfl_xor_sync(0xffffffffu, lo, 2);
+        part[k] = lo;
+    }
+    if (!own) return;
+    const double lo = sub == 0 ? part[0] : sub == 1 ? part[1] : sub == 2 ? part[2] : part[3];
+    uint8_t* tp = taps ? taps + (size_t)b * tap_stride : nullptr;
+    float* out = fin + (size_t)b * (d_in_proj + dm.nheads);
+    const float val = fmul(sx, fadd(fmul(rs, (float)acc_i), fmul(bs, (float)lo)));
+    if (tp) ((float*)(tp + tl.off[4]))[row] = val;                               // ZXBCDT
+    if (row < dm.d_inner) {
+        out[row] = siluf(val);                                                   // the gate factor of S6
+    } else if (is_conv) {
+        const int ps = pos[b] & 3;
+        const float sl[4] = { rg.x, rg.y, rg.z, rg.w };
+        const float s0 = sl[(ps + 1) & 3], s1 = sl[(ps + 2) & 3], s2 = sl[(ps + 3) & 3];
+        float o = cb;
+        o = ffma(cw.x, s0, o);
+        o = ffma(cw.y, s1, o);
+        o = ffma(cw.z, s2, o);
+        o = ffma(cw.w, val, o);
+        ring[ps] = val;
+        const float cv = siluf(o);
+        if (tp) ((float*)(tp + tl.off[5]))[c] = cv;                              // XBC_CONV
+        out[row] = cv;
+    } else {
+        const int h = row - (d_in_proj - dm.nheads);
+        const float dtv = sp_softplusf(fadd(val, L.dt_bias[h]));
+        if (tp) ((float*)(tp + tl.off[6]))[h] = dtv;                             // DT
+        out[row] = dtv;
+        out[row + dm.nheads] = sp_expf(fmul(dtv, -sp_expf(L.A_log[h])));         // dA (Eq. 5)
+    }
+}
+
+// =============================================================================================
+// S5 state update + readout + S6 gate on finished inputs (k_fin): a pure stream over the state.
+//   grid = (headdim / PB, nheads, batch); every load of the CTA is issued before its only barrier.
+//   DS = d_state at compile time (no bounds checks, no tail loop: the kernel is issue-bound once the prologue is gone), 0 = any.
+// =============================================================================================
+#ifndef DFSSM_SSM_MINB
+#define DFSSM_SSM_MINB 5
+#endif
+template <int PB, int DS, typename ST>
+__global__ void __launch_bounds__(SSM_THREADS, DFSSM_SSM_MINB)
+k_ssm_stream(LayerW L, Dims dm, const float* __restrict__ fin, ST* __restrict__ ssm /* [batch][h][p][n] */,
+             float* __restrict__ g /* [batch][d_inner] */, uint8_t* __restrict__ taps, uint32_t tap_stride, TapLayout tl)
+{
+    extern __shared__ __align__(16) uint8_t smem[];
+    const int ds = DS ? DS : dm.d_state;
+    float* Bc = (float*)smem;                      // [d_state]
+    float* Cc = Bc + ds;                           // [d_state]
+    constexpr int LANES = SSM_THREADS / PB;        // lanes per state row
+    const int b = blockIdx.z, h = blockIdx.y, p0 = blockIdx.x * PB;
+    const int grp = dm.ngroups == 1 ? 0 : h / (dm.nheads / dm.ngroups);
+    const int tid = threadIdx.x;
+    const int gs = dm.ngroups * ds, d_in_proj = 2 * dm.d_inner + 2 * gs + dm.nheads;
+    const float* src = fin + (size_t)b * (d_in_proj + dm.nheads);
+
+    const int p = tid / LANES, l16 = tid % LANES;
+    const int ch = h * dm.headdim + p0 + p;
+    ST* Hr = ssm + ((size_t)b * dm.d_inner + ch) * ds;
+    constexpr int H_PRE = DS ? DS / 4 / LANES : 32 / LANES;    // chunks held in registers; with DS = 0 further ones are loaded late
+    static_assert(!DS || DS % (4 * LANES) == 0, "d_state must be a multiple of 4 * lanes per row");
+    float4 hpre[H_PRE];
+#pragma unroll
+    for (int j = 0; j < H_PRE; ++j) {
+        const int n4 = l16 + LANES * j;
+        if (DS || n4 < ds / 4) hpre[j] = state_ld4(Hr + 4 * n4);
+    }
+    const float xv = src[dm.d_inner + ch];
+    const float dtv = src[d_in_proj - dm.nheads + h], dA = src[d_in_proj + h];
+    const float sz = src[ch];                      // silu(z) from k_fin
+    const float Dh = L.D[h];
+    for (int i = tid; i < ds; i += SSM_THREADS) {
+        Bc[i] = src[2 * dm.d_inner + grp * ds + i];
+        Cc[i] = src[2 * dm.d_inner + gs + grp * ds + i];
+    }
+    __syncthreads();
+
+    const float dtx = fmul(dtv, xv);
+    double a = 0.0;
+#pragma unroll
+    for (int j = 0; j < H_PRE; ++j) {
+        const int n4 = l16 + LANES * j;
+        if (!DS && n4 >= ds / 4) break;
+        float4 hv = hpre[j];
+        const float4 bv = *(const float4*)(Bc + 4 * n4);
+        const float4 cv = *(const float4*)(Cc + 4 * n4);
+        hv.x = ffma(dA, hv.x, fmul(dtx, bv.x));
+        hv.y = ffma(dA, hv.y, fmul(dtx, bv.y));
+        hv.z = ffma(dA, hv.z, fmul(dtx, bv.z));
+        hv.w = ffma(dA, hv.w, fmul(dtx, bv.w));
+        state_st4(Hr + 4 * n4, hv);
+        a = dacc(a, cv.x, hv.x);
+        a = dacc(a, cv.y, hv.y);
+        a = dacc(a, cv.z, hv.z);
+        a = dacc(a, cv.w, hv.w);
+    }
+    if (!DS) {
+        for (int n4 = l16 + LANES * H_PRE; n4 < ds / 4; n4 += LANES) {
+            float4 hv = state_ld4(Hr + 4 * n4);
+            const float4 bv = *(const float4*)(Bc + 4 * n4);
+            const float4 cv = *(const float4*)(Cc + 4 * n4);
+            hv.x = ffma(dA, hv.x, fmul(dtx, bv.x));
+            hv.y = ffma(dA, hv.y, fmul(dtx, bv.y));
+            hv.z = ffma(dA, hv.z, fmul(dtx, bv.z));
+            hv.w = ffma(dA, hv.w, fmul(dtx, bv.w));
+            state_st4(Hr + 4 * n4, hv);
+            a = dacc(a, cv.x, hv.x);
+            a = dacc(a, cv.y, hv.y);
+            a = dacc(a, cv.z, hv.z);
+            a = dacc(a, cv.w, hv.w);
+        }
+    }
+#pragma unroll
+    for (int o = LANES / 2; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o, LANES);
+    if (l16 == 0) {
+        a = dacc(a, Dh, xv);
+        const float y = (float)a;
+        const float gv = fmul(y, sz);
+        g[(size_t)b * dm.d_inner + ch] = gv;
+        if (taps) {
+            uint8_t* tp = taps + (size_t)b * tap_stride;
+            ((float*)(tp + tl.off[7]))[ch] = y;
+            ((float*)(tp + tl.off[8]))[ch] = gv;
+        }
+    }
+}
+
+// =============================================================================================
 // S7 epilogue + residual: u_i <- u_i + s_g*( w_s[i]*acc_i + b_s[i]*lo_i )
 // =============================================================================================
 constexpr int EPI_THREADS = 128;
