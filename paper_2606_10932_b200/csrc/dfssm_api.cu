@@ -262,13 +262,14 @@ int launch_proj_mma(dfssm_ctx* ctx, const uint32_t* sign, const int8_t* A, int r
     const Dims& d = ctx->dm;
     const Carve& v = ctx->cv;
     const int mt = (rows + d.r + mma::TM - 1) / mma::TM, nt = (batch + mma::TN - 1) / mma::TN, nchunk = K / mma::KC;
-    int ks = (148 * MMA_CTAS_PER_SM) / (mt * nt);
+    static const int cps = getenv("DFSSM_MMA_CPS") ? atoi(getenv("DFSSM_MMA_CPS")) : MMA_CTAS_PER_SM;
+    int ks = (148 * cps) / (mt * nt);
     if (ks < 1) ks = 1;
     if (ks > nchunk) ks = nchunk;
     int32_t* acc = at<int32_t>(ctx, v.acc);
     int32_t* t = at<int32_t>(ctx, v.t);
     // ks > 1: acc / t were zeroed by the k_normquant launch in front of this projection
-    mma::k_proj_mma<<<dim3(mt, nt, ks), mma::THREADS, 0, ctx->stream>>>(sign, A, rows, d.r, K, at<int8_t>(ctx, v.xq), (int)v.ldq, batch,
+    mma::k_proj_mma<<<dim3(mt, nt, ks), mma::THREADS, mma::SMEM_BYTES, ctx->stream>>>(sign, A, rows, d.r, K, at<int8_t>(ctx, v.xq), (int)v.ldq, batch,
                                                                       acc, (int)v.ld_acc, t, at<int>(ctx, v.err));
     return DFSSM_OK;
 }
@@ -422,7 +423,7 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
 
     tm->begin(DFSSM_KCLASS_LMHEAD);
     if (use_mma(c, batch, d.d_model)) {
-        mma::k_proj_mma<<<dim3((d.vocab + mma::TM - 1) / mma::TM, (batch + mma::TN - 1) / mma::TN, 1), mma::THREADS, 0, st>>>(
+        mma::k_proj_mma<<<dim3((d.vocab + mma::TM - 1) / mma::TM, (batch + mma::TN - 1) / mma::TN, 1), mma::THREADS, mma::SMEM_BYTES, st>>>(
             nullptr, c->emb, 0, d.vocab, d.d_model, xq, ldq, batch, nullptr, 0, nullptr, err, logits, sx, c->emb_s);
     } else {
         const int per = LM_THREADS / 32;
@@ -634,7 +635,7 @@ int prefill_chunk(dfssm_ctx* c, const int32_t* tokens_dev, int T, int seq)
             int ks = (148 * MMA_CTAS_PER_SM) / (mt * nt);
             if (ks < 1) ks = 1;
             if (ks > nchunk) ks = nchunk;
-            mma::k_proj_mma<<<dim3(mt, nt, ks), mma::THREADS, 0, st>>>(sign, A, rows, d.r, K, xq, ldq, T, acc, ld_acc, t, err);
+            mma::k_proj_mma<<<dim3(mt, nt, ks), mma::THREADS, mma::SMEM_BYTES, st>>>(sign, A, rows, d.r, K, xq, ldq, T, acc, ld_acc, t, err);
         } else {
             k_proj<<<dim3(proj_grid(rows + d.r), (T + PROJ_BT - 1) / PROJ_BT), PROJ_THREADS, proj_smem(K), st>>>(sign, A, rows, d.r, K, xq, xqp, ldq, qsum,
                                                                                                               T, acc, ld_acc, t);
@@ -733,6 +734,7 @@ int dfssm_create(const dfssm_config* cfg, void* dev_arena, size_t arena_bytes, v
     CK(cudaMallocHost((void**)&ctx->pinned_err, sizeof(int)));
     CK(cudaFuncSetAttribute(k_proj, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)proj_smem(8192)));
     CK(cudaFuncSetAttribute(k_lmhead, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lm_smem(8192)));
+    CK(cudaFuncSetAttribute(mma::k_proj_mma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mma::SMEM_BYTES));
     {
         const int rc = mega_setup(ctx);
         if (rc != DFSSM_OK) return rc;

@@ -21,9 +21,11 @@ namespace mma {
 constexpr int TM = 128;            // rows of the weight tile (MMA M)
 constexpr int TN = 64;             // sequences per tile (MMA N)
 constexpr int KC = 128;            // bytes of K per shared-memory stage (4 MMAs of K = 32)
-constexpr int THREADS = 128;
+constexpr int THREADS = 512;
 constexpr uint32_t LBO_A = (TM / 8) * 128, LBO_B = (TN / 8) * 128, SBO = 128;
 constexpr uint32_t SPIN_LIMIT = 1u << 22;
+constexpr int STAGES = 2;                                  // shared-memory stages: the unpack of chunk k + 1 runs under the MMAs of chunk k
+constexpr size_t SMEM_BYTES = (size_t)STAGES * (TM + TN) * KC;    // dynamic shared memory of k_proj_mma
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -43,20 +45,22 @@ __device__ __forceinline__ uint32_t signs4(uint32_t bits)
     return 0xffffffffu ^ (spread * 0xfeu);
 }
 
-// grid = (ceil((rows + r) / 128), ceil(batch / 64), ksplit); 128 threads; K % 128 == 0.  LM head: rows = 0, r = vocab,
+// grid = (ceil((rows + r) / 128), ceil(batch / 64), ksplit); 512 threads; K % 128 == 0.  LM head: rows = 0, r = vocab,
 // A = the embedding, ksplit = 1, logits / s_h / e_s given.  With ksplit > 1 every CTA takes a
 // slice of K and ADDS its int32 partial sums into acc / t (exact in any order), which the caller has zeroed.
+// 16 warps: the kernel was bound by the issue latency of 4 warps that unpack, stage and store in turn (ncu: 11 % of the warp
+// slots, one issue per 8 cycles per warp); a thread now unpacks 32 weights and stages 16 codes per chunk, and a warp reads one
+// 32-lane x 16-column block of the accumulators.
 __global__ void __launch_bounds__(THREADS)
 k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int rows, int r, int K,
            const int8_t* __restrict__ xq, int ldq, int batch, int32_t* __restrict__ acc, int ld_acc,
            int32_t* __restrict__ t, int* __restrict__ err,
            float* __restrict__ logits = nullptr, const float* __restrict__ s_h = nullptr, const float* __restrict__ e_s = nullptr)
 {
-    __shared__ __align__(128) uint8_t sA[TM * KC];
-    __shared__ __align__(128) uint8_t sB[TN * KC];
-    __shared__ __align__(8) uint64_t mbar;
+    extern __shared__ __align__(128) uint8_t stage_mem[];     // [STAGES][ A tile TM x KC | B tile TN x KC ]
+    __shared__ __align__(8) uint64_t mbar[STAGES];
     __shared__ uint32_t tmem_base;
-    const int tid = threadIdx.x, wid = tid >> 5;
+    const int tid = threadIdx.x, wid = tid >> 5, lane = tid & 31;
     const int row0 = blockIdx.x * TM, b0 = blockIdx.y * TN;
     const int rows_total = rows + r;
     const int W = K / 32;
@@ -66,7 +70,8 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     if (tid == 0) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&mbar)) : "memory");
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&mbar[s])) : "memory");
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -74,105 +79,113 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem = tmem_base;
 
-    const int grow = row0 + tid;                      // the weight row this thread unpacks
-    const int bn = tid >> 1, bhalf = tid & 1;          // the sequence / half chunk of codes this thread stages
+    // unpack: thread = (K quarter qk, tile row am): 32 weights = the two 16-byte K columns 2 qk, 2 qk + 1 of row am; a warp
+    // writes 32 consecutive rows of one column (512 contiguous bytes of shared memory)
+    const int am = tid & (TM - 1), qk = tid >> 7;
+    const int urow = row0 + am;                        // the weight row this thread unpacks
+    // stage: thread = (16-byte piece xc, sequence bn)
+    const int bn = tid & (TN - 1), xc = tid >> 6;
     const bool b_valid = b0 + bn < batch;
-    uint8_t* a_dst = sA + (tid >> 3) * 128 + (tid & 7) * 16;
-    uint8_t* b_dst = sB + (bn >> 3) * 128 + (bn & 7) * 16;
+    const uint32_t a_off = (uint32_t)(2 * qk) * LBO_A + (am >> 3) * 128 + (am & 7) * 16;
+    const uint32_t b_off = TM * KC + (uint32_t)xc * LBO_B + (bn >> 3) * 128 + (bn & 7) * 16;
     bool dead = false;
+    // waits until the MMAs committed to mbar[s] in phase `parity` have read their stage; a thread that timed out stops waiting
+    // (it still runs through every barrier of the loop, so the CTA stays in step) and the failure is reported at the end
+    auto wait_stage = [&](int s, uint32_t parity) {
+        uint32_t spins = 0, ok = 0;
+        while (!ok && !dead) {
+            asm volatile(
+                "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                : "=r"(ok) : "r"(smem_u32(&mbar[s])), "r"(parity) : "memory");
+            if (!ok && ++spins > SPIN_LIMIT) dead = true;
+        }
+    };
 
     const int nchunk = K / KC, kc0 = (int)(((long long)blockIdx.z * nchunk) / gridDim.z), kc1 = (int)(((long long)(blockIdx.z + 1) * nchunk) / gridDim.z);
     const bool split = gridDim.z > 1;
-    // the sign words and the codes of a chunk are requested one chunk ahead (registers), so that their latency runs under the
-    // MMAs and the wait of the chunk before; the few LoRA-down rows (last tile only) are read directly
-    const bool is_sign = grow < rows;
-    const uint32_t* sign_row = sign + (size_t)(is_sign ? grow : 0) * W;
-    const int8_t* x_row = xq + (size_t)(b_valid ? b0 + bn : 0) * ldq + bhalf * (KC / 2);
-    uint4 w_next = make_uint4(0, 0, 0, 0), x_next[KC / 32];
+    // the sign word and the codes of a chunk are requested one chunk ahead (registers), so that their latency runs under the
+    // MMAs of the chunk before; the few LoRA-down rows (last tile only) are read directly
+    const bool is_sign = urow < rows;
+    const uint32_t* sign_row = sign + (size_t)(is_sign ? urow : 0) * W + qk;
+    const int8_t* x_row = xq + (size_t)(b_valid ? b0 + bn : 0) * ldq + xc * 16;
+    uint32_t w_next = 0;
+    uint4 x_next = make_uint4(0, 0, 0, 0);
     auto request = [&](int kc) {
-        if (is_sign) w_next = *(const uint4*)(sign_row + kc * (KC / 32));
-#pragma unroll
-        for (int c = 0; c < KC / 32; ++c) x_next[c] = b_valid ? ((const uint4*)(x_row + kc * KC))[c] : make_uint4(0, 0, 0, 0);
+        if (is_sign) w_next = sign_row[kc * (KC / 32)];
+        if (b_valid) x_next = *(const uint4*)(x_row + kc * KC);
     };
     if (kc0 < kc1) request(kc0);
     for (int kc = kc0; kc < kc1; ++kc) {
-        // ---- A: 128 weights of this row -> int8 ----
+        const int it = kc - kc0, s = it % STAGES, use = it / STAGES;
+        uint8_t* a_dst = stage_mem + (size_t)s * (TM + TN) * KC + a_off;
+        uint8_t* b_dst = stage_mem + (size_t)s * (TM + TN) * KC + b_off;
+        if (use > 0) wait_stage(s, (uint32_t)(use - 1) & 1u);           // the MMAs that read this stage last are done
+        // ---- A: 32 weights of this row -> int8 ----
         if (is_sign) {
-            const uint32_t ww[4] = { w_next.x, w_next.y, w_next.z, w_next.w };
-#pragma unroll
-            for (int c = 0; c < KC / 16; ++c) {                       // 16 weights per 16-byte K column
-                const uint32_t b16 = (ww[c >> 1] >> (16 * (c & 1))) & 0xffffu;
-                *(uint4*)(a_dst + c * LBO_A) = make_uint4(signs4(b16), signs4(b16 >> 4), signs4(b16 >> 8), signs4(b16 >> 12));
-            }
-        } else if (grow < rows_total) {
-            const uint4* src = (const uint4*)(A + (size_t)(grow - rows) * K + kc * KC);
-#pragma unroll
-            for (int c = 0; c < KC / 16; ++c) *(uint4*)(a_dst + c * LBO_A) = src[c];
+            const uint32_t w = w_next;
+            *(uint4*)a_dst = make_uint4(signs4(w), signs4(w >> 4), signs4(w >> 8), signs4(w >> 12));
+            *(uint4*)(a_dst + LBO_A) = make_uint4(signs4(w >> 16), signs4(w >> 20), signs4(w >> 24), signs4(w >> 28));
+        } else if (urow < rows_total) {
+            const uint4* src = (const uint4*)(A + (size_t)(urow - rows) * K + kc * KC + qk * 32);
+            *(uint4*)a_dst = src[0];
+            *(uint4*)(a_dst + LBO_A) = src[1];
         } else {
-#pragma unroll
-            for (int c = 0; c < KC / 16; ++c) *(uint4*)(a_dst + c * LBO_A) = make_uint4(0, 0, 0, 0);
+            *(uint4*)a_dst = make_uint4(0, 0, 0, 0);
+            *(uint4*)(a_dst + LBO_A) = make_uint4(0, 0, 0, 0);
         }
-        // ---- B: 64 codes of one sequence ----
-#pragma unroll
-        for (int c = 0; c < KC / 32; ++c) *(uint4*)(b_dst + (bhalf * (KC / 32) + c) * LBO_B) = x_next[c];
+        // ---- B: 16 codes of one sequence ----
+        *(uint4*)b_dst = x_next;
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the tensor core
         __syncthreads();
         if (tid == 0) {
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll
             for (int j = 0; j < KC / 32; ++j) {
-                const uint64_t da = smem_desc(smem_u32(sA) + j * 2 * LBO_A, LBO_A, SBO);
-                const uint64_t db = smem_desc(smem_u32(sB) + j * 2 * LBO_B, LBO_B, SBO);
+                const uint32_t sbase = smem_u32(stage_mem) + (uint32_t)s * (TM + TN) * KC;
+                const uint64_t da = smem_desc(sbase + j * 2 * LBO_A, LBO_A, SBO);
+                const uint64_t db = smem_desc(sbase + TM * KC + j * 2 * LBO_B, LBO_B, SBO);
                 const uint32_t accumulate = (kc > kc0 || j > 0) ? 1u : 0u;
                 asm volatile(
                     "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
                     "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, {%5, %6, %7, %8}, p;\n\t}"
                     ::"r"(tmem), "l"(da), "l"(db), "r"(IDESC), "r"(accumulate), "r"(0u), "r"(0u), "r"(0u), "r"(0u) : "memory");
             }
-            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(&mbar)) : "memory");
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(&mbar[s])) : "memory");
         }
         if (kc + 1 < kc1) request(kc + 1);
-        // ---- wait until the MMAs of this stage have read shared memory ----
-        {
-            const uint32_t parity = (uint32_t)(kc - kc0) & 1u;
-            uint32_t spins = 0, ok = 0;
-            while (!ok && !dead) {      // a thread that timed out keeps going through the loop (same barrier count as the others) without waiting
-                asm volatile(
-                    "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                    : "=r"(ok) : "r"(smem_u32(&mbar)), "r"(parity) : "memory");
-                if (!ok && ++spins > SPIN_LIMIT) dead = true;
-            }
-        }
+    }
+    // ---- the last commit covers every MMA before it: wait for it, then read the accumulators ----
+    if (kc1 > kc0) {
+        const int it = kc1 - 1 - kc0;
+        wait_stage(it % STAGES, (uint32_t)(it / STAGES) & 1u);
     }
     if (dead) atomicOr(err, 4);
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 
-    // ---- epilogue: TMEM lane = row of the tile, column = sequence ----
-    if (!__syncthreads_or(dead ? 1 : 0)) {
+    // ---- epilogue: TMEM lane = row of the tile, column = sequence; warp = (lane quarter wid % 4, 16 columns wid / 4) ----
+    if (!__syncthreads_or(dead ? 1 : 0) && kc1 > kc0) {
+        const int grow = row0 + (wid & 3) * 32 + lane, cg = wid >> 2;
         const bool is_acc = grow < rows, is_t = !is_acc && grow < rows_total;
+        uint32_t v[16];
+        const uint32_t taddr = tmem + ((uint32_t)((wid & 3) * 32) << 16) + (uint32_t)(cg * 16);
+        asm volatile(
+            "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+            : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+              "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+            : "r"(taddr) : "memory");
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
-        for (int q = 0; q < TN / 16; ++q) {
-            uint32_t v[16];
-            const uint32_t taddr = tmem + ((uint32_t)(wid * 32) << 16) + (uint32_t)(q * 16);
-            asm volatile(
-                "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
-                  "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                : "r"(taddr) : "memory");
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-            for (int i = 0; i < 16; ++i) {
-                const int b = b0 + q * 16 + i;
-                if (b < batch) {
-                    if (logits) {          // S8: logit_v = float(acc_v) * (s_h * e_s[v])   (R16); rows == 0, r == vocab
-                        if (is_t) logits[(size_t)b * r + grow] = fmul((float)(int32_t)v[i], fmul(s_h[b], e_s[grow]));
-                        continue;
-                    }
-                    int32_t* dst = is_acc ? acc + (size_t)b * ld_acc + grow : t + (size_t)b * T_STRIDE + (grow - rows);
-                    if (is_acc || is_t) {
-                        if (split) atomicAdd(dst, (int32_t)v[i]);
-                        else *dst = (int32_t)v[i];
-                    }
+        for (int i = 0; i < 16; ++i) {
+            const int b = b0 + cg * 16 + i;
+            if (b < batch) {
+                if (logits) {          // S8: logit_v = float(acc_v) * (s_h * e_s[v])   (R16); rows == 0, r == vocab
+                    if (is_t) logits[(size_t)b * r + grow] = fmul((float)(int32_t)v[i], fmul(s_h[b], e_s[grow]));
+                    continue;
+                }
+                int32_t* dst = is_acc ? acc + (size_t)b * ld_acc + grow : t + (size_t)b * T_STRIDE + (grow - rows);
+                if (is_acc || is_t) {
+                    if (split) atomicAdd(dst, (int32_t)v[i]);
+                    else *dst = (int32_t)v[i];
                 }
             }
         }
