@@ -248,7 +248,7 @@ int proj_grid(int rows_total)
 // batch >= 16: the projections run on the tensor cores (tcgen05 kind::i8 on +-1 tiles unpacked in shared memory)
 bool use_mma(const dfssm_ctx* c, int batch, int K)
 {
-    return batch >= 16 && K % mma::KC == 0 && !(c->cfg.flags & DFSSM_FLAG_NO_MMA);
+    return batch >= 16 && K % mma::KMULT == 0 && !(c->cfg.flags & DFSSM_FLAG_NO_MMA);
 }
 
 // one projection on the tensor cores; K is split over CTAs until the grid fills the 148 SMs (partial sums are added
@@ -261,7 +261,7 @@ int launch_proj_mma(dfssm_ctx* ctx, const uint32_t* sign, const int8_t* A, int r
 {
     const Dims& d = ctx->dm;
     const Carve& v = ctx->cv;
-    const int mt = (rows + d.r + mma::TM - 1) / mma::TM, nt = (batch + mma::TN - 1) / mma::TN, nchunk = K / mma::KC;
+    const int mt = (rows + d.r + mma::TM - 1) / mma::TM, nt = (batch + mma::TN - 1) / mma::TN, nchunk = (K + mma::KC - 1) / mma::KC;
     static const int cps = getenv("DFSSM_MMA_CPS") ? atoi(getenv("DFSSM_MMA_CPS")) : MMA_CTAS_PER_SM;
     int ks = (148 * cps) / (mt * nt);
     if (ks < 1) ks = 1;
@@ -631,7 +631,7 @@ int prefill_chunk(dfssm_ctx* c, const int32_t* tokens_dev, int T, int seq)
     const int ldq = (int)v.ldq, ld_acc = (int)v.ld_acc;
     auto proj = [&](const uint32_t* sign, const int8_t* A, int rows, int K) {
         if (use_mma(c, T, K)) {
-            const int mt = (rows + d.r + mma::TM - 1) / mma::TM, nt = (T + mma::TN - 1) / mma::TN, nchunk = K / mma::KC;
+            const int mt = (rows + d.r + mma::TM - 1) / mma::TM, nt = (T + mma::TN - 1) / mma::TN, nchunk = (K + mma::KC - 1) / mma::KC;
             int ks = (148 * MMA_CTAS_PER_SM) / (mt * nt);
             if (ks < 1) ks = 1;
             if (ks > nchunk) ks = nchunk;

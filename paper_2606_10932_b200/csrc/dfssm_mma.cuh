@@ -20,7 +20,8 @@ namespace mma {
 
 constexpr int TM = 128;            // rows of the weight tile (MMA M)
 constexpr int TN = 64;             // sequences per tile (MMA N)
-constexpr int KC = 128;            // bytes of K per shared-memory stage (4 MMAs of K = 32)
+constexpr int KC = 256;            // bytes of K per shared-memory stage (8 MMAs of K = 32); K itself may be any multiple of KMULT
+constexpr int KMULT = 128;         // (a last half stage is filled with zeros)
 constexpr int THREADS = 512;
 constexpr uint32_t LBO_A = (TM / 8) * 128, LBO_B = (TN / 8) * 128, SBO = 128;
 constexpr uint32_t SPIN_LIMIT = 1u << 22;
@@ -79,14 +80,14 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem = tmem_base;
 
-    // unpack: thread = (K quarter qk, tile row am): 32 weights = the two 16-byte K columns 2 qk, 2 qk + 1 of row am; a warp
+    // unpack: thread = (K quarter qk, tile row am): 64 weights = the four 16-byte K columns 4 qk .. 4 qk + 3 of row am; a warp
     // writes 32 consecutive rows of one column (512 contiguous bytes of shared memory)
     const int am = tid & (TM - 1), qk = tid >> 7;
     const int urow = row0 + am;                        // the weight row this thread unpacks
-    // stage: thread = (16-byte piece xc, sequence bn)
+    // stage: thread = (16-byte pieces xc and xc + 8, sequence bn)
     const int bn = tid & (TN - 1), xc = tid >> 6;
     const bool b_valid = b0 + bn < batch;
-    const uint32_t a_off = (uint32_t)(2 * qk) * LBO_A + (am >> 3) * 128 + (am & 7) * 16;
+    const uint32_t a_off = (uint32_t)(4 * qk) * LBO_A + (am >> 3) * 128 + (am & 7) * 16;
     const uint32_t b_off = TM * KC + (uint32_t)xc * LBO_B + (bn >> 3) * 128 + (bn & 7) * 16;
     bool dead = false;
     // waits until the MMAs committed to mbar[s] in phase `parity` have read their stage; a thread that timed out stops waiting
@@ -101,40 +102,49 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
         }
     };
 
-    const int nchunk = K / KC, kc0 = (int)(((long long)blockIdx.z * nchunk) / gridDim.z), kc1 = (int)(((long long)(blockIdx.z + 1) * nchunk) / gridDim.z);
+    const int nchunk = (K + KC - 1) / KC, kc0 = (int)(((long long)blockIdx.z * nchunk) / gridDim.z), kc1 = (int)(((long long)(blockIdx.z + 1) * nchunk) / gridDim.z);
     const bool split = gridDim.z > 1;
-    // the sign word and the codes of a chunk are requested one chunk ahead (registers), so that their latency runs under the
-    // MMAs of the chunk before; the few LoRA-down rows (last tile only) are read directly
+    // the sign words and the codes of a stage are requested one stage ahead (registers), before the stage in hand is unpacked,
+    // so that their latency runs under the unpack and the MMAs; the few LoRA-down rows (last tile only) are read directly
     const bool is_sign = urow < rows;
-    const uint32_t* sign_row = sign + (size_t)(is_sign ? urow : 0) * W + qk;
+    const uint32_t* sign_row = sign + (size_t)(is_sign ? urow : 0) * W + 2 * qk;
     const int8_t* x_row = xq + (size_t)(b_valid ? b0 + bn : 0) * ldq + xc * 16;
-    uint32_t w_next = 0;
-    uint4 x_next = make_uint4(0, 0, 0, 0);
+    uint2 w_next = make_uint2(0, 0), w_cur;
+    uint4 x_next[2] = { make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0) }, x_cur[2];
     auto request = [&](int kc) {
-        if (is_sign) w_next = sign_row[kc * (KC / 32)];
-        if (b_valid) x_next = *(const uint4*)(x_row + kc * KC);
+        // byte offsets of this thread's pieces inside K; beyond K (last half stage) the operands are zero
+        const int ka = kc * KC + qk * 64, kx = kc * KC + xc * 16;
+        w_next = (is_sign && ka < K) ? *(const uint2*)(sign_row + kc * (KC / 32)) : make_uint2(0, 0);
+        x_next[0] = (b_valid && kx < K) ? *(const uint4*)(x_row + kc * KC) : make_uint4(0, 0, 0, 0);
+        x_next[1] = (b_valid && kx + 128 < K) ? *(const uint4*)(x_row + kc * KC + 128) : make_uint4(0, 0, 0, 0);
     };
     if (kc0 < kc1) request(kc0);
     for (int kc = kc0; kc < kc1; ++kc) {
         const int it = kc - kc0, s = it % STAGES, use = it / STAGES;
         uint8_t* a_dst = stage_mem + (size_t)s * (TM + TN) * KC + a_off;
         uint8_t* b_dst = stage_mem + (size_t)s * (TM + TN) * KC + b_off;
+        w_cur = w_next; x_cur[0] = x_next[0]; x_cur[1] = x_next[1];
+        if (kc + 1 < kc1) request(kc + 1);
         if (use > 0) wait_stage(s, (uint32_t)(use - 1) & 1u);           // the MMAs that read this stage last are done
-        // ---- A: 32 weights of this row -> int8 ----
-        if (is_sign) {
-            const uint32_t w = w_next;
-            *(uint4*)a_dst = make_uint4(signs4(w), signs4(w >> 4), signs4(w >> 8), signs4(w >> 12));
-            *(uint4*)(a_dst + LBO_A) = make_uint4(signs4(w >> 16), signs4(w >> 20), signs4(w >> 24), signs4(w >> 28));
-        } else if (urow < rows_total) {
-            const uint4* src = (const uint4*)(A + (size_t)(urow - rows) * K + kc * KC + qk * 32);
-            *(uint4*)a_dst = src[0];
-            *(uint4*)(a_dst + LBO_A) = src[1];
+        // ---- A: 64 weights of this row -> int8 ----
+        const bool a_in = kc * KC + qk * 64 < K;
+        if (is_sign && a_in) {
+            const uint32_t w0 = w_cur.x, w1 = w_cur.y;
+            *(uint4*)a_dst = make_uint4(signs4(w0), signs4(w0 >> 4), signs4(w0 >> 8), signs4(w0 >> 12));
+            *(uint4*)(a_dst + LBO_A) = make_uint4(signs4(w0 >> 16), signs4(w0 >> 20), signs4(w0 >> 24), signs4(w0 >> 28));
+            *(uint4*)(a_dst + 2 * LBO_A) = make_uint4(signs4(w1), signs4(w1 >> 4), signs4(w1 >> 8), signs4(w1 >> 12));
+            *(uint4*)(a_dst + 3 * LBO_A) = make_uint4(signs4(w1 >> 16), signs4(w1 >> 20), signs4(w1 >> 24), signs4(w1 >> 28));
+        } else if (!is_sign && urow < rows_total && a_in) {
+            const uint4* src = (const uint4*)(A + (size_t)(urow - rows) * K + kc * KC + qk * 64);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) *(uint4*)(a_dst + c * LBO_A) = src[c];
         } else {
-            *(uint4*)a_dst = make_uint4(0, 0, 0, 0);
-            *(uint4*)(a_dst + LBO_A) = make_uint4(0, 0, 0, 0);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) *(uint4*)(a_dst + c * LBO_A) = make_uint4(0, 0, 0, 0);
         }
-        // ---- B: 16 codes of one sequence ----
-        *(uint4*)b_dst = x_next;
+        // ---- B: 2 x 16 codes of one sequence ----
+        *(uint4*)b_dst = x_cur[0];
+        *(uint4*)(b_dst + 8 * LBO_B) = x_cur[1];
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the tensor core
         __syncthreads();
         if (tid == 0) {
@@ -152,7 +162,6 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
             }
             asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(&mbar[s])) : "memory");
         }
-        if (kc + 1 < kc1) request(kc + 1);
     }
     // ---- the last commit covers every MMA before it: wait for it, then read the accumulators ----
     if (kc1 > kc0) {
