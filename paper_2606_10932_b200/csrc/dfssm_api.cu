@@ -235,7 +235,6 @@ struct KTimer {                       // optional per-kernel-class device timing
 
 size_t proj_smem(int K) { return (size_t)PROJ_BT * 2 * K; }
 size_t lm_smem(int K) { return (size_t)PROJ_BT * K; }
-size_t ssm_smem(const Dims& d) { return sizeof(float) * (64 + 2 * (size_t)d.d_state + 2 * 32 + 4); }
 
 int proj_grid(int rows_total)
 {
@@ -272,6 +271,22 @@ int launch_proj_mma(dfssm_ctx* ctx, const uint32_t* sign, const int8_t* A, int r
     mma::k_proj_mma<<<dim3(mt, nt, ks), mma::THREADS, mma::SMEM_BYTES, ctx->stream>>>(sign, A, rows, d.r, K, at<int8_t>(ctx, v.xq), (int)v.ldq, batch,
                                                                       acc, (int)v.ld_acc, t, at<int>(ctx, v.err));
     return DFSSM_OK;
+}
+
+// S7 epilogue + residual for n sequences / positions: four lanes per row when the LoRA rank allows (k_epi_out4)
+void launch_epi_out(const LayerW& L, const Dims& d, int n, const int32_t* acc, int ld_acc, const int32_t* t, const float* s_g, float* u,
+                    uint8_t* tp, uint32_t tap_stride, uint32_t tap_off, cudaStream_t st)
+{
+    const dim3 g4((d.d_model + FIN_THREADS - 1) / FIN_THREADS, n);
+    switch (d.r) {
+        case 8: k_epi_out4<2><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off); break;
+        case 16: k_epi_out4<4><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off); break;
+        case 32: k_epi_out4<8><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off); break;
+        case 64: k_epi_out4<16><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off); break;
+        default:
+            k_epi_out<<<dim3((d.d_model + EPI_THREADS - 1) / EPI_THREADS, n), EPI_THREADS, 0, st>>>(L, d.d_model, d.r, acc, ld_acc, t, s_g, u, tp, tap_stride,
+                                                                                                  tap_off);
+    }
 }
 
 // Enqueue S0, L x (S1..S7), S8 for `batch` sequences on the context's stream.  The input tokens are
@@ -340,24 +355,7 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         }
 
         tm->begin(DFSSM_KCLASS_SSM);
-        static const int ssm_v = getenv("DFSSM_SSM_V") ? atoi(getenv("DFSSM_SSM_V")) : 1;
-        if (ssm_v == 0) {
-        k_bcdt<<<dim3((2 * d.ngroups * d.d_state + d.nheads + BCDT_THREADS - 1) / BCDT_THREADS, batch), BCDT_THREADS, 0, st>>>(
-            L, d, acc, ld_acc, t, sx, conv, pos, at<float>(c, v.bcdt), tp, v.tap_stride, v.tl);
-        ++nl;
         {
-            const dim3 g32(d.nheads * (d.headdim / 32), batch), g16(d.nheads * (d.headdim / 16), batch);
-            float* bc = at<float>(c, v.bcdt);
-            if (d.headdim % 32 == 0 && !st16)
-                k_ssm<32, float><<<g32, SSM_THREADS, ssm_smem(d), st>>>(L, d, acc, ld_acc, t, sx, conv, pos, ssm, g, bc, tp, v.tap_stride, v.tl);
-            else if (d.headdim % 32 == 0)
-                k_ssm<32, __half><<<g32, SSM_THREADS, ssm_smem(d), st>>>(L, d, acc, ld_acc, t, sx, conv, pos, ssm_h, g, bc, tp, v.tap_stride, v.tl);
-            else if (!st16)
-                k_ssm<16, float><<<g16, SSM_THREADS, ssm_smem(d), st>>>(L, d, acc, ld_acc, t, sx, conv, pos, ssm, g, bc, tp, v.tap_stride, v.tl);
-            else
-                k_ssm<16, __half><<<g16, SSM_THREADS, ssm_smem(d), st>>>(L, d, acc, ld_acc, t, sx, conv, pos, ssm_h, g, bc, tp, v.tap_stride, v.tl);
-        }
-        } else {
         float* fin = at<float>(c, v.bcdt);
         {
             const dim3 gf((d.d_in_proj + FIN_THREADS - 1) / FIN_THREADS, batch);
@@ -411,8 +409,7 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         }
 
         tm->begin(DFSSM_KCLASS_EPI_OUT);
-        k_epi_out<<<dim3((d.d_model + EPI_THREADS - 1) / EPI_THREADS, batch), EPI_THREADS, 0, st>>>(
-            L, d.d_model, d.r, acc, ld_acc, t, sx, u, tp, v.tap_stride, v.tl.off[DFSSM_TAP_HIDDEN]);
+        launch_epi_out(L, d, batch, acc, ld_acc, t, sx, u, tp, v.tap_stride, v.tl.off[DFSSM_TAP_HIDDEN], st);
         tm->end(); ++nl;
     }
 
@@ -672,7 +669,7 @@ int prefill_chunk(dfssm_ctx* c, const int32_t* tokens_dev, int T, int seq)
         k_normquant<<<T, NQ_THREADS, 0, st>>>(g, d.d_inner, L.gnorm_w, d.d_inner, d.eps, xq, xqp, ldq, sx, qsum, nullptr, 0, 0, 0,
                                               use_mma(c, T, d.d_inner) ? acc : nullptr, ld_acc, t);
         proj(L.out_sign, L.out_A, d.d_model, d.d_inner);
-        k_epi_out<<<dim3((d.d_model + EPI_THREADS - 1) / EPI_THREADS, T), EPI_THREADS, 0, st>>>(L, d.d_model, d.r, acc, ld_acc, t, sx, u, nullptr, 0, 0);
+        launch_epi_out(L, d, T, acc, ld_acc, t, sx, u, nullptr, 0, 0, st);
     }
     // the last position: hidden state, logits and greedy token of the sequence; the conv ring position advances by T
     const float* u_last = u + (size_t)(T - 1) * d.d_model;

@@ -251,62 +251,6 @@ __device__ __forceinline__ float proj_epilogue_row(int acc_i, const __half* __re
     return fmul(s_x, fadd(m1, m2));
 }
 
-// =============================================================================================
-// S3 stage 2 + S4 conv + softplus for the B | C | dt rows, ONCE per sequence (every head reads them):
-//   bcdt[b][e] = silu(conv(B|C row e))  for e < 2*gs,   softplus(dt row + dt_bias)  for the nheads rows behind.
-//   grid = (ceil(n_bcdt / BCDT_THREADS), batch)
-// =============================================================================================
-constexpr int BCDT_THREADS = 128;
-
-__global__ void __launch_bounds__(BCDT_THREADS)
-k_bcdt(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int32_t* __restrict__ t,
-       const float* __restrict__ s_x, float* __restrict__ conv_ring, const int32_t* __restrict__ pos,
-       float* __restrict__ bcdt, uint8_t* __restrict__ taps, uint32_t tap_stride, TapLayout tl)
-{
-    __shared__ float v_sh[64];
-    const int b = blockIdx.y, tid = threadIdx.x;
-    const int gs = dm.ngroups * dm.d_state, n_bcdt = 2 * gs + dm.nheads;
-    if (tid < dm.r) v_sh[tid] = fmul(L.in_a_s[tid], (float)t[(size_t)b * T_STRIDE + tid]);
-    __syncthreads();
-    const int e = blockIdx.x * BCDT_THREADS + tid;
-    if (e >= n_bcdt) return;
-    const int row = 2 * dm.d_inner + e;
-    uint8_t* tp = taps ? taps + (size_t)b * tap_stride : nullptr;
-    const float val = proj_epilogue_row(acc[(size_t)b * ld_acc + row], L.in_row_scale, L.in_B, L.in_b_s, row, dm.r, v_sh, s_x[b]);
-    if (tp) ((float*)(tp + tl.off[4]))[row] = val;                               // ZXBCDT
-    float out;
-    if (e < 2 * gs) {
-        const int ps = pos[b] & 3;
-        const int c = dm.d_inner + e;                                            // conv channel
-        float* ring = conv_ring + ((size_t)b * dm.conv_dim + c) * 4;
-        const float4 rg = *(const float4*)ring;
-        const float sl[4] = { rg.x, rg.y, rg.z, rg.w };
-        const float s0 = sl[(ps + 1) & 3], s1 = sl[(ps + 2) & 3], s2 = sl[(ps + 3) & 3];
-        const float4 cw = *(const float4*)(L.conv_w + 4 * (size_t)c);
-        float o = L.conv_b[c];
-        o = ffma(cw.x, s0, o);
-        o = ffma(cw.y, s1, o);
-        o = ffma(cw.z, s2, o);
-        o = ffma(cw.w, val, o);
-        ring[ps] = val;
-        out = siluf(o);
-        if (tp) ((float*)(tp + tl.off[5]))[c] = out;                             // XBC_CONV
-    } else {
-        const int h = e - 2 * gs;
-        out = sp_softplusf(fadd(val, L.dt_bias[h]));
-        if (tp) ((float*)(tp + tl.off[6]))[h] = out;                             // DT
-    }
-    bcdt[(size_t)b * n_bcdt + e] = out;
-}
-
-// =============================================================================================
-// S3 stage 2 (for the rows a head needs) + S4 conv step + S5 state update/readout + S6 gate.
-//   grid = (nheads * headdim/PB, batch); one CTA owns PB (head, p) rows of the state: PB = 32 when headdim allows
-//   (16 KB of state per CTA: the kernel is bound by per-CTA latency x occupancy, so more state per CTA is faster), else 16.
-//   The B | C | dt rows are finished once per sequence by k_bcdt and read from its buffer.
-//   Conv state is a 4-slot ring per channel: the sample of step t lives in slot t%4, so the
-//   readers of a step never touch the slot its owner writes.
-// =============================================================================================
 constexpr int SSM_THREADS = 256;
 
 // four consecutive state values: fp32 state, or the fp16 state format of DESIGN.md R24 (stored as binary16, RN-even of the
@@ -328,151 +272,10 @@ __device__ __forceinline__ void state_st4(__half* p, float4 v)
     *(uint2*)p = r;
 }
 
-// 6 CTAs per SM (40 registers): the kernel is latency-bound, 4 CTAs of 58 registers were 11 % slower, 8 of 32 spill
-template <int PB, typename ST>
-__global__ void __launch_bounds__(SSM_THREADS, 6)
-k_ssm(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int32_t* __restrict__ t,
-      const float* __restrict__ s_x, float* __restrict__ conv_ring /* [batch][conv_dim][4] */,
-      const int32_t* __restrict__ pos /* [batch] */, ST* __restrict__ ssm /* [batch][h][p][n] */,
-      float* __restrict__ g /* [batch][d_inner] */, const float* __restrict__ bcdt /* [batch][n_bcdt] from k_bcdt */,
-      uint8_t* __restrict__ taps, uint32_t tap_stride, TapLayout tl)
-{
-    extern __shared__ __align__(16) uint8_t smem[];
-    float* v_sh = (float*)smem;                    // [64]
-    float* Bc = v_sh + 64;                         // [d_state]
-    float* Cc = Bc + dm.d_state;                   // [d_state]
-    float* xs = Cc + dm.d_state;                   // [PB]
-    float* zs = xs + PB;                           // [PB]
-    float* dts = zs + PB;                          // [1] (+pad)
-    constexpr int LANES = SSM_THREADS / PB;        // lanes per state row (16 or 8)
-    constexpr int ROWL = SSM_THREADS / (2 * PB);   // lanes per own in_proj row (8 or 4)
-
-    const int b = blockIdx.y;
-    const int pblocks = dm.headdim / PB;
-    const int h = blockIdx.x / pblocks, pblk = blockIdx.x % pblocks;
-    const int p0 = pblk * PB;
-    const int hpg = dm.nheads / dm.ngroups;
-    const int grp = h / hpg;
-    const int tid = threadIdx.x;
-    const int32_t* accb = acc + (size_t)b * ld_acc;
-    const float sx = s_x[b];
-    const int ps = pos[b] & 3;
-    uint8_t* tp = taps ? taps + (size_t)b * tap_stride : nullptr;
-
-    // this thread's slice of the state is requested first, so that HBM works while the rows below are finished
-    const int p = tid / LANES, l16 = tid % LANES;  // PB rows x LANES lanes
-    ST* Hr = ssm + (((size_t)b * dm.nheads + h) * dm.headdim + p0 + p) * dm.d_state;
-    constexpr int H_PRE = 32 / LANES;             // chunks held in registers (all of d_state = 128); further ones are loaded late
-    float4 hpre[H_PRE];
-#pragma unroll
-    for (int j = 0; j < H_PRE; ++j) {
-        const int n4 = l16 + LANES * j;
-        if (n4 < dm.d_state / 4) hpre[j] = state_ld4(Hr + 4 * n4);
-    }
-
-    if (tid < dm.r) v_sh[tid] = fmul(L.in_a_s[tid], (float)t[(size_t)b * T_STRIDE + tid]);
-    const int gs = dm.ngroups * dm.d_state;
-    {   // B', C' of this head's group and dt of this head: made once per sequence by k_bcdt
-        const float* src = bcdt + (size_t)b * (2 * gs + dm.nheads);
-        for (int i = tid; i < dm.d_state; i += SSM_THREADS) {
-            Bc[i] = src[grp * dm.d_state + i];
-            Cc[i] = src[gs + grp * dm.d_state + i];
-        }
-        if (tid == 0) dts[0] = src[2 * gs + h];
-    }
-    __syncthreads();
-
-    // the 2 * PB own rows (z, x): ROWL lanes share a row's LoRA sum (fp64, any tree: DESIGN.md 5.3)
-    {
-        const int i = tid / ROWL, sub = tid % ROWL;
-        const int kind = i < PB ? 0 : 1, idx = i - kind * PB;              // kind 0 z, 1 x
-        const int row = kind * dm.d_inner + h * dm.headdim + p0 + idx;
-        const int8_t* brow = L.in_B + (size_t)row * dm.r;
-        double lo = 0.0;
-        for (int j = sub; j < dm.r; j += ROWL) lo = dacc(lo, (float)brow[j], v_sh[j]);
-#pragma unroll
-        for (int o = 1; o < ROWL; o <<= 1) lo += __shfl_xor_sync(0xffffffffu, lo, o);
-        if (sub == 0) {
-            const float m1 = fmul(__half2float(L.in_row_scale[row]), (float)accb[row]);
-            const float m2 = fmul(L.in_b_s[row], (float)lo);
-            const float val = fmul(sx, fadd(m1, m2));
-            if (tp) ((float*)(tp + tl.off[4]))[row] = val;                         // ZXBCDT
-            if (kind == 0) {
-                zs[idx] = val;
-            } else {
-                const int c = row - dm.d_inner;                                    // conv channel
-                float* ring = conv_ring + ((size_t)b * dm.conv_dim + c) * 4;
-                const float4 rg = *(const float4*)ring;
-                const float sl[4] = { rg.x, rg.y, rg.z, rg.w };
-                const float s0 = sl[(ps + 1) & 3], s1 = sl[(ps + 2) & 3], s2 = sl[(ps + 3) & 3];
-                const float4 cw = *(const float4*)(L.conv_w + 4 * (size_t)c);
-                float o = L.conv_b[c];
-                o = ffma(cw.x, s0, o);
-                o = ffma(cw.y, s1, o);
-                o = ffma(cw.z, s2, o);
-                o = ffma(cw.w, val, o);
-                const float cv = siluf(o);
-                ring[ps] = val;
-                if (tp) ((float*)(tp + tl.off[5]))[c] = cv;                        // XBC_CONV
-                xs[idx] = cv;
-            }
-        }
-    }
-    __syncthreads();
-
-    const float dtv = dts[0];
-    const float An = -sp_expf(L.A_log[h]);
-    const float dA = sp_expf(fmul(dtv, An));
-    const float xv = xs[p];
-    const float dtx = fmul(dtv, xv);
-    double a = 0.0;
-#pragma unroll
-    for (int j = 0; j < H_PRE; ++j) {
-        const int n4 = l16 + LANES * j;
-        if (n4 >= dm.d_state / 4) break;
-        float4 hv = hpre[j];
-        const float4 bv = *(const float4*)(Bc + 4 * n4);
-        const float4 cv = *(const float4*)(Cc + 4 * n4);
-        hv.x = ffma(dA, hv.x, fmul(dtx, bv.x));
-        hv.y = ffma(dA, hv.y, fmul(dtx, bv.y));
-        hv.z = ffma(dA, hv.z, fmul(dtx, bv.z));
-        hv.w = ffma(dA, hv.w, fmul(dtx, bv.w));
-        state_st4(Hr + 4 * n4, hv);
-        a = dacc(a, cv.x, hv.x);
-        a = dacc(a, cv.y, hv.y);
-        a = dacc(a, cv.z, hv.z);
-        a = dacc(a, cv.w, hv.w);
-    }
-    for (int n4 = l16 + LANES * H_PRE; n4 < dm.d_state / 4; n4 += LANES) {
-        float4 hv = state_ld4(Hr + 4 * n4);
-        const float4 bv = *(const float4*)(Bc + 4 * n4);
-        const float4 cv = *(const float4*)(Cc + 4 * n4);
-        hv.x = ffma(dA, hv.x, fmul(dtx, bv.x));
-        hv.y = ffma(dA, hv.y, fmul(dtx, bv.y));
-        hv.z = ffma(dA, hv.z, fmul(dtx, bv.z));
-        hv.w = ffma(dA, hv.w, fmul(dtx, bv.w));
-        state_st4(Hr + 4 * n4, hv);
-        a = dacc(a, cv.x, hv.x);
-        a = dacc(a, cv.y, hv.y);
-        a = dacc(a, cv.z, hv.z);
-        a = dacc(a, cv.w, hv.w);
-    }
-#pragma unroll
-    for (int o = LANES / 2; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o, LANES);
-    if (l16 == 0) {
-        a = dacc(a, L.D[h], xv);
-        const float y = (float)a;
-        const float gv = fmul(y, siluf(zs[p]));
-        const int ch = h * dm.headdim + p0 + p;
-        g[(size_t)b * dm.d_inner + ch] = gv;
-        if (tp) { ((float*)(tp + tl.off[7]))[ch] = y; ((float*)(tp + tl.off[8]))[ch] = gv; }
-    }
-}
-
 // =============================================================================================
 // S3 stage 2 + S4 conv + SiLU / softplus for EVERY in_proj row, once per sequence (the streaming state kernel below reads
 // finished values only):  fin[b] = [ silu(z) : d_inner ][ silu(conv(x | B | C)) : conv_dim ][ dt : nheads ][ dA : nheads ]
-//   grid = (ceil(d_in_proj / FIN_THREADS), batch).  Same arithmetic, value by value, as k_bcdt + the row prologue of k_ssm.
+//   grid = (ceil(d_in_proj / FIN_THREADS), batch).  Same arithmetic, value by value, as the persistent kernel's in_proj epilogue.
 // =============================================================================================
 constexpr int FIN_THREADS = 128;
 
@@ -531,14 +334,45 @@ __device__ __forceinline__ double s8_to_double(uint8_t byte)
     return __hiloint2double(0x43300000, (int)(byte ^ 0x80u)) - 4503599627370624.0;      // 2^52 + 128
 }
 
-#ifndef DFSSM_FIN_MAGIC
-#define DFSSM_FIN_MAGIC 1
-#endif
 template <int JW> struct BytesT;
 template <> struct BytesT<2> { using T = uint16_t; };
 template <> struct BytesT<4> { using T = uint32_t; };
 template <> struct BytesT<8> { using T = uint2; };
 template <> struct BytesT<16> { using T = uint4; };
+
+// LoRA stage 2 of FIN_THREADS consecutive rows (from `base`) by one CTA, lora_rank = 4 * JW: returns, in every thread, the
+// binary64 sum  sum_j float(B[row][j]) * v_j,  v_j = a_s[j] * float(t_j),  of row = base + threadIdx.x (0 beyond n_rows).
+// Lane `sub` of a group of four holds v_j for its JW values of j and reads its JW bytes of a row with one load; the group
+// walks through its four rows, and the tree of the sum is (p0 + p1) + (p2 + p3).  No shared memory, no barrier.
+template <int JW>
+__device__ __forceinline__ double lora_up4(const int8_t* __restrict__ B, const float* __restrict__ a_s,
+                                           const int32_t* __restrict__ t_row, int base, int n_rows)
+{
+    constexpr int R = 4 * JW;
+    const int q = threadIdx.x >> 2, sub = threadIdx.x & 3;
+    double v[JW];
+#pragma unroll
+    for (int i = 0; i < JW; ++i) {
+        const int j = sub * JW + i;
+        v[i] = (double)fmul(a_s[j], (float)t_row[j]);
+    }
+    double part[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int rk = base + q * 4 + k;
+        double lo = 0.0;
+        if (rk < n_rows) {
+            const typename BytesT<JW>::T w = *(const typename BytesT<JW>::T*)(B + (size_t)rk * R + sub * JW);
+            const uint8_t* wb = (const uint8_t*)&w;
+#pragma unroll
+            for (int i = 0; i < JW; ++i) lo = __fma_rn(s8_to_double(wb[i]), v[i], lo);
+        }
+        lo += __shfl_xor_sync(0xffffffffu, lo, 1);
+        lo += __shfl_xor_sync(0xffffffffu, lo, 2);
+        part[k] = lo;
+    }
+    return sub == 0 ? part[0] : sub == 1 ? part[1] : sub == 2 ? part[2] : part[3];
+}
 
 template <int JW>
 __global__ void __launch_bounds__(FIN_THREADS)
@@ -546,10 +380,8 @@ k_fin4(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int
        const float* __restrict__ s_x, float* __restrict__ conv_ring, const int32_t* __restrict__ pos,
        float* __restrict__ fin, uint8_t* __restrict__ taps, uint32_t tap_stride, TapLayout tl)
 {
-    constexpr int R = 4 * JW;
     const int b = blockIdx.y, tid = threadIdx.x;
     const int gs = dm.ngroups * dm.d_state, d_in_proj = 2 * dm.d_inner + 2 * gs + dm.nheads;
-    const int q = tid >> 2, sub = tid & 3;
     const int base = blockIdx.x * FIN_THREADS;
     const int row = base + tid;                                  // the row this lane finishes
     const bool own = row < d_in_proj;
@@ -569,33 +401,8 @@ k_fin4(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int
         cb = L.conv_b[c];
     }
 
-    double v[JW];
-#pragma unroll
-    for (int i = 0; i < JW; ++i) {
-        const int j = sub * JW + i;
-        v[i] = (double)fmul(L.in_a_s[j], (float)t[(size_t)b * T_STRIDE + j]);
-    }
-    double part[4];
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        const int rk = base + q * 4 + k;
-        double lo = 0.0;
-        if (rk < d_in_proj) {
-            const typename BytesT<JW>::T w = *(const typename BytesT<JW>::T*)(L.in_B + (size_t)rk * R + sub * JW);
-            const uint8_t* wb = (const uint8_t*)&w;
-#pragma unroll
-#if DFSSM_FIN_MAGIC
-            for (int i = 0; i < JW; ++i) lo = __fma_rn(s8_to_double(wb[i]), v[i], lo);
-#else
-            for (int i = 0; i < JW; ++i) lo = __fma_rn((double)(int)(int8_t)wb[i], v[i], lo);
-#endif
-        }
-        lo += __shfl_xor_sync(0xffffffffu, lo, 1);
-        lo += __shfl_xor_sync(0xffffffffu, lo, 2);
-        part[k] = lo;
-    }
+    const double lo = lora_up4<JW>(L.in_B, L.in_a_s, t + (size_t)b * T_STRIDE, base, d_in_proj);
     if (!own) return;
-    const double lo = sub == 0 ? part[0] : sub == 1 ? part[1] : sub == 2 ? part[2] : part[3];
     uint8_t* tp = taps ? taps + (size_t)b * tap_stride : nullptr;
     float* out = fin + (size_t)b * (d_in_proj + dm.nheads);
     const float val = fmul(sx, fadd(fmul(rs, (float)acc_i), fmul(bs, (float)lo)));
@@ -738,6 +545,27 @@ k_epi_out(LayerW L, int d_model, int r, const int32_t* __restrict__ acc, int ld_
     const float o = proj_epilogue_row(acc[(size_t)b * ld_acc + i], L.out_row_scale, L.out_B, L.out_b_s, i, r,
                                       v_sh, s_g[b]);
     const float un = fadd(u[(size_t)b * d_model + i], o);
+    u[(size_t)b * d_model + i] = un;
+    if (taps) ((float*)(taps + (size_t)b * tap_stride + tap_hidden_off))[i] = un;
+}
+
+// k_epi_out for lora_rank = 4 * JW: the LoRA sum by lora_up4 (four lanes per row, vector loads of the LoRA-up bytes)
+template <int JW>
+__global__ void __launch_bounds__(FIN_THREADS)
+k_epi_out4(LayerW L, int d_model, const int32_t* __restrict__ acc, int ld_acc,
+           const int32_t* __restrict__ t, const float* __restrict__ s_g, float* __restrict__ u,
+           uint8_t* __restrict__ taps, uint32_t tap_stride, uint32_t tap_hidden_off)
+{
+    const int b = blockIdx.y, base = blockIdx.x * FIN_THREADS, i = base + threadIdx.x;
+    const bool own = i < d_model;
+    const int il = own ? i : 0;
+    const int acc_i = acc[(size_t)b * ld_acc + il];
+    const float rs = __half2float(L.out_row_scale[il]), bs = L.out_b_s[il], sg = s_g[b];
+    const float u0 = u[(size_t)b * d_model + il];
+    const double lo = lora_up4<JW>(L.out_B, L.out_a_s, t + (size_t)b * T_STRIDE, base, d_model);
+    if (!own) return;
+    const float o = fmul(sg, fadd(fmul(rs, (float)acc_i), fmul(bs, (float)lo)));
+    const float un = fadd(u0, o);
     u[(size_t)b * d_model + i] = un;
     if (taps) ((float*)(taps + (size_t)b * tap_stride + tap_hidden_off))[i] = un;
 }
