@@ -244,10 +244,13 @@ int proj_grid(int rows_total)
     return g < cap ? g : cap;
 }
 
-// batch >= 16: the projections run on the tensor cores (tcgen05 kind::i8 on +-1 tiles unpacked in shared memory)
+// the projections run on the tensor cores (tcgen05 kind::i8 on +-1 tiles unpacked in shared memory) from this batch size on
 bool use_mma(const dfssm_ctx* c, int batch, int K)
 {
-    return batch >= 16 && K % mma::KMULT == 0 && !(c->cfg.flags & DFSSM_FLAG_NO_MMA);
+    // measured (ms/step, dp4a rows vs tensor cores; cfg 3: batch 5 1.99 / 1.68, 8 2.50 / 1.82, 15 3.32 / 2.21; cfg 4: batch 5 3.49 / 2.73,
+    // 8 4.34 / 3.10; cfg 1 (d_model 768): batch 8 0.64 / 0.68): from batch 5 on for the wide models, from 16 on for narrow ones
+    const int mma_min = c->dm.d_model >= 1024 ? 5 : 16;
+    return batch >= mma_min && K % mma::KMULT == 0 && !(c->cfg.flags & DFSSM_FLAG_NO_MMA);
 }
 
 // one projection on the tensor cores; K is split over CTAs until the grid fills the 148 SMs (partial sums are added
