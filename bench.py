@@ -60,11 +60,11 @@ def measured_peak():
 # ---------------------------------------------------------------------------------------------
 # algorithmic bytes: what the method itself must move
 # ---------------------------------------------------------------------------------------------
-def algorithmic_bytes(s, batch: int) -> dict:
+def algorithmic_bytes(s, batch: int, state_esize: int = 4) -> dict:
     dm, di, dip, r, cd, nh = s.d_model, s.d_inner, s.d_in_proj, s.lora_rank, s.conv_dim, s.nheads
     scaffold = s.n_layers * (dip * dm + dm * di) // 8
     lora = s.n_layers * r * (dm + dip + di + dm)
-    state = s.n_layers * batch * 2 * (nh * s.headdim * s.d_state * 4)
+    state = s.n_layers * batch * 2 * (nh * s.headdim * s.d_state * state_esize)      # 2 bytes with --state-fp16 (R24)
     lm_head = s.vocab * dm
     per_layer_small = (4 * dm + 2 * dip + 4 * r + 4 * dip + 16 * cd + 4 * cd + 12 * nh + 4 * di
                        + 2 * dm + 4 * r + 4 * dm)
@@ -75,7 +75,7 @@ def algorithmic_bytes(s, batch: int) -> dict:
                 bj_formula=scaffold + lora + state, total=scaffold + lora + state + lm_head + other)
 
 
-def kernel_class_bytes(s, batch: int) -> dict:
+def kernel_class_bytes(s, batch: int, state_esize: int = 4) -> dict:
     """Algorithmic bytes ONE launch of each kernel class moves (weights once, state r+w once)."""
     dm, di, dip, r, cd, nh = s.d_model, s.d_inner, s.d_in_proj, s.lora_rank, s.conv_dim, s.nheads
     B = batch
@@ -83,13 +83,13 @@ def kernel_class_bytes(s, batch: int) -> dict:
         "embed": B * (dm + 4 + 4 * dm),
         "normquant": B * (4 * di + 2 * di) + 4 * di,
         "proj_in": dip * dm // 8 + r * dm + B * (2 * dm + 4 * dip + 4 * r),
-        "ssm": B * (2 * nh * s.headdim * s.d_state * 4 + 2 * cd * 4 * 4 + 4 * dip + 4 * di)
+        "ssm": B * (2 * nh * s.headdim * s.d_state * state_esize + 2 * cd * 4 * 4 + 4 * dip + 4 * di)
         + 2 * dip + dip * r + 4 * dip + 20 * cd + 12 * nh,
         "proj_out": dm * di // 8 + r * di + B * (2 * di + 4 * dm + 4 * r),
         "epi_out": 2 * dm + dm * r + 4 * dm + B * (4 * dm + 8 * dm),
         "lmhead": s.vocab * dm + 4 * s.vocab + B * (dm + 4 * s.vocab),
         "argmax": B * 4 * s.vocab,
-        "mega": algorithmic_bytes(s, B)["total"],      # the whole step is one kernel
+        "mega": algorithmic_bytes(s, B, state_esize)["total"],      # the whole step is one kernel
     }
 
 
@@ -149,13 +149,15 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------
 # the oracle, as it stands, on the host cores (cpu_baseline leg and --impl reference)
 # ---------------------------------------------------------------------------------------------
-def time_oracle(s, blob, cfg_idx: int, batch: int, budget_s: float, max_steps: int, n_prompt: int = 2, threads: int = 0):
+def time_oracle(s, blob, cfg_idx: int, batch: int, budget_s: float, max_steps: int, n_prompt: int = 2, threads: int = 0,
+                state_fp16: bool = False):
     """Feed `n_prompt` prompt tokens (untimed), then time greedy decode steps until the budget or
     max_steps is reached.  Returns (tokens/s, steps, seconds, threads)."""
     import oracle
     oracle.build()
     oracle.set_threads(threads if threads > 0 else n_cores())
     m = oracle.OracleModel(blob, batch)
+    m.set_state_fp16(state_fp16)
     prompt = ds.token_batch(s.vocab, n_prompt, seed=cfg_idx, batch=batch)
     for t in range(n_prompt):
         m.step(prompt[t])
@@ -181,6 +183,7 @@ def run_reference(args, s, blob):
     oracle.build()
     oracle.set_threads(n_cores())
     m = oracle.OracleModel(blob, args.batch)
+    m.set_state_fp16(args.state_fp16)
     toks = ds.token_batch(s.vocab, max(1, min(args.warmup, 8)), seed=args.config, batch=args.batch)
     for t in range(toks.shape[0]):
         m.step(toks[t])
@@ -258,7 +261,9 @@ def run_ours(args, s, blob):
     import paper_2606_10932_b200 as pk
 
     B = args.batch
-    m = pk.Model(pk.Config.from_shape(s, max_batch=B), blob, device=f"cuda:{local}")
+    from paper_2606_10932_b200 import binding
+    esz = 2 if args.state_fp16 else 4
+    m = pk.Model(pk.Config.from_shape(s, max_batch=B, flags=binding.FLAG_STATE_FP16 if args.state_fp16 else 0), blob, device=f"cuda:{local}")
     # every rank is an independent replica with its own token streams ("replicas only")
     prompt = ds.token_batch(s.vocab, max(args.warmup, 1), seed=replica_seed(rank, args.config), batch=B)
     prompt_dev = [torch.from_numpy(prompt[t]).cuda() for t in range(prompt.shape[0])]
@@ -337,12 +342,12 @@ def run_ours(args, s, blob):
             dist.destroy_process_group()
         return
 
-    ab = algorithmic_bytes(s, B)
+    ab = algorithmic_bytes(s, B, esz)
     value = whole_job_rate(world, B, args.steps, ms * 1e-3)
     e2e_val = whole_job_rate(world, B, e2e_steps, e2e_s)
     peak, peak_src = measured_peak()
     step_gbs = ab["total"] * (args.steps / (ms * 1e-3)) / 1e9
-    kb = kernel_class_bytes(s, B)
+    kb = kernel_class_bytes(s, B, esz)
     L = s.n_layers
     counts = {"embed": 1, "normquant": 2 * L + 1, "proj_in": L, "ssm": L, "proj_out": L, "epi_out": L,
               "lmhead": 1, "argmax": 1, "mega": 1}
@@ -364,8 +369,8 @@ def run_ours(args, s, blob):
 
     cpu_baseline = None
     if world == 1 and not args.no_cpu_baseline:
-        v, n, dt, thr = time_oracle(s, blob, args.config, B, budget_s=15.0, max_steps=64)
-        v1, n1, dt1, _ = time_oracle(s, blob, args.config, B, budget_s=6.0, max_steps=8, threads=1)
+        v, n, dt, thr = time_oracle(s, blob, args.config, B, budget_s=15.0, max_steps=64, state_fp16=args.state_fp16)
+        v1, n1, dt1, _ = time_oracle(s, blob, args.config, B, budget_s=6.0, max_steps=8, threads=1, state_fp16=args.state_fp16)
         cpu_baseline = {"value": v, "unit": UNIT, "cores": thr, "kind": "oracle",
                         "sample": f"{n} greedy decode steps of the same workload after 2 prompt steps ({dt:.1f} s)",
                         "single_thread": {"value": v1, "unit": UNIT, "cores": 1, "sample": f"{n1} steps ({dt1:.1f} s)"}}
@@ -377,7 +382,7 @@ def run_ours(args, s, blob):
         "repeats": {"n": len(rep_ms), "steps_each": args.steps, "best_ms_per_step": min(rep_ms) / args.steps,
                     "median_ms_per_step": statistics.median(rep_ms) / args.steps, "extra_warmup_steps": extra_warmup},
         "speedup_vs_cpu_baseline": (value / cpu_baseline["value"]) if cpu_baseline else None,
-        "dtype": "int8 x {-1,+1} -> int32; fp32 state", "data": "synthetic",
+        "dtype": "int8 x {-1,+1} -> int32; " + ("fp16 state (lossy option, DESIGN.md R24)" if args.state_fp16 else "fp32 state"), "data": "synthetic",
         "config": {"workload": workload_name(args.config, B), "seed": args.config, "batch_per_gpu": B,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": f"inputs larger than L2: {ab['total'] / 1e6:.0f} MB streamed per step vs ~126 MB L2"},
@@ -441,6 +446,8 @@ def main():
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--batch", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--state-fp16", action="store_true",
+                    help="SSM state stored as binary16 (DFSSM_FLAG_STATE_FP16, SURVEY 8(f) NEXT-2; lossy; kernel chain only)")
     ap.add_argument("--reps", type=int, default=5, help="repetitions of the K timed steps (the first is the reported value)")
     args = ap.parse_args()
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -327,13 +327,6 @@ k_fin(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
 // registers and reading its JW bytes of the row with one load (a warp reads 8 x 32 contiguous bytes per pass); a CTA of
 // FIN_THREADS threads finishes FIN_THREADS rows in 4 passes, then lane `sub` of a group finishes the row of pass `sub`, so that
 // the row epilogues (conv, SiLU, softplus) run on every lane and row = base + tid is coalesced.  fp64 sum, tree (p0+p1)+(p2+p3).
-// exact int8 -> binary64 without the conversion unit (I2F.F64 runs at a quarter of the fp64 rate): the byte with its sign bit
-// flipped is b + 128 in [0, 255]; as the low word of 2^52 it makes the double 2^52 + 128 + b, and the subtraction is exact.
-__device__ __forceinline__ double s8_to_double(uint8_t byte)
-{
-    return __hiloint2double(0x43300000, (int)(byte ^ 0x80u)) - 4503599627370624.0;      // 2^52 + 128
-}
-
 template <int JW> struct BytesT;
 template <> struct BytesT<2> { using T = uint16_t; };
 template <> struct BytesT<4> { using T = uint32_t; };
@@ -365,7 +358,7 @@ __device__ __forceinline__ double lora_up4(const int8_t* __restrict__ B, const f
             const typename BytesT<JW>::T w = *(const typename BytesT<JW>::T*)(B + (size_t)rk * R + sub * JW);
             const uint8_t* wb = (const uint8_t*)&w;
 #pragma unroll
-            for (int i = 0; i < JW; ++i) lo = __fma_rn(s8_to_double(wb[i]), v[i], lo);
+            for (int i = 0; i < JW; ++i) lo = __fma_rn((double)(int)(int8_t)wb[i], v[i], lo);
         }
         lo += __shfl_xor_sync(0xffffffffu, lo, 1);
         lo += __shfl_xor_sync(0xffffffffu, lo, 2);
