@@ -650,7 +650,18 @@ int prefill_chunk(dfssm_ctx* c, const int32_t* tokens_dev, int T, int seq)
         k_normquant<<<T, NQ_THREADS, 0, st>>>(u, d.d_model, L.norm_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum, nullptr, 0, 0, 0,
                                               use_mma(c, T, d.d_model) ? acc : nullptr, ld_acc, t);
         proj(L.in_sign, L.in_A, d.d_in_proj, d.d_model);
-        prefill::k_pf_epi<<<dim3((d.d_in_proj + prefill::EPI_T - 1) / prefill::EPI_T, T), prefill::EPI_T, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
+        {
+            const dim3 g4((d.d_in_proj + FIN_THREADS - 1) / FIN_THREADS, T);
+            switch (d.r) {
+                case 8: prefill::k_pf_epi4<2><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc); break;
+                case 16: prefill::k_pf_epi4<4><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc); break;
+                case 32: prefill::k_pf_epi4<8><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc); break;
+                case 64: prefill::k_pf_epi4<16><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc); break;
+                default:
+                    prefill::k_pf_epi<<<dim3((d.d_in_proj + prefill::EPI_T - 1) / prefill::EPI_T, T), prefill::EPI_T, 0, st>>>(L, d, acc, ld_acc, t, sx, zx,
+                                                                                                                        ld_acc);
+            }
+        }
         prefill::k_pf_conv<<<dim3((d.conv_dim + d.nheads + prefill::CONV_T - 1) / prefill::CONV_T, T), prefill::CONV_T, 0, st>>>(L, d, zx, ld_acc, T, ring, pos, xbc,
                                                                                                                                dtv);
         prefill::k_pf_ring<<<(d.conv_dim + 255) / 256, 256, 0, st>>>(d, zx, ld_acc, T, ring, pos);

@@ -28,6 +28,21 @@ k_pf_epi(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const i
     zx[(size_t)p * ldz + i] = proj_epilogue_row(acc[(size_t)p * ld_acc + i], L.in_row_scale, L.in_B, L.in_b_s, i, dm.r, v_sh, s_x[p]);
 }
 
+// the same for lora_rank = 4 * JW: the LoRA sum by lora_up4 (four lanes per row, vector loads of the LoRA-up bytes; k_fin4's scheme)
+template <int JW>
+__global__ void __launch_bounds__(FIN_THREADS)
+k_pf_epi4(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int32_t* __restrict__ t, const float* __restrict__ s_x,
+          float* __restrict__ zx, int ldz)
+{
+    const int p = blockIdx.y, base = blockIdx.x * FIN_THREADS, i = base + threadIdx.x;
+    const bool own = i < dm.d_in_proj;
+    const int il = own ? i : 0;
+    const int acc_i = acc[(size_t)p * ld_acc + il];
+    const float rs = __half2float(L.in_row_scale[il]), bs = L.in_b_s[il], sx = s_x[p];
+    const double lo = lora_up4<JW>(L.in_B, L.in_a_s, t + (size_t)p * T_STRIDE, base, dm.d_in_proj);
+    if (own) zx[(size_t)p * ldz + i] = fmul(sx, fadd(fmul(rs, (float)acc_i), fmul(bs, (float)lo)));
+}
+
 // S4 for every (position, conv channel) + softplus of dt: the raw samples of positions < 0 come from the sequence's conv ring
 // (sample of step tau lives in slot tau mod 4; `ps` = slot of position 0)
 constexpr int CONV_T = 256;
