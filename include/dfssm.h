@@ -212,6 +212,34 @@ DFSSM_API const char* dfssm_last_error(const dfssm_ctx* ctx);
 /* Release the context (never frees the arena).  Safe on null. */
 DFSSM_API void dfssm_destroy(dfssm_ctx* ctx);
 
+/* ---- S8 without any allocation, context or arena (paper_2606_10932_b200/csrc/dfssm_noalloc.cu) -------------------------------
+ * For callers that cannot call cudaMalloc and cannot hand over an arena (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid allocation).  Computes, for `batch` sequences, what the end of dfssm_step computes (S8: PAPER.md P:96,
+ * DESIGN.md R16, R19): final RMSNorm + absmax int8 quantiser of the hidden state, tied int8 LM head
+ * logit_v = float(sum_k E_vk q_k) * (s_h * e_s[v]), greedy token = argmax with the lowest index on ties.  Bit-identical to
+ * dfssm_step's logits and tokens for the same hidden state and weights.
+ *   hidden_dev      device, float [batch][d_model]           (e.g. dfssm_hidden)            read
+ *   normf_w_dev     device, float [d_model]                  final norm weight              read
+ *   emb_dev         device, int8  [vocab][d_model], 16-byte aligned; emb_scale_dev device float [vocab]   read
+ *   next_dev        device, int32 [batch]                    greedy tokens                  written
+ *   logits_dev      device, float [batch][vocab] or NULL     copy of the logits             written if given
+ *   cuda_stream     cudaStream_t (0 = the default stream); the three kernels are enqueued on it, nothing is synchronised
+ * All buffers are the caller's.  The intermediates (codes, scales, logits) live in a static device array of
+ * DFSSM_NOALLOC_SCRATCH_BYTES that every GPU holds from the moment libdfssm.so is loaded until the process exits; a call needs
+ * dfssm_head_noalloc_scratch_need(batch, d_model, vocab) = up256(batch*d_model) + up256(4*batch) + 4*batch*vocab bytes of it
+ * (cfg 2: batch <= 20) and is rejected with DFSSM_E_SIZE beyond that.  Calls no cudaMalloc / cudaFree / allocating routine.
+ * The first call on a device takes the array's address (cudaGetSymbolAddress, that device current); later calls only launch.
+ * EVERY call on a device shares the array and finds the previous call's contents in it (nothing needs clearing: every value
+ * read is written earlier in the same call).  Calls that overlap on the GPU (different streams without an ordering between
+ * them) RACE on it: keep them on one stream or order them with events.
+ * Errors: DFSSM_E_ARG (null pointer, batch / vocab < 1, d_model not a positive multiple of 16 or > 6144, misaligned emb_dev),
+ * DFSSM_E_SIZE (scratch), DFSSM_E_ARCH (not sm_100), DFSSM_E_CUDA; text from dfssm_head_noalloc_error (per host thread). */
+#define DFSSM_NOALLOC_SCRATCH_BYTES (4u << 20)
+DFSSM_API size_t dfssm_head_noalloc_scratch_need(int batch, int d_model, int vocab);
+DFSSM_API int dfssm_head_noalloc(const float* hidden_dev, const float* normf_w_dev, const int8_t* emb_dev, const float* emb_scale_dev,
+                                 int batch, int d_model, int vocab, float eps, int32_t* next_dev, float* logits_dev, void* cuda_stream);
+DFSSM_API const char* dfssm_head_noalloc_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -36,6 +36,7 @@ EXPORTED_SYMBOLS = (
     "dfssm_step_host", "dfssm_logits", "dfssm_next_tokens", "dfssm_hidden", "dfssm_debug_tensor",
     "dfssm_get_state", "dfssm_set_state", "dfssm_debug_profile", "dfssm_sync", "dfssm_launches_per_step",
     "dfssm_time_kernels", "dfssm_last_error", "dfssm_destroy",
+    "dfssm_head_noalloc_scratch_need", "dfssm_head_noalloc", "dfssm_head_noalloc_error",
 )
 
 _ERR = {0: "OK", -1: "E_ARG", -2: "E_SIZE", -3: "E_STATE", -4: "E_CUDA", -5: "E_ARCH", -6: "E_TOKEN"}
@@ -134,6 +135,9 @@ def lib() -> C.CDLL:
         "dfssm_time_kernels": (C.c_int, [vp, vp, C.c_int, C.c_int, f32p]),
         "dfssm_last_error": (C.c_char_p, [vp]),
         "dfssm_destroy": (None, [vp]),
+        "dfssm_head_noalloc_scratch_need": (C.c_size_t, [C.c_int, C.c_int, C.c_int]),
+        "dfssm_head_noalloc": (C.c_int, [vp, vp, vp, vp, C.c_int, C.c_int, C.c_int, C.c_float, vp, vp, vp]),
+        "dfssm_head_noalloc_error": (C.c_char_p, []),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -145,6 +149,38 @@ def lib() -> C.CDLL:
 def dfssm_arena_bytes(cfg: Config) -> int:
     c = cfg.c()
     return int(lib().dfssm_arena_bytes(C.byref(c)))
+
+
+NOALLOC_SCRATCH_BYTES = 4 << 20
+
+
+def head_noalloc_scratch_need(batch: int, d_model: int, vocab: int) -> int:
+    return int(lib().dfssm_head_noalloc_scratch_need(int(batch), int(d_model), int(vocab)))
+
+
+def head_noalloc(hidden, normf_w, emb, emb_scale, next_out, logits_out=None, eps: float = 1e-5, stream=None):
+    """dfssm_head_noalloc: S8 (final norm + quantiser, tied int8 LM head, greedy argmax) with the intermediates in the
+    library's static device array: no allocation, no context, no arena.  All arguments are torch CUDA tensors of the caller
+    (hidden float32 [batch][d_model], normf_w float32 [d_model], emb int8 [vocab][d_model], emb_scale float32 [vocab],
+    next_out int32 [batch], logits_out float32 [batch][vocab] or None); enqueued on `stream` (default: torch's current one)."""
+    import torch
+    batch, d_model = hidden.shape
+    vocab = emb.shape[0]
+    for t_, dt in ((hidden, torch.float32), (normf_w, torch.float32), (emb, torch.int8), (emb_scale, torch.float32),
+                   (next_out, torch.int32)) + (((logits_out, torch.float32),) if logits_out is not None else ()):
+        if not (t_.is_cuda and t_.is_contiguous() and t_.dtype == dt):
+            raise DfssmError(-1, "head_noalloc: contiguous CUDA tensors of the documented dtypes are required")
+    if emb.shape[1] != d_model or normf_w.numel() != d_model or emb_scale.numel() != vocab or next_out.numel() < batch or \
+            (logits_out is not None and logits_out.numel() < batch * vocab):
+        raise DfssmError(-1, "head_noalloc: shapes do not match")
+    st = stream if stream is not None else torch.cuda.current_stream(hidden.device)
+    L = lib()
+    with torch.cuda.device(hidden.device):
+        rc = L.dfssm_head_noalloc(hidden.data_ptr(), normf_w.data_ptr(), emb.data_ptr(), emb_scale.data_ptr(), int(batch), int(d_model),
+                                  int(vocab), float(eps), next_out.data_ptr(), logits_out.data_ptr() if logits_out is not None else None,
+                                  st.cuda_stream)
+    if rc != 0:
+        raise DfssmError(rc, L.dfssm_head_noalloc_error().decode())
 
 
 def _f32p(a: Optional[np.ndarray]):
