@@ -10,13 +10,20 @@ Header:
     off 12  i32 x 9  n_layers, d_model, d_inner, headdim, d_state, ngroups, d_conv,
                      vocab, lora_rank
     off 48  f32      norm_eps
-    off 52  u32      0
+    off 52  u32      weight format: bit 0 = 17-level scaffold, bit 1 = int4 LoRA (0 = the paper's deployed format)
     off 56  u64      total blob bytes
     off 64..255      0
 
 Sign matrices: row-major [rows][K/32] uint32; bit b (LSB = 0) of word w of row i is
 element k = 32*w + b; bit 1 -> +1, bit 0 -> -1 (every packed bit
 expands to exactly +-1).
+
+Format variants (R25):
+  17-level scaffold: instead of `sign`, `lvl` = [rows][K/32][5] uint32.  The weight of element k = 32*w + b is level/8 with
+    level = m - 8 in [-8, 8] (Eq. 1 with K_w = 16: {-1, -14/16, ..., 1}); bit b of word [w][p] is bit p of m.
+    `row_scale` multiplies the INTEGER accumulator sum(level * q), i.e. it holds the paper's row scale / 8.
+  int4 LoRA: `A4` = [r][K/2], `B4` = [rows][r/2] uint8; element 2i is the low nibble of byte i, element 2i+1 the high
+    nibble, each a two's-complement 4-bit integer in [-8, 7].
 """
 from __future__ import annotations
 
@@ -25,7 +32,7 @@ from typing import Dict, List, Tuple
 
 import numpy as np
 
-from .shapes import Shape
+from .shapes import Shape, FMT_SCAFFOLD17, FMT_LORA_INT4
 
 BLOB_MAGIC = b"DFSSMW1\0"
 BLOB_VERSION = 1
@@ -37,14 +44,25 @@ Spec = Tuple[str, np.dtype, Tuple[int, ...]]
 
 def layer_tensor_specs(s: Shape) -> List[Spec]:
     r = s.lora_rank
-    u32, f16, f32, i8 = np.dtype("<u4"), np.dtype("<f2"), np.dtype("<f4"), np.dtype("i1")
+    u32, f16, f32, i8, u8 = np.dtype("<u4"), np.dtype("<f2"), np.dtype("<f4"), np.dtype("i1"), np.dtype("u1")
+    s17, i4 = bool(s.fmt & FMT_SCAFFOLD17), bool(s.fmt & FMT_LORA_INT4)
+
+    def scaffold(side, rows, K):
+        return (f"{side}.lvl", u32, (rows, K // 32, 5)) if s17 else (f"{side}.sign", u32, (rows, K // 32))
+
+    def lora_a(side, K):
+        return (f"{side}.A4", u8, (r, K // 2)) if i4 else (f"{side}.A", i8, (r, K))
+
+    def lora_b(side, rows):
+        return (f"{side}.B4", u8, (rows, r // 2)) if i4 else (f"{side}.B", i8, (rows, r))
+
     return [
         ("norm_w", f32, (s.d_model,)),
-        ("in.sign", u32, (s.d_in_proj, s.d_model // 32)),
+        scaffold("in", s.d_in_proj, s.d_model),
         ("in.row_scale", f16, (s.d_in_proj,)),
-        ("in.A", i8, (r, s.d_model)),
+        lora_a("in", s.d_model),
         ("in.a_s", f32, (r,)),
-        ("in.B", i8, (s.d_in_proj, r)),
+        lora_b("in", s.d_in_proj),
         ("in.b_s", f32, (s.d_in_proj,)),
         ("conv_w", f32, (s.conv_dim, 4)),
         ("conv_b", f32, (s.conv_dim,)),
@@ -52,13 +70,48 @@ def layer_tensor_specs(s: Shape) -> List[Spec]:
         ("dt_bias", f32, (s.nheads,)),
         ("D", f32, (s.nheads,)),
         ("gnorm_w", f32, (s.d_inner,)),
-        ("out.sign", u32, (s.d_model, s.d_inner // 32)),
+        scaffold("out", s.d_model, s.d_inner),
         ("out.row_scale", f16, (s.d_model,)),
-        ("out.A", i8, (r, s.d_inner)),
+        lora_a("out", s.d_inner),
         ("out.a_s", f32, (r,)),
-        ("out.B", i8, (s.d_model, r)),
+        lora_b("out", s.d_model),
         ("out.b_s", f32, (s.d_model,)),
     ]
+
+
+# ---- packing of the format variants (byte layout only) ----
+def pack_levels(levels: np.ndarray) -> np.ndarray:
+    """int levels in [-8, 8], [rows][K] -> uint32 [rows][K/32][5] bit planes of m = level + 8"""
+    lv = np.asarray(levels).astype(np.int64)
+    assert lv.ndim == 2 and lv.shape[1] % 32 == 0 and lv.min() >= -8 and lv.max() <= 8
+    m = (lv + 8).reshape(lv.shape[0], -1, 32).astype(np.uint64)
+    w = (np.uint64(1) << np.arange(32, dtype=np.uint64))
+    planes = [(((m >> np.uint64(p)) & np.uint64(1)) * w).sum(-1) for p in range(5)]
+    return np.stack(planes, -1).astype("<u4")
+
+
+def unpack_levels(lvl: np.ndarray) -> np.ndarray:
+    """uint32 [rows][K/32][5] -> int8 levels [rows][K]"""
+    lvl = np.asarray(lvl, dtype=np.uint32)
+    bits = (lvl[:, :, None, :] >> np.arange(32, dtype=np.uint32)[None, None, :, None]) & 1       # [rows][W][32][5]
+    m = (bits.astype(np.int64) << np.arange(5)[None, None, None, :]).sum(-1)
+    return (m - 8).reshape(lvl.shape[0], -1).astype(np.int8)
+
+
+def pack_int4(a: np.ndarray) -> np.ndarray:
+    """int values in [-8, 7], [n][m] (m even) -> uint8 [n][m/2]: element 2i = low nibble of byte i"""
+    a = np.asarray(a).astype(np.int64)
+    assert a.ndim == 2 and a.shape[1] % 2 == 0 and a.min() >= -8 and a.max() <= 7
+    n = (a & 0xF).astype(np.uint8)
+    return (n[:, 0::2] | (n[:, 1::2] << 4)).astype(np.uint8)
+
+
+def unpack_int4(b: np.ndarray) -> np.ndarray:
+    b = np.asarray(b, dtype=np.uint8)
+    out = np.empty((b.shape[0], 2 * b.shape[1]), np.int16)
+    out[:, 0::2] = b & 0xF
+    out[:, 1::2] = b >> 4
+    return ((out ^ 8) - 8).astype(np.int8)
 
 
 def global_tensor_specs(s: Shape) -> List[Spec]:
@@ -98,7 +151,7 @@ def _header(s: Shape, total: int) -> bytes:
     h = bytearray(HEADER_BYTES)
     h[0:8] = BLOB_MAGIC
     struct.pack_into("<I9ifIQ", h, 8, BLOB_VERSION, s.n_layers, s.d_model, s.d_inner, s.headdim,
-                     s.d_state, s.ngroups, s.d_conv, s.vocab, s.lora_rank, float(s.norm_eps), 0, total)
+                     s.d_state, s.ngroups, s.d_conv, s.vocab, s.lora_rank, float(s.norm_eps), int(s.fmt), total)
     return bytes(h)
 
 
@@ -121,10 +174,10 @@ def write_blob(s: Shape, tensors: Dict[str, np.ndarray]) -> np.ndarray:
 def read_header(blob: np.ndarray) -> Shape:
     raw = bytes(blob[:HEADER_BYTES])
     assert raw[0:8] == BLOB_MAGIC, "bad magic"
-    ver, nl, dm, di, hd, ds, ng, dc, vo, r, eps, _z, total = struct.unpack_from("<I9ifIQ", raw, 8)
+    ver, nl, dm, di, hd, ds, ng, dc, vo, r, eps, fmt, total = struct.unpack_from("<I9ifIQ", raw, 8)
     assert ver == BLOB_VERSION
     assert total == blob.nbytes, (total, blob.nbytes)
-    return Shape(nl, dm, di, hd, ds, ng, dc, vo, r, eps)
+    return Shape(nl, dm, di, hd, ds, ng, dc, vo, r, eps, fmt)
 
 
 def blob_views(blob: np.ndarray) -> Tuple[Shape, Dict[str, np.ndarray]]:

@@ -10,6 +10,10 @@ from __future__ import annotations
 from dataclasses import dataclass, replace
 
 
+FMT_SCAFFOLD17 = 1            # 17-level scaffold {-1, -14/16, ..., 1} (Eq. 1 / Eq. 3) as five bit planes
+FMT_LORA_INT4 = 2             # int4 LoRA matrices (Table 4), two values per byte
+
+
 @dataclass(frozen=True)
 class Shape:
     n_layers: int
@@ -22,6 +26,7 @@ class Shape:
     vocab: int
     lora_rank: int
     norm_eps: float = 1e-5
+    fmt: int = 0              # weight format variants: FMT_SCAFFOLD17 | FMT_LORA_INT4; 0 = 1-bit scaffold, int8 LoRA
 
     @property
     def nheads(self) -> int:
@@ -43,16 +48,19 @@ class Shape:
         assert self.d_inner % self.headdim == 0
         assert self.nheads % self.ngroups == 0
         assert self.lora_rank >= 1 and self.vocab >= 1 and self.n_layers >= 0
+        assert 0 <= self.fmt <= 3
+        if self.fmt & FMT_LORA_INT4:
+            assert self.lora_rank % 2 == 0, "int4 LoRA packs two values per byte"
 
     # ---- byte counts used by tests (Table 1 pins) and by bench.py's roofline ----
     def scaffold_bytes(self) -> int:
         per_layer = (self.d_in_proj * self.d_model + self.d_model * self.d_inner) // 8
-        return self.n_layers * per_layer
+        return self.n_layers * per_layer * (5 if self.fmt & FMT_SCAFFOLD17 else 1)
 
     def lora_bytes(self) -> int:
         r = self.lora_rank
         per_layer = r * (self.d_model + self.d_in_proj + self.d_inner + self.d_model)
-        return self.n_layers * per_layer
+        return self.n_layers * per_layer // (2 if self.fmt & FMT_LORA_INT4 else 1)
 
     def embedding_bytes(self) -> int:
         return self.vocab * self.d_model

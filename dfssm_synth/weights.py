@@ -21,8 +21,8 @@ from __future__ import annotations
 
 import numpy as np
 
-from .shapes import Shape
-from .blob import layer_tensor_specs, global_tensor_specs, write_blob
+from .shapes import Shape, FMT_SCAFFOLD17, FMT_LORA_INT4
+from .blob import layer_tensor_specs, global_tensor_specs, write_blob, pack_levels, pack_int4
 
 
 def _rng(seed: int, layer: int, tid: int) -> np.random.Generator:
@@ -33,16 +33,20 @@ def _int8_uniform(g: np.random.Generator, shape) -> np.ndarray:
     return g.integers(-127, 128, size=shape, dtype=np.int8)
 
 
-def _gen(name: str, dt: np.dtype, shp, g: np.random.Generator, varied: bool) -> np.ndarray:
+def _gen(name: str, dt: np.dtype, shp, g: np.random.Generator, varied: bool, fmt: int = 0) -> np.ndarray:
     base = name.split(".")[-1]
     if base == "sign":
         return g.integers(0, 1 << 32, size=shp, dtype=np.uint32).astype("<u4")
-    if base == "row_scale":
-        return (np.abs(g.standard_normal(shp)) * 0.02).astype(np.float16)
+    if base == "lvl":           # 17 levels, uniform (the frozen scaffold of Eq. 3; no trained weights exist here)
+        return pack_levels(g.integers(-8, 9, size=(shp[0], shp[1] * 32)))
+    if base == "row_scale":     # with 17 levels the scale multiplies sum(level * q), |level| <= 8: keep the row outputs O(same)
+        return (np.abs(g.standard_normal(shp)) * (0.02 / 5.0 if fmt & FMT_SCAFFOLD17 else 0.02)).astype(np.float16)
     if base in ("A", "B", "emb"):
         return _int8_uniform(g, shp)
+    if base in ("A4", "B4"):
+        return pack_int4(g.integers(-8, 8, size=(shp[0], shp[1] * 2)))
     if base in ("a_s", "b_s"):
-        v = np.full(shp, 1e-3, dtype=np.float64)
+        v = np.full(shp, 16e-3 if fmt & FMT_LORA_INT4 else 1e-3, dtype=np.float64)
         if varied:
             v = v * g.uniform(0.5, 1.5, size=shp)
         return v.astype(np.float32)
@@ -79,7 +83,7 @@ def make_tensors(s: Shape, seed: int, variant: str = "baseline") -> dict:
     out = {}
     for l in range(s.n_layers):
         for tid, (name, dt, shp) in enumerate(layer_tensor_specs(s)):
-            out[f"L{l}.{name}"] = _gen(name, dt, shp, _rng(seed, l, tid), varied)
+            out[f"L{l}.{name}"] = _gen(name, dt, shp, _rng(seed, l, tid), varied, s.fmt)
     for tid, (name, dt, shp) in enumerate(global_tensor_specs(s)):
         out[f"G.{name}"] = _gen(name, dt, shp, _rng(seed, -1, tid), varied)
     return out

@@ -55,6 +55,8 @@ def lib() -> C.CDLL:
         "dfo_norm_quant": (None, [f32p, f32p, C.c_int, C.c_float, i8p, f32p, f32p, f32p]),
         "dfo_sign_matvec": (None, [u32p, C.c_int, C.c_int, i8p, i32p]),
         "dfo_lora_down": (None, [i8p, C.c_int, C.c_int, i8p, i32p]),
+        "dfo_level_matvec": (None, [u32p, C.c_int, C.c_int, i8p, i32p]),
+        "dfo_unpack_int4": (None, [C.POINTER(C.c_uint8), C.c_int, C.c_int, i8p]),
         "dfo_proj_epilogue": (None, [i32p, i32p, u16p, f32p, i8p, f32p, C.c_int, C.c_int, C.c_float, f32p]),
         "dfo_conv_step": (None, [f32p, f32p, f32p, f32p, C.c_int, f32p]),
         "dfo_ssm_step": (None, [f32p, f32p, f32p, f32p, f32p, f32p, f32p, C.c_int, C.c_int, C.c_int, C.c_int, f32p]),
@@ -146,6 +148,24 @@ def sign_matvec(sign, xq):
     acc = np.empty(rows, np.int32)
     lib().dfo_sign_matvec(_p(sign, C.c_uint32), rows, 32 * W, _p(xq, C.c_int8), _p(acc, C.c_int32))
     return acc
+
+
+def level_matvec(lvl, xq):
+    """17-level scaffold (five bit planes [rows][K/32][5]): acc_i = sum_k level_ik * q_k (R25)"""
+    lvl, xq = _c(lvl, np.uint32), _c(xq, np.int8)
+    rows, W, five = lvl.shape
+    assert five == 5 and xq.size == 32 * W
+    acc = np.empty(rows, np.int32)
+    lib().dfo_level_matvec(_p(lvl, C.c_uint32), rows, 32 * W, _p(xq, C.c_int8), _p(acc, C.c_int32))
+    return acc
+
+
+def unpack_int4(packed):
+    packed = _c(packed, np.uint8)
+    rows, half = packed.shape
+    out = np.empty((rows, 2 * half), np.int8)
+    lib().dfo_unpack_int4(_p(packed, C.c_uint8), rows, 2 * half, _p(out, C.c_int8))
+    return out
 
 
 def lora_down(A, xq):

@@ -248,6 +248,39 @@ void dfo_lora_down(const int8_t* A, int r, int K, const int8_t* xq, int32_t* t)
     }
 }
 
+/* Format variant (R25): the 17-level scaffold of Eq. 1 / Eq. 3,
+ * W_scaffold in {-1, -14/16, ..., 14/16, 1} = level / 8 with level = m - 8, m in [0, 16] stored as five bit planes:
+ * bit b of lvl[i][w][p] is bit p of m of element k = 32*w + b.  acc_i = sum_k level_ik * q_k, exact int32
+ * (the row scale of the blob multiplies this integer sum, i.e. it holds the paper's scale / 8). */
+void dfo_level_matvec(const uint32_t* lvl, int rows, int K, const int8_t* xq, int32_t* acc)
+{
+    const int W = K / 32;
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < rows; ++i) {
+        int32_t a = 0;
+        for (int w = 0; w < W; ++w) {
+            const uint32_t* pl = lvl + ((size_t)i * W + w) * 5;
+            for (int b = 0; b < 32; ++b) {
+                int m = 0;
+                for (int p = 0; p < 5; ++p) m |= (int)((pl[p] >> b) & 1u) << p;
+                a += (int32_t)(m - 8) * (int32_t)xq[32 * w + b];
+            }
+        }
+        acc[i] = a;
+    }
+}
+
+/* Format variant: int4 LoRA (Table 4).  Element 2i of a row is the low nibble of byte i, element 2i + 1 the high
+ * nibble; a nibble is a two's-complement 4-bit integer in [-8, 7].  n = values per row (even). */
+void dfo_unpack_int4(const uint8_t* packed, int rows, int n, int8_t* out)
+{
+    for (int i = 0; i < rows; ++i)
+        for (int j = 0; j < n; ++j) {
+            const int nib = (packed[(size_t)i * (n / 2) + j / 2] >> (4 * (j & 1))) & 0xF;
+            out[(size_t)i * n + j] = (int8_t)(nib >= 8 ? nib - 16 : nib);
+        }
+}
+
 /* S3 stage 2 + dequantisation: y = W_scaffold x + W_A (W_B x), Eq. 3, alpha folded in scales */
 void dfo_proj_epilogue(const int32_t* acc, const int32_t* t, const uint16_t* row_scale_f16,
                        const float* a_s, const int8_t* B, const float* b_s,
@@ -407,12 +440,14 @@ typedef struct {
     const float* gnorm_w;
     const uint32_t* out_sign; const uint16_t* out_row_scale;
     const int8_t* out_A; const float* out_a_s; const int8_t* out_B; const float* out_b_s;
+    int8_t* own[4];            /* int4 LoRA: the unpacked copies of A / B (in, out) this layer owns */
 } dfo_layer;
 
 struct dfo_model {
     uint8_t* blob;
     int n_layers, d_model, d_inner, headdim, d_state, ngroups, d_conv, vocab, r;
     int nheads, d_in_proj, conv_dim;
+    int fmt;                    /* blob header word 52: bit 0 = 17-level scaffold, bit 1 = int4 LoRA (R25) */
     float eps;
     int max_batch, last_batch;
     dfo_layer* layers;
@@ -444,6 +479,9 @@ dfo_model* dfo_load(const void* blob, size_t nbytes, int max_batch, char* err, s
     m->headdim = rd_i32(b + 24);  m->d_state = rd_i32(b + 28); m->ngroups = rd_i32(b + 32);
     m->d_conv = rd_i32(b + 36);   m->vocab = rd_i32(b + 40);   m->r = rd_i32(b + 44);
     memcpy(&m->eps, b + 48, 4);
+    m->fmt = rd_i32(b + 52);
+    if (m->fmt < 0 || m->fmt > 3) FAIL("unknown weight format");
+    if ((m->fmt & 2) && (m->r % 2)) FAIL("int4 LoRA needs an even rank");
     uint64_t total; memcpy(&total, b + 56, 8);
     if (total != (uint64_t)nbytes) FAIL("blob size does not match header");
     if (m->d_conv != 4) FAIL("d_conv must be 4");
@@ -469,11 +507,18 @@ dfo_model* dfo_load(const void* blob, size_t nbytes, int max_batch, char* err, s
     for (int l = 0; l < m->n_layers; ++l) {
         dfo_layer* L = &m->layers[l];
         TAKE(L->norm_w, float, dm);
-        TAKE(L->in_sign, uint32_t, dip * (dm / 32));
+        const size_t planes = (m->fmt & 1) ? 5 : 1;      /* in_sign / out_sign point at the bit planes then */
+        const int i4 = (m->fmt & 2) != 0;
+#define TAKE_LORA(dst, slot, rows_, n_) do { \
+            if (i4) { const uint8_t* pk; TAKE(pk, uint8_t, (size_t)(rows_) * (n_) / 2); \
+                      L->own[slot] = (int8_t*)malloc((size_t)(rows_) * (n_)); if (!L->own[slot]) FAIL("out of memory"); \
+                      dfo_unpack_int4(pk, (int)(rows_), (int)(n_), L->own[slot]); (dst) = L->own[slot]; } \
+            else TAKE(dst, int8_t, (size_t)(rows_) * (n_)); } while (0)
+        TAKE(L->in_sign, uint32_t, dip * (dm / 32) * planes);
         TAKE(L->in_row_scale, uint16_t, dip);
-        TAKE(L->in_A, int8_t, r * dm);
+        TAKE_LORA(L->in_A, 0, r, dm);
         TAKE(L->in_a_s, float, r);
-        TAKE(L->in_B, int8_t, dip * r);
+        TAKE_LORA(L->in_B, 1, dip, r);
         TAKE(L->in_b_s, float, dip);
         TAKE(L->conv_w, float, (size_t)m->conv_dim * 4);
         TAKE(L->conv_b, float, m->conv_dim);
@@ -481,11 +526,11 @@ dfo_model* dfo_load(const void* blob, size_t nbytes, int max_batch, char* err, s
         TAKE(L->dt_bias, float, m->nheads);
         TAKE(L->D, float, m->nheads);
         TAKE(L->gnorm_w, float, di);
-        TAKE(L->out_sign, uint32_t, dm * (di / 32));
+        TAKE(L->out_sign, uint32_t, dm * (di / 32) * planes);
         TAKE(L->out_row_scale, uint16_t, dm);
-        TAKE(L->out_A, int8_t, r * di);
+        TAKE_LORA(L->out_A, 2, r, di);
         TAKE(L->out_a_s, float, r);
-        TAKE(L->out_B, int8_t, dm * r);
+        TAKE_LORA(L->out_B, 3, dm, r);
         TAKE(L->out_b_s, float, dm);
     }
     TAKE(m->emb, int8_t, (size_t)m->vocab * dm);
@@ -516,6 +561,9 @@ dfo_model* dfo_load(const void* blob, size_t nbytes, int max_batch, char* err, s
 void dfo_free(dfo_model* m)
 {
     if (!m) return;
+    if (m->layers)
+        for (int l = 0; l < m->n_layers; ++l)
+            for (int k = 0; k < 4; ++k) free(m->layers[l].own[k]);
     free(m->blob); free(m->layers); free(m->ssm); free(m->conv); free(m->logits);
     free(m->next); free(m->hidden); free(m->taps); free(m);
 }
@@ -613,7 +661,8 @@ static void step_one(dfo_model* m, int s, int32_t tok)
         const dfo_layer* L = &m->layers[l];
         dfo_norm_quant(u, L->norm_w, dm, m->eps, xq, &sx, NULL, NULL);                   /* S1 */
         TAP(DFO_TAP_XQ_IN, xq, (size_t)dm); TAP(DFO_TAP_S_IN, &sx, 4);
-        dfo_sign_matvec(L->in_sign, dip, dm, xq, acc);                                   /* S2 */
+        if (m->fmt & 1) dfo_level_matvec(L->in_sign, dip, dm, xq, acc);                  /* S2, 17-level variant */
+        else dfo_sign_matvec(L->in_sign, dip, dm, xq, acc);                              /* S2 */
         dfo_lora_down(L->in_A, r, dm, xq, t);                                            /* S3 */
         dfo_proj_epilogue(acc, t, L->in_row_scale, L->in_a_s, L->in_B, L->in_b_s, dip, r, sx, zx);
         TAP(DFO_TAP_ACC_IN, acc, 4 * (size_t)dip); TAP(DFO_TAP_T_IN, t, 4 * (size_t)r);
@@ -642,7 +691,8 @@ static void step_one(dfo_model* m, int s, int32_t tok)
         TAP(DFO_TAP_G, g, 4 * (size_t)di);
         dfo_norm_quant(g, L->gnorm_w, di, m->eps, xq, &sx, NULL, NULL);
         TAP(DFO_TAP_GQ, xq, (size_t)di); TAP(DFO_TAP_S_G, &sx, 4);
-        dfo_sign_matvec(L->out_sign, dm, di, xq, acc);                                   /* S7 */
+        if (m->fmt & 1) dfo_level_matvec(L->out_sign, dm, di, xq, acc);                  /* S7, 17-level variant */
+        else dfo_sign_matvec(L->out_sign, dm, di, xq, acc);                              /* S7 */
         dfo_lora_down(L->out_A, r, di, xq, t);
         dfo_proj_epilogue(acc, t, L->out_row_scale, L->out_a_s, L->out_B, L->out_b_s, dm, r, sx, o);
         TAP(DFO_TAP_ACC_OUT, acc, 4 * (size_t)dm); TAP(DFO_TAP_T_OUT, t, 4 * (size_t)r);

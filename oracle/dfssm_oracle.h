@@ -46,6 +46,9 @@ void dfo_sign_matvec(const uint32_t* sign, int rows, int K, const int8_t* xq, in
 
 /* S3 stage 1  t_j = sum_k A_jk * xq_k, exact int32                    (Eq. 3) */
 void dfo_lora_down(const int8_t* A, int r, int K, const int8_t* xq, int32_t* t);
+/* format variants (R25): 17-level scaffold as five bit planes [rows][K/32][5]; int4 pairs per byte */
+void dfo_level_matvec(const uint32_t* lvl, int rows, int K, const int8_t* xq, int32_t* acc);
+void dfo_unpack_int4(const uint8_t* packed, int rows, int n, int8_t* out);
 
 /* S3 stage 2 + epilogue  out_i = s_x*( w_s[i]*float(acc_i) + b_s[i]*lo_i ),
  *   lo_i = round32( sum_j float(B_ij) * (a_s[j]*float(t_j)) )        (Eq. 3) */
