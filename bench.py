@@ -62,8 +62,9 @@ def measured_peak():
 # ---------------------------------------------------------------------------------------------
 def algorithmic_bytes(s, batch: int, state_esize: int = 4) -> dict:
     dm, di, dip, r, cd, nh = s.d_model, s.d_inner, s.d_in_proj, s.lora_rank, s.conv_dim, s.nheads
-    scaffold = s.n_layers * (dip * dm + dm * di) // 8
-    lora = s.n_layers * r * (dm + dip + di + dm)
+    fmt = getattr(s, "fmt", 0)           # weight-format variants (R25): 5 bits per scaffold weight, 4 bits per LoRA value
+    scaffold = s.n_layers * (dip * dm + dm * di) // 8 * (5 if fmt & 1 else 1)
+    lora = s.n_layers * r * (dm + dip + di + dm) // (2 if fmt & 2 else 1)
     state = s.n_layers * batch * 2 * (nh * s.headdim * s.d_state * state_esize)      # 2 bytes with --state-fp16 (R24)
     lm_head = s.vocab * dm
     per_layer_small = (4 * dm + 2 * dip + 4 * r + 4 * dip + 16 * cd + 4 * cd + 12 * nh + 4 * di
@@ -82,10 +83,10 @@ def kernel_class_bytes(s, batch: int, state_esize: int = 4) -> dict:
     return {
         "embed": B * (dm + 4 + 4 * dm),
         "normquant": B * (4 * di + 2 * di) + 4 * di,
-        "proj_in": dip * dm // 8 + r * dm + B * (2 * dm + 4 * dip + 4 * r),
+        "proj_in": dip * dm // 8 * (5 if getattr(s, "fmt", 0) & 1 else 1) + r * dm // (2 if getattr(s, "fmt", 0) & 2 else 1) + B * (2 * dm + 4 * dip + 4 * r),
         "ssm": B * (2 * nh * s.headdim * s.d_state * state_esize + 2 * cd * 4 * 4 + 4 * dip + 4 * di)
         + 2 * dip + dip * r + 4 * dip + 20 * cd + 12 * nh,
-        "proj_out": dm * di // 8 + r * di + B * (2 * di + 4 * dm + 4 * r),
+        "proj_out": dm * di // 8 * (5 if getattr(s, "fmt", 0) & 1 else 1) + r * di // (2 if getattr(s, "fmt", 0) & 2 else 1) + B * (2 * di + 4 * dm + 4 * r),
         "epi_out": 2 * dm + dm * r + 4 * dm + B * (4 * dm + 8 * dm),
         "lmhead": s.vocab * dm + 4 * s.vocab + B * (dm + 4 * s.vocab),
         "argmax": B * 4 * s.vocab,
@@ -201,7 +202,7 @@ def run_reference(args, s, blob):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
         "warmup": int(toks.shape[0]), "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "int8 x {-1,+1} -> int32; fp32 state", "data": "synthetic",
-        "config": {"workload": workload_name(args.config, args.batch), "seed": args.config},
+        "config": {"workload": workload_name(args.config, args.batch, FORMATS[args.format]), "seed": args.config},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.get_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
@@ -231,11 +232,15 @@ def whole_job_rate(world: int, batch: int, steps: int, seconds: float) -> float:
     return world * batch * steps / seconds
 
 
-def workload_name(cfg_idx: int, batch: int) -> str:
+FORMATS = {"1bit": 0, "17level": 1, "int4": 2, "17level+int4": 3}
+
+
+def workload_name(cfg_idx: int, batch: int, fmt: int = 0) -> str:
     names = {0: "cfg0 tiny DF-SSM (2 layers, d_model 256)", 1: "cfg1 Mamba-2-130M-shape DF-SSM",
              2: "cfg2 Mamba-2-1.3B-shape DF-SSM (48 layers, d_model 2048, d_state 128, LoRA r32)",
              3: "cfg3 Mamba-2-1.3B-shape DF-SSM batch sweep", 4: "cfg4 Mamba-2-2.7B-shape DF-SSM"}
-    return f"{names.get(cfg_idx, f'cfg{cfg_idx}')}, batch {batch}, greedy decode after a uniform-random prompt"
+    fm = {0: "", 1: ", 17-level scaffold", 2: ", int4 LoRA", 3: ", 17-level scaffold + int4 LoRA"}[fmt]
+    return f"{names.get(cfg_idx, f'cfg{cfg_idx}')}{fm}, batch {batch}, greedy decode after a uniform-random prompt"
 
 
 # ---------------------------------------------------------------------------------------------
@@ -382,8 +387,8 @@ def run_ours(args, s, blob):
         "repeats": {"n": len(rep_ms), "steps_each": args.steps, "best_ms_per_step": min(rep_ms) / args.steps,
                     "median_ms_per_step": statistics.median(rep_ms) / args.steps, "extra_warmup_steps": extra_warmup},
         "speedup_vs_cpu_baseline": (value / cpu_baseline["value"]) if cpu_baseline else None,
-        "dtype": "int8 x {-1,+1} -> int32; " + ("fp16 state (lossy option, DESIGN.md R24)" if args.state_fp16 else "fp32 state"), "data": "synthetic",
-        "config": {"workload": workload_name(args.config, B), "seed": args.config, "batch_per_gpu": B,
+        "dtype": ("int8 x {-8..8} -> int32; " if FORMATS[args.format] & 1 else "int8 x {-1,+1} -> int32; ") + ("fp16 state (lossy option, DESIGN.md R24)" if args.state_fp16 else "fp32 state"), "data": "synthetic",
+        "config": {"workload": workload_name(args.config, B, FORMATS[args.format]), "seed": args.config, "batch_per_gpu": B,
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": f"inputs larger than L2: {ab['total'] / 1e6:.0f} MB streamed per step vs ~126 MB L2"},
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 4 * B, "d2h_bytes_per_step": 4 * B,
@@ -446,6 +451,8 @@ def main():
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--batch", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--format", default="1bit", choices=sorted(FORMATS),
+                    help="weight format of the synthetic blob (SURVEY 8(f) NEXT-3): 17-level scaffold and / or int4 LoRA; kernel chain only")
     ap.add_argument("--state-fp16", action="store_true",
                     help="SSM state stored as binary16 (DFSSM_FLAG_STATE_FP16, SURVEY 8(f) NEXT-2; lossy; kernel chain only)")
     ap.add_argument("--reps", type=int, default=5, help="repetitions of the K timed steps (the first is the reported value)")
@@ -457,7 +464,7 @@ def main():
         raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: launch with torchrun --nproc-per-node {args.gpus}, or without torchrun")
     if args.impl == "reference" and int(os.environ.get("RANK", "0")) != 0:
         return
-    s = ds.shape_for_config(args.config)
+    s = ds.shape_for_config(args.config).with_(fmt=FORMATS[args.format])
     blob = ds.make_blob(s, args.config)
     if args.impl == "reference":
         run_reference(args, s, blob)

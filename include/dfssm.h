@@ -66,6 +66,12 @@ enum {
                                    * step's binary32 update; the step's own readout uses the unrounded values).  Halves the state bytes (95 % of the
                                    * traffic at batch 64).  LOSSY against the fp32-state model; bit-identical to the oracle in the same mode.
                                    * Served by the kernel chain and dfssm_prefill (the persistent batch-1 kernel keeps fp32 state). */
+#define DFSSM_FLAG_SCAFFOLD17 128u /* the blob holds the 17-level scaffold of PAPER.md Eq. 1 / Eq. 3 (weights level/8,
+                                   * level in [-8, 8], five bit planes per 32 weights) instead of the 1-bit one; row scales apply to sum(level * q) */
+#define DFSSM_FLAG_LORA_INT4 256u /* the blob holds int4 LoRA matrices (Table 4), two values per byte.
+                                   * Both variants: the blob header's format word (offset 52: bit 0 / bit 1) must agree with these flags; served by
+                                   * the kernel chain with tensor-core projections at every batch size and by dfssm_prefill; they need
+                                   * d_model % 128 == 0, d_inner % 128 == 0 and lora_rank in {8, 16, 32, 64}, and exclude DFSSM_FLAG_NO_MMA. */
 #define DFSSM_FLAG_PROF      8u  /* persistent kernel: thread 0 of every CTA stamps its SM clock at every phase */
 
 /* Shape of the model (the paper's Mamba-2-shaped student, Table 1) + capacity.

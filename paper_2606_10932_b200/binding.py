@@ -22,6 +22,8 @@ FLAG_NO_MEGA = 4
 FLAG_PROF = 8
 FLAG_NO_MMA = 16
 FLAG_STATE_FP16 = 64
+FLAG_SCAFFOLD17 = 128      # 17-level scaffold blob (format word bit 0)
+FLAG_LORA_INT4 = 256       # int4 LoRA blob (format word bit 1)
 
 TAPS = dict(XQ_IN=0, S_IN=1, ACC_IN=2, T_IN=3, ZXBCDT=4, XBC_CONV=5, DT=6, Y=7, G=8, GQ=9,
             S_G=10, ACC_OUT=11, T_OUT=12, HIDDEN=13)
@@ -73,7 +75,10 @@ class Config:
 
     @classmethod
     def from_shape(cls, s, max_batch: int = 1, flags: int = 0) -> "Config":
-        """`s` is anything with the shape attributes (e.g. dfssm_synth.Shape)."""
+        """`s` is anything with the shape attributes (e.g. dfssm_synth.Shape); its weight format (`fmt`, if it has one) sets
+        FLAG_SCAFFOLD17 / FLAG_LORA_INT4."""
+        fmt = int(getattr(s, "fmt", 0))
+        flags |= (FLAG_SCAFFOLD17 if fmt & 1 else 0) | (FLAG_LORA_INT4 if fmt & 2 else 0)
         return cls(s.n_layers, s.d_model, s.d_inner, s.headdim, s.d_state, s.ngroups, s.d_conv, s.vocab,
                    s.lora_rank, max_batch, float(s.norm_eps), flags)
 

@@ -93,6 +93,10 @@ bool valid_cfg(const dfssm_config* c)
     if (c->lora_rank < 1 || c->lora_rank > 64) return false;
     if (c->max_batch < 1 || c->max_batch > 256) return false;
     if (!(c->norm_eps > 0.0f)) return false;
+    if (c->flags & (DFSSM_FLAG_SCAFFOLD17 | DFSSM_FLAG_LORA_INT4)) {       // format variants: tensor-core projections only
+        if (c->d_model % 128 || c->d_inner % 128 || (c->flags & DFSSM_FLAG_NO_MMA)) return false;
+        if (c->lora_rank != 8 && c->lora_rank != 16 && c->lora_rank != 32 && c->lora_rank != 64) return false;
+    }
     return true;
 }
 
@@ -105,6 +109,7 @@ Dims make_dims(const dfssm_config& c)
     d.d_in_proj = 2 * c.d_inner + 2 * c.ngroups * c.d_state + d.nheads;
     d.conv_dim = c.d_inner + 2 * c.ngroups * c.d_state;
     d.eps = c.norm_eps;
+    d.fmt = ((c.flags & DFSSM_FLAG_SCAFFOLD17) ? 1 : 0) | ((c.flags & DFSSM_FLAG_LORA_INT4) ? 2 : 0);
     return d;
 }
 
@@ -118,11 +123,12 @@ size_t blob_bytes_for(const Dims& d)
 {
     BlobWalk w;
     const size_t dm = d.d_model, di = d.d_inner, dip = d.d_in_proj, r = d.r, cd = d.conv_dim, nh = d.nheads;
+    const size_t pl = (d.fmt & 1) ? 5 : 1, ld = (d.fmt & 2) ? 2 : 1;      // bit planes per sign word; LoRA values per byte
     for (int l = 0; l < d.n_layers; ++l) {
-        w.take(4 * dm); w.take(4 * dip * (dm / 32)); w.take(2 * dip); w.take(r * dm); w.take(4 * r);
-        w.take(dip * r); w.take(4 * dip); w.take(16 * cd); w.take(4 * cd); w.take(4 * nh); w.take(4 * nh);
-        w.take(4 * nh); w.take(4 * di); w.take(4 * dm * (di / 32)); w.take(2 * dm); w.take(r * di);
-        w.take(4 * r); w.take(dm * r); w.take(4 * dm);
+        w.take(4 * dm); w.take(4 * dip * (dm / 32) * pl); w.take(2 * dip); w.take(r * dm / ld); w.take(4 * r);
+        w.take(dip * r / ld); w.take(4 * dip); w.take(16 * cd); w.take(4 * cd); w.take(4 * nh); w.take(4 * nh);
+        w.take(4 * nh); w.take(4 * di); w.take(4 * dm * (di / 32) * pl); w.take(2 * dm); w.take(r * di / ld);
+        w.take(4 * r); w.take(dm * r / ld); w.take(4 * dm);
     }
     w.take((size_t)d.vocab * dm); w.take(4 * (size_t)d.vocab); w.take(4 * dm);
     return up(w.off, 64);
@@ -173,7 +179,7 @@ Carve carve(const dfssm_config& c)
     v.tap_stride = (uint32_t)to;
     v.taps = (c.flags & DFSSM_FLAG_TAPS) ? put(nl * B * to) : 0;
     mega::Params mp;
-    v.mega_fit = !(c.flags & (DFSSM_FLAG_NO_MEGA | DFSSM_FLAG_STATE_FP16)) && mega::plan(d, mega::GRID, mp);      // the persistent kernel keeps fp32 state
+    v.mega_fit = !(c.flags & (DFSSM_FLAG_NO_MEGA | DFSSM_FLAG_STATE_FP16)) && d.fmt == 0 && mega::plan(d, mega::GRID, mp);      // the persistent kernel keeps fp32 state
     if (v.mega_fit) {
         const mega::Regions rg = mega::regions(mp);
         v.m_chunks = put(rg.chunks);
@@ -249,6 +255,7 @@ bool use_mma(const dfssm_ctx* c, int batch, int K)
 {
     // measured (ms/step, dp4a rows vs tensor cores; cfg 3: batch 5 1.99 / 1.68, 8 2.50 / 1.82, 15 3.32 / 2.21; cfg 4: batch 5 3.49 / 2.73,
     // 8 4.34 / 3.10; cfg 1 (d_model 768): batch 8 0.64 / 0.68): from batch 5 on for the wide models, from 16 on for narrow ones
+    if (c->dm.fmt) return true;                       // the format variants are unpacked by k_proj_mma only
     const int mma_min = c->dm.d_model >= 1024 ? 5 : 16;
     return batch >= mma_min && K % mma::KMULT == 0 && !(c->cfg.flags & DFSSM_FLAG_NO_MMA);
 }
@@ -259,6 +266,16 @@ bool use_mma(const dfssm_ctx* c, int batch, int K)
 // what hides its latencies (measured, cfg 3, ms/step at batch 64 / 16: 1 CTA 5.72 / 3.52, 2 CTAs 5.46 / 3.24, 3 CTAs 5.49 / 3.29,
 // 4 CTAs 5.53 / 3.23)
 constexpr int MMA_CTAS_PER_SM = 2;
+// k_proj_mma<FMT> for the weight format of the model (the LM head always runs FMT = 0: the embedding is int8 in every format)
+#define DFSSM_MMA_LAUNCH(FMT_, GRID_, ST_, ...)                                                                        \
+    do {                                                                                                               \
+        switch (FMT_) {                                                                                                \
+            case 1: mma::k_proj_mma<1><<<GRID_, mma::THREADS, mma::SMEM_BYTES, ST_>>>(__VA_ARGS__); break;             \
+            case 2: mma::k_proj_mma<2><<<GRID_, mma::THREADS, mma::SMEM_BYTES, ST_>>>(__VA_ARGS__); break;             \
+            case 3: mma::k_proj_mma<3><<<GRID_, mma::THREADS, mma::SMEM_BYTES, ST_>>>(__VA_ARGS__); break;             \
+            default: mma::k_proj_mma<0><<<GRID_, mma::THREADS, mma::SMEM_BYTES, ST_>>>(__VA_ARGS__); break;            \
+        }                                                                                                              \
+    } while (0)
 int launch_proj_mma(dfssm_ctx* ctx, const uint32_t* sign, const int8_t* A, int rows, int K, int batch)
 {
     const Dims& d = ctx->dm;
@@ -271,8 +288,8 @@ int launch_proj_mma(dfssm_ctx* ctx, const uint32_t* sign, const int8_t* A, int r
     int32_t* acc = at<int32_t>(ctx, v.acc);
     int32_t* t = at<int32_t>(ctx, v.t);
     // ks > 1: acc / t were zeroed by the k_normquant launch in front of this projection
-    mma::k_proj_mma<<<dim3(mt, nt, ks), mma::THREADS, mma::SMEM_BYTES, ctx->stream>>>(sign, A, rows, d.r, K, at<int8_t>(ctx, v.xq), (int)v.ldq, batch,
-                                                                      acc, (int)v.ld_acc, t, at<int>(ctx, v.err));
+    DFSSM_MMA_LAUNCH(d.fmt, dim3(mt, nt, ks), ctx->stream, sign, A, rows, d.r, K, at<int8_t>(ctx, v.xq), (int)v.ldq, batch, acc, (int)v.ld_acc, t,
+                     at<int>(ctx, v.err), nullptr, nullptr, nullptr);
     return DFSSM_OK;
 }
 
@@ -281,11 +298,24 @@ void launch_epi_out(const LayerW& L, const Dims& d, int n, const int32_t* acc, i
                     uint8_t* tp, uint32_t tap_stride, uint32_t tap_off, cudaStream_t st)
 {
     const dim3 g4((d.d_model + FIN_THREADS - 1) / FIN_THREADS, n);
+    const bool i4 = (d.fmt & 2) != 0;
     switch (d.r) {
-        case 8: k_epi_out4<2><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off); break;
-        case 16: k_epi_out4<4><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off); break;
-        case 32: k_epi_out4<8><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off); break;
-        case 64: k_epi_out4<16><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off); break;
+        case 8:
+            if (i4) k_epi_out4<2, true><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
+            else k_epi_out4<2><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
+            break;
+        case 16:
+            if (i4) k_epi_out4<4, true><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
+            else k_epi_out4<4><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
+            break;
+        case 32:
+            if (i4) k_epi_out4<8, true><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
+            else k_epi_out4<8><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
+            break;
+        case 64:
+            if (i4) k_epi_out4<16, true><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
+            else k_epi_out4<16><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
+            break;
         default:
             k_epi_out<<<dim3((d.d_model + EPI_THREADS - 1) / EPI_THREADS, n), EPI_THREADS, 0, st>>>(L, d.d_model, d.r, acc, ld_acc, t, s_g, u, tp, tap_stride,
                                                                                                   tap_off);
@@ -364,10 +394,22 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
             const dim3 gf((d.d_in_proj + FIN_THREADS - 1) / FIN_THREADS, batch);
 #define DFSSM_FIN_ARGS L, d, acc, ld_acc, t, sx, conv, pos, fin, tp, v.tap_stride, v.tl
             switch (d.r) {
-                case 8: k_fin4<2><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS); break;
-                case 16: k_fin4<4><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS); break;
-                case 32: k_fin4<8><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS); break;
-                case 64: k_fin4<16><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS); break;
+                case 8:
+                    if (d.fmt & 2) k_fin4<2, true><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS);
+                    else k_fin4<2><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS);
+                    break;
+                case 16:
+                    if (d.fmt & 2) k_fin4<4, true><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS);
+                    else k_fin4<4><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS);
+                    break;
+                case 32:
+                    if (d.fmt & 2) k_fin4<8, true><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS);
+                    else k_fin4<8><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS);
+                    break;
+                case 64:
+                    if (d.fmt & 2) k_fin4<16, true><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS);
+                    else k_fin4<16><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS);
+                    break;
                 default: k_fin<<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS); break;
             }
 #undef DFSSM_FIN_ARGS
@@ -423,7 +465,7 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
 
     tm->begin(DFSSM_KCLASS_LMHEAD);
     if (use_mma(c, batch, d.d_model)) {
-        mma::k_proj_mma<<<dim3((d.vocab + mma::TM - 1) / mma::TM, (batch + mma::TN - 1) / mma::TN, 1), mma::THREADS, mma::SMEM_BYTES, st>>>(
+        mma::k_proj_mma<0><<<dim3((d.vocab + mma::TM - 1) / mma::TM, (batch + mma::TN - 1) / mma::TN, 1), mma::THREADS, mma::SMEM_BYTES, st>>>(
             nullptr, c->emb, 0, d.vocab, d.d_model, xq, ldq, batch, nullptr, 0, nullptr, err, logits, sx, c->emb_s);
     } else {
         const int per = LM_THREADS / 32;
@@ -635,7 +677,7 @@ int prefill_chunk(dfssm_ctx* c, const int32_t* tokens_dev, int T, int seq)
             int ks = (148 * MMA_CTAS_PER_SM) / (mt * nt);
             if (ks < 1) ks = 1;
             if (ks > nchunk) ks = nchunk;
-            mma::k_proj_mma<<<dim3(mt, nt, ks), mma::THREADS, mma::SMEM_BYTES, st>>>(sign, A, rows, d.r, K, xq, ldq, T, acc, ld_acc, t, err);
+            DFSSM_MMA_LAUNCH(d.fmt, dim3(mt, nt, ks), st, sign, A, rows, d.r, K, xq, ldq, T, acc, ld_acc, t, err, nullptr, nullptr, nullptr);
         } else {
             k_proj<<<dim3(proj_grid(rows + d.r), (T + PROJ_BT - 1) / PROJ_BT), PROJ_THREADS, proj_smem(K), st>>>(sign, A, rows, d.r, K, xq, xqp, ldq, qsum,
                                                                                                               T, acc, ld_acc, t);
@@ -653,10 +695,22 @@ int prefill_chunk(dfssm_ctx* c, const int32_t* tokens_dev, int T, int seq)
         {
             const dim3 g4((d.d_in_proj + FIN_THREADS - 1) / FIN_THREADS, T);
             switch (d.r) {
-                case 8: prefill::k_pf_epi4<2><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc); break;
-                case 16: prefill::k_pf_epi4<4><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc); break;
-                case 32: prefill::k_pf_epi4<8><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc); break;
-                case 64: prefill::k_pf_epi4<16><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc); break;
+                case 8:
+                    if (d.fmt & 2) prefill::k_pf_epi4<2, true><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
+                    else prefill::k_pf_epi4<2><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
+                    break;
+                case 16:
+                    if (d.fmt & 2) prefill::k_pf_epi4<4, true><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
+                    else prefill::k_pf_epi4<4><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
+                    break;
+                case 32:
+                    if (d.fmt & 2) prefill::k_pf_epi4<8, true><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
+                    else prefill::k_pf_epi4<8><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
+                    break;
+                case 64:
+                    if (d.fmt & 2) prefill::k_pf_epi4<16, true><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
+                    else prefill::k_pf_epi4<16><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
+                    break;
                 default:
                     prefill::k_pf_epi<<<dim3((d.d_in_proj + prefill::EPI_T - 1) / prefill::EPI_T, T), prefill::EPI_T, 0, st>>>(L, d, acc, ld_acc, t, sx, zx,
                                                                                                                         ld_acc);
@@ -745,7 +799,10 @@ int dfssm_create(const dfssm_config* cfg, void* dev_arena, size_t arena_bytes, v
     CK(cudaMallocHost((void**)&ctx->pinned_err, sizeof(int)));
     CK(cudaFuncSetAttribute(k_proj, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)proj_smem(8192)));
     CK(cudaFuncSetAttribute(k_lmhead, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lm_smem(8192)));
-    CK(cudaFuncSetAttribute(mma::k_proj_mma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mma::SMEM_BYTES));
+    CK(cudaFuncSetAttribute(mma::k_proj_mma<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mma::SMEM_BYTES));
+    CK(cudaFuncSetAttribute(mma::k_proj_mma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mma::SMEM_BYTES));
+    CK(cudaFuncSetAttribute(mma::k_proj_mma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mma::SMEM_BYTES));
+    CK(cudaFuncSetAttribute(mma::k_proj_mma<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mma::SMEM_BYTES));
     {
         const int rc = mega_setup(ctx);
         if (rc != DFSSM_OK) return rc;
@@ -762,13 +819,16 @@ int dfssm_load_weights(dfssm_ctx* ctx, const void* host_blob, size_t nbytes)
     const Dims& d = ctx->dm;
     const uint8_t* hb = (const uint8_t*)host_blob;
     if (nbytes < 256 || memcmp(hb, "DFSSMW1\0", 8) != 0) return fail(ctx, DFSSM_E_SIZE, "bad magic or short blob");
-    uint32_t ver; int32_t hdr[9]; float eps; uint64_t total;
+    uint32_t ver, hfmt; int32_t hdr[9]; float eps; uint64_t total;
+    memcpy(&hfmt, hb + 52, 4);
     memcpy(&ver, hb + 8, 4); memcpy(hdr, hb + 12, 36); memcpy(&eps, hb + 48, 4); memcpy(&total, hb + 56, 8);
     if (ver != 1) return fail(ctx, DFSSM_E_ARG, "unsupported blob version %u", ver);
     const int32_t want[9] = { d.n_layers, d.d_model, d.d_inner, d.headdim, d.d_state, d.ngroups, 4, d.vocab, d.r };
     for (int i = 0; i < 9; ++i)
         if (hdr[i] != want[i]) return fail(ctx, DFSSM_E_ARG, "blob header field %d = %d does not match the config (%d)", i, hdr[i], want[i]);
     if (eps != d.eps) return fail(ctx, DFSSM_E_ARG, "blob norm_eps does not match the config");
+    if ((int)hfmt != d.fmt)
+        return fail(ctx, DFSSM_E_ARG, "blob weight format %u (bit 0: 17-level scaffold, bit 1: int4 LoRA) does not match the config flags (%d)", hfmt, d.fmt);
     const size_t expect = blob_bytes_for(d);
     if (total != nbytes || nbytes != expect)
         return fail(ctx, DFSSM_E_SIZE, "blob size %zu does not match its header (%llu) / the shape (%zu)", nbytes,
@@ -778,16 +838,17 @@ int dfssm_load_weights(dfssm_ctx* ctx, const void* host_blob, size_t nbytes)
     CK(cudaMemcpyAsync(db, hb, nbytes, cudaMemcpyHostToDevice, ctx->stream));
     BlobWalk w;
     const size_t dm = d.d_model, di = d.d_inner, dip = d.d_in_proj, r = d.r, cd = d.conv_dim, nh = d.nheads;
+    const size_t pl = (d.fmt & 1) ? 5 : 1, ld = (d.fmt & 2) ? 2 : 1;
     ctx->layers.assign((size_t)d.n_layers, LayerW());
     std::vector<mega::HostLayer> HL((size_t)d.n_layers);
     for (int l = 0; l < d.n_layers; ++l) {
         LayerW& L = ctx->layers[l];
         L.norm_w = (const float*)(db + w.take(4 * dm));
-        L.in_sign = (const uint32_t*)(db + w.take(4 * dip * (dm / 32)));
+        L.in_sign = (const uint32_t*)(db + w.take(4 * dip * (dm / 32) * pl));
         L.in_row_scale = (const __half*)(db + w.take(2 * dip));
-        L.in_A = (const int8_t*)(db + w.take(r * dm));
+        L.in_A = (const int8_t*)(db + w.take(r * dm / ld));
         L.in_a_s = (const float*)(db + w.take(4 * r));
-        L.in_B = (const int8_t*)(db + w.take(dip * r));
+        L.in_B = (const int8_t*)(db + w.take(dip * r / ld));
         L.in_b_s = (const float*)(db + w.take(4 * dip));
         L.conv_w = (const float*)(db + w.take(16 * cd));
         L.conv_b = (const float*)(db + w.take(4 * cd));
@@ -795,11 +856,11 @@ int dfssm_load_weights(dfssm_ctx* ctx, const void* host_blob, size_t nbytes)
         L.dt_bias = (const float*)(db + w.take(4 * nh));
         L.D = (const float*)(db + w.take(4 * nh));
         L.gnorm_w = (const float*)(db + w.take(4 * di));
-        L.out_sign = (const uint32_t*)(db + w.take(4 * dm * (di / 32)));
+        L.out_sign = (const uint32_t*)(db + w.take(4 * dm * (di / 32) * pl));
         L.out_row_scale = (const __half*)(db + w.take(2 * dm));
-        L.out_A = (const int8_t*)(db + w.take(r * di));
+        L.out_A = (const int8_t*)(db + w.take(r * di / ld));
         L.out_a_s = (const float*)(db + w.take(4 * r));
-        L.out_B = (const int8_t*)(db + w.take(dm * r));
+        L.out_B = (const int8_t*)(db + w.take(dm * r / ld));
         L.out_b_s = (const float*)(db + w.take(4 * dm));
         // the same tensors in the host blob (for the mega repack)
         mega::HostLayer& H = HL[l];

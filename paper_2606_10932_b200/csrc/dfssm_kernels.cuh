@@ -26,6 +26,7 @@ struct Dims {
     int n_layers, d_model, d_inner, headdim, d_state, ngroups, vocab, r;
     int nheads, d_in_proj, conv_dim;
     float eps;
+    int fmt;          // weight format variants (R25): bit 0 = 17-level scaffold (five bit planes), bit 1 = int4 LoRA
 };
 
 // debug taps: byte offsets inside one (layer, seq) record; stride = off[DFSSM_TAP_COUNT]
@@ -328,6 +329,7 @@ k_fin(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
 // FIN_THREADS threads finishes FIN_THREADS rows in 4 passes, then lane `sub` of a group finishes the row of pass `sub`, so that
 // the row epilogues (conv, SiLU, softplus) run on every lane and row = base + tid is coalesced.  fp64 sum, tree (p0+p1)+(p2+p3).
 template <int JW> struct BytesT;
+template <> struct BytesT<1> { using T = uint8_t; };
 template <> struct BytesT<2> { using T = uint16_t; };
 template <> struct BytesT<4> { using T = uint32_t; };
 template <> struct BytesT<8> { using T = uint2; };
@@ -337,7 +339,8 @@ template <> struct BytesT<16> { using T = uint4; };
 // binary64 sum  sum_j float(B[row][j]) * v_j,  v_j = a_s[j] * float(t_j),  of row = base + threadIdx.x (0 beyond n_rows).
 // Lane `sub` of a group of four holds v_j for its JW values of j and reads its JW bytes of a row with one load; the group
 // walks through its four rows, and the tree of the sum is (p0 + p1) + (p2 + p3).  No shared memory, no barrier.
-template <int JW>
+// I4: the matrix holds int4 pairs (format variant, R25): a lane's JW values are JW / 2 bytes, element 2i = low nibble.
+template <int JW, bool I4 = false>
 __device__ __forceinline__ double lora_up4(const int8_t* __restrict__ B, const float* __restrict__ a_s,
                                            const int32_t* __restrict__ t_row, int base, int n_rows)
 {
@@ -355,10 +358,20 @@ __device__ __forceinline__ double lora_up4(const int8_t* __restrict__ B, const f
         const int rk = base + q * 4 + k;
         double lo = 0.0;
         if (rk < n_rows) {
-            const typename BytesT<JW>::T w = *(const typename BytesT<JW>::T*)(B + (size_t)rk * R + sub * JW);
-            const uint8_t* wb = (const uint8_t*)&w;
+            if constexpr (I4) {
+                const typename BytesT<JW / 2>::T w = *(const typename BytesT<JW / 2>::T*)((const uint8_t*)B + ((size_t)rk * R + sub * JW) / 2);
+                const uint8_t* wb = (const uint8_t*)&w;
 #pragma unroll
-            for (int i = 0; i < JW; ++i) lo = __fma_rn((double)(int)(int8_t)wb[i], v[i], lo);
+                for (int i = 0; i < JW; ++i) {
+                    const int nib = (wb[i >> 1] >> (4 * (i & 1))) & 0xf;
+                    lo = __fma_rn((double)((nib ^ 8) - 8), v[i], lo);
+                }
+            } else {
+                const typename BytesT<JW>::T w = *(const typename BytesT<JW>::T*)(B + (size_t)rk * R + sub * JW);
+                const uint8_t* wb = (const uint8_t*)&w;
+#pragma unroll
+                for (int i = 0; i < JW; ++i) lo = __fma_rn((double)(int)(int8_t)wb[i], v[i], lo);
+            }
         }
         lo += __shfl_xor_sync(0xffffffffu, lo, 1);
         lo += __shfl_xor_sync(0xffffffffu, lo, 2);
@@ -367,7 +380,7 @@ __device__ __forceinline__ double lora_up4(const int8_t* __restrict__ B, const f
     return sub == 0 ? part[0] : sub == 1 ? part[1] : sub == 2 ? part[2] : part[3];
 }
 
-template <int JW>
+template <int JW, bool I4 = false>
 __global__ void __launch_bounds__(FIN_THREADS)
 k_fin4(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int32_t* __restrict__ t,
        const float* __restrict__ s_x, float* __restrict__ conv_ring, const int32_t* __restrict__ pos,
@@ -394,7 +407,7 @@ k_fin4(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int
         cb = L.conv_b[c];
     }
 
-    const double lo = lora_up4<JW>(L.in_B, L.in_a_s, t + (size_t)b * T_STRIDE, base, d_in_proj);
+    const double lo = lora_up4<JW, I4>(L.in_B, L.in_a_s, t + (size_t)b * T_STRIDE, base, d_in_proj);
     if (!own) return;
     uint8_t* tp = taps ? taps + (size_t)b * tap_stride : nullptr;
     float* out = fin + (size_t)b * (d_in_proj + dm.nheads);
@@ -543,7 +556,7 @@ k_epi_out(LayerW L, int d_model, int r, const int32_t* __restrict__ acc, int ld_
 }
 
 // k_epi_out for lora_rank = 4 * JW: the LoRA sum by lora_up4 (four lanes per row, vector loads of the LoRA-up bytes)
-template <int JW>
+template <int JW, bool I4 = false>
 __global__ void __launch_bounds__(FIN_THREADS)
 k_epi_out4(LayerW L, int d_model, const int32_t* __restrict__ acc, int ld_acc,
            const int32_t* __restrict__ t, const float* __restrict__ s_g, float* __restrict__ u,
@@ -555,7 +568,7 @@ k_epi_out4(LayerW L, int d_model, const int32_t* __restrict__ acc, int ld_acc,
     const int acc_i = acc[(size_t)b * ld_acc + il];
     const float rs = __half2float(L.out_row_scale[il]), bs = L.out_b_s[il], sg = s_g[b];
     const float u0 = u[(size_t)b * d_model + il];
-    const double lo = lora_up4<JW>(L.out_B, L.out_a_s, t + (size_t)b * T_STRIDE, base, d_model);
+    const double lo = lora_up4<JW, I4>(L.out_B, L.out_a_s, t + (size_t)b * T_STRIDE, base, d_model);
     if (!own) return;
     const float o = fmul(sg, fadd(fmul(rs, (float)acc_i), fmul(bs, (float)lo)));
     const float un = fadd(u0, o);

@@ -46,12 +46,31 @@ __device__ __forceinline__ uint32_t signs4(uint32_t bits)
     return 0xffffffffu ^ (spread * 0xfeu);
 }
 
+// ---- format variants (R25) ----
+// 17-level scaffold: four weights (bits sh .. sh+3 of the five planes of one 32-weight word) -> four int8 levels m - 8 in [-8, 8]
+__device__ __forceinline__ uint32_t spread4(uint32_t bits) { return ((bits & 0xfu) * 0x00204081u) & 0x01010101u; }
+__device__ __forceinline__ uint32_t levels4(const uint32_t* pl, int sh)
+{
+    const uint32_t m = spread4(pl[0] >> sh) + (spread4(pl[1] >> sh) << 1) + (spread4(pl[2] >> sh) << 2) + (spread4(pl[3] >> sh) << 3) +
+                       (spread4(pl[4] >> sh) << 4);              // bytes 0 .. 16: no carry between bytes
+    return __vsub4(m, 0x08080808u);
+}
+// int4 LoRA: eight two's-complement nibbles (element 2i = low nibble of byte i) -> eight int8 in element order
+__device__ __forceinline__ uint2 nibbles8(uint32_t w)
+{
+    const uint32_t lo = w & 0x0f0f0f0fu, hi = (w >> 4) & 0x0f0f0f0fu;
+    const uint32_t a = __byte_perm(lo, hi, 0x5140), b = __byte_perm(lo, hi, 0x7362);
+    return make_uint2(__vsub4(a ^ 0x08080808u, 0x08080808u), __vsub4(b ^ 0x08080808u, 0x08080808u));
+}
+
 // grid = (ceil((rows + r) / 128), ceil(batch / 64), ksplit); 512 threads; K % 128 == 0.  LM head: rows = 0, r = vocab,
 // A = the embedding, ksplit = 1, logits / s_h / e_s given.  With ksplit > 1 every CTA takes a
 // slice of K and ADDS its int32 partial sums into acc / t (exact in any order), which the caller has zeroed.
 // 16 warps: the kernel was bound by the issue latency of 4 warps that unpack, stage and store in turn (ncu: 11 % of the warp
 // slots, one issue per 8 cycles per warp); a thread now unpacks 32 weights and stages 16 codes per chunk, and a warp reads one
 // 32-lane x 16-column block of the accumulators.
+// FMT: bit 0 = `sign` holds the five bit planes of the 17-level scaffold ([row][K/32][5]), bit 1 = `A` holds int4 pairs ([r][K/2]).
+template <int FMT>
 __global__ void __launch_bounds__(THREADS)
 k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int rows, int r, int K,
            const int8_t* __restrict__ xq, int ldq, int batch, int32_t* __restrict__ acc, int ld_acc,
@@ -107,14 +126,23 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
     // the sign words and the codes of a stage are requested one stage ahead (registers), before the stage in hand is unpacked,
     // so that their latency runs under the unpack and the MMAs; the few LoRA-down rows (last tile only) are read directly
     const bool is_sign = urow < rows;
-    const uint32_t* sign_row = sign + (size_t)(is_sign ? urow : 0) * W + 2 * qk;
+    constexpr int PL = (FMT & 1) ? 5 : 1;               // words per 32 weights
+    constexpr int NWD = 2 * PL;                         // words of this thread per stage (64 weights)
+    const uint32_t* sign_row = sign + ((size_t)(is_sign ? urow : 0) * W + 2 * qk) * PL;
     const int8_t* x_row = xq + (size_t)(b_valid ? b0 + bn : 0) * ldq + xc * 16;
-    uint2 w_next = make_uint2(0, 0), w_cur;
+    uint32_t w_next[NWD], w_cur[NWD];
+#pragma unroll
+    for (int i = 0; i < NWD; ++i) w_next[i] = 0;
     uint4 x_next[2] = { make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0) }, x_cur[2];
     auto request = [&](int kc) {
         // byte offsets of this thread's pieces inside K; beyond K (last half stage) the operands are zero
         const int ka = kc * KC + qk * 64, kx = kc * KC + xc * 16;
-        w_next = (is_sign && ka < K) ? *(const uint2*)(sign_row + kc * (KC / 32)) : make_uint2(0, 0);
+#pragma unroll
+        for (int i = 0; i < NWD / 2; ++i) {
+            const uint2 ww = (is_sign && ka < K) ? *(const uint2*)(sign_row + (size_t)kc * (KC / 32) * PL + 2 * i) : make_uint2(0, 0);
+            w_next[2 * i] = ww.x;
+            w_next[2 * i + 1] = ww.y;
+        }
         x_next[0] = (b_valid && kx < K) ? *(const uint4*)(x_row + kc * KC) : make_uint4(0, 0, 0, 0);
         x_next[1] = (b_valid && kx + 128 < K) ? *(const uint4*)(x_row + kc * KC + 128) : make_uint4(0, 0, 0, 0);
     };
@@ -123,17 +151,35 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
         const int it = kc - kc0, s = it % STAGES, use = it / STAGES;
         uint8_t* a_dst = stage_mem + (size_t)s * (TM + TN) * KC + a_off;
         uint8_t* b_dst = stage_mem + (size_t)s * (TM + TN) * KC + b_off;
-        w_cur = w_next; x_cur[0] = x_next[0]; x_cur[1] = x_next[1];
+#pragma unroll
+        for (int i = 0; i < NWD; ++i) w_cur[i] = w_next[i];
+        x_cur[0] = x_next[0]; x_cur[1] = x_next[1];
         if (kc + 1 < kc1) request(kc + 1);
         if (use > 0) wait_stage(s, (uint32_t)(use - 1) & 1u);           // the MMAs that read this stage last are done
         // ---- A: 64 weights of this row -> int8 ----
         const bool a_in = kc * KC + qk * 64 < K;
-        if (is_sign && a_in) {
-            const uint32_t w0 = w_cur.x, w1 = w_cur.y;
+        if ((FMT & 1) && is_sign && a_in) {              // 17 levels: word j of the stage = planes w_cur[5 j .. 5 j + 4]
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const uint32_t* pl = w_cur + 5 * (c >> 1);
+                const int sh = 16 * (c & 1);
+                *(uint4*)(a_dst + c * LBO_A) = make_uint4(levels4(pl, sh), levels4(pl, sh + 4), levels4(pl, sh + 8), levels4(pl, sh + 12));
+            }
+        } else if (is_sign && a_in) {
+            const uint32_t w0 = w_cur[0], w1 = w_cur[1 % NWD];
             *(uint4*)a_dst = make_uint4(signs4(w0), signs4(w0 >> 4), signs4(w0 >> 8), signs4(w0 >> 12));
             *(uint4*)(a_dst + LBO_A) = make_uint4(signs4(w0 >> 16), signs4(w0 >> 20), signs4(w0 >> 24), signs4(w0 >> 28));
             *(uint4*)(a_dst + 2 * LBO_A) = make_uint4(signs4(w1), signs4(w1 >> 4), signs4(w1 >> 8), signs4(w1 >> 12));
             *(uint4*)(a_dst + 3 * LBO_A) = make_uint4(signs4(w1 >> 16), signs4(w1 >> 20), signs4(w1 >> 24), signs4(w1 >> 28));
+        } else if ((FMT & 2) && !is_sign && urow < rows_total && a_in) {      // int4 LoRA-down row: 64 values in 32 bytes
+            const uint4* src = (const uint4*)((const uint8_t*)A + ((size_t)(urow - rows) * K + kc * KC + qk * 64) / 2);
+            const uint4 p0 = src[0], p1 = src[1];
+            const uint32_t pw[8] = { p0.x, p0.y, p0.z, p0.w, p1.x, p1.y, p1.z, p1.w };
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const uint2 e0 = nibbles8(pw[2 * c]), e1 = nibbles8(pw[2 * c + 1]);
+                *(uint4*)(a_dst + c * LBO_A) = make_uint4(e0.x, e0.y, e1.x, e1.y);
+            }
         } else if (!is_sign && urow < rows_total && a_in) {
             const uint4* src = (const uint4*)(A + (size_t)(urow - rows) * K + kc * KC + qk * 64);
 #pragma unroll

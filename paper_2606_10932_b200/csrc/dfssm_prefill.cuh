@@ -29,7 +29,7 @@ k_pf_epi(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const i
 }
 
 // the same for lora_rank = 4 * JW: the LoRA sum by lora_up4 (four lanes per row, vector loads of the LoRA-up bytes; k_fin4's scheme)
-template <int JW>
+template <int JW, bool I4 = false>
 __global__ void __launch_bounds__(FIN_THREADS)
 k_pf_epi4(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int32_t* __restrict__ t, const float* __restrict__ s_x,
           float* __restrict__ zx, int ldz)
@@ -39,7 +39,7 @@ k_pf_epi4(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const 
     const int il = own ? i : 0;
     const int acc_i = acc[(size_t)p * ld_acc + il];
     const float rs = __half2float(L.in_row_scale[il]), bs = L.in_b_s[il], sx = s_x[p];
-    const double lo = lora_up4<JW>(L.in_B, L.in_a_s, t + (size_t)p * T_STRIDE, base, dm.d_in_proj);
+    const double lo = lora_up4<JW, I4>(L.in_B, L.in_a_s, t + (size_t)p * T_STRIDE, base, dm.d_in_proj);
     if (own) zx[(size_t)p * ldz + i] = fmul(sx, fadd(fmul(rs, (float)acc_i), fmul(bs, (float)lo)));
 }
 
