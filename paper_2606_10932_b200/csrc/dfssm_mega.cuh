@@ -945,6 +945,10 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     // ([r_pad / 4][n_bcdt]) so that one thread per row reads shared memory without bank conflicts
                     const int* bw = own ? (const int*)(stage + P.c_in_B + (size_t)slot * x.r_pad()) : (const int*)(blk + P.b_eB) + e;
                     const int bstep = own ? 1 : x.n_bcdt();
+                    // first look at the accumulator of a B|C|dt row BEFORE the LoRA sum: its trip to L2 runs under the sum; the spin
+                    // behind the sum starts only if the word was not there yet (it is: the rows are published ~300 ns earlier)
+                    uint32_t early = SENT;
+                    if (!own && sub == 0 && valid) asm volatile("ld.relaxed.gpu.global.b32 %0, [%1];" : "=r"(early) : "l"(recA + e) : "memory");
                     double lo0 = 0.0, lo1 = 0.0;
                     for (int j4 = 4 * sub; j4 < x.r_pad(); j4 += 4 * LP) {         // pad entries of B are 0, pad entries of v are 0
                         const int w = bw[(j4 >> 2) * bstep];
@@ -960,7 +964,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_mega(const Params P)
                     if (sub != 0 || !valid) continue;
                     const float scale = own ? ((const float*)(stage + P.c_in_scale))[slot] : ((const float*)(blk + P.b_escale))[e];
                     const float bsv = own ? ((const float*)(stage + P.c_in_bs))[slot] : ((const float*)(blk + P.b_ebs))[e];
-                    const int acc = own ? s_acc_in[slot] : (int)(poll_word(x, recA + e) ^ IBIAS);
+                    const int acc = own ? s_acc_in[slot] : (int)((early != SENT ? early : poll_word(x, recA + e)) ^ IBIAS);
                     const float lo = (float)lo0;
                     const float val = fmul(s_act, fadd(fmul(scale, (float)acc), fmul(bsv, lo)));
                     int row;                       // canonical in_proj row (for the taps)
