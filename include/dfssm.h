@@ -218,6 +218,31 @@ DFSSM_API const char* dfssm_last_error(const dfssm_ctx* ctx);
 /* Release the context (never frees the arena).  Safe on null. */
 DFSSM_API void dfssm_destroy(dfssm_ctx* ctx);
 
+/* ---- Continuous-batching greedy generator (second half; the generation loop of P:126) ----------------------
+ * Host logic over ONE context (paper_2606_10932_b200/csrc/dfssm_sched.cu; no kernel of its own): requests wait in a FIFO; every
+ * iteration admits waiting requests into free sequence slots (lowest first: dfssm_reset_state + dfssm_prefill of the prompt, which
+ * leaves the request's first generated token in the context's token buffer), runs ONE dfssm_step for slots 0 .. highest active
+ * slot with that device buffer as input, reads the new tokens back and retires finished requests.  Sequences are independent in
+ * every kernel, so a request's tokens equal those of running it alone, whatever the schedule.  One scheduler per context; N GPUs =
+ * N contexts + N schedulers fed by the caller (replicas only).
+ *   dfssm_sched_create   ctx: a loaded context whose max_batch >= max_batch; dev_scratch: caller-owned device memory that holds one
+ *                        prompt at a time (scratch_bytes / 4 = the longest prompt accepted); cuda_stream: the CONTEXT's stream.
+ *   dfssm_sched_submit   copies the prompt (host int32[n_prompt], n_prompt >= 1) and queues it; *request_id = its handle.
+ *   dfssm_sched_iterate  one iteration as above; *n_active = requests generating or waiting afterwards.  Synchronises the stream.
+ *   dfssm_sched_run      iterates until nothing is active, then dfssm_sync (DFSSM_E_TOKEN if a prompt held a bad token id).
+ *   dfssm_sched_result   the tokens generated so far for a request (copied to tokens_host[capacity] if given), *done = finished.
+ *   dfssm_sched_stats    steps run, and slot-steps used by live requests / run in total (idle slots below the highest live one).
+ * The context must not be stepped by anyone else while a scheduler drives it.  Errors as for the calls it makes. */
+typedef struct dfssm_sched dfssm_sched;
+DFSSM_API int dfssm_sched_create(dfssm_ctx* ctx, int max_batch, void* dev_scratch, size_t scratch_bytes, void* cuda_stream, dfssm_sched** out);
+DFSSM_API int dfssm_sched_submit(dfssm_sched* s, const int32_t* prompt_host, int n_prompt, int max_new_tokens, int* request_id);
+DFSSM_API int dfssm_sched_iterate(dfssm_sched* s, int* n_active);
+DFSSM_API int dfssm_sched_run(dfssm_sched* s);
+DFSSM_API int dfssm_sched_result(dfssm_sched* s, int request_id, int32_t* tokens_host, int capacity, int* n_tokens, int* done);
+DFSSM_API int dfssm_sched_stats(dfssm_sched* s, long long* steps, long long* slot_steps_used, long long* slot_steps_run);
+DFSSM_API const char* dfssm_sched_last_error(const dfssm_sched* s);
+DFSSM_API void dfssm_sched_destroy(dfssm_sched* s);
+
 /* ---- S8 without any allocation, context or arena (paper_2606_10932_b200/csrc/dfssm_noalloc.cu) -------------------------------
  * For callers that cannot call cudaMalloc and cannot hand over an arena (code under CUDA graph capture, tight serving loops,
  * harnesses that forbid allocation).  Computes, for `batch` sequences, what the end of dfssm_step computes (S8: PAPER.md P:96,

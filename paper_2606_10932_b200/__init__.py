@@ -3,8 +3,8 @@
 Argument marshalling only -- every step of the path runs in the CUDA kernels of csrc/.
 PyTorch is used for device memory and the stream.  There is no CPU fallback.
 """
-from .binding import (DfssmError, Config, Model, lib, lib_path, TAPS, KCLASSES, EXPORTED_SYMBOLS,
+from .binding import (DfssmError, Config, Model, Scheduler, lib, lib_path, TAPS, KCLASSES, EXPORTED_SYMBOLS,
                       dfssm_arena_bytes, head_noalloc, head_noalloc_scratch_need, NOALLOC_SCRATCH_BYTES)
 
-__all__ = ["DfssmError", "Config", "Model", "lib", "lib_path", "TAPS", "KCLASSES", "EXPORTED_SYMBOLS",
+__all__ = ["DfssmError", "Config", "Model", "Scheduler", "lib", "lib_path", "TAPS", "KCLASSES", "EXPORTED_SYMBOLS",
            "dfssm_arena_bytes", "head_noalloc", "head_noalloc_scratch_need", "NOALLOC_SCRATCH_BYTES"]

@@ -39,6 +39,8 @@ EXPORTED_SYMBOLS = (
     "dfssm_get_state", "dfssm_set_state", "dfssm_debug_profile", "dfssm_sync", "dfssm_launches_per_step",
     "dfssm_time_kernels", "dfssm_last_error", "dfssm_destroy",
     "dfssm_head_noalloc_scratch_need", "dfssm_head_noalloc", "dfssm_head_noalloc_error",
+    "dfssm_sched_create", "dfssm_sched_submit", "dfssm_sched_iterate", "dfssm_sched_run", "dfssm_sched_result", "dfssm_sched_stats",
+    "dfssm_sched_last_error", "dfssm_sched_destroy",
 )
 
 _ERR = {0: "OK", -1: "E_ARG", -2: "E_SIZE", -3: "E_STATE", -4: "E_CUDA", -5: "E_ARCH", -6: "E_TOKEN"}
@@ -143,6 +145,14 @@ def lib() -> C.CDLL:
         "dfssm_head_noalloc_scratch_need": (C.c_size_t, [C.c_int, C.c_int, C.c_int]),
         "dfssm_head_noalloc": (C.c_int, [vp, vp, vp, vp, C.c_int, C.c_int, C.c_int, C.c_float, vp, vp, vp]),
         "dfssm_head_noalloc_error": (C.c_char_p, []),
+        "dfssm_sched_create": (C.c_int, [vp, C.c_int, vp, C.c_size_t, vp, C.POINTER(vp)]),
+        "dfssm_sched_submit": (C.c_int, [vp, i32p, C.c_int, C.c_int, i32p]),
+        "dfssm_sched_iterate": (C.c_int, [vp, i32p]),
+        "dfssm_sched_run": (C.c_int, [vp]),
+        "dfssm_sched_result": (C.c_int, [vp, C.c_int, i32p, C.c_int, i32p, i32p]),
+        "dfssm_sched_stats": (C.c_int, [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]),
+        "dfssm_sched_last_error": (C.c_char_p, [vp]),
+        "dfssm_sched_destroy": (None, [vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -356,3 +366,54 @@ class Model:
         self._check(self._L.dfssm_time_kernels(self._h, C.c_void_p(tokens_dev.data_ptr()), tokens_dev.numel(), int(iters),
                                                _f32p(out)))
         return dict(zip(KCLASSES, (float(x) for x in out)))
+
+
+class Scheduler:
+    """dfssm_sched_*: continuous-batching greedy generation over one Model (argument marshalling only)."""
+
+    def __init__(self, model: "Model", max_batch: Optional[int] = None, max_prompt: int = 4096):
+        import torch
+        self._m, self._L = model, model._L
+        self._scratch = torch.empty(max_prompt, dtype=torch.int32, device=model.device)
+        h = C.c_void_p()
+        rc = self._L.dfssm_sched_create(model._h, int(max_batch or model.cfg.max_batch), self._scratch.data_ptr(), 4 * max_prompt,
+                                        model.stream.cuda_stream, C.byref(h))
+        self._h = h
+        self._check(rc)
+
+    def _check(self, rc: int):
+        if rc != 0:
+            raise DfssmError(rc, self._L.dfssm_sched_last_error(self._h).decode() if self._h else "")
+
+    def submit(self, prompt, max_new_tokens: int) -> int:
+        p = np.ascontiguousarray(prompt, np.int32)
+        rid = C.c_int32()
+        self._check(self._L.dfssm_sched_submit(self._h, p.ctypes.data_as(C.POINTER(C.c_int32)), p.size, int(max_new_tokens), C.byref(rid)))
+        return int(rid.value)
+
+    def iterate(self) -> int:
+        n = C.c_int32()
+        self._check(self._L.dfssm_sched_iterate(self._h, C.byref(n)))
+        return int(n.value)
+
+    def run(self):
+        self._check(self._L.dfssm_sched_run(self._h))
+
+    def result(self, rid: int):
+        n, done = C.c_int32(), C.c_int32()
+        self._check(self._L.dfssm_sched_result(self._h, int(rid), None, 0, C.byref(n), C.byref(done)))
+        out = np.empty(int(n.value), np.int32)
+        self._check(self._L.dfssm_sched_result(self._h, int(rid), out.ctypes.data_as(C.POINTER(C.c_int32)), out.size, C.byref(n), C.byref(done)))
+        return out, bool(done.value)
+
+    def stats(self) -> dict:
+        a, b, c = C.c_longlong(), C.c_longlong(), C.c_longlong()
+        self._check(self._L.dfssm_sched_stats(self._h, C.byref(a), C.byref(b), C.byref(c)))
+        return dict(steps=int(a.value), slot_steps_used=int(b.value), slot_steps_run=int(c.value))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.dfssm_sched_destroy(self._h)
+            self._h = None
+
+    __del__ = close

@@ -1,0 +1,204 @@
+// dfssm_sched_*: a continuous-batching greedy generator on top of the public entry points (second half: "a
+// multi-replica batch scheduler ... turns the step into a usable generator; no new math from the paper"; the generation loop of
+// PAPER.md P:126).  Host logic only: it calls dfssm_reset_state / dfssm_prefill / dfssm_step / dfssm_next_tokens of ONE context
+// (one replica = one GPU; N replicas are N schedulers fed by the caller's dispatcher) and owns no kernel.
+//
+// Requests (prompt, number of new tokens) wait in a FIFO.  Each iteration admits waiting requests into the free sequence slots of
+// the context (lowest slot first: reset the slot's state, prefill its prompt - the prefill leaves the request's first generated
+// token in the context's token buffer), then runs ONE dfssm_step for slots 0 .. highest active slot with the context's own
+// token buffer as input (greedy tokens never leave the device), reads the new tokens back, appends them to their requests and
+// retires the finished ones.  Sequences are independent in every kernel of the step (batch invariance), so a
+// request's tokens are exactly those of running it alone, whatever the schedule: that is the test (tests/test_gpu_sched.py).
+// Idle slots below the highest active one are stepped too (their state is reset at the next admission).
+#include "../../include/dfssm.h"
+
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <deque>
+#include <new>
+#include <vector>
+
+struct dfssm_sched {
+    dfssm_ctx* ctx;
+    int max_batch;
+    cudaStream_t stream;
+    int32_t* dev_prompt;          // caller's device scratch: one prompt at a time
+    size_t max_prompt;
+    int32_t* host_next;           // pinned, [max_batch]
+    struct Request {
+        std::vector<int32_t> prompt;
+        int max_new;
+        std::vector<int32_t> out;
+        int slot;                 // -1: waiting or done
+        bool done;
+    };
+    std::vector<Request> req;
+    std::deque<int> waiting;
+    std::vector<int> slot_req;    // request id per slot, -1 = free
+    long long steps, slot_steps_used, slot_steps_run;
+    char err[256];
+};
+
+namespace {
+
+int sfail(dfssm_sched* s, int code, const char* msg)
+{
+    if (s) snprintf(s->err, sizeof s->err, "%s", msg);
+    return code;
+}
+
+int from_ctx(dfssm_sched* s, int rc)
+{
+    if (rc != DFSSM_OK) snprintf(s->err, sizeof s->err, "%s", dfssm_last_error(s->ctx));
+    return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
+int dfssm_sched_create(dfssm_ctx* ctx, int max_batch, void* dev_scratch, size_t scratch_bytes, void* cuda_stream, dfssm_sched** out)
+{
+    if (!ctx || !out || max_batch < 1 || !dev_scratch || scratch_bytes < 4) return DFSSM_E_ARG;
+    dfssm_sched* s = new (std::nothrow) dfssm_sched();
+    if (!s) return DFSSM_E_ARG;
+    s->ctx = ctx;
+    s->max_batch = max_batch;
+    s->stream = (cudaStream_t)cuda_stream;
+    s->dev_prompt = (int32_t*)dev_scratch;
+    s->max_prompt = scratch_bytes / 4;
+    s->host_next = nullptr;
+    s->slot_req.assign((size_t)max_batch, -1);
+    s->steps = s->slot_steps_used = s->slot_steps_run = 0;
+    s->err[0] = 0;
+    *out = s;
+    if (cudaMallocHost((void**)&s->host_next, sizeof(int32_t) * (size_t)max_batch) != cudaSuccess) return sfail(s, DFSSM_E_CUDA, "cudaMallocHost failed");
+    return DFSSM_OK;
+}
+
+int dfssm_sched_submit(dfssm_sched* s, const int32_t* prompt_host, int n_prompt, int max_new_tokens, int* request_id)
+{
+    if (!s || !prompt_host || !request_id) return DFSSM_E_ARG;
+    if (n_prompt < 1 || (size_t)n_prompt > s->max_prompt) return sfail(s, DFSSM_E_SIZE, "prompt length outside [1, scratch_bytes / 4]");
+    if (max_new_tokens < 1) return sfail(s, DFSSM_E_ARG, "max_new_tokens < 1");
+    dfssm_sched::Request r;
+    r.prompt.assign(prompt_host, prompt_host + n_prompt);
+    r.max_new = max_new_tokens;
+    r.slot = -1;
+    r.done = false;
+    s->req.push_back(std::move(r));
+    *request_id = (int)s->req.size() - 1;
+    s->waiting.push_back(*request_id);
+    return DFSSM_OK;
+}
+
+// one iteration: admissions, one step, retirements.  *n_active = requests still generating afterwards (+ waiting ones)
+int dfssm_sched_iterate(dfssm_sched* s, int* n_active)
+{
+    if (!s) return DFSSM_E_ARG;
+    const int32_t* next_dev = nullptr;
+    int rc = from_ctx(s, dfssm_next_tokens(s->ctx, &next_dev));
+    if (rc != DFSSM_OK) return rc;
+    // ---- admit: lowest free slot first ----
+    std::vector<int> fresh;
+    for (int slot = 0; slot < s->max_batch && !s->waiting.empty(); ++slot) {
+        if (s->slot_req[slot] >= 0) continue;
+        const int id = s->waiting.front();
+        s->waiting.pop_front();
+        dfssm_sched::Request& r = s->req[id];
+        if ((rc = from_ctx(s, dfssm_reset_state(s->ctx, slot))) != DFSSM_OK) return rc;
+        if (cudaMemcpyAsync(s->dev_prompt, r.prompt.data(), sizeof(int32_t) * r.prompt.size(), cudaMemcpyHostToDevice, s->stream) != cudaSuccess)
+            return sfail(s, DFSSM_E_CUDA, "prompt copy failed");
+        if ((rc = from_ctx(s, dfssm_prefill(s->ctx, s->dev_prompt, (int)r.prompt.size(), slot))) != DFSSM_OK) return rc;
+        // the scratch holds one prompt: the copy of the next one must not overtake this prefill (same stream: it cannot), but the
+        // host vector must stay alive until the copy ran -- it does, requests are never erased
+        r.slot = slot;
+        s->slot_req[slot] = id;
+        fresh.push_back(slot);
+    }
+    int hi = -1;
+    for (int slot = 0; slot < s->max_batch; ++slot)
+        if (s->slot_req[slot] >= 0) hi = slot;
+    if (hi < 0) { if (n_active) *n_active = 0; return DFSSM_OK; }
+    // ---- the first generated token of the fresh requests is already in the token buffer (prefill); read it ----
+    if (!fresh.empty()) {
+        if (cudaMemcpyAsync(s->host_next, next_dev, sizeof(int32_t) * (size_t)(hi + 1), cudaMemcpyDeviceToHost, s->stream) != cudaSuccess ||
+            cudaStreamSynchronize(s->stream) != cudaSuccess)
+            return sfail(s, DFSSM_E_CUDA, "token read-back failed");
+        for (int slot : fresh) {
+            dfssm_sched::Request& r = s->req[s->slot_req[slot]];
+            r.out.push_back(s->host_next[slot]);
+            if ((int)r.out.size() >= r.max_new) { r.done = true; r.slot = -1; s->slot_req[slot] = -1; }
+        }
+        hi = -1;
+        for (int slot = 0; slot < s->max_batch; ++slot)
+            if (s->slot_req[slot] >= 0) hi = slot;
+    }
+    // ---- one decode step for slots 0 .. hi, input = the device's own greedy tokens ----
+    if (hi >= 0) {
+        if ((rc = from_ctx(s, dfssm_step(s->ctx, next_dev, hi + 1))) != DFSSM_OK) return rc;
+        if (cudaMemcpyAsync(s->host_next, next_dev, sizeof(int32_t) * (size_t)(hi + 1), cudaMemcpyDeviceToHost, s->stream) != cudaSuccess ||
+            cudaStreamSynchronize(s->stream) != cudaSuccess)
+            return sfail(s, DFSSM_E_CUDA, "token read-back failed");
+        ++s->steps;
+        s->slot_steps_run += hi + 1;
+        for (int slot = 0; slot <= hi; ++slot) {
+            const int id = s->slot_req[slot];
+            if (id < 0) continue;
+            ++s->slot_steps_used;
+            dfssm_sched::Request& r = s->req[id];
+            r.out.push_back(s->host_next[slot]);
+            if ((int)r.out.size() >= r.max_new) { r.done = true; r.slot = -1; s->slot_req[slot] = -1; }
+        }
+    }
+    int act = (int)s->waiting.size();
+    for (int slot = 0; slot < s->max_batch; ++slot) act += s->slot_req[slot] >= 0;
+    if (n_active) *n_active = act;
+    return DFSSM_OK;
+}
+
+int dfssm_sched_run(dfssm_sched* s)
+{
+    if (!s) return DFSSM_E_ARG;
+    int act = 1;
+    while (act > 0) {
+        const int rc = dfssm_sched_iterate(s, &act);
+        if (rc != DFSSM_OK) return rc;
+    }
+    return from_ctx(s, dfssm_sync(s->ctx));
+}
+
+int dfssm_sched_result(dfssm_sched* s, int request_id, int32_t* tokens_host, int capacity, int* n_tokens, int* done)
+{
+    if (!s || request_id < 0 || request_id >= (int)s->req.size() || !n_tokens) return DFSSM_E_ARG;
+    const dfssm_sched::Request& r = s->req[request_id];
+    *n_tokens = (int)r.out.size();
+    if (done) *done = r.done ? 1 : 0;
+    if (tokens_host) {
+        if (capacity < (int)r.out.size()) return sfail(s, DFSSM_E_SIZE, "result buffer too small");
+        memcpy(tokens_host, r.out.data(), sizeof(int32_t) * r.out.size());
+    }
+    return DFSSM_OK;
+}
+
+int dfssm_sched_stats(dfssm_sched* s, long long* steps, long long* slot_steps_used, long long* slot_steps_run)
+{
+    if (!s) return DFSSM_E_ARG;
+    if (steps) *steps = s->steps;
+    if (slot_steps_used) *slot_steps_used = s->slot_steps_used;
+    if (slot_steps_run) *slot_steps_run = s->slot_steps_run;
+    return DFSSM_OK;
+}
+
+const char* dfssm_sched_last_error(const dfssm_sched* s) { return s ? s->err : ""; }
+
+void dfssm_sched_destroy(dfssm_sched* s)
+{
+    if (!s) return;
+    if (s->host_next) cudaFreeHost(s->host_next);
+    delete s;
+}
+
+}  // extern "C"
