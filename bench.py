@@ -405,7 +405,7 @@ def run_ours(args, s, blob):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
 # captures (profiles/r02_traffic.csv: config,batch,kernel,dram_bytes_per_launch,commit).  NOT measured by this run: the
-# value is reported only while no commit after the one it was captured at touches the kernels (csrc/); on a box without
+# value is reported only while no commit after the one it was captured at touches the kernel's sources; on a box without
 # the git history (gpurun snapshots) that cannot be checked and the source string says so.
 def ncu_traffic(cfg_idx: int, batch: int, kernel: str):
     t = ROOT / "profiles" / "r02_traffic.csv"
@@ -420,7 +420,10 @@ def ncu_traffic(cfg_idx: int, batch: int, kernel: str):
         return None, "no capture of this workload"
     src = f"profiles/r02_traffic.csv (ncu --set full capture at commit {row[4][:12]}, not this run)"
     try:
-        res = subprocess.run(["git", "-C", str(ROOT), "rev-list", f"{row[4]}..HEAD", "--", "paper_2606_10932_b200/csrc"],
+        # the files the captured kernel is built from (k_mega: its own two headers and the shared arithmetic)
+        srcs = [f"paper_2606_10932_b200/csrc/{f}" for f in ("dfssm_mega.cuh", "dfssm_mega_host.cuh", "dfssm_math.cuh")] if kernel == "mega" \
+            else ["paper_2606_10932_b200/csrc"]
+        res = subprocess.run(["git", "-C", str(ROOT), "rev-list", f"{row[4]}..HEAD", "--", *srcs],
                              capture_output=True, text=True, timeout=20)
         if res.returncode != 0:
             return int(row[3]), src + "; staleness unchecked (no git history here)"
