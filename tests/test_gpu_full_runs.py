@@ -115,6 +115,35 @@ def test_cfg3_first_32_steps_every_sequence(env, batch):
     assert st.steps == T and st.diff_hidden == 0 and st.diff_logits == 0, st
 
 
+@pytest.mark.parametrize("cfg_idx,batch,n_prompt,n_decode,seqs", [(3, 64, 0, 256, (63,)), (3, 16, 0, 256, (15,)), (4, 8, 64, 512, (5,))],
+                         ids=["cfg3-b64", "cfg3-b16", "cfg4-b8"])
+def test_batched_full_length_sampled_sequences(env, cfg_idx, batch, n_prompt, n_decode, seqs):
+    """BASELINE.json's full run lengths of the BATCHED configs (cfg 3: 256 greedy decode steps at batch 16 / 64; cfg 4: 64-token
+    prompt + 512 decode steps at batch 8) on the CUDA-graph path, greedy tokens kept on the device; the sampled sequences against
+    batch-1 oracles fed the GPU's own tokens, EVERY step: hidden state and logits bit for bit, greedy token equal."""
+    import os
+    from _parity import compare_step
+    if cfg_idx == 4 and not os.environ.get("DFSSM_LONG_TESTS"):
+        pytest.skip("3 minutes of CPU oracle (passed at commit time): set DFSSM_LONG_TESTS=1 to run")
+    pk, oracle, torch = env["pk"], env["oracle"], env["torch"]
+    s, blob = blob_for(2 if cfg_idx == 3 else cfg_idx)
+    gpu = pk.Model(pk.Config.from_shape(s, max_batch=batch), blob)
+    orcs = {q: oracle.OracleModel(blob, 1) for q in seqs}
+    first = np.stack([ds.token_stream(s.vocab, max(n_prompt, 1), seed=cfg_idx, seq_index=i) for i in range(batch)], 1)      # [step][seq]
+    st = Stats()
+    nxt = None
+    for t in range(n_prompt + n_decode):
+        tk = torch.from_numpy(np.ascontiguousarray(first[t], np.int32)).cuda() if (t < n_prompt or t == 0) else nxt
+        gpu.step(tk)
+        fed = tk.cpu().numpy()
+        for q, o in orcs.items():
+            o.step(fed[q:q + 1])
+            compare_step(gpu, o, q, st, t, f"cfg{cfg_idx}-b{batch}")
+        nxt = gpu.next_tokens()[:batch].clone()
+    print(f"cfg{cfg_idx} b={batch} sequences {seqs}", st)
+    assert st.steps == (n_prompt + n_decode) * len(seqs) and st.diff_hidden == 0 and st.diff_logits == 0, st
+
+
 def test_cfg4_batch8_first_32_steps_every_sequence(env):
     st = run_prompt_then_greedy(env, 4, 8, 32, 0, "cfg4-b8")
     assert st.steps == 32 and st.diff_hidden == 0 and st.diff_logits == 0, st
