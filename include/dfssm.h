@@ -226,7 +226,8 @@ DFSSM_API void dfssm_destroy(dfssm_ctx* ctx);
  * every kernel, so a request's tokens equal those of running it alone, whatever the schedule.  One scheduler per context; N GPUs =
  * N contexts + N schedulers fed by the caller (replicas only).
  *   dfssm_sched_create   ctx: a loaded context whose max_batch >= max_batch; dev_scratch: caller-owned device memory that holds one
- *                        prompt at a time (scratch_bytes / 4 = the longest prompt accepted); cuda_stream: the CONTEXT's stream.
+ *                        prompt at a time and max_batch uniforms (scratch_bytes / 4 - max_batch = the longest prompt accepted);
+ *                        cuda_stream: the CONTEXT's stream.
  *   dfssm_sched_submit   copies the prompt (host int32[n_prompt], n_prompt >= 1) and queues it; *request_id = its handle.
  *   dfssm_sched_iterate  one iteration as above; *n_active = requests generating or waiting afterwards.  Synchronises the stream.
  *   dfssm_sched_run      iterates until nothing is active, then dfssm_sync (DFSSM_E_TOKEN if a prompt held a bad token id).
@@ -236,6 +237,13 @@ DFSSM_API void dfssm_destroy(dfssm_ctx* ctx);
 typedef struct dfssm_sched dfssm_sched;
 DFSSM_API int dfssm_sched_create(dfssm_ctx* ctx, int max_batch, void* dev_scratch, size_t scratch_bytes, void* cuda_stream, dfssm_sched** out);
 DFSSM_API int dfssm_sched_submit(dfssm_sched* s, const int32_t* prompt_host, int n_prompt, int max_new_tokens, int* request_id);
+/* Sampled instead of greedy generation (only while no request is generating): one temperature / top_k (1..64) for the scheduler
+ * (temperature <= 0 or top_k == 1: greedy); token k (0-based) of request id is drawn by dfssm_sample with the uniform
+ * dfssm_sched_uniform(seed + id, k), a counter-based generator (splitmix64 finaliser of seed' + (k + 1) * 0x9E3779B97F4A7C15; its top
+ * 24 bits / 2^24, in [0, 1)), so a request's tokens do not depend on the schedule.  The last max_batch words of dev_scratch hold
+ * the uniforms: the longest prompt accepted is scratch_bytes / 4 - max_batch. */
+DFSSM_API int dfssm_sched_set_sampling(dfssm_sched* s, float temperature, int top_k, unsigned long long seed);
+DFSSM_API float dfssm_sched_uniform(unsigned long long seed, int k);
 DFSSM_API int dfssm_sched_iterate(dfssm_sched* s, int* n_active);
 DFSSM_API int dfssm_sched_run(dfssm_sched* s);
 DFSSM_API int dfssm_sched_result(dfssm_sched* s, int request_id, int32_t* tokens_host, int capacity, int* n_tokens, int* done);

@@ -40,7 +40,7 @@ EXPORTED_SYMBOLS = (
     "dfssm_time_kernels", "dfssm_last_error", "dfssm_destroy",
     "dfssm_head_noalloc_scratch_need", "dfssm_head_noalloc", "dfssm_head_noalloc_error",
     "dfssm_sched_create", "dfssm_sched_submit", "dfssm_sched_iterate", "dfssm_sched_run", "dfssm_sched_result", "dfssm_sched_stats",
-    "dfssm_sched_last_error", "dfssm_sched_destroy",
+    "dfssm_sched_last_error", "dfssm_sched_destroy", "dfssm_sched_set_sampling", "dfssm_sched_uniform",
 )
 
 _ERR = {0: "OK", -1: "E_ARG", -2: "E_SIZE", -3: "E_STATE", -4: "E_CUDA", -5: "E_ARCH", -6: "E_TOKEN"}
@@ -153,6 +153,8 @@ def lib() -> C.CDLL:
         "dfssm_sched_stats": (C.c_int, [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]),
         "dfssm_sched_last_error": (C.c_char_p, [vp]),
         "dfssm_sched_destroy": (None, [vp]),
+        "dfssm_sched_set_sampling": (C.c_int, [vp, C.c_float, C.c_int, C.c_ulonglong]),
+        "dfssm_sched_uniform": (C.c_float, [C.c_ulonglong, C.c_int]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -374,9 +376,10 @@ class Scheduler:
     def __init__(self, model: "Model", max_batch: Optional[int] = None, max_prompt: int = 4096):
         import torch
         self._m, self._L = model, model._L
-        self._scratch = torch.empty(max_prompt, dtype=torch.int32, device=model.device)
+        nb = int(max_batch or model.cfg.max_batch)
+        self._scratch = torch.empty(max_prompt + nb, dtype=torch.int32, device=model.device)       # one prompt + nb uniforms
         h = C.c_void_p()
-        rc = self._L.dfssm_sched_create(model._h, int(max_batch or model.cfg.max_batch), self._scratch.data_ptr(), 4 * max_prompt,
+        rc = self._L.dfssm_sched_create(model._h, nb, self._scratch.data_ptr(), 4 * (max_prompt + nb),
                                         model.stream.cuda_stream, C.byref(h))
         self._h = h
         self._check(rc)
@@ -390,6 +393,9 @@ class Scheduler:
         rid = C.c_int32()
         self._check(self._L.dfssm_sched_submit(self._h, p.ctypes.data_as(C.POINTER(C.c_int32)), p.size, int(max_new_tokens), C.byref(rid)))
         return int(rid.value)
+
+    def set_sampling(self, temperature: float, top_k: int, seed: int = 0):
+        self._check(self._L.dfssm_sched_set_sampling(self._h, float(temperature), int(top_k), int(seed)))
 
     def iterate(self) -> int:
         n = C.c_int32()

@@ -10,6 +10,11 @@
 // retires the finished ones.  Sequences are independent in every kernel of the step (batch invariance), so a
 // request's tokens are exactly those of running it alone, whatever the schedule: that is the test (tests/test_gpu_sched.py).
 // Idle slots below the highest active one are stepped too (their state is reset at the next admission).
+//
+// Sampling (dfssm_sched_set_sampling): one temperature / top-k for the scheduler; token k of request id draws the uniform
+// dfssm_sched_uniform(seed + id, k), a counter-based generator (splitmix64 finaliser of seed' + (k + 1) * 0x9E3779B97F4A7C15, top
+// 24 bits / 2^24) - so a request's random numbers do not depend on the schedule either.  dfssm_sample (R23) is a
+// pure function of (logits, u): slots that already drew their token are re-sampled with the same u and get the same token.
 #include "../../include/dfssm.h"
 
 #include <cuda_runtime.h>
@@ -38,6 +43,11 @@ struct dfssm_sched {
     std::deque<int> waiting;
     std::vector<int> slot_req;    // request id per slot, -1 = free
     long long steps, slot_steps_used, slot_steps_run;
+    float temperature;            // <= 0: greedy
+    int top_k;
+    unsigned long long seed;
+    float* dev_u;                 // [max_batch] uniforms, the tail of the caller's scratch
+    float* host_u;                // pinned, [max_batch]: the uniform each slot drew last
     char err[256];
 };
 
@@ -55,26 +65,69 @@ int from_ctx(dfssm_sched* s, int rc)
     return rc;
 }
 
+// sample the next token of slots 0 .. hi (no-op when greedy): `draw` lists the slots that draw a NEW uniform (token index = the
+// number of tokens their request has so far); every other slot keeps its last one
+int sample_slots(dfssm_sched* s, int hi, const std::vector<int>& draw)
+{
+    if (!(s->temperature > 0.0f) || s->top_k <= 1 || hi < 0) return DFSSM_OK;
+    for (int slot : draw) {
+        const int id = s->slot_req[slot];
+        s->host_u[slot] = dfssm_sched_uniform(s->seed + (unsigned long long)id, (int)s->req[id].out.size());
+    }
+    if (cudaMemcpyAsync(s->dev_u, s->host_u, sizeof(float) * (size_t)(hi + 1), cudaMemcpyHostToDevice, s->stream) != cudaSuccess)
+        return sfail(s, DFSSM_E_CUDA, "uniform copy failed");
+    return from_ctx(s, dfssm_sample(s->ctx, hi + 1, s->temperature, s->top_k, s->dev_u));
+}
+
 }  // namespace
 
 extern "C" {
 
+float dfssm_sched_uniform(unsigned long long seed, int k)
+{
+    unsigned long long x = seed + (unsigned long long)(k + 1) * 0x9E3779B97F4A7C15ull;
+    x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
+    x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
+    x ^= x >> 31;
+    return (float)(x >> 40) * (1.0f / 16777216.0f);       // 24 bits: exact in binary32, in [0, 1)
+}
+
 int dfssm_sched_create(dfssm_ctx* ctx, int max_batch, void* dev_scratch, size_t scratch_bytes, void* cuda_stream, dfssm_sched** out)
 {
-    if (!ctx || !out || max_batch < 1 || !dev_scratch || scratch_bytes < 4) return DFSSM_E_ARG;
+    if (!ctx || !out || max_batch < 1 || !dev_scratch || scratch_bytes < 4 * ((size_t)max_batch + 1)) return DFSSM_E_ARG;
     dfssm_sched* s = new (std::nothrow) dfssm_sched();
     if (!s) return DFSSM_E_ARG;
     s->ctx = ctx;
     s->max_batch = max_batch;
     s->stream = (cudaStream_t)cuda_stream;
     s->dev_prompt = (int32_t*)dev_scratch;
-    s->max_prompt = scratch_bytes / 4;
+    s->max_prompt = scratch_bytes / 4 - (size_t)max_batch;          // the last max_batch words hold the uniforms of dfssm_sample
+    s->dev_u = (float*)dev_scratch + s->max_prompt;
     s->host_next = nullptr;
+    s->host_u = nullptr;
+    s->temperature = 0.0f;
+    s->top_k = 1;
+    s->seed = 0;
     s->slot_req.assign((size_t)max_batch, -1);
     s->steps = s->slot_steps_used = s->slot_steps_run = 0;
     s->err[0] = 0;
     *out = s;
-    if (cudaMallocHost((void**)&s->host_next, sizeof(int32_t) * (size_t)max_batch) != cudaSuccess) return sfail(s, DFSSM_E_CUDA, "cudaMallocHost failed");
+    if (cudaMallocHost((void**)&s->host_next, sizeof(int32_t) * (size_t)max_batch) != cudaSuccess ||
+        cudaMallocHost((void**)&s->host_u, sizeof(float) * (size_t)max_batch) != cudaSuccess)
+        return sfail(s, DFSSM_E_CUDA, "cudaMallocHost failed");
+    memset(s->host_u, 0, sizeof(float) * (size_t)max_batch);
+    return DFSSM_OK;
+}
+
+int dfssm_sched_set_sampling(dfssm_sched* s, float temperature, int top_k, unsigned long long seed)
+{
+    if (!s) return DFSSM_E_ARG;
+    if (top_k < 1 || top_k > 64) return sfail(s, DFSSM_E_ARG, "top_k outside [1, 64]");
+    for (int id : s->slot_req)
+        if (id >= 0) return sfail(s, DFSSM_E_STATE, "sampling parameters cannot change while requests are generating");
+    s->temperature = temperature;
+    s->top_k = top_k;
+    s->seed = seed;
     return DFSSM_OK;
 }
 
@@ -124,6 +177,7 @@ int dfssm_sched_iterate(dfssm_sched* s, int* n_active)
     if (hi < 0) { if (n_active) *n_active = 0; return DFSSM_OK; }
     // ---- the first generated token of the fresh requests is already in the token buffer (prefill); read it ----
     if (!fresh.empty()) {
+        if ((rc = sample_slots(s, hi, fresh)) != DFSSM_OK) return rc;
         if (cudaMemcpyAsync(s->host_next, next_dev, sizeof(int32_t) * (size_t)(hi + 1), cudaMemcpyDeviceToHost, s->stream) != cudaSuccess ||
             cudaStreamSynchronize(s->stream) != cudaSuccess)
             return sfail(s, DFSSM_E_CUDA, "token read-back failed");
@@ -139,6 +193,12 @@ int dfssm_sched_iterate(dfssm_sched* s, int* n_active)
     // ---- one decode step for slots 0 .. hi, input = the device's own greedy tokens ----
     if (hi >= 0) {
         if ((rc = from_ctx(s, dfssm_step(s->ctx, next_dev, hi + 1))) != DFSSM_OK) return rc;
+        {
+            std::vector<int> live;
+            for (int slot = 0; slot <= hi; ++slot)
+                if (s->slot_req[slot] >= 0) live.push_back(slot);
+            if ((rc = sample_slots(s, hi, live)) != DFSSM_OK) return rc;
+        }
         if (cudaMemcpyAsync(s->host_next, next_dev, sizeof(int32_t) * (size_t)(hi + 1), cudaMemcpyDeviceToHost, s->stream) != cudaSuccess ||
             cudaStreamSynchronize(s->stream) != cudaSuccess)
             return sfail(s, DFSSM_E_CUDA, "token read-back failed");
@@ -198,6 +258,7 @@ void dfssm_sched_destroy(dfssm_sched* s)
 {
     if (!s) return;
     if (s->host_next) cudaFreeHost(s->host_next);
+    if (s->host_u) cudaFreeHost(s->host_u);
     delete s;
 }
 

@@ -101,3 +101,62 @@ def test_iterate_admits_in_fifo_order_and_errors(env):
         sch.result(99)
     sch.close()
     m.close()
+
+
+def splitmix_uniform(seed: int, k: int) -> np.float32:
+    """the generator of include/dfssm.h (dfssm_sched_uniform), restated"""
+    M = (1 << 64) - 1
+    x = (seed + (k + 1) * 0x9E3779B97F4A7C15) & M
+    x = ((x ^ (x >> 30)) * 0xBF58476D1CE4E5B9) & M
+    x = ((x ^ (x >> 27)) * 0x94D049BB133111EB) & M
+    x ^= x >> 31
+    return np.float32((x >> 40) / 16777216.0)
+
+
+def test_sampled_generation_is_schedule_independent(env):
+    """temperature / top-k through the scheduler: every request equals its solo run drawn with the same counter-based uniforms,
+    and one request is re-derived on the CPU oracle (dfo_sample on the oracle's logits)."""
+    torch, pk, oracle = env["torch"], env["pk"], env["oracle"]
+    L = pk.lib()
+    for seed, k in ((0, 0), (5, 3), (2 ** 63 + 11, 1000)):
+        u = splitmix_uniform(seed, k)
+        assert 0.0 <= u < 1.0 and np.float32(L.dfssm_sched_uniform(seed, k)) == u
+    us = np.array([splitmix_uniform(9, k) for k in range(4000)])
+    assert abs(us.mean() - 0.5) < 0.02 and np.unique(us).size > 3990
+    s = ds.tiny_shape(n_layers=2, d_model=96, d_inner=192, headdim=32, d_state=32, ngroups=2, lora_rank=5, vocab=101)
+    blob = ds.make_blob(s, seed=23, variant="varied")
+    T, K, SEED, slots = 25.0, 12, 77, 3         # a temperature at which this model leaves the greedy token often
+    rng = np.random.default_rng(8)
+    reqs = [(ds.token_stream(s.vocab, int(rng.integers(1, 20)), seed=300 + i), int(rng.integers(1, 16))) for i in range(8)]
+    m = pk.Model(pk.Config.from_shape(s, max_batch=slots), blob)
+    sch = pk.Scheduler(m, max_prompt=32)
+    sch.set_sampling(T, K, SEED)
+    ids = [sch.submit(p, n) for p, n in reqs]
+    sch.run()
+    got = [sch.result(r)[0] for r in ids]
+    greedy_same = 0
+    for rid, (p, n) in zip(ids, reqs):
+        # solo, on the GPU: prefill-free token-by-token run with dfssm_sample and the request's own uniforms
+        g = pk.Model(pk.Config.from_shape(s, max_batch=1), blob)
+        o = oracle.OracleModel(blob, 1)
+        for t in p:
+            g.step(torch.tensor([int(t)], dtype=torch.int32, device="cuda"))
+            o.step(np.array([t], np.int32))
+        want_g, want_o = [], []
+        for k in range(n):
+            u = splitmix_uniform(SEED + rid, k)
+            g.sample(T, K, torch.tensor([u], dtype=torch.float32, device="cuda"))
+            g.sync()
+            want_g.append(int(g.next_tokens()[0].item()))
+            want_o.append(oracle.sample(o.logits()[0], T, K, float(u)))
+            greedy_same += want_o[-1] == int(o.next_tokens()[0])
+            g.step(g.next_tokens()[:1])
+            o.step(np.array([want_o[-1]], np.int32))
+        assert np.array_equal(got[rid], np.array(want_g, np.int32)), (rid, got[rid], want_g)
+        assert want_g == want_o, (rid, want_g, want_o)
+        g.close()
+    assert greedy_same < sum(n for _, n in reqs), "the sampler never left the greedy path: the test would not see a wrong uniform"
+    with pytest.raises(pk.binding.DfssmError):
+        sch.set_sampling(1.0, 65)
+    sch.close()
+    m.close()
