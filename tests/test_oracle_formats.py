@@ -18,10 +18,14 @@ def setup_module():
 def test_level_codes_are_eq1_levels():
     """Eq. 1 with K_w = 16: w_q = round(clamp((w+1)/2, 0, 1) * 16) / 16 * 2 - 1 takes exactly the 17 values (m - 8) / 8,
     m = 0..16 -- the integer level the planes hold is 8 * w_q."""
+    from pathlib import Path
+    txt = [l for l in (Path(__file__).parent / "golden" / "paper_eq1_levels.txt").read_text().splitlines() if l.strip() and not l.startswith("#")]
+    sixteenths = [int(v) for v in txt[0].split()]
+    assert len(sixteenths) == 17 and sixteenths[0] == -16 and sixteenths[-1] == 16
     w = np.linspace(-1.3, 1.3, 2001)
     m = np.round(np.clip((w + 1) / 2, 0, 1) * 16)
     wq = m / 16 * 2 - 1
-    assert set(np.unique(wq)) == {(k - 8) / 8 for k in range(17)}
+    assert sorted(set(np.unique(wq))) == [v / 16 for v in sixteenths] == [(k - 8) / 8 for k in range(17)]
     lv = (m - 8).astype(np.int64)[None, :1984]                       # 1984 = 62 words
     planes = ds.pack_levels(lv)
     one_hot = np.eye(1984, dtype=np.int8)

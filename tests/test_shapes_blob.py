@@ -28,14 +28,47 @@ def test_table1_embedding_103MB():
     assert round(s.embedding_bytes() / 1e6) == 103
 
 
+def _golden(name):
+    from pathlib import Path
+    rows = {}
+    for line in (Path(__file__).parent / "golden" / name).read_text().splitlines():
+        if line.strip() and not line.startswith("#"):
+            k, *v = line.split()
+            rows[k] = v
+    return rows
+
+
+def test_table1_fixture_is_consistent_and_matches_the_shape_calculator():
+    """tests/golden/paper_table1_sizes.txt = Table 1 as printed: the printed total is the sum of the printed
+    components, the printed ratio is teacher / total, the printed fractions are size / total, and the three components the
+    shape fixes (scaffold, tied embedding, rank-16 LoRA) come out of dfssm_synth's byte counts."""
+    t = _golden("paper_table1_sizes.txt")
+    size = {k: float(v[0]) for k, v in t.items()}
+    parts = ("scaffold_1bit_packed", "embedding_lm_head_tied_int8", "lora_r16_int8", "other_conv_norms_ssm")
+    assert sum(size[k] for k in parts) == size["total"] == 278
+    assert round(size["teacher_fp16"] / size["total"], 1) == size["compression_ratio"]
+    for k in parts:
+        assert round(100 * size[k] / size["total"]) == int(t[k][1]), k
+    s = S.shape_for_config(2)
+    assert round(s.scaffold_bytes() / 1e6) == size["scaffold_1bit_packed"]
+    assert round(s.embedding_bytes() / 1e6) == size["embedding_lm_head_tied_int8"]
+    assert int(s.with_(lora_rank=16).lora_bytes() / 1e6) == size["lora_r16_int8"]        # 12.83 MB, printed as 12
+    # the teacher: 1.3B parameters in FP16 (P:11 "A 1.3B parameter model in FP16 requires 2.7 GB")
+    assert abs(size["teacher_fp16"] / 2 - 1344) < 1
+
+
 def test_state_524k_elements_per_layer():
     # P:13 "fixed-size hidden state (524 KB for Mamba-2 1.3B)" = 64*64*128 elements of one layer
+    c = {k: int(v[0]) for k, v in _golden("paper_constants.txt").items()}
     assert S.shape_for_config(2).ssm_state_elems_per_layer() == 524_288
+    assert S.shape_for_config(2).ssm_state_elems_per_layer() // 1000 == c["state_kb_per_layer_1p3b"]
+    assert S.shape_for_config(2).n_layers == c["n_layers_1p3b"]
 
 
 def test_vnni_row_is_32_instructions():
     # P:138 "32 VPDPBUSD instructions per 2048-element row": 64 weights per instruction
-    assert S.shape_for_config(2).d_model // 64 == 32
+    c = {k: int(v[0]) for k, v in _golden("paper_constants.txt").items()}
+    assert S.shape_for_config(2).d_model // 64 == c["vpdpbusd_per_2048_row"]
 
 
 @pytest.mark.parametrize("idx,dip,cd", [(0, 1160, 640), (1, 3352, 1792), (2, 8512, 4352), (4, 10576, 5376)])
