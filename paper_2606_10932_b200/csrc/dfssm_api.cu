@@ -266,17 +266,34 @@ bool use_mma(const dfssm_ctx* c, int batch, int K)
 // what hides its latencies (measured, cfg 3, ms/step at batch 64 / 16: 1 CTA 5.72 / 3.52, 2 CTAs 5.46 / 3.24, 3 CTAs 5.49 / 3.29,
 // 4 CTAs 5.53 / 3.23)
 constexpr int MMA_CTAS_PER_SM = 2;
+// Launch with (PDL_ true) or without the programmatic-stream-serialization attribute: with it the kernel may be scheduled while the
+// kernel in front of it in the stream drains; it runs its independent prologue and blocks in pdl_wait() until that kernel has
+// completed.  KERNEL_ in parentheses if it has template commas.
+#define DFSSM_LAUNCH_EX(PDL_, KERNEL_, GRID_, BLOCK_, SMEM_, ST_, ...)                                \
+    do {                                                                                              \
+        cudaLaunchConfig_t cfg_ = {};                                                                 \
+        cfg_.gridDim = GRID_;                                                                         \
+        cfg_.blockDim = BLOCK_;                                                                       \
+        cfg_.dynamicSmemBytes = SMEM_;                                                                \
+        cfg_.stream = ST_;                                                                            \
+        cudaLaunchAttribute at_[1];                                                                   \
+        at_[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;                               \
+        at_[0].val.programmaticStreamSerializationAllowed = 1;                                        \
+        cfg_.attrs = at_;                                                                             \
+        cfg_.numAttrs = (PDL_) ? 1 : 0;                                                               \
+        cudaLaunchKernelEx(&cfg_, KERNEL_, __VA_ARGS__);                                              \
+    } while (0)
 // k_proj_mma<FMT> for the weight format of the model (the LM head always runs FMT = 0: the embedding is int8 in every format)
-#define DFSSM_MMA_LAUNCH(FMT_, GRID_, ST_, ...)                                                                        \
+#define DFSSM_MMA_LAUNCH(PDL_, FMT_, GRID_, ST_, ...)                                                                        \
     do {                                                                                                               \
         switch (FMT_) {                                                                                                \
-            case 1: mma::k_proj_mma<1><<<GRID_, mma::THREADS, mma::SMEM_BYTES, ST_>>>(__VA_ARGS__); break;             \
-            case 2: mma::k_proj_mma<2><<<GRID_, mma::THREADS, mma::SMEM_BYTES, ST_>>>(__VA_ARGS__); break;             \
-            case 3: mma::k_proj_mma<3><<<GRID_, mma::THREADS, mma::SMEM_BYTES, ST_>>>(__VA_ARGS__); break;             \
-            default: mma::k_proj_mma<0><<<GRID_, mma::THREADS, mma::SMEM_BYTES, ST_>>>(__VA_ARGS__); break;            \
+            case 1: DFSSM_LAUNCH_EX(PDL_, mma::k_proj_mma<1>, GRID_, mma::THREADS, mma::SMEM_BYTES, ST_, __VA_ARGS__); break;             \
+            case 2: DFSSM_LAUNCH_EX(PDL_, mma::k_proj_mma<2>, GRID_, mma::THREADS, mma::SMEM_BYTES, ST_, __VA_ARGS__); break;             \
+            case 3: DFSSM_LAUNCH_EX(PDL_, mma::k_proj_mma<3>, GRID_, mma::THREADS, mma::SMEM_BYTES, ST_, __VA_ARGS__); break;             \
+            default: DFSSM_LAUNCH_EX(PDL_, mma::k_proj_mma<0>, GRID_, mma::THREADS, mma::SMEM_BYTES, ST_, __VA_ARGS__); break;            \
         }                                                                                                              \
     } while (0)
-int launch_proj_mma(dfssm_ctx* ctx, const uint32_t* sign, const int8_t* A, int rows, int K, int batch)
+int launch_proj_mma(dfssm_ctx* ctx, const uint32_t* sign, const int8_t* A, int rows, int K, int batch, bool pdl)
 {
     const Dims& d = ctx->dm;
     const Carve& v = ctx->cv;
@@ -288,33 +305,33 @@ int launch_proj_mma(dfssm_ctx* ctx, const uint32_t* sign, const int8_t* A, int r
     int32_t* acc = at<int32_t>(ctx, v.acc);
     int32_t* t = at<int32_t>(ctx, v.t);
     // ks > 1: acc / t were zeroed by the k_normquant launch in front of this projection
-    DFSSM_MMA_LAUNCH(d.fmt, dim3(mt, nt, ks), ctx->stream, sign, A, rows, d.r, K, at<int8_t>(ctx, v.xq), (int)v.ldq, batch, acc, (int)v.ld_acc, t,
+    DFSSM_MMA_LAUNCH(pdl, d.fmt, dim3(mt, nt, ks), ctx->stream, sign, A, rows, d.r, K, at<int8_t>(ctx, v.xq), (int)v.ldq, batch, acc, (int)v.ld_acc, t,
                      at<int>(ctx, v.err), nullptr, nullptr, nullptr);
     return DFSSM_OK;
 }
 
 // S7 epilogue + residual for n sequences / positions: four lanes per row when the LoRA rank allows (k_epi_out4)
 void launch_epi_out(const LayerW& L, const Dims& d, int n, const int32_t* acc, int ld_acc, const int32_t* t, const float* s_g, float* u,
-                    uint8_t* tp, uint32_t tap_stride, uint32_t tap_off, cudaStream_t st)
+                    uint8_t* tp, uint32_t tap_stride, uint32_t tap_off, cudaStream_t st, bool pdl = false)
 {
     const dim3 g4((d.d_model + FIN_THREADS - 1) / FIN_THREADS, n);
     const bool i4 = (d.fmt & 2) != 0;
     switch (d.r) {
         case 8:
-            if (i4) k_epi_out4<2, true><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
-            else k_epi_out4<2><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
+            if (i4) DFSSM_LAUNCH_EX(pdl, (k_epi_out4<2, true>), g4, FIN_THREADS, 0, st, L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
+            else DFSSM_LAUNCH_EX(pdl, (k_epi_out4<2, false>), g4, FIN_THREADS, 0, st, L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
             break;
         case 16:
-            if (i4) k_epi_out4<4, true><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
-            else k_epi_out4<4><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
+            if (i4) DFSSM_LAUNCH_EX(pdl, (k_epi_out4<4, true>), g4, FIN_THREADS, 0, st, L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
+            else DFSSM_LAUNCH_EX(pdl, (k_epi_out4<4, false>), g4, FIN_THREADS, 0, st, L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
             break;
         case 32:
-            if (i4) k_epi_out4<8, true><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
-            else k_epi_out4<8><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
+            if (i4) DFSSM_LAUNCH_EX(pdl, (k_epi_out4<8, true>), g4, FIN_THREADS, 0, st, L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
+            else DFSSM_LAUNCH_EX(pdl, (k_epi_out4<8, false>), g4, FIN_THREADS, 0, st, L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
             break;
         case 64:
-            if (i4) k_epi_out4<16, true><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
-            else k_epi_out4<16><<<g4, FIN_THREADS, 0, st>>>(L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
+            if (i4) DFSSM_LAUNCH_EX(pdl, (k_epi_out4<16, true>), g4, FIN_THREADS, 0, st, L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
+            else DFSSM_LAUNCH_EX(pdl, (k_epi_out4<16, false>), g4, FIN_THREADS, 0, st, L, d.d_model, acc, ld_acc, t, s_g, u, tp, tap_stride, tap_off);
             break;
         default:
             k_epi_out<<<dim3((d.d_model + EPI_THREADS - 1) / EPI_THREADS, n), EPI_THREADS, 0, st>>>(L, d.d_model, d.r, acc, ld_acc, t, s_g, u, tp, tap_stride,
@@ -351,6 +368,13 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
     int* err = at<int>(c, v.err);
     const bool taps_on = (c->cfg.flags & DFSSM_FLAG_TAPS) != 0;
     const int ldq = (int)v.ldq, ld_acc = (int)v.ld_acc;
+    // programmatic dependent launch, per kind of kernel (bit set = that kernel may start under the one in front of it):
+    // 1 k_normquant(u), 2 in_proj, 4 k_fin4, 8 k_ssm_stream, 16 k_normquant(g), 32 out_proj, 64 k_epi_out4.  Tensor-core chain only.
+    // Measured (cfg 3, ms/step without / with): batch 5 1.78 / 1.55, 8 1.90 / 1.69, 16 2.20 / 2.01, 32 2.72 / 2.66, 64 3.99 / 3.93; cfg 4
+    // batch 8 3.02 / 2.72; cfg 1 batch 16 0.81 / 0.71.  From batch 32 on k_normquant(g) stays behind k_ssm_stream (its 512-thread CTAs
+    // would take the slots of that kernel's last wave).  DFSSM_PDL_MASK in the environment overrides the choice (0 = off).
+    static const int pdl_env = getenv("DFSSM_PDL_MASK") ? atoi(getenv("DFSSM_PDL_MASK")) : -1;
+    const int pdl = (tm == &dummy && !taps_on) ? (pdl_env >= 0 ? pdl_env : (batch >= 32 ? 111 : 127)) : 0;
 
     tm->begin(DFSSM_KCLASS_EMBED);
     k_embed<<<dim3((d.d_model + 255) / 256, batch), 256, 0, st>>>(tokens, c->emb, c->emb_s, d.vocab, d.d_model, u, err);
@@ -366,19 +390,18 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         float* conv = at<float>(c, v.conv) + (size_t)l * B * (size_t)d.conv_dim * 4;
 
         tm->begin(DFSSM_KCLASS_NORMQUANT);
-        k_normquant<<<batch, NQ_THREADS, 0, st>>>(u, d.d_model, L.norm_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum,
-                                                  tp, v.tap_stride, v.tl.off[DFSSM_TAP_XQ_IN], v.tl.off[DFSSM_TAP_S_IN],
-                                                  use_mma(c, batch, d.d_model) ? acc : nullptr, (int)ld_acc, t);
+        DFSSM_LAUNCH_EX((pdl & 1) && l > 0, k_normquant, batch, NQ_THREADS, 0, st, u, d.d_model, L.norm_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum,
+                        tp, v.tap_stride, v.tl.off[DFSSM_TAP_XQ_IN], v.tl.off[DFSSM_TAP_S_IN],
+                        use_mma(c, batch, d.d_model) ? acc : nullptr, (int)ld_acc, t);
         tm->end(); ++nl;
 
         tm->begin(DFSSM_KCLASS_PROJ_IN);
         if (use_mma(c, batch, d.d_model)) {
-            const int rc = launch_proj_mma(c, L.in_sign, L.in_A, d.d_in_proj, d.d_model, batch);
+            const int rc = launch_proj_mma(c, L.in_sign, L.in_A, d.d_in_proj, d.d_model, batch, (pdl & 2) != 0);
             if (rc != DFSSM_OK) return rc;
         } else
-        k_proj<<<dim3(proj_grid(d.d_in_proj + d.r), (batch + PROJ_BT - 1) / PROJ_BT), PROJ_THREADS,
-                 proj_smem(d.d_model), st>>>(L.in_sign, L.in_A, d.d_in_proj, d.r, d.d_model, xq, xqp, ldq, qsum,
-                                             batch, acc, ld_acc, t);
+        DFSSM_LAUNCH_EX(pdl & 2, k_proj, dim3(proj_grid(d.d_in_proj + d.r), (batch + PROJ_BT - 1) / PROJ_BT), PROJ_THREADS, proj_smem(d.d_model), st,
+                        L.in_sign, L.in_A, d.d_in_proj, d.r, d.d_model, xq, xqp, ldq, qsum, batch, acc, ld_acc, t);
         tm->end(); ++nl;
         if (tp) {
             k_tap_copy_i32<<<dim3((d.d_in_proj + 255) / 256, batch), 256, 0, st>>>(acc, ld_acc, d.d_in_proj, tp,
@@ -395,20 +418,20 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
 #define DFSSM_FIN_ARGS L, d, acc, ld_acc, t, sx, conv, pos, fin, tp, v.tap_stride, v.tl
             switch (d.r) {
                 case 8:
-                    if (d.fmt & 2) k_fin4<2, true><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS);
-                    else k_fin4<2><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS);
+                    if (d.fmt & 2) DFSSM_LAUNCH_EX(pdl & 4, (k_fin4<2, true>), gf, FIN_THREADS, 0, st, DFSSM_FIN_ARGS);
+                    else DFSSM_LAUNCH_EX(pdl & 4, (k_fin4<2, false>), gf, FIN_THREADS, 0, st, DFSSM_FIN_ARGS);
                     break;
                 case 16:
-                    if (d.fmt & 2) k_fin4<4, true><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS);
-                    else k_fin4<4><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS);
+                    if (d.fmt & 2) DFSSM_LAUNCH_EX(pdl & 4, (k_fin4<4, true>), gf, FIN_THREADS, 0, st, DFSSM_FIN_ARGS);
+                    else DFSSM_LAUNCH_EX(pdl & 4, (k_fin4<4, false>), gf, FIN_THREADS, 0, st, DFSSM_FIN_ARGS);
                     break;
                 case 32:
-                    if (d.fmt & 2) k_fin4<8, true><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS);
-                    else k_fin4<8><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS);
+                    if (d.fmt & 2) DFSSM_LAUNCH_EX(pdl & 4, (k_fin4<8, true>), gf, FIN_THREADS, 0, st, DFSSM_FIN_ARGS);
+                    else DFSSM_LAUNCH_EX(pdl & 4, (k_fin4<8, false>), gf, FIN_THREADS, 0, st, DFSSM_FIN_ARGS);
                     break;
                 case 64:
-                    if (d.fmt & 2) k_fin4<16, true><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS);
-                    else k_fin4<16><<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS);
+                    if (d.fmt & 2) DFSSM_LAUNCH_EX(pdl & 4, (k_fin4<16, true>), gf, FIN_THREADS, 0, st, DFSSM_FIN_ARGS);
+                    else DFSSM_LAUNCH_EX(pdl & 4, (k_fin4<16, false>), gf, FIN_THREADS, 0, st, DFSSM_FIN_ARGS);
                     break;
                 default: k_fin<<<gf, FIN_THREADS, 0, st>>>(DFSSM_FIN_ARGS); break;
             }
@@ -419,8 +442,8 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
             const dim3 g32(d.headdim / 32, d.nheads, batch), g16(d.headdim / 16, d.nheads, batch);
             const size_t sm = 2 * (size_t)d.d_state * sizeof(float);
 #define DFSSM_SSM_GO(PB_, DS_, G_)                                                                                          \
-    if (st16) k_ssm_stream<PB_, DS_, __half><<<G_, SSM_THREADS, sm, st>>>(L, d, fin, ssm_h, g, tp, v.tap_stride, v.tl);    \
-    else k_ssm_stream<PB_, DS_, float><<<G_, SSM_THREADS, sm, st>>>(L, d, fin, ssm, g, tp, v.tap_stride, v.tl)
+    if (st16) DFSSM_LAUNCH_EX(pdl & 8, (k_ssm_stream<PB_, DS_, __half>), G_, SSM_THREADS, sm, st, L, d, fin, ssm_h, g, tp, v.tap_stride, v.tl);    \
+    else DFSSM_LAUNCH_EX(pdl & 8, (k_ssm_stream<PB_, DS_, float>), G_, SSM_THREADS, sm, st, L, d, fin, ssm, g, tp, v.tap_stride, v.tl)
             if (d.headdim % 32 == 0) {
                 if (d.d_state == 128) { DFSSM_SSM_GO(32, 128, g32); }
                 else if (d.d_state == 64) { DFSSM_SSM_GO(32, 64, g32); }
@@ -432,19 +455,18 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         tm->end(); ++nl;
 
         tm->begin(DFSSM_KCLASS_NORMQUANT);
-        k_normquant<<<batch, NQ_THREADS, 0, st>>>(g, d.d_inner, L.gnorm_w, d.d_inner, d.eps, xq, xqp, ldq, sx, qsum,
-                                                  tp, v.tap_stride, v.tl.off[DFSSM_TAP_GQ], v.tl.off[DFSSM_TAP_S_G],
-                                                  use_mma(c, batch, d.d_inner) ? acc : nullptr, (int)ld_acc, t);
+        DFSSM_LAUNCH_EX(pdl & 16, k_normquant, batch, NQ_THREADS, 0, st, g, d.d_inner, L.gnorm_w, d.d_inner, d.eps, xq, xqp, ldq, sx, qsum,
+                        tp, v.tap_stride, v.tl.off[DFSSM_TAP_GQ], v.tl.off[DFSSM_TAP_S_G],
+                        use_mma(c, batch, d.d_inner) ? acc : nullptr, (int)ld_acc, t);
         tm->end(); ++nl;
 
         tm->begin(DFSSM_KCLASS_PROJ_OUT);
         if (use_mma(c, batch, d.d_inner)) {
-            const int rc = launch_proj_mma(c, L.out_sign, L.out_A, d.d_model, d.d_inner, batch);
+            const int rc = launch_proj_mma(c, L.out_sign, L.out_A, d.d_model, d.d_inner, batch, (pdl & 32) != 0);
             if (rc != DFSSM_OK) return rc;
         } else
-        k_proj<<<dim3(proj_grid(d.d_model + d.r), (batch + PROJ_BT - 1) / PROJ_BT), PROJ_THREADS,
-                 proj_smem(d.d_inner), st>>>(L.out_sign, L.out_A, d.d_model, d.r, d.d_inner, xq, xqp, ldq, qsum,
-                                             batch, acc, ld_acc, t);
+        DFSSM_LAUNCH_EX(pdl & 32, k_proj, dim3(proj_grid(d.d_model + d.r), (batch + PROJ_BT - 1) / PROJ_BT), PROJ_THREADS, proj_smem(d.d_inner), st,
+                        L.out_sign, L.out_A, d.d_model, d.r, d.d_inner, xq, xqp, ldq, qsum, batch, acc, ld_acc, t);
         tm->end(); ++nl;
         if (tp) {
             k_tap_copy_i32<<<dim3((d.d_model + 255) / 256, batch), 256, 0, st>>>(acc, ld_acc, d.d_model, tp,
@@ -454,7 +476,7 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         }
 
         tm->begin(DFSSM_KCLASS_EPI_OUT);
-        launch_epi_out(L, d, batch, acc, ld_acc, t, sx, u, tp, v.tap_stride, v.tl.off[DFSSM_TAP_HIDDEN], st);
+        launch_epi_out(L, d, batch, acc, ld_acc, t, sx, u, tp, v.tap_stride, v.tl.off[DFSSM_TAP_HIDDEN], st, (pdl & 64) != 0);
         tm->end(); ++nl;
     }
 
@@ -677,7 +699,7 @@ int prefill_chunk(dfssm_ctx* c, const int32_t* tokens_dev, int T, int seq)
             int ks = (148 * MMA_CTAS_PER_SM) / (mt * nt);
             if (ks < 1) ks = 1;
             if (ks > nchunk) ks = nchunk;
-            DFSSM_MMA_LAUNCH(d.fmt, dim3(mt, nt, ks), st, sign, A, rows, d.r, K, xq, ldq, T, acc, ld_acc, t, err, nullptr, nullptr, nullptr);
+            DFSSM_MMA_LAUNCH(false, d.fmt, dim3(mt, nt, ks), st, sign, A, rows, d.r, K, xq, ldq, T, acc, ld_acc, t, err, nullptr, nullptr, nullptr);
         } else {
             k_proj<<<dim3(proj_grid(rows + d.r), (T + PROJ_BT - 1) / PROJ_BT), PROJ_THREADS, proj_smem(K), st>>>(sign, A, rows, d.r, K, xq, xqp, ldq, qsum,
                                                                                                               T, acc, ld_acc, t);

@@ -10,6 +10,17 @@
 
 namespace dfssm {
 
+// Programmatic dependent launch (launch_pdl in dfssm_api.cu): wait until the kernel in front of this one in the chain has completed
+// and its writes are visible, then let the kernel behind this one be scheduled.  Everything a kernel reads from or writes to
+// buffers of the chain comes after this call; loads of weights (and of the SSM state, which only the same layer's kernel of the
+// step before wrote) may come before it.  A no-op for a launch without the attribute.
+__device__ __forceinline__ void pdl_wait()
+{
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");      // behind the wait: at most two kernels of the chain overlap
+}
+
+
 // ---- device-side view of one layer's weights (pointers into the arena copy of the blob) ----
 struct LayerW {
     const float* norm_w;
@@ -70,6 +81,7 @@ k_normquant(const float* __restrict__ v, int ldv, const float* __restrict__ w, i
             uint32_t tap_q_off, uint32_t tap_s_off,
             int32_t* __restrict__ zero_acc = nullptr, int ld_acc = 0, int32_t* __restrict__ zero_t = nullptr)
 {
+    pdl_wait();
     // the split-K tensor-core projection that follows adds into acc / t: this sequence's rows are zeroed here (their last
     // reader ran before this kernel) instead of by two memset nodes per projection
     if (zero_acc) {
@@ -154,6 +166,7 @@ k_proj(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int rows
        const int32_t* __restrict__ qsum, int batch, int32_t* __restrict__ acc, int ld_acc,
        int32_t* __restrict__ t)
 {
+    pdl_wait();
     extern __shared__ __align__(16) uint8_t smem[];
     const int b0 = blockIdx.y * PROJ_BT;
     const int nb = min(PROJ_BT, batch - b0);
@@ -285,6 +298,7 @@ k_fin(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int3
       const float* __restrict__ s_x, float* __restrict__ conv_ring, const int32_t* __restrict__ pos,
       float* __restrict__ fin, uint8_t* __restrict__ taps, uint32_t tap_stride, TapLayout tl)
 {
+    pdl_wait();
     __shared__ float v_sh[64];
     const int b = blockIdx.y, tid = threadIdx.x;
     const int gs = dm.ngroups * dm.d_state, d_in_proj = 2 * dm.d_inner + 2 * gs + dm.nheads;
@@ -386,6 +400,7 @@ k_fin4(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int
        const float* __restrict__ s_x, float* __restrict__ conv_ring, const int32_t* __restrict__ pos,
        float* __restrict__ fin, uint8_t* __restrict__ taps, uint32_t tap_stride, TapLayout tl)
 {
+    pdl_wait();
     const int b = blockIdx.y, tid = threadIdx.x;
     const int gs = dm.ngroups * dm.d_state, d_in_proj = 2 * dm.d_inner + 2 * gs + dm.nheads;
     const int base = blockIdx.x * FIN_THREADS;
@@ -472,6 +487,7 @@ k_ssm_stream(LayerW L, Dims dm, const float* __restrict__ fin, ST* __restrict__ 
         const int n4 = l16 + LANES * j;
         if (DS || n4 < ds / 4) hpre[j] = state_ld4(Hr + 4 * n4);
     }
+    pdl_wait();                                    // the state was requested above: only this layer's kernel of the step before wrote it
     const float xv = src[dm.d_inner + ch];
     const float dtv = src[d_in_proj - dm.nheads + h], dA = src[d_in_proj + h];
     const float sz = src[ch];                      // silu(z) from k_fin
@@ -542,6 +558,7 @@ k_epi_out(LayerW L, int d_model, int r, const int32_t* __restrict__ acc, int ld_
           const int32_t* __restrict__ t, const float* __restrict__ s_g, float* __restrict__ u,
           uint8_t* __restrict__ taps, uint32_t tap_stride, uint32_t tap_hidden_off)
 {
+    pdl_wait();
     __shared__ float v_sh[64];
     const int b = blockIdx.y;
     if (threadIdx.x < r) v_sh[threadIdx.x] = fmul(L.out_a_s[threadIdx.x], (float)t[(size_t)b * T_STRIDE + threadIdx.x]);
@@ -562,6 +579,7 @@ k_epi_out4(LayerW L, int d_model, const int32_t* __restrict__ acc, int ld_acc,
            const int32_t* __restrict__ t, const float* __restrict__ s_g, float* __restrict__ u,
            uint8_t* __restrict__ taps, uint32_t tap_stride, uint32_t tap_hidden_off)
 {
+    pdl_wait();
     const int b = blockIdx.y, base = blockIdx.x * FIN_THREADS, i = base + threadIdx.x;
     const bool own = i < d_model;
     const int il = own ? i : 0;

@@ -146,6 +146,7 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
         x_next[0] = (b_valid && kx < K) ? *(const uint4*)(x_row + kc * KC) : make_uint4(0, 0, 0, 0);
         x_next[1] = (b_valid && kx + 128 < K) ? *(const uint4*)(x_row + kc * KC + 128) : make_uint4(0, 0, 0, 0);
     };
+    pdl_wait();          // TMEM allocation, barrier initialisation and the index arithmetic above run under the kernel in front
     if (kc0 < kc1) request(kc0);
     for (int kc = kc0; kc < kc1; ++kc) {
         const int it = kc - kc0, s = it % STAGES, use = it / STAGES;
