@@ -674,6 +674,7 @@ bool prefill_supported(const Dims& d)
 int prefill_chunk(dfssm_ctx* c, const int32_t* tokens_dev, int T, int seq)
 {
     dfssm_ctx* ctx = c;
+    static const bool pdl = !(getenv("DFSSM_PDL_MASK") && atoi(getenv("DFSSM_PDL_MASK")) == 0);      // programmatic dependent launch, see enqueue_step
     const Dims& d = c->dm;
     const Carve& v = c->cv;
     cudaStream_t st = c->stream;
@@ -699,9 +700,9 @@ int prefill_chunk(dfssm_ctx* c, const int32_t* tokens_dev, int T, int seq)
             int ks = (148 * MMA_CTAS_PER_SM) / (mt * nt);
             if (ks < 1) ks = 1;
             if (ks > nchunk) ks = nchunk;
-            DFSSM_MMA_LAUNCH(false, d.fmt, dim3(mt, nt, ks), st, sign, A, rows, d.r, K, xq, ldq, T, acc, ld_acc, t, err, nullptr, nullptr, nullptr);
+            DFSSM_MMA_LAUNCH(pdl, d.fmt, dim3(mt, nt, ks), st, sign, A, rows, d.r, K, xq, ldq, T, acc, ld_acc, t, err, nullptr, nullptr, nullptr);
         } else {
-            k_proj<<<dim3(proj_grid(rows + d.r), (T + PROJ_BT - 1) / PROJ_BT), PROJ_THREADS, proj_smem(K), st>>>(sign, A, rows, d.r, K, xq, xqp, ldq, qsum,
+            DFSSM_LAUNCH_EX(pdl, k_proj, dim3(proj_grid(rows + d.r), (T + PROJ_BT - 1) / PROJ_BT), PROJ_THREADS, proj_smem(K), st, sign, A, rows, d.r, K, xq, xqp, ldq, qsum,
                                                                                                               T, acc, ld_acc, t);
         }
     };
@@ -711,42 +712,42 @@ int prefill_chunk(dfssm_ctx* c, const int32_t* tokens_dev, int T, int seq)
         const LayerW& L = c->layers[l];
         uint8_t* ssm_b = c->arena + v.ssm + ((size_t)l * B + seq) * v.ssm_elems * v.ssm_esize;
         float* ring = at<float>(c, v.conv) + ((size_t)l * B + seq) * (size_t)d.conv_dim * 4;
-        k_normquant<<<T, NQ_THREADS, 0, st>>>(u, d.d_model, L.norm_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum, nullptr, 0, 0, 0,
+        DFSSM_LAUNCH_EX(pdl, k_normquant, T, NQ_THREADS, 0, st, u, d.d_model, L.norm_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum, nullptr, 0, 0, 0,
                                               use_mma(c, T, d.d_model) ? acc : nullptr, ld_acc, t);
         proj(L.in_sign, L.in_A, d.d_in_proj, d.d_model);
         {
             const dim3 g4((d.d_in_proj + FIN_THREADS - 1) / FIN_THREADS, T);
             switch (d.r) {
                 case 8:
-                    if (d.fmt & 2) prefill::k_pf_epi4<2, true><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
-                    else prefill::k_pf_epi4<2><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
+                    if (d.fmt & 2) DFSSM_LAUNCH_EX(pdl, (prefill::k_pf_epi4<2, true>), g4, FIN_THREADS, 0, st, L, d, acc, ld_acc, t, sx, zx, ld_acc);
+                    else DFSSM_LAUNCH_EX(pdl, (prefill::k_pf_epi4<2, false>), g4, FIN_THREADS, 0, st, L, d, acc, ld_acc, t, sx, zx, ld_acc);
                     break;
                 case 16:
-                    if (d.fmt & 2) prefill::k_pf_epi4<4, true><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
-                    else prefill::k_pf_epi4<4><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
+                    if (d.fmt & 2) DFSSM_LAUNCH_EX(pdl, (prefill::k_pf_epi4<4, true>), g4, FIN_THREADS, 0, st, L, d, acc, ld_acc, t, sx, zx, ld_acc);
+                    else DFSSM_LAUNCH_EX(pdl, (prefill::k_pf_epi4<4, false>), g4, FIN_THREADS, 0, st, L, d, acc, ld_acc, t, sx, zx, ld_acc);
                     break;
                 case 32:
-                    if (d.fmt & 2) prefill::k_pf_epi4<8, true><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
-                    else prefill::k_pf_epi4<8><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
+                    if (d.fmt & 2) DFSSM_LAUNCH_EX(pdl, (prefill::k_pf_epi4<8, true>), g4, FIN_THREADS, 0, st, L, d, acc, ld_acc, t, sx, zx, ld_acc);
+                    else DFSSM_LAUNCH_EX(pdl, (prefill::k_pf_epi4<8, false>), g4, FIN_THREADS, 0, st, L, d, acc, ld_acc, t, sx, zx, ld_acc);
                     break;
                 case 64:
-                    if (d.fmt & 2) prefill::k_pf_epi4<16, true><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
-                    else prefill::k_pf_epi4<16><<<g4, FIN_THREADS, 0, st>>>(L, d, acc, ld_acc, t, sx, zx, ld_acc);
+                    if (d.fmt & 2) DFSSM_LAUNCH_EX(pdl, (prefill::k_pf_epi4<16, true>), g4, FIN_THREADS, 0, st, L, d, acc, ld_acc, t, sx, zx, ld_acc);
+                    else DFSSM_LAUNCH_EX(pdl, (prefill::k_pf_epi4<16, false>), g4, FIN_THREADS, 0, st, L, d, acc, ld_acc, t, sx, zx, ld_acc);
                     break;
                 default:
                     prefill::k_pf_epi<<<dim3((d.d_in_proj + prefill::EPI_T - 1) / prefill::EPI_T, T), prefill::EPI_T, 0, st>>>(L, d, acc, ld_acc, t, sx, zx,
                                                                                                                         ld_acc);
             }
         }
-        prefill::k_pf_conv<<<dim3((d.conv_dim + d.nheads + prefill::CONV_T - 1) / prefill::CONV_T, T), prefill::CONV_T, 0, st>>>(L, d, zx, ld_acc, T, ring, pos, xbc,
+        DFSSM_LAUNCH_EX(pdl, prefill::k_pf_conv, dim3((d.conv_dim + d.nheads + prefill::CONV_T - 1) / prefill::CONV_T, T), prefill::CONV_T, 0, st, L, d, zx, ld_acc, T, ring, pos, xbc,
                                                                                                                                dtv);
-        prefill::k_pf_ring<<<(d.conv_dim + 255) / 256, 256, 0, st>>>(d, zx, ld_acc, T, ring, pos);
+        DFSSM_LAUNCH_EX(pdl, prefill::k_pf_ring, (d.conv_dim + 255) / 256, 256, 0, st, d, zx, ld_acc, T, ring, pos);
         {
             const dim3 gr(d.nheads * (d.headdim / prefill::SEQ_PB));
             const size_t sm = prefill::seq_smem(d);
 #define DFSSM_PF_SSM(N_)                                                                                                             \
-    if (v.ssm_esize == 2) prefill::k_pf_ssm<N_, __half><<<gr, prefill::SEQ_T, sm, st>>>(L, d, zx, ld_acc, xbc, dtv, T, (__half*)ssm_b, g); \
-    else prefill::k_pf_ssm<N_, float><<<gr, prefill::SEQ_T, sm, st>>>(L, d, zx, ld_acc, xbc, dtv, T, (float*)ssm_b, g)
+    if (v.ssm_esize == 2) DFSSM_LAUNCH_EX(pdl, (prefill::k_pf_ssm<N_, __half>), gr, prefill::SEQ_T, sm, st, L, d, zx, ld_acc, xbc, dtv, T, (__half*)ssm_b, g); \
+    else DFSSM_LAUNCH_EX(pdl, (prefill::k_pf_ssm<N_, float>), gr, prefill::SEQ_T, sm, st, L, d, zx, ld_acc, xbc, dtv, T, (float*)ssm_b, g)
             switch (d.d_state / prefill::SEQ_LANES) {
                 case 1: DFSSM_PF_SSM(1); break;
                 case 2: DFSSM_PF_SSM(2); break;
@@ -756,10 +757,10 @@ int prefill_chunk(dfssm_ctx* c, const int32_t* tokens_dev, int T, int seq)
             }
 #undef DFSSM_PF_SSM
         }
-        k_normquant<<<T, NQ_THREADS, 0, st>>>(g, d.d_inner, L.gnorm_w, d.d_inner, d.eps, xq, xqp, ldq, sx, qsum, nullptr, 0, 0, 0,
+        DFSSM_LAUNCH_EX(pdl, k_normquant, T, NQ_THREADS, 0, st, g, d.d_inner, L.gnorm_w, d.d_inner, d.eps, xq, xqp, ldq, sx, qsum, nullptr, 0, 0, 0,
                                               use_mma(c, T, d.d_inner) ? acc : nullptr, ld_acc, t);
         proj(L.out_sign, L.out_A, d.d_model, d.d_inner);
-        launch_epi_out(L, d, T, acc, ld_acc, t, sx, u, nullptr, 0, 0, st);
+        launch_epi_out(L, d, T, acc, ld_acc, t, sx, u, nullptr, 0, 0, st, pdl);
     }
     // the last position: hidden state, logits and greedy token of the sequence; the conv ring position advances by T
     const float* u_last = u + (size_t)(T - 1) * d.d_model;

@@ -19,6 +19,7 @@ __global__ void __launch_bounds__(EPI_T)
 k_pf_epi(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int32_t* __restrict__ t, const float* __restrict__ s_x,
          float* __restrict__ zx, int ldz /* row stride of zx: a multiple of 4 floats */)
 {
+    pdl_wait();
     __shared__ float v_sh[64];
     const int p = blockIdx.y;
     if (threadIdx.x < dm.r) v_sh[threadIdx.x] = fmul(L.in_a_s[threadIdx.x], (float)t[(size_t)p * T_STRIDE + threadIdx.x]);
@@ -34,6 +35,7 @@ __global__ void __launch_bounds__(FIN_THREADS)
 k_pf_epi4(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int32_t* __restrict__ t, const float* __restrict__ s_x,
           float* __restrict__ zx, int ldz)
 {
+    pdl_wait();
     const int p = blockIdx.y, base = blockIdx.x * FIN_THREADS, i = base + threadIdx.x;
     const bool own = i < dm.d_in_proj;
     const int il = own ? i : 0;
@@ -50,6 +52,7 @@ __global__ void __launch_bounds__(CONV_T)
 k_pf_conv(LayerW L, Dims dm, const float* __restrict__ zx, int ldz, int T, const float* __restrict__ ring /* [conv_dim][4] of the sequence */,
           const int32_t* __restrict__ pos, float* __restrict__ xbc /* [T][conv_dim] */, float* __restrict__ dt /* [T][nheads] */)
 {
+    pdl_wait();
     const int p = blockIdx.y;
     const int c = blockIdx.x * CONV_T + threadIdx.x;
     const int ps = pos[0] & 3;
@@ -77,6 +80,7 @@ k_pf_conv(LayerW L, Dims dm, const float* __restrict__ zx, int ldz, int T, const
 // the conv ring after the chunk: the last min(T, 4) raw samples go to their slots (a separate launch: k_pf_conv reads the ring)
 __global__ void k_pf_ring(Dims dm, const float* __restrict__ zx, int ldz, int T, float* __restrict__ ring, const int32_t* __restrict__ pos)
 {
+    pdl_wait();
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= dm.conv_dim) return;
     const int ps = pos[0] & 3;
@@ -129,6 +133,7 @@ k_pf_ssm(LayerW L, Dims dm, const float* __restrict__ zx, int ldz, const float* 
     constexpr int nper = NPER;                            // contiguous state values of this lane
 #pragma unroll
     for (int k = 0; k < NPER; ++k) hreg[k] = st_get(Hr + ln * nper + k);
+    pdl_wait();                                           // (the state rows above were written by this kernel of the chunk before, or by a reset)
     const float An = -sp_expf(L.A_log[h]);
     const float Dh = L.D[h];
 
