@@ -390,7 +390,7 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         float* conv = at<float>(c, v.conv) + (size_t)l * B * (size_t)d.conv_dim * 4;
 
         tm->begin(DFSSM_KCLASS_NORMQUANT);
-        DFSSM_LAUNCH_EX((pdl & 1) && l > 0, k_normquant, batch, NQ_THREADS, 0, st, u, d.d_model, L.norm_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum,
+        DFSSM_LAUNCH_EX(pdl & 1, k_normquant, batch, NQ_THREADS, 0, st, u, d.d_model, L.norm_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum,
                         tp, v.tap_stride, v.tl.off[DFSSM_TAP_XQ_IN], v.tl.off[DFSSM_TAP_S_IN],
                         use_mma(c, batch, d.d_model) ? acc : nullptr, (int)ld_acc, t);
         tm->end(); ++nl;
@@ -481,25 +481,25 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
     }
 
     tm->begin(DFSSM_KCLASS_NORMQUANT);
-    k_normquant<<<batch, NQ_THREADS, 0, st>>>(u, d.d_model, c->normf_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum,
-                                              nullptr, 0, 0, 0);
+    DFSSM_LAUNCH_EX(pdl & 1, k_normquant, batch, NQ_THREADS, 0, st, u, d.d_model, c->normf_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum,
+                    nullptr, 0, 0, 0, nullptr, 0, nullptr);
     tm->end(); ++nl;
 
     tm->begin(DFSSM_KCLASS_LMHEAD);
     if (use_mma(c, batch, d.d_model)) {
-        mma::k_proj_mma<0><<<dim3((d.vocab + mma::TM - 1) / mma::TM, (batch + mma::TN - 1) / mma::TN, 1), mma::THREADS, mma::SMEM_BYTES, st>>>(
-            nullptr, c->emb, 0, d.vocab, d.d_model, xq, ldq, batch, nullptr, 0, nullptr, err, logits, sx, c->emb_s);
+        DFSSM_LAUNCH_EX(pdl & 2, mma::k_proj_mma<0>, dim3((d.vocab + mma::TM - 1) / mma::TM, (batch + mma::TN - 1) / mma::TN, 1), mma::THREADS, mma::SMEM_BYTES, st,
+                        nullptr, c->emb, 0, d.vocab, d.d_model, xq, ldq, batch, nullptr, 0, nullptr, err, logits, sx, c->emb_s);
     } else {
         const int per = LM_THREADS / 32;
         int gx = (d.vocab + per - 1) / per;
         if (gx > 148 * 16) gx = 148 * 16;
-        k_lmhead<<<dim3(gx, (batch + PROJ_BT - 1) / PROJ_BT), LM_THREADS, lm_smem(d.d_model), st>>>(
-            c->emb, c->emb_s, d.vocab, d.d_model, xq, ldq, sx, batch, logits);
+        DFSSM_LAUNCH_EX(pdl & 2, k_lmhead, dim3(gx, (batch + PROJ_BT - 1) / PROJ_BT), LM_THREADS, lm_smem(d.d_model), st,
+                        c->emb, c->emb_s, d.vocab, d.d_model, xq, ldq, sx, batch, logits);
     }
     tm->end(); ++nl;
 
     tm->begin(DFSSM_KCLASS_ARGMAX);
-    k_argmax<<<batch, AM_THREADS, 0, st>>>(logits, d.vocab, next, tokens, pos);
+    DFSSM_LAUNCH_EX(pdl & 2, k_argmax, batch, AM_THREADS, 0, st, logits, d.vocab, next, tokens, pos, 1);
     tm->end(); ++nl;
 
     if (n_launch) *n_launch = nl;

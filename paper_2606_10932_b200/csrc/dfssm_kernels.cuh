@@ -614,6 +614,7 @@ k_lmhead(const int8_t* __restrict__ E, const float* __restrict__ e_s, int vocab,
          const int8_t* __restrict__ xq, int ldq, const float* __restrict__ s_h, int batch,
          float* __restrict__ logits)
 {
+    pdl_wait();
     extern __shared__ __align__(16) uint8_t smem[];
     const int b0 = blockIdx.y * PROJ_BT;
     const int nb = min(PROJ_BT, batch - b0);
@@ -662,6 +663,7 @@ __global__ void __launch_bounds__(AM_THREADS)
 k_argmax(const float* __restrict__ logits, int vocab, int32_t* __restrict__ next, int32_t* __restrict__ tok,
          int32_t* __restrict__ pos, int pos_inc = 1)
 {
+    pdl_wait();
     __shared__ float sv[AM_THREADS / 32];
     __shared__ int si[AM_THREADS / 32];
     const int b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
