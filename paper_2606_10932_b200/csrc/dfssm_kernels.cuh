@@ -400,27 +400,28 @@ k_fin4(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int
        const float* __restrict__ s_x, float* __restrict__ conv_ring, const int32_t* __restrict__ pos,
        float* __restrict__ fin, uint8_t* __restrict__ taps, uint32_t tap_stride, TapLayout tl)
 {
-    pdl_wait();
     const int b = blockIdx.y, tid = threadIdx.x;
     const int gs = dm.ngroups * dm.d_state, d_in_proj = 2 * dm.d_inner + 2 * gs + dm.nheads;
     const int base = blockIdx.x * FIN_THREADS;
     const int row = base + tid;                                  // the row this lane finishes
     const bool own = row < d_in_proj;
 
-    // requested early: everything the row epilogue needs
+    // requested early: everything the row epilogue needs - the weights before pdl_wait (they do not depend on the kernel in front)
     const int rl = own ? row : 0;
-    const int acc_i = acc[(size_t)b * ld_acc + rl];
-    const float rs = __half2float(L.in_row_scale[rl]), bs = L.in_b_s[rl], sx = s_x[b];
+    const float rs = __half2float(L.in_row_scale[rl]), bs = L.in_b_s[rl];
     const bool is_conv = own && row >= dm.d_inner && row < d_in_proj - dm.nheads;
     const int c = is_conv ? row - dm.d_inner : 0;                // conv channel
     float* ring = conv_ring + ((size_t)b * dm.conv_dim + c) * 4;
     float4 rg = make_float4(0.f, 0.f, 0.f, 0.f), cw = rg;
     float cb = 0.f;
     if (is_conv) {
-        rg = *(const float4*)ring;
         cw = *(const float4*)(L.conv_w + 4 * (size_t)c);
         cb = L.conv_b[c];
     }
+    pdl_wait();
+    const int acc_i = acc[(size_t)b * ld_acc + rl];
+    const float sx = s_x[b];
+    if (is_conv) rg = *(const float4*)ring;
 
     const double lo = lora_up4<JW, I4>(L.in_B, L.in_a_s, t + (size_t)b * T_STRIDE, base, d_in_proj);
     if (!own) return;
@@ -579,12 +580,13 @@ k_epi_out4(LayerW L, int d_model, const int32_t* __restrict__ acc, int ld_acc,
            const int32_t* __restrict__ t, const float* __restrict__ s_g, float* __restrict__ u,
            uint8_t* __restrict__ taps, uint32_t tap_stride, uint32_t tap_hidden_off)
 {
-    pdl_wait();
     const int b = blockIdx.y, base = blockIdx.x * FIN_THREADS, i = base + threadIdx.x;
     const bool own = i < d_model;
     const int il = own ? i : 0;
+    const float rs = __half2float(L.out_row_scale[il]), bs = L.out_b_s[il];      // weights: before pdl_wait
+    pdl_wait();
     const int acc_i = acc[(size_t)b * ld_acc + il];
-    const float rs = __half2float(L.out_row_scale[il]), bs = L.out_b_s[il], sg = s_g[b];
+    const float sg = s_g[b];
     const float u0 = u[(size_t)b * d_model + il];
     const double lo = lora_up4<JW, I4>(L.out_B, L.out_a_s, t + (size_t)b * T_STRIDE, base, d_model);
     if (!own) return;
