@@ -354,37 +354,45 @@ template <> struct BytesT<16> { using T = uint4; };
 // Lane `sub` of a group of four holds v_j for its JW values of j and reads its JW bytes of a row with one load; the group
 // walks through its four rows, and the tree of the sum is (p0 + p1) + (p2 + p3).  No shared memory, no barrier.
 // I4: the matrix holds int4 pairs (format variant, R25): a lane's JW values are JW / 2 bytes, element 2i = low nibble.
-template <int JW, bool I4 = false>
-__device__ __forceinline__ double lora_up4(const int8_t* __restrict__ B, const float* __restrict__ a_s,
-                                           const int32_t* __restrict__ t_row, int base, int n_rows)
+// Two halves, so that the weight half can run before pdl_wait(): lora_load4 reads the lane's bytes of its group's four rows and
+// its JW scales a_s; lora_sum4 makes v from the (dependent) t and sums.
+template <int JW, bool I4> struct LoraRegs {
+    typename BytesT<I4 ? JW / 2 : JW>::T w[4];
+    float as[JW];
+};
+template <int JW, bool I4>
+__device__ __forceinline__ void lora_load4(const int8_t* __restrict__ B, const float* __restrict__ a_s, int base, int n_rows, LoraRegs<JW, I4>& R)
 {
-    constexpr int R = 4 * JW;
+    constexpr int RK = 4 * JW;
     const int q = threadIdx.x >> 2, sub = threadIdx.x & 3;
+    using WT = typename BytesT<I4 ? JW / 2 : JW>::T;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int rk = min(base + q * 4 + k, n_rows - 1);          // rows beyond the end are summed and never used
+        R.w[k] = *(const WT*)((const uint8_t*)B + ((size_t)rk * RK + sub * JW) / (I4 ? 2 : 1));
+    }
+#pragma unroll
+    for (int i = 0; i < JW; ++i) R.as[i] = a_s[sub * JW + i];
+}
+template <int JW, bool I4>
+__device__ __forceinline__ double lora_sum4(const LoraRegs<JW, I4>& R, const int32_t* __restrict__ t_row)
+{
+    const int sub = threadIdx.x & 3;
     double v[JW];
 #pragma unroll
-    for (int i = 0; i < JW; ++i) {
-        const int j = sub * JW + i;
-        v[i] = (double)fmul(a_s[j], (float)t_row[j]);
-    }
+    for (int i = 0; i < JW; ++i) v[i] = (double)fmul(R.as[i], (float)t_row[sub * JW + i]);
     double part[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        const int rk = base + q * 4 + k;
         double lo = 0.0;
-        if (rk < n_rows) {
+        const uint8_t* wb = (const uint8_t*)&R.w[k];
+#pragma unroll
+        for (int i = 0; i < JW; ++i) {
             if constexpr (I4) {
-                const typename BytesT<JW / 2>::T w = *(const typename BytesT<JW / 2>::T*)((const uint8_t*)B + ((size_t)rk * R + sub * JW) / 2);
-                const uint8_t* wb = (const uint8_t*)&w;
-#pragma unroll
-                for (int i = 0; i < JW; ++i) {
-                    const int nib = (wb[i >> 1] >> (4 * (i & 1))) & 0xf;
-                    lo = __fma_rn((double)((nib ^ 8) - 8), v[i], lo);
-                }
+                const int nib = (wb[i >> 1] >> (4 * (i & 1))) & 0xf;
+                lo = __fma_rn((double)((nib ^ 8) - 8), v[i], lo);
             } else {
-                const typename BytesT<JW>::T w = *(const typename BytesT<JW>::T*)(B + (size_t)rk * R + sub * JW);
-                const uint8_t* wb = (const uint8_t*)&w;
-#pragma unroll
-                for (int i = 0; i < JW; ++i) lo = __fma_rn((double)(int)(int8_t)wb[i], v[i], lo);
+                lo = __fma_rn((double)(int)(int8_t)wb[i], v[i], lo);
             }
         }
         lo += __shfl_xor_sync(0xffffffffu, lo, 1);
@@ -392,6 +400,14 @@ __device__ __forceinline__ double lora_up4(const int8_t* __restrict__ B, const f
         part[k] = lo;
     }
     return sub == 0 ? part[0] : sub == 1 ? part[1] : sub == 2 ? part[2] : part[3];
+}
+template <int JW, bool I4 = false>
+__device__ __forceinline__ double lora_up4(const int8_t* __restrict__ B, const float* __restrict__ a_s,
+                                           const int32_t* __restrict__ t_row, int base, int n_rows)
+{
+    LoraRegs<JW, I4> R;
+    lora_load4<JW, I4>(B, a_s, base, n_rows, R);
+    return lora_sum4<JW, I4>(R, t_row);
 }
 
 template <int JW, bool I4 = false>
@@ -418,12 +434,14 @@ k_fin4(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int
         cw = *(const float4*)(L.conv_w + 4 * (size_t)c);
         cb = L.conv_b[c];
     }
+    LoraRegs<JW, I4> lr;
+    lora_load4<JW, I4>(L.in_B, L.in_a_s, base, d_in_proj, lr);
     pdl_wait();
     const int acc_i = acc[(size_t)b * ld_acc + rl];
     const float sx = s_x[b];
     if (is_conv) rg = *(const float4*)ring;
 
-    const double lo = lora_up4<JW, I4>(L.in_B, L.in_a_s, t + (size_t)b * T_STRIDE, base, d_in_proj);
+    const double lo = lora_sum4<JW, I4>(lr, t + (size_t)b * T_STRIDE);
     if (!own) return;
     uint8_t* tp = taps ? taps + (size_t)b * tap_stride : nullptr;
     float* out = fin + (size_t)b * (d_in_proj + dm.nheads);
@@ -584,11 +602,13 @@ k_epi_out4(LayerW L, int d_model, const int32_t* __restrict__ acc, int ld_acc,
     const bool own = i < d_model;
     const int il = own ? i : 0;
     const float rs = __half2float(L.out_row_scale[il]), bs = L.out_b_s[il];      // weights: before pdl_wait
+    LoraRegs<JW, I4> lr;
+    lora_load4<JW, I4>(L.out_B, L.out_a_s, base, d_model, lr);
     pdl_wait();
     const int acc_i = acc[(size_t)b * ld_acc + il];
     const float sg = s_g[b];
     const float u0 = u[(size_t)b * d_model + il];
-    const double lo = lora_up4<JW, I4>(L.out_B, L.out_a_s, t + (size_t)b * T_STRIDE, base, d_model);
+    const double lo = lora_sum4<JW, I4>(lr, t + (size_t)b * T_STRIDE);
     if (!own) return;
     const float o = fmul(sg, fadd(fmul(rs, (float)acc_i), fmul(bs, (float)lo)));
     const float un = fadd(u0, o);
