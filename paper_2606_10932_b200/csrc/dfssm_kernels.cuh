@@ -81,6 +81,17 @@ k_normquant(const float* __restrict__ v, int ldv, const float* __restrict__ w, i
             uint32_t tap_q_off, uint32_t tap_s_off,
             int32_t* __restrict__ zero_acc = nullptr, int ld_acc = 0, int32_t* __restrict__ zero_t = nullptr)
 {
+    // up to NQ_R elements per thread stay in registers between the two passes; their norm weights are read before pdl_wait
+    constexpr int NQ_R = 8;
+    const bool in_regs = d <= NQ_R * NQ_THREADS;
+    float wv[NQ_R], tv[NQ_R];
+    if (in_regs) {
+#pragma unroll
+        for (int i = 0; i < NQ_R; ++i) {
+            const int k = threadIdx.x + i * NQ_THREADS;
+            wv[i] = k < d ? w[k] : 0.0f;
+        }
+    }
     pdl_wait();
     // the split-K tensor-core projection that follows adds into acc / t: this sequence's rows are zeroed here (their last
     // reader ran before this kernel) instead of by two memset nodes per projection
@@ -98,10 +109,21 @@ k_normquant(const float* __restrict__ v, int ldv, const float* __restrict__ w, i
 
     double ss = 0.0;
     float amax = 0.0f;
-    for (int k = tid; k < d; k += NQ_THREADS) {
-        const float x = vb[k];
-        ss = dacc(ss, x, x);
-        amax = fmaxf(amax, fabsf(fmul(x, w[k])));
+    if (in_regs) {
+#pragma unroll
+        for (int i = 0; i < NQ_R; ++i) {
+            const int k = tid + i * NQ_THREADS;
+            const float x = k < d ? vb[k] : 0.0f;          // (a zero adds +0 to the sum and 0 to the maximum)
+            ss = dacc(ss, x, x);
+            tv[i] = fmul(x, wv[i]);
+            amax = fmaxf(amax, fabsf(tv[i]));
+        }
+    } else {
+        for (int k = tid; k < d; k += NQ_THREADS) {
+            const float x = vb[k];
+            ss = dacc(ss, x, x);
+            amax = fmaxf(amax, fabsf(fmul(x, w[k])));
+        }
     }
     ss = warp_sum(ss);
     amax = warp_max(amax);
@@ -128,13 +150,22 @@ k_normquant(const float* __restrict__ v, int ldv, const float* __restrict__ w, i
     int8_t* qb = xq + (size_t)b * ldq;
     int8_t* qpb = xqp + (size_t)b * ldq;
     uint8_t* tp = taps ? taps + (size_t)b * tap_stride : nullptr;
-    for (int k = tid; k < d; k += NQ_THREADS) {
-        const int q = amax == 0.0f ? 0 : quant_code(fmul(vb[k], w[k]), inv);
+    auto emit = [&](int k, float tk) {
+        const int q = amax == 0.0f ? 0 : quant_code(tk, inv);
         qs += q;
         qb[k] = (int8_t)q;
         const int p = k & 31;
         qpb[(k & ~31) + 4 * (p & 7) + (p >> 3)] = (int8_t)q;
         if (tp) ((int8_t*)(tp + tap_q_off))[k] = (int8_t)q;
+    };
+    if (in_regs) {
+#pragma unroll
+        for (int i = 0; i < NQ_R; ++i) {
+            const int k = tid + i * NQ_THREADS;
+            if (k < d) emit(k, tv[i]);
+        }
+    } else {
+        for (int k = tid; k < d; k += NQ_THREADS) emit(k, fmul(vb[k], w[k]));
     }
     qs = warp_sum_i(qs);
     if (lane == 0) sh_i[wid] = qs;

@@ -35,13 +35,16 @@ __global__ void __launch_bounds__(FIN_THREADS)
 k_pf_epi4(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int32_t* __restrict__ t, const float* __restrict__ s_x,
           float* __restrict__ zx, int ldz)
 {
-    pdl_wait();
     const int p = blockIdx.y, base = blockIdx.x * FIN_THREADS, i = base + threadIdx.x;
     const bool own = i < dm.d_in_proj;
     const int il = own ? i : 0;
+    const float rs = __half2float(L.in_row_scale[il]), bs = L.in_b_s[il];      // weights: before pdl_wait
+    LoraRegs<JW, I4> lr;
+    lora_load4<JW, I4>(L.in_B, L.in_a_s, base, dm.d_in_proj, lr);
+    pdl_wait();
     const int acc_i = acc[(size_t)p * ld_acc + il];
-    const float rs = __half2float(L.in_row_scale[il]), bs = L.in_b_s[il], sx = s_x[p];
-    const double lo = lora_up4<JW, I4>(L.in_B, L.in_a_s, t + (size_t)p * T_STRIDE, base, dm.d_in_proj);
+    const float sx = s_x[p];
+    const double lo = lora_sum4<JW, I4>(lr, t + (size_t)p * T_STRIDE);
     if (own) zx[(size_t)p * ldz + i] = fmul(sx, fadd(fmul(rs, (float)acc_i), fmul(bs, (float)lo)));
 }
 
