@@ -373,6 +373,7 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
     // Measured (cfg 3, ms/step without / with): batch 5 1.78 / 1.55, 8 1.90 / 1.69, 16 2.20 / 2.01, 32 2.72 / 2.66, 64 3.99 / 3.93; cfg 4
     // batch 8 3.02 / 2.72; cfg 1 batch 16 0.81 / 0.71.  From batch 32 on k_normquant(g) stays behind k_ssm_stream (its 512-thread CTAs
     // would take the slots of that kernel's last wave).  DFSSM_PDL_MASK in the environment overrides the choice (0 = off).
+    const bool mma_in = use_mma(c, batch, d.d_model), mma_out = use_mma(c, batch, d.d_inner);      // K = d_model: in_proj and the LM head
     static const int pdl_env = getenv("DFSSM_PDL_MASK") ? atoi(getenv("DFSSM_PDL_MASK")) : -1;
     const int pdl = (tm == &dummy && !taps_on) ? (pdl_env >= 0 ? pdl_env : (batch >= 32 ? 111 : 127)) : 0;
 
@@ -390,7 +391,8 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         float* conv = at<float>(c, v.conv) + (size_t)l * B * (size_t)d.conv_dim * 4;
 
         tm->begin(DFSSM_KCLASS_NORMQUANT);
-        DFSSM_LAUNCH_EX(pdl & 1, k_normquant, batch, NQ_THREADS, 0, st, u, d.d_model, L.norm_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum,
+        DFSSM_LAUNCH_EX(pdl & 1, k_normquant, batch, NQ_THREADS, 0, st, u, d.d_model, L.norm_w, d.d_model, d.eps, xq, mma_in ? nullptr : xqp, ldq, sx,
+                        mma_in ? nullptr : qsum,
                         tp, v.tap_stride, v.tl.off[DFSSM_TAP_XQ_IN], v.tl.off[DFSSM_TAP_S_IN],
                         use_mma(c, batch, d.d_model) ? acc : nullptr, (int)ld_acc, t);
         tm->end(); ++nl;
@@ -455,7 +457,8 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         tm->end(); ++nl;
 
         tm->begin(DFSSM_KCLASS_NORMQUANT);
-        DFSSM_LAUNCH_EX(pdl & 16, k_normquant, batch, NQ_THREADS, 0, st, g, d.d_inner, L.gnorm_w, d.d_inner, d.eps, xq, xqp, ldq, sx, qsum,
+        DFSSM_LAUNCH_EX(pdl & 16, k_normquant, batch, NQ_THREADS, 0, st, g, d.d_inner, L.gnorm_w, d.d_inner, d.eps, xq, mma_out ? nullptr : xqp, ldq, sx,
+                        mma_out ? nullptr : qsum,
                         tp, v.tap_stride, v.tl.off[DFSSM_TAP_GQ], v.tl.off[DFSSM_TAP_S_G],
                         use_mma(c, batch, d.d_inner) ? acc : nullptr, (int)ld_acc, t);
         tm->end(); ++nl;
@@ -481,7 +484,8 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
     }
 
     tm->begin(DFSSM_KCLASS_NORMQUANT);
-    DFSSM_LAUNCH_EX(pdl & 1, k_normquant, batch, NQ_THREADS, 0, st, u, d.d_model, c->normf_w, d.d_model, d.eps, xq, xqp, ldq, sx, qsum,
+    DFSSM_LAUNCH_EX(pdl & 1, k_normquant, batch, NQ_THREADS, 0, st, u, d.d_model, c->normf_w, d.d_model, d.eps, xq, mma_in ? nullptr : xqp, ldq, sx,
+                    mma_in ? nullptr : qsum,
                     nullptr, 0, 0, 0, nullptr, 0, nullptr);
     tm->end(); ++nl;
 

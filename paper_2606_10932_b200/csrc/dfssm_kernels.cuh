@@ -154,8 +154,10 @@ k_normquant(const float* __restrict__ v, int ldv, const float* __restrict__ w, i
         const int q = amax == 0.0f ? 0 : quant_code(tk, inv);
         qs += q;
         qb[k] = (int8_t)q;
-        const int p = k & 31;
-        qpb[(k & ~31) + 4 * (p & 7) + (p >> 3)] = (int8_t)q;
+        if (xqp) {                                         // plane order and code sum: only the dp4a sign rows read them
+            const int p = k & 31;
+            qpb[(k & ~31) + 4 * (p & 7) + (p >> 3)] = (int8_t)q;
+        }
         if (tp) ((int8_t*)(tp + tap_q_off))[k] = (int8_t)q;
     };
     if (in_regs) {
@@ -166,6 +168,13 @@ k_normquant(const float* __restrict__ v, int ldv, const float* __restrict__ w, i
         }
     } else {
         for (int k = tid; k < d; k += NQ_THREADS) emit(k, fmul(vb[k], w[k]));
+    }
+    if (!qsum_out) {                                       // tensor-core projections behind this kernel: no code sum needed
+        if (tid == 0) {
+            s_out[b] = s;
+            if (tp) *(float*)(tp + tap_s_off) = s;
+        }
+        return;
     }
     qs = warp_sum_i(qs);
     if (lane == 0) sh_i[wid] = qs;
