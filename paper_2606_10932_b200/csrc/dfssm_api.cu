@@ -370,12 +370,11 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
     const int ldq = (int)v.ldq, ld_acc = (int)v.ld_acc;
     // programmatic dependent launch, per kind of kernel (bit set = that kernel may start under the one in front of it):
     // 1 k_normquant(u), 2 in_proj, 4 k_fin4, 8 k_ssm_stream, 16 k_normquant(g), 32 out_proj, 64 k_epi_out4.  Tensor-core chain only.
-    // Measured (cfg 3, ms/step without / with): batch 5 1.78 / 1.55, 8 1.90 / 1.69, 16 2.20 / 2.01, 32 2.72 / 2.66, 64 3.99 / 3.93; cfg 4
-    // batch 8 3.02 / 2.72; cfg 1 batch 16 0.81 / 0.71.  From batch 32 on k_normquant(g) stays behind k_ssm_stream (its 512-thread CTAs
-    // would take the slots of that kernel's last wave).  DFSSM_PDL_MASK in the environment overrides the choice (0 = off).
+    // Measured (cfg 3, ms/step without / with, final build): batch 5 1.78 / 1.36, 8 1.90 / 1.53, 16 2.20 / 1.85, 32 2.72 / 2.53,
+    // 64 3.99 / 3.80; cfg 4 batch 8 3.02 / 2.53.  DFSSM_PDL_MASK in the environment overrides the choice (0 = off).
     const bool mma_in = use_mma(c, batch, d.d_model), mma_out = use_mma(c, batch, d.d_inner);      // K = d_model: in_proj and the LM head
     static const int pdl_env = getenv("DFSSM_PDL_MASK") ? atoi(getenv("DFSSM_PDL_MASK")) : -1;
-    const int pdl = (tm == &dummy && !taps_on) ? (pdl_env >= 0 ? pdl_env : (batch >= 32 ? 111 : 127)) : 0;
+    const int pdl = (tm == &dummy && !taps_on) ? (pdl_env >= 0 ? pdl_env : 127) : 0;
 
     tm->begin(DFSSM_KCLASS_EMBED);
     k_embed<<<dim3((d.d_model + 255) / 256, batch), 256, 0, st>>>(tokens, c->emb, c->emb_s, d.vocab, d.d_model, u, err);

@@ -546,11 +546,11 @@ k_ssm_stream(LayerW L, Dims dm, const float* __restrict__ fin, ST* __restrict__ 
         const int n4 = l16 + LANES * j;
         if (DS || n4 < ds / 4) hpre[j] = state_ld4(Hr + 4 * n4);
     }
+    const float Dh = L.D[h];
     pdl_wait();                                    // the state was requested above: only this layer's kernel of the step before wrote it
     const float xv = src[dm.d_inner + ch];
     const float dtv = src[d_in_proj - dm.nheads + h], dA = src[d_in_proj + h];
     const float sz = src[ch];                      // silu(z) from k_fin
-    const float Dh = L.D[h];
     for (int i = tid; i < ds; i += SSM_THREADS) {
         Bc[i] = src[2 * dm.d_inner + grp * ds + i];
         Cc[i] = src[2 * dm.d_inner + gs + grp * ds + i];

@@ -149,9 +149,8 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
         x_next[1] = (b_valid && kx + 128 < K) ? *(const uint4*)(x_row + kc * KC + 128) : make_uint4(0, 0, 0, 0);
     };
     auto request = [&](int kc) { request_w(kc); request_x(kc); };
-    // TMEM allocation, barrier initialisation and - for small batches - the first weight request run under the kernel in front
-    // (measured, cfg 3, ms/step with / without the early request: batch 5 1.526 / 1.554, 16 1.991 / 2.005, 32 2.714 / 2.658, 64 4.026 / 3.928)
-    const bool early_w = batch <= 16 && kc0 < kc1;
+    // TMEM allocation, barrier initialisation and the first weight request run under the kernel in front
+    const bool early_w = kc0 < kc1;
     if (early_w) request_w(kc0);
     pdl_wait();
     if (kc0 < kc1) {
