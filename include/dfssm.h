@@ -61,7 +61,7 @@ enum {
 #define DFSSM_FLAG_TAPS      1u  /* allocate per-layer debug taps and record them every step (slower)   */
 #define DFSSM_FLAG_NO_GRAPH  2u  /* launch the step's kernels one by one instead of one CUDA-graph launch */
 #define DFSSM_FLAG_NO_MEGA   4u  /* never use the single persistent kernel ("mega" path) for batch-1 steps    */
-#define DFSSM_FLAG_NO_MMA   16u  /* batch >= 16: keep the projections on the dp4a path instead of tcgen05 kind::i8 tiles  */
+#define DFSSM_FLAG_NO_MMA   16u  /* keep the projections on the dp4a path at every batch size instead of tcgen05 kind::i8 tiles  */
 #define DFSSM_FLAG_STATE_FP16 64u /* SURVEY 8(f) NEXT-2, first step (R24): the SSM state is STORED as binary16 (round to nearest even of each
                                    * step's binary32 update; the step's own readout uses the unrounded values).  Halves the state bytes (95 % of the
                                    * traffic at batch 64).  LOSSY against the fp32-state model; bit-identical to the oracle in the same mode.
@@ -133,9 +133,10 @@ DFSSM_API int dfssm_reset_state(dfssm_ctx* ctx, int seq_index);
  * (device int32[batch]; it may be the pointer returned by dfssm_next_tokens -- greedy decode
  * without leaving the device).  Async: for batch 1 exactly one launch of the persistent cooperative
  * kernel (the "mega" path: 148 co-resident CTAs, weights and state prefetched ahead of the layer
- * dependencies), for batch 2..4 one such launch per sequence, otherwise one CUDA graph of the kernel chain
- * (projections on tcgen05 kind::i8 tiles from batch 16 on) -- unless DFSSM_FLAG_NO_GRAPH or
- * DFSSM_FLAG_TAPS asks for the chain's kernels one by one.  The two paths share the state layout
+ * dependencies), for batch 2..3 of models with d_model >= 1024 one such launch per sequence, otherwise one CUDA graph of
+ * the kernel chain, its kernels launched dependently (each runs its weight prologue while the one in front drains), with the
+ * projections on tcgen05 kind::i8 tiles from batch 4 on (d_model >= 1024; from batch 8 on for narrower models) -- unless
+ * DFSSM_FLAG_NO_GRAPH or DFSSM_FLAG_TAPS asks for the chain's kernels one by one.  The paths share the state layout
  * and compute bit-identical results.  Token ids outside [0, vocab) are clamped on the
  * device and a sticky error is raised, reported as DFSSM_E_TOKEN by the next dfssm_sync. */
 DFSSM_API int dfssm_step(dfssm_ctx* ctx, const int32_t* tokens_dev, int batch);

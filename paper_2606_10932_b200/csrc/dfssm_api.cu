@@ -253,10 +253,10 @@ int proj_grid(int rows_total)
 // the projections run on the tensor cores (tcgen05 kind::i8 on +-1 tiles unpacked in shared memory) from this batch size on
 bool use_mma(const dfssm_ctx* c, int batch, int K)
 {
-    // measured (ms/step, dp4a rows vs tensor cores; cfg 3: batch 5 1.99 / 1.68, 8 2.50 / 1.82, 15 3.32 / 2.21; cfg 4: batch 5 3.49 / 2.73,
-    // 8 4.34 / 3.10; cfg 1 (d_model 768): batch 8 0.64 / 0.68): from batch 5 on for the wide models, from 16 on for narrow ones
+    // measured (ms/step, dp4a rows / tensor cores, final build): cfg 3 batch 4 1.63 / 1.29; cfg 1 (d_model 768) batch 3 0.46 / 0.47,
+    // 5 0.49 / 0.50, 8 0.56 / 0.54, 12 0.64 / 0.58: from batch 4 on for the wide models, from 8 on for narrow ones
     if (c->dm.fmt) return true;                       // the format variants are unpacked by k_proj_mma only
-    const int mma_min = c->dm.d_model >= 1024 ? 5 : 16;
+    const int mma_min = c->dm.d_model >= 1024 ? 4 : 8;
     return batch >= mma_min && K % mma::KMULT == 0 && !(c->cfg.flags & DFSSM_FLAG_NO_MMA);
 }
 
@@ -542,10 +542,12 @@ int get_graph(dfssm_ctx* c, int batch, cudaGraphExec_t* out)
 // =================================================================================================
 namespace {
 
-// The persistent kernel serves one sequence per launch.  Up to MEGA_MAX_BATCH sequences are stepped by back-to-back launches
-// (each sequence with its own state, token and logits slice): measured on cfg 2, 4 x 0.40 ms beats the 340-node chain (1.97 ms).
-constexpr int MEGA_MAX_BATCH = 4;
-bool use_mega(const dfssm_ctx* c, int batch) { return batch <= MEGA_MAX_BATCH && c->mega_ok && !(c->cfg.flags & DFSSM_FLAG_TAPS && batch > 1); }
+// The persistent kernel serves one sequence per launch; a few sequences are stepped by back-to-back launches while that beats the
+// kernel chain.  Measured (ms/step, launches of the persistent kernel / chain with tensor-core projections [/ dp4a rows], final
+// build): cfg 3 (d_model 2048) batch 2 0.77 / 1.2, 3 1.15 / 1.27, 4 1.53 / 1.29; cfg 4 (2560) batch 2 1.35 / 1.96, 3 2.01 / 2.12,
+// 4 2.69 / 2.21; cfg 1 (768) batch 2 0.44 / 0.45 / 0.42, 3 0.66 / 0.47 / 0.46; cfg 0 (256) batch 2 0.057 / 0.046.
+int mega_max_batch(const dfssm_ctx* c) { return c->dm.d_model >= 1024 ? 3 : 1; }
+bool use_mega(const dfssm_ctx* c, int batch) { return batch <= mega_max_batch(c) && c->mega_ok && !(c->cfg.flags & DFSSM_FLAG_TAPS && batch > 1); }
 
 int mega_setup(dfssm_ctx* ctx)                      // at create: can this device run the mega grid?
 {
