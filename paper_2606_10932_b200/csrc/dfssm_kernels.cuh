@@ -476,10 +476,13 @@ k_fin4(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int
     }
     LoraRegs<JW, I4> lr;
     lora_load4<JW, I4>(L.in_B, L.in_a_s, base, d_in_proj, lr);
-    pdl_wait();
-    const int acc_i = acc[(size_t)b * ld_acc + rl];
+    // also before the wait: what kernels further back than the one in front wrote (at most two kernels of the chain overlap, so
+    // those have completed): the scale of k_normquant, the conv ring and the ring position of the step before
     const float sx = s_x[b];
     if (is_conv) rg = *(const float4*)ring;
+    const int ps = pos[b] & 3;
+    pdl_wait();
+    const int acc_i = acc[(size_t)b * ld_acc + rl];
 
     const double lo = lora_sum4<JW, I4>(lr, t + (size_t)b * T_STRIDE);
     if (!own) return;
@@ -490,7 +493,6 @@ k_fin4(LayerW L, Dims dm, const int32_t* __restrict__ acc, int ld_acc, const int
     if (row < dm.d_inner) {
         out[row] = siluf(val);                                                   // the gate factor of S6
     } else if (is_conv) {
-        const int ps = pos[b] & 3;
         const float sl[4] = { rg.x, rg.y, rg.z, rg.w };
         const float s0 = sl[(ps + 1) & 3], s1 = sl[(ps + 2) & 3], s2 = sl[(ps + 3) & 3];
         float o = cb;
@@ -644,10 +646,10 @@ k_epi_out4(LayerW L, int d_model, const int32_t* __restrict__ acc, int ld_acc,
     const float rs = __half2float(L.out_row_scale[il]), bs = L.out_b_s[il];      // weights: before pdl_wait
     LoraRegs<JW, I4> lr;
     lora_load4<JW, I4>(L.out_B, L.out_a_s, base, d_model, lr);
+    const float sg = s_g[b];                               // k_normquant(g): two kernels back, complete (see k_fin4)
+    const float u0 = u[(size_t)b * d_model + il];          // the layer before
     pdl_wait();
     const int acc_i = acc[(size_t)b * ld_acc + il];
-    const float sg = s_g[b];
-    const float u0 = u[(size_t)b * d_model + il];
     const double lo = lora_sum4<JW, I4>(lr, t + (size_t)b * T_STRIDE);
     if (!own) return;
     const float o = fmul(sg, fadd(fmul(rs, (float)acc_i), fmul(bs, (float)lo)));
