@@ -489,7 +489,9 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
     tm->end(); ++nl;
 
     tm->begin(DFSSM_KCLASS_LMHEAD);
-    if (use_mma(c, batch, d.d_model)) {
+    // up to one sequence tile of k_lmhead (8) the warp-per-row dp4a kernel reads the embedding once and beats the tensor-core tiles
+    // (cfg 3, us: batch 5 40 / 61, 8 46 / 63, 16 81 / 66)
+    if (use_mma(c, batch, d.d_model) && batch > PROJ_BT) {
         DFSSM_LAUNCH_EX(pdl & 2, mma::k_proj_mma<0>, dim3((d.vocab + mma::TM - 1) / mma::TM, (batch + mma::TN - 1) / mma::TN, 1), mma::THREADS, mma::SMEM_BYTES, st,
                         nullptr, c->emb, 0, d.vocab, d.d_model, xq, ldq, batch, nullptr, 0, nullptr, err, logits, sx, c->emb_s);
     } else {
