@@ -134,6 +134,7 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
 #pragma unroll
     for (int i = 0; i < NWD; ++i) w_next[i] = 0;
     uint4 x_next[2] = { make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0) }, x_cur[2];
+    uint4 a_next[4] = { make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0) }, a_cur[4];
     auto request_w = [&](int kc) {     // the weights: independent of the kernel in front
         const int ka = kc * KC + qk * 64;      // byte offset of this thread's piece inside K; beyond K (last half stage) the operands are zero
 #pragma unroll
@@ -141,6 +142,16 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
             const uint2 ww = (is_sign && ka < K) ? *(const uint2*)(sign_row + (size_t)kc * (KC / 32) * PL + 2 * i) : make_uint2(0, 0);
             w_next[2 * i] = ww.x;
             w_next[2 * i + 1] = ww.y;
+        }
+        if (!is_sign && urow < rows_total && ka < K) {      // int8 / int4 rows (LoRA-down, the LM head's embedding): a stage ahead as well
+            if (FMT & 2) {
+                const uint4* src = (const uint4*)((const uint8_t*)A + ((size_t)(urow - rows) * K + ka) / 2);
+                a_next[0] = src[0]; a_next[1] = src[1];
+            } else {
+                const uint4* src = (const uint4*)(A + (size_t)(urow - rows) * K + ka);
+#pragma unroll
+                for (int c = 0; c < 4; ++c) a_next[c] = src[c];
+            }
         }
     };
     auto request_x = [&](int kc) {     // the codes: written by the kernel in front
@@ -164,6 +175,8 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
 #pragma unroll
         for (int i = 0; i < NWD; ++i) w_cur[i] = w_next[i];
         x_cur[0] = x_next[0]; x_cur[1] = x_next[1];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) a_cur[c] = a_next[c];
         if (kc + 1 < kc1) request(kc + 1);
         if (use > 0) wait_stage(s, (uint32_t)(use - 1) & 1u);           // the MMAs that read this stage last are done
         // ---- A: 64 weights of this row -> int8 ----
@@ -182,8 +195,7 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
             *(uint4*)(a_dst + 2 * LBO_A) = make_uint4(signs4(w1), signs4(w1 >> 4), signs4(w1 >> 8), signs4(w1 >> 12));
             *(uint4*)(a_dst + 3 * LBO_A) = make_uint4(signs4(w1 >> 16), signs4(w1 >> 20), signs4(w1 >> 24), signs4(w1 >> 28));
         } else if ((FMT & 2) && !is_sign && urow < rows_total && a_in) {      // int4 LoRA-down row: 64 values in 32 bytes
-            const uint4* src = (const uint4*)((const uint8_t*)A + ((size_t)(urow - rows) * K + kc * KC + qk * 64) / 2);
-            const uint4 p0 = src[0], p1 = src[1];
+            const uint4 p0 = a_cur[0], p1 = a_cur[1];
             const uint32_t pw[8] = { p0.x, p0.y, p0.z, p0.w, p1.x, p1.y, p1.z, p1.w };
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
@@ -191,9 +203,8 @@ k_proj_mma(const uint32_t* __restrict__ sign, const int8_t* __restrict__ A, int 
                 *(uint4*)(a_dst + c * LBO_A) = make_uint4(e0.x, e0.y, e1.x, e1.y);
             }
         } else if (!is_sign && urow < rows_total && a_in) {
-            const uint4* src = (const uint4*)(A + (size_t)(urow - rows) * K + kc * KC + qk * 64);
 #pragma unroll
-            for (int c = 0; c < 4; ++c) *(uint4*)(a_dst + c * LBO_A) = src[c];
+            for (int c = 0; c < 4; ++c) *(uint4*)(a_dst + c * LBO_A) = a_cur[c];
         } else {
 #pragma unroll
             for (int c = 0; c < 4; ++c) *(uint4*)(a_dst + c * LBO_A) = make_uint4(0, 0, 0, 0);
