@@ -310,6 +310,59 @@ int launch_proj_mma(dfssm_ctx* ctx, const uint32_t* sign, const int8_t* A, int r
     return DFSSM_OK;
 }
 
+// threads per CTA of k_epi_norm4 (S7 + the norm / quantiser behind it in one cluster launch), 0 = this shape runs them apart
+int epi_norm_threads(const Dims& d)
+{
+    if (d.r != 8 && d.r != 16 && d.r != 32 && d.r != 64) return 0;
+    if (d.d_model % 256 == 0 && d.d_model / 256 <= 8) return 256;
+    if (d.d_model % 512 == 0 && d.d_model / 512 <= 8) return 512;
+    return 0;
+}
+#define DFSSM_LAUNCH_CL(PDL_, KERNEL_, GRID_, BLOCK_, ST_, ...)                                       \
+    do {                                                                                              \
+        cudaLaunchConfig_t cfg_ = {};                                                                 \
+        cfg_.gridDim = GRID_;                                                                         \
+        cfg_.blockDim = BLOCK_;                                                                       \
+        cfg_.stream = ST_;                                                                            \
+        cudaLaunchAttribute at_[2];                                                                   \
+        at_[0].id = cudaLaunchAttributeClusterDimension;                                              \
+        at_[0].val.clusterDim.x = (GRID_).x;                                                          \
+        at_[0].val.clusterDim.y = 1;                                                                  \
+        at_[0].val.clusterDim.z = 1;                                                                  \
+        at_[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;                               \
+        at_[1].val.programmaticStreamSerializationAllowed = 1;                                        \
+        cfg_.attrs = at_;                                                                             \
+        cfg_.numAttrs = (PDL_) ? 2 : 1;                                                               \
+        cudaLaunchKernelEx(&cfg_, KERNEL_, __VA_ARGS__);                                              \
+    } while (0)
+void launch_epi_norm(const LayerW& L, const Dims& d, int n, const int32_t* acc, int ld_acc, const int32_t* t, const float* s_g, float* u,
+                     const float* w_next, int8_t* xq, int ldq, float* s_out, int32_t* zero_acc, int32_t* zero_t, cudaStream_t st, bool pdl)
+{
+    const int nthr = epi_norm_threads(d);
+    const dim3 g(d.d_model / nthr, n);
+    const bool i4 = (d.fmt & 2) != 0;
+#define DFSSM_EPN_ARGS L, d.d_model, acc, ld_acc, t, s_g, u, w_next, d.eps, xq, ldq, s_out, zero_acc, zero_t
+    switch (d.r) {
+        case 8:
+            if (i4) DFSSM_LAUNCH_CL(pdl, (k_epi_norm4<2, true>), g, nthr, st, DFSSM_EPN_ARGS);
+            else DFSSM_LAUNCH_CL(pdl, (k_epi_norm4<2, false>), g, nthr, st, DFSSM_EPN_ARGS);
+            break;
+        case 16:
+            if (i4) DFSSM_LAUNCH_CL(pdl, (k_epi_norm4<4, true>), g, nthr, st, DFSSM_EPN_ARGS);
+            else DFSSM_LAUNCH_CL(pdl, (k_epi_norm4<4, false>), g, nthr, st, DFSSM_EPN_ARGS);
+            break;
+        case 32:
+            if (i4) DFSSM_LAUNCH_CL(pdl, (k_epi_norm4<8, true>), g, nthr, st, DFSSM_EPN_ARGS);
+            else DFSSM_LAUNCH_CL(pdl, (k_epi_norm4<8, false>), g, nthr, st, DFSSM_EPN_ARGS);
+            break;
+        default:
+            if (i4) DFSSM_LAUNCH_CL(pdl, (k_epi_norm4<16, true>), g, nthr, st, DFSSM_EPN_ARGS);
+            else DFSSM_LAUNCH_CL(pdl, (k_epi_norm4<16, false>), g, nthr, st, DFSSM_EPN_ARGS);
+            break;
+    }
+#undef DFSSM_EPN_ARGS
+}
+
 // S7 epilogue + residual for n sequences / positions: four lanes per row when the LoRA rank allows (k_epi_out4)
 void launch_epi_out(const LayerW& L, const Dims& d, int n, const int32_t* acc, int ld_acc, const int32_t* t, const float* s_g, float* u,
                     uint8_t* tp, uint32_t tap_stride, uint32_t tap_off, cudaStream_t st, bool pdl = false)
@@ -376,6 +429,10 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
     static const int pdl_env = getenv("DFSSM_PDL_MASK") ? atoi(getenv("DFSSM_PDL_MASK")) : -1;
     const int pdl = (tm == &dummy && !taps_on) ? (pdl_env >= 0 ? pdl_env : 127) : 0;
 
+    // S7 + the norm / quantiser behind it as one cluster launch (k_epi_norm4): tensor-core chain under the graph only
+    static const int fuse_env = getenv("DFSSM_FUSE_EPI") ? atoi(getenv("DFSSM_FUSE_EPI")) : 1;
+    const bool fuse = fuse_env && pdl && mma_in && mma_out && epi_norm_threads(d) != 0;
+
     tm->begin(DFSSM_KCLASS_EMBED);
     k_embed<<<dim3((d.d_model + 255) / 256, batch), 256, 0, st>>>(tokens, c->emb, c->emb_s, d.vocab, d.d_model, u, err);
     tm->end(); ++nl;
@@ -390,6 +447,7 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         float* conv = at<float>(c, v.conv) + (size_t)l * B * (size_t)d.conv_dim * 4;
 
         tm->begin(DFSSM_KCLASS_NORMQUANT);
+        if (!fuse || l == 0)
         DFSSM_LAUNCH_EX(pdl & 1, k_normquant, batch, NQ_THREADS, 0, st, u, d.d_model, L.norm_w, d.d_model, d.eps, xq, mma_in ? nullptr : xqp, ldq, sx,
                         mma_in ? nullptr : qsum,
                         tp, v.tap_stride, v.tl.off[DFSSM_TAP_XQ_IN], v.tl.off[DFSSM_TAP_S_IN],
@@ -478,11 +536,17 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
         }
 
         tm->begin(DFSSM_KCLASS_EPI_OUT);
+        if (fuse) {
+            const bool last = l + 1 == d.n_layers;
+            launch_epi_norm(L, d, batch, acc, ld_acc, t, sx, u, last ? c->normf_w : c->layers[l + 1].norm_w, xq, ldq, sx,
+                            last ? nullptr : acc, last ? nullptr : t, st, (pdl & 64) != 0);
+        } else
         launch_epi_out(L, d, batch, acc, ld_acc, t, sx, u, tp, v.tap_stride, v.tl.off[DFSSM_TAP_HIDDEN], st, (pdl & 64) != 0);
         tm->end(); ++nl;
     }
 
     tm->begin(DFSSM_KCLASS_NORMQUANT);
+    if (!fuse)
     DFSSM_LAUNCH_EX(pdl & 1, k_normquant, batch, NQ_THREADS, 0, st, u, d.d_model, c->normf_w, d.d_model, d.eps, xq, mma_in ? nullptr : xqp, ldq, sx,
                     mma_in ? nullptr : qsum,
                     nullptr, 0, 0, 0, nullptr, 0, nullptr);
@@ -507,6 +571,7 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
     DFSSM_LAUNCH_EX(pdl & 2, k_argmax, batch, AM_THREADS, 0, st, logits, d.vocab, next, tokens, pos, 1);
     tm->end(); ++nl;
 
+    if (fuse) nl -= d.n_layers;                 // the k_normquant launches k_epi_norm4 replaced
     if (n_launch) *n_launch = nl;
     CK(cudaGetLastError());
     return DFSSM_OK;

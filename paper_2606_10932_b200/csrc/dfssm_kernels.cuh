@@ -658,6 +658,89 @@ k_epi_out4(LayerW L, int d_model, const int32_t* __restrict__ acc, int ld_acc,
     if (taps) ((float*)(taps + (size_t)b * tap_stride + tap_hidden_off))[i] = un;
 }
 
+// k_epi_out4 fused with the RMSNorm + quantiser that follows it (S7 of layer l, then S1 of layer l + 1 or S8(a)): the CTAs of one
+// sequence form a thread-block cluster (d_model / blockDim.x <= 8 CTAs), exchange their partial sum of squares and maximum through
+// distributed shared memory and quantise their own elements, so the separate k_normquant launch (one CTA per sequence, 5 us) goes.
+// Tensor-core chain without taps only; d_model % blockDim.x == 0.  w_next: norm weights of the sub-layer that follows.
+// zero_acc / zero_t as in k_normquant (this sequence's rows, zeroed once every CTA of the cluster has read them).
+constexpr int EPN_MAX_THREADS = 512;
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+
+template <int JW, bool I4 = false>
+__global__ void __launch_bounds__(EPN_MAX_THREADS)
+k_epi_norm4(LayerW L, int d_model, const int32_t* acc, int ld_acc, const int32_t* t,
+            const float* s_g, float* __restrict__ u, const float* __restrict__ w_next, float eps,
+            int8_t* __restrict__ xq, int ldq, float* s_out, int32_t* zero_acc, int32_t* zero_t)      // s_out may be s_g, zero_acc / zero_t are acc / t
+{
+    __shared__ double sh_d[EPN_MAX_THREADS / 32];
+    __shared__ float sh_f[EPN_MAX_THREADS / 32];
+    __shared__ double cl_ss;                 // this CTA's partials, read by every CTA of the cluster
+    __shared__ float cl_amax;
+    __shared__ float sh_bcast[2];
+    const int b = blockIdx.y, nthr = blockDim.x, base = blockIdx.x * nthr, tid = threadIdx.x, i = base + tid;
+    const int lane = tid & 31, wid = tid >> 5, ncta = gridDim.x, rank = blockIdx.x;
+    const float rs = __half2float(L.out_row_scale[i]), bs = L.out_b_s[i];      // weights: before pdl_wait
+    const float wn = w_next[i];
+    LoraRegs<JW, I4> lr;
+    lora_load4<JW, I4>(L.out_B, L.out_a_s, base, d_model, lr);
+    const float sg = s_g[b];                               // k_normquant(g): two kernels back, complete (see k_fin4)
+    const float u0 = u[(size_t)b * d_model + i];           // the layer before
+    pdl_wait();
+    const int acc_i = acc[(size_t)b * ld_acc + i];
+    const double lo = lora_sum4<JW, I4>(lr, t + (size_t)b * T_STRIDE);
+    const float o = fmul(sg, fadd(fmul(rs, (float)acc_i), fmul(bs, (float)lo)));
+    const float un = fadd(u0, o);
+    u[(size_t)b * d_model + i] = un;
+    // ---- the norm of what follows: partials of this CTA ----
+    const float tk = fmul(un, wn);
+    double ss = warp_sum(dacc(0.0, un, un));
+    float amax = warp_max(fabsf(tk));
+    if (lane == 0) { sh_d[wid] = ss; sh_f[wid] = amax; }
+    __syncthreads();
+    if (wid == 0) {
+        double s2 = lane < nthr / 32 ? sh_d[lane] : 0.0;
+        float m2 = lane < nthr / 32 ? sh_f[lane] : 0.0f;
+        s2 = warp_sum(s2);
+        m2 = warp_max(m2);
+        if (lane == 0) { cl_ss = s2; cl_amax = m2; }
+    }
+    cluster_arrive();
+    cluster_wait();                          // every CTA of the sequence has published its partials and read its acc / t
+    if (wid == 0) {
+        double s2 = 0.0;
+        float m2 = 0.0f;
+        if (lane < ncta) {
+            uint32_t ra, rb;
+            asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"((uint32_t)__cvta_generic_to_shared(&cl_ss)), "r"(lane));
+            asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rb) : "r"((uint32_t)__cvta_generic_to_shared(&cl_amax)), "r"(lane));
+            asm volatile("ld.shared::cluster.f64 %0, [%1];" : "=d"(s2) : "r"(ra) : "memory");
+            asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(m2) : "r"(rb) : "memory");
+        }
+        s2 = warp_sum(s2);
+        m2 = warp_max(m2);
+        if (lane == 0) {
+            const float ms = (float)(s2 / (double)d_model);
+            sh_bcast[0] = m2;
+            sh_bcast[1] = fdiv(1.0f, __fsqrt_rn(fadd(ms, eps)));
+        }
+    }
+    __syncthreads();
+    cluster_arrive();                        // this CTA has read its peers; it leaves only when they have read it (wait at the end)
+    amax = sh_bcast[0];
+    const float rstd = sh_bcast[1];
+    const float inv = amax == 0.0f ? 0.0f : fdiv(127.0f, amax);
+    xq[(size_t)b * ldq + i] = (int8_t)(amax == 0.0f ? 0 : quant_code(tk, inv));
+    if (rank == 0 && tid == 0) s_out[b] = amax == 0.0f ? 0.0f : fdiv(fmul(amax, rstd), 127.0f);
+    if (zero_acc) {                          // rows of the split-K projection that follows
+        int32_t* za = zero_acc + (size_t)b * ld_acc;
+        const int per = (ld_acc + ncta - 1) / ncta, k1 = min(ld_acc, (rank + 1) * per);
+        for (int k = rank * per + tid; k < k1; k += nthr) za[k] = 0;
+        if (rank == 0 && tid < T_STRIDE) zero_t[(size_t)b * T_STRIDE + tid] = 0;
+    }
+    cluster_wait();
+}
+
 // debug-only: copy int32 vectors into the taps (acc, t)
 __global__ void k_tap_copy_i32(const int32_t* __restrict__ src, int ld_src, int n, uint8_t* __restrict__ taps,
                                uint32_t tap_stride, uint32_t off)
