@@ -392,6 +392,15 @@ void launch_epi_out(const LayerW& L, const Dims& d, int n, const int32_t* acc, i
     }
 }
 
+// S7 + the norm / quantiser behind it as one cluster launch (k_epi_norm4): tensor-core chain with dependent launches, no taps
+bool fused_epi_norm(const dfssm_ctx* c, int batch)
+{
+    static const int fuse_env = getenv("DFSSM_FUSE_EPI") ? atoi(getenv("DFSSM_FUSE_EPI")) : 1;
+    static const int pdl_env = getenv("DFSSM_PDL_MASK") ? atoi(getenv("DFSSM_PDL_MASK")) : -1;
+    if (!fuse_env || pdl_env == 0 || (c->cfg.flags & DFSSM_FLAG_TAPS)) return false;
+    return use_mma(c, batch, c->dm.d_model) && use_mma(c, batch, c->dm.d_inner) && epi_norm_threads(c->dm) != 0;
+}
+
 // Enqueue S0, L x (S1..S7), S8 for `batch` sequences on the context's stream.  The input tokens are
 // read from the arena's own token buffer (cv.tok), which the argmax kernel also refreshes with the
 // greedy tokens -- so a graph captured once per batch size serves every caller pointer.
@@ -429,9 +438,7 @@ int enqueue_step(dfssm_ctx* c, int batch, KTimer* tm, int* n_launch)
     static const int pdl_env = getenv("DFSSM_PDL_MASK") ? atoi(getenv("DFSSM_PDL_MASK")) : -1;
     const int pdl = (tm == &dummy && !taps_on) ? (pdl_env >= 0 ? pdl_env : 127) : 0;
 
-    // S7 + the norm / quantiser behind it as one cluster launch (k_epi_norm4): tensor-core chain under the graph only
-    static const int fuse_env = getenv("DFSSM_FUSE_EPI") ? atoi(getenv("DFSSM_FUSE_EPI")) : 1;
-    const bool fuse = fuse_env && pdl && mma_in && mma_out && epi_norm_threads(d) != 0;
+    const bool fuse = pdl && fused_epi_norm(c, batch);
 
     tm->begin(DFSSM_KCLASS_EMBED);
     k_embed<<<dim3((d.d_model + 255) / 256, batch), 256, 0, st>>>(tokens, c->emb, c->emb_s, d.vocab, d.d_model, u, err);
@@ -1227,7 +1234,7 @@ int dfssm_launches_per_step(dfssm_ctx* ctx, int batch)
     if (!ctx || batch < 1) return DFSSM_E_ARG;
     if (use_mega(ctx, batch)) return batch;
     const int per_layer = (ctx->cfg.flags & DFSSM_FLAG_TAPS) ? 11 : 7;
-    return 1 + ctx->dm.n_layers * per_layer + 3;
+    return 1 + ctx->dm.n_layers * per_layer + 3 - (fused_epi_norm(ctx, batch) ? ctx->dm.n_layers : 0);
 }
 
 int dfssm_time_kernels(dfssm_ctx* ctx, const int32_t* tokens_dev, int batch, int iters, float* out_us)

@@ -403,3 +403,45 @@ def test_every_baseline_shape_runs_the_persistent_kernel_at_batch_1(env, cfg_idx
     m = pk.Model(pk.Config.from_shape(s, max_batch=1))
     assert m.launches_per_step(1) == 1
     m.close()
+
+
+# k_epi_norm4 (out_proj epilogue + the norm / quantiser behind it as one cluster launch): the graph path of the
+# tensor-core chain on shapes that take 1, 3, 8 CTAs of 256 threads and 5 CTAs of 512 threads per sequence, and one (d_model 384)
+# that keeps the two kernels apart; the taps path (two kernels) must agree bit for bit with it.
+EPN_SHAPES = [
+    dict(n_layers=2, d_model=256, d_inner=512, headdim=64, d_state=16, lora_rank=8, vocab=97, batch=9),
+    dict(n_layers=3, d_model=768, d_inner=768, headdim=32, d_state=32, lora_rank=16, vocab=211, batch=8),
+    dict(n_layers=2, d_model=2048, d_inner=1024, headdim=64, d_state=16, lora_rank=32, vocab=150, batch=5),
+    dict(n_layers=2, d_model=2560, d_inner=1280, headdim=64, d_state=16, lora_rank=64, vocab=131, batch=4),
+    dict(n_layers=2, d_model=384, d_inner=768, headdim=64, d_state=16, lora_rank=8, vocab=90, batch=8),
+]
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("kw", EPN_SHAPES, ids=[f"d{k['d_model']}" for k in EPN_SHAPES])
+def test_fused_epilogue_norm_graph_path(env, kw):
+    pk, oracle, torch = env["pk"], env["oracle"], env["torch"]
+    kw = dict(kw)
+    B = kw.pop("batch")
+    s = ds.tiny_shape(**kw)
+    blob = ds.make_blob(s, seed=77, variant="varied")
+    gpu = pk.Model(pk.Config.from_shape(s, max_batch=B), blob)
+    tap = pk.Model(pk.Config.from_shape(s, max_batch=B, flags=pk.binding.FLAG_TAPS), blob)
+    seqs = sorted({0, B - 1})
+    orcs = {q: oracle.OracleModel(blob, 1) for q in seqs}
+    T = 6
+    toks = ds.token_batch(s.vocab, T, seed=31, batch=B)
+    st = Stats()
+    for t in range(T):
+        gpu.step(dev_tokens(torch, toks[t]))
+        tap.step(dev_tokens(torch, toks[t]))
+        gpu.sync(); tap.sync()
+        assert torch.equal(gpu.logits(), tap.logits()) and torch.equal(gpu.hidden(), tap.hidden())
+        for q, o in orcs.items():
+            o.step(toks[t, q:q + 1])
+            compare_step(gpu, o, q, st, t, f"epn-d{s.d_model}")
+    assert st.diff_hidden == 0 and st.diff_logits == 0, st
+    for q, o in orcs.items():
+        for l in range(s.n_layers):
+            sg, cg = gpu.get_state(l, q)
+            assert n_diff_bits(sg, o.ssm_state(l, 0)) == 0 and n_diff_bits(cg, o.conv_state(l, 0)) == 0
