@@ -135,7 +135,7 @@ DFSSM_API int dfssm_reset_state(dfssm_ctx* ctx, int seq_index);
  * kernel (the "mega" path: 148 co-resident CTAs, weights and state prefetched ahead of the layer
  * dependencies), for batch 2..3 of models with d_model >= 1024 one such launch per sequence, otherwise one CUDA graph of
  * the kernel chain, its kernels launched dependently (each runs its weight prologue while the one in front drains), with the
- * projections on tcgen05 kind::i8 tiles from batch 4 on (d_model >= 1024; from batch 8 on for narrower models) -- unless
+ * projections on tcgen05 kind::i8 tiles from batch 4 on (d_model >= 1024; from 2 on for d_model 512..1023, from 8 on below) -- unless
  * DFSSM_FLAG_NO_GRAPH or DFSSM_FLAG_TAPS asks for the chain's kernels one by one.  The paths share the state layout
  * and compute bit-identical results.  Token ids outside [0, vocab) are clamped on the
  * device and a sticky error is raised, reported as DFSSM_E_TOKEN by the next dfssm_sync. */

@@ -253,10 +253,13 @@ int proj_grid(int rows_total)
 // the projections run on the tensor cores (tcgen05 kind::i8 on +-1 tiles unpacked in shared memory) from this batch size on
 bool use_mma(const dfssm_ctx* c, int batch, int K)
 {
-    // measured (ms/step, dp4a rows / tensor cores, final build): cfg 3 batch 4 1.63 / 1.29; cfg 1 (d_model 768) batch 3 0.46 / 0.47,
-    // 5 0.49 / 0.50, 8 0.56 / 0.54, 12 0.64 / 0.58: from batch 4 on for the wide models, from 8 on for narrow ones
+    // measured (ms/step, dp4a rows / tensor cores, final build with k_epi_norm4 on the tensor-core chain): cfg 3 batch 4 1.63 / 1.20;
+    // cfg 1 (d_model 768) batch 2 0.413 / 0.406, 3 0.458 / 0.424, 5 0.492 / 0.453, 7 0.541 / 0.482; cfg 0 (d_model 256) batch 2
+    // 0.037 / 0.041, 4 0.040 / 0.043, 7 0.044 / 0.046, 8 0.046 / 0.046: from batch 4 on for the wide models (up to 3 the persistent
+    // kernel serves them), from 2 on for d_model 512 .. 1023, from 8 on below
     if (c->dm.fmt) return true;                       // the format variants are unpacked by k_proj_mma only
-    const int mma_min = c->dm.d_model >= 1024 ? 4 : 8;
+    static const int mma_env = getenv("DFSSM_MMA_MIN") ? atoi(getenv("DFSSM_MMA_MIN")) : 0;      // measurement switch
+    const int mma_min = mma_env > 0 ? mma_env : c->dm.d_model >= 1024 ? 4 : c->dm.d_model >= 512 ? 2 : 8;
     return batch >= mma_min && K % mma::KMULT == 0 && !(c->cfg.flags & DFSSM_FLAG_NO_MMA);
 }
 
@@ -620,7 +623,11 @@ namespace {
 // kernel chain.  Measured (ms/step, launches of the persistent kernel / chain with tensor-core projections [/ dp4a rows], final
 // build): cfg 3 (d_model 2048) batch 2 0.77 / 1.2, 3 1.15 / 1.27, 4 1.53 / 1.29; cfg 4 (2560) batch 2 1.35 / 1.96, 3 2.01 / 2.12,
 // 4 2.69 / 2.21; cfg 1 (768) batch 2 0.44 / 0.45 / 0.42, 3 0.66 / 0.47 / 0.46; cfg 0 (256) batch 2 0.057 / 0.046.
-int mega_max_batch(const dfssm_ctx* c) { return c->dm.d_model >= 1024 ? 3 : 1; }
+int mega_max_batch(const dfssm_ctx* c)
+{
+    static const int mega_env = getenv("DFSSM_MEGA_MAX") ? atoi(getenv("DFSSM_MEGA_MAX")) : 0;      // measurement switch
+    return mega_env > 0 ? mega_env : c->dm.d_model >= 1024 ? 3 : 1;
+}
 bool use_mega(const dfssm_ctx* c, int batch) { return batch <= mega_max_batch(c) && c->mega_ok && !(c->cfg.flags & DFSSM_FLAG_TAPS && batch > 1); }
 
 int mega_setup(dfssm_ctx* ctx)                      // at create: can this device run the mega grid?
